@@ -1,0 +1,110 @@
+"""CPU oracle (TEST INFRASTRUCTURE, NOT THE PRODUCT): ctypes binding of oracle/liboracle.so.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may import this.
+It shares no code with the CUDA path; the only common input is a `qss_synth.Mechanism` (pure data).
+"""
+from __future__ import annotations
+
+import ctypes as ct
+
+import numpy as np
+
+from . import build as _build
+
+EXPLICIT_F64, EXPLICIT_F128, JAC_DUAL, JAC_CSTEP, JAC_CONST_QSS = 0, 1, 2, 3, 4
+
+_lib = None
+
+
+class _Mech(ct.Structure):
+    _fields_ = [("n_nqss", ct.c_int32), ("n_qss", ct.c_int32), ("n_reac", ct.c_int32),
+                ("nasa_T", ct.c_void_p), ("nasa_lo", ct.c_void_p), ("nasa_hi", ct.c_void_p),
+                ("rtype", ct.c_void_p), ("dir_mask", ct.c_void_p),
+                ("reac_ptr", ct.c_void_p), ("reac_sp", ct.c_void_p), ("reac_nu", ct.c_void_p),
+                ("prod_ptr", ct.c_void_p), ("prod_sp", ct.c_void_p), ("prod_nu", ct.c_void_p),
+                ("arr", ct.c_void_p), ("arr_low", ct.c_void_p), ("troe", ct.c_void_p),
+                ("eff_ptr", ct.c_void_p), ("eff_sp", ct.c_void_p), ("eff_val", ct.c_void_p)]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = ct.CDLL(_build.build())
+        _lib.oracle_eval.restype = ct.c_int
+        _lib.oracle_eval.argtypes = [ct.c_void_p, ct.c_int64, ct.c_int64] + [ct.c_void_p] * 7 + [ct.c_int, ct.c_int]
+        _lib.oracle_rate_constants.restype = ct.c_int
+        _lib.oracle_rate_constants.argtypes = [ct.c_void_p, ct.c_void_p, ct.c_double, ct.c_void_p, ct.c_void_p]
+        _lib.oracle_closure_check.restype = ct.c_int
+        _lib.oracle_closure_check.argtypes = [ct.c_void_p, ct.c_void_p, ct.c_double] + [ct.c_void_p] * 3
+        _lib.oracle_max_threads.restype = ct.c_int
+    return _lib
+
+
+class OracleMech:
+    """Holds contiguous copies of a qss_synth.Mechanism's arrays and the C struct pointing at them."""
+
+    def __init__(self, mech):
+        self.N, self.Nq, self.M = mech.n_nqss, mech.n_qss, mech.n_reac
+        self._keep = {}
+        s = _Mech()
+        s.n_nqss, s.n_qss, s.n_reac = mech.n_nqss, mech.n_qss, mech.n_reac
+        spec = dict(nasa_T=np.float64, nasa_lo=np.float64, nasa_hi=np.float64, rtype=np.int32, dir_mask=np.uint8,
+                    reac_ptr=np.int32, reac_sp=np.int32, reac_nu=np.int32, prod_ptr=np.int32, prod_sp=np.int32,
+                    prod_nu=np.int32, arr=np.float64, arr_low=np.float64, troe=np.float64, eff_ptr=np.int32,
+                    eff_sp=np.int32, eff_val=np.float64)
+        for name, dt in spec.items():
+            a = np.ascontiguousarray(getattr(mech, name), dtype=dt)
+            if a.size == 0:
+                a = np.zeros(1, dtype=dt)
+            self._keep[name] = a
+            setattr(s, name, a.ctypes.data)
+        self.c = s
+
+    def _ptr(self):
+        return ct.addressof(self.c)
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data
+
+
+def evaluate(om: OracleMech, C: np.ndarray, T: np.ndarray, n_cells: int | None = None, *, want_jac=True,
+             want_scale=False, mode=EXPLICIT_F64, nthreads=0):
+    """C [N, ld], T [ld] float64. Returns dict(wdot [N,ld], cqss [Nq,ld], S [N,ld], jac [N,N+1,ld], jscale)."""
+    assert C.dtype == np.float64 and T.dtype == np.float64 and C.flags.c_contiguous and T.flags.c_contiguous
+    N, Nq = om.N, om.Nq
+    ld = C.shape[1]
+    n_cells = ld if n_cells is None else n_cells
+    assert C.shape[0] == N and T.shape[0] == ld and n_cells <= ld
+    out = dict(wdot=np.zeros((N, ld)), cqss=np.zeros((max(Nq, 1), ld)), S=np.zeros((N, ld)))
+    out["jac"] = np.zeros((N, N + 1, ld)) if want_jac else None
+    out["jscale"] = np.zeros((N, N + 1, ld)) if (want_jac and want_scale) else None
+    rc = lib().oracle_eval(om._ptr(), n_cells, ld, _p(C), _p(T), _p(out["wdot"]), _p(out["cqss"]), _p(out["S"]),
+                           _p(out["jac"]), _p(out["jscale"]), mode, nthreads)
+    if rc != 0:
+        raise RuntimeError(f"oracle_eval failed rc={rc}")
+    out["cqss"] = out["cqss"][:Nq]
+    return out
+
+
+def rate_constants(om: OracleMech, C1: np.ndarray, T: float):
+    C1 = np.ascontiguousarray(C1, dtype=np.float64)
+    kf = np.zeros(om.M); kb = np.zeros(om.M)
+    rc = lib().oracle_rate_constants(om._ptr(), _p(C1), float(T), _p(kf), _p(kb))
+    if rc != 0:
+        raise RuntimeError("oracle_rate_constants failed")
+    return kf, kb
+
+
+def closure_check(om: OracleMech, C1: np.ndarray, T: float):
+    C1 = np.ascontiguousarray(C1, dtype=np.float64)
+    n = max(om.Nq, 1)
+    y = np.zeros(n); res = np.zeros(n); sc = np.zeros(n)
+    rc = lib().oracle_closure_check(om._ptr(), _p(C1), float(T), _p(y), _p(res), _p(sc))
+    if rc != 0:
+        raise RuntimeError("oracle_closure_check failed")
+    return y[:om.Nq], res[:om.Nq], sc[:om.Nq]
+
+
+def max_threads() -> int:
+    return int(lib().oracle_max_threads())

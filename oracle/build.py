@@ -1,0 +1,27 @@
+"""Builds oracle/liboracle.so (host only, g++ -O2 -march=native -fopenmp). TEST INFRASTRUCTURE."""
+from __future__ import annotations
+
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(HERE, "qss_oracle.cpp")
+HDR = os.path.join(HERE, "qss_oracle.h")
+LIB = os.path.join(HERE, "liboracle.so")
+
+
+def build(force: bool = False) -> str:
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= max(os.path.getmtime(SRC), os.path.getmtime(HDR)):
+        return LIB
+    tmp = LIB + f".tmp{os.getpid()}"
+    # -ffp-contract=off: the oracle is the plain definition, operation by operation (no fused multiply-add)
+    cmd = ["g++", "-O2", "-march=native", "-ffp-contract=off", "-fopenmp", "-std=c++17", "-fPIC", "-shared",
+           "-o", tmp, SRC, "-lquadmath"]
+    subprocess.run(cmd, check=True)
+    os.replace(tmp, LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv))
