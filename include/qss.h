@@ -1,0 +1,131 @@
+/* qss.h -- C-ABI of libqss: batched per-cell evaluation of QSS-reduced chemistry on one B200 (sm_100a).
+ *
+ * What is computed (PAPER.md = arXiv 2405.05974; readings G1..G15 are listed in DESIGN.md):
+ *   - mass-action rates  Q_j = kf_j prod C^nu' - kb_j prod C^nu''           PAPER.md Eq. 2 (L59)
+ *   - net production     wdot_i = sum_j nu_ij Q_j                             PAPER.md Eq. 3 (L64)
+ *   - QSS closure        dC_q/dt = 0 for the N_q QSS species, a linear system
+ *                        A C_QSS = b solved per cell, group by group          PAPER.md Eq. 4 (L71), Eq. 6 (L150-157),
+ *                                                                             ordering L159-173, App. B
+ *   - analytical Jacobian J_ik = d wdot_i / d phi_k, phi = {C_1..C_N, T},
+ *                        with the chain rule through the closure              PAPER.md Eq. 7 (L185), Eq. 9 (L224)
+ *   Rate-constant forms (Arrhenius, third body, Troe fall-off, reverse rates from NASA-7 equilibrium
+ *   constants) are the standard CHEMKIN forms the paper leaves implicit (L278, L461); DESIGN.md "Readings" G4.
+ *
+ * Layout (all DEVICE buffers are SoA, cell innermost; `ld` is the cell stride, ld >= ncells):
+ *   C[k*ld + c]      k < N transported species, mol/m^3        T[c]   K
+ *   wdot[i*ld + c]   i < N, mol/(m^3 s)                         cqss[q*ld + c]  q < N_q, mol/m^3
+ *   jac[(i*(N+1) + k)*ld + c]   row i < N: species whose rate is differentiated,
+ *                               column k < N: d/dC_k, column k = N: d/dT        (N x (N+1) block, reading G5)
+ * Units: mol, m^3, s, K, J.  R = 8.31446261815324 J/(mol K), P0 = 101325 Pa.  Pressure is not an input.
+ *
+ * Ownership: the caller owns every device buffer including `workspace` (size from qss_mech_info); the
+ * library owns only the handle and its device tables (allocated in qss_mech_create on `device`, freed in
+ * qss_mech_destroy).  The arrays of qss_mech_desc_t are HOST pointers borrowed for the duration of
+ * qss_mech_create only.
+ *
+ * Execution: qss_eval_* enqueue kernels on `stream` (a cudaStream_t passed as void*) and return; they do
+ * not synchronise, allocate, or touch the default stream, and may be captured in a CUDA graph.
+ *
+ * Errors: every function returns QSS_OK (0) or a negative qss_status; nothing throws or aborts across the
+ * ABI.  qss_last_error() returns a thread-local message for the last failure.
+ * Preconditions NOT checked on the hot path: T > 0, C >= 0, every QSS species has a positive consumption
+ * coefficient, third-body concentration > 0 for fall-off reactions.  NaN/Inf propagate.
+ * There is no CPU fallback: without a CUDA device qss_mech_create fails with QSS_E_CUDA.
+ */
+#ifndef QSS_H
+#define QSS_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    QSS_OK = 0,
+    QSS_E_INVALID = -1,      /* null pointer, bad size / index / alignment, ld < ncells, workspace too small */
+    QSS_E_QUADRATIC = -2,    /* an enabled direction consumes >= 2 QSS molecules (linearise first, L77) */
+    QSS_E_QSS_FANOUT = -3,   /* an enabled direction produces >= 2 QSS molecules                                  */
+    QSS_E_NO_SINK = -4,      /* a QSS species cannot reach a transported species: closure structurally singular  */
+    QSS_E_UNSUPPORTED = -5,  /* reaction type outside {0,1,2}, non-positive stoichiometric coefficient          */
+    QSS_E_CUDA = -6          /* a CUDA runtime call failed (message in qss_last_error)                         */
+} qss_status;
+
+typedef struct qss_mech qss_mech_t;   /* opaque */
+
+/* Mechanism description. All pointers are HOST pointers. Species 0..n_nqss-1 are transported,
+ * n_nqss..n_nqss+n_qss-1 are QSS. */
+typedef struct {
+    int32_t n_elem, n_nqss, n_qss, n_reac;
+    const double  *elem_weight;            /* [n_elem] g/mol (may be NULL; not used on the hot path)          */
+    const int32_t *comp;                   /* [(n_nqss+n_qss)*n_elem] species-major (may be NULL)             */
+    const double  *nasa_T;                 /* [n_sp*3]  Tlow, Tmid, Thigh                                     */
+    const double  *nasa_lo, *nasa_hi;      /* [n_sp*7]  a1..a7 for T < Tmid / T >= Tmid (reading G9)           */
+    const int32_t *type;                   /* [n_reac]  0 Arrhenius, 1 third-body, 2 Troe fall-off            */
+    const uint8_t *dir_mask;               /* [n_reac]  bit0 forward enabled, bit1 reverse enabled (G10)      */
+    const int32_t *reac_ptr, *reac_sp, *reac_nu;   /* CSR reactants, nu' positive integers (G11)              */
+    const int32_t *prod_ptr, *prod_sp, *prod_nu;   /* CSR products,  nu''                                     */
+    const double  *arr;                    /* [n_reac*3] A, beta, Ea[J/mol]; high-pressure limit for type 2   */
+    const double  *arr_low;                /* [n_reac*3] low-pressure limit, read for type 2 only             */
+    const double  *troe;                   /* [n_reac*4] alpha, T***, T*, T**, read for type 2 only           */
+    const int32_t *eff_ptr, *eff_sp;       /* CSR non-unity third-body efficiencies, transported species only */
+    const double  *eff_val;                /*   (third-body concentration M = sum_{k<N} alpha_k C_k, G7)      */
+} qss_mech_desc_t;
+
+typedef struct {
+    int32_t n_nqss, n_qss, n_reac;
+    int32_t n_groups, max_group;           /* QSS coupling groups (SCCs of the QSS digraph)  */
+    int32_t n_levels;                      /* depth of the condensed DAG of groups                             */
+    int32_t group_size[64];                /* sizes of the first min(n_groups, 64) groups, in solve order      */
+    /* algorithmic cost per cell of the sparse method: fp64-pipe instruction slots
+     * (add = mul = fma = 1, exp 18, log 30, division 24, reciprocal 22) and bytes (inputs read once, outputs
+     * written once) */
+    double  slots_wdot, slots_jac;
+    double  bytes_wdot, bytes_jac;
+    /* workspace the caller must supply to qss_eval_wdot / qss_eval_jac (device memory, 256-byte aligned);
+     * independent of ncells */
+    size_t  workspace_bytes_wdot, workspace_bytes_jac;
+    int32_t kernel_variant_wdot, kernel_variant_jac;   /* which kernel the library selected       */
+} qss_mech_info_t;
+
+/* Validate `desc`, order the QSS groups (Tarjan SCC + topological order), build the static elimination
+ * schedules and gather tables, and upload them to `device`.  On success *out receives the handle. */
+int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech_t **out);
+int qss_mech_destroy(qss_mech_t *mech);
+int qss_mech_info(const qss_mech_t *mech, qss_mech_info_t *out);
+
+/* Solve order of the QSS species: order[i] is the local QSS index (0..n_qss-1) solved i-th, group_of[i]
+ * the group it belongs to (groups numbered in solve order).  HOST arrays of n_qss entries. For tests. */
+int qss_mech_qss_order(const qss_mech_t *mech, int32_t *order, int32_t *group_of);
+
+/* Host-only part of qss_mech_create (no CUDA call): validates `desc` and reports the QSS solve order.
+ * n_groups, order[n_qss], group_of[n_qss] may each be NULL. Same return codes as qss_mech_create. */
+int qss_mech_validate(const qss_mech_desc_t *desc, int32_t *n_groups, int32_t *order, int32_t *group_of);
+
+/* wdot (and optionally the closure's C_QSS) for ncells cells.  C, T, wdot, cqss_or_null, workspace are
+ * DEVICE pointers, 16-byte aligned; stream is a cudaStream_t.  ncells == 0 is a no-op. */
+int qss_eval_wdot(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *C, const double *T,
+                  double *wdot, double *cqss_or_null, void *workspace, size_t workspace_bytes, void *stream);
+
+/* Analytical Jacobian d wdot / d[C,T] (and optionally wdot in the same pass). */
+int qss_eval_jac(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *C, const double *T,
+                 double *jac, double *wdot_or_null, void *workspace, size_t workspace_bytes, void *stream);
+
+/* Host-buffer convenience used for end-to-end timing: copies C and T to the device (in `dev_scratch`, which
+ * must hold qss_host_scratch_bytes() bytes), evaluates, copies the Jacobian (and wdot if not NULL) back to
+ * the HOST buffers, and synchronises `stream`.  Host buffers should be pinned for full copy bandwidth. */
+size_t qss_host_scratch_bytes(const qss_mech_t *mech, int64_t ncells, int64_t ld);
+int qss_eval_jac_host(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *C_host,
+                      const double *T_host, double *jac_host, double *wdot_host_or_null,
+                      void *dev_scratch, size_t dev_scratch_bytes, void *stream);
+
+/* fp64 FMA-pipe micro-benchmark used as the roofline denominator: launches
+ * `blocks` x 256 threads each running `iters` rounds of 8 independent dependent-chain DFMAs.
+ * Returns the number of DFMA lane-operations issued in *n_fma (time it with CUDA events on `stream`). */
+int qss_bench_dfma(int blocks, int iters, double *sink_dev, double *n_fma, void *stream);
+
+const char *qss_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

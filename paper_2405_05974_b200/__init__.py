@@ -1,0 +1,214 @@
+"""paper_2405_05974_b200 -- thin Python binding of libqss (include/qss.h).
+
+Argument marshalling only: every step of the hot path (rate constants, QSS closure, wdot, analytical
+Jacobian; Eq. 2-4, 6, 7, 9) runs in the CUDA kernels of csrc/.  PyTorch is used for device memory
+and streams.  There is no CPU fallback: importing works without a GPU (so the ABI can be checked), but
+creating a mechanism or evaluating anything requires a CUDA device and the built library.
+"""
+from __future__ import annotations
+
+import ctypes as ct
+import os
+
+import numpy as np
+
+from . import build as _build
+
+__all__ = ["lib", "QssMech", "QssError", "EXPORTS", "STATUS"]
+
+EXPORTS = ["qss_mech_create", "qss_mech_validate", "qss_mech_destroy", "qss_mech_info", "qss_mech_qss_order", "qss_eval_wdot",
+           "qss_eval_jac", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
+STATUS = {0: "QSS_OK", -1: "QSS_E_INVALID", -2: "QSS_E_QUADRATIC", -3: "QSS_E_QSS_FANOUT", -4: "QSS_E_NO_SINK",
+          -5: "QSS_E_UNSUPPORTED", -6: "QSS_E_CUDA"}
+
+
+class QssError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{STATUS.get(code, code)}: {msg}")
+        self.code = code
+
+
+class _Desc(ct.Structure):
+    _fields_ = [("n_elem", ct.c_int32), ("n_nqss", ct.c_int32), ("n_qss", ct.c_int32), ("n_reac", ct.c_int32),
+                ("elem_weight", ct.c_void_p), ("comp", ct.c_void_p),
+                ("nasa_T", ct.c_void_p), ("nasa_lo", ct.c_void_p), ("nasa_hi", ct.c_void_p),
+                ("type", ct.c_void_p), ("dir_mask", ct.c_void_p),
+                ("reac_ptr", ct.c_void_p), ("reac_sp", ct.c_void_p), ("reac_nu", ct.c_void_p),
+                ("prod_ptr", ct.c_void_p), ("prod_sp", ct.c_void_p), ("prod_nu", ct.c_void_p),
+                ("arr", ct.c_void_p), ("arr_low", ct.c_void_p), ("troe", ct.c_void_p),
+                ("eff_ptr", ct.c_void_p), ("eff_sp", ct.c_void_p), ("eff_val", ct.c_void_p)]
+
+
+class _Info(ct.Structure):
+    _fields_ = [("n_nqss", ct.c_int32), ("n_qss", ct.c_int32), ("n_reac", ct.c_int32),
+                ("n_groups", ct.c_int32), ("max_group", ct.c_int32), ("n_levels", ct.c_int32),
+                ("group_size", ct.c_int32 * 64),
+                ("slots_wdot", ct.c_double), ("slots_jac", ct.c_double),
+                ("bytes_wdot", ct.c_double), ("bytes_jac", ct.c_double),
+                ("workspace_bytes_wdot", ct.c_size_t), ("workspace_bytes_jac", ct.c_size_t),
+                ("kernel_variant_wdot", ct.c_int32), ("kernel_variant_jac", ct.c_int32)]
+
+
+_lib = None
+
+
+def lib():
+    """Loads (building first if the sources are newer) libqss.so. Raises if it cannot be built or loaded."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = ct.CDLL(path)
+        vp, i64 = ct.c_void_p, ct.c_int64
+        L.qss_mech_create.restype = ct.c_int; L.qss_mech_create.argtypes = [vp, ct.c_int, ct.POINTER(vp)]
+        L.qss_mech_validate.restype = ct.c_int; L.qss_mech_validate.argtypes = [vp, vp, vp, vp]
+        L.qss_mech_destroy.restype = ct.c_int; L.qss_mech_destroy.argtypes = [vp]
+        L.qss_mech_info.restype = ct.c_int; L.qss_mech_info.argtypes = [vp, ct.POINTER(_Info)]
+        L.qss_mech_qss_order.restype = ct.c_int; L.qss_mech_qss_order.argtypes = [vp, vp, vp]
+        L.qss_eval_wdot.restype = ct.c_int; L.qss_eval_wdot.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, ct.c_size_t, vp]
+        L.qss_eval_jac.restype = ct.c_int; L.qss_eval_jac.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, ct.c_size_t, vp]
+        L.qss_host_scratch_bytes.restype = ct.c_size_t; L.qss_host_scratch_bytes.argtypes = [vp, i64, i64]
+        L.qss_eval_jac_host.restype = ct.c_int; L.qss_eval_jac_host.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, ct.c_size_t, vp]
+        L.qss_bench_dfma.restype = ct.c_int; L.qss_bench_dfma.argtypes = [ct.c_int, ct.c_int, vp, ct.POINTER(ct.c_double), vp]
+        L.qss_last_error.restype = ct.c_char_p; L.qss_last_error.argtypes = []
+        _lib = L
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise QssError(rc, lib().qss_last_error().decode())
+
+
+_DESC_SPEC = dict(elem_weight=np.float64, comp=np.int32, nasa_T=np.float64, nasa_lo=np.float64, nasa_hi=np.float64,
+                  type=np.int32, dir_mask=np.uint8, reac_ptr=np.int32, reac_sp=np.int32, reac_nu=np.int32,
+                  prod_ptr=np.int32, prod_sp=np.int32, prod_nu=np.int32, arr=np.float64, arr_low=np.float64,
+                  troe=np.float64, eff_ptr=np.int32, eff_sp=np.int32, eff_val=np.float64)
+
+
+def make_desc(mech):
+    """qss_mech_desc_t from any object with the fields of qss_synth.Mechanism. Returns (desc, keepalive)."""
+    d = _Desc()
+    d.n_elem, d.n_nqss, d.n_qss, d.n_reac = int(mech.n_elem), int(mech.n_nqss), int(mech.n_qss), int(mech.n_reac)
+    keep = {}
+    for name, dt in _DESC_SPEC.items():
+        src = getattr(mech, "rtype" if name == "type" else name)
+        a = np.ascontiguousarray(src, dtype=dt)
+        if a.size == 0:
+            a = np.zeros(1, dtype=dt)
+        keep[name] = a
+        setattr(d, name, a.ctypes.data)
+    return d, keep
+
+
+def validate(mech):
+    """Host-only validation + QSS solve order (no CUDA). Returns (n_groups, order, group_of)."""
+    d, keep = make_desc(mech)
+    ng = ct.c_int32()
+    nq = max(int(mech.n_qss), 1)
+    order = np.zeros(nq, dtype=np.int32); grp = np.zeros(nq, dtype=np.int32)
+    _check(lib().qss_mech_validate(ct.addressof(d), ct.addressof(ng), order.ctypes.data, grp.ctypes.data))
+    del keep
+    return ng.value, order[:mech.n_qss], grp[:mech.n_qss]
+
+
+def _ptr(t):
+    return None if t is None else ct.c_void_p(t.data_ptr())
+
+
+class QssMech:
+    """A compiled mechanism on one CUDA device (qss_mech_create / qss_mech_destroy)."""
+
+    def __init__(self, mech, device: int = 0):
+        self._h = ct.c_void_p()
+        d, keep = make_desc(mech)
+        _check(lib().qss_mech_create(ct.addressof(d), int(device), ct.byref(self._h)))
+        del keep
+        self.device = int(device)
+        info = _Info()
+        _check(lib().qss_mech_info(self._h, ct.byref(info)))
+        self.info = info
+        self.N, self.Nq, self.M = info.n_nqss, info.n_qss, info.n_reac
+        self._ws = {}
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().qss_mech_destroy(self._h)
+            self._h = ct.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def qss_order(self):
+        order = np.zeros(max(self.Nq, 1), dtype=np.int32); grp = np.zeros(max(self.Nq, 1), dtype=np.int32)
+        _check(lib().qss_mech_qss_order(self._h, order.ctypes.data, grp.ctypes.data))
+        return order[:self.Nq], grp[:self.Nq]
+
+    def group_sizes(self):
+        return [int(self.info.group_size[g]) for g in range(min(self.info.n_groups, 64))]
+
+    def workspace(self, jac: bool):
+        import torch
+        key = bool(jac)
+        if key not in self._ws:
+            nbytes = self.info.workspace_bytes_jac if jac else self.info.workspace_bytes_wdot
+            self._ws[key] = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=f"cuda:{self.device}")
+        return self._ws[key]
+
+    @staticmethod
+    def _stream():
+        import torch
+        return ct.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+    def eval_wdot(self, C, T, ncells=None, wdot=None, cqss=None, want_cqss=False):
+        """C [N, ld], T [ld] float64 CUDA tensors. Returns wdot [N, ld] (and cqss [Nq, ld])."""
+        import torch
+        ld = C.shape[1]
+        ncells = ld if ncells is None else int(ncells)
+        assert C.dtype == torch.float64 and T.dtype == torch.float64 and C.is_contiguous() and T.is_contiguous()
+        assert C.shape[0] == self.N and T.shape[0] == ld
+        if wdot is None:
+            wdot = torch.empty((self.N, ld), dtype=torch.float64, device=C.device)
+        if want_cqss and cqss is None:
+            cqss = torch.empty((max(self.Nq, 1), ld), dtype=torch.float64, device=C.device)
+        ws = self.workspace(False)
+        _check(lib().qss_eval_wdot(self._h, ncells, ld, _ptr(C), _ptr(T), _ptr(wdot), _ptr(cqss), _ptr(ws),
+                                   ws.numel(), self._stream()))
+        return (wdot, cqss[:self.Nq]) if want_cqss else wdot
+
+    def eval_jac(self, C, T, ncells=None, jac=None, wdot=None, want_wdot=False):
+        """Returns jac [N, N+1, ld] (and wdot [N, ld])."""
+        import torch
+        ld = C.shape[1]
+        ncells = ld if ncells is None else int(ncells)
+        assert C.dtype == torch.float64 and T.dtype == torch.float64 and C.is_contiguous() and T.is_contiguous()
+        assert C.shape[0] == self.N and T.shape[0] == ld
+        if jac is None:
+            jac = torch.empty((self.N, self.N + 1, ld), dtype=torch.float64, device=C.device)
+        if want_wdot and wdot is None:
+            wdot = torch.empty((self.N, ld), dtype=torch.float64, device=C.device)
+        ws = self.workspace(True)
+        _check(lib().qss_eval_jac(self._h, ncells, ld, _ptr(C), _ptr(T), _ptr(jac), _ptr(wdot), _ptr(ws),
+                                  ws.numel(), self._stream()))
+        return (jac, wdot) if want_wdot else jac
+
+    def host_scratch_bytes(self, ncells, ld):
+        return int(lib().qss_host_scratch_bytes(self._h, int(ncells), int(ld)))
+
+    def eval_jac_host(self, C_host, T_host, jac_host, wdot_host, scratch, ncells=None):
+        """End-to-end call on HOST (ideally pinned) torch tensors; `scratch` is a CUDA uint8 tensor."""
+        ld = C_host.shape[1]
+        ncells = ld if ncells is None else int(ncells)
+        _check(lib().qss_eval_jac_host(self._h, ncells, ld, _ptr(C_host), _ptr(T_host), _ptr(jac_host),
+                                       _ptr(wdot_host), _ptr(scratch), scratch.numel(), self._stream()))
+
+
+def bench_dfma(blocks: int, iters: int, sink):
+    """Launches the fp64-FMA micro-benchmark on the current stream; returns the number of lane-FMAs issued."""
+    n = ct.c_double()
+    import torch
+    _check(lib().qss_bench_dfma(int(blocks), int(iters), _ptr(sink), ct.byref(n),
+                                ct.c_void_p(torch.cuda.current_stream().cuda_stream)))
+    return n.value

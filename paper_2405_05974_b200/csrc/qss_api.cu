@@ -1,0 +1,201 @@
+// C-ABI of libqss (include/qss.h): handle management, argument checks, kernel selection and launch.
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/qss.h"
+#include "qss_compile.h"
+
+size_t qss_slab_ws_doubles(const QssTab &t, bool jac, int nwarp);
+cudaError_t qss_launch_slab(const QssTab &t, bool jac, int64_t ncells, int64_t ld, const double *C, const double *T,
+                            double *wdot, double *cqss, double *jacp, double *ws, int nblocks, int nwarp,
+                            cudaStream_t stream);
+cudaError_t qss_launch_dfma(int blocks, int iters, double *sink, cudaStream_t stream);
+
+struct qss_mech {
+    QssCompiled c;
+    int device = 0;
+    int n_sm = 0;
+    int32_t *dI = nullptr;
+    double *dD = nullptr;
+    int nwarp = 8;            // warps per block of the slab kernel
+    int blocks_per_sm = 2;
+    int nblocks = 0;
+};
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string &msg) { g_err = msg; return code; }
+int cuda_fail(cudaError_t e, const char *what) {
+    g_err = std::string(what) + ": " + cudaGetErrorString(e);
+    return QSS_E_CUDA;
+}
+
+struct DeviceGuard {
+    int prev = -1; bool ok = false;
+    explicit DeviceGuard(int dev) { if (cudaGetDevice(&prev) == cudaSuccess && cudaSetDevice(dev) == cudaSuccess) ok = true; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int check_eval(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T, const void *out,
+               const void *ws, size_t ws_bytes, size_t need) {
+    if (!m) return fail(QSS_E_INVALID, "mech is NULL");
+    if (ncells < 0 || ld < ncells) return fail(QSS_E_INVALID, "need 0 <= ncells <= ld");
+    if (ncells == 0) return QSS_OK;
+    if (!C || !T || !out) return fail(QSS_E_INVALID, "C, T or the output pointer is NULL");
+    if (((uintptr_t)C | (uintptr_t)T | (uintptr_t)out) & 15) return fail(QSS_E_INVALID, "device pointers must be 16-byte aligned");
+    if (!ws || ws_bytes < need) return fail(QSS_E_INVALID, "workspace is NULL or smaller than qss_mech_info reports");
+    if ((uintptr_t)ws & 255) return fail(QSS_E_INVALID, "workspace must be 256-byte aligned");
+    return QSS_OK;
+}
+
+}  // namespace
+
+extern "C" const char *qss_last_error(void) { return g_err.c_str(); }
+
+extern "C" int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech_t **out) {
+    if (!out) return fail(QSS_E_INVALID, "out is NULL");
+    *out = nullptr;
+    qss_mech *m = new (std::nothrow) qss_mech();
+    if (!m) return fail(QSS_E_INVALID, "out of host memory");
+    std::string err;
+    int rc;
+    try {
+        rc = qss_compile(desc, m->c, err);
+    } catch (const std::exception &e) {
+        rc = QSS_E_INVALID; err = std::string("mechanism compiler: ") + e.what();
+    }
+    if (rc != QSS_OK) { delete m; return fail(rc, err); }
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) { delete m; return e != cudaSuccess ? cuda_fail(e, "cudaGetDeviceCount") : fail(QSS_E_CUDA, "no CUDA device (libqss has no CPU fallback)"); }
+    if (device < 0 || device >= ndev) { delete m; return fail(QSS_E_INVALID, "device index out of range"); }
+    DeviceGuard guard(device);
+    if (!guard.ok) { delete m; return fail(QSS_E_CUDA, "cudaSetDevice failed"); }
+    m->device = device;
+    cudaDeviceProp prop;
+    if ((e = cudaGetDeviceProperties(&prop, device)) != cudaSuccess) { delete m; return cuda_fail(e, "cudaGetDeviceProperties"); }
+    m->n_sm = prop.multiProcessorCount;
+    m->nblocks = m->n_sm * m->blocks_per_sm;
+    const size_t nI = m->c.I.size() ? m->c.I.size() : 1, nD = m->c.D.size() ? m->c.D.size() : 1;
+    if ((e = cudaMalloc(&m->dI, nI * sizeof(int32_t))) != cudaSuccess) { delete m; return cuda_fail(e, "cudaMalloc(tables)"); }
+    if ((e = cudaMalloc(&m->dD, nD * sizeof(double))) != cudaSuccess) { cudaFree(m->dI); delete m; return cuda_fail(e, "cudaMalloc(tables)"); }
+    if (m->c.I.size()) e = cudaMemcpy(m->dI, m->c.I.data(), m->c.I.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && m->c.D.size()) e = cudaMemcpy(m->dD, m->c.D.data(), m->c.D.size() * sizeof(double), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(m->dI); cudaFree(m->dD); delete m; return cuda_fail(e, "cudaMemcpy(tables)"); }
+    m->c.tab.I = m->dI; m->c.tab.D = m->dD;
+    *out = m;
+    return QSS_OK;
+}
+
+extern "C" int qss_mech_validate(const qss_mech_desc_t *desc, int32_t *n_groups, int32_t *order, int32_t *group_of) {
+    QssCompiled c;
+    std::string err;
+    int rc;
+    try {
+        rc = qss_compile(desc, c, err);
+    } catch (const std::exception &e) {
+        rc = QSS_E_INVALID; err = std::string("mechanism compiler: ") + e.what();
+    }
+    if (rc != QSS_OK) return fail(rc, err);
+    if (n_groups) *n_groups = c.tab.n_groups;
+    for (int i = 0; i < c.tab.Nq; ++i) { if (order) order[i] = c.order[i]; if (group_of) group_of[i] = c.group_of[i]; }
+    return QSS_OK;
+}
+
+extern "C" int qss_mech_destroy(qss_mech_t *m) {
+    if (!m) return QSS_OK;
+    DeviceGuard guard(m->device);
+    cudaFree(m->dI); cudaFree(m->dD);
+    delete m;
+    return QSS_OK;
+}
+
+static size_t ws_bytes(const qss_mech_t *m, bool jac) {
+    return qss_slab_ws_doubles(m->c.tab, jac, m->nwarp) * sizeof(double) * (size_t)m->nblocks;
+}
+
+extern "C" int qss_mech_info(const qss_mech_t *m, qss_mech_info_t *o) {
+    if (!m || !o) return fail(QSS_E_INVALID, "NULL argument");
+    std::memset(o, 0, sizeof *o);
+    const QssTab &t = m->c.tab;
+    o->n_nqss = t.N; o->n_qss = t.Nq; o->n_reac = t.M;
+    o->n_groups = t.n_groups; o->max_group = t.max_group; o->n_levels = t.n_levels;
+    for (int g = 0; g < t.n_groups && g < 64; ++g) o->group_size[g] = m->c.group_size[g];
+    o->slots_wdot = m->c.slots_wdot; o->slots_jac = m->c.slots_jac;
+    o->bytes_wdot = m->c.bytes_wdot; o->bytes_jac = m->c.bytes_jac;
+    o->workspace_bytes_wdot = ws_bytes(m, false);
+    o->workspace_bytes_jac = ws_bytes(m, true);
+    o->kernel_variant_wdot = 0; o->kernel_variant_jac = 0;
+    return QSS_OK;
+}
+
+extern "C" int qss_mech_qss_order(const qss_mech_t *m, int32_t *order, int32_t *group_of) {
+    if (!m || !order || !group_of) return fail(QSS_E_INVALID, "NULL argument");
+    for (int i = 0; i < m->c.tab.Nq; ++i) { order[i] = m->c.order[i]; group_of[i] = m->c.group_of[i]; }
+    return QSS_OK;
+}
+
+extern "C" int qss_eval_wdot(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T,
+                             double *wdot, double *cqss, void *workspace, size_t workspace_bytes, void *stream) {
+    int rc = check_eval(m, ncells, ld, C, T, wdot, workspace, workspace_bytes, m ? ws_bytes(m, false) : 0);
+    if (rc != QSS_OK || ncells == 0) return rc;
+    cudaError_t e = qss_launch_slab(m->c.tab, false, ncells, ld, C, T, wdot, cqss, nullptr, (double *)workspace,
+                                    m->nblocks, m->nwarp, (cudaStream_t)stream);
+    return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_eval_wdot launch");
+}
+
+extern "C" int qss_eval_jac(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T,
+                            double *jac, double *wdot, void *workspace, size_t workspace_bytes, void *stream) {
+    int rc = check_eval(m, ncells, ld, C, T, jac, workspace, workspace_bytes, m ? ws_bytes(m, true) : 0);
+    if (rc != QSS_OK || ncells == 0) return rc;
+    cudaError_t e = qss_launch_slab(m->c.tab, true, ncells, ld, C, T, wdot, nullptr, jac, (double *)workspace,
+                                    m->nblocks, m->nwarp, (cudaStream_t)stream);
+    return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_eval_jac launch");
+}
+
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+extern "C" size_t qss_host_scratch_bytes(const qss_mech_t *m, int64_t ncells, int64_t ld) {
+    if (!m || ncells < 0 || ld < ncells) return 0;
+    const size_t N = m->c.tab.N, L = (size_t)ld * sizeof(double);
+    return align256(N * L) + align256(L) + align256(N * L) + align256(N * (N + 1) * L) + align256(ws_bytes(m, true));
+}
+
+extern "C" int qss_eval_jac_host(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *Ch, const double *Th,
+                                 double *jach, double *wdoth, void *scratch, size_t scratch_bytes, void *stream) {
+    if (!m) return fail(QSS_E_INVALID, "mech is NULL");
+    if (ncells < 0 || ld < ncells || !Ch || !Th || !jach) return fail(QSS_E_INVALID, "bad host arguments");
+    if (ncells == 0) return QSS_OK;
+    if (!scratch || scratch_bytes < qss_host_scratch_bytes(m, ncells, ld) || ((uintptr_t)scratch & 255))
+        return fail(QSS_E_INVALID, "dev_scratch is NULL, misaligned or smaller than qss_host_scratch_bytes()");
+    const size_t N = m->c.tab.N, L = (size_t)ld * sizeof(double);
+    char *p = (char *)scratch;
+    double *dC = (double *)p; p += align256(N * L);
+    double *dT = (double *)p; p += align256(L);
+    double *dW = (double *)p; p += align256(N * L);
+    double *dJ = (double *)p; p += align256(N * (N + 1) * L);
+    void *ws = p;
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e;
+    if ((e = cudaMemcpyAsync(dC, Ch, N * L, cudaMemcpyHostToDevice, s)) != cudaSuccess) return cuda_fail(e, "H2D C");
+    if ((e = cudaMemcpyAsync(dT, Th, L, cudaMemcpyHostToDevice, s)) != cudaSuccess) return cuda_fail(e, "H2D T");
+    int rc = qss_eval_jac(m, ncells, ld, dC, dT, dJ, wdoth ? dW : nullptr, ws, ws_bytes(m, true), stream);
+    if (rc != QSS_OK) return rc;
+    if ((e = cudaMemcpyAsync(jach, dJ, N * (N + 1) * L, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return cuda_fail(e, "D2H jac");
+    if (wdoth && (e = cudaMemcpyAsync(wdoth, dW, N * L, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return cuda_fail(e, "D2H wdot");
+    if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return cuda_fail(e, "cudaStreamSynchronize");
+    return QSS_OK;
+}
+
+extern "C" int qss_bench_dfma(int blocks, int iters, double *sink, double *n_fma, void *stream) {
+    if (blocks < 1 || iters < 1 || !sink) return fail(QSS_E_INVALID, "bad arguments");
+    cudaError_t e = qss_launch_dfma(blocks, iters, sink, (cudaStream_t)stream);
+    if (n_fma) *n_fma = (double)blocks * 256.0 * (double)iters * 16.0 * 8.0;
+    return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_bench_dfma launch");
+}

@@ -1,0 +1,453 @@
+// Host-side mechanism compiler: qss_mech_desc_t -> flat device tables (QssTab).
+//
+// This is the run-time replacement of the paper's offline pre-processing (section 2.3;
+// App. B): validate the linear-coupling premise (L73-77, L146), build the QSS dependency digraph,
+// find its strongly connected components with Tarjan's algorithm, order the condensed DAG, and emit static
+// gather / elimination schedules.  No symbolic expressions are generated (the paper's sympy + CSE path,
+// L262-276, is prior art here): the kernels interpret these tables.
+#include "qss_compile.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <functional>
+#include <map>
+
+namespace {
+
+struct Term { int sp, nu; };
+
+struct Reaction {
+    int type, mask;
+    std::vector<Term> side[2];     // side[0] reactants, side[1] products (as given)
+    std::vector<Term> net;         // nu'' - nu', non-zero only
+    int q[2];                      // local QSS index consumed by direction 0 / 1, or -1
+    int dnu;
+    int tb;                        // index among third-body / fall-off reactions, or -1
+};
+
+std::string fmt(const char *f, int a = 0, int b = 0, int c = 0) {
+    char buf[256];
+    std::snprintf(buf, sizeof buf, f, a, b, c);
+    return buf;
+}
+
+// Tarjan's SCC algorithm on the QSS digraph (App. B): one DFS, adjacency lists.
+// Returns component id per vertex; components are numbered in the order they are completed, which is a
+// reverse topological order of the condensed DAG (a component is completed after everything it reaches).
+int tarjan(int n, const std::vector<std::vector<int>> &adj, std::vector<int> &comp) {
+    std::vector<int> index(n, -1), low(n, 0), stack;
+    std::vector<char> on(n, 0);
+    comp.assign(n, -1);
+    int counter = 0, ncomp = 0;
+    // iterative DFS (mechanisms may have hundreds of QSS species)
+    struct Frame { int v; size_t e; };
+    for (int root = 0; root < n; ++root) {
+        if (index[root] != -1) continue;
+        std::vector<Frame> call;
+        call.push_back({root, 0});
+        index[root] = low[root] = counter++;
+        stack.push_back(root); on[root] = 1;
+        while (!call.empty()) {
+            Frame &f = call.back();
+            int v = f.v;
+            if (f.e < adj[v].size()) {
+                int w = adj[v][f.e++];
+                if (index[w] == -1) {
+                    index[w] = low[w] = counter++;
+                    stack.push_back(w); on[w] = 1;
+                    call.push_back({w, 0});
+                } else if (on[w]) {
+                    low[v] = std::min(low[v], index[w]);
+                }
+            } else {
+                if (low[v] == index[v]) {
+                    for (;;) {
+                        int w = stack.back(); stack.pop_back(); on[w] = 0;
+                        comp[w] = ncomp;
+                        if (w == v) break;
+                    }
+                    ++ncomp;
+                }
+                call.pop_back();
+                if (!call.empty()) low[call.back().v] = std::min(low[call.back().v], low[v]);
+            }
+        }
+    }
+    return ncomp;
+}
+
+}  // namespace
+
+int qss_compile(const qss_mech_desc_t *d, QssCompiled &out, std::string &err) {
+    if (!d) { err = "desc is NULL"; return QSS_E_INVALID; }
+    const int N = d->n_nqss, Nq = d->n_qss, M = d->n_reac, nsp = N + Nq;
+    if (N < 1 || Nq < 0 || M < 0) { err = "n_nqss must be >= 1, n_qss and n_reac >= 0"; return QSS_E_INVALID; }
+    if (!d->nasa_T || !d->nasa_lo || !d->nasa_hi) { err = "NASA-7 tables are NULL"; return QSS_E_INVALID; }
+    if (M > 0 && (!d->type || !d->dir_mask || !d->reac_ptr || !d->prod_ptr || !d->arr)) {
+        err = "reaction arrays are NULL"; return QSS_E_INVALID;
+    }
+    // ---------------------------------------------------------------- reactions: parse + validate
+    std::vector<Reaction> R(M);
+    int n_tb = 0;
+    for (int j = 0; j < M; ++j) {
+        Reaction &r = R[j];
+        r.type = d->type[j]; r.mask = d->dir_mask[j] & 3;
+        if (r.type < 0 || r.type > 2) { err = fmt("reaction %d: unsupported type %d", j, r.type); return QSS_E_UNSUPPORTED; }
+        if (r.type == 2 && (!d->arr_low || !d->troe)) { err = fmt("reaction %d: fall-off without arr_low/troe", j); return QSS_E_INVALID; }
+        r.tb = r.type >= 1 ? n_tb++ : -1;
+        const int32_t *ptr[2] = {d->reac_ptr, d->prod_ptr}, *sp[2] = {d->reac_sp, d->prod_sp}, *nu[2] = {d->reac_nu, d->prod_nu};
+        std::map<int, int> net;
+        r.dnu = 0;
+        for (int s = 0; s < 2; ++s) {
+            if (ptr[s][j + 1] < ptr[s][j]) { err = fmt("reaction %d: CSR pointers decrease", j); return QSS_E_INVALID; }
+            int nq = 0;
+            r.q[s] = -1;
+            for (int p = ptr[s][j]; p < ptr[s][j + 1]; ++p) {
+                if (!sp[s] || !nu[s]) { err = "species CSR arrays are NULL"; return QSS_E_INVALID; }
+                Term t{sp[s][p], nu[s][p]};
+                if (t.sp < 0 || t.sp >= nsp) { err = fmt("reaction %d: species index %d out of range", j, t.sp); return QSS_E_INVALID; }
+                if (t.nu < 1) { err = fmt("reaction %d: stoichiometric coefficient %d < 1", j, t.nu); return QSS_E_UNSUPPORTED; }
+                for (const Term &o : r.side[s]) if (o.sp == t.sp) { err = fmt("reaction %d: species %d listed twice on one side", j, t.sp); return QSS_E_INVALID; }
+                r.side[s].push_back(t);
+                net[t.sp] += s == 0 ? -t.nu : t.nu;
+                r.dnu += s == 0 ? -t.nu : t.nu;
+                if (t.sp >= N) { nq += t.nu; r.q[s] = t.sp - N; }
+            }
+            if (nq > 1) {
+                // side s is consumed by direction s and produced by direction 1-s
+                if (r.mask & (1 << s)) { err = fmt("reaction %d: an enabled direction consumes %d QSS molecules (quadratic coupling)", j, nq); return QSS_E_QUADRATIC; }
+                if (r.mask & (1 << (1 - s))) { err = fmt("reaction %d: an enabled direction produces %d QSS molecules", j, nq); return QSS_E_QSS_FANOUT; }
+            }
+        }
+        for (auto &kv : net) if (kv.second != 0) r.net.push_back({kv.first, kv.second});
+        if (r.type >= 1 && d->eff_ptr) {
+            for (int p = d->eff_ptr[j]; p < d->eff_ptr[j + 1]; ++p)
+                if (d->eff_sp[p] < 0 || d->eff_sp[p] >= N) { err = fmt("reaction %d: third-body efficiency on species %d (must be transported)", j, d->eff_sp[p]); return QSS_E_INVALID; }
+        }
+    }
+    auto enabled = [&](int j, int dir) { return (R[j].mask >> dir) & 1; };
+
+    // ---------------------------------------------------------------- QSS digraph, SCCs, levels
+    // edge n -> m iff an enabled direction consumes QSS n and produces QSS m != n
+    std::vector<std::vector<int>> adj(Nq);
+    std::vector<char> has_leak(Nq, 0);
+    for (int j = 0; j < M; ++j)
+        for (int dir = 0; dir < 2; ++dir) {
+            if (!enabled(j, dir)) continue;
+            int n = R[j].q[dir], m = R[j].q[1 - dir];
+            if (n < 0) continue;
+            if (m >= 0 && m != n) adj[n].push_back(m);
+            else if (m < 0) has_leak[n] = 1;
+        }
+    for (auto &a : adj) { std::sort(a.begin(), a.end()); a.erase(std::unique(a.begin(), a.end()), a.end()); }
+    // every QSS species must reach a leak, else the closure matrix is structurally singular
+    {
+        std::vector<std::vector<int>> radj(Nq);
+        for (int n = 0; n < Nq; ++n) for (int m : adj[n]) radj[m].push_back(n);
+        std::vector<char> ok(has_leak);
+        std::vector<int> st;
+        for (int n = 0; n < Nq; ++n) if (ok[n]) st.push_back(n);
+        while (!st.empty()) { int v = st.back(); st.pop_back(); for (int u : radj[v]) if (!ok[u]) { ok[u] = 1; st.push_back(u); } }
+        for (int n = 0; n < Nq; ++n) if (!ok[n]) { err = fmt("QSS species %d (index %d) has no path to a transported species", n, N + n); return QSS_E_NO_SINK; }
+    }
+    std::vector<int> comp;
+    const int ncomp = tarjan(Nq, adj, comp);
+    // level of a component = longest chain of components feeding it (its sources must be solved first)
+    std::vector<int> level(ncomp, 0);
+    // Tarjan numbers components in reverse topological order: comp id larger => earlier in the DAG.
+    for (int c = ncomp - 1; c >= 0; --c)
+        for (int n = 0; n < Nq; ++n) if (comp[n] == c)
+            for (int m : adj[n]) if (comp[m] != c) level[comp[m]] = std::max(level[comp[m]], level[c] + 1);
+    std::vector<int> gorder(ncomp);
+    for (int c = 0; c < ncomp; ++c) gorder[c] = c;
+    std::stable_sort(gorder.begin(), gorder.end(), [&](int a, int b) {
+        if (level[a] != level[b]) return level[a] < level[b];
+        return a > b;
+    });
+    std::vector<int> gid(ncomp);             // component -> group number in solve order
+    for (int g = 0; g < ncomp; ++g) gid[gorder[g]] = g;
+    const int n_groups = ncomp;
+    int n_levels = 0;
+    for (int c = 0; c < ncomp; ++c) n_levels = std::max(n_levels, level[c] + 1);
+    std::vector<std::vector<int>> members(n_groups);
+    for (int n = 0; n < Nq; ++n) members[gid[comp[n]]].push_back(n);     // natural order inside a group
+    std::vector<int> grp_of_q(Nq), pos_in_grp(Nq);
+    int max_group = 0;
+    for (int g = 0; g < n_groups; ++g) {
+        max_group = std::max(max_group, (int)members[g].size());
+        for (size_t p = 0; p < members[g].size(); ++p) { grp_of_q[members[g][p]] = g; pos_in_grp[members[g][p]] = (int)p; }
+    }
+
+    // ---------------------------------------------------------------- closure storage + gather lists
+    // per group of size g: P[g*g] (P[m*g+n] = production of m from n), leak[g], p0[g], invD[g]
+    std::vector<int> gbase(n_groups);
+    int cl_size = 0;
+    for (int g = 0; g < n_groups; ++g) { int sz = (int)members[g].size(); gbase[g] = cl_size; cl_size += sz * sz + 3 * sz; }
+    std::map<int, std::vector<int>> ce;                    // closure slot -> directions
+    std::map<std::pair<int, int>, std::vector<int>> xp;    // (m, n) cross-group -> directions
+    for (int j = 0; j < M; ++j)
+        for (int dir = 0; dir < 2; ++dir) {
+            if (!enabled(j, dir)) continue;
+            const int n = R[j].q[dir], m = R[j].q[1 - dir], dd = 2 * j + dir;
+            if (n >= 0) {
+                const int g = grp_of_q[n], sz = (int)members[g].size();
+                if (m >= 0 && m != n && grp_of_q[m] == g) ce[gbase[g] + pos_in_grp[m] * sz + pos_in_grp[n]].push_back(dd);
+                else if (m >= 0 && m != n) { ce[gbase[g] + sz * sz + pos_in_grp[n]].push_back(dd); xp[{m, n}].push_back(dd); }
+                else if (m < 0) ce[gbase[g] + sz * sz + pos_in_grp[n]].push_back(dd);
+            } else if (m >= 0) {
+                const int g = grp_of_q[m], sz = (int)members[g].size();
+                ce[gbase[g] + sz * sz + sz + pos_in_grp[m]].push_back(dd);
+            }
+        }
+    for (int g = 0; g < n_groups; ++g) {                    // every P / leak / p0 slot is written, even when no direction feeds it
+        const int sz = (int)members[g].size();
+        for (int o = 0; o < sz * sz + 2 * sz; ++o) ce[gbase[g] + o];
+    }
+    // cross entries sorted by the group of their target m
+    std::vector<std::pair<std::pair<int, int>, std::vector<int>>> xpl(xp.begin(), xp.end());
+    std::stable_sort(xpl.begin(), xpl.end(), [&](const auto &a, const auto &b) { return grp_of_q[a.first.first] < grp_of_q[b.first.first]; });
+    std::vector<int> xp_begin(n_groups, 0), xp_end(n_groups, 0);
+    for (int g = 0, p = 0; g < n_groups; ++g) {
+        xp_begin[g] = p;
+        while (p < (int)xpl.size() && grp_of_q[xpl[p].first.first] == g) ++p;
+        xp_end[g] = p;
+    }
+
+    // ---------------------------------------------------------------- blobs
+    std::vector<int32_t> &I = out.I; std::vector<double> &D = out.D;
+    I.clear(); D.clear();
+    QssTab &t = out.tab;
+    t = QssTab();
+    t.N = N; t.Nq = Nq; t.M = M; t.nsp = nsp; t.n_tb = n_tb;
+    t.n_groups = n_groups; t.n_levels = n_levels; t.max_group = max_group; t.cl_size = cl_size;
+    auto atI = [&]() { return (int32_t)I.size(); };
+    auto atD = [&]() { return (int32_t)D.size(); };
+
+    // thermo (NASA-7; the h and s polynomials pre-divided as in the definition, reading G4)
+    t.d_thermo = atD();
+    for (int s = 0; s < nsp; ++s) {
+        double rec[QSS_TH_STRIDE] = {0};
+        rec[0] = d->nasa_T[3 * s + 1];
+        for (int rg = 0; rg < 2; ++rg) {
+            const double *a = (rg == 0 ? d->nasa_lo : d->nasa_hi) + 7 * s;
+            double *o = rec + 1 + 11 * rg;
+            o[0] = a[0]; o[1] = a[1] / 2.0; o[2] = a[2] / 3.0; o[3] = a[3] / 4.0; o[4] = a[4] / 5.0; o[5] = a[5];
+            o[6] = a[1]; o[7] = a[2] / 2.0; o[8] = a[3] / 3.0; o[9] = a[4] / 4.0; o[10] = a[6];
+        }
+        D.insert(D.end(), rec, rec + QSS_TH_STRIDE);
+    }
+    const double RGAS = 8.31446261815324;
+    t.d_rate = atD();
+    for (int j = 0; j < M; ++j) {
+        double rec[QSS_RD_STRIDE] = {0};
+        const double A = d->arr[3 * j];
+        if (!(A > 0)) { err = fmt("reaction %d: pre-exponential factor must be > 0", j); return QSS_E_INVALID; }
+        rec[0] = std::log(A); rec[1] = d->arr[3 * j + 1]; rec[2] = d->arr[3 * j + 2] / RGAS;
+        if (R[j].type == 2) {
+            const double A0 = d->arr_low[3 * j];
+            if (!(A0 > 0)) { err = fmt("reaction %d: low-pressure pre-exponential factor must be > 0", j); return QSS_E_INVALID; }
+            rec[3] = std::log(A0); rec[4] = d->arr_low[3 * j + 1]; rec[5] = d->arr_low[3 * j + 2] / RGAS;
+            rec[6] = d->troe[4 * j]; rec[7] = 1.0 / d->troe[4 * j + 1]; rec[8] = 1.0 / d->troe[4 * j + 2]; rec[9] = d->troe[4 * j + 3];
+        }
+        rec[10] = (double)R[j].dnu;
+        D.insert(D.end(), rec, rec + QSS_RD_STRIDE);
+    }
+    // reaction order: fall-off first, then third-body, then Arrhenius (balances the warps of a block)
+    std::vector<int> rorder(M);
+    for (int j = 0; j < M; ++j) rorder[j] = j;
+    std::stable_sort(rorder.begin(), rorder.end(), [&](int a, int b) { return R[a].type > R[b].type; });
+    t.i_reac = atI();
+    for (int j = 0; j < M; ++j) {
+        int32_t rec[QSS_RI_STRIDE] = {R[j].type, R[j].mask, R[j].tb, R[j].q[0], R[j].q[1], 0, 0, 0};
+        I.insert(I.end(), rec, rec + QSS_RI_STRIDE);
+    }
+    t.i_rorder = atI(); I.insert(I.end(), rorder.begin(), rorder.end());
+    // direction reactant lists
+    {
+        std::vector<int32_t> ptr{0}, sp, nu;
+        for (int j = 0; j < M; ++j) for (int dir = 0; dir < 2; ++dir) {
+            for (const Term &x : R[j].side[dir]) { sp.push_back(x.sp); nu.push_back(x.nu); }
+            ptr.push_back((int32_t)sp.size());
+        }
+        t.i_side_ptr = atI(); I.insert(I.end(), ptr.begin(), ptr.end());
+        t.i_side_sp = atI(); I.insert(I.end(), sp.begin(), sp.end());
+        t.i_side_nu = atI(); I.insert(I.end(), nu.begin(), nu.end());
+    }
+    {   // net stoichiometry by reaction
+        std::vector<int32_t> ptr{0}, sp, nu;
+        for (int j = 0; j < M; ++j) { for (const Term &x : R[j].net) { sp.push_back(x.sp); nu.push_back(x.nu); } ptr.push_back((int32_t)sp.size()); }
+        t.i_net_ptr = atI(); I.insert(I.end(), ptr.begin(), ptr.end());
+        t.i_net_sp = atI(); I.insert(I.end(), sp.begin(), sp.end());
+        t.i_net_nu = atI(); I.insert(I.end(), nu.begin(), nu.end());
+    }
+    std::vector<std::vector<std::pair<int, double>>> effc(N);
+    {   // efficiencies by reaction
+        std::vector<int32_t> ptr{0}, sp; std::vector<double> val;
+        for (int j = 0; j < M; ++j) {
+            if (R[j].type >= 1 && d->eff_ptr)
+                for (int p = d->eff_ptr[j]; p < d->eff_ptr[j + 1]; ++p) {
+                    sp.push_back(d->eff_sp[p]); val.push_back(d->eff_val[p] - 1.0);
+                    effc[d->eff_sp[p]].push_back({j, d->eff_val[p] - 1.0});
+                }
+            ptr.push_back((int32_t)sp.size());
+        }
+        t.i_eff_ptr = atI(); I.insert(I.end(), ptr.begin(), ptr.end());
+        t.i_eff_sp = atI(); I.insert(I.end(), sp.begin(), sp.end());
+        t.d_effm1 = atD(); D.insert(D.end(), val.begin(), val.end());
+    }
+    {   // efficiencies by column
+        std::vector<int32_t> ptr{0}, rj; std::vector<double> val;
+        for (int k = 0; k < N; ++k) { for (auto &e : effc[k]) { rj.push_back(e.first); val.push_back(e.second); } ptr.push_back((int32_t)rj.size()); }
+        t.i_effc_ptr = atI(); I.insert(I.end(), ptr.begin(), ptr.end());
+        t.i_effc_reac = atI(); I.insert(I.end(), rj.begin(), rj.end());
+        t.d_effc = atD(); D.insert(D.end(), val.begin(), val.end());
+    }
+    // groups
+    {
+        std::vector<int> lvl_of_group(n_groups);
+        for (int c = 0; c < ncomp; ++c) lvl_of_group[gid[c]] = level[c];
+        t.i_group = atI();
+        int moff = 0;
+        for (int g = 0; g < n_groups; ++g) {
+            int32_t rec[QSS_GI_STRIDE] = {(int32_t)members[g].size(), moff, gbase[g], lvl_of_group[g], xp_begin[g], xp_end[g], 0, 0};
+            I.insert(I.end(), rec, rec + QSS_GI_STRIDE);
+            moff += (int)members[g].size();
+        }
+        t.i_gmember = atI();
+        for (int g = 0; g < n_groups; ++g) I.insert(I.end(), members[g].begin(), members[g].end());
+        std::vector<int32_t> lp(n_levels + 1, 0);
+        for (int g = 0; g < n_groups; ++g) lp[lvl_of_group[g] + 1]++;
+        for (int l = 0; l < n_levels; ++l) lp[l + 1] += lp[l];
+        t.i_level_ptr = atI(); I.insert(I.end(), lp.begin(), lp.end());
+        out.order.clear(); out.group_of.clear(); out.group_size.clear();
+        for (int g = 0; g < n_groups; ++g) {
+            out.group_size.push_back((int)members[g].size());
+            for (int q : members[g]) { out.order.push_back(q); out.group_of.push_back(g); }
+        }
+    }
+    {   // closure gather entries
+        std::vector<int32_t> ptr{0}, dst, dir;
+        for (auto &kv : ce) { dst.push_back(kv.first); dir.insert(dir.end(), kv.second.begin(), kv.second.end()); ptr.push_back((int32_t)dir.size()); }
+        t.n_centry = (int32_t)dst.size();
+        t.i_ce_ptr = atI(); I.insert(I.end(), ptr.begin(), ptr.end());
+        t.i_ce_dst = atI(); I.insert(I.end(), dst.begin(), dst.end());
+        t.i_ce_dir = atI(); I.insert(I.end(), dir.begin(), dir.end());
+    }
+    {   // cross-group couplings
+        std::vector<int32_t> ptr{0}, dir, xm, xn;
+        for (auto &e : xpl) {
+            xm.push_back(pos_in_grp[e.first.first]); xn.push_back(e.first.second);
+            dir.insert(dir.end(), e.second.begin(), e.second.end()); ptr.push_back((int32_t)dir.size());
+        }
+        t.n_xp = (int32_t)xm.size();
+        t.i_xp_ptr = atI(); I.insert(I.end(), ptr.begin(), ptr.end());
+        t.i_xp_dir = atI(); I.insert(I.end(), dir.begin(), dir.end());
+        t.i_xp_m = atI(); I.insert(I.end(), xm.begin(), xm.end());
+        t.i_xp_n = atI(); I.insert(I.end(), xn.begin(), xn.end());
+    }
+    size_t n_inc = 0;
+    {   // species incidence
+        std::vector<std::vector<Term>> inc(nsp);     // (reaction, nu_net)
+        for (int j = 0; j < M; ++j) if (R[j].mask) for (const Term &x : R[j].net) inc[x.sp].push_back({j, x.nu});
+        std::vector<int32_t> ptr{0}, rj, nu;
+        for (int s = 0; s < nsp; ++s) { for (const Term &x : inc[s]) { rj.push_back(x.sp); nu.push_back(x.nu); } ptr.push_back((int32_t)rj.size()); }
+        n_inc = rj.size();
+        t.i_sp_ptr = atI(); I.insert(I.end(), ptr.begin(), ptr.end());
+        t.i_sp_reac = atI(); I.insert(I.end(), rj.begin(), rj.end());
+        t.i_sp_nu = atI(); I.insert(I.end(), nu.begin(), nu.end());
+    }
+    size_t n_wy_terms = 0;
+    {   // W_y[i][q] = sum over directions consuming q of (+-) nu_net(i) kappa_d
+        std::map<std::pair<int, int>, std::vector<std::pair<int, int>>> wy;
+        for (int j = 0; j < M; ++j) for (int dir = 0; dir < 2; ++dir) {
+            if (!enabled(j, dir) || R[j].q[dir] < 0) continue;
+            for (const Term &x : R[j].net) if (x.sp < N) wy[{x.sp, R[j].q[dir]}].push_back({2 * j + dir, dir == 0 ? x.nu : -x.nu});
+        }
+        std::vector<int32_t> ptr{0}, dir, coef, rptr{0}, rq, re;
+        int e = 0, row = 0;
+        for (auto &kv : wy) {
+            while (row < kv.first.first) { rptr.push_back((int32_t)rq.size()); ++row; }
+            rq.push_back(kv.first.second); re.push_back(e++);
+            for (auto &dc : kv.second) { dir.push_back(dc.first); coef.push_back(dc.second); }
+            ptr.push_back((int32_t)dir.size());
+        }
+        while (row < N) { rptr.push_back((int32_t)rq.size()); ++row; }
+        n_wy_terms = dir.size();
+        t.n_wy = e;
+        t.i_wy_ptr = atI(); I.insert(I.end(), ptr.begin(), ptr.end());
+        t.i_wy_dir = atI(); I.insert(I.end(), dir.begin(), dir.end());
+        t.i_wy_coef = atI(); I.insert(I.end(), coef.begin(), coef.end());
+        t.i_wyrow_ptr = atI(); I.insert(I.end(), rptr.begin(), rptr.end());
+        t.i_wyrow_q = atI(); I.insert(I.end(), rq.begin(), rq.end());
+        t.i_wyrow_e = atI(); I.insert(I.end(), re.begin(), re.end());
+    }
+    size_t n_colinc = 0, n_scatter = 0;
+    {   // Jacobian column incidences
+        std::vector<std::vector<std::pair<int, int>>> col(N);
+        for (int j = 0; j < M; ++j) for (int dir = 0; dir < 2; ++dir) {
+            if (!enabled(j, dir)) continue;
+            for (size_t p = 0; p < R[j].side[dir].size(); ++p)
+                if (R[j].side[dir][p].sp < N) { col[R[j].side[dir][p].sp].push_back({2 * j + dir, (int)p}); n_scatter += R[j].net.size(); }
+        }
+        std::vector<int32_t> ptr{0}, dir, pos;
+        for (int k = 0; k < N; ++k) { for (auto &x : col[k]) { dir.push_back(x.first); pos.push_back(x.second); } ptr.push_back((int32_t)dir.size()); }
+        n_colinc = dir.size();
+        t.i_col_ptr = atI(); I.insert(I.end(), ptr.begin(), ptr.end());
+        t.i_col_dir = atI(); I.insert(I.end(), dir.begin(), dir.end());
+        t.i_col_pos = atI(); I.insert(I.end(), pos.begin(), pos.end());
+    }
+    // ---------------------------------------------------------------- per-cell workspace layout (doubles)
+    {
+        int o = 0;
+        auto take = [&](int n) { int r = o; o += n; return r; };
+        t.w_G = take(nsp); t.w_H = take(nsp); t.w_K = take(2 * M); t.w_KAP = take(2 * M);
+        t.w_MM = take(n_tb); t.w_CL = take(cl_size); t.w_XP = take(t.n_xp); t.w_Y = take(Nq); t.w_Q = take(M);
+        t.ws_wdot = o;
+        t.w_DF = take(M); t.w_DC = take(M); t.w_DLM = take(n_tb);
+        t.w_QT = take(M); t.w_QM = take(n_tb); t.w_ET = take(nsp); t.w_TV = take(nsp); t.w_WY = take(t.n_wy);
+        t.w_COL = o; t.ws_jac_base = o;
+    }
+    // ---------------------------------------------------------------- algorithmic cost
+    {
+        const double EXP = 18, LOG = 30, DIV = 24, RCP = 22;
+        double s = 0;
+        s += LOG + RCP + 6 + N;                                   // lnT, 1/T, powers of T, ln(P0/RT), Ctot
+        s += nsp * 13.0;                                          // NASA-7 h and g
+        size_t n_eff = 0, n_side = 0, n_net = 0;
+        int n_troe = 0, n_rev = 0;
+        for (int j = 0; j < M; ++j) {
+            n_side += R[j].side[0].size() + R[j].side[1].size(); n_net += R[j].net.size();
+            if (R[j].type == 2) ++n_troe;
+            if (R[j].mask & 2) ++n_rev;
+            if (R[j].type >= 1 && d->eff_ptr) n_eff += d->eff_ptr[j + 1] - d->eff_ptr[j];
+        }
+        s += M * (2.0 + EXP);                                     // Arrhenius
+        s += n_rev * (EXP + 2.0) + (double)n_side;                // Kc: sum nu g, dnu ln(P0/RT), exp, multiply
+        s += (double)n_eff + n_tb;                                // third-body concentrations
+        s += n_troe * (2.0 + EXP + 3 * EXP + 4 + 2 * LOG + 12 + 2 * DIV + EXP + DIV + 3);   // k0, Fcent, F, Pr/(1+Pr)
+        s += (double)n_side + 2.0 * M;                            // kappa_d products, r_d
+        for (auto &kv : ce) s += kv.second.size();                // closure assembly
+        for (auto &e : xpl) s += e.second.size() + 1;
+        for (int g = 0; g < n_groups; ++g) { double sz = (double)members[g].size(); s += sz * sz * sz / 3.0 + 2 * sz * sz + sz * RCP; }
+        s += M + (double)n_inc;                                   // Q_j and wdot_i
+        out.slots_wdot = s;
+        double jx = 0;
+        jx += nsp * 6.0 + M * 4.0 + n_rev * ((double)n_side / std::max(M, 1) + 3.0);   // h/RT sums, dlnk/dT, dlnKc/dT
+        jx += n_troe * (40.0 + 3 * DIV);                          // fall-off derivatives
+        jx += 3.0 * M + 2.0 * n_inc;                              // QT, QM, ET, t vectors
+        jx += (double)n_wy_terms;                                 // W_y assembly
+        jx += 3.0 * n_colinc + (double)n_scatter;                 // partials (product of others) + scatter
+        for (int k = 0; k < N; ++k) for (auto &e : effc[k]) jx += 1.0 + R[e.first].net.size();   // (alpha-1) corrections
+        jx += (double)nsp * N;                                    // rank-1 third-body term added to every species column
+        double sg2 = 0;
+        for (int g = 0; g < n_groups; ++g) sg2 += (double)members[g].size() * members[g].size();
+        jx += (sg2 + Nq + t.n_xp) * (N + 1);                      // Y_x solves
+        jx += (double)t.n_wy * (N + 1);                           // W_y * Y_x
+        out.slots_jac = s + jx;
+        out.bytes_wdot = 8.0 * (N + 1) + 8.0 * N;
+        out.bytes_jac = 8.0 * (N + 1) + 8.0 * N * (N + 1);
+    }
+    err.clear();
+    return QSS_OK;
+}

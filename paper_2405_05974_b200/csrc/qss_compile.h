@@ -1,0 +1,23 @@
+// Internal: host-side mechanism compiler interface (qss_compile.cpp -> qss_api.cu).
+#ifndef QSS_COMPILE_H
+#define QSS_COMPILE_H
+#include <string>
+#include <vector>
+
+#include "../../include/qss.h"
+#include "qss_tables.h"
+
+struct QssCompiled {
+    QssTab tab;                    // offsets filled in; I / D pointers are set after upload
+    std::vector<int32_t> I;        // host image of the int blob
+    std::vector<double> D;         // host image of the double blob
+    std::vector<int32_t> order;    // [Nq] local QSS index solved i-th
+    std::vector<int32_t> group_of; // [Nq] group (in solve order) of order[i]
+    std::vector<int32_t> group_size;
+    double slots_wdot = 0, slots_jac = 0, bytes_wdot = 0, bytes_jac = 0;
+};
+
+// Validates `desc` and builds the tables. Returns QSS_OK or a negative qss_status with `err` set.
+int qss_compile(const qss_mech_desc_t *desc, QssCompiled &out, std::string &err);
+
+#endif

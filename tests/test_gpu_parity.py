@@ -1,0 +1,151 @@
+"""GPU parity: libqss (CUDA, through the C-ABI binding) against the CPU oracle, element by element on the
+same seeded inputs.  Gates: tests/gates.py (wdot relative 1e-10, Jacobian normwise
+relative 1e-9 per cell and per column, two tiers)."""
+import numpy as np
+import pytest
+
+import gates
+import oracle
+import qss_synth
+from qss_synth import make_states
+
+pytestmark = pytest.mark.gpu
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _gpu_eval(mech, C, T, n_cells, want_jac=True):
+    import paper_2405_05974_b200 as qss
+    torch = _torch()
+    qm = qss.QssMech(mech, 0)
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda()
+    ld = C.shape[1]
+    out = {}
+    # poison outputs so that untouched entries are detected
+    wdot = torch.full((qm.N, ld), float("nan"), dtype=torch.float64, device="cuda")
+    cq = torch.full((max(qm.Nq, 1), ld), float("nan"), dtype=torch.float64, device="cuda")
+    w, y = qm.eval_wdot(Cd, Td, n_cells, wdot=wdot, cqss=cq, want_cqss=True)
+    out["wdot"] = w.cpu().numpy(); out["cqss"] = y.cpu().numpy()
+    if want_jac:
+        jac = torch.full((qm.N, qm.N + 1, ld), float("nan"), dtype=torch.float64, device="cuda")
+        wd2 = torch.full((qm.N, ld), float("nan"), dtype=torch.float64, device="cuda")
+        J, w2 = qm.eval_jac(Cd, Td, n_cells, jac=jac, wdot=wd2, want_wdot=True)
+        out["jac"] = J.cpu().numpy(); out["wdot_from_jac"] = w2.cpu().numpy()
+        jac.fill_(float("nan"))
+        out["jac_only"] = qm.eval_jac(Cd, Td, n_cells, jac=jac).cpu().numpy()
+    torch.cuda.synchronize()
+    qm.close()
+    return out
+
+
+def _check(mech, C, T, n_cells, what, want_jac=True):
+    om = oracle.OracleMech(mech)
+    ref = oracle.evaluate(om, C, T, n_cells, want_jac=want_jac, want_scale=want_jac)
+    got = _gpu_eval(mech, C, T, n_cells, want_jac)
+    n = n_cells
+    g = gates.assert_wdot(got["wdot"], ref["wdot"], ref["S"], n, what + " wdot")
+    if mech.n_qss:
+        y, yr = got["cqss"][:, :n], ref["cqss"][:, :n]
+        assert np.isfinite(y).all() and (y >= 0).all()
+        assert np.max(np.abs(y - yr) / np.abs(yr)) < 1e-9, what + " cqss"
+    # padding cells (c >= n_cells) must not be written
+    if C.shape[1] > n:
+        assert np.isnan(got["wdot"][:, n:]).all(), what + ": wdot padding was written"
+    if want_jac:
+        gates.assert_wdot(got["wdot_from_jac"], ref["wdot"], ref["S"], n, what + " wdot (jac pass)")
+        gj = gates.assert_jac(got["jac"], ref["jac"], ref["jscale"], n, what + " jac")
+        assert np.array_equal(got["jac"][:, :, :n], got["jac_only"][:, :, :n]), what + ": jac differs with/without wdot output"
+        if C.shape[1] > n:
+            assert np.isnan(got["jac"][:, :, n:]).all(), what + ": jac padding was written"
+        g.update(gj)
+    return g
+
+
+@pytest.mark.parametrize("name", ["toy1", "toy2", "toy3", "toy_dag", "toy_nonqss"])
+def test_toys(name):
+    mech = getattr(qss_synth, name)()
+    n = 77                                     # ragged: 2 full warps of cells + a tail, ld padded to 96
+    C, T = make_states(mech.n_nqss, n, seed=5)
+    _check(mech, C, T, n, name)
+
+
+def test_cfg1_full():
+    mech = qss_synth.config_mechanism(1)
+    C, T = qss_synth.config_states(1)
+    _check(mech, C, T, 4096, "cfg1")
+
+
+@pytest.mark.parametrize("cfg,n", [(2, 4096 + 37), (3, 1024 + 5), (5, 160 + 3)])
+def test_configs_small(cfg, n):
+    mech = qss_synth.config_mechanism(cfg)
+    C, T = qss_synth.config_states(cfg, n)
+    g = _check(mech, C, T, n, f"cfg{cfg}")
+    print(f"cfg{cfg}", g)
+
+
+def test_cfg4_field_small():
+    mech = qss_synth.config_mechanism(4)
+    C, T = qss_synth.config_states(4, 16 ** 3)           # 16^3 cells of the multipulse-shaped field
+    _check(mech, np.ascontiguousarray(C), np.ascontiguousarray(T), C.shape[1], "cfg4")
+
+
+@pytest.mark.parametrize("n", [1, 31, 32, 33])
+def test_tiny_and_ragged_cell_counts(n):
+    mech = qss_synth.config_mechanism(1)
+    C, T = make_states(mech.n_nqss, n, seed=11, ld=64)
+    _check(mech, C, T, n, f"cfg1 n={n}")
+
+
+def test_zero_cells_is_a_noop():
+    import paper_2405_05974_b200 as qss
+    torch = _torch()
+    mech = qss_synth.config_mechanism(1)
+    qm = qss.QssMech(mech, 0)
+    C = torch.ones((qm.N, 32), dtype=torch.float64, device="cuda"); T = torch.full((32,), 1000.0, dtype=torch.float64, device="cuda")
+    w = torch.full((qm.N, 32), -7.0, dtype=torch.float64, device="cuda")
+    qm.eval_wdot(C, T, 0, wdot=w)
+    torch.cuda.synchronize()
+    assert (w == -7.0).all()
+
+
+def test_bad_arguments_are_rejected():
+    import paper_2405_05974_b200 as qss
+    torch = _torch()
+    mech = qss_synth.config_mechanism(1)
+    qm = qss.QssMech(mech, 0)
+    C = torch.ones((qm.N, 32), dtype=torch.float64, device="cuda"); T = torch.full((32,), 1000.0, dtype=torch.float64, device="cuda")
+    with pytest.raises(qss.QssError) as e:
+        qm.eval_wdot(C, T, 64)                            # ncells > ld
+    assert e.value.code == -1
+    small = torch.empty(256, dtype=torch.uint8, device="cuda")
+    qm._ws[True] = small
+    with pytest.raises(qss.QssError) as e:
+        qm.eval_jac(C, T, 32)                             # workspace too small
+    assert e.value.code == -1
+
+
+def test_full_size_cfg2_sampled():
+    """BASELINE.json configs[1] at full size (2^20 cells) in the launch configuration bench.py times;
+    256 sampled cells are recomputed one by one by the oracle."""
+    import paper_2405_05974_b200 as qss
+    torch = _torch()
+    mech = qss_synth.config_mechanism(2)
+    C, T = qss_synth.config_states(2)
+    n = C.shape[1]
+    qm = qss.QssMech(mech, 0)
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda()
+    J, w = qm.eval_jac(Cd, Td, n, want_wdot=True)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(99)
+    idx = np.sort(rng.choice(n, size=256, replace=False))
+    idx[0], idx[-1] = 0, n - 1
+    it = torch.from_numpy(idx).cuda()
+    Js = J[:, :, it].cpu().numpy(); ws = w[:, it].cpu().numpy()
+    assert torch.isfinite(w).all() and torch.isfinite(J).all()
+    Cs = np.ascontiguousarray(C[:, idx]); Ts = np.ascontiguousarray(T[idx])
+    ref = oracle.evaluate(oracle.OracleMech(mech), Cs, Ts, want_jac=True, want_scale=True)
+    gates.assert_wdot(ws, ref["wdot"], ref["S"], what="cfg2 full wdot")
+    gates.assert_jac(Js, ref["jac"], ref["jscale"], what="cfg2 full jac")
