@@ -1,0 +1,281 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the QSS-chemistry hot path (wdot + analytical QSS Jacobian, fp64) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A "step" is one pass of the whole hot path (rate constants -> QSS closure -> wdot ->
+analytical Jacobian with the chain rule, Eq. 2-4, 6, 7, 9) over one batch of synthetic cells: one
+`qss_eval_jac` call with the wdot output enabled.  Workload at N=1: BASELINE.json configs[1] (the mid-size
+35+18-species, 270-reaction synthetic mechanism, 2^20 cells), the config the metric's target is quoted on.
+At N>1 every rank evaluates its own 2^20 cells (cells are independent: no data-path collective; "weak").
+
+Prints ONE JSON line (rank 0).  Keys: DESIGN.md "Measurement".
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores on a bounded sample of the
+same workload; the oracle is never used on the product path.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cells/sec for wdot+analytical QSS Jacobian (fp64) per B200; % of roofline"
+UNIT = "cells/s"
+ORACLE_SAMPLE = {1: 4096, 2: 1 << 14, 3: 1 << 12, 4: 1 << 14, 5: 1 << 9}   # cells of the CPU-oracle sample
+FP64_LANES_PER_SM = 64          # 148 SMs x 64 fp64 FMA lanes x 1.965 GHz
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "MEASURED_PEAKS.json", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback (B200_PROFILING.md)", 1965.0
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except Exception:
+            self.p.kill(); out = ""
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def run_reference(args, cfg: int, rank: int):
+    """The oracle, as it stands, on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    import numpy as np
+    import oracle
+    import qss_synth
+    mech = qss_synth.config_mechanism(cfg)
+    n = ORACLE_SAMPLE[cfg]
+    C, T = qss_synth.config_states(cfg, n)
+    n = min(n, C.shape[1])
+    om = oracle.OracleMech(mech)
+    cores = oracle.max_threads()
+    for _ in range(args.warmup):
+        oracle.evaluate(om, C, T, min(n, 256), want_jac=True)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.evaluate(om, C, T, n, want_jac=True)
+    dt = (time.perf_counter() - t0) / args.steps
+    v = n / dt
+    sample = f"first {n} cells of cfg{cfg} per step (explicit-formula fp64 oracle, OpenMP over cells)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": _config(cfg, mech, n, args.gpus),
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def _config(cfg, mech, n_cells, n_gpus):
+    return {"workload": f"BASELINE.json configs[{cfg - 1}] (cfg{cfg}): synthetic QSS mechanism {mech.n_nqss} transported + "
+                        f"{mech.n_qss} QSS species, {mech.n_reac} reactions; {n_cells} cells per GPU; Jacobian "
+                        f"{mech.n_nqss}x{mech.n_nqss + 1} per cell + wdot",
+            "cfg": cfg, "n_nqss": mech.n_nqss, "n_qss": mech.n_qss, "n_reac": mech.n_reac, "cells_per_gpu": n_cells,
+            "parallelism": f"cells sharded over {n_gpus} GPU(s), no collective",
+            "l2_policy": "inputs (C,T) and outputs (J,wdot) per step exceed the 126 MB L2; no flush needed"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (1-based); default 2 = configs[1]")
+    ap.add_argument("--cells", type=int, default=0, help="override the cell count (0 = the config's)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = args.config
+    if args.impl == "reference":
+        run_reference(args, cfg, rank)
+        return
+
+    import numpy as np
+    import torch
+    import qss_synth
+    import paper_2405_05974_b200 as qss
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libqss has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    mech = qss_synth.config_mechanism(cfg)
+    n_full = qss_synth.CONFIGS[cfg]["n_cells"]
+    n = args.cells or n_full
+    C, T = qss_synth.config_states(cfg, n)
+    n = min(n, C.shape[1]) if cfg == 4 else n
+    ld = C.shape[1]
+    qm = qss.QssMech(mech, local)
+    N = qm.N
+    Cd = torch.from_numpy(C).to(dev); Td = torch.from_numpy(T).to(dev)
+    J = torch.empty((N, N + 1, ld), dtype=torch.float64, device=dev)
+    W = torch.empty((N, ld), dtype=torch.float64, device=dev)
+    qm.workspace(True)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        qm.eval_jac(Cd, Td, n, jac=J, wdot=W, want_wdot=True)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- fp64 FMA-pipe peak, measured in the same run (roofline denominator cross-check)
+    sink = torch.zeros(8, dtype=torch.float64, device=dev)
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    qss.bench_dfma(sms * 8, 200, sink); torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream); nf = qss.bench_dfma(sms * 8, 4000, sink); e1.record(stream); torch.cuda.synchronize()
+    dfma_slots_s = nf / (e0.elapsed_time(e1) * 1e-3)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    evs[0].record(stream)
+    for i in range(args.steps):
+        step()
+        evs[i + 1].record(stream)
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    total_ms = evs[0].elapsed_time(evs[-1])
+    launch_ms = [evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)]
+    tt = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    total_ms_max = float(tt.item())
+    value = world * n * args.steps / (total_ms_max * 1e-3)
+
+    # ---- end to end through the C-ABI host-buffer call: pinned host buffers, H2D + D2H inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        del J, W
+        torch.cuda.empty_cache()
+        Ch = torch.from_numpy(C).pin_memory(); Th = torch.from_numpy(T).pin_memory()
+        Jh = torch.empty((N, N + 1, ld), dtype=torch.float64).pin_memory()
+        Wh = torch.empty((N, ld), dtype=torch.float64).pin_memory()
+        scratch = torch.empty(qm.host_scratch_bytes(n, ld) + 256, dtype=torch.uint8, device=dev)
+        ke = max(1, min(args.steps, 3))
+        qm.eval_jac_host(Ch, Th, Jh, Wh, scratch, n)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ke):
+            qm.eval_jac_host(Ch, Th, Jh, Wh, scratch, n)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        te = torch.tensor([dt], dtype=torch.float64, device=dev)
+        if dist is not None:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * n * ke / float(te.item()), "unit": UNIT,
+               "h2d_bytes_per_step": int((N + 1) * ld * 8), "d2h_bytes_per_step": int((N * (N + 1) + N) * ld * 8),
+               "steps": ke, "api": "qss_eval_jac_host (C-ABI, pinned host buffers, copies + kernel + sync timed by wall clock)"}
+        assert bool(torch.isfinite(Wh[:, :n]).all())
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant (only) kernel: qss Jacobian kernel
+    hbm_gbs, peak_src, sm_max_mhz = _peaks()
+    info = qm.info
+    avg_s = statistics.mean(launch_ms) * 1e-3
+    bytes_launch = (info.bytes_jac + 8.0 * N) * n            # + wdot written
+    slots_launch = info.slots_jac * n
+    fp64_peak_slots = sms * FP64_LANES_PER_SM * sm_max_mhz * 1e6
+    t_hbm = bytes_launch / (hbm_gbs * 1e9); t_alu = slots_launch / fp64_peak_slots
+    if t_alu >= t_hbm:
+        roof = {"bound": "alu", "achieved": 2 * slots_launch / avg_s / 1e12, "peak": 2 * fp64_peak_slots / 1e12, "unit": "TFLOP/s"}
+    else:
+        roof = {"bound": "hbm", "achieved": bytes_launch / avg_s / 1e9, "peak": hbm_gbs, "unit": "GB/s"}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof.update({"traffic": None, "kernel": "qss jacobian kernel (qss_eval_jac, wdot output on)",
+                 "launch_ms_avg": avg_s * 1e3, "launch_ms_min": min(launch_ms),
+                 "alg_fp64_slots_per_cell": info.slots_jac, "alg_bytes_per_cell": info.bytes_jac + 8.0 * N,
+                 "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3,
+                 "hbm_achieved_gbs": bytes_launch / avg_s / 1e9, "hbm_frac": bytes_launch / avg_s / 1e9 / hbm_gbs,
+                 "peak_source": f"alu: {sms} SMs x {FP64_LANES_PER_SM} fp64 FMA lanes x {sm_max_mhz:.0f} MHz (nominal; DESIGN.md); "
+                                f"hbm: {peak_src}",
+                 "dfma_measured_tflops": 2 * dfma_slots_s / 1e12})
+
+    cpu = None
+    if not args.no_cpu:
+        import oracle
+        ns = min(ORACLE_SAMPLE[cfg], n)
+        Cs = np.ascontiguousarray(C[:, :ns]); Ts = np.ascontiguousarray(T[:ns])
+        om = oracle.OracleMech(mech)
+        oracle.evaluate(om, Cs, Ts, min(ns, 256), want_jac=True)
+        t0 = time.perf_counter()
+        oracle.evaluate(om, Cs, Ts, ns, want_jac=True)
+        dt = time.perf_counter() - t0
+        cpu = {"value": ns / dt, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+               "sample": f"first {ns} cells of the same cfg{cfg} input, explicit-formula fp64 oracle, OpenMP over cells, {dt:.2f} s"}
+
+    print(json.dumps({
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": _config(cfg, mech, n, world),
+        "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps, "roofline": roof, "cpu_baseline": cpu,
+        "kernel_variant": {"wdot": info.kernel_variant_wdot, "jac": info.kernel_variant_jac}}))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

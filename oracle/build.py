@@ -1,4 +1,5 @@
-"""Builds oracle/liboracle.so (host only, g++ -O2 -march=native -fopenmp). TEST INFRASTRUCTURE."""
+"""Builds oracle/liboracle.so (host only, g++ -O2 -fopenmp; no -march=native: the built library travels to
+another host). TEST INFRASTRUCTURE."""
 from __future__ import annotations
 
 import os
@@ -16,7 +17,7 @@ def build(force: bool = False) -> str:
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
     # -ffp-contract=off: the oracle is the plain definition, operation by operation (no fused multiply-add)
-    cmd = ["g++", "-O2", "-march=native", "-ffp-contract=off", "-fopenmp", "-std=c++17", "-fPIC", "-shared",
+    cmd = ["g++", "-O2", "-ffp-contract=off", "-fopenmp", "-std=c++17", "-fPIC", "-shared",
            "-o", tmp, SRC, "-lquadmath"]
     subprocess.run(cmd, check=True)
     os.replace(tmp, LIB)
