@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libqss.so")
-SOURCES = ["qss_api.cu", "qss_kernels.cu", "qss_compile.cpp"]
+SOURCES = ["qss_api.cu", "qss_kernels.cu", "qss_kernel_v1.cu", "qss_compile.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 

@@ -2,6 +2,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -14,6 +15,9 @@ cudaError_t qss_launch_slab(const QssTab &t, bool jac, int64_t ncells, int64_t l
                             double *wdot, double *cqss, double *jacp, double *ws, int nblocks, int nwarp,
                             cudaStream_t stream);
 cudaError_t qss_launch_dfma(int blocks, int iters, double *sink, cudaStream_t stream);
+size_t qss_v1_scratch_doubles(const QssV1 &v);
+cudaError_t qss_v1_prepare();
+cudaError_t qss_launch_v1(const QssV1 &v, bool jac, int nblocks, cudaStream_t stream);
 
 struct qss_mech {
     QssCompiled c;
@@ -24,6 +28,7 @@ struct qss_mech {
     int nwarp = 8;            // warps per block of the slab kernel
     int blocks_per_sm = 2;
     int nblocks = 0;
+    int variant = 0;          // 0: general slab kernel (workspace in global memory); 1: slab-smem kernel (qss_kernel_v1.cu)
 };
 
 namespace {
@@ -89,6 +94,14 @@ extern "C" int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech
     if (e == cudaSuccess && m->c.D.size()) e = cudaMemcpy(m->dD, m->c.D.data(), m->c.D.size() * sizeof(double), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(m->dI); cudaFree(m->dD); delete m; return cuda_fail(e, "cudaMemcpy(tables)"); }
     m->c.tab.I = m->dI; m->c.tab.D = m->dD;
+    // kernel selection: variant 1 when the mechanism fits it (QSS_VARIANT=0 in the environment forces the general kernel)
+    const char *force = std::getenv("QSS_VARIANT");
+    if (m->c.v1_ok && !(force && force[0] == '0')) {
+        if ((e = qss_v1_prepare()) != cudaSuccess) { cudaFree(m->dI); cudaFree(m->dD); delete m; return cuda_fail(e, "cudaFuncSetAttribute(variant 1)"); }
+        m->variant = 1;
+        m->nblocks = m->n_sm;
+        m->c.v1.gI = m->dI; m->c.v1.gD = m->dD;
+    }
     *out = m;
     return QSS_OK;
 }
@@ -117,6 +130,7 @@ extern "C" int qss_mech_destroy(qss_mech_t *m) {
 }
 
 static size_t ws_bytes(const qss_mech_t *m, bool jac) {
+    if (m->variant == 1) return qss_v1_scratch_doubles(m->c.v1) * sizeof(double) * (size_t)m->nblocks;
     return qss_slab_ws_doubles(m->c.tab, jac, m->nwarp) * sizeof(double) * (size_t)m->nblocks;
 }
 
@@ -131,7 +145,7 @@ extern "C" int qss_mech_info(const qss_mech_t *m, qss_mech_info_t *o) {
     o->bytes_wdot = m->c.bytes_wdot; o->bytes_jac = m->c.bytes_jac;
     o->workspace_bytes_wdot = ws_bytes(m, false);
     o->workspace_bytes_jac = ws_bytes(m, true);
-    o->kernel_variant_wdot = 0; o->kernel_variant_jac = 0;
+    o->kernel_variant_wdot = m->variant; o->kernel_variant_jac = m->variant;
     return QSS_OK;
 }
 
@@ -145,8 +159,16 @@ extern "C" int qss_eval_wdot(const qss_mech_t *m, int64_t ncells, int64_t ld, co
                              double *wdot, double *cqss, void *workspace, size_t workspace_bytes, void *stream) {
     int rc = check_eval(m, ncells, ld, C, T, wdot, workspace, workspace_bytes, m ? ws_bytes(m, false) : 0);
     if (rc != QSS_OK || ncells == 0) return rc;
-    cudaError_t e = qss_launch_slab(m->c.tab, false, ncells, ld, C, T, wdot, cqss, nullptr, (double *)workspace,
-                                    m->nblocks, m->nwarp, (cudaStream_t)stream);
+    cudaError_t e;
+    if (m->variant == 1) {
+        QssV1 v = m->c.v1;
+        v.C = C; v.T = T; v.wdot = wdot; v.cqss = cqss; v.jac = nullptr; v.scratch = (double *)workspace;
+        v.ncells = ncells; v.ld = ld; v.scratch_stride = (int64_t)qss_v1_scratch_doubles(v);
+        e = qss_launch_v1(v, false, m->nblocks, (cudaStream_t)stream);
+    } else {
+        e = qss_launch_slab(m->c.tab, false, ncells, ld, C, T, wdot, cqss, nullptr, (double *)workspace, m->nblocks, m->nwarp,
+                            (cudaStream_t)stream);
+    }
     return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_eval_wdot launch");
 }
 
@@ -154,8 +176,16 @@ extern "C" int qss_eval_jac(const qss_mech_t *m, int64_t ncells, int64_t ld, con
                             double *jac, double *wdot, void *workspace, size_t workspace_bytes, void *stream) {
     int rc = check_eval(m, ncells, ld, C, T, jac, workspace, workspace_bytes, m ? ws_bytes(m, true) : 0);
     if (rc != QSS_OK || ncells == 0) return rc;
-    cudaError_t e = qss_launch_slab(m->c.tab, true, ncells, ld, C, T, wdot, nullptr, jac, (double *)workspace,
-                                    m->nblocks, m->nwarp, (cudaStream_t)stream);
+    cudaError_t e;
+    if (m->variant == 1) {
+        QssV1 v = m->c.v1;
+        v.C = C; v.T = T; v.wdot = wdot; v.cqss = nullptr; v.jac = jac; v.scratch = (double *)workspace;
+        v.ncells = ncells; v.ld = ld; v.scratch_stride = (int64_t)qss_v1_scratch_doubles(v);
+        e = qss_launch_v1(v, true, m->nblocks, (cudaStream_t)stream);
+    } else {
+        e = qss_launch_slab(m->c.tab, true, ncells, ld, C, T, wdot, nullptr, jac, (double *)workspace, m->nblocks, m->nwarp,
+                            (cudaStream_t)stream);
+    }
     return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_eval_jac launch");
 }
 

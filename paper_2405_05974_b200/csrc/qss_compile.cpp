@@ -11,6 +11,7 @@
 #include <cmath>
 #include <cstdio>
 #include <functional>
+#include <cstring>
 #include <map>
 
 namespace {
@@ -75,6 +76,234 @@ int tarjan(int n, const std::vector<std::vector<int>> &adj, std::vector<int> &co
         }
     }
     return ncomp;
+}
+
+
+// ---------------------------------------------------------------------------------------------------------
+// Kernel variant 1 ("slab-smem", qss_kernel_v1.cu): hot tables for the kernel-parameter constant bank, reaction
+// records, shared-memory / scratch layout.  Applies when the mechanism is small enough (see the checks below);
+// otherwise the general variant 0 is used.
+// ---------------------------------------------------------------------------------------------------------
+struct V1Ctx {
+    int N, Nq, M, nsp, n_tb, n_groups, n_levels, cl_size;
+    const std::vector<Reaction> *R;
+    const std::vector<std::vector<int>> *members;
+    const std::vector<int> *gbase, *xp_begin, *xp_end, *lvl_of_group, *pos_in_grp, *rorder;
+    const std::map<int, std::vector<int>> *ce;
+    const std::vector<std::pair<std::pair<int, int>, std::vector<int>>> *xpl;
+    const std::vector<std::vector<std::pair<int, double>>> *effc;
+};
+
+bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
+    const int N = c.N, Nq = c.Nq, M = c.M, nsp = c.nsp;
+    const std::vector<Reaction> &R = *c.R;
+    QssV1 &v = out.v1;
+    v = QssV1();
+    if (N > QSS_V1_NT || Nq > QSS_V1_NQ) { why = "more species than the register column of variant 1 holds"; return false; }
+    if (2 * M > 4096 || c.n_tb + 1 >= 4096) { why = "too many reactions for the packed tables of variant 1"; return false; }
+    for (int j = 0; j < M; ++j) {
+        for (int s = 0; s < 2; ++s) { int n = 0; for (const Term &x : R[j].side[s]) n += x.nu; if (n > 3) { why = "a reaction side has more than 3 molecules"; return false; } }
+        for (const Term &x : R[j].net) if (x.nu < -7 || x.nu > 7) { why = "net stoichiometric coefficient out of range"; return false; }
+    }
+    std::vector<int32_t> H;
+    auto at = [&]() { return (int32_t)H.size(); };
+    auto nucode = [](int nu) { return nu + 8; };
+    // closure gather
+    {
+        std::vector<int32_t> ptr{0}, dst, dir;
+        for (auto &kv : *c.ce) { dst.push_back(kv.first); dir.insert(dir.end(), kv.second.begin(), kv.second.end()); ptr.push_back((int32_t)dir.size()); }
+        v.n_centry = (int32_t)dst.size();
+        v.h_ce_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
+        v.h_ce_dst = at(); H.insert(H.end(), dst.begin(), dst.end());
+        v.h_ce_dir = at(); H.insert(H.end(), dir.begin(), dir.end());
+    }
+    {
+        std::vector<int32_t> ptr{0}, dir, xm, xn;
+        for (auto &e : *c.xpl) {
+            xm.push_back((*c.pos_in_grp)[e.first.first]); xn.push_back(e.first.second);
+            dir.insert(dir.end(), e.second.begin(), e.second.end()); ptr.push_back((int32_t)dir.size());
+        }
+        v.n_xp = (int32_t)xm.size();
+        v.h_xp_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
+        v.h_xp_dir = at(); H.insert(H.end(), dir.begin(), dir.end());
+        v.h_xp_m = at(); H.insert(H.end(), xm.begin(), xm.end());
+        v.h_xp_n = at(); H.insert(H.end(), xn.begin(), xn.end());
+    }
+    {
+        v.h_group = at();
+        int moff = 0;
+        for (int g = 0; g < c.n_groups; ++g) {
+            const int sz = (int)(*c.members)[g].size();
+            int32_t rec[QSS_GI_STRIDE] = {sz, moff, (*c.gbase)[g], (*c.lvl_of_group)[g], (*c.xp_begin)[g], (*c.xp_end)[g], 0, 0};
+            H.insert(H.end(), rec, rec + QSS_GI_STRIDE);
+            moff += sz;
+        }
+        v.h_gmember = at();
+        for (int g = 0; g < c.n_groups; ++g) H.insert(H.end(), (*c.members)[g].begin(), (*c.members)[g].end());
+        std::vector<int32_t> lp(c.n_levels + 1, 0);
+        for (int g = 0; g < c.n_groups; ++g) lp[(*c.lvl_of_group)[g] + 1]++;
+        for (int l = 0; l < c.n_levels; ++l) lp[l + 1] += lp[l];
+        v.h_level_ptr = at(); H.insert(H.end(), lp.begin(), lp.end());
+    }
+    // V rows: transported s -> s, the constant 1 -> N, QSS q -> N + 1 + q
+    auto vrow = [&](int sp) { return sp < N ? sp : N + 1 + (sp - N); };
+    {   // per reaction: V rows of the QSS reactant of each direction (or the 1.0 row), third-body index
+        v.h_q = at();
+        for (int j = 0; j < M; ++j) {
+            const int qf = R[j].q[0] >= 0 ? N + 1 + R[j].q[0] : N, qb = R[j].q[1] >= 0 ? N + 1 + R[j].q[1] : N;
+            H.push_back(qf | (qb << 8) | ((R[j].tb + 1) << 16));
+        }
+    }
+    const int nw_max = 12;
+    // species incidence lists and their balanced assignment to warps (filled once nw is known)
+    std::vector<std::vector<int32_t>> ss(nsp);
+    for (int j = 0; j < M; ++j) if (R[j].mask) for (const Term &x : R[j].net) ss[x.sp].push_back(j | (nucode(x.nu) << 12) | ((R[j].tb + 1) << 16));
+    {
+        std::vector<int32_t> ptr{0}, all;
+        for (int s = 0; s < nsp; ++s) { all.insert(all.end(), ss[s].begin(), ss[s].end()); ptr.push_back((int32_t)all.size()); }
+        v.h_ss_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
+        v.h_ss = at(); H.insert(H.end(), all.begin(), all.end());
+    }
+    // W_y entries, row-major (i, then q): gather lists over the directions consuming q
+    std::map<std::pair<int, int>, std::vector<int32_t>> wy;
+    for (int j = 0; j < M; ++j) for (int dir = 0; dir < 2; ++dir) {
+        if (!((R[j].mask >> dir) & 1) || R[j].q[dir] < 0) continue;
+        for (const Term &x : R[j].net) if (x.sp < N) wy[{x.sp, R[j].q[dir]}].push_back((2 * j + dir) | (nucode(dir == 0 ? x.nu : -x.nu) << 12));
+    }
+    {
+        std::vector<int32_t> ptr{0}, all, rptr{0}, rq;
+        int row = 0;
+        for (auto &kv : wy) {
+            while (row < kv.first.first) { rptr.push_back((int32_t)rq.size()); ++row; }
+            rq.push_back(kv.first.second);
+            all.insert(all.end(), kv.second.begin(), kv.second.end()); ptr.push_back((int32_t)all.size());
+        }
+        while (row < N) { rptr.push_back((int32_t)rq.size()); ++row; }
+        v.n_wy = (int32_t)rq.size();
+        v.h_wya_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
+        v.h_wya = at(); H.insert(H.end(), all.begin(), all.end());
+        v.h_wyrow_ptr = at(); H.insert(H.end(), rptr.begin(), rptr.end());
+        v.h_wyq = at(); H.insert(H.end(), rq.begin(), rq.end());
+    }
+    // column incidences: one per (enabled direction, molecule slot holding a transported species)
+    std::vector<std::vector<int32_t>> inc(N);
+    {
+        for (int j = 0; j < M; ++j) for (int dir = 0; dir < 2; ++dir) {
+            if (!((R[j].mask >> dir) & 1)) continue;
+            std::vector<int> slots;                          // species of each molecule of the reactant side
+            for (const Term &x : R[j].side[dir]) for (int u = 0; u < x.nu; ++u) slots.push_back(x.sp);
+            for (size_t p = 0; p < slots.size(); ++p) {
+                if (slots[p] >= N) continue;
+                int o[2] = {N, N}, no = 0;
+                for (size_t q = 0; q < slots.size(); ++q) if (q != p) o[no++] = vrow(slots[q]);
+                inc[slots[p]].push_back((2 * j + dir) | (o[0] << 12) | (o[1] << 20));
+            }
+        }
+        std::vector<int32_t> ptr{0}, all;
+        for (int k = 0; k < N; ++k) { all.insert(all.end(), inc[k].begin(), inc[k].end()); ptr.push_back((int32_t)all.size()); }
+        v.h_col_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
+        v.h_inc = at(); H.insert(H.end(), all.begin(), all.end());
+    }
+    {   // net stoichiometry by reaction; register slot: transported s -> s, QSS q -> QSS_V1_NT + q
+        std::vector<int32_t> ptr{0}, all;
+        for (int j = 0; j < M; ++j) {
+            for (const Term &x : R[j].net) all.push_back((x.sp < N ? x.sp : QSS_V1_NT + (x.sp - N)) | (nucode(x.nu) << 8));
+            ptr.push_back((int32_t)all.size());
+        }
+        v.h_net_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
+        v.h_net = at(); H.insert(H.end(), all.begin(), all.end());
+    }
+    {   // (alpha_k - 1) dQ/dM corrections by column
+        std::vector<int32_t> ptr{0}, all; std::vector<double> val;
+        for (int k = 0; k < N; ++k) {
+            for (auto &e : (*c.effc)[k]) if (R[e.first].mask) { all.push_back(e.first | (R[e.first].tb << 12)); val.push_back(e.second); }
+            ptr.push_back((int32_t)all.size());
+        }
+        v.h_effc_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
+        v.h_effc = at(); H.insert(H.end(), all.begin(), all.end());
+        if (H.size() & 1) H.push_back(0);
+        v.h_effc_val = at();
+        for (double x : val) { int32_t w[2]; std::memcpy(w, &x, 8); H.push_back(w[0]); H.push_back(w[1]); }
+    }
+    {
+        if (H.size() & 1) H.push_back(0);
+        v.h_nulut = at();
+        for (int cde = 0; cde < 16; ++cde) { double x = (double)(cde - 8); int32_t w[2]; std::memcpy(w, &x, 8); H.push_back(w[0]); H.push_back(w[1]); }
+    }
+    // ---- shared-memory layout and the number of warps
+    const int n_wy = v.n_wy;
+    int rows_fixed = 0;
+    auto take = [&](int n) { int r = rows_fixed; rows_fixed += n; return r; };
+    v.s_V = take(N + 1 + Nq); v.s_CT = take(1); v.s_CL = take(c.cl_size); v.s_XP = take(v.n_xp); v.s_TV = take(nsp); v.s_QM = take(c.n_tb);
+    const int max_rows = (227 * 1024) / 256;
+    int nw = 0;
+    for (int cand = nw_max; cand >= 4; --cand) {
+        const int region = std::max(std::max(n_wy + cand * Nq, 2 * (nsp + 1)), M);
+        if (rows_fixed + region <= max_rows) { nw = cand; break; }
+    }
+    if (nw == 0) { why = "per-cell state does not fit the shared memory of one SM"; return false; }
+    const int region = std::max(std::max(n_wy + nw * Nq, 2 * (nsp + 1)), M);
+    v.nw = nw;
+    v.s_WY = rows_fixed; v.s_YC = rows_fixed + n_wy;
+    v.s_G = rows_fixed; v.s_H = rows_fixed + nsp + 1;
+    v.s_Q = rows_fixed; v.s_QT = region >= 2 * M ? rows_fixed + M : -1;
+    v.smem_rows = rows_fixed + region;
+    {
+        int o = 0;
+        auto tk = [&](int n) { int r = o; o += n; return r; };
+        v.g_K = tk(2 * M); v.g_KAP = tk(2 * M); v.g_DF = tk(M); v.g_DC = tk(M); v.g_ET = tk(nsp);
+        v.scratch_rows = o;
+    }
+    // ---- balanced (longest-processing-time) assignment of species sums and Jacobian columns to warps
+    auto lpt = [&](const std::vector<double> &cost, int32_t &h_ptr, int32_t &h_list) {
+        std::vector<int> idx(cost.size());
+        for (size_t i = 0; i < idx.size(); ++i) idx[i] = (int)i;
+        std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return cost[a] > cost[b]; });
+        std::vector<std::vector<int32_t>> bin(nw);
+        std::vector<double> load(nw, 0.0);
+        for (int i : idx) { int b = (int)(std::min_element(load.begin(), load.end()) - load.begin()); bin[b].push_back(i); load[b] += cost[i]; }
+        std::vector<int32_t> ptr{0}, all;
+        for (int w = 0; w < nw; ++w) { all.insert(all.end(), bin[w].begin(), bin[w].end()); ptr.push_back((int32_t)all.size()); }
+        h_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
+        h_list = at(); H.insert(H.end(), all.begin(), all.end());
+    };
+    {
+        std::vector<double> cost(nsp);
+        for (int s = 0; s < nsp; ++s) cost[s] = 6.0 + (double)ss[s].size();
+        lpt(cost, v.h_ssw_ptr, v.h_ssw);
+        std::vector<double> ccost(N + 1);
+        for (int k = 0; k < N; ++k) {
+            double sc = 0; for (int32_t w : inc[k]) sc += 10.0 + 7.0 * R[(w & 4095) >> 1].net.size();
+            for (auto &e : (*c.effc)[k]) sc += 6.0 + 7.0 * R[e.first].net.size();
+            ccost[k] = 600.0 + 5.0 * n_wy + sc;
+        }
+        ccost[N] = 600.0 + 5.0 * n_wy;
+        lpt(ccost, v.h_cw_ptr, v.h_cw);
+    }
+    if ((int)H.size() > QSS_V1_HMAX) { why = "hot tables exceed the kernel-parameter budget of variant 1"; return false; }
+    v.h_used = (int32_t)H.size();
+    std::memcpy(v.h, H.data(), H.size() * sizeof(int32_t));
+    // ---- reaction records (appended to the int blob), in processing order
+    {
+        std::vector<int32_t> &I = out.I;
+        while (I.size() & 3) I.push_back(0);               // records are read as 16-byte vectors
+        v.i_rrec = (int32_t)I.size();
+        for (int r = 0; r < M; ++r) {
+            const int j = (*c.rorder)[r];
+            int32_t rec[QSS_V1_RREC] = {j, R[j].type | (R[j].mask << 2) | ((R[j].tb + 1) << 4), 0, 0, 0, 0, 0, 0};
+            for (int s = 0; s < 2; ++s) {
+                int kap[3] = {N, N, N}, gr[3] = {nsp, nsp, nsp}, n = 0;
+                for (const Term &x : R[j].side[s]) for (int u = 0; u < x.nu; ++u) { kap[n] = x.sp < N ? x.sp : N; gr[n] = x.sp; ++n; }
+                rec[2 + s] = kap[0] | (kap[1] << 8) | (kap[2] << 16);
+                rec[4 + s] = gr[0] | (gr[1] << 8) | (gr[2] << 16);
+            }
+            I.insert(I.end(), rec, rec + QSS_V1_RREC);
+        }
+    }
+    v.N = N; v.Nq = Nq; v.M = M; v.nsp = nsp; v.n_tb = c.n_tb; v.n_groups = c.n_groups; v.n_levels = c.n_levels;
+    v.d_thermo = out.tab.d_thermo; v.d_rate = out.tab.d_rate; v.d_effm1 = out.tab.d_effm1;
+    v.i_eff_ptr = out.tab.i_eff_ptr; v.i_eff_sp = out.tab.i_eff_sp;
+    return true;
 }
 
 }  // namespace
@@ -304,9 +533,9 @@ int qss_compile(const qss_mech_desc_t *d, QssCompiled &out, std::string &err) {
         t.d_effc = atD(); D.insert(D.end(), val.begin(), val.end());
     }
     // groups
+    std::vector<int> lvl_of_group(n_groups);
+    for (int c = 0; c < ncomp; ++c) lvl_of_group[gid[c]] = level[c];
     {
-        std::vector<int> lvl_of_group(n_groups);
-        for (int c = 0; c < ncomp; ++c) lvl_of_group[gid[c]] = level[c];
         t.i_group = atI();
         int moff = 0;
         for (int g = 0; g < n_groups; ++g) {
@@ -447,6 +676,11 @@ int qss_compile(const qss_mech_desc_t *d, QssCompiled &out, std::string &err) {
         out.slots_jac = s + jx;
         out.bytes_wdot = 8.0 * (N + 1) + 8.0 * N;
         out.bytes_jac = 8.0 * (N + 1) + 8.0 * N * (N + 1);
+    }
+    {
+        V1Ctx vc{N, Nq, M, nsp, n_tb, n_groups, n_levels, cl_size, &R, &members, &gbase, &xp_begin, &xp_end, &lvl_of_group,
+                 &pos_in_grp, &rorder, &ce, &xpl, &effc};
+        out.v1_ok = build_v1(vc, out, out.v1_why);
     }
     err.clear();
     return QSS_OK;

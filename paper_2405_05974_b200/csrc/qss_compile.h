@@ -6,6 +6,7 @@
 
 #include "../../include/qss.h"
 #include "qss_tables.h"
+#include "qss_v1.h"
 
 struct QssCompiled {
     QssTab tab;                    // offsets filled in; I / D pointers are set after upload
@@ -15,6 +16,9 @@ struct QssCompiled {
     std::vector<int32_t> group_of; // [Nq] group (in solve order) of order[i]
     std::vector<int32_t> group_size;
     double slots_wdot = 0, slots_jac = 0, bytes_wdot = 0, bytes_jac = 0;
+    QssV1 v1;                      // launch descriptor of kernel variant 1 (valid iff v1_ok)
+    bool v1_ok = false;
+    std::string v1_why;            // why variant 1 does not apply
 };
 
 // Validates `desc` and builds the tables. Returns QSS_OK or a negative qss_status with `err` set.

@@ -1,0 +1,345 @@
+// Kernel variant 1 ("slab-smem") for sm_100a: per-cell QSS chemistry -- rate constants -> QSS closure -> wdot ->
+// analytical Jacobian with the chain rule through the closure (Eq. 2-4, 6, 7, 9).
+//
+// Mapping: one thread block per SM works on a slab of 32 consecutive cells; lane l of EVERY
+// warp is cell l of the slab, the warps split the items of each phase (species, reactions, closure slots, QSS
+// groups, Jacobian columns) and meet at block barriers.  Consequences:
+//   - every table read is warp-uniform (tables come from the kernel-parameter constant bank, `p.h`);
+//   - every per-cell array access is one conflict-free 256-byte row, in shared memory for the hot state
+//     (concentrations, closure factors, W_y, third-body vectors, dy/dx column) and in an L2-resident scratch slab
+//     for the write-once / read-once per-direction arrays (k_d, kappa_d, dlnk/dT);
+//   - one Jacobian column at a time is accumulated in REGISTERS (the temporaries that replace the paper's CSE
+//     scalars): partial derivatives are scattered into it through a uniform indexed branch,
+//     the dy/dx_k solve runs on a per-warp shared-memory vector, and the finished column leaves as 35 coalesced
+//     256-byte streaming stores.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "qss_tables.h"
+#include "qss_v1.h"
+
+namespace {
+
+constexpr double kLn10 = 2.302585092994045684017991454684;
+constexpr double kInvLn10 = 0.434294481903251827651128918916605;
+constexpr double kLnP0R = 9.4080919689433160;  // ln(101325 / 8.31446261815324)
+
+extern __shared__ double qss_smem[];
+
+#define HT(off, i) p.h[(off) + (i)]
+#define HD(off, i) (*reinterpret_cast<const double *>(&p.h[(off) + 2 * (i)]))
+#define SM(row, i) qss_smem[((row) + (i)) * 32 + lane]
+#define SC(row, i) sc[(size_t)((row) + (i)) * 32]
+
+// col[slot] += a * b with a warp-uniform run-time slot.  The column lives in REGISTERS; the run-time index is
+// resolved by one indexed branch (PTX brx.idx -> SASS BRX through a jump table) into a DFMA on the right register:
+// LDC + BRX + DFMA + BRA instead of a shared-memory read-modify-write.  nvcc lowers a C++ switch to a compare tree
+// (no jump tables in the NVPTX back end), hence the inline PTX.  Operands %0..%35 = ct[], %36..%55 = cq[].
+#define QSS_L(i) "L" #i ": fma.rn.f64 %" #i ", %56, %57, %" #i "; bra.uni LEND;\n\t"
+#define QSS_SCATTER(slot, a, b)                                                                                   \
+    asm volatile("{\n\t.reg .u32 ix;\n\tmov.u32 ix, %58;\n\t"                                                     \
+                 "TL: .branchtargets L0, L1, L2, L3, L4, L5, L6, L7, L8, L9, L10, L11, L12, L13, L14, L15, L16, L17, L18, L19, L20, L21, L22, L23, L24, L25, L26, L27, L28, L29, L30, L31, L32, L33, L34, L35, L36, L37, L38, L39, L40, L41, L42, L43, L44, L45, L46, L47, L48, L49, L50, L51, L52, L53, L54, L55;\n\t" \
+                 "brx.idx.uni ix, TL;\n\t"                                                                         \
+        QSS_L(0) QSS_L(1) QSS_L(2) QSS_L(3) QSS_L(4) QSS_L(5) QSS_L(6) QSS_L(7) \
+        QSS_L(8) QSS_L(9) QSS_L(10) QSS_L(11) QSS_L(12) QSS_L(13) QSS_L(14) QSS_L(15) \
+        QSS_L(16) QSS_L(17) QSS_L(18) QSS_L(19) QSS_L(20) QSS_L(21) QSS_L(22) QSS_L(23) \
+        QSS_L(24) QSS_L(25) QSS_L(26) QSS_L(27) QSS_L(28) QSS_L(29) QSS_L(30) QSS_L(31) \
+        QSS_L(32) QSS_L(33) QSS_L(34) QSS_L(35) QSS_L(36) QSS_L(37) QSS_L(38) QSS_L(39) \
+        QSS_L(40) QSS_L(41) QSS_L(42) QSS_L(43) QSS_L(44) QSS_L(45) QSS_L(46) QSS_L(47) \
+        QSS_L(48) QSS_L(49) QSS_L(50) QSS_L(51) QSS_L(52) QSS_L(53) QSS_L(54) QSS_L(55) \
+                 "LEND:\n\t}"                                                                                     \
+                 : "+d"(ct[0]), "+d"(ct[1]), "+d"(ct[2]), "+d"(ct[3]), "+d"(ct[4]), "+d"(ct[5]), "+d"(ct[6]), "+d"(ct[7]), "+d"(ct[8]), "+d"(ct[9]), "+d"(ct[10]), "+d"(ct[11]), "+d"(ct[12]), "+d"(ct[13]), "+d"(ct[14]), "+d"(ct[15]), "+d"(ct[16]), "+d"(ct[17]), "+d"(ct[18]), "+d"(ct[19]), "+d"(ct[20]), "+d"(ct[21]), "+d"(ct[22]), "+d"(ct[23]), "+d"(ct[24]), "+d"(ct[25]), "+d"(ct[26]), "+d"(ct[27]), "+d"(ct[28]), "+d"(ct[29]), "+d"(ct[30]), "+d"(ct[31]), "+d"(ct[32]), "+d"(ct[33]), "+d"(ct[34]), "+d"(ct[35]), \
+                   "+d"(cq[0]), "+d"(cq[1]), "+d"(cq[2]), "+d"(cq[3]), "+d"(cq[4]), "+d"(cq[5]), "+d"(cq[6]), "+d"(cq[7]), "+d"(cq[8]), "+d"(cq[9]), "+d"(cq[10]), "+d"(cq[11]), "+d"(cq[12]), "+d"(cq[13]), "+d"(cq[14]), "+d"(cq[15]), "+d"(cq[16]), "+d"(cq[17]), "+d"(cq[18]), "+d"(cq[19]) \
+                 : "d"((double)(a)), "d"((double)(b)), "r"((int)(slot)))
+static_assert(QSS_V1_NT == 36 && QSS_V1_NQ == 20, "QSS_SCATTER is written out for 36 + 20 register rows");
+
+template <bool JAC>
+__global__ void __launch_bounds__(384, 1) qss_v1_kernel(const __grid_constant__ QssV1 p) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int N = p.N, Nq = p.Nq, M = p.M, nsp = p.nsp;
+    const int64_t ld = p.ld;
+    const int64_t nslab = (p.ncells + 31) / 32;
+    double *sc = p.scratch + (size_t)blockIdx.x * p.scratch_stride + lane;
+    const int32_t *gI = p.gI;
+    const double *gD = p.gD;
+
+    for (int64_t slab = blockIdx.x; slab < nslab; slab += gridDim.x) {
+        const int64_t cell = slab * 32 + lane;
+        const bool active = cell < p.ncells;
+        const int64_t cc = active ? cell : p.ncells - 1;       // idle lanes of a ragged tail shadow the last cell
+        const double T = p.T[cc];
+        const double lnT = log(T), invT = 1.0 / T;
+        const double lnP0RT = kLnP0R - lnT;                    // ln(P0 / (R T))
+        // ---- P0: stage the concentrations
+        for (int s = warp; s < N; s += nw) SM(p.s_V, s) = p.C[(size_t)s * ld + cc];
+        if (warp == 0) { SM(p.s_V, N) = 1.0; SM(p.s_G, nsp) = 0.0; SM(p.s_H, nsp) = 0.0; }
+        __syncthreads();
+        // ---- P1: NASA-7 thermo (readings G4, G9); total concentration
+        for (int s = warp; s < nsp; s += nw) {
+            const double *th = gD + p.d_thermo + s * QSS_TH_STRIDE;
+            const double *a = th + 1 + (T < th[0] ? 0 : 11);
+            const double h = a[0] + T * (a[1] + T * (a[2] + T * (a[3] + T * a[4]))) + a[5] * invT;
+            const double sR = a[0] * lnT + T * (a[6] + T * (a[7] + T * (a[8] + T * a[9]))) + a[10];
+            SM(p.s_H, s) = h;
+            SM(p.s_G, s) = h - sR;
+        }
+        if (warp == nw - 1) {
+            double ct_ = 0.0;
+            for (int k = 0; k < N; ++k) ct_ += SM(p.s_V, k);
+            SM(p.s_CT, 0) = ct_;
+        }
+        __syncthreads();
+        // ---- P2: rate constants, direction coefficients kappa_d (Eq. 2, Eq. 6)
+        {
+            const double Ctot = SM(p.s_CT, 0);
+            for (int r = warp; r < M; r += nw) {
+                const int4 ra = __ldg(reinterpret_cast<const int4 *>(gI + p.i_rrec + r * QSS_V1_RREC));
+                const int4 rb = __ldg(reinterpret_cast<const int4 *>(gI + p.i_rrec + r * QSS_V1_RREC + 4));
+                const int j = ra.x, type = ra.y & 3, mask = (ra.y >> 2) & 3, tb = (ra.y >> 4) - 1;
+                const double *rd = gD + p.d_rate + j * QSS_RD_STRIDE;
+                const double lnkinf = rd[0] + rd[1] * lnT - rd[2] * invT;
+                const double dlnkinf = (rd[1] + rd[2] * invT) * invT;
+                double k = exp(lnkinf), dlnk = dlnkinf;
+                if (type >= 1) {
+                    double Mc = Ctot;                              // M = sum_k alpha_k C_k, transported only (G7)
+                    const int e0 = gI[p.i_eff_ptr + j], e1 = gI[p.i_eff_ptr + j + 1];
+                    for (int e = e0; e < e1; ++e) Mc += gD[p.d_effm1 + e] * SM(p.s_V, gI[p.i_eff_sp + e]);
+                    double dlm;
+                    if (type == 1) {
+                        k *= Mc;
+                        dlm = 1.0 / Mc;
+                    } else {                                       // Troe fall-off
+                        const double lnk0 = rd[3] + rd[4] * lnT - rd[5] * invT;
+                        const double dlnk0 = (rd[4] + rd[5] * invT) * invT;
+                        const double Pr = exp(lnk0 - lnkinf) * Mc;
+                        const double al = rd[6], i3 = rd[7], i1 = rd[8], T2s = rd[9];
+                        const double e3 = exp(-T * i3), e1x = exp(-T * i1), e2 = exp(-T2s * invT);
+                        const double Fc = (1.0 - al) * e3 + al * e1x + e2;
+                        const double L = log(Pr) * kInvLn10, Lc = log(Fc) * kInvLn10;
+                        const double c = -0.4 - 0.67 * Lc, n = 0.75 - 1.27 * Lc;
+                        const double num = L + c, den = n - 0.14 * num;
+                        const double iden = 1.0 / den;
+                        const double f1 = num * iden;
+                        const double ione_f = 1.0 / (1.0 + f1 * f1);
+                        const double F = exp(kLn10 * Lc * ione_f);
+                        const double i1pr = 1.0 / (1.0 + Pr);
+                        k = k * (Pr * i1pr) * F;
+                        const double df1_dL = n * iden * iden;
+                        const double dlF_dL = -2.0 * Lc * f1 * df1_dL * ione_f * ione_f;
+                        dlm = (i1pr + dlF_dL) / Mc;
+                        if (JAC) {
+                            const double dFc = -(1.0 - al) * i3 * e3 - al * i1 * e1x + T2s * invT * invT * e2;
+                            const double df1_dLc = (-0.67 * den - num * (-1.27 + 0.14 * 0.67)) * iden * iden;
+                            const double dlF_dLc = ione_f - 2.0 * Lc * f1 * df1_dLc * ione_f * ione_f;
+                            const double delta = dlnk0 - dlnkinf;
+                            dlnk = dlnkinf + delta * i1pr + dlF_dL * delta + dlF_dLc * dFc / Fc;
+                        }
+                    }
+                    if (JAC) SM(p.s_QM, tb) = dlm;
+                }
+                double kf = (mask & 1) ? k : 0.0, kb = 0.0, dlnKc = 0.0;
+                if (mask & 2) {                                    // reverse rate from the equilibrium constant (G10)
+                    const double dG = (SM(p.s_G, rb.y & 255) + SM(p.s_G, (rb.y >> 8) & 255) + SM(p.s_G, (rb.y >> 16) & 255)) -
+                                      (SM(p.s_G, rb.x & 255) + SM(p.s_G, (rb.x >> 8) & 255) + SM(p.s_G, (rb.x >> 16) & 255));
+                    kb = k * exp(dG - rd[10] * lnP0RT);            // k / Kc, ln Kc = -dG + dnu ln(P0/RT)
+                    if (JAC) {
+                        const double dH = (SM(p.s_H, rb.y & 255) + SM(p.s_H, (rb.y >> 8) & 255) + SM(p.s_H, (rb.y >> 16) & 255)) -
+                                          (SM(p.s_H, rb.x & 255) + SM(p.s_H, (rb.x >> 8) & 255) + SM(p.s_H, (rb.x >> 16) & 255));
+                        dlnKc = (dH - rd[10]) * invT;
+                    }
+                }
+                SC(p.g_K, 2 * j) = kf;
+                SC(p.g_K, 2 * j + 1) = kb;
+                // kappa_d = k_d * product of the TRANSPORTED reactant molecules (QSS and empty slots read the 1.0 row)
+                SC(p.g_KAP, 2 * j) = kf * SM(p.s_V, ra.z & 255) * SM(p.s_V, (ra.z >> 8) & 255) * SM(p.s_V, (ra.z >> 16) & 255);
+                SC(p.g_KAP, 2 * j + 1) = kb * SM(p.s_V, ra.w & 255) * SM(p.s_V, (ra.w >> 8) & 255) * SM(p.s_V, (ra.w >> 16) & 255);
+                if (JAC) { SC(p.g_DF, j) = dlnk; SC(p.g_DC, j) = dlnKc; }
+            }
+        }
+        __syncthreads();
+        // ---- P3: closure assembly: every P / leak / p0 slot gathers the kappas feeding it (no atomics)
+        for (int e = warp; e < p.n_centry; e += nw) {
+            double acc = 0.0;
+            for (int x = HT(p.h_ce_ptr, e); x < HT(p.h_ce_ptr, e + 1); ++x) acc += SC(p.g_KAP, HT(p.h_ce_dir, x));
+            SM(p.s_CL, HT(p.h_ce_dst, e)) = acc;
+        }
+        for (int e = warp; e < p.n_xp; e += nw) {
+            double acc = 0.0;
+            for (int x = HT(p.h_xp_ptr, e); x < HT(p.h_xp_ptr, e + 1); ++x) acc += SC(p.g_KAP, HT(p.h_xp_dir, x));
+            SM(p.s_XP, e) = acc;
+        }
+        __syncthreads();
+        // ---- P4: closure solve, level by level of the condensed DAG; subtraction-free elimination
+        //          (Eq. 6; readings G2, G8)
+        for (int l = 0; l < p.n_levels; ++l) {
+            for (int g = HT(p.h_level_ptr, l) + warp; g < HT(p.h_level_ptr, l + 1); g += nw) {
+                const int gi = p.h_group + g * QSS_GI_STRIDE;
+                const int sz = HT(gi, 0), moff = HT(gi, 1), base = p.s_CL + HT(gi, 2), x0 = HT(gi, 4), x1 = HT(gi, 5);
+                const int oL = base + sz * sz, oP0 = oL + sz, oID = oP0 + sz;
+                for (int x = x0; x < x1; ++x) SM(oP0, HT(p.h_xp_m, x)) += SM(p.s_XP, x) * SM(p.s_V, N + 1 + HT(p.h_xp_n, x));
+                for (int k = sz - 1; k >= 1; --k) {
+                    const double lk = SM(oL, k);
+                    double Dk = lk;
+                    for (int m = 0; m < k; ++m) Dk += SM(base, m * sz + k);
+                    const double iD = 1.0 / Dk;
+                    SM(oID, k) = iD;
+                    for (int jj = 0; jj < k; ++jj) {
+                        const double f = SM(base, k * sz + jj) * iD;
+                        SM(oL, jj) += f * lk;
+                        for (int m = 0; m < k; ++m)
+                            if (m != jj) SM(base, m * sz + jj) += SM(base, m * sz + k) * f;
+                    }
+                }
+                SM(oID, 0) = 1.0 / SM(oL, 0);
+                for (int k = sz - 1; k >= 1; --k) {
+                    const double tk = SM(oP0, k) * SM(oID, k);
+                    for (int m = 0; m < k; ++m) SM(oP0, m) += SM(base, m * sz + k) * tk;
+                }
+                for (int k = 0; k < sz; ++k) {
+                    double acc = SM(oP0, k);
+                    for (int jj = 0; jj < k; ++jj) acc += SM(base, k * sz + jj) * SM(oP0, jj);
+                    acc *= SM(oID, k);
+                    SM(oP0, k) = acc;
+                    SM(p.s_V, N + 1 + HT(p.h_gmember, moff + k)) = acc;
+                }
+            }
+            __syncthreads();
+        }
+        // ---- P5: net rates of progress Q_j (Eq. 2), dQ/dT at fixed y and M, dQ/dM
+        for (int j = warp; j < M; j += nw) {
+            const int w = HT(p.h_q, j);
+            const double rf = SC(p.g_KAP, 2 * j) * SM(p.s_V, w & 255);
+            const double rb = SC(p.g_KAP, 2 * j + 1) * SM(p.s_V, (w >> 8) & 255);
+            const double Q = rf - rb;
+            SM(p.s_Q, j) = Q;
+            if (JAC) {
+                const double qt = Q * SC(p.g_DF, j) + rb * SC(p.g_DC, j);
+                if (p.s_QT >= 0) SM(p.s_QT, j) = qt; else SC(p.g_DC, j) = qt;
+                const int tb = (w >> 16) - 1;
+                if (tb >= 0) SM(p.s_QM, tb) *= Q;
+            }
+        }
+        __syncthreads();
+        // ---- P6: species sums: wdot (Eq. 3); for the Jacobian the T-column vector and the third-body vector
+        for (int u = HT(p.h_ssw_ptr, warp); u < HT(p.h_ssw_ptr, warp + 1); ++u) {
+            const int s = HT(p.h_ssw, u);
+            double w = 0.0, et = 0.0, tv = 0.0;
+            for (int x = HT(p.h_ss_ptr, s); x < HT(p.h_ss_ptr, s + 1); ++x) {
+                const int e = HT(p.h_ss, x), j = e & 4095;
+                const double nu = HD(p.h_nulut, (e >> 12) & 15);
+                w = fma(nu, SM(p.s_Q, j), w);
+                if (JAC) {
+                    et = fma(nu, p.s_QT >= 0 ? SM(p.s_QT, j) : SC(p.g_DC, j), et);
+                    const int tb = (e >> 16) - 1;
+                    if (tb >= 0) tv = fma(nu, SM(p.s_QM, tb), tv);
+                }
+            }
+            if (s < N && p.wdot && active) p.wdot[(size_t)s * ld + cell] = w;
+            if (JAC) { SM(p.s_TV, s) = tv; SC(p.g_ET, s) = et; }
+        }
+        if (p.cqss && active)
+            for (int q = warp; q < Nq; q += nw) p.cqss[(size_t)q * ld + cell] = SM(p.s_V, N + 1 + q);
+        if (JAC) {
+            __syncthreads();
+            // ---- P7: W_y[i][q] = d wdot_i / d y_q at fixed x: sums of kappas (Eq. 9 second parenthesis, L224)
+            for (int e = warp; e < p.n_wy; e += nw) {
+                double acc = 0.0;
+                for (int x = HT(p.h_wya_ptr, e); x < HT(p.h_wya_ptr, e + 1); ++x) {
+                    const int w = HT(p.h_wya, x);
+                    acc = fma(HD(p.h_nulut, (w >> 12) & 15), SC(p.g_KAP, w & 4095), acc);
+                }
+                SM(p.s_WY, e) = acc;
+            }
+            __syncthreads();
+            // ---- P8: column sweep: column k of [W_x; G_x] in registers -> dy/dx_k -> J[:,k] = W_x[:,k] + W_y dy/dx_k
+            const int yrow = p.s_YC + warp * Nq;
+            for (int u = HT(p.h_cw_ptr, warp); u < HT(p.h_cw_ptr, warp + 1); ++u) {
+                const int k = HT(p.h_cw, u);
+                double ct[QSS_V1_NT], cq[QSS_V1_NQ];
+                if (k < N) {
+#pragma unroll
+                    for (int s = 0; s < QSS_V1_NT; ++s) ct[s] = s < N ? SM(p.s_TV, s) : 0.0;      // rank-1 third-body term
+#pragma unroll
+                    for (int q = 0; q < QSS_V1_NQ; ++q) cq[q] = q < Nq ? SM(p.s_TV, N + q) : 0.0;
+                    for (int x = HT(p.h_col_ptr, k); x < HT(p.h_col_ptr, k + 1); ++x) {
+                        const int w = HT(p.h_inc, x), d = w & 4095, j = d >> 1;
+                        // d r_d / d C_k for one molecule slot: k_d times the other two slots (Eq. 9 first parenthesis)
+                        double part = SC(p.g_K, d) * SM(p.s_V, (w >> 12) & 255) * SM(p.s_V, (w >> 20) & 255);
+                        if (d & 1) part = -part;
+                        for (int y = HT(p.h_net_ptr, j); y < HT(p.h_net_ptr, j + 1); ++y) {
+                            const int e = HT(p.h_net, y);
+                            QSS_SCATTER(e & 255, HD(p.h_nulut, (e >> 8) & 15), part);
+                        }
+                    }
+                    for (int x = HT(p.h_effc_ptr, k); x < HT(p.h_effc_ptr, k + 1); ++x) {         // (alpha_k - 1) dQ/dM
+                        const int w = HT(p.h_effc, x), j = w & 4095;
+                        const double v = HD(p.h_effc_val, x) * SM(p.s_QM, w >> 12);
+                        for (int y = HT(p.h_net_ptr, j); y < HT(p.h_net_ptr, j + 1); ++y) {
+                            const int e = HT(p.h_net, y);
+                            QSS_SCATTER(e & 255, HD(p.h_nulut, (e >> 8) & 15), v);
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int s = 0; s < QSS_V1_NT; ++s) ct[s] = s < N ? SC(p.g_ET, s) : 0.0;
+#pragma unroll
+                    for (int q = 0; q < QSS_V1_NQ; ++q) cq[q] = q < Nq ? SC(p.g_ET, N + q) : 0.0;
+                }
+                // dy/dx_k: (diag D - P) ycol = G_x[:,k], group by group with the closure's elimination factors
+#pragma unroll
+                for (int q = 0; q < QSS_V1_NQ; ++q) if (q < Nq) SM(yrow, q) = cq[q];   // (a thread only ever touches its own lane's slot)
+                for (int g = 0; g < p.n_groups; ++g) {
+                    const int gi = p.h_group + g * QSS_GI_STRIDE;
+                    const int sz = HT(gi, 0), mo = p.h_gmember + HT(gi, 1), base = p.s_CL + HT(gi, 2);
+                    const int oID = base + sz * sz + 2 * sz;
+                    for (int x = HT(gi, 4); x < HT(gi, 5); ++x)
+                        SM(yrow, HT(mo, HT(p.h_xp_m, x))) += SM(p.s_XP, x) * SM(yrow, HT(p.h_xp_n, x));
+                    for (int kk = sz - 1; kk >= 1; --kk) {
+                        const double tk = SM(yrow, HT(mo, kk)) * SM(oID, kk);
+                        for (int m = 0; m < kk; ++m) SM(yrow, HT(mo, m)) += SM(base, m * sz + kk) * tk;
+                    }
+                    for (int kk = 0; kk < sz; ++kk) {
+                        double acc = SM(yrow, HT(mo, kk));
+                        for (int jj = 0; jj < kk; ++jj) acc += SM(base, kk * sz + jj) * SM(yrow, HT(mo, jj));
+                        SM(yrow, HT(mo, kk)) = acc * SM(oID, kk);
+                    }
+                }
+                // J[:,k] = W_x[:,k] + W_y dy/dx_k, one coalesced 256-byte streaming store per entry
+#pragma unroll
+                for (int i = 0; i < QSS_V1_NT; ++i) {
+                    if (i < N) {
+                        double acc = ct[i];
+                        for (int x = HT(p.h_wyrow_ptr, i); x < HT(p.h_wyrow_ptr, i + 1); ++x)
+                            acc = fma(SM(p.s_WY, x), SM(yrow, HT(p.h_wyq, x)), acc);
+                        if (active) __stcs(&p.jac[((size_t)i * (N + 1) + k) * ld + cell], acc);
+                    }
+                }
+            }
+        }
+        __syncthreads();      // shared memory and the scratch slab are reused by the next cell slab
+    }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------------
+// launcher (called by qss_api.cu)
+// ---------------------------------------------------------------------------------------------------
+size_t qss_v1_smem_bytes(const QssV1 &v) { return (size_t)v.smem_rows * 256; }
+size_t qss_v1_scratch_doubles(const QssV1 &v) { return (size_t)v.scratch_rows * 32; }
+
+cudaError_t qss_v1_prepare() {
+    cudaError_t e = cudaFuncSetAttribute(qss_v1_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(qss_v1_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+}
+
+cudaError_t qss_launch_v1(const QssV1 &v, bool jac, int nblocks, cudaStream_t stream) {
+    const int64_t nslab = (v.ncells + 31) / 32;
+    if (nslab == 0) return cudaSuccess;
+    const int grid = (int)(nslab < nblocks ? nslab : nblocks);
+    const size_t smem = qss_v1_smem_bytes(v);
+    if (jac) qss_v1_kernel<true><<<grid, v.nw * 32, smem, stream>>>(v);
+    else qss_v1_kernel<false><<<grid, v.nw * 32, smem, stream>>>(v);
+    return cudaGetLastError();
+}
