@@ -10,6 +10,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <functional>
 #include <cstring>
 #include <map>
@@ -154,8 +155,9 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
             H.push_back(qf | (qb << 8) | ((R[j].tb + 1) << 16));
         }
     }
-    const int nw_max = 12;
-    // species incidence lists and their balanced assignment to warps (filled once nw is known)
+    const int nw = QSS_V1_NW;
+    if (N + 1 > QSS_V1_NT) { why = "more Jacobian columns than the register tile of variant 1 holds"; return false; }
+    // species incidence lists (their balanced assignment to warps follows below)
     std::vector<std::vector<int32_t>> ss(nsp);
     for (int j = 0; j < M; ++j) if (R[j].mask) for (const Term &x : R[j].net) ss[x.sp].push_back(j | (nucode(x.nu) << 12) | ((R[j].tb + 1) << 16));
     {
@@ -164,125 +166,155 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         v.h_ss_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
         v.h_ss = at(); H.insert(H.end(), all.begin(), all.end());
     }
-    // W_y entries, row-major (i, then q): gather lists over the directions consuming q
+    // W_y entries, row-major (i, then q): gather lists over the directions consuming q (lists go to the global blob)
     std::map<std::pair<int, int>, std::vector<int32_t>> wy;
     for (int j = 0; j < M; ++j) for (int dir = 0; dir < 2; ++dir) {
         if (!((R[j].mask >> dir) & 1) || R[j].q[dir] < 0) continue;
         for (const Term &x : R[j].net) if (x.sp < N) wy[{x.sp, R[j].q[dir]}].push_back((2 * j + dir) | (nucode(dir == 0 ? x.nu : -x.nu) << 12));
     }
+    std::vector<int32_t> wya_ptr{0}, wya_all;
     {
-        std::vector<int32_t> ptr{0}, all, rptr{0}, rq;
+        std::vector<int32_t> rptr{0}, roff;
         int row = 0;
         for (auto &kv : wy) {
-            while (row < kv.first.first) { rptr.push_back((int32_t)rq.size()); ++row; }
-            rq.push_back(kv.first.second);
-            all.insert(all.end(), kv.second.begin(), kv.second.end()); ptr.push_back((int32_t)all.size());
+            while (row < kv.first.first) { rptr.push_back((int32_t)roff.size()); ++row; }
+            roff.push_back(kv.first.second * nw * 256);          // byte offset of dy_q/dx rows inside the s_YC region
+            wya_all.insert(wya_all.end(), kv.second.begin(), kv.second.end()); wya_ptr.push_back((int32_t)wya_all.size());
         }
-        while (row < N) { rptr.push_back((int32_t)rq.size()); ++row; }
-        v.n_wy = (int32_t)rq.size();
-        v.h_wya_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
-        v.h_wya = at(); H.insert(H.end(), all.begin(), all.end());
-        v.h_wyrow_ptr = at(); H.insert(H.end(), rptr.begin(), rptr.end());
-        v.h_wyq = at(); H.insert(H.end(), rq.begin(), rq.end());
+        while (row < N) { rptr.push_back((int32_t)roff.size()); ++row; }
+        v.n_wy = (int32_t)roff.size();
+        v.h_wr_ptr = at(); H.insert(H.end(), rptr.begin(), rptr.end());
+        v.h_wr = at(); H.insert(H.end(), roff.begin(), roff.end());
     }
-    // column incidences: one per (enabled direction, molecule slot holding a transported species)
-    std::vector<std::vector<int32_t>> inc(N);
+    // ---- shared-memory layout (rows of 256 bytes) and scratch layout
+    int rows_fixed = 0;
+    auto take = [&](int n) { int r = rows_fixed; rows_fixed += n; return r; };
+    v.s_V = take(N + 1 + Nq); v.s_CT = take(1); v.s_CL = take(c.cl_size); v.s_XP = take(v.n_xp); v.s_TV = take(nsp);
+    const int max_rows = (227 * 1024) / 256;
+    const int region = std::max(std::max((Nq + N) * nw, 2 * (nsp + 1)), 2 * M);
+    if (rows_fixed + region > max_rows) { why = "per-cell state does not fit the shared memory of one SM"; return false; }
+    if ((v.s_XP + v.n_xp) * 256 > 65535 || Nq * nw * 256 > 65535) { why = "closure storage beyond the 16-bit offsets of variant 1"; return false; }
+    v.nw = nw;
+    v.s_YC = rows_fixed; v.s_WX = rows_fixed + Nq * nw;
+    v.s_G = rows_fixed; v.s_H = rows_fixed + nsp + 1;
+    v.s_Q = rows_fixed; v.s_QT = rows_fixed + M;
+    v.smem_rows = rows_fixed + region;
     {
-        for (int j = 0; j < M; ++j) for (int dir = 0; dir < 2; ++dir) {
-            if (!((R[j].mask >> dir) & 1)) continue;
-            std::vector<int> slots;                          // species of each molecule of the reactant side
-            for (const Term &x : R[j].side[dir]) for (int u = 0; u < x.nu; ++u) slots.push_back(x.sp);
-            for (size_t p = 0; p < slots.size(); ++p) {
-                if (slots[p] >= N) continue;
-                int o[2] = {N, N}, no = 0;
-                for (size_t q = 0; q < slots.size(); ++q) if (q != p) o[no++] = vrow(slots[q]);
-                inc[slots[p]].push_back((2 * j + dir) | (o[0] << 12) | (o[1] << 20));
+        int o = 0;
+        auto tk = [&](int n) { int r = o; o += n; return r; };
+        v.g_K = tk(2 * M); v.g_KAP = tk(2 * M); v.g_DF = tk(M); v.g_DC = tk(M); v.g_ET = tk(nsp); v.g_QM = tk(c.n_tb); v.g_WY = tk(v.n_wy);
+        v.scratch_rows = o;
+        if (o > 65535) { why = "scratch rows beyond the 16-bit offsets of variant 1"; return false; }
+    }
+    // ---- column stream: everything that is scattered into column k of [W_x; G_x], as records
+    //   w0 = scratch row of A | n_entries << 16 | has_val << 20      part = A * V[o1] * V[o2] (* val)
+    //   w1 = byte offset of V row o1 | byte offset of V row o2 << 16
+    //   w2, w3 = up to 8 scatter indices (bytes): 2 * register row + (1 if the term is subtracted); QSS_V1_NULL = none
+    //   [w4, w5 = val (double)]                                       only when has_val
+    // One record per (enabled direction, molecule slot holding species k): A = k_d, o1/o2 = the other two slots
+    // (Eq. 9 first parenthesis); one per non-unity third-body efficiency: A = dQ_j/dM, val = alpha_jk - 1.
+    auto regrow = [&](int sp) { return sp < N ? sp : QSS_V1_NT + (sp - N); };
+    auto voff = [&](int vr) { return (v.s_V + vr) * 256; };
+    std::vector<std::vector<int32_t>> cs(N);
+    bool cs_ok = true;
+    auto push_record = [&](int k, int rowA, int o1, int o2, const std::vector<Term> &net, int sgn, bool has_val, double val) {
+        std::vector<int> idx;
+        for (const Term &x : net) { const int e = sgn * x.nu; for (int u = 0; u < std::abs(e); ++u) idx.push_back(2 * regrow(x.sp) + (e < 0 ? 1 : 0)); }
+        if (idx.size() > 8) { cs_ok = false; return; }
+        const uint32_t none = QSS_V1_NULL * 0x01010101u;
+        uint32_t w[2] = {none, none};
+        for (size_t u = 0; u < idx.size(); ++u) { w[u / 4] &= ~(0xFFu << (8 * (u % 4))); w[u / 4] |= (uint32_t)idx[u] << (8 * (u % 4)); }
+        cs[k].push_back(rowA | ((int)idx.size() << 16) | ((has_val ? 1 : 0) << 20));
+        cs[k].push_back(o1 | (o2 << 16));
+        cs[k].push_back((int32_t)w[0]); cs[k].push_back((int32_t)w[1]);
+        if (has_val) { int32_t d2[2]; std::memcpy(d2, &val, 8); cs[k].push_back(d2[0]); cs[k].push_back(d2[1]); }
+    };
+    for (int j = 0; j < M; ++j) for (int dir = 0; dir < 2; ++dir) {
+        if (!((R[j].mask >> dir) & 1)) continue;
+        std::vector<int> slots;                              // species of each molecule of the reactant side
+        for (const Term &x : R[j].side[dir]) for (int u = 0; u < x.nu; ++u) slots.push_back(x.sp);
+        for (size_t pp = 0; pp < slots.size(); ++pp) {
+            if (slots[pp] >= N) continue;
+            int o[2] = {N, N}, no = 0;
+            for (size_t q = 0; q < slots.size(); ++q) if (q != pp) o[no++] = vrow(slots[q]);
+            push_record(slots[pp], v.g_K + 2 * j + dir, voff(o[0]), voff(o[1]), R[j].net, dir == 0 ? 1 : -1, false, 0.0);
+        }
+    }
+    for (int k = 0; k < N; ++k)
+        for (auto &e : (*c.effc)[k]) if (R[e.first].mask) push_record(k, v.g_QM + R[e.first].tb, voff(N), voff(N), R[e.first].net, 1, true, e.second);
+    if (!cs_ok) { why = "a reaction changes more than 8 molecules (scatter record of variant 1)"; return false; }
+    if (voff(N + Nq) > 65535) { why = "V rows beyond the 16-bit offsets of variant 1"; return false; }
+    {
+        if (H.size() & 1) H.push_back(0);
+        std::vector<int32_t> ptr{0}, all;
+        for (int k = 0; k < N; ++k) { all.insert(all.end(), cs[k].begin(), cs[k].end()); ptr.push_back((int32_t)all.size()); }
+        ptr.push_back((int32_t)all.size());                  // the T column has an empty stream
+        v.h_cs = at(); H.insert(H.end(), all.begin(), all.end());
+        v.h_cs_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
+    }
+    // ---- dy/dx solve program: row operations y[a] = (y[a] + sum_t F_t * y[b_t]) [* ID] on the warp's dy/dx column,
+    //      in the order cross-group terms, back-elimination (with U[m][k] = P[m][k] / D_k), forward substitution
+    //   header = a_off | n_terms << 16 | has_scale << 24 ; [id_off] ; n_terms x (f_off | b_off << 16)
+    {
+        std::vector<int32_t> sp;
+        int nops = 0;
+        auto yoff = [&](int q) { return q * nw * 256; };
+        for (int g = 0; g < c.n_groups; ++g) {
+            const std::vector<int> &mem = (*c.members)[g];
+            const int sz = (int)mem.size(), base = v.s_CL + (*c.gbase)[g];
+            for (int x = (*c.xp_begin)[g]; x < (*c.xp_end)[g]; ++x) {
+                const auto &e = (*c.xpl)[x];
+                sp.push_back(yoff(e.first.first) | (1 << 16)); sp.push_back(((v.s_XP + x) * 256) | (yoff(e.first.second) << 16)); ++nops;
+            }
+            for (int m = sz - 2; m >= 0; --m) {
+                sp.push_back(yoff(mem[m]) | ((sz - 1 - m) << 16)); ++nops;
+                for (int k = m + 1; k < sz; ++k) sp.push_back(((base + m * sz + k) * 256) | (yoff(mem[k]) << 16));
+            }
+            for (int k = 0; k < sz; ++k) {
+                sp.push_back(yoff(mem[k]) | (k << 16) | (1 << 24)); ++nops;
+                sp.push_back((base + sz * sz + 2 * sz + k) * 256);
+                for (int jj = 0; jj < k; ++jj) sp.push_back(((base + k * sz + jj) * 256) | (yoff(mem[jj]) << 16));
             }
         }
-        std::vector<int32_t> ptr{0}, all;
-        for (int k = 0; k < N; ++k) { all.insert(all.end(), inc[k].begin(), inc[k].end()); ptr.push_back((int32_t)all.size()); }
-        v.h_col_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
-        v.h_inc = at(); H.insert(H.end(), all.begin(), all.end());
+        v.n_sp_ops = nops;
+        v.h_sp = at(); H.insert(H.end(), sp.begin(), sp.end());
     }
-    {   // net stoichiometry by reaction; register slot: transported s -> s, QSS q -> QSS_V1_NT + q
+    // ---- species sums: balanced (longest-processing-time) assignment to warps
+    {
+        std::vector<int> idx(nsp);
+        for (int s = 0; s < nsp; ++s) idx[s] = s;
+        std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return ss[a].size() > ss[b].size(); });
+        std::vector<std::vector<int32_t>> bin(nw);
+        std::vector<double> load(nw, 0.0);
+        for (int i : idx) { int b = (int)(std::min_element(load.begin(), load.end()) - load.begin()); bin[b].push_back(i); load[b] += 6.0 + ss[i].size(); }
         std::vector<int32_t> ptr{0}, all;
-        for (int j = 0; j < M; ++j) {
-            for (const Term &x : R[j].net) all.push_back((x.sp < N ? x.sp : QSS_V1_NT + (x.sp - N)) | (nucode(x.nu) << 8));
-            ptr.push_back((int32_t)all.size());
-        }
-        v.h_net_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
-        v.h_net = at(); H.insert(H.end(), all.begin(), all.end());
+        for (int w = 0; w < nw; ++w) { all.insert(all.end(), bin[w].begin(), bin[w].end()); ptr.push_back((int32_t)all.size()); }
+        v.h_ssw_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
+        v.h_ssw = at(); H.insert(H.end(), all.begin(), all.end());
     }
-    {   // (alpha_k - 1) dQ/dM corrections by column
-        std::vector<int32_t> ptr{0}, all; std::vector<double> val;
-        for (int k = 0; k < N; ++k) {
-            for (auto &e : (*c.effc)[k]) if (R[e.first].mask) { all.push_back(e.first | (R[e.first].tb << 12)); val.push_back(e.second); }
-            ptr.push_back((int32_t)all.size());
-        }
-        v.h_effc_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
-        v.h_effc = at(); H.insert(H.end(), all.begin(), all.end());
-        if (H.size() & 1) H.push_back(0);
-        v.h_effc_val = at();
-        for (double x : val) { int32_t w[2]; std::memcpy(w, &x, 8); H.push_back(w[0]); H.push_back(w[1]); }
+    // ---- Jacobian columns: rounds of nw columns of similar cost (the warps meet at a barrier after every round)
+    {
+        std::vector<int> idx(N + 1);
+        for (int k = 0; k <= N; ++k) idx[k] = k;
+        std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return (a < N ? cs[a].size() : 0) > (b < N ? cs[b].size() : 0); });
+        v.n_rounds = (N + 1 + nw - 1) / nw;
+        v.h_cw = at();
+        for (int i = 0; i < v.n_rounds * nw; ++i) H.push_back(i <= N ? idx[i] : -1);
     }
     {
         if (H.size() & 1) H.push_back(0);
         v.h_nulut = at();
         for (int cde = 0; cde < 16; ++cde) { double x = (double)(cde - 8); int32_t w[2]; std::memcpy(w, &x, 8); H.push_back(w[0]); H.push_back(w[1]); }
     }
-    // ---- shared-memory layout and the number of warps
-    const int n_wy = v.n_wy;
-    int rows_fixed = 0;
-    auto take = [&](int n) { int r = rows_fixed; rows_fixed += n; return r; };
-    v.s_V = take(N + 1 + Nq); v.s_CT = take(1); v.s_CL = take(c.cl_size); v.s_XP = take(v.n_xp); v.s_TV = take(nsp); v.s_QM = take(c.n_tb);
-    const int max_rows = (227 * 1024) / 256;
-    int nw = 0;
-    for (int cand = nw_max; cand >= 4; --cand) {
-        const int region = std::max(std::max(n_wy + cand * Nq, 2 * (nsp + 1)), M);
-        if (rows_fixed + region <= max_rows) { nw = cand; break; }
-    }
-    if (nw == 0) { why = "per-cell state does not fit the shared memory of one SM"; return false; }
-    const int region = std::max(std::max(n_wy + nw * Nq, 2 * (nsp + 1)), M);
-    v.nw = nw;
-    v.s_WY = rows_fixed; v.s_YC = rows_fixed + n_wy;
-    v.s_G = rows_fixed; v.s_H = rows_fixed + nsp + 1;
-    v.s_Q = rows_fixed; v.s_QT = region >= 2 * M ? rows_fixed + M : -1;
-    v.smem_rows = rows_fixed + region;
-    {
-        int o = 0;
-        auto tk = [&](int n) { int r = o; o += n; return r; };
-        v.g_K = tk(2 * M); v.g_KAP = tk(2 * M); v.g_DF = tk(M); v.g_DC = tk(M); v.g_ET = tk(nsp);
-        v.scratch_rows = o;
-    }
-    // ---- balanced (longest-processing-time) assignment of species sums and Jacobian columns to warps
-    auto lpt = [&](const std::vector<double> &cost, int32_t &h_ptr, int32_t &h_list) {
-        std::vector<int> idx(cost.size());
-        for (size_t i = 0; i < idx.size(); ++i) idx[i] = (int)i;
-        std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return cost[a] > cost[b]; });
-        std::vector<std::vector<int32_t>> bin(nw);
-        std::vector<double> load(nw, 0.0);
-        for (int i : idx) { int b = (int)(std::min_element(load.begin(), load.end()) - load.begin()); bin[b].push_back(i); load[b] += cost[i]; }
-        std::vector<int32_t> ptr{0}, all;
-        for (int w = 0; w < nw; ++w) { all.insert(all.end(), bin[w].begin(), bin[w].end()); ptr.push_back((int32_t)all.size()); }
-        h_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
-        h_list = at(); H.insert(H.end(), all.begin(), all.end());
-    };
-    {
-        std::vector<double> cost(nsp);
-        for (int s = 0; s < nsp; ++s) cost[s] = 6.0 + (double)ss[s].size();
-        lpt(cost, v.h_ssw_ptr, v.h_ssw);
-        std::vector<double> ccost(N + 1);
-        for (int k = 0; k < N; ++k) {
-            double sc = 0; for (int32_t w : inc[k]) sc += 10.0 + 7.0 * R[(w & 4095) >> 1].net.size();
-            for (auto &e : (*c.effc)[k]) sc += 6.0 + 7.0 * R[e.first].net.size();
-            ccost[k] = 600.0 + 5.0 * n_wy + sc;
-        }
-        ccost[N] = 600.0 + 5.0 * n_wy;
-        lpt(ccost, v.h_cw_ptr, v.h_cw);
-    }
     if ((int)H.size() > QSS_V1_HMAX) { why = "hot tables exceed the kernel-parameter budget of variant 1"; return false; }
     v.h_used = (int32_t)H.size();
     std::memcpy(v.h, H.data(), H.size() * sizeof(int32_t));
+    // ---- W_y assembly lists (appended to the int blob)
+    {
+        std::vector<int32_t> &I = out.I;
+        v.i_wya_ptr = (int32_t)I.size(); I.insert(I.end(), wya_ptr.begin(), wya_ptr.end());
+        v.i_wya = (int32_t)I.size(); I.insert(I.end(), wya_all.begin(), wya_all.end());
+    }
     // ---- reaction records (appended to the int blob), in processing order
     {
         std::vector<int32_t> &I = out.I;
@@ -681,6 +713,10 @@ int qss_compile(const qss_mech_desc_t *d, QssCompiled &out, std::string &err) {
         V1Ctx vc{N, Nq, M, nsp, n_tb, n_groups, n_levels, cl_size, &R, &members, &gbase, &xp_begin, &xp_end, &lvl_of_group,
                  &pos_in_grp, &rorder, &ce, &xpl, &effc};
         out.v1_ok = build_v1(vc, out, out.v1_why);
+        if (std::getenv("QSS_DEBUG"))
+            std::fprintf(stderr, "[qss] variant 1: %s%s (hot table %d/%d words, smem rows %d, scratch rows %d, rounds %d, solve ops %d)\n",
+                         out.v1_ok ? "ok" : "not applicable: ", out.v1_ok ? "" : out.v1_why.c_str(), out.v1.h_used, QSS_V1_HMAX,
+                         out.v1.smem_rows, out.v1.scratch_rows, out.v1.n_rounds, out.v1.n_sp_ops);
     }
     err.clear();
     return QSS_OK;

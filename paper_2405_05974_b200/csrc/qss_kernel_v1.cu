@@ -8,15 +8,18 @@
 //   - every per-cell array access is one conflict-free 256-byte row, in shared memory for the hot state
 //     (concentrations, closure factors, W_y, third-body vectors, dy/dx column) and in an L2-resident scratch slab
 //     for the write-once / read-once per-direction arrays (k_d, kappa_d, dlnk/dT);
-//   - one Jacobian column at a time is accumulated in REGISTERS (the temporaries that replace the paper's CSE
-//     scalars): partial derivatives are scattered into it through a uniform indexed branch,
-//     the dy/dx_k solve runs on a per-warp shared-memory vector, and the finished column leaves as 35 coalesced
-//     256-byte streaming stores.
+//   - the Jacobian is swept in rounds of 12 columns.  Pass A: each warp accumulates ONE column of [W_x; G_x] in
+//     REGISTERS (the temporaries that replace the paper's CSE scalars): partial derivatives are
+//     scattered into it through an indexed branch (qss_v1_scatter.h), then the dy/dx_k solve runs on the warp's
+//     shared-memory vector.  Pass B: the warps switch to ROWS and add W_y * dy/dx for all 12 columns of the round
+//     from a register tile (one W_y load and one table word per 12 FMAs); every entry leaves as one coalesced
+//     256-byte streaming store.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 #include "qss_tables.h"
 #include "qss_v1.h"
+#include "qss_v1_scatter.h"
 
 namespace {
 
@@ -31,30 +34,10 @@ extern __shared__ double qss_smem[];
 #define SM(row, i) qss_smem[((row) + (i)) * 32 + lane]
 #define SC(row, i) sc[(size_t)((row) + (i)) * 32]
 
-// col[slot] += a * b with a warp-uniform run-time slot.  The column lives in REGISTERS; the run-time index is
-// resolved by one indexed branch (PTX brx.idx -> SASS BRX through a jump table) into a DFMA on the right register:
-// LDC + BRX + DFMA + BRA instead of a shared-memory read-modify-write.  nvcc lowers a C++ switch to a compare tree
-// (no jump tables in the NVPTX back end), hence the inline PTX.  Operands %0..%35 = ct[], %36..%55 = cq[].
-#define QSS_L(i) "L" #i ": fma.rn.f64 %" #i ", %56, %57, %" #i "; bra.uni LEND;\n\t"
-#define QSS_SCATTER(slot, a, b)                                                                                   \
-    asm volatile("{\n\t.reg .u32 ix;\n\tmov.u32 ix, %58;\n\t"                                                     \
-                 "TL: .branchtargets L0, L1, L2, L3, L4, L5, L6, L7, L8, L9, L10, L11, L12, L13, L14, L15, L16, L17, L18, L19, L20, L21, L22, L23, L24, L25, L26, L27, L28, L29, L30, L31, L32, L33, L34, L35, L36, L37, L38, L39, L40, L41, L42, L43, L44, L45, L46, L47, L48, L49, L50, L51, L52, L53, L54, L55;\n\t" \
-                 "brx.idx.uni ix, TL;\n\t"                                                                         \
-        QSS_L(0) QSS_L(1) QSS_L(2) QSS_L(3) QSS_L(4) QSS_L(5) QSS_L(6) QSS_L(7) \
-        QSS_L(8) QSS_L(9) QSS_L(10) QSS_L(11) QSS_L(12) QSS_L(13) QSS_L(14) QSS_L(15) \
-        QSS_L(16) QSS_L(17) QSS_L(18) QSS_L(19) QSS_L(20) QSS_L(21) QSS_L(22) QSS_L(23) \
-        QSS_L(24) QSS_L(25) QSS_L(26) QSS_L(27) QSS_L(28) QSS_L(29) QSS_L(30) QSS_L(31) \
-        QSS_L(32) QSS_L(33) QSS_L(34) QSS_L(35) QSS_L(36) QSS_L(37) QSS_L(38) QSS_L(39) \
-        QSS_L(40) QSS_L(41) QSS_L(42) QSS_L(43) QSS_L(44) QSS_L(45) QSS_L(46) QSS_L(47) \
-        QSS_L(48) QSS_L(49) QSS_L(50) QSS_L(51) QSS_L(52) QSS_L(53) QSS_L(54) QSS_L(55) \
-                 "LEND:\n\t}"                                                                                     \
-                 : "+d"(ct[0]), "+d"(ct[1]), "+d"(ct[2]), "+d"(ct[3]), "+d"(ct[4]), "+d"(ct[5]), "+d"(ct[6]), "+d"(ct[7]), "+d"(ct[8]), "+d"(ct[9]), "+d"(ct[10]), "+d"(ct[11]), "+d"(ct[12]), "+d"(ct[13]), "+d"(ct[14]), "+d"(ct[15]), "+d"(ct[16]), "+d"(ct[17]), "+d"(ct[18]), "+d"(ct[19]), "+d"(ct[20]), "+d"(ct[21]), "+d"(ct[22]), "+d"(ct[23]), "+d"(ct[24]), "+d"(ct[25]), "+d"(ct[26]), "+d"(ct[27]), "+d"(ct[28]), "+d"(ct[29]), "+d"(ct[30]), "+d"(ct[31]), "+d"(ct[32]), "+d"(ct[33]), "+d"(ct[34]), "+d"(ct[35]), \
-                   "+d"(cq[0]), "+d"(cq[1]), "+d"(cq[2]), "+d"(cq[3]), "+d"(cq[4]), "+d"(cq[5]), "+d"(cq[6]), "+d"(cq[7]), "+d"(cq[8]), "+d"(cq[9]), "+d"(cq[10]), "+d"(cq[11]), "+d"(cq[12]), "+d"(cq[13]), "+d"(cq[14]), "+d"(cq[15]), "+d"(cq[16]), "+d"(cq[17]), "+d"(cq[18]), "+d"(cq[19]) \
-                 : "d"((double)(a)), "d"((double)(b)), "r"((int)(slot)))
-static_assert(QSS_V1_NT == 36 && QSS_V1_NQ == 20, "QSS_SCATTER is written out for 36 + 20 register rows");
+#define LB(off) (*reinterpret_cast<double *>(sml + (off)))     // shared memory, byte offset of a row, this lane
 
 template <bool JAC>
-__global__ void __launch_bounds__(384, 1) qss_v1_kernel(const __grid_constant__ QssV1 p) {
+__global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_constant__ QssV1 p) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const int N = p.N, Nq = p.Nq, M = p.M, nsp = p.nsp;
     const int64_t ld = p.ld;
@@ -62,6 +45,7 @@ __global__ void __launch_bounds__(384, 1) qss_v1_kernel(const __grid_constant__ 
     double *sc = p.scratch + (size_t)blockIdx.x * p.scratch_stride + lane;
     const int32_t *gI = p.gI;
     const double *gD = p.gD;
+    char *const sml = reinterpret_cast<char *>(qss_smem) + lane * 8;
 
     for (int64_t slab = blockIdx.x; slab < nslab; slab += gridDim.x) {
         const int64_t cell = slab * 32 + lane;
@@ -135,7 +119,7 @@ __global__ void __launch_bounds__(384, 1) qss_v1_kernel(const __grid_constant__ 
                             dlnk = dlnkinf + delta * i1pr + dlF_dL * delta + dlF_dLc * dFc / Fc;
                         }
                     }
-                    if (JAC) SM(p.s_QM, tb) = dlm;
+                    if (JAC) SC(p.g_QM, tb) = dlm;
                 }
                 double kf = (mask & 1) ? k : 0.0, kb = 0.0, dlnKc = 0.0;
                 if (mask & 2) {                                    // reverse rate from the equilibrium constant (G10)
@@ -191,9 +175,13 @@ __global__ void __launch_bounds__(384, 1) qss_v1_kernel(const __grid_constant__ 
                     }
                 }
                 SM(oID, 0) = 1.0 / SM(oL, 0);
-                for (int k = sz - 1; k >= 1; --k) {
-                    const double tk = SM(oP0, k) * SM(oID, k);
-                    for (int m = 0; m < k; ++m) SM(oP0, m) += SM(base, m * sz + k) * tk;
+                for (int k = sz - 1; k >= 1; --k) {          // U[m][k] = P[m][k] / D_k (reused by every dy/dx solve)
+                    const double iD = SM(oID, k), tk = SM(oP0, k) * iD;
+                    for (int m = 0; m < k; ++m) {
+                        const double pmk = SM(base, m * sz + k);
+                        SM(base, m * sz + k) = pmk * iD;
+                        SM(oP0, m) += pmk * tk;
+                    }
                 }
                 for (int k = 0; k < sz; ++k) {
                     double acc = SM(oP0, k);
@@ -214,9 +202,9 @@ __global__ void __launch_bounds__(384, 1) qss_v1_kernel(const __grid_constant__ 
             SM(p.s_Q, j) = Q;
             if (JAC) {
                 const double qt = Q * SC(p.g_DF, j) + rb * SC(p.g_DC, j);
-                if (p.s_QT >= 0) SM(p.s_QT, j) = qt; else SC(p.g_DC, j) = qt;
+                SM(p.s_QT, j) = qt;
                 const int tb = (w >> 16) - 1;
-                if (tb >= 0) SM(p.s_QM, tb) *= Q;
+                if (tb >= 0) SC(p.g_QM, tb) *= Q;
             }
         }
         __syncthreads();
@@ -229,9 +217,9 @@ __global__ void __launch_bounds__(384, 1) qss_v1_kernel(const __grid_constant__ 
                 const double nu = HD(p.h_nulut, (e >> 12) & 15);
                 w = fma(nu, SM(p.s_Q, j), w);
                 if (JAC) {
-                    et = fma(nu, p.s_QT >= 0 ? SM(p.s_QT, j) : SC(p.g_DC, j), et);
+                    et = fma(nu, SM(p.s_QT, j), et);
                     const int tb = (e >> 16) - 1;
-                    if (tb >= 0) tv = fma(nu, SM(p.s_QM, tb), tv);
+                    if (tb >= 0) tv = fma(nu, SC(p.g_QM, tb), tv);
                 }
             }
             if (s < N && p.wdot && active) p.wdot[(size_t)s * ld + cell] = w;
@@ -244,76 +232,99 @@ __global__ void __launch_bounds__(384, 1) qss_v1_kernel(const __grid_constant__ 
             // ---- P7: W_y[i][q] = d wdot_i / d y_q at fixed x: sums of kappas (Eq. 9 second parenthesis, L224)
             for (int e = warp; e < p.n_wy; e += nw) {
                 double acc = 0.0;
-                for (int x = HT(p.h_wya_ptr, e); x < HT(p.h_wya_ptr, e + 1); ++x) {
-                    const int w = HT(p.h_wya, x);
+                for (int x = __ldg(gI + p.i_wya_ptr + e), xe = __ldg(gI + p.i_wya_ptr + e + 1); x < xe; ++x) {
+                    const int w = __ldg(gI + p.i_wya + x);
                     acc = fma(HD(p.h_nulut, (w >> 12) & 15), SC(p.g_KAP, w & 4095), acc);
                 }
-                SM(p.s_WY, e) = acc;
+                SC(p.g_WY, e) = acc;
             }
             __syncthreads();
-            // ---- P8: column sweep: column k of [W_x; G_x] in registers -> dy/dx_k -> J[:,k] = W_x[:,k] + W_y dy/dx_k
-            const int yrow = p.s_YC + warp * Nq;
-            for (int u = HT(p.h_cw_ptr, warp); u < HT(p.h_cw_ptr, warp + 1); ++u) {
-                const int k = HT(p.h_cw, u);
-                double ct[QSS_V1_NT], cq[QSS_V1_NQ];
-                if (k < N) {
+            // ---- P8: Jacobian sweep in rounds of nw columns (Eq. 7, Eq. 9)
+            char *const ycw = sml + (p.s_YC + warp) * 256;           // this warp's dy/dx column: row q at + q * nw * 256
+            for (int r = 0; r < p.n_rounds; ++r) {
+                // -- pass A: warp = column k.  [W_x; G_x][:,k] in registers, then (diag D - P) dy/dx_k = G_x[:,k]
+                const int k = HT(p.h_cw, r * nw + warp);
+                if (k >= 0) {
+                    double ct[QSS_V1_NT], cq[QSS_V1_NQ];
+                    if (k < N) {                                      // rank-1 third-body term (every species column)
 #pragma unroll
-                    for (int s = 0; s < QSS_V1_NT; ++s) ct[s] = s < N ? SM(p.s_TV, s) : 0.0;      // rank-1 third-body term
+                        for (int s = 0; s < QSS_V1_NT; ++s) ct[s] = s < N ? SM(p.s_TV, s) : 0.0;
 #pragma unroll
-                    for (int q = 0; q < QSS_V1_NQ; ++q) cq[q] = q < Nq ? SM(p.s_TV, N + q) : 0.0;
-                    for (int x = HT(p.h_col_ptr, k); x < HT(p.h_col_ptr, k + 1); ++x) {
-                        const int w = HT(p.h_inc, x), d = w & 4095, j = d >> 1;
-                        // d r_d / d C_k for one molecule slot: k_d times the other two slots (Eq. 9 first parenthesis)
-                        double part = SC(p.g_K, d) * SM(p.s_V, (w >> 12) & 255) * SM(p.s_V, (w >> 20) & 255);
-                        if (d & 1) part = -part;
-                        for (int y = HT(p.h_net_ptr, j); y < HT(p.h_net_ptr, j + 1); ++y) {
-                            const int e = HT(p.h_net, y);
-                            QSS_SCATTER(e & 255, HD(p.h_nulut, (e >> 8) & 15), part);
+                        for (int q = 0; q < QSS_V1_NQ; ++q) cq[q] = q < Nq ? SM(p.s_TV, N + q) : 0.0;
+                    } else {                                          // T column
+#pragma unroll
+                        for (int s = 0; s < QSS_V1_NT; ++s) ct[s] = s < N ? SC(p.g_ET, s) : 0.0;
+#pragma unroll
+                        for (int q = 0; q < QSS_V1_NQ; ++q) cq[q] = q < Nq ? SC(p.g_ET, N + q) : 0.0;
+                    }
+                    // column stream: part = A * V[o1] * V[o2] (* val), added to / subtracted from up to 8 register rows
+                    const int xe = p.h_cs + HT(p.h_cs_ptr, k + 1);
+#pragma unroll 1
+                    for (int x = p.h_cs + HT(p.h_cs_ptr, k); x < xe;) {
+                        const int2 a = *reinterpret_cast<const int2 *>(&p.h[x]);
+                        const int2 b = *reinterpret_cast<const int2 *>(&p.h[x + 2]);
+                        double part = sc[(size_t)(a.x & 0xffff) * 32] * LB(a.y & 0xffff) * LB((unsigned)a.y >> 16);
+                        x += 4;
+                        if (a.x & (1 << 20)) { part *= *reinterpret_cast<const double *>(&p.h[x]); x += 2; }
+                        unsigned w = (unsigned)b.x;
+                        QSS_SCAT(w & 255, part); QSS_SCAT((w >> 8) & 255, part);
+                        QSS_SCAT((w >> 16) & 255, part); QSS_SCAT(w >> 24, part);
+                        if ((unsigned)b.y != QSS_V1_NULL * 0x01010101u) {
+                            w = (unsigned)b.y;
+                            QSS_SCAT(w & 255, part); QSS_SCAT((w >> 8) & 255, part);
+                            QSS_SCAT((w >> 16) & 255, part); QSS_SCAT(w >> 24, part);
                         }
                     }
-                    for (int x = HT(p.h_effc_ptr, k); x < HT(p.h_effc_ptr, k + 1); ++x) {         // (alpha_k - 1) dQ/dM
-                        const int w = HT(p.h_effc, x), j = w & 4095;
-                        const double v = HD(p.h_effc_val, x) * SM(p.s_QM, w >> 12);
-                        for (int y = HT(p.h_net_ptr, j); y < HT(p.h_net_ptr, j + 1); ++y) {
-                            const int e = HT(p.h_net, y);
-                            QSS_SCATTER(e & 255, HD(p.h_nulut, (e >> 8) & 15), v);
+#pragma unroll
+                    for (int q = 0; q < QSS_V1_NQ; ++q) if (q < Nq) *reinterpret_cast<double *>(ycw + q * (QSS_V1_NW * 256)) = cq[q];
+                    // dy/dx solve program: y[a] = (y[a] + sum_t F_t * y[b_t]) [* 1/D]  (a thread only touches its own lane)
+                    int pc = p.h_sp;
+#pragma unroll 1
+                    for (int op = 0; op < p.n_sp_ops; ++op) {
+                        const unsigned hd = (unsigned)HT(pc, 0);
+                        ++pc;
+                        double *ya = reinterpret_cast<double *>(ycw + (hd & 0xffff));
+                        double acc = *ya;
+                        const int nt = (hd >> 16) & 255;
+                        const bool scale = (hd >> 24) != 0;
+                        const int idoff = scale ? HT(pc, 0) : 0;
+                        pc += scale ? 1 : 0;
+                        for (int t = 0; t < nt; ++t) {
+                            const unsigned w = (unsigned)HT(pc, t);
+                            acc = fma(LB(w & 0xffff), *reinterpret_cast<const double *>(ycw + (w >> 16)), acc);
+                        }
+                        pc += nt;
+                        if (scale) acc *= LB(idoff);
+                        *ya = acc;
+                    }
+                    char *const wxw = sml + (p.s_WX + warp) * 256;    // W_x[:,k] of this round: row i at + i * nw * 256
+#pragma unroll
+                    for (int i = 0; i < QSS_V1_NT; ++i) if (i < N) *reinterpret_cast<double *>(wxw + i * (QSS_V1_NW * 256)) = ct[i];
+                }
+                __syncthreads();
+                // -- pass B: warp = row i.  J[i, round] = W_x[i, round] + sum_q W_y[i][q] * dy_q/dx[round]
+                for (int i = warp; i < N; i += nw) {
+                    double acc[QSS_V1_NW];
+                    const char *wx = sml + (p.s_WX + i * nw) * 256;
+#pragma unroll
+                    for (int w = 0; w < QSS_V1_NW; ++w) acc[w] = *reinterpret_cast<const double *>(wx + w * 256);
+                    const int xe = HT(p.h_wr_ptr, i + 1);
+#pragma unroll 1
+                    for (int x = HT(p.h_wr_ptr, i); x < xe; ++x) {
+                        const double a = SC(p.g_WY, x);
+                        const char *yr = sml + p.s_YC * 256 + HT(p.h_wr, x);
+#pragma unroll
+                        for (int w = 0; w < QSS_V1_NW; ++w) acc[w] = fma(a, *reinterpret_cast<const double *>(yr + w * 256), acc[w]);
+                    }
+                    if (active) {
+#pragma unroll
+                        for (int w = 0; w < QSS_V1_NW; ++w) {
+                            const int kk = HT(p.h_cw, r * nw + w);
+                            if (kk >= 0) __stcs(&p.jac[((size_t)i * (N + 1) + kk) * ld + cell], acc[w]);
                         }
                     }
-                } else {
-#pragma unroll
-                    for (int s = 0; s < QSS_V1_NT; ++s) ct[s] = s < N ? SC(p.g_ET, s) : 0.0;
-#pragma unroll
-                    for (int q = 0; q < QSS_V1_NQ; ++q) cq[q] = q < Nq ? SC(p.g_ET, N + q) : 0.0;
                 }
-                // dy/dx_k: (diag D - P) ycol = G_x[:,k], group by group with the closure's elimination factors
-#pragma unroll
-                for (int q = 0; q < QSS_V1_NQ; ++q) if (q < Nq) SM(yrow, q) = cq[q];   // (a thread only ever touches its own lane's slot)
-                for (int g = 0; g < p.n_groups; ++g) {
-                    const int gi = p.h_group + g * QSS_GI_STRIDE;
-                    const int sz = HT(gi, 0), mo = p.h_gmember + HT(gi, 1), base = p.s_CL + HT(gi, 2);
-                    const int oID = base + sz * sz + 2 * sz;
-                    for (int x = HT(gi, 4); x < HT(gi, 5); ++x)
-                        SM(yrow, HT(mo, HT(p.h_xp_m, x))) += SM(p.s_XP, x) * SM(yrow, HT(p.h_xp_n, x));
-                    for (int kk = sz - 1; kk >= 1; --kk) {
-                        const double tk = SM(yrow, HT(mo, kk)) * SM(oID, kk);
-                        for (int m = 0; m < kk; ++m) SM(yrow, HT(mo, m)) += SM(base, m * sz + kk) * tk;
-                    }
-                    for (int kk = 0; kk < sz; ++kk) {
-                        double acc = SM(yrow, HT(mo, kk));
-                        for (int jj = 0; jj < kk; ++jj) acc += SM(base, kk * sz + jj) * SM(yrow, HT(mo, jj));
-                        SM(yrow, HT(mo, kk)) = acc * SM(oID, kk);
-                    }
-                }
-                // J[:,k] = W_x[:,k] + W_y dy/dx_k, one coalesced 256-byte streaming store per entry
-#pragma unroll
-                for (int i = 0; i < QSS_V1_NT; ++i) {
-                    if (i < N) {
-                        double acc = ct[i];
-                        for (int x = HT(p.h_wyrow_ptr, i); x < HT(p.h_wyrow_ptr, i + 1); ++x)
-                            acc = fma(SM(p.s_WY, x), SM(yrow, HT(p.h_wyq, x)), acc);
-                        if (active) __stcs(&p.jac[((size_t)i * (N + 1) + k) * ld + cell], acc);
-                    }
-                }
+                __syncthreads();
             }
         }
         __syncthreads();      // shared memory and the scratch slab are reused by the next cell slab

@@ -2,19 +2,22 @@
 // (qss_compile.cpp) and the kernel (qss_kernel_v1.cu).  Not part of the public ABI.
 //
 // Variant 1 processes a slab of 32 consecutive cells per thread block, lane = cell (so every table read is
-// warp-uniform and every per-cell array access is a conflict-free 256-byte row), one block per SM.  The hot
-// per-cell state lives in shared memory, one Jacobian column at a time lives in REGISTERS (scatter through a
-// uniform indexed branch), the interpreter tables live in the kernel-parameter constant bank (`h`), and only
-// the write-once / read-once per-direction arrays (k_d, kappa_d, dlnk/dT) go to an L2-resident scratch slab.
-// DESIGN.md "Kernels" gives the layout and the reasons.
+// warp-uniform and every per-cell array access is a conflict-free 256-byte row), one block of QSS_V1_NW warps per
+// SM.  The hot per-cell state lives in shared memory; the Jacobian is swept in rounds of QSS_V1_NW columns: each
+// warp builds one column of [W_x; G_x] in REGISTERS (scatter through an indexed branch) and solves for dy/dx_k,
+// then the warps switch to rows and add W_y * dy/dx for the whole round from a register tile.  The interpreter
+// tables live in the kernel-parameter constant bank (`h`); the write-once / read-few per-direction arrays go to an
+// L2-resident scratch slab.  DESIGN.md "Kernels" gives the layout and the reasons.
 #ifndef QSS_V1_H
 #define QSS_V1_H
 #include <stdint.h>
 
-#define QSS_V1_HMAX 7600        // 32-bit words of hot tables carried in the kernel parameters (<= 32 KB total)
-#define QSS_V1_NT 36            // max transported species (register column rows)
-#define QSS_V1_NQ 20            // max QSS species
+#define QSS_V1_HMAX 8000        // 32-bit words of hot tables carried in the kernel parameters (<= 32 KB total)
+#define QSS_V1_NT 36            // register column: rows for transported species (needs N + 1 <= 36 columns too)
+#define QSS_V1_NQ 20            // register column: rows for QSS species
+#define QSS_V1_NW 12            // warps per block = Jacobian columns per round
 #define QSS_V1_RREC 8           // int32 words per reaction record
+#define QSS_V1_NULL 112         // scatter index that does nothing (2 * (NT + NQ))
 
 struct QssV1 {
     // ---- filled at launch
@@ -25,24 +28,26 @@ struct QssV1 {
     const int32_t *gI;
     const double *gD;
     int32_t d_thermo, d_rate, d_effm1, i_eff_ptr, i_eff_sp, i_rrec;
+    int32_t i_wya_ptr, i_wya;                        // W_y assembly lists: dir | nucode<<12 (global, read once per slab)
     // ---- sizes
-    int32_t N, Nq, M, nsp, n_tb, nw, n_groups, n_levels, n_centry, n_xp, n_wy;
-    // ---- shared-memory rows (one row = 32 doubles, lane = cell)
-    int32_t s_V;        // [N+1+Nq]  C_0..C_{N-1}, 1.0, y_0..y_{Nq-1}
+    int32_t N, Nq, M, nsp, n_tb, nw, n_groups, n_levels, n_centry, n_xp, n_wy, n_rounds, n_sp_ops;
+    // ---- shared-memory rows (one row = 32 doubles = 256 bytes, lane = cell)
+    int32_t s_V;        // [N+1+Nq]  C_0..C_{N-1}, 1.0, y_0..y_{Nq-1}      (must start at row 0)
     int32_t s_CT;       // [1]       sum_k C_k
     int32_t s_CL;       // [cl_size] closure storage: per group P[g*g], leak[g], p0[g], 1/D[g]
     int32_t s_XP;       // [n_xp]    cross-group couplings
     int32_t s_TV;       // [nsp]     third-body vector  sum_j nu_sj dQ_j/dM
-    int32_t s_QM;       // [n_tb]    d ln k / dM, then dQ/dM
-    int32_t s_WY;       // [n_wy]    W_y entries, row-major            } region R, time-shared with
-    int32_t s_YC;       // [nw*Nq]   per-warp dy/dx_k column           }   s_G, s_H (thermo, rate phases)
-    int32_t s_G, s_H;   // [nsp+1]   g/RT, h/RT (+ a zero row)          }   s_Q, s_QT (net rates phase)
-    int32_t s_Q, s_QT;  // [M]       Q_j, dQ_j/dT at fixed y, M; s_QT < 0: kept in the scratch DC rows
+    int32_t s_YC;       // [Nq*nw]   dy/dx of the round's columns, row q*nw + w   } region R, time-shared with
+    int32_t s_WX;       // [N*nw]    W_x of the round's columns, row i*nw + w     }   s_G, s_H (thermo, rate phases)
+    int32_t s_G, s_H;   // [nsp+1]   g/RT, h/RT (+ a zero row)                    }   s_Q, s_QT (net rates phase)
+    int32_t s_Q, s_QT;  // [M]       Q_j, dQ_j/dT at fixed y, M
     int32_t smem_rows;
     // ---- scratch rows
     int32_t g_K, g_KAP; // [2M]      k_d, kappa_d
     int32_t g_DF, g_DC; // [M]       dlnk/dT, dlnKc/dT
     int32_t g_ET;       // [nsp]     T-column vector sum_j nu_sj dQ_j/dT
+    int32_t g_QM;       // [n_tb]    d ln k / dM, then dQ/dM
+    int32_t g_WY;       // [n_wy]    W_y entries, row-major
     int32_t scratch_rows;
     // ---- hot tables (offsets into h)
     int32_t h_ce_ptr, h_ce_dst, h_ce_dir;            // closure gather
@@ -51,15 +56,13 @@ struct QssV1 {
     int32_t h_q;                                     // [M] qf | qb<<8 | (tb+1)<<16  (V rows of the QSS reactants)
     int32_t h_ssw_ptr, h_ssw;                        // species assigned to each warp (balanced)
     int32_t h_ss_ptr, h_ss;                          // species incidence: j | nucode<<12 | (tb+1)<<16
-    int32_t h_wya_ptr, h_wya;                        // W_y assembly: dir | nucode<<12
-    int32_t h_cw_ptr, h_cw;                          // Jacobian columns assigned to each warp (balanced)
-    int32_t h_col_ptr, h_inc;                        // column incidences: d | o1<<12 | o2<<20
-    int32_t h_net_ptr, h_net;                        // net stoichiometry by reaction: slot | nucode<<8
-    int32_t h_effc_ptr, h_effc, h_effc_val;          // (alpha-1) corrections by column: j | tb<<12 ; double values
-    int32_t h_wyrow_ptr, h_wyq;                      // W_y rows: QSS index of each entry
+    int32_t h_cw;                                    // [n_rounds*nw] Jacobian column of (round, warp), -1: none
+    int32_t h_cs_ptr, h_cs;                          // column streams (see qss_compile.cpp "column stream")
+    int32_t h_sp;                                    // dy/dx solve program (row operations)
+    int32_t h_wr_ptr, h_wr;                          // W_y rows: byte offset q*nw*256 of each entry's dy/dx row
     int32_t h_nulut;                                 // 16 doubles: nucode -> nu (nucode = nu + 8)
     int32_t h_used;
-    int32_t h[QSS_V1_HMAX];
+    alignas(8) int32_t h[QSS_V1_HMAX];
 };
 
 #endif
