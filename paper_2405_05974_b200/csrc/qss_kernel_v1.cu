@@ -18,6 +18,7 @@
 #include <stdint.h>
 
 #include "qss_tables.h"
+#include "qss_math.h"
 #include "qss_v1.h"
 #include "qss_v1_scatter.h"
 
@@ -34,7 +35,14 @@ extern __shared__ double qss_smem[];
 #define SM(row, i) qss_smem[((row) + (i)) * 32 + lane]
 #define SC(row, i) sc[(size_t)((row) + (i)) * 32]
 
-#define LB(off) (*reinterpret_cast<double *>(sml + (off)))     // shared memory, byte offset of a row, this lane
+// shared memory through 32-bit shared-window addresses (a generic pointer costs a window-base computation per access)
+__device__ __forceinline__ double lds(unsigned a) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
+__device__ __forceinline__ int2 ldc2(const int32_t *q) { return *reinterpret_cast<const int2 *>(q); }
 
 template <bool JAC>
 __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_constant__ QssV1 p) {
@@ -45,7 +53,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
     double *sc = p.scratch + (size_t)blockIdx.x * p.scratch_stride + lane;
     const int32_t *gI = p.gI;
     const double *gD = p.gD;
-    char *const sml = reinterpret_cast<char *>(qss_smem) + lane * 8;
+    const unsigned sml = (unsigned)__cvta_generic_to_shared(qss_smem) + lane * 8;   // this lane's column of the rows
 
     for (int64_t slab = blockIdx.x; slab < nslab; slab += gridDim.x) {
         const int64_t cell = slab * 32 + lane;
@@ -83,7 +91,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                 const double *rd = gD + p.d_rate + j * QSS_RD_STRIDE;
                 const double lnkinf = rd[0] + rd[1] * lnT - rd[2] * invT;
                 const double dlnkinf = (rd[1] + rd[2] * invT) * invT;
-                double k = exp(lnkinf), dlnk = dlnkinf;
+                double k = qss_exp(lnkinf), dlnk = dlnkinf;
                 if (type >= 1) {
                     double Mc = Ctot;                              // M = sum_k alpha_k C_k, transported only (G7)
                     const int e0 = gI[p.i_eff_ptr + j], e1 = gI[p.i_eff_ptr + j + 1];
@@ -95,9 +103,9 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                     } else {                                       // Troe fall-off
                         const double lnk0 = rd[3] + rd[4] * lnT - rd[5] * invT;
                         const double dlnk0 = (rd[4] + rd[5] * invT) * invT;
-                        const double Pr = exp(lnk0 - lnkinf) * Mc;
+                        const double Pr = qss_exp(lnk0 - lnkinf) * Mc;
                         const double al = rd[6], i3 = rd[7], i1 = rd[8], T2s = rd[9];
-                        const double e3 = exp(-T * i3), e1x = exp(-T * i1), e2 = exp(-T2s * invT);
+                        const double e3 = qss_exp(-T * i3), e1x = qss_exp(-T * i1), e2 = qss_exp(-T2s * invT);
                         const double Fc = (1.0 - al) * e3 + al * e1x + e2;
                         const double L = log(Pr) * kInvLn10, Lc = log(Fc) * kInvLn10;
                         const double c = -0.4 - 0.67 * Lc, n = 0.75 - 1.27 * Lc;
@@ -105,7 +113,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                         const double iden = 1.0 / den;
                         const double f1 = num * iden;
                         const double ione_f = 1.0 / (1.0 + f1 * f1);
-                        const double F = exp(kLn10 * Lc * ione_f);
+                        const double F = qss_exp(kLn10 * Lc * ione_f);
                         const double i1pr = 1.0 / (1.0 + Pr);
                         k = k * (Pr * i1pr) * F;
                         const double df1_dL = n * iden * iden;
@@ -125,7 +133,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                 if (mask & 2) {                                    // reverse rate from the equilibrium constant (G10)
                     const double dG = (SM(p.s_G, rb.y & 255) + SM(p.s_G, (rb.y >> 8) & 255) + SM(p.s_G, (rb.y >> 16) & 255)) -
                                       (SM(p.s_G, rb.x & 255) + SM(p.s_G, (rb.x >> 8) & 255) + SM(p.s_G, (rb.x >> 16) & 255));
-                    kb = k * exp(dG - rd[10] * lnP0RT);            // k / Kc, ln Kc = -dG + dnu ln(P0/RT)
+                    kb = k * qss_exp(dG - rd[10] * lnP0RT);            // k / Kc, ln Kc = -dG + dnu ln(P0/RT)
                     if (JAC) {
                         const double dH = (SM(p.s_H, rb.y & 255) + SM(p.s_H, (rb.y >> 8) & 255) + SM(p.s_H, (rb.y >> 16) & 255)) -
                                           (SM(p.s_H, rb.x & 255) + SM(p.s_H, (rb.x >> 8) & 255) + SM(p.s_H, (rb.x >> 16) & 255));
@@ -240,7 +248,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             }
             __syncthreads();
             // ---- P8: Jacobian sweep in rounds of nw columns (Eq. 7, Eq. 9)
-            char *const ycw = sml + (p.s_YC + warp) * 256;           // this warp's dy/dx column: row q at + q * nw * 256
+            const unsigned ycw = sml + (p.s_YC + warp) * 256;        // this warp's dy/dx column: row q at + q * nw * 256
             for (int r = 0; r < p.n_rounds; ++r) {
                 // -- pass A: warp = column k.  [W_x; G_x][:,k] in registers, then (diag D - P) dy/dx_k = G_x[:,k]
                 const int k = HT(p.h_cw, r * nw + warp);
@@ -257,15 +265,22 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
 #pragma unroll
                         for (int q = 0; q < QSS_V1_NQ; ++q) cq[q] = q < Nq ? SC(p.g_ET, N + q) : 0.0;
                     }
-                    // column stream: part = A * V[o1] * V[o2] (* val), added to / subtracted from up to 8 register rows
+                    // column stream: part = A * V[o1] * V[o2] (* val), added to / subtracted from up to 8 register rows.
+                    // The next record and its A (an L2 read) are fetched before the current one is scattered.
+                    int x = p.h_cs + HT(p.h_cs_ptr, k);
                     const int xe = p.h_cs + HT(p.h_cs_ptr, k + 1);
+                    int2 na = make_int2(0, 0), nb = make_int2(0, 0);
+                    double nA = 0.0;
+                    if (x < xe) { na = ldc2(&p.h[x]); nb = ldc2(&p.h[x + 2]); nA = sc[(size_t)(na.x & 0xffff) * 32]; }
 #pragma unroll 1
-                    for (int x = p.h_cs + HT(p.h_cs_ptr, k); x < xe;) {
-                        const int2 a = *reinterpret_cast<const int2 *>(&p.h[x]);
-                        const int2 b = *reinterpret_cast<const int2 *>(&p.h[x + 2]);
-                        double part = sc[(size_t)(a.x & 0xffff) * 32] * LB(a.y & 0xffff) * LB((unsigned)a.y >> 16);
-                        x += 4;
-                        if (a.x & (1 << 20)) { part *= *reinterpret_cast<const double *>(&p.h[x]); x += 2; }
+                    while (x < xe) {
+                        const int2 a = na, b = nb;
+                        double part = nA;
+                        const bool has_val = (a.x & (1 << 20)) != 0;
+                        if (has_val) part *= *reinterpret_cast<const double *>(&p.h[x + 4]);
+                        x += has_val ? 6 : 4;
+                        if (x < xe) { na = ldc2(&p.h[x]); nb = ldc2(&p.h[x + 2]); nA = sc[(size_t)(na.x & 0xffff) * 32]; }
+                        part *= lds(sml + (a.y & 0xffff)) * lds(sml + ((unsigned)a.y >> 16));
                         unsigned w = (unsigned)b.x;
                         QSS_SCAT(w & 255, part); QSS_SCAT((w >> 8) & 255, part);
                         QSS_SCAT((w >> 16) & 255, part); QSS_SCAT(w >> 24, part);
@@ -276,51 +291,55 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                         }
                     }
 #pragma unroll
-                    for (int q = 0; q < QSS_V1_NQ; ++q) if (q < Nq) *reinterpret_cast<double *>(ycw + q * (QSS_V1_NW * 256)) = cq[q];
+                    for (int q = 0; q < QSS_V1_NQ; ++q) if (q < Nq) sts(ycw + q * (QSS_V1_NW * 256), cq[q]);
                     // dy/dx solve program: y[a] = (y[a] + sum_t F_t * y[b_t]) [* 1/D]  (a thread only touches its own lane)
                     int pc = p.h_sp;
 #pragma unroll 1
-                    for (int op = 0; op < p.n_sp_ops; ++op) {
+                    for (int op = p.n_sp_ops; op > 0; --op) {
                         const unsigned hd = (unsigned)HT(pc, 0);
+                        const unsigned ya = ycw + (hd & 0xffff);
+                        double acc = lds(ya);
+                        int nt = (hd >> 16) & 255;
                         ++pc;
-                        double *ya = reinterpret_cast<double *>(ycw + (hd & 0xffff));
-                        double acc = *ya;
-                        const int nt = (hd >> 16) & 255;
-                        const bool scale = (hd >> 24) != 0;
-                        const int idoff = scale ? HT(pc, 0) : 0;
-                        pc += scale ? 1 : 0;
-                        for (int t = 0; t < nt; ++t) {
-                            const unsigned w = (unsigned)HT(pc, t);
-                            acc = fma(LB(w & 0xffff), *reinterpret_cast<const double *>(ycw + (w >> 16)), acc);
+                        unsigned idoff = 0;
+                        if (hd >> 24) { idoff = (unsigned)HT(pc, 0); ++pc; }
+#pragma unroll 1
+                        for (; nt > 0; --nt, ++pc) {
+                            const unsigned w = (unsigned)HT(pc, 0);
+                            acc = fma(lds(sml + (w & 0xffff)), lds(ycw + (w >> 16)), acc);
                         }
-                        pc += nt;
-                        if (scale) acc *= LB(idoff);
-                        *ya = acc;
+                        if (hd >> 24) acc *= lds(sml + idoff);
+                        sts(ya, acc);
                     }
-                    char *const wxw = sml + (p.s_WX + warp) * 256;    // W_x[:,k] of this round: row i at + i * nw * 256
+                    const unsigned wxw = sml + (p.s_WX + warp) * 256;  // W_x[:,k] of this round: row i at + i * nw * 256
 #pragma unroll
-                    for (int i = 0; i < QSS_V1_NT; ++i) if (i < N) *reinterpret_cast<double *>(wxw + i * (QSS_V1_NW * 256)) = ct[i];
+                    for (int i = 0; i < QSS_V1_NT; ++i) if (i < N) sts(wxw + i * (QSS_V1_NW * 256), ct[i]);
                 }
                 __syncthreads();
                 // -- pass B: warp = row i.  J[i, round] = W_x[i, round] + sum_q W_y[i][q] * dy_q/dx[round]
                 for (int i = warp; i < N; i += nw) {
                     double acc[QSS_V1_NW];
-                    const char *wx = sml + (p.s_WX + i * nw) * 256;
+                    const unsigned wx = sml + (p.s_WX + i * nw) * 256;
 #pragma unroll
-                    for (int w = 0; w < QSS_V1_NW; ++w) acc[w] = *reinterpret_cast<const double *>(wx + w * 256);
+                    for (int w = 0; w < QSS_V1_NW; ++w) acc[w] = lds(wx + w * 256);
+                    int x = HT(p.h_wr_ptr, i);
                     const int xe = HT(p.h_wr_ptr, i + 1);
+                    double na = x < xe ? SC(p.g_WY, x) : 0.0;
+                    unsigned ny = x < xe ? (unsigned)HT(p.h_wr, x) : 0u;
 #pragma unroll 1
-                    for (int x = HT(p.h_wr_ptr, i); x < xe; ++x) {
-                        const double a = SC(p.g_WY, x);
-                        const char *yr = sml + p.s_YC * 256 + HT(p.h_wr, x);
+                    for (; x < xe; ++x) {
+                        const double a = na;
+                        const unsigned yr = sml + p.s_YC * 256 + ny;
+                        if (x + 1 < xe) { na = SC(p.g_WY, x + 1); ny = (unsigned)HT(p.h_wr, x + 1); }
 #pragma unroll
-                        for (int w = 0; w < QSS_V1_NW; ++w) acc[w] = fma(a, *reinterpret_cast<const double *>(yr + w * 256), acc[w]);
+                        for (int w = 0; w < QSS_V1_NW; ++w) acc[w] = fma(a, lds(yr + w * 256), acc[w]);
                     }
                     if (active) {
+                        double *jrow = p.jac + (size_t)i * (N + 1) * ld + cell;
 #pragma unroll
                         for (int w = 0; w < QSS_V1_NW; ++w) {
                             const int kk = HT(p.h_cw, r * nw + w);
-                            if (kk >= 0) __stcs(&p.jac[((size_t)i * (N + 1) + kk) * ld + cell], acc[w]);
+                            if (kk >= 0) __stcs(jrow + (size_t)(unsigned)kk * (size_t)ld, acc[w]);
                         }
                     }
                 }
