@@ -1,0 +1,169 @@
+"""Host-side logic of libqss (no GPU): ABI surface, mechanism validation, SCC ordering of the QSS groups
+(App. B), the branch-free exp, and the cell sharding used at N > 1."""
+import ctypes as ct
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+import paper_2405_05974_b200 as qss
+import qss_synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_symbol_of_the_header():
+    hdr = open(os.path.join(ROOT, "include", "qss.h")).read()
+    declared = sorted(set(re.findall(r"\b(qss_[a-z0-9_]+)\s*\(", hdr)))
+    assert set(declared) == set(qss.EXPORTS), (declared, qss.EXPORTS)
+    L = qss.lib()
+    for name in declared:
+        assert getattr(L, name) is not None
+
+
+def test_no_cpu_fallback_create_fails_without_a_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    with pytest.raises(qss.QssError) as e:
+        qss.QssMech(qss_synth.toy1(), 0)
+    assert e.value.code == -6            # QSS_E_CUDA
+
+
+@pytest.mark.parametrize("cfg,gmax", [(1, 3), (2, 4), (3, 6)])
+def test_group_sizes_of_the_configs(cfg, gmax):
+    mech = qss_synth.config_mechanism(cfg)
+    ng, order, grp = qss.validate(mech)
+    assert sorted(order.tolist()) == list(range(mech.n_qss))
+    sizes = np.bincount(grp, minlength=ng)
+    assert sizes.max() == gmax and sizes.sum() == mech.n_qss
+
+
+def _edges(mech):
+    """QSS digraph: n -> m iff an enabled direction consumes QSS n and produces QSS m."""
+    N = mech.n_nqss
+    E = set()
+    for j in range(mech.n_reac):
+        R = [int(s) for s in mech.reac_sp[mech.reac_ptr[j]:mech.reac_ptr[j + 1]] if s >= N]
+        P = [int(s) for s in mech.prod_sp[mech.prod_ptr[j]:mech.prod_ptr[j + 1]] if s >= N]
+        if mech.dir_mask[j] & 1:
+            E |= {(n - N, m - N) for n in R for m in P if n != m}
+        if mech.dir_mask[j] & 2:
+            E |= {(n - N, m - N) for n in P for m in R if n != m}
+    return E
+
+
+@pytest.mark.parametrize("make", [qss_synth.toy_dag, lambda: qss_synth.config_mechanism(2), lambda: qss_synth.config_mechanism(3)])
+def test_groups_are_the_sccs_in_topological_order(make):
+    mech = make()
+    ng, order, grp = qss.validate(mech)
+    g_of = {int(q): int(g) for q, g in zip(order, grp)}
+    E = _edges(mech)
+    # solve order respects every edge: the producer side n of n -> m is solved no later than m
+    assert all(g_of[n] <= g_of[m] for n, m in E)
+    # two species share a group iff they reach each other (brute-force transitive closure)
+    nq = mech.n_qss
+    reach = np.eye(nq, dtype=bool)
+    for n, m in E:
+        reach[n, m] = True
+    for k in range(nq):
+        reach |= reach[:, k:k + 1] & reach[k:k + 1, :]
+    for a in range(nq):
+        for b in range(nq):
+            assert (g_of[a] == g_of[b]) == bool(reach[a, b] and reach[b, a])
+
+
+def _with(mech, **kw):
+    import dataclasses
+    return dataclasses.replace(mech, **kw)
+
+
+def test_validation_errors():
+    m = qss_synth.toy2()                                   # A <=> Q1, Q1 <=> Q2, Q2 <=> B ; species A B Q1 Q2
+    # quadratic coupling: 2 Q1 on the reactant side of an enabled direction
+    bad = _with(m, reac_nu=np.array([1, 2, 1], dtype=np.int32))
+    with pytest.raises(qss.QssError) as e:
+        qss.validate(bad)
+    assert e.value.code == -2
+    # the same side only produced (reverse disabled... forward consumes Q1 twice) -> still quadratic; disable forward: fan-out
+    bad2 = _with(bad, dir_mask=np.array([3, 2, 3], dtype=np.uint8))
+    with pytest.raises(qss.QssError) as e:
+        qss.validate(bad2)
+    assert e.value.code == -3
+    # no sink: Q2 can only be produced, never consumed towards a transported species
+    bad3 = _with(m, dir_mask=np.array([3, 1, 2], dtype=np.uint8))
+    with pytest.raises(qss.QssError) as e:
+        qss.validate(bad3)
+    assert e.value.code == -4
+    # unsupported reaction type, bad species index
+    with pytest.raises(qss.QssError) as e:
+        qss.validate(_with(m, rtype=np.array([0, 7, 0], dtype=np.int32)))
+    assert e.value.code == -5
+    with pytest.raises(qss.QssError) as e:
+        qss.validate(_with(m, reac_sp=np.array([0, 2, 9], dtype=np.int32)))
+    assert e.value.code == -1
+
+
+def test_branch_free_exp_against_float128(tmp_path):
+    """csrc/qss_math.h compiled for the host: <= 1.5 ulp against libquadmath over the whole finite range."""
+    src = tmp_path / "t.cpp"
+    src.write_text(r'''
+#include "qss_math.h"
+#include <cstdio>
+#include <random>
+#include <quadmath.h>
+int main() {
+  std::mt19937_64 g(1); double worst = 0;
+  std::uniform_real_distribution<double> u(-745.0, 709.0), s(-1.0, 1.0);
+  for (int i = 0; i < 2000000; ++i) {
+    double x = (i & 1) ? u(g) : s(g), a = qss_exp(x); __float128 r = expq((__float128)x); double rd = (double)r;
+    if (rd == 0 || std::isinf(rd)) continue;
+    double ulp = std::fabs(std::nextafter(rd, INFINITY) - rd), e = (double)fabsq((__float128)a - r) / ulp;
+    if (e > worst) worst = e;
+  }
+  printf("%.4f %d %d %d\n", worst, qss_exp(0.0) == 1.0, qss_exp(-1000.0) == 0.0, std::isinf(qss_exp(1000.0)));
+}''')
+    exe = tmp_path / "t"
+    subprocess.run(["g++", "-O2", "-ffp-contract=off", "-I", os.path.join(ROOT, "paper_2405_05974_b200", "csrc"), "-o", str(exe),
+                    str(src), "-lquadmath"], check=True)
+    worst, one, zero, inf = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()
+    assert float(worst) <= 1.5 and one == "1" and zero == "1" and inf == "1"
+
+
+def test_cell_ranges_tile_the_cells():
+    from paper_2405_05974_b200.shard import cell_range
+    for n in (0, 1, 31, 32, 33, 4096, 2 ** 20, 2 ** 20 + 5):
+        for world in (1, 2, 3, 8):
+            r = [cell_range(n, k, world) for k in range(world)]
+            assert r[0][0] == 0 and r[-1][1] == n
+            assert all(a[1] == b[0] for a, b in zip(r, r[1:]))
+            assert all(b % 32 == 0 or b == n for b, _ in r)
+            sizes = [e - b for b, e in r]
+            assert max(sizes) - min(sizes) < 64 or n < 32 * world
+
+
+def _gloo_worker(rank, world, port, q):
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from paper_2405_05974_b200.shard import cell_range, max_over_ranks
+    b, e = cell_range(1000, rank, world)
+    t = max_over_ranks(1.0 + rank, dist)
+    q.put((rank, b, e, t))
+    dist.destroy_process_group()
+
+
+def test_two_rank_sharding_and_timing_reduction_gloo():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29500 + os.getpid() % 500
+    ps = [ctx.Process(target=_gloo_worker, args=(r, 2, port, q)) for r in range(2)]
+    [p.start() for p in ps]
+    out = sorted(q.get(timeout=120) for _ in ps)
+    [p.join(60) for p in ps]
+    assert out[0][1:3] == (0, 512) and out[1][1:3] == (512, 1000)
+    assert out[0][3] == 2.0 and out[1][3] == 2.0          # max over ranks
