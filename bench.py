@@ -196,10 +196,8 @@ def main():
     clocks = sampler.stop() if sampler else None
     total_ms = evs[0].elapsed_time(evs[-1])
     launch_ms = [evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)]
-    tt = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    total_ms_max = float(tt.item())
+    from paper_2405_05974_b200.shard import max_over_ranks
+    total_ms_max = max_over_ranks(total_ms, dist, dev)
     value = world * n * args.steps / (total_ms_max * 1e-3)
 
     # ---- end to end through the C-ABI host-buffer call: pinned host buffers, H2D + D2H inside the timed region
@@ -219,10 +217,7 @@ def main():
             qm.eval_jac_host(Ch, Th, Jh, Wh, scratch, n)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        te = torch.tensor([dt], dtype=torch.float64, device=dev)
-        if dist is not None:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * n * ke / float(te.item()), "unit": UNIT,
+        e2e = {"value": world * n * ke / max_over_ranks(dt, dist, dev), "unit": UNIT,
                "h2d_bytes_per_step": int((N + 1) * ld * 8), "d2h_bytes_per_step": int((N * (N + 1) + N) * ld * 8),
                "steps": ke, "api": "qss_eval_jac_host (C-ABI, pinned host buffers, copies + kernel + sync timed by wall clock)"}
         assert bool(torch.isfinite(Wh[:, :n]).all())
