@@ -240,7 +240,15 @@ def main():
     else:
         roof = {"bound": "hbm", "achieved": bytes_launch / avg_s / 1e9, "peak": hbm_gbs, "unit": "GB/s"}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof.update({"traffic": None, "kernel": "qss jacobian kernel (qss_eval_jac, wdot output on)",
+    traffic = None
+    try:        # bytes of one launch from the committed ncu capture of the same workload and kernel variant, else null
+        with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
+            tj = json.load(f)
+        if tj["cfg"] == cfg and tj["cells"] == n and tj["kernel_variant"] == info.kernel_variant_jac:
+            traffic = tj["dram_bytes_per_launch"]
+    except Exception:
+        traffic = None
+    roof.update({"traffic": traffic, "traffic_unit": "bytes per launch (dram read + write, ncu)", "kernel": "qss jacobian kernel (qss_eval_jac, wdot output on)",
                  "launch_ms_avg": avg_s * 1e3, "launch_ms_min": min(launch_ms),
                  "alg_fp64_slots_per_cell": info.slots_jac, "alg_bytes_per_cell": info.bytes_jac + 8.0 * N,
                  "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3,
