@@ -191,18 +191,17 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     auto take = [&](int n) { int r = rows_fixed; rows_fixed += n; return r; };
     v.s_V = take(N + 1 + Nq); v.s_CT = take(1); v.s_CL = take(c.cl_size); v.s_XP = take(v.n_xp); v.s_TV = take(nsp);
     const int max_rows = (227 * 1024) / 256;
-    const int region = std::max(std::max((Nq + N) * nw, 2 * (nsp + 1)), 2 * M);
+    const int region = std::max((Nq + N) * nw, 2 * M + 2 * (nsp + 1));
     if (rows_fixed + region > max_rows) { why = "per-cell state does not fit the shared memory of one SM"; return false; }
     if ((v.s_XP + v.n_xp) * 256 > 65535 || Nq * nw * 256 > 65535) { why = "closure storage beyond the 16-bit offsets of variant 1"; return false; }
     v.nw = nw;
     v.s_YC = rows_fixed; v.s_WX = rows_fixed + Nq * nw;
-    v.s_G = rows_fixed; v.s_H = rows_fixed + nsp + 1;
-    v.s_Q = rows_fixed; v.s_QT = rows_fixed + M;
+    v.s_KAP = rows_fixed; v.s_G = rows_fixed + 2 * M; v.s_H = v.s_G + nsp + 1;
     v.smem_rows = rows_fixed + region;
     {
         int o = 0;
         auto tk = [&](int n) { int r = o; o += n; return r; };
-        v.g_K = tk(2 * M); v.g_KAP = tk(2 * M); v.g_DF = tk(M); v.g_DC = tk(M); v.g_ET = tk(nsp); v.g_QM = tk(c.n_tb); v.g_WY = tk(v.n_wy);
+        v.g_K = tk(2 * M); v.g_DF = tk(M); v.g_DC = tk(M); v.g_ET = tk(nsp); v.g_QM = tk(c.n_tb); v.g_WY = tk(v.n_wy);
         v.scratch_rows = o;
         if (o > 65535) { why = "scratch rows beyond the 16-bit offsets of variant 1"; return false; }
     }
@@ -292,6 +291,19 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         v.h_ssw_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
         v.h_ssw = at(); H.insert(H.end(), all.begin(), all.end());
     }
+    {   // pass B rows: balanced by the number of W_y entries
+        std::vector<int> idx(N), cnt(N, 0);
+        for (auto &kv : wy) cnt[kv.first.first]++;
+        for (int i = 0; i < N; ++i) idx[i] = i;
+        std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return cnt[a] > cnt[b]; });
+        std::vector<std::vector<int32_t>> bin(nw);
+        std::vector<double> load(nw, 0.0);
+        for (int i : idx) { int b = (int)(std::min_element(load.begin(), load.end()) - load.begin()); bin[b].push_back(i); load[b] += 14.0 + cnt[i]; }
+        std::vector<int32_t> ptr{0}, all;
+        for (int w = 0; w < nw; ++w) { all.insert(all.end(), bin[w].begin(), bin[w].end()); ptr.push_back((int32_t)all.size()); }
+        v.h_rw_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
+        v.h_rw = at(); H.insert(H.end(), all.begin(), all.end());
+    }
     // ---- Jacobian columns: rounds of nw columns of similar cost (the warps meet at a barrier after every round)
     {
         std::vector<int> idx(N + 1);
@@ -333,7 +345,15 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         }
     }
     v.N = N; v.Nq = Nq; v.M = M; v.nsp = nsp; v.n_tb = c.n_tb; v.n_groups = c.n_groups; v.n_levels = c.n_levels;
-    v.d_thermo = out.tab.d_thermo; v.d_rate = out.tab.d_rate; v.d_effm1 = out.tab.d_effm1;
+    v.d_thermo = out.tab.d_thermo; v.d_effm1 = out.tab.d_effm1;
+    {   // rate records again, in processing order (so that a warp can prefetch the next one without knowing j)
+        std::vector<double> &Dd = out.D;
+        v.d_rate_r = (int32_t)Dd.size();
+        for (int r = 0; r < M; ++r) {
+            const size_t src = (size_t)out.tab.d_rate + (size_t)(*c.rorder)[r] * QSS_RD_STRIDE;
+            for (int u = 0; u < QSS_RD_STRIDE; ++u) Dd.push_back(Dd[src + u]);
+        }
+    }
     v.i_eff_ptr = out.tab.i_eff_ptr; v.i_eff_sp = out.tab.i_eff_sp;
     return true;
 }

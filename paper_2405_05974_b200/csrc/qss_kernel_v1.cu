@@ -84,13 +84,30 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         // ---- P2: rate constants, direction coefficients kappa_d (Eq. 2, Eq. 6)
         {
             const double Ctot = SM(p.s_CT, 0);
+            // records and Arrhenius parameters are stored in processing order; those of the warp's NEXT reaction are
+            // fetched (L2 reads, the L1 is a few KB next to the shared memory) before the current one is evaluated
+            int4 nra = make_int4(0, 0, 0, 0), nrb = nra;
+            double nq0 = 0.0, nq1 = 0.0, nq2 = 0.0, nq10 = 0.0;
+            if (warp < M) {
+                nra = __ldg(reinterpret_cast<const int4 *>(gI + p.i_rrec + warp * QSS_V1_RREC));
+                nrb = __ldg(reinterpret_cast<const int4 *>(gI + p.i_rrec + warp * QSS_V1_RREC + 4));
+                const double *rn = gD + p.d_rate_r + warp * QSS_RD_STRIDE;
+                nq0 = __ldg(rn); nq1 = __ldg(rn + 1); nq2 = __ldg(rn + 2); nq10 = __ldg(rn + 10);
+            }
+#pragma unroll 1
             for (int r = warp; r < M; r += nw) {
-                const int4 ra = __ldg(reinterpret_cast<const int4 *>(gI + p.i_rrec + r * QSS_V1_RREC));
-                const int4 rb = __ldg(reinterpret_cast<const int4 *>(gI + p.i_rrec + r * QSS_V1_RREC + 4));
+                const int4 ra = nra, rb = nrb;
+                const double q0 = nq0, q1 = nq1, q2 = nq2, q10 = nq10;
+                const double *rd = gD + p.d_rate_r + r * QSS_RD_STRIDE;
+                if (r + nw < M) {
+                    nra = __ldg(reinterpret_cast<const int4 *>(gI + p.i_rrec + (r + nw) * QSS_V1_RREC));
+                    nrb = __ldg(reinterpret_cast<const int4 *>(gI + p.i_rrec + (r + nw) * QSS_V1_RREC + 4));
+                    const double *rn = rd + nw * QSS_RD_STRIDE;
+                    nq0 = __ldg(rn); nq1 = __ldg(rn + 1); nq2 = __ldg(rn + 2); nq10 = __ldg(rn + 10);
+                }
                 const int j = ra.x, type = ra.y & 3, mask = (ra.y >> 2) & 3, tb = (ra.y >> 4) - 1;
-                const double *rd = gD + p.d_rate + j * QSS_RD_STRIDE;
-                const double lnkinf = rd[0] + rd[1] * lnT - rd[2] * invT;
-                const double dlnkinf = (rd[1] + rd[2] * invT) * invT;
+                const double lnkinf = q0 + q1 * lnT - q2 * invT;
+                const double dlnkinf = (q1 + q2 * invT) * invT;
                 double k = qss_exp(lnkinf), dlnk = dlnkinf;
                 if (type >= 1) {
                     double Mc = Ctot;                              // M = sum_k alpha_k C_k, transported only (G7)
@@ -133,18 +150,18 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                 if (mask & 2) {                                    // reverse rate from the equilibrium constant (G10)
                     const double dG = (SM(p.s_G, rb.y & 255) + SM(p.s_G, (rb.y >> 8) & 255) + SM(p.s_G, (rb.y >> 16) & 255)) -
                                       (SM(p.s_G, rb.x & 255) + SM(p.s_G, (rb.x >> 8) & 255) + SM(p.s_G, (rb.x >> 16) & 255));
-                    kb = k * qss_exp(dG - rd[10] * lnP0RT);            // k / Kc, ln Kc = -dG + dnu ln(P0/RT)
+                    kb = k * qss_exp(dG - q10 * lnP0RT);            // k / Kc, ln Kc = -dG + dnu ln(P0/RT)
                     if (JAC) {
                         const double dH = (SM(p.s_H, rb.y & 255) + SM(p.s_H, (rb.y >> 8) & 255) + SM(p.s_H, (rb.y >> 16) & 255)) -
                                           (SM(p.s_H, rb.x & 255) + SM(p.s_H, (rb.x >> 8) & 255) + SM(p.s_H, (rb.x >> 16) & 255));
-                        dlnKc = (dH - rd[10]) * invT;
+                        dlnKc = (dH - q10) * invT;
                     }
                 }
                 SC(p.g_K, 2 * j) = kf;
                 SC(p.g_K, 2 * j + 1) = kb;
                 // kappa_d = k_d * product of the TRANSPORTED reactant molecules (QSS and empty slots read the 1.0 row)
-                SC(p.g_KAP, 2 * j) = kf * SM(p.s_V, ra.z & 255) * SM(p.s_V, (ra.z >> 8) & 255) * SM(p.s_V, (ra.z >> 16) & 255);
-                SC(p.g_KAP, 2 * j + 1) = kb * SM(p.s_V, ra.w & 255) * SM(p.s_V, (ra.w >> 8) & 255) * SM(p.s_V, (ra.w >> 16) & 255);
+                SM(p.s_KAP, 2 * j) = kf * SM(p.s_V, ra.z & 255) * SM(p.s_V, (ra.z >> 8) & 255) * SM(p.s_V, (ra.z >> 16) & 255);
+                SM(p.s_KAP, 2 * j + 1) = kb * SM(p.s_V, ra.w & 255) * SM(p.s_V, (ra.w >> 8) & 255) * SM(p.s_V, (ra.w >> 16) & 255);
                 if (JAC) { SC(p.g_DF, j) = dlnk; SC(p.g_DC, j) = dlnKc; }
             }
         }
@@ -152,13 +169,25 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         // ---- P3: closure assembly: every P / leak / p0 slot gathers the kappas feeding it (no atomics)
         for (int e = warp; e < p.n_centry; e += nw) {
             double acc = 0.0;
-            for (int x = HT(p.h_ce_ptr, e); x < HT(p.h_ce_ptr, e + 1); ++x) acc += SC(p.g_KAP, HT(p.h_ce_dir, x));
+            for (int x = HT(p.h_ce_ptr, e); x < HT(p.h_ce_ptr, e + 1); ++x) acc += SM(p.s_KAP, HT(p.h_ce_dir, x));
             SM(p.s_CL, HT(p.h_ce_dst, e)) = acc;
         }
         for (int e = warp; e < p.n_xp; e += nw) {
             double acc = 0.0;
-            for (int x = HT(p.h_xp_ptr, e); x < HT(p.h_xp_ptr, e + 1); ++x) acc += SC(p.g_KAP, HT(p.h_xp_dir, x));
+            for (int x = HT(p.h_xp_ptr, e); x < HT(p.h_xp_ptr, e + 1); ++x) acc += SM(p.s_KAP, HT(p.h_xp_dir, x));
             SM(p.s_XP, e) = acc;
+        }
+        if (JAC) {
+            // ---- P7 (same phase: reads kappa only): W_y[i][q] = d wdot_i / d y_q at fixed x, sums of kappas
+            //      (Eq. 9 second parenthesis, L224); the entries go to the scratch slab, pass B reads each once per round
+            for (int e = warp; e < p.n_wy; e += nw) {
+                double acc = 0.0;
+                for (int x = __ldg(gI + p.i_wya_ptr + e), xe = __ldg(gI + p.i_wya_ptr + e + 1); x < xe; ++x) {
+                    const int w = __ldg(gI + p.i_wya + x);
+                    acc = fma(HD(p.h_nulut, (w >> 12) & 15), SM(p.s_KAP, w & 4095), acc);
+                }
+                SC(p.g_WY, e) = acc;
+            }
         }
         __syncthreads();
         // ---- P4: closure solve, level by level of the condensed DAG; subtraction-free elimination
@@ -204,13 +233,13 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         // ---- P5: net rates of progress Q_j (Eq. 2), dQ/dT at fixed y and M, dQ/dM
         for (int j = warp; j < M; j += nw) {
             const int w = HT(p.h_q, j);
-            const double rf = SC(p.g_KAP, 2 * j) * SM(p.s_V, w & 255);
-            const double rb = SC(p.g_KAP, 2 * j + 1) * SM(p.s_V, (w >> 8) & 255);
+            const double rf = SM(p.s_KAP, 2 * j) * SM(p.s_V, w & 255);
+            const double rb = SM(p.s_KAP, 2 * j + 1) * SM(p.s_V, (w >> 8) & 255);
             const double Q = rf - rb;
-            SM(p.s_Q, j) = Q;
+            SM(p.s_KAP, 2 * j) = Q;                                 // Q_j and dQ_j/dT replace the two kappas in place
             if (JAC) {
                 const double qt = Q * SC(p.g_DF, j) + rb * SC(p.g_DC, j);
-                SM(p.s_QT, j) = qt;
+                SM(p.s_KAP, 2 * j + 1) = qt;
                 const int tb = (w >> 16) - 1;
                 if (tb >= 0) SC(p.g_QM, tb) *= Q;
             }
@@ -223,9 +252,9 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             for (int x = HT(p.h_ss_ptr, s); x < HT(p.h_ss_ptr, s + 1); ++x) {
                 const int e = HT(p.h_ss, x), j = e & 4095;
                 const double nu = HD(p.h_nulut, (e >> 12) & 15);
-                w = fma(nu, SM(p.s_Q, j), w);
+                w = fma(nu, SM(p.s_KAP, 2 * j), w);
                 if (JAC) {
-                    et = fma(nu, SM(p.s_QT, j), et);
+                    et = fma(nu, SM(p.s_KAP, 2 * j + 1), et);
                     const int tb = (e >> 16) - 1;
                     if (tb >= 0) tv = fma(nu, SC(p.g_QM, tb), tv);
                 }
@@ -236,16 +265,6 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         if (p.cqss && active)
             for (int q = warp; q < Nq; q += nw) p.cqss[(size_t)q * ld + cell] = SM(p.s_V, N + 1 + q);
         if (JAC) {
-            __syncthreads();
-            // ---- P7: W_y[i][q] = d wdot_i / d y_q at fixed x: sums of kappas (Eq. 9 second parenthesis, L224)
-            for (int e = warp; e < p.n_wy; e += nw) {
-                double acc = 0.0;
-                for (int x = __ldg(gI + p.i_wya_ptr + e), xe = __ldg(gI + p.i_wya_ptr + e + 1); x < xe; ++x) {
-                    const int w = __ldg(gI + p.i_wya + x);
-                    acc = fma(HD(p.h_nulut, (w >> 12) & 15), SC(p.g_KAP, w & 4095), acc);
-                }
-                SC(p.g_WY, e) = acc;
-            }
             __syncthreads();
             // ---- P8: Jacobian sweep in rounds of nw columns (Eq. 7, Eq. 9)
             const unsigned ycw = sml + (p.s_YC + warp) * 256;        // this warp's dy/dx column: row q at + q * nw * 256
@@ -317,7 +336,8 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                 }
                 __syncthreads();
                 // -- pass B: warp = row i.  J[i, round] = W_x[i, round] + sum_q W_y[i][q] * dy_q/dx[round]
-                for (int i = warp; i < N; i += nw) {
+                for (int u = HT(p.h_rw_ptr, warp); u < HT(p.h_rw_ptr, warp + 1); ++u) {
+                    const int i = HT(p.h_rw, u);
                     double acc[QSS_V1_NW];
                     const unsigned wx = sml + (p.s_WX + i * nw) * 256;
 #pragma unroll

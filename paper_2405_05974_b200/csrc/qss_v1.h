@@ -27,7 +27,7 @@ struct QssV1 {
     // ---- global tables (the QssTab blobs)
     const int32_t *gI;
     const double *gD;
-    int32_t d_thermo, d_rate, d_effm1, i_eff_ptr, i_eff_sp, i_rrec;
+    int32_t d_thermo, d_rate_r, d_effm1, i_eff_ptr, i_eff_sp, i_rrec;   // d_rate_r: rate records in processing order
     int32_t i_wya_ptr, i_wya;                        // W_y assembly lists: dir | nucode<<12 (global, read once per slab)
     // ---- sizes
     int32_t N, Nq, M, nsp, n_tb, nw, n_groups, n_levels, n_centry, n_xp, n_wy, n_rounds, n_sp_ops;
@@ -39,11 +39,11 @@ struct QssV1 {
     int32_t s_TV;       // [nsp]     third-body vector  sum_j nu_sj dQ_j/dM
     int32_t s_YC;       // [Nq*nw]   dy/dx of the round's columns, row q*nw + w   } region R, time-shared with
     int32_t s_WX;       // [N*nw]    W_x of the round's columns, row i*nw + w     }   s_G, s_H (thermo, rate phases)
-    int32_t s_G, s_H;   // [nsp+1]   g/RT, h/RT (+ a zero row)                    }   s_Q, s_QT (net rates phase)
-    int32_t s_Q, s_QT;  // [M]       Q_j, dQ_j/dT at fixed y, M
+    int32_t s_KAP;      // [2M]      kappa_d; then in place Q_j (row 2j), dQ_j/dT (row 2j+1) }   (phases P2-P6)
+    int32_t s_G, s_H;   // [nsp+1]   g/RT, h/RT (+ a zero row), after s_KAP                  }   (phases P1-P2)
     int32_t smem_rows;
     // ---- scratch rows
-    int32_t g_K, g_KAP; // [2M]      k_d, kappa_d
+    int32_t g_K;        // [2M]      k_d
     int32_t g_DF, g_DC; // [M]       dlnk/dT, dlnKc/dT
     int32_t g_ET;       // [nsp]     T-column vector sum_j nu_sj dQ_j/dT
     int32_t g_QM;       // [n_tb]    d ln k / dM, then dQ/dM
@@ -60,6 +60,7 @@ struct QssV1 {
     int32_t h_cs_ptr, h_cs;                          // column streams (see qss_compile.cpp "column stream")
     int32_t h_sp;                                    // dy/dx solve program (row operations)
     int32_t h_wr_ptr, h_wr;                          // W_y rows: byte offset q*nw*256 of each entry's dy/dx row
+    int32_t h_rw_ptr, h_rw;                          // Jacobian rows of pass B assigned to each warp (balanced)
     int32_t h_nulut;                                 // 16 doubles: nucode -> nu (nucode = nu + 8)
     int32_t h_used;
     alignas(8) int32_t h[QSS_V1_HMAX];
