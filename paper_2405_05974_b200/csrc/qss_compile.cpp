@@ -157,14 +157,24 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     }
     const int nw = QSS_V1_NW;
     if (N + 1 > QSS_V1_NT) { why = "more Jacobian columns than the register tile of variant 1 holds"; return false; }
-    // species incidence lists (their balanced assignment to warps follows below)
-    std::vector<std::vector<int32_t>> ss(nsp);
-    for (int j = 0; j < M; ++j) if (R[j].mask) for (const Term &x : R[j].net) ss[x.sp].push_back(j | (nucode(x.nu) << 12) | ((R[j].tb + 1) << 16));
+    // species incidence lists (their balanced assignment to warps follows below): one entry per unit of |nu|,
+    //   h_ss: byte offset of Q_j (row 2j of s_KAP, dQ_j/dT follows at +256) | sign bit;  h_st: scratch row of dQ_j/dM | sign bit
+    std::vector<std::vector<int32_t>> ss(nsp), st(nsp);
+    for (int j = 0; j < M; ++j) if (R[j].mask) for (const Term &x : R[j].net) for (int u = 0; u < std::abs(x.nu); ++u) {
+        const int32_t sgn = x.nu < 0 ? (int32_t)0x80000000 : 0;
+        ss[x.sp].push_back((j * 512) | sgn);
+        if (R[j].tb >= 0) st[x.sp].push_back(R[j].tb | sgn);
+    }
     {
-        std::vector<int32_t> ptr{0}, all;
-        for (int s = 0; s < nsp; ++s) { all.insert(all.end(), ss[s].begin(), ss[s].end()); ptr.push_back((int32_t)all.size()); }
+        std::vector<int32_t> ptr{0}, all, tptr{0}, tall;
+        for (int s = 0; s < nsp; ++s) {
+            all.insert(all.end(), ss[s].begin(), ss[s].end()); ptr.push_back((int32_t)all.size());
+            tall.insert(tall.end(), st[s].begin(), st[s].end()); tptr.push_back((int32_t)tall.size());
+        }
         v.h_ss_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
         v.h_ss = at(); H.insert(H.end(), all.begin(), all.end());
+        v.h_st_ptr = at(); H.insert(H.end(), tptr.begin(), tptr.end());
+        v.h_st = at(); H.insert(H.end(), tall.begin(), tall.end());
     }
     // W_y entries, row-major (i, then q): gather lists over the directions consuming q (lists go to the global blob)
     std::map<std::pair<int, int>, std::vector<int32_t>> wy;
@@ -207,14 +217,14 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     }
     // ---- column stream: everything that is scattered into column k of [W_x; G_x], as records
     //   w0 = scratch row of A | n_entries << 16 | has_val << 20      part = A * V[o1] * V[o2] (* val)
-    //   w1 = byte offset of V row o1 | byte offset of V row o2 << 16
+    //   w1 = byte offset of V row o1 | byte offset of V row o2 << 16        (has_val: index of val in the double blob)
     //   w2, w3 = up to 8 scatter indices (bytes): 2 * register row + (1 if the term is subtracted); QSS_V1_NULL = none
-    //   [w4, w5 = val (double)]                                       only when has_val
     // One record per (enabled direction, molecule slot holding species k): A = k_d, o1/o2 = the other two slots
     // (Eq. 9 first parenthesis); one per non-unity third-body efficiency: A = dQ_j/dM, val = alpha_jk - 1.
     auto regrow = [&](int sp) { return sp < N ? sp : QSS_V1_NT + (sp - N); };
     auto voff = [&](int vr) { return (v.s_V + vr) * 256; };
     std::vector<std::vector<int32_t>> cs(N);
+    std::vector<double> effv;                              // (alpha - 1) values, read from the double blob
     bool cs_ok = true;
     auto push_record = [&](int k, int rowA, int o1, int o2, const std::vector<Term> &net, int sgn, bool has_val, double val) {
         std::vector<int> idx;
@@ -224,9 +234,9 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         uint32_t w[2] = {none, none};
         for (size_t u = 0; u < idx.size(); ++u) { w[u / 4] &= ~(0xFFu << (8 * (u % 4))); w[u / 4] |= (uint32_t)idx[u] << (8 * (u % 4)); }
         cs[k].push_back(rowA | ((int)idx.size() << 16) | ((has_val ? 1 : 0) << 20));
-        cs[k].push_back(o1 | (o2 << 16));
+        if (has_val) { cs[k].push_back((int32_t)effv.size()); effv.push_back(val); }
+        else cs[k].push_back(o1 | (o2 << 16));
         cs[k].push_back((int32_t)w[0]); cs[k].push_back((int32_t)w[1]);
-        if (has_val) { int32_t d2[2]; std::memcpy(d2, &val, 8); cs[k].push_back(d2[0]); cs[k].push_back(d2[1]); }
     };
     for (int j = 0; j < M; ++j) for (int dir = 0; dir < 2; ++dir) {
         if (!((R[j].mask >> dir) & 1)) continue;
@@ -334,18 +344,26 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         v.i_rrec = (int32_t)I.size();
         for (int r = 0; r < M; ++r) {
             const int j = (*c.rorder)[r];
-            int32_t rec[QSS_V1_RREC] = {j, R[j].type | (R[j].mask << 2) | ((R[j].tb + 1) << 4), 0, 0, 0, 0, 0, 0};
+            // w0 = j | type << 12 | mask << 14 | (tb + 1) << 16; w1..w3 = six 16-bit byte offsets of the V rows of the
+            // reactant / product molecules (QSS and empty slots -> the 1.0 row); w4..w6 = six byte offsets (relative to
+            // s_G) of their g/RT rows (empty slots -> the zero row)
+            int32_t rec[QSS_V1_RREC] = {j | (R[j].type << 12) | (R[j].mask << 14) | ((R[j].tb + 1) << 16), 0, 0, 0, 0, 0, 0, 0};
+            uint32_t kap[6], gr[6];
             for (int s = 0; s < 2; ++s) {
-                int kap[3] = {N, N, N}, gr[3] = {nsp, nsp, nsp}, n = 0;
-                for (const Term &x : R[j].side[s]) for (int u = 0; u < x.nu; ++u) { kap[n] = x.sp < N ? x.sp : N; gr[n] = x.sp; ++n; }
-                rec[2 + s] = kap[0] | (kap[1] << 8) | (kap[2] << 16);
-                rec[4 + s] = gr[0] | (gr[1] << 8) | (gr[2] << 16);
+                int n = 0;
+                for (int u = 0; u < 3; ++u) { kap[3 * s + u] = (uint32_t)(v.s_V + N) * 256u; gr[3 * s + u] = (uint32_t)nsp * 256u; }
+                for (const Term &x : R[j].side[s]) for (int u = 0; u < x.nu; ++u) {
+                    kap[3 * s + n] = (uint32_t)(v.s_V + (x.sp < N ? x.sp : N)) * 256u; gr[3 * s + n] = (uint32_t)x.sp * 256u; ++n;
+                }
             }
+            for (int u = 0; u < 3; ++u) { rec[1 + u] = (int32_t)(kap[2 * u] | (kap[2 * u + 1] << 16)); rec[4 + u] = (int32_t)(gr[2 * u] | (gr[2 * u + 1] << 16)); }
             I.insert(I.end(), rec, rec + QSS_V1_RREC);
         }
     }
     v.N = N; v.Nq = Nq; v.M = M; v.nsp = nsp; v.n_tb = c.n_tb; v.n_groups = c.n_groups; v.n_levels = c.n_levels;
     v.d_thermo = out.tab.d_thermo; v.d_effm1 = out.tab.d_effm1;
+    v.d_effv = (int32_t)out.D.size();
+    out.D.insert(out.D.end(), effv.begin(), effv.end());
     {   // rate records again, in processing order (so that a warp can prefetch the next one without knowing j)
         std::vector<double> &Dd = out.D;
         v.d_rate_r = (int32_t)Dd.size();

@@ -84,6 +84,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         // ---- P2: rate constants, direction coefficients kappa_d (Eq. 2, Eq. 6)
         {
             const double Ctot = SM(p.s_CT, 0);
+            const unsigned gbase = sml + p.s_G * 256, hbase = sml + p.s_H * 256, kbase = sml + p.s_KAP * 256;
             // records and Arrhenius parameters are stored in processing order; those of the warp's NEXT reaction are
             // fetched (L2 reads, the L1 is a few KB next to the shared memory) before the current one is evaluated
             int4 nra = make_int4(0, 0, 0, 0), nrb = nra;
@@ -105,7 +106,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                     const double *rn = rd + nw * QSS_RD_STRIDE;
                     nq0 = __ldg(rn); nq1 = __ldg(rn + 1); nq2 = __ldg(rn + 2); nq10 = __ldg(rn + 10);
                 }
-                const int j = ra.x, type = ra.y & 3, mask = (ra.y >> 2) & 3, tb = (ra.y >> 4) - 1;
+                const int j = ra.x & 4095, type = (ra.x >> 12) & 3, mask = (ra.x >> 14) & 3, tb = (ra.x >> 16) - 1;
                 const double lnkinf = q0 + q1 * lnT - q2 * invT;
                 const double dlnkinf = (q1 + q2 * invT) * invT;
                 double k = qss_exp(lnkinf), dlnk = dlnkinf;
@@ -148,20 +149,20 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                 }
                 double kf = (mask & 1) ? k : 0.0, kb = 0.0, dlnKc = 0.0;
                 if (mask & 2) {                                    // reverse rate from the equilibrium constant (G10)
-                    const double dG = (SM(p.s_G, rb.y & 255) + SM(p.s_G, (rb.y >> 8) & 255) + SM(p.s_G, (rb.y >> 16) & 255)) -
-                                      (SM(p.s_G, rb.x & 255) + SM(p.s_G, (rb.x >> 8) & 255) + SM(p.s_G, (rb.x >> 16) & 255));
-                    kb = k * qss_exp(dG - q10 * lnP0RT);            // k / Kc, ln Kc = -dG + dnu ln(P0/RT)
+                    const unsigned g0 = rb.x & 0xffff, g1 = (unsigned)rb.x >> 16, g2 = rb.y & 0xffff;      // reactant molecules
+                    const unsigned g3 = (unsigned)rb.y >> 16, g4 = rb.z & 0xffff, g5 = (unsigned)rb.z >> 16;  // product molecules
+                    const double dG = (lds(gbase + g3) + lds(gbase + g4) + lds(gbase + g5)) - (lds(gbase + g0) + lds(gbase + g1) + lds(gbase + g2));
+                    kb = k * qss_exp(dG - q10 * lnP0RT);           // k / Kc, ln Kc = -dG + dnu ln(P0/RT)
                     if (JAC) {
-                        const double dH = (SM(p.s_H, rb.y & 255) + SM(p.s_H, (rb.y >> 8) & 255) + SM(p.s_H, (rb.y >> 16) & 255)) -
-                                          (SM(p.s_H, rb.x & 255) + SM(p.s_H, (rb.x >> 8) & 255) + SM(p.s_H, (rb.x >> 16) & 255));
+                        const double dH = (lds(hbase + g3) + lds(hbase + g4) + lds(hbase + g5)) - (lds(hbase + g0) + lds(hbase + g1) + lds(hbase + g2));
                         dlnKc = (dH - q10) * invT;
                     }
                 }
                 SC(p.g_K, 2 * j) = kf;
                 SC(p.g_K, 2 * j + 1) = kb;
                 // kappa_d = k_d * product of the TRANSPORTED reactant molecules (QSS and empty slots read the 1.0 row)
-                SM(p.s_KAP, 2 * j) = kf * SM(p.s_V, ra.z & 255) * SM(p.s_V, (ra.z >> 8) & 255) * SM(p.s_V, (ra.z >> 16) & 255);
-                SM(p.s_KAP, 2 * j + 1) = kb * SM(p.s_V, ra.w & 255) * SM(p.s_V, (ra.w >> 8) & 255) * SM(p.s_V, (ra.w >> 16) & 255);
+                sts(kbase + j * 512, kf * lds(sml + (ra.y & 0xffff)) * lds(sml + ((unsigned)ra.y >> 16)) * lds(sml + (ra.z & 0xffff)));
+                sts(kbase + j * 512 + 256, kb * lds(sml + ((unsigned)ra.z >> 16)) * lds(sml + (ra.w & 0xffff)) * lds(sml + ((unsigned)ra.w >> 16)));
                 if (JAC) { SC(p.g_DF, j) = dlnk; SC(p.g_DC, j) = dlnKc; }
             }
         }
@@ -245,22 +246,35 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             }
         }
         __syncthreads();
-        // ---- P6: species sums: wdot (Eq. 3); for the Jacobian the T-column vector and the third-body vector
-        for (int u = HT(p.h_ssw_ptr, warp); u < HT(p.h_ssw_ptr, warp + 1); ++u) {
-            const int s = HT(p.h_ssw, u);
-            double w = 0.0, et = 0.0, tv = 0.0;
-            for (int x = HT(p.h_ss_ptr, s); x < HT(p.h_ss_ptr, s + 1); ++x) {
-                const int e = HT(p.h_ss, x), j = e & 4095;
-                const double nu = HD(p.h_nulut, (e >> 12) & 15);
-                w = fma(nu, SM(p.s_KAP, 2 * j), w);
-                if (JAC) {
-                    et = fma(nu, SM(p.s_KAP, 2 * j + 1), et);
-                    const int tb = (e >> 16) - 1;
-                    if (tb >= 0) tv = fma(nu, SC(p.g_QM, tb), tv);
+        // ---- P6: species sums: wdot (Eq. 3); for the Jacobian the T-column vector and the third-body vector.
+        //      One table entry per unit of |nu|: the sign bit of the entry flips the sign bit of the value.
+        {
+            const unsigned kbase = sml + p.s_KAP * 256;
+            for (int u = HT(p.h_ssw_ptr, warp); u < HT(p.h_ssw_ptr, warp + 1); ++u) {
+                const int s = HT(p.h_ssw, u);
+                double w = 0.0, et = 0.0, tv = 0.0;
+                const int xe = HT(p.h_ss_ptr, s + 1);
+                for (int x = HT(p.h_ss_ptr, s); x < xe; ++x) {
+                    const int e = HT(p.h_ss, x), sg = e & 0x80000000;
+                    const unsigned a = kbase + (e & 0x7fffffff);
+                    const double q = lds(a);
+                    w += __hiloint2double(__double2hiint(q) ^ sg, __double2loint(q));
+                    if (JAC) {
+                        const double qt = lds(a + 256);
+                        et += __hiloint2double(__double2hiint(qt) ^ sg, __double2loint(qt));
+                    }
                 }
+                if (JAC) {
+                    const int te = HT(p.h_st_ptr, s + 1);
+                    for (int x = HT(p.h_st_ptr, s); x < te; ++x) {
+                        const int e = HT(p.h_st, x), sg = e & 0x80000000;
+                        const double qm = SC(p.g_QM, e & 0x7fffffff);
+                        tv += __hiloint2double(__double2hiint(qm) ^ sg, __double2loint(qm));
+                    }
+                }
+                if (s < N && p.wdot && active) p.wdot[(size_t)s * ld + cell] = w;
+                if (JAC) { SM(p.s_TV, s) = tv; SC(p.g_ET, s) = et; }
             }
-            if (s < N && p.wdot && active) p.wdot[(size_t)s * ld + cell] = w;
-            if (JAC) { SM(p.s_TV, s) = tv; SC(p.g_ET, s) = et; }
         }
         if (p.cqss && active)
             for (int q = warp; q < Nq; q += nw) p.cqss[(size_t)q * ld + cell] = SM(p.s_V, N + 1 + q);
@@ -289,17 +303,22 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                     int x = p.h_cs + HT(p.h_cs_ptr, k);
                     const int xe = p.h_cs + HT(p.h_cs_ptr, k + 1);
                     int2 na = make_int2(0, 0), nb = make_int2(0, 0);
-                    double nA = 0.0;
-                    if (x < xe) { na = ldc2(&p.h[x]); nb = ldc2(&p.h[x + 2]); nA = sc[(size_t)(na.x & 0xffff) * 32]; }
+                    double nA = 0.0, nV = 0.0;
+                    if (x < xe) {
+                        na = ldc2(&p.h[x]); nb = ldc2(&p.h[x + 2]); nA = sc[(size_t)(na.x & 0xffff) * 32];
+                        if (na.x & (1 << 20)) nV = __ldg(gD + p.d_effv + na.y);
+                    }
 #pragma unroll 1
                     while (x < xe) {
                         const int2 a = na, b = nb;
-                        double part = nA;
                         const bool has_val = (a.x & (1 << 20)) != 0;
-                        if (has_val) part *= *reinterpret_cast<const double *>(&p.h[x + 4]);
-                        x += has_val ? 6 : 4;
-                        if (x < xe) { na = ldc2(&p.h[x]); nb = ldc2(&p.h[x + 2]); nA = sc[(size_t)(na.x & 0xffff) * 32]; }
-                        part *= lds(sml + (a.y & 0xffff)) * lds(sml + ((unsigned)a.y >> 16));
+                        double part = has_val ? nA * nV : nA;
+                        x += 4;
+                        if (x < xe) {
+                            na = ldc2(&p.h[x]); nb = ldc2(&p.h[x + 2]); nA = sc[(size_t)(na.x & 0xffff) * 32];
+                            if (na.x & (1 << 20)) nV = __ldg(gD + p.d_effv + na.y);
+                        }
+                        if (!has_val) part *= lds(sml + (a.y & 0xffff)) * lds(sml + ((unsigned)a.y >> 16));
                         unsigned w = (unsigned)b.x;
                         QSS_SCAT(w & 255, part); QSS_SCAT((w >> 8) & 255, part);
                         QSS_SCAT((w >> 16) & 255, part); QSS_SCAT(w >> 24, part);

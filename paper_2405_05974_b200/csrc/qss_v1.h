@@ -28,6 +28,7 @@ struct QssV1 {
     const int32_t *gI;
     const double *gD;
     int32_t d_thermo, d_rate_r, d_effm1, i_eff_ptr, i_eff_sp, i_rrec;   // d_rate_r: rate records in processing order
+    int32_t d_effv;                                  // (alpha - 1) values of the column streams
     int32_t i_wya_ptr, i_wya;                        // W_y assembly lists: dir | nucode<<12 (global, read once per slab)
     // ---- sizes
     int32_t N, Nq, M, nsp, n_tb, nw, n_groups, n_levels, n_centry, n_xp, n_wy, n_rounds, n_sp_ops;
@@ -55,7 +56,8 @@ struct QssV1 {
     int32_t h_group, h_gmember, h_level_ptr;         // group records (8 words), members, levels
     int32_t h_q;                                     // [M] qf | qb<<8 | (tb+1)<<16  (V rows of the QSS reactants)
     int32_t h_ssw_ptr, h_ssw;                        // species assigned to each warp (balanced)
-    int32_t h_ss_ptr, h_ss;                          // species incidence: j | nucode<<12 | (tb+1)<<16
+    int32_t h_ss_ptr, h_ss;                          // species incidence: byte offset of Q_j in s_KAP | sign bit
+    int32_t h_st_ptr, h_st;                          // third-body incidence: index of dQ_j/dM | sign bit
     int32_t h_cw;                                    // [n_rounds*nw] Jacobian column of (round, warp), -1: none
     int32_t h_cs_ptr, h_cs;                          // column streams (see qss_compile.cpp "column stream")
     int32_t h_sp;                                    // dy/dx solve program (row operations)
