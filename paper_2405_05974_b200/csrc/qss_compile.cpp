@@ -100,7 +100,7 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     const std::vector<Reaction> &R = *c.R;
     QssV1 &v = out.v1;
     v = QssV1();
-    if (N > QSS_V1_NT || Nq > QSS_V1_NQ) { why = "more species than the register column of variant 1 holds"; return false; }
+    if (nsp > 126) { why = "more species than the one-byte row index of the column stream holds"; return false; }
     if (2 * M > 4096 || c.n_tb + 1 >= 4096) { why = "too many reactions for the packed tables of variant 1"; return false; }
     for (int j = 0; j < M; ++j) {
         for (int s = 0; s < 2; ++s) { int n = 0; for (const Term &x : R[j].side[s]) n += x.nu; if (n > 3) { why = "a reaction side has more than 3 molecules"; return false; } }
@@ -156,7 +156,6 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         }
     }
     const int nw = QSS_V1_NW;
-    if (N + 1 > QSS_V1_NT) { why = "more Jacobian columns than the register tile of variant 1 holds"; return false; }
     // species incidence lists (their balanced assignment to warps follows below): one entry per unit of |nu|,
     //   h_ss: byte offset of Q_j (row 2j of s_KAP, dQ_j/dT follows at +256) | sign bit;  h_st: scratch row of dQ_j/dM | sign bit
     std::vector<std::vector<int32_t>> ss(nsp), st(nsp);
@@ -201,11 +200,10 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     auto take = [&](int n) { int r = rows_fixed; rows_fixed += n; return r; };
     v.s_V = take(N + 1 + Nq); v.s_CT = take(1); v.s_CL = take(c.cl_size); v.s_XP = take(v.n_xp); v.s_TV = take(nsp);
     const int max_rows = (227 * 1024) / 256;
-    const int region = std::max((Nq + N) * nw, 2 * M + 2 * (nsp + 1));
+    const int region = std::max((nsp + 1) * nw, 2 * M + 2 * (nsp + 1));    // round buffers: nsp rows + 1 junk row per column
     if (rows_fixed + region > max_rows) { why = "per-cell state does not fit the shared memory of one SM"; return false; }
-    if ((v.s_XP + v.n_xp) * 256 > 65535 || Nq * nw * 256 > 65535) { why = "closure storage beyond the 16-bit offsets of variant 1"; return false; }
     v.nw = nw;
-    v.s_YC = rows_fixed; v.s_WX = rows_fixed + Nq * nw;
+    v.s_WX = rows_fixed; v.s_YC = rows_fixed + N * nw;       // one column buffer: row (species) r of column w at r * nw + w
     v.s_KAP = rows_fixed; v.s_G = rows_fixed + 2 * M; v.s_H = v.s_G + nsp + 1;
     v.smem_rows = rows_fixed + region;
     {
@@ -216,27 +214,29 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         if (o > 65535) { why = "scratch rows beyond the 16-bit offsets of variant 1"; return false; }
     }
     // ---- column stream: everything that is scattered into column k of [W_x; G_x], as records
-    //   w0 = scratch row of A | n_entries << 16 | has_val << 20      part = A * V[o1] * V[o2] (* val)
+    //   w0 = scratch row of A | n_entries << 16 | has_val << 20 | |nu| << 21      part = |nu| * A * V[o1] * V[o2] (* val)
     //   w1 = byte offset of V row o1 | byte offset of V row o2 << 16        (has_val: index of val in the double blob)
-    //   w2, w3 = up to 8 scatter indices (bytes): 2 * register row + (1 if the term is subtracted); QSS_V1_NULL = none
+    //   w2, w3 = up to 8 targets (bytes): species row of the column buffer | 0x80 if the term is subtracted; nsp = none (junk row)
     // One record per (enabled direction, molecule slot holding species k): A = k_d, o1/o2 = the other two slots
     // (Eq. 9 first parenthesis); one per non-unity third-body efficiency: A = dQ_j/dM, val = alpha_jk - 1.
-    auto regrow = [&](int sp) { return sp < N ? sp : QSS_V1_NT + (sp - N); };
     auto voff = [&](int vr) { return (v.s_V + vr) * 256; };
     std::vector<std::vector<int32_t>> cs(N);
     std::vector<double> effv;                              // (alpha - 1) values, read from the double blob
     bool cs_ok = true;
     auto push_record = [&](int k, int rowA, int o1, int o2, const std::vector<Term> &net, int sgn, bool has_val, double val) {
-        std::vector<int> idx;
-        for (const Term &x : net) { const int e = sgn * x.nu; for (int u = 0; u < std::abs(e); ++u) idx.push_back(2 * regrow(x.sp) + (e < 0 ? 1 : 0)); }
-        if (idx.size() > 8) { cs_ok = false; return; }
-        const uint32_t none = QSS_V1_NULL * 0x01010101u;
-        uint32_t w[2] = {none, none};
-        for (size_t u = 0; u < idx.size(); ++u) { w[u / 4] &= ~(0xFFu << (8 * (u % 4))); w[u / 4] |= (uint32_t)idx[u] << (8 * (u % 4)); }
-        cs[k].push_back(rowA | ((int)idx.size() << 16) | ((has_val ? 1 : 0) << 20));
-        if (has_val) { cs[k].push_back((int32_t)effv.size()); effv.push_back(val); }
-        else cs[k].push_back(o1 | (o2 << 16));
-        cs[k].push_back((int32_t)w[0]); cs[k].push_back((int32_t)w[1]);
+        for (int mag = 1; mag <= 7; ++mag) {                 // one record per magnitude |nu| (almost always only 1)
+            std::vector<int> idx;
+            for (const Term &x : net) if (std::abs(x.nu) == mag) idx.push_back(x.sp | (sgn * x.nu < 0 ? 0x80 : 0));
+            if (idx.empty()) continue;
+            if (idx.size() > 8) { cs_ok = false; return; }
+            const uint32_t none = (uint32_t)nsp * 0x01010101u;   // the junk row of the column buffer
+            uint32_t w[2] = {none, none};
+            for (size_t u = 0; u < idx.size(); ++u) { w[u / 4] &= ~(0xFFu << (8 * (u % 4))); w[u / 4] |= (uint32_t)idx[u] << (8 * (u % 4)); }
+            cs[k].push_back(rowA | ((int)idx.size() << 16) | ((has_val ? 1 : 0) << 20) | (mag << 21));
+            if (has_val) { cs[k].push_back((int32_t)effv.size()); effv.push_back(val); }
+            else cs[k].push_back(o1 | (o2 << 16));
+            cs[k].push_back((int32_t)w[0]); cs[k].push_back((int32_t)w[1]);
+        }
     };
     for (int j = 0; j < M; ++j) for (int dir = 0; dir < 2; ++dir) {
         if (!((R[j].mask >> dir) & 1)) continue;
@@ -263,26 +263,27 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     }
     // ---- dy/dx solve program: row operations y[a] = (y[a] + sum_t F_t * y[b_t]) [* ID] on the warp's dy/dx column,
     //      in the order cross-group terms, back-elimination (with U[m][k] = P[m][k] / D_k), forward substitution
-    //   header = a_off | n_terms << 16 | has_scale << 24 ; [id_off] ; n_terms x (f_off | b_off << 16)
+    //   header = a_row | n_terms << 16 | has_scale << 24 ; [id_row] ; n_terms x (f_row | b_row << 16)
+    //   a_row, b_row: rows relative to the warp's dy/dx column; f_row, id_row: absolute shared-memory rows
     {
         std::vector<int32_t> sp;
         int nops = 0;
-        auto yoff = [&](int q) { return q * nw * 256; };
+        auto yoff = [&](int q) { return q * nw; };              // rows; the kernel scales by 256
         for (int g = 0; g < c.n_groups; ++g) {
             const std::vector<int> &mem = (*c.members)[g];
             const int sz = (int)mem.size(), base = v.s_CL + (*c.gbase)[g];
             for (int x = (*c.xp_begin)[g]; x < (*c.xp_end)[g]; ++x) {
                 const auto &e = (*c.xpl)[x];
-                sp.push_back(yoff(e.first.first) | (1 << 16)); sp.push_back(((v.s_XP + x) * 256) | (yoff(e.first.second) << 16)); ++nops;
+                sp.push_back(yoff(e.first.first) | (1 << 16)); sp.push_back((v.s_XP + x) | (yoff(e.first.second) << 16)); ++nops;
             }
             for (int m = sz - 2; m >= 0; --m) {
                 sp.push_back(yoff(mem[m]) | ((sz - 1 - m) << 16)); ++nops;
-                for (int k = m + 1; k < sz; ++k) sp.push_back(((base + m * sz + k) * 256) | (yoff(mem[k]) << 16));
+                for (int k = m + 1; k < sz; ++k) sp.push_back((base + m * sz + k) | (yoff(mem[k]) << 16));
             }
             for (int k = 0; k < sz; ++k) {
                 sp.push_back(yoff(mem[k]) | (k << 16) | (1 << 24)); ++nops;
-                sp.push_back((base + sz * sz + 2 * sz + k) * 256);
-                for (int jj = 0; jj < k; ++jj) sp.push_back(((base + k * sz + jj) * 256) | (yoff(mem[jj]) << 16));
+                sp.push_back(base + sz * sz + 2 * sz + k);
+                for (int jj = 0; jj < k; ++jj) sp.push_back((base + k * sz + jj) | (yoff(mem[jj]) << 16));
             }
         }
         v.n_sp_ops = nops;

@@ -8,19 +8,18 @@
 //   - every per-cell array access is one conflict-free 256-byte row, in shared memory for the hot state
 //     (concentrations, closure factors, W_y, third-body vectors, dy/dx column) and in an L2-resident scratch slab
 //     for the write-once / read-once per-direction arrays (k_d, kappa_d, dlnk/dT);
-//   - the Jacobian is swept in rounds of 12 columns.  Pass A: each warp accumulates ONE column of [W_x; G_x] in
-//     REGISTERS (the temporaries that replace the paper's CSE scalars): partial derivatives are
-//     scattered into it through an indexed branch (qss_v1_scatter.h), then the dy/dx_k solve runs on the warp's
-//     shared-memory vector.  Pass B: the warps switch to ROWS and add W_y * dy/dx for all 12 columns of the round
-//     from a register tile (one W_y load and one table word per 12 FMAs); every entry leaves as one coalesced
-//     256-byte streaming store.
+//   - the Jacobian is swept in rounds of 12 columns.  Pass A: each warp accumulates ONE column of [W_x; G_x] (the
+//     temporaries that replace the paper's CSE scalars) in its own shared-memory column buffer: a
+//     packed column stream is interpreted, the (distinct) rows of a record are loaded together, updated and stored
+//     back, so no dependent chain builds up; then the dy/dx_k solve program runs in place on the QSS rows.  Pass B:
+//     the warps switch to ROWS and add W_y * dy/dx for all 12 columns of the round from a register tile (one W_y
+//     load and one table word per 12 FMAs); every entry leaves as one coalesced 256-byte streaming store.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 #include "qss_tables.h"
 #include "qss_math.h"
 #include "qss_v1.h"
-#include "qss_v1_scatter.h"
 
 namespace {
 
@@ -281,25 +280,23 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         if (JAC) {
             __syncthreads();
             // ---- P8: Jacobian sweep in rounds of nw columns (Eq. 7, Eq. 9)
-            const unsigned ycw = sml + (p.s_YC + warp) * 256;        // this warp's dy/dx column: row q at + q * nw * 256
+            constexpr unsigned RS = QSS_V1_NW * 256;                 // byte stride between rows of a column buffer
+            const unsigned colw = sml + (p.s_WX + warp) * 256;       // this warp's column of [W_x; G_x]: species row r at + r * RS
+            const unsigned ycw = colw + N * RS;                      //   its QSS part, solved in place into dy/dx_k
             for (int r = 0; r < p.n_rounds; ++r) {
-                // -- pass A: warp = column k.  [W_x; G_x][:,k] in registers, then (diag D - P) dy/dx_k = G_x[:,k]
+                // -- pass A: warp = column k.  [W_x; G_x][:,k] in shared memory, then (diag D - P) dy/dx_k = G_x[:,k]
                 const int k = HT(p.h_cw, r * nw + warp);
                 if (k >= 0) {
-                    double ct[QSS_V1_NT], cq[QSS_V1_NQ];
                     if (k < N) {                                      // rank-1 third-body term (every species column)
-#pragma unroll
-                        for (int s = 0; s < QSS_V1_NT; ++s) ct[s] = s < N ? SM(p.s_TV, s) : 0.0;
-#pragma unroll
-                        for (int q = 0; q < QSS_V1_NQ; ++q) cq[q] = q < Nq ? SM(p.s_TV, N + q) : 0.0;
+#pragma unroll 4
+                        for (int s = 0; s < nsp; ++s) sts(colw + s * RS, SM(p.s_TV, s));
                     } else {                                          // T column
-#pragma unroll
-                        for (int s = 0; s < QSS_V1_NT; ++s) ct[s] = s < N ? SC(p.g_ET, s) : 0.0;
-#pragma unroll
-                        for (int q = 0; q < QSS_V1_NQ; ++q) cq[q] = q < Nq ? SC(p.g_ET, N + q) : 0.0;
+#pragma unroll 4
+                        for (int s = 0; s < nsp; ++s) sts(colw + s * RS, SC(p.g_ET, s));
                     }
-                    // column stream: part = A * V[o1] * V[o2] (* val), added to / subtracted from up to 8 register rows.
-                    // The next record and its A (an L2 read) are fetched before the current one is scattered.
+                    // column stream: part = |nu| * A * V[o1] * V[o2] (* val), added to / subtracted from up to 8 rows of the
+                    // column.  The rows of a record are distinct, so its loads are issued together (no dependent chain);
+                    // the next record and its A (an L2 read) are fetched before the current one is applied.
                     int x = p.h_cs + HT(p.h_cs_ptr, k);
                     const int xe = p.h_cs + HT(p.h_cs_ptr, k + 1);
                     int2 na = make_int2(0, 0), nb = make_int2(0, 0);
@@ -319,39 +316,49 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                             if (na.x & (1 << 20)) nV = __ldg(gD + p.d_effv + na.y);
                         }
                         if (!has_val) part *= lds(sml + (a.y & 0xffff)) * lds(sml + ((unsigned)a.y >> 16));
-                        unsigned w = (unsigned)b.x;
-                        QSS_SCAT(w & 255, part); QSS_SCAT((w >> 8) & 255, part);
-                        QSS_SCAT((w >> 16) & 255, part); QSS_SCAT(w >> 24, part);
-                        if ((unsigned)b.y != QSS_V1_NULL * 0x01010101u) {
-                            w = (unsigned)b.y;
-                            QSS_SCAT(w & 255, part); QSS_SCAT((w >> 8) & 255, part);
-                            QSS_SCAT((w >> 16) & 255, part); QSS_SCAT(w >> 24, part);
+                        const int mag = (a.x >> 21) & 7;
+                        if (mag > 1) part *= (double)mag;
+                        const double npart = -part;
+                        {
+                            const unsigned w = (unsigned)b.x;
+                            const unsigned a0 = colw + (w & 127) * RS, a1 = colw + ((w >> 8) & 127) * RS;
+                            const unsigned a2 = colw + ((w >> 16) & 127) * RS, a3 = colw + ((w >> 24) & 127) * RS;
+                            const double v0 = lds(a0), v1 = lds(a1), v2 = lds(a2), v3 = lds(a3);
+                            sts(a0, v0 + ((w & 0x80u) ? npart : part));
+                            sts(a1, v1 + ((w & 0x8000u) ? npart : part));
+                            sts(a2, v2 + ((w & 0x800000u) ? npart : part));
+                            sts(a3, v3 + ((w & 0x80000000u) ? npart : part));
+                        }
+                        if (((a.x >> 16) & 15) > 4) {
+                            const unsigned w = (unsigned)b.y;
+                            const unsigned a0 = colw + (w & 127) * RS, a1 = colw + ((w >> 8) & 127) * RS;
+                            const unsigned a2 = colw + ((w >> 16) & 127) * RS, a3 = colw + ((w >> 24) & 127) * RS;
+                            const double v0 = lds(a0), v1 = lds(a1), v2 = lds(a2), v3 = lds(a3);
+                            sts(a0, v0 + ((w & 0x80u) ? npart : part));
+                            sts(a1, v1 + ((w & 0x8000u) ? npart : part));
+                            sts(a2, v2 + ((w & 0x800000u) ? npart : part));
+                            sts(a3, v3 + ((w & 0x80000000u) ? npart : part));
                         }
                     }
-#pragma unroll
-                    for (int q = 0; q < QSS_V1_NQ; ++q) if (q < Nq) sts(ycw + q * (QSS_V1_NW * 256), cq[q]);
                     // dy/dx solve program: y[a] = (y[a] + sum_t F_t * y[b_t]) [* 1/D]  (a thread only touches its own lane)
                     int pc = p.h_sp;
 #pragma unroll 1
                     for (int op = p.n_sp_ops; op > 0; --op) {
                         const unsigned hd = (unsigned)HT(pc, 0);
-                        const unsigned ya = ycw + (hd & 0xffff);
+                        const unsigned ya = ycw + (hd & 0xffff) * 256;
                         double acc = lds(ya);
                         int nt = (hd >> 16) & 255;
                         ++pc;
-                        unsigned idoff = 0;
-                        if (hd >> 24) { idoff = (unsigned)HT(pc, 0); ++pc; }
+                        unsigned idrow = 0;
+                        if (hd >> 24) { idrow = (unsigned)HT(pc, 0); ++pc; }
 #pragma unroll 1
                         for (; nt > 0; --nt, ++pc) {
                             const unsigned w = (unsigned)HT(pc, 0);
-                            acc = fma(lds(sml + (w & 0xffff)), lds(ycw + (w >> 16)), acc);
+                            acc = fma(lds(sml + (w & 0xffff) * 256), lds(ycw + (w >> 16) * 256), acc);
                         }
-                        if (hd >> 24) acc *= lds(sml + idoff);
+                        if (hd >> 24) acc *= lds(sml + idrow * 256);
                         sts(ya, acc);
                     }
-                    const unsigned wxw = sml + (p.s_WX + warp) * 256;  // W_x[:,k] of this round: row i at + i * nw * 256
-#pragma unroll
-                    for (int i = 0; i < QSS_V1_NT; ++i) if (i < N) sts(wxw + i * (QSS_V1_NW * 256), ct[i]);
                 }
                 __syncthreads();
                 // -- pass B: warp = row i.  J[i, round] = W_x[i, round] + sum_q W_y[i][q] * dy_q/dx[round]

@@ -13,11 +13,8 @@
 #include <stdint.h>
 
 #define QSS_V1_HMAX 8000        // 32-bit words of hot tables carried in the kernel parameters (<= 32 KB total)
-#define QSS_V1_NT 36            // register column: rows for transported species (needs N + 1 <= 36 columns too)
-#define QSS_V1_NQ 20            // register column: rows for QSS species
 #define QSS_V1_NW 12            // warps per block = Jacobian columns per round
 #define QSS_V1_RREC 8           // int32 words per reaction record
-#define QSS_V1_NULL 112         // scatter index that does nothing (2 * (NT + NQ))
 
 struct QssV1 {
     // ---- filled at launch
