@@ -179,7 +179,10 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     std::map<std::pair<int, int>, std::vector<int32_t>> wy;
     for (int j = 0; j < M; ++j) for (int dir = 0; dir < 2; ++dir) {
         if (!((R[j].mask >> dir) & 1) || R[j].q[dir] < 0) continue;
-        for (const Term &x : R[j].net) if (x.sp < N) wy[{x.sp, R[j].q[dir]}].push_back((2 * j + dir) | (nucode(dir == 0 ? x.nu : -x.nu) << 12));
+        for (const Term &x : R[j].net) if (x.sp < N) {        // one word per unit of |nu|: byte offset of kappa_d in s_KAP | sign bit
+            const int e = dir == 0 ? x.nu : -x.nu;
+            for (int u = 0; u < std::abs(e); ++u) wy[{x.sp, R[j].q[dir]}].push_back(((2 * j + dir) * 256) | (e < 0 ? (int32_t)0x80000000 : 0));
+        }
     }
     std::vector<int32_t> wya_ptr{0}, wya_all;
     {
@@ -205,7 +208,11 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     v.nw = nw;
     v.s_WX = rows_fixed; v.s_YC = rows_fixed + N * nw;       // one column buffer: row (species) r of column w at r * nw + w
     v.s_KAP = rows_fixed; v.s_G = rows_fixed + 2 * M; v.s_H = v.s_G + nsp + 1;
-    v.smem_rows = rows_fixed + region;
+    // the W_y assembly lists are staged once per block in the spare shared memory behind the per-cell rows
+    v.n_tab_words = (int32_t)(wya_ptr.size() + wya_all.size());
+    v.s_TAB = rows_fixed + region;
+    v.smem_rows = v.s_TAB + (v.n_tab_words * 4 + 255) / 256;
+    if (v.smem_rows > max_rows) { why = "per-cell state and staged tables do not fit the shared memory of one SM"; return false; }
     {
         int o = 0;
         auto tk = [&](int n) { int r = o; o += n; return r; };
@@ -335,8 +342,8 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     // ---- W_y assembly lists (appended to the int blob)
     {
         std::vector<int32_t> &I = out.I;
-        v.i_wya_ptr = (int32_t)I.size(); I.insert(I.end(), wya_ptr.begin(), wya_ptr.end());
-        v.i_wya = (int32_t)I.size(); I.insert(I.end(), wya_all.begin(), wya_all.end());
+        v.i_wya_ptr = (int32_t)I.size(); I.insert(I.end(), wya_ptr.begin(), wya_ptr.end());   // [n_wy + 1] then the words
+        I.insert(I.end(), wya_all.begin(), wya_all.end());
     }
     // ---- reaction records (appended to the int blob), in processing order
     {

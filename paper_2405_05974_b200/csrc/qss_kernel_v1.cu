@@ -54,6 +54,11 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
     const double *gD = p.gD;
     const unsigned sml = (unsigned)__cvta_generic_to_shared(qss_smem) + lane * 8;   // this lane's column of the rows
 
+    // stage the W_y assembly lists behind the per-cell rows (once per block; the block is persistent over slabs)
+    const int *tab = reinterpret_cast<const int *>(qss_smem + (size_t)p.s_TAB * 32);
+    for (int i = threadIdx.x; i < p.n_tab_words; i += blockDim.x) reinterpret_cast<int *>(qss_smem + (size_t)p.s_TAB * 32)[i] = __ldg(gI + p.i_wya_ptr + i);
+    __syncthreads();
+
     for (int64_t slab = blockIdx.x; slab < nslab; slab += gridDim.x) {
         const int64_t cell = slab * 32 + lane;
         const bool active = cell < p.ncells;
@@ -180,11 +185,14 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         if (JAC) {
             // ---- P7 (same phase: reads kappa only): W_y[i][q] = d wdot_i / d y_q at fixed x, sums of kappas
             //      (Eq. 9 second parenthesis, L224); the entries go to the scratch slab, pass B reads each once per round
+            const unsigned kb = sml + p.s_KAP * 256;
             for (int e = warp; e < p.n_wy; e += nw) {
                 double acc = 0.0;
-                for (int x = __ldg(gI + p.i_wya_ptr + e), xe = __ldg(gI + p.i_wya_ptr + e + 1); x < xe; ++x) {
-                    const int w = __ldg(gI + p.i_wya + x);
-                    acc = fma(HD(p.h_nulut, (w >> 12) & 15), SM(p.s_KAP, w & 4095), acc);
+                const int xe = tab[e + 1];
+                for (int x = tab[e]; x < xe; ++x) {
+                    const int w = tab[p.n_wy + 1 + x], sg = w & 0x80000000;
+                    const double kap = lds(kb + (w & 0x7fffffff));
+                    acc += __hiloint2double(__double2hiint(kap) ^ sg, __double2loint(kap));
                 }
                 SC(p.g_WY, e) = acc;
             }

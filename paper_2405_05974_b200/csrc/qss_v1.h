@@ -26,7 +26,7 @@ struct QssV1 {
     const double *gD;
     int32_t d_thermo, d_rate_r, d_effm1, i_eff_ptr, i_eff_sp, i_rrec;   // d_rate_r: rate records in processing order
     int32_t d_effv;                                  // (alpha - 1) values of the column streams
-    int32_t i_wya_ptr, i_wya;                        // W_y assembly lists: dir | nucode<<12 (global, read once per slab)
+    int32_t i_wya_ptr, n_tab_words;                  // W_y assembly lists: [n_wy + 1] pointers, then byte offset of kappa_d | sign bit
     // ---- sizes
     int32_t N, Nq, M, nsp, n_tb, nw, n_groups, n_levels, n_centry, n_xp, n_wy, n_rounds, n_sp_ops;
     // ---- shared-memory rows (one row = 32 doubles = 256 bytes, lane = cell)
@@ -39,6 +39,7 @@ struct QssV1 {
     int32_t s_WX;       // [N*nw]    W_x of the round's columns, row i*nw + w     }   s_G, s_H (thermo, rate phases)
     int32_t s_KAP;      // [2M]      kappa_d; then in place Q_j (row 2j), dQ_j/dT (row 2j+1) }   (phases P2-P6)
     int32_t s_G, s_H;   // [nsp+1]   g/RT, h/RT (+ a zero row), after s_KAP                  }   (phases P1-P2)
+    int32_t s_TAB;      // staged once per block: the W_y assembly lists (n_tab_words int32)
     int32_t smem_rows;
     // ---- scratch rows
     int32_t g_K;        // [2M]      k_d
