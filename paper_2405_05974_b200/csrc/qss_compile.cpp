@@ -108,7 +108,6 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     }
     std::vector<int32_t> H;
     auto at = [&]() { return (int32_t)H.size(); };
-    auto nucode = [](int nu) { return nu + 8; };
     // closure gather
     {
         std::vector<int32_t> ptr{0}, dst, dir;
@@ -330,11 +329,6 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         v.n_rounds = (N + 1 + nw - 1) / nw;
         v.h_cw = at();
         for (int i = 0; i < v.n_rounds * nw; ++i) H.push_back(i <= N ? idx[i] : -1);
-    }
-    {
-        if (H.size() & 1) H.push_back(0);
-        v.h_nulut = at();
-        for (int cde = 0; cde < 16; ++cde) { double x = (double)(cde - 8); int32_t w[2]; std::memcpy(w, &x, 8); H.push_back(w[0]); H.push_back(w[1]); }
     }
     if ((int)H.size() > QSS_V1_HMAX) { why = "hot tables exceed the kernel-parameter budget of variant 1"; return false; }
     v.h_used = (int32_t)H.size();

@@ -30,7 +30,6 @@ constexpr double kLnP0R = 9.4080919689433160;  // ln(101325 / 8.31446261815324)
 extern __shared__ double qss_smem[];
 
 #define HT(off, i) p.h[(off) + (i)]
-#define HD(off, i) (*reinterpret_cast<const double *>(&p.h[(off) + 2 * (i)]))
 #define SM(row, i) qss_smem[((row) + (i)) * 32 + lane]
 #define SC(row, i) sc[(size_t)((row) + (i)) * 32]
 

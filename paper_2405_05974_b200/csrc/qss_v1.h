@@ -4,7 +4,7 @@
 // Variant 1 processes a slab of 32 consecutive cells per thread block, lane = cell (so every table read is
 // warp-uniform and every per-cell array access is a conflict-free 256-byte row), one block of QSS_V1_NW warps per
 // SM.  The hot per-cell state lives in shared memory; the Jacobian is swept in rounds of QSS_V1_NW columns: each
-// warp builds one column of [W_x; G_x] in REGISTERS (scatter through an indexed branch) and solves for dy/dx_k,
+// warp builds one column of [W_x; G_x] in its shared-memory column buffer and solves for dy/dx_k in place,
 // then the warps switch to rows and add W_y * dy/dx for the whole round from a register tile.  The interpreter
 // tables live in the kernel-parameter constant bank (`h`); the write-once / read-few per-direction arrays go to an
 // L2-resident scratch slab.  DESIGN.md "Kernels" gives the layout and the reasons.
@@ -61,7 +61,6 @@ struct QssV1 {
     int32_t h_sp;                                    // dy/dx solve program (row operations)
     int32_t h_wr_ptr, h_wr;                          // W_y rows: byte offset q*nw*256 of each entry's dy/dx row
     int32_t h_rw_ptr, h_rw;                          // Jacobian rows of pass B assigned to each warp (balanced)
-    int32_t h_nulut;                                 // 16 doubles: nucode -> nu (nucode = nu + 8)
     int32_t h_used;
     alignas(8) int32_t h[QSS_V1_HMAX];
 };
