@@ -86,6 +86,24 @@ def test_configs_small(cfg, n):
     print(f"cfg{cfg}", g)
 
 
+def test_kernel_variants_selected_and_general_kernel_on_cfg2(monkeypatch):
+    """cfg1/cfg2 run on kernel variant 1 (slab-smem), cfg3 on the general variant 0; QSS_VARIANT=0 forces the general
+    kernel, which must meet the same gates on cfg2."""
+    import paper_2405_05974_b200 as qss
+    for cfg, want in ((1, 1), (2, 1), (3, 0)):
+        qm = qss.QssMech(qss_synth.config_mechanism(cfg), 0)
+        assert qm.info.kernel_variant_jac == want and qm.info.kernel_variant_wdot == want
+        qm.close()
+    monkeypatch.setenv("QSS_VARIANT", "0")
+    mech = qss_synth.config_mechanism(2)
+    qm = qss.QssMech(mech, 0)
+    assert qm.info.kernel_variant_jac == 0
+    qm.close()
+    n = 256 + 9
+    C, T = qss_synth.config_states(2, n)
+    _check(mech, C, T, n, "cfg2 (variant 0)")
+
+
 def test_cfg4_field_small():
     mech = qss_synth.config_mechanism(4)
     C, T = qss_synth.config_states(4, 16 ** 3)           # 16^3 cells of the multipulse-shaped field
