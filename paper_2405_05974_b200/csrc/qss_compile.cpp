@@ -264,6 +264,11 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         std::vector<int32_t> ptr{0}, all;
         for (int k = 0; k < N; ++k) { all.insert(all.end(), cs[k].begin(), cs[k].end()); ptr.push_back((int32_t)all.size()); }
         ptr.push_back((int32_t)all.size());                  // the T column has an empty stream
+        // two harmless sentinel records: the kernel's software pipeline fetches two records ahead of the one it applies
+        for (int u = 0; u < 2; ++u) {
+            all.push_back(v.g_K); all.push_back(voff(N) | (voff(N) << 16));
+            all.push_back((int32_t)((uint32_t)nsp * 0x01010101u)); all.push_back((int32_t)((uint32_t)nsp * 0x01010101u));
+        }
         v.h_cs = at(); H.insert(H.end(), all.begin(), all.end());
         v.h_cs_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
     }

@@ -302,49 +302,62 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                         for (int s = 0; s < nsp; ++s) sts(colw + s * RS, SC(p.g_ET, s));
                     }
                     // column stream: part = |nu| * A * V[o1] * V[o2] (* val), added to / subtracted from up to 8 rows of the
-                    // column.  The rows of a record are distinct, so its loads are issued together (no dependent chain);
-                    // the next record and its A (an L2 read) are fetched before the current one is applied.
-                    int x = p.h_cs + HT(p.h_cs_ptr, k);
-                    const int xe = p.h_cs + HT(p.h_cs_ptr, k + 1);
-                    int2 na = make_int2(0, 0), nb = make_int2(0, 0);
-                    double nA = 0.0, nV = 0.0;
-                    if (x < xe) {
-                        na = ldc2(&p.h[x]); nb = ldc2(&p.h[x + 2]); nA = sc[(size_t)(na.x & 0xffff) * 32];
-                        if (na.x & (1 << 20)) nV = __ldg(gD + p.d_effv + na.y);
-                    }
-#pragma unroll 1
-                    while (x < xe) {
-                        const int2 a = na, b = nb;
-                        const bool has_val = (a.x & (1 << 20)) != 0;
-                        double part = has_val ? nA * nV : nA;
-                        x += 4;
-                        if (x < xe) {
-                            na = ldc2(&p.h[x]); nb = ldc2(&p.h[x + 2]); nA = sc[(size_t)(na.x & 0xffff) * 32];
-                            if (na.x & (1 << 20)) nV = __ldg(gD + p.d_effv + na.y);
-                        }
-                        if (!has_val) part *= lds(sml + (a.y & 0xffff)) * lds(sml + ((unsigned)a.y >> 16));
-                        const int mag = (a.x >> 21) & 7;
-                        if (mag > 1) part *= (double)mag;
-                        const double npart = -part;
+                    // column.  Software pipeline over records: while record i is applied (its distinct rows are loaded
+                    // together, updated, stored back), the factors of record i+1 are read from shared memory and the
+                    // table words and A (an L2 read) of record i+2 are fetched.  Reads past the end of a column hit the
+                    // next column's records or the two sentinel records and are discarded.
+                    {
+                        const int x0 = p.h_cs + HT(p.h_cs_ptr, k);
+                        const int nrec = (HT(p.h_cs_ptr, k + 1) - HT(p.h_cs_ptr, k)) >> 2;
+                        const unsigned one = sml + (p.s_V + N) * 256;
+                        int2 sa = ldc2(&p.h[x0]), sb = ldc2(&p.h[x0 + 2]);                  // record i
+                        int2 ma = ldc2(&p.h[x0 + 4]), mb = ldc2(&p.h[x0 + 6]);              // record i + 1
+                        double mA = sc[(size_t)(ma.x & 0xffff) * 32];
+                        double mV = (ma.x & (1 << 20)) ? __ldg(gD + p.d_effv + ma.y) : 1.0;
+                        double part;
                         {
-                            const unsigned w = (unsigned)b.x;
-                            const unsigned a0 = colw + (w & 127) * RS, a1 = colw + ((w >> 8) & 127) * RS;
-                            const unsigned a2 = colw + ((w >> 16) & 127) * RS, a3 = colw + ((w >> 24) & 127) * RS;
-                            const double v0 = lds(a0), v1 = lds(a1), v2 = lds(a2), v3 = lds(a3);
-                            sts(a0, v0 + ((w & 0x80u) ? npart : part));
-                            sts(a1, v1 + ((w & 0x8000u) ? npart : part));
-                            sts(a2, v2 + ((w & 0x800000u) ? npart : part));
-                            sts(a3, v3 + ((w & 0x80000000u) ? npart : part));
+                            const bool hv = (sa.x & (1 << 20)) != 0;
+                            part = sc[(size_t)(sa.x & 0xffff) * 32] * (hv ? __ldg(gD + p.d_effv + sa.y) : 1.0);
+                            part *= lds(hv ? one : sml + (sa.y & 0xffff)) * lds(hv ? one : sml + ((unsigned)sa.y >> 16));
+                            const int mag = (sa.x >> 21) & 7;
+                            if (mag > 1) part *= (double)mag;
                         }
-                        if (((a.x >> 16) & 15) > 4) {
-                            const unsigned w = (unsigned)b.y;
+#pragma unroll 1
+                        for (int i = 0; i < nrec; ++i) {
+                            // apply record i, first half: load its rows
+                            const unsigned w = (unsigned)sb.x;
                             const unsigned a0 = colw + (w & 127) * RS, a1 = colw + ((w >> 8) & 127) * RS;
                             const unsigned a2 = colw + ((w >> 16) & 127) * RS, a3 = colw + ((w >> 24) & 127) * RS;
                             const double v0 = lds(a0), v1 = lds(a1), v2 = lds(a2), v3 = lds(a3);
+                            // factors of record i + 1
+                            const bool hv = (ma.x & (1 << 20)) != 0;
+                            const double u1 = lds(hv ? one : sml + (ma.y & 0xffff)), u2 = lds(hv ? one : sml + ((unsigned)ma.y >> 16));
+                            // table words and A of record i + 2
+                            const int xl = x0 + 4 * (i + 2);
+                            const int2 na = ldc2(&p.h[xl]), nb = ldc2(&p.h[xl + 2]);
+                            const double nA = sc[(size_t)(na.x & 0xffff) * 32];
+                            const double nV = (na.x & (1 << 20)) ? __ldg(gD + p.d_effv + na.y) : 1.0;
+                            // apply record i, second half
+                            const double npart = -part;
                             sts(a0, v0 + ((w & 0x80u) ? npart : part));
                             sts(a1, v1 + ((w & 0x8000u) ? npart : part));
                             sts(a2, v2 + ((w & 0x800000u) ? npart : part));
                             sts(a3, v3 + ((w & 0x80000000u) ? npart : part));
+                            if (((sa.x >> 16) & 15) > 4) {
+                                const unsigned w2 = (unsigned)sb.y;
+                                const unsigned c0 = colw + (w2 & 127) * RS, c1 = colw + ((w2 >> 8) & 127) * RS;
+                                const unsigned c2 = colw + ((w2 >> 16) & 127) * RS, c3 = colw + ((w2 >> 24) & 127) * RS;
+                                const double t0 = lds(c0), t1 = lds(c1), t2 = lds(c2), t3 = lds(c3);
+                                sts(c0, t0 + ((w2 & 0x80u) ? npart : part));
+                                sts(c1, t1 + ((w2 & 0x8000u) ? npart : part));
+                                sts(c2, t2 + ((w2 & 0x800000u) ? npart : part));
+                                sts(c3, t3 + ((w2 & 0x80000000u) ? npart : part));
+                            }
+                            // part of record i + 1; rotate the pipeline
+                            double np = mA * mV * u1 * u2;
+                            const int mag = (ma.x >> 21) & 7;
+                            if (mag > 1) np *= (double)mag;
+                            part = np; sa = ma; sb = mb; ma = na; mb = nb; mA = nA; mV = nV;
                         }
                     }
                     // dy/dx solve program: y[a] = (y[a] + sum_t F_t * y[b_t]) [* 1/D]  (a thread only touches its own lane)
