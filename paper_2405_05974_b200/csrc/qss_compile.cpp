@@ -200,7 +200,7 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     // ---- shared-memory layout (rows of 256 bytes) and scratch layout
     int rows_fixed = 0;
     auto take = [&](int n) { int r = rows_fixed; rows_fixed += n; return r; };
-    v.s_V = take(N + 1 + Nq); v.s_CT = take(1); v.s_CL = take(c.cl_size); v.s_XP = take(v.n_xp); v.s_TV = take(nsp);
+    v.s_V = take(N + 1 + Nq); v.s_CT = take(1); v.s_CL = take(c.cl_size); v.s_XP = take(v.n_xp); v.s_TV = take(nsp); v.s_Z0 = take(1);
     const int max_rows = (227 * 1024) / 256;
     const int region = std::max((nsp + 1) * nw, 2 * M + 2 * (nsp + 1));    // round buffers: nsp rows + 1 junk row per column
     if (rows_fixed + region > max_rows) { why = "per-cell state does not fit the shared memory of one SM"; return false; }
@@ -272,33 +272,57 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         v.h_cs = at(); H.insert(H.end(), all.begin(), all.end());
         v.h_cs_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
     }
-    // ---- dy/dx solve program: row operations y[a] = (y[a] + sum_t F_t * y[b_t]) [* ID] on the warp's dy/dx column,
-    //      in the order cross-group terms, back-elimination (with U[m][k] = P[m][k] / D_k), forward substitution
-    //   header = a_row | n_terms << 16 | has_scale << 24 ; [id_row] ; n_terms x (f_row | b_row << 16)
-    //   a_row, b_row: rows relative to the warp's dy/dx column; f_row, id_row: absolute shared-memory rows
+    // ---- dy/dx solve program: fixed-format row operations on the warp's dy/dx column,
+    //          y[a] = (y[a] + F0 y[b0] + F1 y[b1] + F2 y[b2]) * S
+    //      in the order cross-group terms, back-elimination (with U[m][k] = P[m][k] / D_k), forward substitution (S = 1/D),
+    //      longer rows chained over several operations; unused terms read the zero row, unused scales the 1.0 row.
+    //   4 words: a | b0 << 16 ; b1 | b2 << 16 ; F0 | F1 << 16 ; F2 | S << 16   (a, b: rows relative to the warp's dy/dx
+    //   column; F, S: absolute shared-memory rows).  Independent groups are dealt to TWO chains that the kernel
+    //   advances together (one operation of each per step), which halves the length of the dependent chain.
     {
-        std::vector<int32_t> sp;
-        int nops = 0;
-        auto yoff = [&](int q) { return q * nw; };              // rows; the kernel scales by 256
+        const int one = v.s_V + N, zero = v.s_Z0, junk = (nsp - N) * nw;       // junk: the column's spare row, relative to dy/dx
+        auto yoff = [&](int q) { return q * nw; };
+        typedef std::vector<int32_t> Ops;
+        auto emit = [&](Ops &o, int a, std::vector<std::pair<int, int>> terms, int scale) {   // terms: (F row, b row)
+            size_t t = 0;
+            do {
+                int f[3] = {zero, zero, zero}, bb[3] = {a, a, a};
+                for (int u = 0; u < 3 && t < terms.size(); ++u, ++t) { f[u] = terms[t].first; bb[u] = terms[t].second; }
+                const int sc_ = t >= terms.size() ? scale : one;
+                o.push_back(a | (bb[0] << 16)); o.push_back(bb[1] | (bb[2] << 16)); o.push_back(f[0] | (f[1] << 16)); o.push_back(f[2] | (sc_ << 16));
+            } while (t < terms.size());
+        };
+        std::vector<Ops> gops(c.n_groups);
         for (int g = 0; g < c.n_groups; ++g) {
             const std::vector<int> &mem = (*c.members)[g];
             const int sz = (int)mem.size(), base = v.s_CL + (*c.gbase)[g];
             for (int x = (*c.xp_begin)[g]; x < (*c.xp_end)[g]; ++x) {
                 const auto &e = (*c.xpl)[x];
-                sp.push_back(yoff(e.first.first) | (1 << 16)); sp.push_back((v.s_XP + x) | (yoff(e.first.second) << 16)); ++nops;
+                emit(gops[g], yoff(e.first.first), {{v.s_XP + x, yoff(e.first.second)}}, one);
             }
             for (int m = sz - 2; m >= 0; --m) {
-                sp.push_back(yoff(mem[m]) | ((sz - 1 - m) << 16)); ++nops;
-                for (int k = m + 1; k < sz; ++k) sp.push_back((base + m * sz + k) | (yoff(mem[k]) << 16));
+                std::vector<std::pair<int, int>> t;
+                for (int k = m + 1; k < sz; ++k) t.push_back({base + m * sz + k, yoff(mem[k])});
+                emit(gops[g], yoff(mem[m]), t, one);
             }
             for (int k = 0; k < sz; ++k) {
-                sp.push_back(yoff(mem[k]) | (k << 16) | (1 << 24)); ++nops;
-                sp.push_back(base + sz * sz + 2 * sz + k);
-                for (int jj = 0; jj < k; ++jj) sp.push_back((base + k * sz + jj) | (yoff(mem[jj]) << 16));
+                std::vector<std::pair<int, int>> t;
+                for (int jj = 0; jj < k; ++jj) t.push_back({base + k * sz + jj, yoff(mem[jj])});
+                emit(gops[g], yoff(mem[k]), t, base + sz * sz + 2 * sz + k);
             }
         }
-        v.n_sp_ops = nops;
-        v.h_sp = at(); H.insert(H.end(), sp.begin(), sp.end());
+        Ops chain[2];
+        for (int g = 0; g < c.n_groups; ++g) {               // groups coupled across (n_xp > 0) stay in order on one chain
+            Ops &dst = v.n_xp > 0 ? chain[0] : (chain[0].size() <= chain[1].size() ? chain[0] : chain[1]);
+            dst.insert(dst.end(), gops[g].begin(), gops[g].end());
+        }
+        const int32_t nop[4] = {junk | (junk << 16), junk | (junk << 16), zero | (zero << 16), zero | (one << 16)};
+        while (chain[0].size() < chain[1].size()) chain[0].insert(chain[0].end(), nop, nop + 4);
+        while (chain[1].size() < chain[0].size()) chain[1].insert(chain[1].end(), nop, nop + 4);
+        if (H.size() & 1) H.push_back(0);
+        v.n_sp_ops = (int32_t)chain[0].size() / 4;
+        v.h_sp = at();
+        for (int i = 0; i < v.n_sp_ops; ++i) { H.insert(H.end(), chain[0].begin() + 4 * i, chain[0].begin() + 4 * i + 4); H.insert(H.end(), chain[1].begin() + 4 * i, chain[1].begin() + 4 * i + 4); }
     }
     // ---- species sums: balanced (longest-processing-time) assignment to warps
     {

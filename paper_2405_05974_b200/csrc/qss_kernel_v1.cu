@@ -67,7 +67,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         const double lnP0RT = kLnP0R - lnT;                    // ln(P0 / (R T))
         // ---- P0: stage the concentrations
         for (int s = warp; s < N; s += nw) SM(p.s_V, s) = p.C[(size_t)s * ld + cc];
-        if (warp == 0) { SM(p.s_V, N) = 1.0; SM(p.s_G, nsp) = 0.0; SM(p.s_H, nsp) = 0.0; }
+        if (warp == 0) { SM(p.s_V, N) = 1.0; SM(p.s_Z0, 0) = 0.0; SM(p.s_G, nsp) = 0.0; SM(p.s_H, nsp) = 0.0; }
         __syncthreads();
         // ---- P1: NASA-7 thermo (readings G4, G9); total concentration
         for (int s = warp; s < nsp; s += nw) {
@@ -360,24 +360,24 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                             part = np; sa = ma; sb = mb; ma = na; mb = nb; mA = nA; mV = nV;
                         }
                     }
-                    // dy/dx solve program: y[a] = (y[a] + sum_t F_t * y[b_t]) [* 1/D]  (a thread only touches its own lane)
-                    int pc = p.h_sp;
+                    // dy/dx solve program: pairs of independent fixed-format row operations
+                    // y[a] = (y[a] + F0 y[b0] + F1 y[b1] + F2 y[b2]) * S; all 16 loads of a pair are issued together
+                    // (a thread only touches its own lane)
 #pragma unroll 1
-                    for (int op = p.n_sp_ops; op > 0; --op) {
-                        const unsigned hd = (unsigned)HT(pc, 0);
-                        const unsigned ya = ycw + (hd & 0xffff) * 256;
-                        double acc = lds(ya);
-                        int nt = (hd >> 16) & 255;
-                        ++pc;
-                        unsigned idrow = 0;
-                        if (hd >> 24) { idrow = (unsigned)HT(pc, 0); ++pc; }
-#pragma unroll 1
-                        for (; nt > 0; --nt, ++pc) {
-                            const unsigned w = (unsigned)HT(pc, 0);
-                            acc = fma(lds(sml + (w & 0xffff) * 256), lds(ycw + (w >> 16) * 256), acc);
-                        }
-                        if (hd >> 24) acc *= lds(sml + idrow * 256);
-                        sts(ya, acc);
+                    for (int pc = p.h_sp, pe = p.h_sp + 8 * p.n_sp_ops; pc < pe; pc += 8) {
+                        const int2 A0 = ldc2(&p.h[pc]), A1 = ldc2(&p.h[pc + 2]), B0 = ldc2(&p.h[pc + 4]), B1 = ldc2(&p.h[pc + 6]);
+                        const unsigned ya = ycw + (A0.x & 0xffff) * 256, yb = ycw + (B0.x & 0xffff) * 256;
+                        double acc = lds(ya), bcc = lds(yb);
+                        const double y0 = lds(ycw + ((unsigned)A0.x >> 16) * 256), y1 = lds(ycw + (A0.y & 0xffff) * 256), y2 = lds(ycw + ((unsigned)A0.y >> 16) * 256);
+                        const double z0 = lds(ycw + ((unsigned)B0.x >> 16) * 256), z1 = lds(ycw + (B0.y & 0xffff) * 256), z2 = lds(ycw + ((unsigned)B0.y >> 16) * 256);
+                        const double f0 = lds(sml + (A1.x & 0xffff) * 256), f1 = lds(sml + ((unsigned)A1.x >> 16) * 256), f2 = lds(sml + (A1.y & 0xffff) * 256);
+                        const double g0 = lds(sml + (B1.x & 0xffff) * 256), g1 = lds(sml + ((unsigned)B1.x >> 16) * 256), g2 = lds(sml + (B1.y & 0xffff) * 256);
+                        const double sa_ = lds(sml + ((unsigned)A1.y >> 16) * 256), sb_ = lds(sml + ((unsigned)B1.y >> 16) * 256);
+                        acc = fma(f0, y0, acc); bcc = fma(g0, z0, bcc);
+                        acc = fma(f1, y1, acc); bcc = fma(g1, z1, bcc);
+                        acc = fma(f2, y2, acc); bcc = fma(g2, z2, bcc);
+                        sts(ya, acc * sa_);
+                        sts(yb, bcc * sb_);
                     }
                 }
                 __syncthreads();

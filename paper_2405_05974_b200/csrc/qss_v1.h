@@ -35,6 +35,7 @@ struct QssV1 {
     int32_t s_CL;       // [cl_size] closure storage: per group P[g*g], leak[g], p0[g], 1/D[g]
     int32_t s_XP;       // [n_xp]    cross-group couplings
     int32_t s_TV;       // [nsp]     third-body vector  sum_j nu_sj dQ_j/dM
+    int32_t s_Z0;       // [1]       zeros (padding of the fixed-format solve operations)
     int32_t s_YC;       // [Nq*nw]   dy/dx of the round's columns, row q*nw + w   } region R, time-shared with
     int32_t s_WX;       // [N*nw]    W_x of the round's columns, row i*nw + w     }   s_G, s_H (thermo, rate phases)
     int32_t s_KAP;      // [2M]      kappa_d; then in place Q_j (row 2j), dQ_j/dT (row 2j+1) }   (phases P2-P6)
@@ -58,7 +59,7 @@ struct QssV1 {
     int32_t h_st_ptr, h_st;                          // third-body incidence: index of dQ_j/dM | sign bit
     int32_t h_cw;                                    // [n_rounds*nw] Jacobian column of (round, warp), -1: none
     int32_t h_cs_ptr, h_cs;                          // column streams (see qss_compile.cpp "column stream")
-    int32_t h_sp;                                    // dy/dx solve program (row operations)
+    int32_t h_sp;                                    // dy/dx solve program: n_sp_ops pairs of fixed-format row operations
     int32_t h_wr_ptr, h_wr;                          // W_y rows: byte offset q*nw*256 of each entry's dy/dx row
     int32_t h_rw_ptr, h_rw;                          // Jacobian rows of pass B assigned to each warp (balanced)
     int32_t h_used;
