@@ -28,6 +28,7 @@ struct qss_mech {
     int nwarp = 8;            // warps per block of the slab kernel
     int blocks_per_sm = 2;
     int nblocks = 0;
+    long long *timing = nullptr;   // device counters when QSS_TIMING=1 (variant 1 only)
     int variant = 0;          // 0: general slab kernel (workspace in global memory); 1: slab-smem kernel (qss_kernel_v1.cu)
 };
 
@@ -101,6 +102,7 @@ extern "C" int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech
         m->variant = 1;
         m->nblocks = m->n_sm;
         m->c.v1.gI = m->dI; m->c.v1.gD = m->dD;
+        if (std::getenv("QSS_TIMING") && cudaMalloc(&m->timing, 16 * sizeof(long long)) == cudaSuccess) cudaMemset(m->timing, 0, 16 * sizeof(long long));
     }
     *out = m;
     return QSS_OK;
@@ -124,6 +126,16 @@ extern "C" int qss_mech_validate(const qss_mech_desc_t *desc, int32_t *n_groups,
 extern "C" int qss_mech_destroy(qss_mech_t *m) {
     if (!m) return QSS_OK;
     DeviceGuard guard(m->device);
+    if (m->timing) {
+        long long t[16];
+        static const char *name[9] = {"P0 stage", "P1 thermo", "P2 rates", "P3+P7 gather", "P4 closure", "P5 net rates", "P6 sums", "P8 pass A", "P8 pass B"};
+        if (cudaMemcpy(t, m->timing, sizeof t, cudaMemcpyDeviceToHost) == cudaSuccess) {
+            long long tot = 0;
+            for (int i = 0; i < 9; ++i) tot += t[i];
+            for (int i = 0; i < 9 && tot > 0; ++i) std::fprintf(stderr, "[qss timing] %-14s %6.2f %%\n", name[i], 100.0 * (double)t[i] / (double)tot);
+        }
+        cudaFree(m->timing);
+    }
     cudaFree(m->dI); cudaFree(m->dD);
     delete m;
     return QSS_OK;
@@ -162,7 +174,7 @@ extern "C" int qss_eval_wdot(const qss_mech_t *m, int64_t ncells, int64_t ld, co
     cudaError_t e;
     if (m->variant == 1) {
         QssV1 v = m->c.v1;
-        v.C = C; v.T = T; v.wdot = wdot; v.cqss = cqss; v.jac = nullptr; v.scratch = (double *)workspace;
+        v.C = C; v.T = T; v.wdot = wdot; v.cqss = cqss; v.jac = nullptr; v.scratch = (double *)workspace; v.timing = nullptr;
         v.ncells = ncells; v.ld = ld; v.scratch_stride = (int64_t)qss_v1_scratch_doubles(v);
         e = qss_launch_v1(v, false, m->nblocks, (cudaStream_t)stream);
     } else {
@@ -179,7 +191,7 @@ extern "C" int qss_eval_jac(const qss_mech_t *m, int64_t ncells, int64_t ld, con
     cudaError_t e;
     if (m->variant == 1) {
         QssV1 v = m->c.v1;
-        v.C = C; v.T = T; v.wdot = wdot; v.cqss = nullptr; v.jac = jac; v.scratch = (double *)workspace;
+        v.C = C; v.T = T; v.wdot = wdot; v.cqss = nullptr; v.jac = jac; v.scratch = (double *)workspace; v.timing = m->timing;
         v.ncells = ncells; v.ld = ld; v.scratch_stride = (int64_t)qss_v1_scratch_doubles(v);
         e = qss_launch_v1(v, true, m->nblocks, (cudaStream_t)stream);
     } else {

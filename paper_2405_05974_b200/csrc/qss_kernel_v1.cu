@@ -42,6 +42,16 @@ __device__ __forceinline__ double lds(unsigned a) {
 __device__ __forceinline__ void sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
 __device__ __forceinline__ int2 ldc2(const int32_t *q) { return *reinterpret_cast<const int2 *>(q); }
 
+// optional phase timing (QSS_TIMING=1): thread 0 of block 0 accumulates the cycles between block barriers
+#define QSS_TICK(ph)                                                                   \
+    do {                                                                               \
+        if (p.timing && blockIdx.x == 0 && threadIdx.x == 0) {                         \
+            const long long t_ = clock64();                                            \
+            p.timing[ph] += t_ - tick_;                                                \
+            tick_ = t_;                                                                \
+        }                                                                              \
+    } while (0)
+
 template <bool JAC>
 __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_constant__ QssV1 p) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
@@ -58,6 +68,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
     for (int i = threadIdx.x; i < p.n_tab_words; i += blockDim.x) reinterpret_cast<int *>(qss_smem + (size_t)p.s_TAB * 32)[i] = __ldg(gI + p.i_wya_ptr + i);
     __syncthreads();
 
+    long long tick_ = clock64();
     for (int64_t slab = blockIdx.x; slab < nslab; slab += gridDim.x) {
         const int64_t cell = slab * 32 + lane;
         const bool active = cell < p.ncells;
@@ -69,6 +80,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         for (int s = warp; s < N; s += nw) SM(p.s_V, s) = p.C[(size_t)s * ld + cc];
         if (warp == 0) { SM(p.s_V, N) = 1.0; SM(p.s_Z0, 0) = 0.0; SM(p.s_G, nsp) = 0.0; SM(p.s_H, nsp) = 0.0; }
         __syncthreads();
+        QSS_TICK(0);
         // ---- P1: NASA-7 thermo (readings G4, G9); total concentration
         for (int s = warp; s < nsp; s += nw) {
             const double *th = gD + p.d_thermo + s * QSS_TH_STRIDE;
@@ -84,6 +96,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             SM(p.s_CT, 0) = ct_;
         }
         __syncthreads();
+        QSS_TICK(1);
         // ---- P2: rate constants, direction coefficients kappa_d (Eq. 2, Eq. 6)
         {
             const double Ctot = SM(p.s_CT, 0);
@@ -170,6 +183,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             }
         }
         __syncthreads();
+        QSS_TICK(2);
         // ---- P3: closure assembly: every P / leak / p0 slot gathers the kappas feeding it (no atomics)
         for (int e = warp; e < p.n_centry; e += nw) {
             double acc = 0.0;
@@ -197,6 +211,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             }
         }
         __syncthreads();
+        QSS_TICK(3);
         // ---- P4: closure solve, level by level of the condensed DAG; subtraction-free elimination
         //          (Eq. 6; readings G2, G8)
         for (int l = 0; l < p.n_levels; ++l) {
@@ -236,6 +251,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                 }
             }
             __syncthreads();
+            QSS_TICK(4);
         }
         // ---- P5: net rates of progress Q_j (Eq. 2), dQ/dT at fixed y and M, dQ/dM
         for (int j = warp; j < M; j += nw) {
@@ -252,6 +268,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             }
         }
         __syncthreads();
+        QSS_TICK(5);
         // ---- P6: species sums: wdot (Eq. 3); for the Jacobian the T-column vector and the third-body vector.
         //      One table entry per unit of |nu|: the sign bit of the entry flips the sign bit of the value.
         {
@@ -286,6 +303,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             for (int q = warp; q < Nq; q += nw) p.cqss[(size_t)q * ld + cell] = SM(p.s_V, N + 1 + q);
         if (JAC) {
             __syncthreads();
+            QSS_TICK(6);
             // ---- P8: Jacobian sweep in rounds of nw columns (Eq. 7, Eq. 9)
             constexpr unsigned RS = QSS_V1_NW * 256;                 // byte stride between rows of a column buffer
             const unsigned colw = sml + (p.s_WX + warp) * 256;       // this warp's column of [W_x; G_x]: species row r at + r * RS
@@ -381,6 +399,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                     }
                 }
                 __syncthreads();
+                QSS_TICK(7);
                 // -- pass B: warp = row i.  J[i, round] = W_x[i, round] + sum_q W_y[i][q] * dy_q/dx[round]
                 for (int u = HT(p.h_rw_ptr, warp); u < HT(p.h_rw_ptr, warp + 1); ++u) {
                     const int i = HT(p.h_rw, u);
@@ -388,15 +407,23 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                     const unsigned wx = sml + (p.s_WX + i * nw) * 256;
 #pragma unroll
                     for (int w = 0; w < QSS_V1_NW; ++w) acc[w] = lds(wx + w * 256);
-                    int x = HT(p.h_wr_ptr, i);
-                    const int xe = HT(p.h_wr_ptr, i + 1);
-                    double na = x < xe ? SC(p.g_WY, x) : 0.0;
-                    unsigned ny = x < xe ? (unsigned)HT(p.h_wr, x) : 0u;
+                    // the W_y entries of the row are L2 reads: up to 16 are issued together before the first is used
+                    const int x0 = HT(p.h_wr_ptr, i), xe = HT(p.h_wr_ptr, i + 1);
+                    double wy[16];
+#pragma unroll
+                    for (int u = 0; u < 16; ++u) wy[u] = x0 + u < xe ? SC(p.g_WY, x0 + u) : 0.0;
+#pragma unroll
+                    for (int u = 0; u < 16; ++u) {
+                        if (x0 + u < xe) {
+                            const unsigned yr = sml + p.s_YC * 256 + (unsigned)HT(p.h_wr, x0 + u);
+#pragma unroll
+                            for (int w = 0; w < QSS_V1_NW; ++w) acc[w] = fma(wy[u], lds(yr + w * 256), acc[w]);
+                        }
+                    }
 #pragma unroll 1
-                    for (; x < xe; ++x) {
-                        const double a = na;
-                        const unsigned yr = sml + p.s_YC * 256 + ny;
-                        if (x + 1 < xe) { na = SC(p.g_WY, x + 1); ny = (unsigned)HT(p.h_wr, x + 1); }
+                    for (int x = x0 + 16; x < xe; ++x) {
+                        const double a = SC(p.g_WY, x);
+                        const unsigned yr = sml + p.s_YC * 256 + (unsigned)HT(p.h_wr, x);
 #pragma unroll
                         for (int w = 0; w < QSS_V1_NW; ++w) acc[w] = fma(a, lds(yr + w * 256), acc[w]);
                     }
@@ -410,6 +437,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                     }
                 }
                 __syncthreads();
+                QSS_TICK(8);
             }
         }
         __syncthreads();      // shared memory and the scratch slab are reused by the next cell slab

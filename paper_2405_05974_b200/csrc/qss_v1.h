@@ -21,6 +21,7 @@ struct QssV1 {
     const double *C, *T;
     double *wdot, *cqss, *jac, *scratch;
     int64_t ncells, ld, scratch_stride;          // scratch_stride: doubles per block
+    long long *timing;                           // NULL, or 16 counters for the phase timing (QSS_TIMING=1, debugging aid)
     // ---- global tables (the QssTab blobs)
     const int32_t *gI;
     const double *gD;
