@@ -106,16 +106,17 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         for (int s = 0; s < 2; ++s) { int n = 0; for (const Term &x : R[j].side[s]) n += x.nu; if (n > 3) { why = "a reaction side has more than 3 molecules"; return false; } }
         for (const Term &x : R[j].net) if (x.nu < -7 || x.nu > 7) { why = "net stoichiometric coefficient out of range"; return false; }
     }
-    std::vector<int32_t> H;
+    std::vector<int32_t> H, ce_tab;
     auto at = [&]() { return (int32_t)H.size(); };
     // closure gather
     {
         std::vector<int32_t> ptr{0}, dst, dir;
         for (auto &kv : *c.ce) { dst.push_back(kv.first); dir.insert(dir.end(), kv.second.begin(), kv.second.end()); ptr.push_back((int32_t)dir.size()); }
         v.n_centry = (int32_t)dst.size();
-        v.h_ce_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
-        v.h_ce_dst = at(); H.insert(H.end(), dst.begin(), dst.end());
-        v.h_ce_dir = at(); H.insert(H.end(), dir.begin(), dir.end());
+        // staged in shared memory with the W_y lists (t_ce_* are offsets into that table): pointers, destinations, kappa rows
+        ce_tab.insert(ce_tab.end(), ptr.begin(), ptr.end());
+        ce_tab.insert(ce_tab.end(), dst.begin(), dst.end());
+        ce_tab.insert(ce_tab.end(), dir.begin(), dir.end());
     }
     {
         std::vector<int32_t> ptr{0}, dir, xm, xn;
@@ -208,7 +209,8 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     v.s_WX = rows_fixed; v.s_YC = rows_fixed + N * nw;       // one column buffer: row (species) r of column w at r * nw + w
     v.s_KAP = rows_fixed; v.s_G = rows_fixed + 2 * M; v.s_H = v.s_G + nsp + 1;
     // the W_y assembly lists are staged once per block in the spare shared memory behind the per-cell rows
-    v.n_tab_words = (int32_t)(wya_ptr.size() + wya_all.size());
+    v.t_ce_ptr = (int32_t)(wya_ptr.size() + wya_all.size()); v.t_ce_dst = v.t_ce_ptr + v.n_centry + 1; v.t_ce_dir = v.t_ce_dst + v.n_centry;
+    v.n_tab_words = (int32_t)(wya_ptr.size() + wya_all.size() + ce_tab.size());
     v.s_TAB = rows_fixed + region;
     v.smem_rows = v.s_TAB + (v.n_tab_words * 4 + 255) / 256;
     if (v.smem_rows > max_rows) { why = "per-cell state and staged tables do not fit the shared memory of one SM"; return false; }
@@ -220,7 +222,8 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         if (o > 65535) { why = "scratch rows beyond the 16-bit offsets of variant 1"; return false; }
     }
     // ---- column stream: everything that is scattered into column k of [W_x; G_x], as records
-    //   w0 = scratch row of A | n_entries << 16 | has_val << 20 | |nu| << 21      part = |nu| * A * V[o1] * V[o2] (* val)
+    //   w0 = scratch row of A | n_entries << 16 | has_val << 20 | |nu| << 21 | own << 24      part = |nu| * A * V[o1] * V[o2] (* val)
+    //        own: the contribution to the column's own row k (almost every record has one) is kept in a register: 1 add, 2 subtract
     //   w1 = byte offset of V row o1 | byte offset of V row o2 << 16        (has_val: index of val in the double blob)
     //   w2, w3 = up to 8 targets (bytes): species row of the column buffer | 0x80 if the term is subtracted; nsp = none (junk row)
     // One record per (enabled direction, molecule slot holding species k): A = k_d, o1/o2 = the other two slots
@@ -232,13 +235,17 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     auto push_record = [&](int k, int rowA, int o1, int o2, const std::vector<Term> &net, int sgn, bool has_val, double val) {
         for (int mag = 1; mag <= 7; ++mag) {                 // one record per magnitude |nu| (almost always only 1)
             std::vector<int> idx;
-            for (const Term &x : net) if (std::abs(x.nu) == mag) idx.push_back(x.sp | (sgn * x.nu < 0 ? 0x80 : 0));
-            if (idx.empty()) continue;
+            int own = 0;                                     // the column's own row k is accumulated in a register: 1 add, 2 subtract
+            for (const Term &x : net) if (std::abs(x.nu) == mag) {
+                if (x.sp == k) own = sgn * x.nu < 0 ? 2 : 1;
+                else idx.push_back(x.sp | (sgn * x.nu < 0 ? 0x80 : 0));
+            }
+            if (idx.empty() && !own) continue;
             if (idx.size() > 8) { cs_ok = false; return; }
             const uint32_t none = (uint32_t)nsp * 0x01010101u;   // the junk row of the column buffer
             uint32_t w[2] = {none, none};
             for (size_t u = 0; u < idx.size(); ++u) { w[u / 4] &= ~(0xFFu << (8 * (u % 4))); w[u / 4] |= (uint32_t)idx[u] << (8 * (u % 4)); }
-            cs[k].push_back(rowA | ((int)idx.size() << 16) | ((has_val ? 1 : 0) << 20) | (mag << 21));
+            cs[k].push_back(rowA | ((int)idx.size() << 16) | ((has_val ? 1 : 0) << 20) | (mag << 21) | (own << 24));
             if (has_val) { cs[k].push_back((int32_t)effv.size()); effv.push_back(val); }
             else cs[k].push_back(o1 | (o2 << 16));
             cs[k].push_back((int32_t)w[0]); cs[k].push_back((int32_t)w[1]);
@@ -261,14 +268,33 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     if (voff(N + Nq) > 65535) { why = "V rows beyond the 16-bit offsets of variant 1"; return false; }
     {
         if (H.size() & 1) H.push_back(0);
+        // records are applied two at a time (the kernel issues the row loads of both together), so they are packed into
+        // PAIRS with disjoint target rows; a record without a partner gets the null record
+        const uint32_t junk4 = (uint32_t)nsp * 0x01010101u;
+        const int32_t null_rec[4] = {v.g_K, voff(N) | (voff(N) << 16), (int32_t)junk4, (int32_t)junk4};
+        auto rows_of = [&](const int32_t *r) {
+            uint64_t m0 = 0, m1 = 0;
+            for (int u = 0; u < 8; ++u) { const int row = ((uint32_t)r[2 + u / 4] >> (8 * (u % 4))) & 127; if (row != nsp) (row < 64 ? m0 : m1) |= 1ull << (row & 63); }
+            return std::make_pair(m0, m1);
+        };
         std::vector<int32_t> ptr{0}, all;
-        for (int k = 0; k < N; ++k) { all.insert(all.end(), cs[k].begin(), cs[k].end()); ptr.push_back((int32_t)all.size()); }
-        ptr.push_back((int32_t)all.size());                  // the T column has an empty stream
-        // two harmless sentinel records: the kernel's software pipeline fetches two records ahead of the one it applies
-        for (int u = 0; u < 2; ++u) {
-            all.push_back(v.g_K); all.push_back(voff(N) | (voff(N) << 16));
-            all.push_back((int32_t)((uint32_t)nsp * 0x01010101u)); all.push_back((int32_t)((uint32_t)nsp * 0x01010101u));
+        for (int k = 0; k < N; ++k) {
+            std::vector<const int32_t *> pending;
+            for (size_t o = 0; o < cs[k].size(); o += 4) {
+                const int32_t *r = &cs[k][o];
+                const auto mr = rows_of(r);
+                size_t hit = pending.size();
+                for (size_t q = 0; q < pending.size(); ++q) { const auto mq = rows_of(pending[q]); if (!(mq.first & mr.first) && !(mq.second & mr.second)) { hit = q; break; } }
+                if (hit == pending.size()) { pending.push_back(r); continue; }
+                all.insert(all.end(), pending[hit], pending[hit] + 4); all.insert(all.end(), r, r + 4);
+                pending.erase(pending.begin() + hit);
+            }
+            for (const int32_t *r : pending) { all.insert(all.end(), r, r + 4); all.insert(all.end(), null_rec, null_rec + 4); }
+            ptr.push_back((int32_t)all.size());
         }
+        ptr.push_back((int32_t)all.size());                  // the T column has an empty stream
+        // two harmless sentinel pairs: the kernel's software pipeline fetches two pairs ahead of the one it applies
+        for (int u = 0; u < 4; ++u) all.insert(all.end(), null_rec, null_rec + 4);
         v.h_cs = at(); H.insert(H.end(), all.begin(), all.end());
         v.h_cs_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
     }
@@ -367,6 +393,7 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         std::vector<int32_t> &I = out.I;
         v.i_wya_ptr = (int32_t)I.size(); I.insert(I.end(), wya_ptr.begin(), wya_ptr.end());   // [n_wy + 1] then the words
         I.insert(I.end(), wya_all.begin(), wya_all.end());
+        I.insert(I.end(), ce_tab.begin(), ce_tab.end());
     }
     // ---- reaction records (appended to the int blob), in processing order
     {

@@ -187,8 +187,8 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         // ---- P3: closure assembly: every P / leak / p0 slot gathers the kappas feeding it (no atomics)
         for (int e = warp; e < p.n_centry; e += nw) {
             double acc = 0.0;
-            for (int x = HT(p.h_ce_ptr, e); x < HT(p.h_ce_ptr, e + 1); ++x) acc += SM(p.s_KAP, HT(p.h_ce_dir, x));
-            SM(p.s_CL, HT(p.h_ce_dst, e)) = acc;
+            for (int x = tab[p.t_ce_ptr + e], xe = tab[p.t_ce_ptr + e + 1]; x < xe; ++x) acc += SM(p.s_KAP, tab[p.t_ce_dir + x]);
+            SM(p.s_CL, tab[p.t_ce_dst + e]) = acc;
         }
         for (int e = warp; e < p.n_xp; e += nw) {
             double acc = 0.0;
@@ -320,63 +320,95 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                         for (int s = 0; s < nsp; ++s) sts(colw + s * RS, SC(p.g_ET, s));
                     }
                     // column stream: part = |nu| * A * V[o1] * V[o2] (* val), added to / subtracted from up to 8 rows of the
-                    // column.  Software pipeline over records: while record i is applied (its distinct rows are loaded
-                    // together, updated, stored back), the factors of record i+1 are read from shared memory and the
-                    // table words and A (an L2 read) of record i+2 are fetched.  Reads past the end of a column hit the
-                    // next column's records or the two sentinel records and are discarded.
+                    // column.  Records come in PAIRS with disjoint rows.  Software pipeline over pairs: while pair i is
+                    // applied (the rows of both records are loaded together, updated, stored back), the factors of pair
+                    // i+1 are read from shared memory and the table words and A (L2 reads) of pair i+2 are fetched.  Reads
+                    // past the end of a column hit the next column's records or the sentinel pairs and are discarded.
                     {
                         const int x0 = p.h_cs + HT(p.h_cs_ptr, k);
-                        const int nrec = (HT(p.h_cs_ptr, k + 1) - HT(p.h_cs_ptr, k)) >> 2;
+                        const int npair = (HT(p.h_cs_ptr, k + 1) - HT(p.h_cs_ptr, k)) >> 3;
                         const unsigned one = sml + (p.s_V + N) * 256;
-                        int2 sa = ldc2(&p.h[x0]), sb = ldc2(&p.h[x0 + 2]);                  // record i
-                        int2 ma = ldc2(&p.h[x0 + 4]), mb = ldc2(&p.h[x0 + 6]);              // record i + 1
-                        double mA = sc[(size_t)(ma.x & 0xffff) * 32];
-                        double mV = (ma.x & (1 << 20)) ? __ldg(gD + p.d_effv + ma.y) : 1.0;
-                        double part;
+#define QSS_FETCH(XO, ra, rb, rA, rV)                                                    \
+    ra = ldc2(&p.h[XO]); rb = ldc2(&p.h[(XO) + 2]);                                      \
+    rA = sc[(size_t)(ra.x & 0xffff) * 32];                                               \
+    rV = (ra.x & (1 << 20)) ? __ldg(gD + p.d_effv + ra.y) : 1.0
+#define QSS_FACTORS(ra, f1, f2)                                                          \
+    const double f1 = lds((ra.x & (1 << 20)) ? one : sml + (ra.y & 0xffff)),             \
+                 f2 = lds((ra.x & (1 << 20)) ? one : sml + ((unsigned)ra.y >> 16))
+#define QSS_PART(ra, rA, rV, f1, f2, out)                                                \
+    double out = rA * rV * f1 * f2;                                                      \
+    if (((ra.x >> 21) & 7) > 1) out *= (double)((ra.x >> 21) & 7)
+#define QSS_ROWS(w, q0, q1, q2, q3)                                                      \
+    const unsigned q0 = colw + ((w) & 127) * RS, q1 = colw + (((w) >> 8) & 127) * RS,    \
+                   q2 = colw + (((w) >> 16) & 127) * RS, q3 = colw + (((w) >> 24) & 127) * RS
+#define QSS_APPLY(w, q0, q1, q2, q3, v0, v1, v2, v3, pt)                                 \
+    sts(q0, v0 + (((w) & 0x80u) ? -pt : pt)); sts(q1, v1 + (((w) & 0x8000u) ? -pt : pt)); \
+    sts(q2, v2 + (((w) & 0x800000u) ? -pt : pt)); sts(q3, v3 + (((w) & 0x80000000u) ? -pt : pt))
+                        double own = 0.0;                                 // contributions to the column's own row k
+                        int2 sa0, sb0, sa1, sb1, ma0, mb0, ma1, mb1;
+                        double tA, tV, mA0, mV0, mA1, mV1, part0, part1;
                         {
-                            const bool hv = (sa.x & (1 << 20)) != 0;
-                            part = sc[(size_t)(sa.x & 0xffff) * 32] * (hv ? __ldg(gD + p.d_effv + sa.y) : 1.0);
-                            part *= lds(hv ? one : sml + (sa.y & 0xffff)) * lds(hv ? one : sml + ((unsigned)sa.y >> 16));
-                            const int mag = (sa.x >> 21) & 7;
-                            if (mag > 1) part *= (double)mag;
+                            QSS_FETCH(x0, sa0, sb0, tA, tV);
+                            QSS_FACTORS(sa0, f1, f2);
+                            QSS_PART(sa0, tA, tV, f1, f2, pt);
+                            part0 = pt;
                         }
+                        {
+                            QSS_FETCH(x0 + 4, sa1, sb1, tA, tV);
+                            QSS_FACTORS(sa1, f1, f2);
+                            QSS_PART(sa1, tA, tV, f1, f2, pt);
+                            part1 = pt;
+                        }
+                        QSS_FETCH(x0 + 8, ma0, mb0, mA0, mV0);
+                        QSS_FETCH(x0 + 12, ma1, mb1, mA1, mV1);
 #pragma unroll 1
-                        for (int i = 0; i < nrec; ++i) {
-                            // apply record i, first half: load its rows
-                            const unsigned w = (unsigned)sb.x;
-                            const unsigned a0 = colw + (w & 127) * RS, a1 = colw + ((w >> 8) & 127) * RS;
-                            const unsigned a2 = colw + ((w >> 16) & 127) * RS, a3 = colw + ((w >> 24) & 127) * RS;
+                        for (int i = 0; i < npair; ++i) {
+                            // apply pair i, first half: load the rows of both records
+                            const unsigned w0 = (unsigned)sb0.x, w1 = (unsigned)sb1.x;
+                            QSS_ROWS(w0, a0, a1, a2, a3);
+                            QSS_ROWS(w1, c0, c1, c2, c3);
                             const double v0 = lds(a0), v1 = lds(a1), v2 = lds(a2), v3 = lds(a3);
-                            // factors of record i + 1
-                            const bool hv = (ma.x & (1 << 20)) != 0;
-                            const double u1 = lds(hv ? one : sml + (ma.y & 0xffff)), u2 = lds(hv ? one : sml + ((unsigned)ma.y >> 16));
-                            // table words and A of record i + 2
-                            const int xl = x0 + 4 * (i + 2);
-                            const int2 na = ldc2(&p.h[xl]), nb = ldc2(&p.h[xl + 2]);
-                            const double nA = sc[(size_t)(na.x & 0xffff) * 32];
-                            const double nV = (na.x & (1 << 20)) ? __ldg(gD + p.d_effv + na.y) : 1.0;
-                            // apply record i, second half
-                            const double npart = -part;
-                            sts(a0, v0 + ((w & 0x80u) ? npart : part));
-                            sts(a1, v1 + ((w & 0x8000u) ? npart : part));
-                            sts(a2, v2 + ((w & 0x800000u) ? npart : part));
-                            sts(a3, v3 + ((w & 0x80000000u) ? npart : part));
-                            if (((sa.x >> 16) & 15) > 4) {
-                                const unsigned w2 = (unsigned)sb.y;
-                                const unsigned c0 = colw + (w2 & 127) * RS, c1 = colw + ((w2 >> 8) & 127) * RS;
-                                const unsigned c2 = colw + ((w2 >> 16) & 127) * RS, c3 = colw + ((w2 >> 24) & 127) * RS;
-                                const double t0 = lds(c0), t1 = lds(c1), t2 = lds(c2), t3 = lds(c3);
-                                sts(c0, t0 + ((w2 & 0x80u) ? npart : part));
-                                sts(c1, t1 + ((w2 & 0x8000u) ? npart : part));
-                                sts(c2, t2 + ((w2 & 0x800000u) ? npart : part));
-                                sts(c3, t3 + ((w2 & 0x80000000u) ? npart : part));
+                            const double t0 = lds(c0), t1 = lds(c1), t2 = lds(c2), t3 = lds(c3);
+                            // factors of pair i + 1
+                            QSS_FACTORS(ma0, f1, f2);
+                            QSS_FACTORS(ma1, g1, g2);
+                            // table words and A of pair i + 2
+                            const int xl = x0 + 8 * (i + 2);
+                            int2 na0, nb0, na1, nb1;
+                            double nA0, nV0, nA1, nV1;
+                            QSS_FETCH(xl, na0, nb0, nA0, nV0);
+                            QSS_FETCH(xl + 4, na1, nb1, nA1, nV1);
+                            // apply pair i, second half
+                            own += (sa0.x & (1 << 24)) ? part0 : ((sa0.x & (2 << 24)) ? -part0 : 0.0);
+                            own += (sa1.x & (1 << 24)) ? part1 : ((sa1.x & (2 << 24)) ? -part1 : 0.0);
+                            QSS_APPLY(w0, a0, a1, a2, a3, v0, v1, v2, v3, part0);
+                            QSS_APPLY(w1, c0, c1, c2, c3, t0, t1, t2, t3, part1);
+                            if (((sa0.x >> 16) & 15) > 4) {
+                                const unsigned w2 = (unsigned)sb0.y;
+                                QSS_ROWS(w2, d0, d1, d2, d3);
+                                const double u0 = lds(d0), u1 = lds(d1), u2 = lds(d2), u3 = lds(d3);
+                                QSS_APPLY(w2, d0, d1, d2, d3, u0, u1, u2, u3, part0);
                             }
-                            // part of record i + 1; rotate the pipeline
-                            double np = mA * mV * u1 * u2;
-                            const int mag = (ma.x >> 21) & 7;
-                            if (mag > 1) np *= (double)mag;
-                            part = np; sa = ma; sb = mb; ma = na; mb = nb; mA = nA; mV = nV;
+                            if (((sa1.x >> 16) & 15) > 4) {
+                                const unsigned w2 = (unsigned)sb1.y;
+                                QSS_ROWS(w2, d0, d1, d2, d3);
+                                const double u0 = lds(d0), u1 = lds(d1), u2 = lds(d2), u3 = lds(d3);
+                                QSS_APPLY(w2, d0, d1, d2, d3, u0, u1, u2, u3, part1);
+                            }
+                            // parts of pair i + 1; rotate the pipeline
+                            QSS_PART(ma0, mA0, mV0, f1, f2, np0);
+                            QSS_PART(ma1, mA1, mV1, g1, g2, np1);
+                            part0 = np0; part1 = np1;
+                            sa0 = ma0; sb0 = mb0; sa1 = ma1; sb1 = mb1;
+                            ma0 = na0; mb0 = nb0; mA0 = nA0; mV0 = nV0;
+                            ma1 = na1; mb1 = nb1; mA1 = nA1; mV1 = nV1;
                         }
+                        if (k < N) sts(colw + k * RS, lds(colw + k * RS) + own);
+#undef QSS_FETCH
+#undef QSS_FACTORS
+#undef QSS_PART
+#undef QSS_ROWS
+#undef QSS_APPLY
                     }
                     // dy/dx solve program: pairs of independent fixed-format row operations
                     // y[a] = (y[a] + F0 y[b0] + F1 y[b1] + F2 y[b2]) * S; all 16 loads of a pair are issued together
