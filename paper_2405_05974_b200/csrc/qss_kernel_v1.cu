@@ -41,6 +41,28 @@ __device__ __forceinline__ double lds(unsigned a) {
 }
 __device__ __forceinline__ void sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
 __device__ __forceinline__ int2 ldc2(const int32_t *q) { return *reinterpret_cast<const int2 *>(q); }
+// mechanism tables in global memory: read-only loads with an L2 evict_last policy, so that the 10 GB of Jacobian
+// entries streaming through the L2 do not push the (tiny, re-read by every block for every slab) tables out to DRAM
+__device__ __forceinline__ unsigned long long l2_keep_policy() {
+    unsigned long long pol;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ int4 ldg_keep(const int4 *q, unsigned long long pol) {
+    int4 v;
+    asm volatile("ld.global.nc.L2::cache_hint.v4.s32 {%0, %1, %2, %3}, [%4], %5;" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(q), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ double ldg_keep(const double *q, unsigned long long pol) {
+    double v;
+    asm volatile("ld.global.nc.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(q), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ int ldg_keep(const int *q, unsigned long long pol) {
+    int v;
+    asm volatile("ld.global.nc.L2::cache_hint.s32 %0, [%1], %2;" : "=r"(v) : "l"(q), "l"(pol));
+    return v;
+}
 
 // optional phase timing (QSS_TIMING=1): thread 0 of block 0 accumulates the cycles between block barriers
 #define QSS_TICK(ph)                                                                   \
@@ -62,6 +84,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
     const int32_t *gI = p.gI;
     const double *gD = p.gD;
     const unsigned sml = (unsigned)__cvta_generic_to_shared(qss_smem) + lane * 8;   // this lane's column of the rows
+    const unsigned long long keep = l2_keep_policy();
 
     // stage the W_y assembly lists behind the per-cell rows (once per block; the block is persistent over slabs)
     const int *tab = reinterpret_cast<const int *>(qss_smem + (size_t)p.s_TAB * 32);
@@ -106,10 +129,10 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             int4 nra = make_int4(0, 0, 0, 0), nrb = nra;
             double nq0 = 0.0, nq1 = 0.0, nq2 = 0.0, nq10 = 0.0;
             if (warp < M) {
-                nra = __ldg(reinterpret_cast<const int4 *>(gI + p.i_rrec + warp * QSS_V1_RREC));
-                nrb = __ldg(reinterpret_cast<const int4 *>(gI + p.i_rrec + warp * QSS_V1_RREC + 4));
+                nra = ldg_keep(reinterpret_cast<const int4 *>(gI + p.i_rrec + warp * QSS_V1_RREC), keep);
+                nrb = ldg_keep(reinterpret_cast<const int4 *>(gI + p.i_rrec + warp * QSS_V1_RREC + 4), keep);
                 const double *rn = gD + p.d_rate_r + warp * QSS_RD_STRIDE;
-                nq0 = __ldg(rn); nq1 = __ldg(rn + 1); nq2 = __ldg(rn + 2); nq10 = __ldg(rn + 10);
+                nq0 = ldg_keep(rn, keep); nq1 = ldg_keep(rn + 1, keep); nq2 = ldg_keep(rn + 2, keep); nq10 = ldg_keep(rn + 10, keep);
             }
 #pragma unroll 1
             for (int r = warp; r < M; r += nw) {
@@ -117,68 +140,70 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                 const double q0 = nq0, q1 = nq1, q2 = nq2, q10 = nq10;
                 const double *rd = gD + p.d_rate_r + r * QSS_RD_STRIDE;
                 if (r + nw < M) {
-                    nra = __ldg(reinterpret_cast<const int4 *>(gI + p.i_rrec + (r + nw) * QSS_V1_RREC));
-                    nrb = __ldg(reinterpret_cast<const int4 *>(gI + p.i_rrec + (r + nw) * QSS_V1_RREC + 4));
+                    nra = ldg_keep(reinterpret_cast<const int4 *>(gI + p.i_rrec + (r + nw) * QSS_V1_RREC), keep);
+                    nrb = ldg_keep(reinterpret_cast<const int4 *>(gI + p.i_rrec + (r + nw) * QSS_V1_RREC + 4), keep);
                     const double *rn = rd + nw * QSS_RD_STRIDE;
-                    nq0 = __ldg(rn); nq1 = __ldg(rn + 1); nq2 = __ldg(rn + 2); nq10 = __ldg(rn + 10);
+                    nq0 = ldg_keep(rn, keep); nq1 = ldg_keep(rn + 1, keep); nq2 = ldg_keep(rn + 2, keep); nq10 = ldg_keep(rn + 10, keep);
                 }
                 const int j = ra.x & 4095, type = (ra.x >> 12) & 3, mask = (ra.x >> 14) & 3, tb = (ra.x >> 16) - 1;
+                // all shared-memory reads of the reaction first, then the two exponentials side by side (two independent
+                // Horner chains), then the type-specific factor
+                const unsigned g0 = rb.x & 0xffff, g1 = (unsigned)rb.x >> 16, g2 = rb.y & 0xffff;      // reactant molecules
+                const unsigned g3 = (unsigned)rb.y >> 16, g4 = rb.z & 0xffff, g5 = (unsigned)rb.z >> 16;  // product molecules
+                const double dG = (lds(gbase + g3) + lds(gbase + g4) + lds(gbase + g5)) - (lds(gbase + g0) + lds(gbase + g1) + lds(gbase + g2));
+                double dH = 0.0;
+                if (JAC) dH = (lds(hbase + g3) + lds(hbase + g4) + lds(hbase + g5)) - (lds(hbase + g0) + lds(hbase + g1) + lds(hbase + g2));
+                const double vf = lds(sml + (ra.y & 0xffff)) * lds(sml + ((unsigned)ra.y >> 16)) * lds(sml + (ra.z & 0xffff));
+                const double vb = lds(sml + ((unsigned)ra.z >> 16)) * lds(sml + (ra.w & 0xffff)) * lds(sml + ((unsigned)ra.w >> 16));
                 const double lnkinf = q0 + q1 * lnT - q2 * invT;
                 const double dlnkinf = (q1 + q2 * invT) * invT;
                 double k = qss_exp(lnkinf), dlnk = dlnkinf;
+                const double iKc = qss_exp(dG - q10 * lnP0RT);      // 1 / Kc, ln Kc = -dG + dnu ln(P0/RT)
                 if (type >= 1) {
                     double Mc = Ctot;                              // M = sum_k alpha_k C_k, transported only (G7)
-                    const int e0 = gI[p.i_eff_ptr + j], e1 = gI[p.i_eff_ptr + j + 1];
-                    for (int e = e0; e < e1; ++e) Mc += gD[p.d_effm1 + e] * SM(p.s_V, gI[p.i_eff_sp + e]);
+                    const int e0 = ldg_keep(gI + p.i_eff_ptr + j, keep), e1 = ldg_keep(gI + p.i_eff_ptr + j + 1, keep);
+                    for (int e = e0; e < e1; ++e) Mc += ldg_keep(gD + p.d_effm1 + e, keep) * SM(p.s_V, ldg_keep(gI + p.i_eff_sp + e, keep));
                     double dlm;
                     if (type == 1) {
                         k *= Mc;
-                        dlm = 1.0 / Mc;
+                        dlm = qss_rcp(Mc);
                     } else {                                       // Troe fall-off
-                        const double lnk0 = rd[3] + rd[4] * lnT - rd[5] * invT;
-                        const double dlnk0 = (rd[4] + rd[5] * invT) * invT;
+                        const double lnk0 = ldg_keep(rd + 3, keep) + ldg_keep(rd + 4, keep) * lnT - ldg_keep(rd + 5, keep) * invT;
+                        const double dlnk0 = (ldg_keep(rd + 4, keep) + ldg_keep(rd + 5, keep) * invT) * invT;
                         const double Pr = qss_exp(lnk0 - lnkinf) * Mc;
-                        const double al = rd[6], i3 = rd[7], i1 = rd[8], T2s = rd[9];
+                        const double al = ldg_keep(rd + 6, keep), i3 = ldg_keep(rd + 7, keep), i1 = ldg_keep(rd + 8, keep), T2s = ldg_keep(rd + 9, keep);
                         const double e3 = qss_exp(-T * i3), e1x = qss_exp(-T * i1), e2 = qss_exp(-T2s * invT);
                         const double Fc = (1.0 - al) * e3 + al * e1x + e2;
                         const double L = log(Pr) * kInvLn10, Lc = log(Fc) * kInvLn10;
                         const double c = -0.4 - 0.67 * Lc, n = 0.75 - 1.27 * Lc;
                         const double num = L + c, den = n - 0.14 * num;
-                        const double iden = 1.0 / den;
+                        const double iden = qss_rcp(den);
                         const double f1 = num * iden;
-                        const double ione_f = 1.0 / (1.0 + f1 * f1);
+                        const double ione_f = qss_rcp(1.0 + f1 * f1);
                         const double F = qss_exp(kLn10 * Lc * ione_f);
-                        const double i1pr = 1.0 / (1.0 + Pr);
+                        const double i1pr = qss_rcp(1.0 + Pr);
                         k = k * (Pr * i1pr) * F;
                         const double df1_dL = n * iden * iden;
                         const double dlF_dL = -2.0 * Lc * f1 * df1_dL * ione_f * ione_f;
-                        dlm = (i1pr + dlF_dL) / Mc;
+                        dlm = (i1pr + dlF_dL) * qss_rcp(Mc);
                         if (JAC) {
                             const double dFc = -(1.0 - al) * i3 * e3 - al * i1 * e1x + T2s * invT * invT * e2;
                             const double df1_dLc = (-0.67 * den - num * (-1.27 + 0.14 * 0.67)) * iden * iden;
                             const double dlF_dLc = ione_f - 2.0 * Lc * f1 * df1_dLc * ione_f * ione_f;
                             const double delta = dlnk0 - dlnkinf;
-                            dlnk = dlnkinf + delta * i1pr + dlF_dL * delta + dlF_dLc * dFc / Fc;
+                            dlnk = dlnkinf + delta * i1pr + dlF_dL * delta + dlF_dLc * dFc * qss_rcp(Fc);
                         }
                     }
                     if (JAC) SC(p.g_QM, tb) = dlm;
                 }
-                double kf = (mask & 1) ? k : 0.0, kb = 0.0, dlnKc = 0.0;
-                if (mask & 2) {                                    // reverse rate from the equilibrium constant (G10)
-                    const unsigned g0 = rb.x & 0xffff, g1 = (unsigned)rb.x >> 16, g2 = rb.y & 0xffff;      // reactant molecules
-                    const unsigned g3 = (unsigned)rb.y >> 16, g4 = rb.z & 0xffff, g5 = (unsigned)rb.z >> 16;  // product molecules
-                    const double dG = (lds(gbase + g3) + lds(gbase + g4) + lds(gbase + g5)) - (lds(gbase + g0) + lds(gbase + g1) + lds(gbase + g2));
-                    kb = k * qss_exp(dG - q10 * lnP0RT);           // k / Kc, ln Kc = -dG + dnu ln(P0/RT)
-                    if (JAC) {
-                        const double dH = (lds(hbase + g3) + lds(hbase + g4) + lds(hbase + g5)) - (lds(hbase + g0) + lds(hbase + g1) + lds(hbase + g2));
-                        dlnKc = (dH - q10) * invT;
-                    }
-                }
+                // reverse rate from the equilibrium constant; a disabled direction contributes nothing (G10)
+                const double kf = (mask & 1) ? k : 0.0, kb = (mask & 2) ? k * iKc : 0.0;
+                const double dlnKc = (mask & 2) ? (dH - q10) * invT : 0.0;
                 SC(p.g_K, 2 * j) = kf;
                 SC(p.g_K, 2 * j + 1) = kb;
                 // kappa_d = k_d * product of the TRANSPORTED reactant molecules (QSS and empty slots read the 1.0 row)
-                sts(kbase + j * 512, kf * lds(sml + (ra.y & 0xffff)) * lds(sml + ((unsigned)ra.y >> 16)) * lds(sml + (ra.z & 0xffff)));
-                sts(kbase + j * 512 + 256, kb * lds(sml + ((unsigned)ra.z >> 16)) * lds(sml + (ra.w & 0xffff)) * lds(sml + ((unsigned)ra.w >> 16)));
+                sts(kbase + j * 512, kf * vf);
+                sts(kbase + j * 512 + 256, kb * vb);
                 if (JAC) { SC(p.g_DF, j) = dlnk; SC(p.g_DC, j) = dlnKc; }
             }
         }
@@ -224,7 +249,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                     const double lk = SM(oL, k);
                     double Dk = lk;
                     for (int m = 0; m < k; ++m) Dk += SM(base, m * sz + k);
-                    const double iD = 1.0 / Dk;
+                    const double iD = qss_rcp(Dk);
                     SM(oID, k) = iD;
                     for (int jj = 0; jj < k; ++jj) {
                         const double f = SM(base, k * sz + jj) * iD;
@@ -233,7 +258,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                             if (m != jj) SM(base, m * sz + jj) += SM(base, m * sz + k) * f;
                     }
                 }
-                SM(oID, 0) = 1.0 / SM(oL, 0);
+                SM(oID, 0) = qss_rcp(SM(oL, 0));
                 for (int k = sz - 1; k >= 1; --k) {          // U[m][k] = P[m][k] / D_k (reused by every dy/dx solve)
                     const double iD = SM(oID, k), tk = SM(oP0, k) * iD;
                     for (int m = 0; m < k; ++m) {
@@ -331,7 +356,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
 #define QSS_FETCH(XO, ra, rb, rA, rV)                                                    \
     ra = ldc2(&p.h[XO]); rb = ldc2(&p.h[(XO) + 2]);                                      \
     rA = sc[(size_t)(ra.x & 0xffff) * 32];                                               \
-    rV = (ra.x & (1 << 20)) ? __ldg(gD + p.d_effv + ra.y) : 1.0
+    rV = (ra.x & (1 << 20)) ? ldg_keep(gD + p.d_effv + ra.y, keep) : 1.0
 #define QSS_FACTORS(ra, f1, f2)                                                          \
     const double f1 = lds((ra.x & (1 << 20)) ? one : sml + (ra.y & 0xffff)),             \
                  f2 = lds((ra.x & (1 << 20)) ? one : sml + ((unsigned)ra.y >> 16))
