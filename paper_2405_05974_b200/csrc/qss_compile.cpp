@@ -302,7 +302,7 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     //          y[a] = (y[a] + F0 y[b0] + F1 y[b1] + F2 y[b2]) * S
     //      in the order cross-group terms, back-elimination (with U[m][k] = P[m][k] / D_k), forward substitution (S = 1/D),
     //      longer rows chained over several operations; unused terms read the zero row, unused scales the 1.0 row.
-    //   4 words: a | b0 << 16 ; b1 | b2 << 16 ; F0 | F1 << 16 ; F2 | S << 16   (a, b: rows relative to the warp's dy/dx
+    //   4 words: a | n_terms << 12 | b0 << 16 ; b1 | b2 << 16 ; F0 | F1 << 16 ; F2 | S << 16   (a, b: rows relative to the warp's dy/dx
     //   column; F, S: absolute shared-memory rows).  Independent groups are dealt to TWO chains that the kernel
     //   advances together (one operation of each per step), which halves the length of the dependent chain.
     {
@@ -312,10 +312,10 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         auto emit = [&](Ops &o, int a, std::vector<std::pair<int, int>> terms, int scale) {   // terms: (F row, b row)
             size_t t = 0;
             do {
-                int f[3] = {zero, zero, zero}, bb[3] = {a, a, a};
-                for (int u = 0; u < 3 && t < terms.size(); ++u, ++t) { f[u] = terms[t].first; bb[u] = terms[t].second; }
+                int f[3] = {zero, zero, zero}, bb[3] = {a, a, a}, nt = 0;
+                for (int u = 0; u < 3 && t < terms.size(); ++u, ++t, ++nt) { f[u] = terms[t].first; bb[u] = terms[t].second; }
                 const int sc_ = t >= terms.size() ? scale : one;
-                o.push_back(a | (bb[0] << 16)); o.push_back(bb[1] | (bb[2] << 16)); o.push_back(f[0] | (f[1] << 16)); o.push_back(f[2] | (sc_ << 16));
+                o.push_back(a | (nt << 12) | (bb[0] << 16)); o.push_back(bb[1] | (bb[2] << 16)); o.push_back(f[0] | (f[1] << 16)); o.push_back(f[2] | (sc_ << 16));
             } while (t < terms.size());
         };
         std::vector<Ops> gops(c.n_groups);
@@ -342,6 +342,7 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
             Ops &dst = v.n_xp > 0 ? chain[0] : (chain[0].size() <= chain[1].size() ? chain[0] : chain[1]);
             dst.insert(dst.end(), gops[g].begin(), gops[g].end());
         }
+        if ((Nq + 1) * nw >= 4096) { why = "dy/dx rows beyond the 12-bit field of the solve operations"; return false; }
         const int32_t nop[4] = {junk | (junk << 16), junk | (junk << 16), zero | (zero << 16), zero | (one << 16)};
         while (chain[0].size() < chain[1].size()) chain[0].insert(chain[0].end(), nop, nop + 4);
         while (chain[1].size() < chain[0].size()) chain[1].insert(chain[1].end(), nop, nop + 4);

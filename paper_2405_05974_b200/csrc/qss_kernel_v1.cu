@@ -441,13 +441,17 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
 #pragma unroll 1
                     for (int pc = p.h_sp, pe = p.h_sp + 8 * p.n_sp_ops; pc < pe; pc += 8) {
                         const int2 A0 = ldc2(&p.h[pc]), A1 = ldc2(&p.h[pc + 2]), B0 = ldc2(&p.h[pc + 4]), B1 = ldc2(&p.h[pc + 6]);
-                        const unsigned ya = ycw + (A0.x & 0xffff) * 256, yb = ycw + (B0.x & 0xffff) * 256;
+                        const unsigned ya = ycw + (A0.x & 0xfff) * 256, yb = ycw + (B0.x & 0xfff) * 256;
+                        const int na_ = (A0.x >> 12) & 3, nb_ = (B0.x >> 12) & 3;        // terms actually present (the rest is padding)
                         double acc = lds(ya), bcc = lds(yb);
-                        const double y0 = lds(ycw + ((unsigned)A0.x >> 16) * 256), y1 = lds(ycw + (A0.y & 0xffff) * 256), y2 = lds(ycw + ((unsigned)A0.y >> 16) * 256);
-                        const double z0 = lds(ycw + ((unsigned)B0.x >> 16) * 256), z1 = lds(ycw + (B0.y & 0xffff) * 256), z2 = lds(ycw + ((unsigned)B0.y >> 16) * 256);
-                        const double f0 = lds(sml + (A1.x & 0xffff) * 256), f1 = lds(sml + ((unsigned)A1.x >> 16) * 256), f2 = lds(sml + (A1.y & 0xffff) * 256);
-                        const double g0 = lds(sml + (B1.x & 0xffff) * 256), g1 = lds(sml + ((unsigned)B1.x >> 16) * 256), g2 = lds(sml + (B1.y & 0xffff) * 256);
                         const double sa_ = lds(sml + ((unsigned)A1.y >> 16) * 256), sb_ = lds(sml + ((unsigned)B1.y >> 16) * 256);
+                        double y0 = 0.0, y1 = 0.0, y2 = 0.0, f0 = 0.0, f1 = 0.0, f2 = 0.0, z0 = 0.0, z1 = 0.0, z2 = 0.0, g0 = 0.0, g1 = 0.0, g2 = 0.0;
+                        if (na_ > 0) { y0 = lds(ycw + ((unsigned)A0.x >> 16) * 256); f0 = lds(sml + (A1.x & 0xffff) * 256); }
+                        if (nb_ > 0) { z0 = lds(ycw + ((unsigned)B0.x >> 16) * 256); g0 = lds(sml + (B1.x & 0xffff) * 256); }
+                        if (na_ > 1) { y1 = lds(ycw + (A0.y & 0xffff) * 256); f1 = lds(sml + ((unsigned)A1.x >> 16) * 256); }
+                        if (nb_ > 1) { z1 = lds(ycw + (B0.y & 0xffff) * 256); g1 = lds(sml + ((unsigned)B1.x >> 16) * 256); }
+                        if (na_ > 2) { y2 = lds(ycw + ((unsigned)A0.y >> 16) * 256); f2 = lds(sml + (A1.y & 0xffff) * 256); }
+                        if (nb_ > 2) { z2 = lds(ycw + ((unsigned)B0.y >> 16) * 256); g2 = lds(sml + (B1.y & 0xffff) * 256); }
                         acc = fma(f0, y0, acc); bcc = fma(g0, z0, bcc);
                         acc = fma(f1, y1, acc); bcc = fma(g1, z1, bcc);
                         acc = fma(f2, y2, acc); bcc = fma(g2, z2, bcc);
