@@ -117,6 +117,50 @@ def test_tiny_and_ragged_cell_counts(n):
     _check(mech, C, T, n, f"cfg1 n={n}")
 
 
+def test_zero_concentrations_and_tmid_tie_break():
+    """Degenerate inputs: species with C_k = 0 (the partial derivatives are products of the OTHER molecules, never
+    r / C_k: reading G12) and cells exactly at T = Tmid = 1000 K (reading G9: the high NASA range applies)."""
+    mech = qss_synth.config_mechanism(2)
+    n = 128 + 7
+    C, T = qss_synth.config_states(2, n)
+    rng = np.random.default_rng(3)
+    for c in range(0, n, 3):                               # zero out 1-4 random species in every third cell
+        C[rng.choice(mech.n_nqss, size=rng.integers(1, 5), replace=False), c] = 0.0
+    T[5:n:11] = 1000.0
+    g = _check(mech, np.ascontiguousarray(C), np.ascontiguousarray(T), n, "cfg2 zeros/Tmid")
+    print(g)
+
+
+def test_non_default_stream_graph_capture_and_padding():
+    """qss_eval_* only enqueue on the caller's stream: a captured CUDA graph replays to the same result; ld > ncells
+    with a large pad leaves the padding untouched."""
+    import paper_2405_05974_b200 as qss
+    torch = _torch()
+    mech = qss_synth.config_mechanism(2)
+    n, ld = 500, 1024
+    C, T = make_states(mech.n_nqss, n, seed=21, ld=ld)
+    qm = qss.QssMech(mech, 0)
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda()
+    J0, w0 = qm.eval_jac(Cd, Td, n, want_wdot=True)
+    torch.cuda.synchronize()
+    J = torch.full_like(J0, float("nan")); w = torch.full_like(w0, float("nan"))
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        qm.eval_jac(Cd, Td, n, jac=J, wdot=w, want_wdot=True)          # warm-up on the side stream
+        s.synchronize()
+        J.fill_(float("nan")); w.fill_(float("nan"))
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            qm.eval_jac(Cd, Td, n, jac=J, wdot=w, want_wdot=True)
+        g.replay()
+        s.synchronize()
+    assert torch.equal(J[:, :, :n], J0[:, :, :n]) and torch.equal(w[:, :n], w0[:, :n])
+    assert torch.isnan(J[:, :, n:]).all() and torch.isnan(w[:, n:]).all()
+    ref = oracle.evaluate(oracle.OracleMech(mech), C, T, n, want_jac=True, want_scale=True)
+    gates.assert_jac(J.cpu().numpy(), ref["jac"], ref["jscale"], n, "graph replay jac")
+
+
 def test_zero_cells_is_a_noop():
     import paper_2405_05974_b200 as qss
     torch = _torch()
