@@ -196,7 +196,6 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         while (row < N) { rptr.push_back((int32_t)roff.size()); ++row; }
         v.n_wy = (int32_t)roff.size();
         v.h_wr_ptr = at(); H.insert(H.end(), rptr.begin(), rptr.end());
-        v.h_wr = at(); H.insert(H.end(), roff.begin(), roff.end());
     }
     // ---- shared-memory layout (rows of 256 bytes) and scratch layout
     int rows_fixed = 0;
@@ -364,18 +363,35 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         v.h_ssw_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
         v.h_ssw = at(); H.insert(H.end(), all.begin(), all.end());
     }
-    {   // pass B rows: balanced by the number of W_y entries
+    {   // pass B tiles: every warp owns up to 3 Jacobian rows (balanced by their number of W_y entries) and sweeps the union
+        // of their W_y columns once per round: h_tile word = q | row mask << 8, in ascending q (the W_y entries of a row are
+        // stored in the same order, so a running index per row finds them)
+        if (N > 3 * nw) { why = "more than 3 Jacobian rows per warp (register tile of pass B)"; return false; }
         std::vector<int> idx(N), cnt(N, 0);
-        for (auto &kv : wy) cnt[kv.first.first]++;
+        std::vector<std::vector<int>> qs(N);
+        for (auto &kv : wy) { cnt[kv.first.first]++; qs[kv.first.first].push_back(kv.first.second); }
         for (int i = 0; i < N; ++i) idx[i] = i;
         std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return cnt[a] > cnt[b]; });
         std::vector<std::vector<int32_t>> bin(nw);
         std::vector<double> load(nw, 0.0);
-        for (int i : idx) { int b = (int)(std::min_element(load.begin(), load.end()) - load.begin()); bin[b].push_back(i); load[b] += 14.0 + cnt[i]; }
-        std::vector<int32_t> ptr{0}, all;
-        for (int w = 0; w < nw; ++w) { all.insert(all.end(), bin[w].begin(), bin[w].end()); ptr.push_back((int32_t)all.size()); }
-        v.h_rw_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
-        v.h_rw = at(); H.insert(H.end(), all.begin(), all.end());
+        for (int i : idx) {
+            int best = -1;
+            for (int w = 0; w < nw; ++w) if (bin[w].size() < 3 && (best < 0 || load[w] < load[best])) best = w;
+            bin[best].push_back(i); load[best] += 14.0 + cnt[i];
+        }
+        std::vector<int32_t> rows, tptr{0}, tile;
+        for (int w = 0; w < nw; ++w) {
+            for (int r = 0; r < 3; ++r) rows.push_back(r < (int)bin[w].size() ? bin[w][r] : -1);
+            for (int q = 0; q < Nq; ++q) {
+                int mask = 0;
+                for (int r = 0; r < (int)bin[w].size(); ++r) if (std::find(qs[bin[w][r]].begin(), qs[bin[w][r]].end(), q) != qs[bin[w][r]].end()) mask |= 1 << r;
+                if (mask) tile.push_back(q | (mask << 8));
+            }
+            tptr.push_back((int32_t)tile.size());
+        }
+        v.h_rw = at(); H.insert(H.end(), rows.begin(), rows.end());
+        v.h_tile_ptr = at(); H.insert(H.end(), tptr.begin(), tptr.end());
+        v.h_tile = at(); H.insert(H.end(), tile.begin(), tile.end());
     }
     // ---- Jacobian columns: rounds of nw columns of similar cost (the warps meet at a barrier after every round)
     {

@@ -461,39 +461,65 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                 }
                 __syncthreads();
                 QSS_TICK(7);
-                // -- pass B: warp = row i.  J[i, round] = W_x[i, round] + sum_q W_y[i][q] * dy_q/dx[round]
-                for (int u = HT(p.h_rw_ptr, warp); u < HT(p.h_rw_ptr, warp + 1); ++u) {
-                    const int i = HT(p.h_rw, u);
-                    double acc[QSS_V1_NW];
-                    const unsigned wx = sml + (p.s_WX + i * nw) * 256;
+                // -- pass B: warp = a tile of up to 3 rows x the 12 columns of the round.
+                //    J[i, round] = W_x[i, round] + sum_q W_y[i][q] * dy_q/dx[round]: dy_q/dx (12 LDS) is read once for the
+                //    rows of the tile that have a W_y entry in column q; the W_y entries are L2 reads fetched two steps ahead
+                {
+                    const int i0 = HT(p.h_rw, warp * 3), i1 = HT(p.h_rw, warp * 3 + 1), i2 = HT(p.h_rw, warp * 3 + 2);
+                    double acc0[QSS_V1_NW], acc1[QSS_V1_NW], acc2[QSS_V1_NW];
 #pragma unroll
-                    for (int w = 0; w < QSS_V1_NW; ++w) acc[w] = lds(wx + w * 256);
-                    // the W_y entries of the row are L2 reads: up to 16 are issued together before the first is used
-                    const int x0 = HT(p.h_wr_ptr, i), xe = HT(p.h_wr_ptr, i + 1);
-                    double wy[16];
-#pragma unroll
-                    for (int u = 0; u < 16; ++u) wy[u] = x0 + u < xe ? SC(p.g_WY, x0 + u) : 0.0;
-#pragma unroll
-                    for (int u = 0; u < 16; ++u) {
-                        if (x0 + u < xe) {
-                            const unsigned yr = sml + p.s_YC * 256 + (unsigned)HT(p.h_wr, x0 + u);
-#pragma unroll
-                            for (int w = 0; w < QSS_V1_NW; ++w) acc[w] = fma(wy[u], lds(yr + w * 256), acc[w]);
-                        }
+                    for (int w = 0; w < QSS_V1_NW; ++w) {
+                        acc0[w] = i0 >= 0 ? lds(sml + (p.s_WX + i0 * nw + w) * 256) : 0.0;
+                        acc1[w] = i1 >= 0 ? lds(sml + (p.s_WX + i1 * nw + w) * 256) : 0.0;
+                        acc2[w] = i2 >= 0 ? lds(sml + (p.s_WX + i2 * nw + w) * 256) : 0.0;
                     }
+                    int x0 = i0 >= 0 ? HT(p.h_wr_ptr, i0) : 0, x1 = i1 >= 0 ? HT(p.h_wr_ptr, i1) : 0, x2 = i2 >= 0 ? HT(p.h_wr_ptr, i2) : 0;
+                    int e = HT(p.h_tile_ptr, warp);
+                    const int ee = HT(p.h_tile_ptr, warp + 1);
+                    int w0 = e < ee ? HT(p.h_tile, e) : 0, w1 = e + 1 < ee ? HT(p.h_tile, e + 1) : 0;
+                    double a00 = 0.0, a01 = 0.0, a02 = 0.0, a10 = 0.0, a11 = 0.0, a12 = 0.0;
+                    if (w0 & 0x100) a00 = SC(p.g_WY, x0++);
+                    if (w0 & 0x200) a01 = SC(p.g_WY, x1++);
+                    if (w0 & 0x400) a02 = SC(p.g_WY, x2++);
+                    if (w1 & 0x100) a10 = SC(p.g_WY, x0++);
+                    if (w1 & 0x200) a11 = SC(p.g_WY, x1++);
+                    if (w1 & 0x400) a12 = SC(p.g_WY, x2++);
 #pragma unroll 1
-                    for (int x = x0 + 16; x < xe; ++x) {
-                        const double a = SC(p.g_WY, x);
-                        const unsigned yr = sml + p.s_YC * 256 + (unsigned)HT(p.h_wr, x);
+                    for (; e < ee; ++e) {
+                        const int w2 = e + 2 < ee ? HT(p.h_tile, e + 2) : 0;
+                        double a20 = 0.0, a21 = 0.0, a22 = 0.0;
+                        if (w2 & 0x100) a20 = SC(p.g_WY, x0++);
+                        if (w2 & 0x200) a21 = SC(p.g_WY, x1++);
+                        if (w2 & 0x400) a22 = SC(p.g_WY, x2++);
+                        const unsigned yr = sml + p.s_YC * 256 + (w0 & 255) * RS;
+                        double y[QSS_V1_NW];
 #pragma unroll
-                        for (int w = 0; w < QSS_V1_NW; ++w) acc[w] = fma(a, lds(yr + w * 256), acc[w]);
+                        for (int w = 0; w < QSS_V1_NW; ++w) y[w] = lds(yr + w * 256);
+                        if (w0 & 0x100) {
+#pragma unroll
+                            for (int w = 0; w < QSS_V1_NW; ++w) acc0[w] = fma(a00, y[w], acc0[w]);
+                        }
+                        if (w0 & 0x200) {
+#pragma unroll
+                            for (int w = 0; w < QSS_V1_NW; ++w) acc1[w] = fma(a01, y[w], acc1[w]);
+                        }
+                        if (w0 & 0x400) {
+#pragma unroll
+                            for (int w = 0; w < QSS_V1_NW; ++w) acc2[w] = fma(a02, y[w], acc2[w]);
+                        }
+                        w0 = w1; w1 = w2;
+                        a00 = a10; a01 = a11; a02 = a12; a10 = a20; a11 = a21; a12 = a22;
                     }
                     if (active) {
-                        double *jrow = p.jac + (size_t)i * (N + 1) * ld + cell;
 #pragma unroll
                         for (int w = 0; w < QSS_V1_NW; ++w) {
                             const int kk = HT(p.h_cw, r * nw + w);
-                            if (kk >= 0) __stcs(jrow + (size_t)(unsigned)kk * (size_t)ld, acc[w]);
+                            if (kk >= 0) {
+                                double *jc = p.jac + (size_t)(unsigned)kk * (size_t)ld + cell;
+                                if (i0 >= 0) __stcs(jc + (size_t)i0 * (N + 1) * ld, acc0[w]);
+                                if (i1 >= 0) __stcs(jc + (size_t)i1 * (N + 1) * ld, acc1[w]);
+                                if (i2 >= 0) __stcs(jc + (size_t)i2 * (N + 1) * ld, acc2[w]);
+                            }
                         }
                     }
                 }

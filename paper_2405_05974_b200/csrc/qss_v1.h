@@ -61,8 +61,9 @@ struct QssV1 {
     int32_t h_cw;                                    // [n_rounds*nw] Jacobian column of (round, warp), -1: none
     int32_t h_cs_ptr, h_cs;                          // column streams (see qss_compile.cpp "column stream")
     int32_t h_sp;                                    // dy/dx solve program: n_sp_ops pairs of fixed-format row operations
-    int32_t h_wr_ptr, h_wr;                          // W_y rows: byte offset q*nw*256 of each entry's dy/dx row
-    int32_t h_rw_ptr, h_rw;                          // Jacobian rows of pass B assigned to each warp (balanced)
+    int32_t h_wr_ptr;                                // [N+1] W_y rows: index of the first entry of each row
+    int32_t h_rw;                                    // [nw][3] Jacobian rows of each warp's pass-B tile (-1: none)
+    int32_t h_tile_ptr, h_tile;                      // per warp: q | row mask << 8 over the union of the rows' W_y columns
     int32_t h_used;
     alignas(8) int32_t h[QSS_V1_HMAX];
 };
