@@ -337,13 +337,21 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                 // -- pass A: warp = column k.  [W_x; G_x][:,k] in shared memory, then (diag D - P) dy/dx_k = G_x[:,k]
                 const int k = HT(p.h_cw, r * nw + warp);
                 if (k >= 0) {
-                    if (k < N) {                                      // rank-1 third-body term (every species column)
-#pragma unroll 4
-                        for (int s = 0; s < nsp; ++s) sts(colw + s * RS, SM(p.s_TV, s));
-                    } else {                                          // T column
+                    // initialise the column: rank-1 third-body vector (every species column) or the T-column vector;
+                    // 8 rows are read before they are written so that the copies do not serialise on the load latency
+                    if (k < N) {
+                        for (int s0 = 0; s0 < nsp; s0 += 8) {
+                            double t[8];
+#pragma unroll
+                            for (int u = 0; u < 8; ++u) t[u] = lds(sml + (p.s_TV + min(s0 + u, nsp - 1)) * 256);
+#pragma unroll
+                            for (int u = 0; u < 8; ++u) if (s0 + u < nsp) sts(colw + (s0 + u) * RS, t[u]);
+                        }
+                    } else {
 #pragma unroll 4
                         for (int s = 0; s < nsp; ++s) sts(colw + s * RS, SC(p.g_ET, s));
                     }
+                    QSS_TICK(11);
                     // column stream: part = |nu| * A * V[o1] * V[o2] (* val), added to / subtracted from up to 8 rows of the
                     // column.  Records come in PAIRS with disjoint rows.  Software pipeline over pairs: while pair i is
                     // applied (the rows of both records are loaded together, updated, stored back), the factors of pair
@@ -435,6 +443,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
 #undef QSS_ROWS
 #undef QSS_APPLY
                     }
+                    QSS_TICK(12);
                     // dy/dx solve program: pairs of independent fixed-format row operations
                     // y[a] = (y[a] + F0 y[b0] + F1 y[b1] + F2 y[b2]) * S; all 16 loads of a pair are issued together
                     // (a thread only touches its own lane)
@@ -459,6 +468,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                         sts(yb, bcc * sb_);
                     }
                 }
+                QSS_TICK(13);
                 __syncthreads();
                 QSS_TICK(7);
                 // -- pass B: warp = a tile of up to 3 rows x the 12 columns of the round.
@@ -510,6 +520,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                         w0 = w1; w1 = w2;
                         a00 = a10; a01 = a11; a02 = a12; a10 = a20; a11 = a21; a12 = a22;
                     }
+                    QSS_TICK(9);
                     if (active) {
 #pragma unroll
                         for (int w = 0; w < QSS_V1_NW; ++w) {
@@ -523,6 +534,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                         }
                     }
                 }
+                QSS_TICK(10);
                 __syncthreads();
                 QSS_TICK(8);
             }
