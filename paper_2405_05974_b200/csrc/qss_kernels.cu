@@ -11,6 +11,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "qss_math.h"
 #include "qss_tables.h"
 
 namespace {
@@ -60,7 +61,7 @@ __device__ __forceinline__ void rates(const QssTab &t, const CellCtx &cx, int j)
     const double T = cx.T, invT = cx.invT;
     const double lnkinf = rd[0] + rd[1] * cx.lnT - rd[2] * invT;
     const double dlnkinf = (rd[1] + rd[2] * invT) * invT;
-    double k = exp(lnkinf), dlnk = dlnkinf, dlm = 0.0;
+    double k = qss_exp(lnkinf), dlnk = dlnkinf, dlm = 0.0;
     if (type >= 1) {
         double Mc = cx.Ctot;                                   // M = sum_k alpha_k C_k, transported only (G7)
         const int e0 = t.I[t.i_eff_ptr + j], e1 = t.I[t.i_eff_ptr + j + 1];
@@ -71,9 +72,9 @@ __device__ __forceinline__ void rates(const QssTab &t, const CellCtx &cx, int j)
         } else {                                               // Troe fall-off
             const double lnk0 = rd[3] + rd[4] * cx.lnT - rd[5] * invT;
             const double dlnk0 = (rd[4] + rd[5] * invT) * invT;
-            const double Pr = exp(lnk0 - lnkinf) * Mc;
+            const double Pr = qss_exp(lnk0 - lnkinf) * Mc;
             const double al = rd[6], i3 = rd[7], i1 = rd[8], T2s = rd[9];
-            const double e3 = exp(-T * i3), e1x = exp(-T * i1), e2 = exp(-T2s * invT);
+            const double e3 = qss_exp(-T * i3), e1x = qss_exp(-T * i1), e2 = qss_exp(-T2s * invT);
             const double Fc = (1.0 - al) * e3 + al * e1x + e2;
             const double dFc = -(1.0 - al) * i3 * e3 - al * i1 * e1x + T2s * invT * invT * e2;
             const double L = log(Pr) * kInvLn10, Lc = log(Fc) * kInvLn10;
@@ -82,7 +83,7 @@ __device__ __forceinline__ void rates(const QssTab &t, const CellCtx &cx, int j)
             const double iden = 1.0 / den;
             const double f1 = num * iden;
             const double one_f = 1.0 + f1 * f1, ione_f = 1.0 / one_f;
-            const double F = exp(kLn10 * Lc * ione_f);
+            const double F = qss_exp(kLn10 * Lc * ione_f);
             const double i1pr = 1.0 / (1.0 + Pr);
             k = k * (Pr * i1pr) * F;
             const double df1_dL = n * iden * iden;
@@ -107,7 +108,7 @@ __device__ __forceinline__ void rates(const QssTab &t, const CellCtx &cx, int j)
             dG += nu * WS(t.w_G, s);
             if (JAC) dH += nu * WS(t.w_H, s);
         }
-        kb = k * exp(dG - rd[10] * cx.lnP0RT);                 // k / Kc, ln Kc = -dG + dnu ln(P0/RT)
+        kb = k * qss_exp(dG - rd[10] * cx.lnP0RT);                 // k / Kc, ln Kc = -dG + dnu ln(P0/RT)
         dlnKc = (dH - rd[10]) * invT;
     }
     WS(t.w_K, 2 * j) = kf;
