@@ -129,6 +129,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (1-based); default 2 = configs[1]")
     ap.add_argument("--cells", type=int, default=0, help="override the cell count (0 = the config's)")
+    ap.add_argument("--call", default="jac+wdot", choices=["jac+wdot", "jac", "wdot"],
+                    help="which C-ABI call a step is: qss_eval_jac with wdot output (the metric), qss_eval_jac alone, qss_eval_wdot alone")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
@@ -167,8 +169,15 @@ def main():
     qm.workspace(True)
     stream = torch.cuda.current_stream()
 
+    qm.workspace(False)
+
     def step():
-        qm.eval_jac(Cd, Td, n, jac=J, wdot=W, want_wdot=True)
+        if args.call == "jac+wdot":
+            qm.eval_jac(Cd, Td, n, jac=J, wdot=W, want_wdot=True)
+        elif args.call == "jac":
+            qm.eval_jac(Cd, Td, n, jac=J)
+        else:
+            qm.eval_wdot(Cd, Td, n, wdot=W)
 
     def barrier():
         if dist is not None:
@@ -202,7 +211,7 @@ def main():
 
     # ---- end to end through the C-ABI host-buffer call: pinned host buffers, H2D + D2H inside the timed region
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and args.call == "jac+wdot":
         del J, W
         torch.cuda.empty_cache()
         Ch = torch.from_numpy(C).pin_memory(); Th = torch.from_numpy(T).pin_memory()
@@ -231,8 +240,12 @@ def main():
     hbm_gbs, peak_src, sm_max_mhz = _peaks()
     info = qm.info
     avg_s = statistics.mean(launch_ms) * 1e-3
-    bytes_launch = (info.bytes_jac + 8.0 * N) * n            # + wdot written
-    slots_launch = info.slots_jac * n
+    if args.call == "wdot":
+        bytes_cell, slots_cell = info.bytes_wdot, info.slots_wdot
+    else:
+        bytes_cell, slots_cell = info.bytes_jac + (8.0 * N if args.call == "jac+wdot" else 0.0), info.slots_jac
+    bytes_launch = bytes_cell * n
+    slots_launch = slots_cell * n
     fp64_peak_slots = sms * FP64_LANES_PER_SM * sm_max_mhz * 1e6
     t_hbm = bytes_launch / (hbm_gbs * 1e9); t_alu = slots_launch / fp64_peak_slots
     if t_alu >= t_hbm:
@@ -244,13 +257,14 @@ def main():
     try:        # bytes of one launch from the committed ncu capture of the same workload and kernel variant, else null
         with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
             tj = json.load(f)
-        if tj["cfg"] == cfg and tj["cells"] == n and tj["kernel_variant"] == info.kernel_variant_jac:
+        if args.call == "jac+wdot" and tj["cfg"] == cfg and tj["cells"] == n and tj["kernel_variant"] == info.kernel_variant_jac:
             traffic = tj["dram_bytes_per_launch"]
     except Exception:
         traffic = None
-    roof.update({"traffic": traffic, "traffic_unit": "bytes per launch (dram read + write, ncu)", "kernel": "qss jacobian kernel (qss_eval_jac, wdot output on)",
+    roof.update({"traffic": traffic, "traffic_unit": "bytes per launch (dram read + write, ncu)", "kernel": {"jac+wdot": "qss jacobian kernel (qss_eval_jac, wdot output on)", "jac": "qss jacobian kernel (qss_eval_jac)",
+                            "wdot": "qss wdot kernel (qss_eval_wdot)"}[args.call],
                  "launch_ms_avg": avg_s * 1e3, "launch_ms_min": min(launch_ms),
-                 "alg_fp64_slots_per_cell": info.slots_jac, "alg_bytes_per_cell": info.bytes_jac + 8.0 * N,
+                 "alg_fp64_slots_per_cell": slots_cell, "alg_bytes_per_cell": bytes_cell,
                  "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3,
                  "hbm_achieved_gbs": bytes_launch / avg_s / 1e9, "hbm_frac": bytes_launch / avg_s / 1e9 / hbm_gbs,
                  "peak_source": f"alu: {sms} SMs x {FP64_LANES_PER_SM} fp64 FMA lanes x {sm_max_mhz:.0f} MHz (nominal; DESIGN.md); "
@@ -275,7 +289,7 @@ def main():
         "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic", "config": _config(cfg, mech, n, world),
         "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps, "roofline": roof, "cpu_baseline": cpu,
-        "kernel_variant": {"wdot": info.kernel_variant_wdot, "jac": info.kernel_variant_jac}}))
+        "kernel_variant": {"wdot": info.kernel_variant_wdot, "jac": info.kernel_variant_jac}, "call": args.call}))
     if dist is not None:
         dist.destroy_process_group()
 
