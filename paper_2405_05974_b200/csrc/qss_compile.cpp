@@ -148,12 +148,10 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     }
     // V rows: transported s -> s, the constant 1 -> N, QSS q -> N + 1 + q
     auto vrow = [&](int sp) { return sp < N ? sp : N + 1 + (sp - N); };
-    {   // per reaction: V rows of the QSS reactant of each direction (or the 1.0 row), third-body index
-        v.h_q = at();
-        for (int j = 0; j < M; ++j) {
-            const int qf = R[j].q[0] >= 0 ? N + 1 + R[j].q[0] : N, qb = R[j].q[1] >= 0 ? N + 1 + R[j].q[1] : N;
-            H.push_back(qf | (qb << 8) | ((R[j].tb + 1) << 16));
-        }
+    std::vector<int32_t> q_tab;                            // per reaction: V rows of the QSS reactant of each direction (or the
+    for (int j = 0; j < M; ++j) {                          //   1.0 row), third-body index; staged in shared memory
+        const int qf = R[j].q[0] >= 0 ? N + 1 + R[j].q[0] : N, qb = R[j].q[1] >= 0 ? N + 1 + R[j].q[1] : N;
+        q_tab.push_back(qf | (qb << 8) | ((R[j].tb + 1) << 16));
     }
     const int nw = QSS_V1_NW;
     // species incidence lists (their balanced assignment to warps follows below): one entry per unit of |nu|,
@@ -203,13 +201,15 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     v.s_V = take(N + 1 + Nq); v.s_CT = take(1); v.s_CL = take(c.cl_size); v.s_XP = take(v.n_xp); v.s_TV = take(nsp); v.s_Z0 = take(1);
     const int max_rows = (227 * 1024) / 256;
     const int region = std::max((nsp + 1) * nw, 2 * M + 2 * (nsp + 1));    // round buffers: nsp rows + 1 junk row per column
+    if (c.n_tb > 2 * (nsp + 1)) { why = "more third-body reactions than the shared-memory rows that hold dQ/dM for the species sums"; return false; }
     if (rows_fixed + region > max_rows) { why = "per-cell state does not fit the shared memory of one SM"; return false; }
     v.nw = nw;
     v.s_WX = rows_fixed; v.s_YC = rows_fixed + N * nw;       // one column buffer: row (species) r of column w at r * nw + w
     v.s_KAP = rows_fixed; v.s_G = rows_fixed + 2 * M; v.s_H = v.s_G + nsp + 1;
     // the W_y assembly lists are staged once per block in the spare shared memory behind the per-cell rows
     v.t_ce_ptr = (int32_t)(wya_ptr.size() + wya_all.size()); v.t_ce_dst = v.t_ce_ptr + v.n_centry + 1; v.t_ce_dir = v.t_ce_dst + v.n_centry;
-    v.n_tab_words = (int32_t)(wya_ptr.size() + wya_all.size() + ce_tab.size());
+    v.t_q = (int32_t)(wya_ptr.size() + wya_all.size() + ce_tab.size());
+    v.n_tab_words = v.t_q + (int32_t)q_tab.size();
     v.s_TAB = rows_fixed + region;
     v.smem_rows = v.s_TAB + (v.n_tab_words * 4 + 255) / 256;
     if (v.smem_rows > max_rows) { why = "per-cell state and staged tables do not fit the shared memory of one SM"; return false; }
@@ -411,6 +411,7 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         v.i_wya_ptr = (int32_t)I.size(); I.insert(I.end(), wya_ptr.begin(), wya_ptr.end());   // [n_wy + 1] then the words
         I.insert(I.end(), wya_all.begin(), wya_all.end());
         I.insert(I.end(), ce_tab.begin(), ce_tab.end());
+        I.insert(I.end(), q_tab.begin(), q_tab.end());
     }
     // ---- reaction records (appended to the int blob), in processing order
     {

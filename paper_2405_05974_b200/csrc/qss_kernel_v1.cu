@@ -40,6 +40,12 @@ __device__ __forceinline__ double lds(unsigned a) {
     return v;
 }
 __device__ __forceinline__ void sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
+// scratch-slab read pinned where it is written in the source (the prefetch distance is the point)
+__device__ __forceinline__ double ldg_pin(const double *q) {
+    double v;
+    asm volatile("ld.global.f64 %0, [%1];" : "=d"(v) : "l"(q) : "memory");
+    return v;
+}
 __device__ __forceinline__ int2 ldc2(const int32_t *q) { return *reinterpret_cast<const int2 *>(q); }
 // mechanism tables in global memory: read-only loads with an L2 evict_last policy, so that the 10 GB of Jacobian
 // entries streaming through the L2 do not push the (tiny, re-read by every block for every slab) tables out to DRAM
@@ -278,18 +284,37 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             __syncthreads();
             QSS_TICK(4);
         }
-        // ---- P5: net rates of progress Q_j (Eq. 2), dQ/dT at fixed y and M, dQ/dM
-        for (int j = warp; j < M; j += nw) {
-            const int w = HT(p.h_q, j);
-            const double rf = SM(p.s_KAP, 2 * j) * SM(p.s_V, w & 255);
-            const double rb = SM(p.s_KAP, 2 * j + 1) * SM(p.s_V, (w >> 8) & 255);
-            const double Q = rf - rb;
-            SM(p.s_KAP, 2 * j) = Q;                                 // Q_j and dQ_j/dT replace the two kappas in place
-            if (JAC) {
-                const double qt = Q * SC(p.g_DF, j) + rb * SC(p.g_DC, j);
-                SM(p.s_KAP, 2 * j + 1) = qt;
-                const int tb = (w >> 16) - 1;
-                if (tb >= 0) SC(p.g_QM, tb) *= Q;
+        // ---- P5: net rates of progress Q_j (Eq. 2), dQ/dT at fixed y and M, dQ/dM.  dlnk/dT, dlnKc/dT and dlnk/dM are L2
+        //      reads (~700 cycles): those of 8 of the warp's reactions are in flight together.  dQ/dM goes to the scratch
+        //      slab (the column streams read it) and to the dead g/RT rows of shared memory (the species sums read it).
+        for (int j0 = warp; j0 < M; j0 += 8 * nw) {
+            int wq[8];
+            double df[8], dc[8], qm[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int j = j0 + u * nw;
+                wq[u] = j < M ? tab[p.t_q + j] : 0;
+                df[u] = dc[u] = qm[u] = 0.0;
+                if (JAC && j < M) {
+                    df[u] = ldg_pin(&SC(p.g_DF, j)); dc[u] = ldg_pin(&SC(p.g_DC, j));
+                    if ((wq[u] >> 16) > 0) qm[u] = ldg_pin(&SC(p.g_QM, (wq[u] >> 16) - 1));
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int j = j0 + u * nw;
+                if (j < M) {
+                    const int w = wq[u];
+                    const double rf = SM(p.s_KAP, 2 * j) * SM(p.s_V, w & 255);
+                    const double rb = SM(p.s_KAP, 2 * j + 1) * SM(p.s_V, (w >> 8) & 255);
+                    const double Q = rf - rb;
+                    SM(p.s_KAP, 2 * j) = Q;                         // Q_j and dQ_j/dT replace the two kappas in place
+                    if (JAC) {
+                        SM(p.s_KAP, 2 * j + 1) = Q * df[u] + rb * dc[u];
+                        const int tb = (w >> 16) - 1;
+                        if (tb >= 0) { SC(p.g_QM, tb) = qm[u] * Q; SM(p.s_G, tb) = qm[u] * Q; }
+                    }
+                }
             }
         }
         __syncthreads();
@@ -316,7 +341,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                     const int te = HT(p.h_st_ptr, s + 1);
                     for (int x = HT(p.h_st_ptr, s); x < te; ++x) {
                         const int e = HT(p.h_st, x), sg = e & 0x80000000;
-                        const double qm = SC(p.g_QM, e & 0x7fffffff);
+                        const double qm = SM(p.s_G, e & 0x7fffffff);
                         tv += __hiloint2double(__double2hiint(qm) ^ sg, __double2loint(qm));
                     }
                 }
@@ -348,8 +373,13 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                             for (int u = 0; u < 8; ++u) if (s0 + u < nsp) sts(colw + (s0 + u) * RS, t[u]);
                         }
                     } else {
-#pragma unroll 4
-                        for (int s = 0; s < nsp; ++s) sts(colw + s * RS, SC(p.g_ET, s));
+                        for (int s0 = 0; s0 < nsp; s0 += 16) {          // L2 reads: 16 in flight together
+                            double t[16];
+#pragma unroll
+                            for (int u = 0; u < 16; ++u) t[u] = ldg_pin(&SC(p.g_ET, min(s0 + u, nsp - 1)));
+#pragma unroll
+                            for (int u = 0; u < 16; ++u) if (s0 + u < nsp) sts(colw + (s0 + u) * RS, t[u]);
+                        }
                     }
                     QSS_TICK(11);
                     // column stream: part = |nu| * A * V[o1] * V[o2] (* val), added to / subtracted from up to 8 rows of the

@@ -42,6 +42,7 @@ struct QssV1 {
     int32_t s_KAP;      // [2M]      kappa_d; then in place Q_j (row 2j), dQ_j/dT (row 2j+1) }   (phases P2-P6)
     int32_t s_G, s_H;   // [nsp+1]   g/RT, h/RT (+ a zero row), after s_KAP                  }   (phases P1-P2)
     int32_t s_TAB;      // staged once per block (n_tab_words int32): the W_y assembly lists, then the closure gather lists
+    int32_t t_q;                                     //   offset of [M] qf | qb<<8 | (tb+1)<<16 (V rows of the QSS reactants) in it
     int32_t t_ce_ptr, t_ce_dst, t_ce_dir;            //   offsets of the closure gather pointers / destinations / kappa rows in it
     int32_t smem_rows;
     // ---- scratch rows
@@ -54,7 +55,6 @@ struct QssV1 {
     // ---- hot tables (offsets into h)
     int32_t h_xp_ptr, h_xp_dir, h_xp_m, h_xp_n;      // cross-group gather
     int32_t h_group, h_gmember, h_level_ptr;         // group records (8 words), members, levels
-    int32_t h_q;                                     // [M] qf | qb<<8 | (tb+1)<<16  (V rows of the QSS reactants)
     int32_t h_ssw_ptr, h_ssw;                        // species assigned to each warp (balanced)
     int32_t h_ss_ptr, h_ss;                          // species incidence: byte offset of Q_j in s_KAP | sign bit
     int32_t h_st_ptr, h_st;                          // third-body incidence: index of dQ_j/dM | sign bit
