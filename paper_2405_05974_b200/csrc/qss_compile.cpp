@@ -402,6 +402,23 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         v.h_cw = at();
         for (int i = 0; i < v.n_rounds * nw; ++i) H.push_back(i <= N ? idx[i] : -1);
     }
+    // ---- third-body efficiencies (alpha - 1) by reaction, in the constant bank: the rate phase walks them for every
+    //      third-body / fall-off reaction, and a walk through global memory is a chain of ~700-cycle L2 reads
+    std::vector<int> eff_first(M, 0), eff_count(M, 0);
+    {
+        std::vector<double> val; std::vector<uint32_t> off;
+        for (int j = 0; j < M; ++j) {
+            eff_first[j] = (int)val.size();
+            if (R[j].type >= 1) for (int k = 0; k < N; ++k) for (auto &e : (*c.effc)[k]) if (e.first == j) { val.push_back(e.second); off.push_back((uint32_t)voff(k)); }
+            eff_count[j] = (int)val.size() - eff_first[j];
+        }
+        if (val.size() > 65535) { why = "too many third-body efficiencies for variant 1"; return false; }
+        if (H.size() & 1) H.push_back(0);
+        v.h_eff_val = at();
+        for (double x : val) { int32_t w[2]; std::memcpy(w, &x, 8); H.push_back(w[0]); H.push_back(w[1]); }
+        v.h_eff_off = at();
+        for (size_t i = 0; i < off.size(); i += 2) H.push_back((int32_t)(off[i] | ((i + 1 < off.size() ? off[i + 1] : 0u) << 16)));
+    }
     if ((int)H.size() > QSS_V1_HMAX) { why = "hot tables exceed the kernel-parameter budget of variant 1"; return false; }
     v.h_used = (int32_t)H.size();
     std::memcpy(v.h, H.data(), H.size() * sizeof(int32_t));
@@ -422,7 +439,7 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
             const int j = (*c.rorder)[r];
             // w0 = j | type << 12 | mask << 14 | (tb + 1) << 16; w1..w3 = six 16-bit byte offsets of the V rows of the
             // reactant / product molecules (QSS and empty slots -> the 1.0 row); w4..w6 = six byte offsets (relative to
-            // s_G) of their g/RT rows (empty slots -> the zero row)
+            // s_G) of their g/RT rows (empty slots -> the zero row); w7 = first third-body efficiency | count << 16
             int32_t rec[QSS_V1_RREC] = {j | (R[j].type << 12) | (R[j].mask << 14) | ((R[j].tb + 1) << 16), 0, 0, 0, 0, 0, 0, 0};
             uint32_t kap[6], gr[6];
             for (int s = 0; s < 2; ++s) {
@@ -433,6 +450,7 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
                 }
             }
             for (int u = 0; u < 3; ++u) { rec[1 + u] = (int32_t)(kap[2 * u] | (kap[2 * u + 1] << 16)); rec[4 + u] = (int32_t)(gr[2 * u] | (gr[2 * u + 1] << 16)); }
+            rec[7] = eff_first[j] | (eff_count[j] << 16);        // third-body efficiencies of this reaction in h_eff_*
             I.insert(I.end(), rec, rec + QSS_V1_RREC);
         }
     }

@@ -167,8 +167,10 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                 const double iKc = qss_exp(dG - q10 * lnP0RT);      // 1 / Kc, ln Kc = -dG + dnu ln(P0/RT)
                 if (type >= 1) {
                     double Mc = Ctot;                              // M = sum_k alpha_k C_k, transported only (G7)
-                    const int e0 = ldg_keep(gI + p.i_eff_ptr + j, keep), e1 = ldg_keep(gI + p.i_eff_ptr + j + 1, keep);
-                    for (int e = e0; e < e1; ++e) Mc += ldg_keep(gD + p.d_effm1 + e, keep) * SM(p.s_V, ldg_keep(gI + p.i_eff_sp + e, keep));
+                    for (int e = rb.w & 0xffff, ee = e + ((unsigned)rb.w >> 16); e < ee; ++e) {
+                        const unsigned off = ((unsigned)HT(p.h_eff_off, e >> 1) >> ((e & 1) * 16)) & 0xffffu;
+                        Mc = fma(*reinterpret_cast<const double *>(&p.h[p.h_eff_val + 2 * e]), lds(sml + off), Mc);
+                    }
                     double dlm;
                     if (type == 1) {
                         k *= Mc;

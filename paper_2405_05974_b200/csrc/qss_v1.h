@@ -58,6 +58,7 @@ struct QssV1 {
     int32_t h_ssw_ptr, h_ssw;                        // species assigned to each warp (balanced)
     int32_t h_ss_ptr, h_ss;                          // species incidence: byte offset of Q_j in s_KAP | sign bit
     int32_t h_st_ptr, h_st;                          // third-body incidence: index of dQ_j/dM | sign bit
+    int32_t h_eff_val, h_eff_off;                    // third-body (alpha - 1) doubles; V-row byte offsets, two 16-bit per word
     int32_t h_cw;                                    // [n_rounds*nw] Jacobian column of (round, warp), -1: none
     int32_t h_cs_ptr, h_cs;                          // column streams (see qss_compile.cpp "column stream")
     int32_t h_sp;                                    // dy/dx solve program: n_sp_ops pairs of fixed-format row operations
