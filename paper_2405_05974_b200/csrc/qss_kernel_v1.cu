@@ -64,11 +64,6 @@ __device__ __forceinline__ double ldg_keep(const double *q, unsigned long long p
     asm volatile("ld.global.nc.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(q), "l"(pol));
     return v;
 }
-__device__ __forceinline__ int ldg_keep(const int *q, unsigned long long pol) {
-    int v;
-    asm volatile("ld.global.nc.L2::cache_hint.s32 %0, [%1], %2;" : "=r"(v) : "l"(q), "l"(pol));
-    return v;
-}
 
 // optional phase timing (QSS_TIMING=1): thread 0 of block 0 accumulates the cycles between block barriers
 #define QSS_TICK(ph)                                                                   \
