@@ -29,6 +29,8 @@ struct qss_mech {
     int nwarp = 8;            // warps per block of the slab kernel
     int blocks_per_sm = 4;    // general kernel: 4 x 8 warps per SM (64 registers); measured 193 -> 123 ms on cfg3 vs 2 blocks
     int nblocks = 0;
+    cudaStream_t copy_stream = nullptr;   // qss_eval_jac_host: device-to-host copies overlap the next chunk's kernel
+    cudaEvent_t ev[2] = {nullptr, nullptr};
     long long *timing = nullptr;   // device counters when QSS_TIMING=1 (variant 1 only)
     int variant = 0;          // 0: general slab kernel (workspace in global memory); 1: slab-smem kernel (qss_kernel_v1.cu)
 };
@@ -139,6 +141,7 @@ extern "C" int qss_mech_destroy(qss_mech_t *m) {
         }
         cudaFree(m->timing);
     }
+    if (m->copy_stream) { cudaStreamDestroy(m->copy_stream); cudaEventDestroy(m->ev[0]); cudaEventDestroy(m->ev[1]); }
     cudaFree(m->dI); cudaFree(m->dD);
     delete m;
     return QSS_OK;
@@ -228,12 +231,31 @@ extern "C" int qss_eval_jac_host(const qss_mech_t *m, int64_t ncells, int64_t ld
     void *ws = p;
     cudaStream_t s = (cudaStream_t)stream;
     cudaError_t e;
-    if ((e = cudaMemcpyAsync(dC, Ch, N * L, cudaMemcpyHostToDevice, s)) != cudaSuccess) return cuda_fail(e, "H2D C");
+    // Pipelined over chunks of cells: the kernel of chunk c runs on `stream` while the Jacobian of chunk c-1 streams back
+    // to the host on an internal copy stream (the device-to-host copy of N(N+1) doubles per cell dominates the call).
+    // The SoA arrays are copied as 2D blocks: `rows` rows of `chunk` cells with row pitch ld.
+    qss_mech *mm = const_cast<qss_mech *>(m);
+    DeviceGuard guard(m->device);
+    if (!mm->copy_stream) {
+        if ((e = cudaStreamCreateWithFlags(&mm->copy_stream, cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(e, "cudaStreamCreate");
+        for (int i = 0; i < 2; ++i)
+            if ((e = cudaEventCreateWithFlags(&mm->ev[i], cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e, "cudaEventCreate");
+    }
+    const int64_t nchunk = ncells >= (1 << 16) ? 8 : 1;
+    const int64_t chunk = ((ncells + nchunk - 1) / nchunk + 31) / 32 * 32;
     if ((e = cudaMemcpyAsync(dT, Th, L, cudaMemcpyHostToDevice, s)) != cudaSuccess) return cuda_fail(e, "H2D T");
-    int rc = qss_eval_jac(m, ncells, ld, dC, dT, dJ, wdoth ? dW : nullptr, ws, ws_bytes(m, true), stream);
-    if (rc != QSS_OK) return rc;
-    if ((e = cudaMemcpyAsync(jach, dJ, N * (N + 1) * L, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return cuda_fail(e, "D2H jac");
-    if (wdoth && (e = cudaMemcpyAsync(wdoth, dW, N * L, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return cuda_fail(e, "D2H wdot");
+    for (int64_t c0 = 0; c0 < ncells; c0 += chunk) {
+        const int64_t nc = std::min(chunk, ncells - c0);
+        const size_t wbytes = (size_t)nc * sizeof(double);
+        if ((e = cudaMemcpy2DAsync(dC + c0, L, Ch + c0, L, wbytes, N, cudaMemcpyHostToDevice, s)) != cudaSuccess) return cuda_fail(e, "H2D C");
+        int rc = qss_eval_jac(m, nc, ld, dC + c0, dT + c0, dJ + c0, wdoth ? dW + c0 : nullptr, ws, ws_bytes(m, true), stream);
+        if (rc != QSS_OK) return rc;
+        if ((e = cudaEventRecord(mm->ev[0], s)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
+        if ((e = cudaStreamWaitEvent(mm->copy_stream, mm->ev[0], 0)) != cudaSuccess) return cuda_fail(e, "cudaStreamWaitEvent");
+        if ((e = cudaMemcpy2DAsync(jach + c0, L, dJ + c0, L, wbytes, N * (N + 1), cudaMemcpyDeviceToHost, mm->copy_stream)) != cudaSuccess) return cuda_fail(e, "D2H jac");
+        if (wdoth && (e = cudaMemcpy2DAsync(wdoth + c0, L, dW + c0, L, wbytes, N, cudaMemcpyDeviceToHost, mm->copy_stream)) != cudaSuccess) return cuda_fail(e, "D2H wdot");
+    }
+    if ((e = cudaStreamSynchronize(mm->copy_stream)) != cudaSuccess) return cuda_fail(e, "cudaStreamSynchronize(copy)");
     if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return cuda_fail(e, "cudaStreamSynchronize");
     return QSS_OK;
 }

@@ -161,6 +161,26 @@ def test_non_default_stream_graph_capture_and_padding():
     gates.assert_jac(J.cpu().numpy(), ref["jac"], ref["jscale"], n, "graph replay jac")
 
 
+def test_host_buffer_call_matches_the_device_call():
+    """qss_eval_jac_host (pinned host buffers, chunked copy/compute pipeline) returns exactly what qss_eval_jac does."""
+    import paper_2405_05974_b200 as qss
+    torch = _torch()
+    mech = qss_synth.config_mechanism(1)
+    n = 70000 + 13                                         # > 2^16 cells: 8 chunks with a ragged last one
+    C, T = make_states(mech.n_nqss, n, seed=31)
+    ld = C.shape[1]
+    qm = qss.QssMech(mech, 0)
+    J0, w0 = qm.eval_jac(torch.from_numpy(C).cuda(), torch.from_numpy(T).cuda(), n, want_wdot=True)
+    torch.cuda.synchronize()
+    Ch = torch.from_numpy(C).pin_memory(); Th = torch.from_numpy(T).pin_memory()
+    Jh = torch.full((qm.N, qm.N + 1, ld), float("nan"), dtype=torch.float64).pin_memory()
+    Wh = torch.full((qm.N, ld), float("nan"), dtype=torch.float64).pin_memory()
+    scratch = torch.empty(qm.host_scratch_bytes(n, ld) + 256, dtype=torch.uint8, device="cuda")
+    qm.eval_jac_host(Ch, Th, Jh, Wh, scratch, n)
+    assert torch.equal(Jh[:, :, :n], J0[:, :, :n].cpu()) and torch.equal(Wh[:, :n], w0[:, :n].cpu())
+    assert torch.isnan(Jh[:, :, n:]).all() and torch.isnan(Wh[:, n:]).all()
+
+
 def test_zero_cells_is_a_noop():
     import paper_2405_05974_b200 as qss
     torch = _torch()
