@@ -112,7 +112,9 @@ int qss_eval_jac(const qss_mech_t *mech, int64_t ncells, int64_t ld, const doubl
 
 /* Host-buffer convenience used for end-to-end timing: copies C and T to the device (in `dev_scratch`, which
  * must hold qss_host_scratch_bytes() bytes), evaluates, copies the Jacobian (and wdot if not NULL) back to
- * the HOST buffers, and synchronises `stream`.  Host buffers should be pinned for full copy bandwidth. */
+ * the HOST buffers, and synchronises `stream`.  Host buffers should be pinned for full copy bandwidth.  Large batches are
+ * pipelined in chunks of cells: kernels run on `stream`, the copies back run on a stream owned by the handle (created on
+ * first use, released by qss_mech_destroy), so this call is not capturable in a CUDA graph and not re-entrant per handle. */
 size_t qss_host_scratch_bytes(const qss_mech_t *mech, int64_t ncells, int64_t ld);
 int qss_eval_jac_host(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *C_host,
                       const double *T_host, double *jac_host, double *wdot_host_or_null,
