@@ -209,6 +209,32 @@ def test_bad_arguments_are_rejected():
     assert e.value.code == -1
 
 
+@pytest.mark.parametrize("cfg,nsample", [(3, 128), (4, 128), (5, 48)])
+def test_full_size_other_configs_sampled(cfg, nsample):
+    """BASELINE.json configs[2], [3], [4] at their full sizes (2^19 cells, the 128^3 field, 2^18 cells) in the launch
+    configuration bench.py uses; sampled cells (first, last, random) are recomputed one by one by the oracle and every
+    output must be finite."""
+    import paper_2405_05974_b200 as qss
+    torch = _torch()
+    mech = qss_synth.config_mechanism(cfg)
+    C, T = qss_synth.config_states(cfg)
+    n = qss_synth.CONFIGS[cfg]["n_cells"]
+    qm = qss.QssMech(mech, 0)
+    Cd = torch.from_numpy(np.ascontiguousarray(C)).cuda(); Td = torch.from_numpy(np.ascontiguousarray(T)).cuda()
+    J, w = qm.eval_jac(Cd, Td, n, want_wdot=True)
+    torch.cuda.synchronize()
+    assert torch.isfinite(w[:, :n]).all() and torch.isfinite(J[:, :, :n]).all()
+    idx = np.sort(np.random.default_rng(100 + cfg).choice(n, size=nsample, replace=False))
+    idx[0], idx[-1] = 0, n - 1
+    it = torch.from_numpy(idx).cuda()
+    Js = J[:, :, it].cpu().numpy(); ws = w[:, it].cpu().numpy()
+    del J, w
+    Cs = np.ascontiguousarray(C[:, idx]); Ts = np.ascontiguousarray(T[idx])
+    ref = oracle.evaluate(oracle.OracleMech(mech), Cs, Ts, want_jac=True, want_scale=True)
+    gates.assert_wdot(ws, ref["wdot"], ref["S"], what=f"cfg{cfg} full wdot")
+    gates.assert_jac(Js, ref["jac"], ref["jscale"], what=f"cfg{cfg} full jac")
+
+
 def test_full_size_cfg2_sampled():
     """BASELINE.json configs[1] at full size (2^20 cells) in the launch configuration bench.py times;
     256 sampled cells are recomputed one by one by the oracle."""
