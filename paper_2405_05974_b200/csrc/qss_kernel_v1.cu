@@ -401,9 +401,10 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
 #define QSS_ROWS(w, q0, q1, q2, q3)                                                      \
     const unsigned q0 = colw + ((w) & 127) * RS, q1 = colw + (((w) >> 8) & 127) * RS,    \
                    q2 = colw + (((w) >> 16) & 127) * RS, q3 = colw + (((w) >> 24) & 127) * RS
+#define QSS_SIGNED(pt, w, sh) __hiloint2double(__double2hiint(pt) ^ (int)(((w) << (sh)) & 0x80000000u), __double2loint(pt))
 #define QSS_APPLY(w, q0, q1, q2, q3, v0, v1, v2, v3, pt)                                 \
-    sts(q0, v0 + (((w) & 0x80u) ? -pt : pt)); sts(q1, v1 + (((w) & 0x8000u) ? -pt : pt)); \
-    sts(q2, v2 + (((w) & 0x800000u) ? -pt : pt)); sts(q3, v3 + (((w) & 0x80000000u) ? -pt : pt))
+    sts(q0, v0 + QSS_SIGNED(pt, w, 24)); sts(q1, v1 + QSS_SIGNED(pt, w, 16));            \
+    sts(q2, v2 + QSS_SIGNED(pt, w, 8)); sts(q3, v3 + QSS_SIGNED(pt, w, 0))
                         double own = 0.0;                                 // contributions to the column's own row k
                         int2 sa0, sb0, sa1, sb1, ma0, mb0, ma1, mb1;
                         double tA, tV, mA0, mV0, mA1, mV1, part0, part1;
@@ -469,6 +470,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
 #undef QSS_PART
 #undef QSS_ROWS
 #undef QSS_APPLY
+#undef QSS_SIGNED
                     }
                     QSS_TICK(12);
                     // dy/dx solve program: pairs of independent fixed-format row operations
