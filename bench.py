@@ -255,7 +255,7 @@ def main():
     roof["frac"] = roof["achieved"] / roof["peak"]
     traffic = None
     try:        # bytes of one launch from the committed ncu capture of the same workload and kernel variant, else null
-        with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
+        with open(os.path.join(ROOT, "profiles", "r01_traffic.txt")) as f:
             tj = json.load(f)
         if args.call == "jac+wdot" and tj["cfg"] == cfg and tj["cells"] == n and tj["kernel_variant"] == info.kernel_variant_jac:
             traffic = tj["dram_bytes_per_launch"]
