@@ -132,12 +132,12 @@ extern "C" int qss_mech_destroy(qss_mech_t *m) {
     DeviceGuard guard(m->device);
     if (m->timing) {
         long long t[16];
-        static const char *name[14] = {"P0 stage", "P1 thermo", "P2 rates", "P3+P7 gather", "P4 closure", "P5 net rates", "P6 sums", "A: barrier wait", "B: barrier wait",
-                                        "B: tile", "B: stores", "A: init", "A: stream", "A: solve"};
+        static const char *name[15] = {"P0 stage", "P1 thermo", "P2 Arrhenius+wait", "P3+P7 gather", "P4 closure", "P5 net rates", "P6 sums", "A: barrier wait", "B: barrier wait",
+                                        "B: tile", "B: stores", "A: init", "A: stream", "A: solve", "P2 third-body/fall-off"};
         if (cudaMemcpy(t, m->timing, sizeof t, cudaMemcpyDeviceToHost) == cudaSuccess) {
             long long tot = 0;
-            for (int i = 0; i < 14; ++i) tot += t[i];
-            for (int i = 0; i < 14 && tot > 0; ++i) std::fprintf(stderr, "[qss timing] %-14s %6.2f %%\n", name[i], 100.0 * (double)t[i] / (double)tot);
+            for (int i = 0; i < 15; ++i) tot += t[i];
+            for (int i = 0; i < 15 && tot > 0; ++i) std::fprintf(stderr, "[qss timing] %-14s %6.2f %%\n", name[i], 100.0 * (double)t[i] / (double)tot);
         }
         cudaFree(m->timing);
     }

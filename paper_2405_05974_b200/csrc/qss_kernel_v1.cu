@@ -129,24 +129,30 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             // fetched (L2 reads, the L1 is a few KB next to the shared memory) before the current one is evaluated
             int4 nra = make_int4(0, 0, 0, 0), nrb = nra;
             double nq0 = 0.0, nq1 = 0.0, nq2 = 0.0, nq10 = 0.0;
-            if (warp < M) {
+            const int n_typed = p.n_tb;                            // third-body and fall-off reactions come first
+            if (warp < n_typed) {
                 nra = ldg_keep(reinterpret_cast<const int4 *>(gI + p.i_rrec + warp * QSS_V1_RREC), keep);
                 nrb = ldg_keep(reinterpret_cast<const int4 *>(gI + p.i_rrec + warp * QSS_V1_RREC + 4), keep);
                 const double *rn = gD + p.d_rate_r + warp * QSS_RD_STRIDE;
                 nq0 = ldg_keep(rn, keep); nq1 = ldg_keep(rn + 1, keep); nq2 = ldg_keep(rn + 2, keep); nq10 = ldg_keep(rn + 10, keep);
             }
 #pragma unroll 1
-            for (int r = warp; r < M; r += nw) {
+            for (int r = warp; r < n_typed; r += nw) {
                 const int4 ra = nra, rb = nrb;
                 const double q0 = nq0, q1 = nq1, q2 = nq2, q10 = nq10;
                 const double *rd = gD + p.d_rate_r + r * QSS_RD_STRIDE;
-                if (r + nw < M) {
+                if (r + nw < n_typed) {
                     nra = ldg_keep(reinterpret_cast<const int4 *>(gI + p.i_rrec + (r + nw) * QSS_V1_RREC), keep);
                     nrb = ldg_keep(reinterpret_cast<const int4 *>(gI + p.i_rrec + (r + nw) * QSS_V1_RREC + 4), keep);
                     const double *rn = rd + nw * QSS_RD_STRIDE;
                     nq0 = ldg_keep(rn, keep); nq1 = ldg_keep(rn + 1, keep); nq2 = ldg_keep(rn + 2, keep); nq10 = ldg_keep(rn + 10, keep);
                 }
                 const int j = ra.x & 4095, type = (ra.x >> 12) & 3, mask = (ra.x >> 14) & 3, tb = (ra.x >> 16) - 1;
+                double t3 = 0.0, t4 = 0.0, t5 = 0.0, t6 = 0.0, t7 = 0.0, t8 = 0.0, t9 = 0.0;   // fall-off parameters (L2 reads, issued early)
+                if (type == 2) {
+                    t3 = ldg_keep(rd + 3, keep); t4 = ldg_keep(rd + 4, keep); t5 = ldg_keep(rd + 5, keep); t6 = ldg_keep(rd + 6, keep);
+                    t7 = ldg_keep(rd + 7, keep); t8 = ldg_keep(rd + 8, keep); t9 = ldg_keep(rd + 9, keep);
+                }
                 // all shared-memory reads of the reaction first, then the two exponentials side by side (two independent
                 // Horner chains), then the type-specific factor
                 const unsigned g0 = rb.x & 0xffff, g1 = (unsigned)rb.x >> 16, g2 = rb.y & 0xffff;      // reactant molecules
@@ -171,10 +177,10 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                         k *= Mc;
                         dlm = qss_rcp(Mc);
                     } else {                                       // Troe fall-off
-                        const double lnk0 = ldg_keep(rd + 3, keep) + ldg_keep(rd + 4, keep) * lnT - ldg_keep(rd + 5, keep) * invT;
-                        const double dlnk0 = (ldg_keep(rd + 4, keep) + ldg_keep(rd + 5, keep) * invT) * invT;
+                        const double lnk0 = t3 + t4 * lnT - t5 * invT;
+                        const double dlnk0 = (t4 + t5 * invT) * invT;
                         const double Pr = qss_exp(lnk0 - lnkinf) * Mc;
-                        const double al = ldg_keep(rd + 6, keep), i3 = ldg_keep(rd + 7, keep), i1 = ldg_keep(rd + 8, keep), T2s = ldg_keep(rd + 9, keep);
+                        const double al = t6, i3 = t7, i1 = t8, T2s = t9;
                         const double e3 = qss_exp(-T * i3), e1x = qss_exp(-T * i1), e2 = qss_exp(-T2s * invT);
                         const double Fc = (1.0 - al) * e3 + al * e1x + e2;
                         const double L = log(Pr) * kInvLn10, Lc = log(Fc) * kInvLn10;
@@ -209,6 +215,60 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                 sts(kbase + j * 512 + 256, kb * vb);
                 if (JAC) { SC(p.g_DF, j) = dlnk; SC(p.g_DC, j) = dlnKc; }
             }
+                    QSS_TICK(14);
+            // Arrhenius reactions, two at a time (four independent exponential chains): reads of both, arithmetic, stores
+#define QSS_RX_FETCH(R_, A_, B_, Q0_, Q1_, Q2_, Q10_)                                                            \
+    if ((R_) < M) {                                                                                              \
+        A_ = ldg_keep(reinterpret_cast<const int4 *>(gI + p.i_rrec + (R_) * QSS_V1_RREC), keep);                   \
+        B_ = ldg_keep(reinterpret_cast<const int4 *>(gI + p.i_rrec + (R_) * QSS_V1_RREC + 4), keep);               \
+        const double *rn_ = gD + p.d_rate_r + (size_t)(R_) * QSS_RD_STRIDE;                                       \
+        Q0_ = ldg_keep(rn_, keep); Q1_ = ldg_keep(rn_ + 1, keep); Q2_ = ldg_keep(rn_ + 2, keep); Q10_ = ldg_keep(rn_ + 10, keep); \
+    }
+#define QSS_RX_READ(A_, B_, DG_, DH_, VF_, VB_)                                                                   \
+    const double DG_ = (lds(gbase + ((unsigned)B_.y >> 16)) + lds(gbase + (B_.z & 0xffff)) + lds(gbase + ((unsigned)B_.z >> 16))) -  \
+                       (lds(gbase + (B_.x & 0xffff)) + lds(gbase + ((unsigned)B_.x >> 16)) + lds(gbase + (B_.y & 0xffff)));        \
+    double DH_ = 0.0;                                                                                             \
+    if (JAC) DH_ = (lds(hbase + ((unsigned)B_.y >> 16)) + lds(hbase + (B_.z & 0xffff)) + lds(hbase + ((unsigned)B_.z >> 16))) -    \
+                   (lds(hbase + (B_.x & 0xffff)) + lds(hbase + ((unsigned)B_.x >> 16)) + lds(hbase + (B_.y & 0xffff)));            \
+    const double VF_ = lds(sml + (A_.y & 0xffff)) * lds(sml + ((unsigned)A_.y >> 16)) * lds(sml + (A_.z & 0xffff));                \
+    const double VB_ = lds(sml + ((unsigned)A_.z >> 16)) * lds(sml + (A_.w & 0xffff)) * lds(sml + ((unsigned)A_.w >> 16))
+#define QSS_RX_STORE(A_, Q1_, Q2_, Q10_, K_, IKC_, DH_, VF_, VB_)                                                 \
+    {                                                                                                             \
+        const int j_ = A_.x & 4095, mask_ = (A_.x >> 14) & 3;                                                     \
+        const double kf_ = (mask_ & 1) ? K_ : 0.0, kb_ = (mask_ & 2) ? K_ * IKC_ : 0.0;                           \
+        SC(p.g_K, 2 * j_) = kf_; SC(p.g_K, 2 * j_ + 1) = kb_;                                                     \
+        sts(kbase + j_ * 512, kf_ * VF_); sts(kbase + j_ * 512 + 256, kb_ * VB_);                                 \
+        if (JAC) { SC(p.g_DF, j_) = (Q1_ + Q2_ * invT) * invT; SC(p.g_DC, j_) = (mask_ & 2) ? (DH_ - Q10_) * invT : 0.0; } \
+    }
+            {
+                int4 xa = make_int4(0, 0, 0, 0), xb = xa, ya = xa, yb = xa;
+                double xq0 = 0.0, xq1 = 0.0, xq2 = 0.0, xq10 = 0.0, yq0 = 0.0, yq1 = 0.0, yq2 = 0.0, yq10 = 0.0;
+                int r = n_typed + warp;
+                QSS_RX_FETCH(r, xa, xb, xq0, xq1, xq2, xq10)
+                QSS_RX_FETCH(r + nw, ya, yb, yq0, yq1, yq2, yq10)
+#pragma unroll 1
+                for (; r < M; r += 2 * nw) {
+                    const int4 a0 = xa, b0 = xb, a1 = ya, b1 = yb;
+                    const double p0 = xq0, p1 = xq1, p2 = xq2, p10 = xq10, s0 = yq0, s1 = yq1, s2 = yq2, s10 = yq10;
+                    const bool two = r + nw < M;
+                    QSS_RX_FETCH(r + 2 * nw, xa, xb, xq0, xq1, xq2, xq10)
+                    QSS_RX_FETCH(r + 3 * nw, ya, yb, yq0, yq1, yq2, yq10)
+                    QSS_RX_READ(a0, b0, dG0, dH0, vf0, vb0);
+                    if (two) {
+                        QSS_RX_READ(a1, b1, dG1, dH1, vf1, vb1);
+                        const double k0 = qss_exp(p0 + p1 * lnT - p2 * invT), k1 = qss_exp(s0 + s1 * lnT - s2 * invT);
+                        const double i0 = qss_exp(dG0 - p10 * lnP0RT), i1 = qss_exp(dG1 - s10 * lnP0RT);
+                        QSS_RX_STORE(a0, p1, p2, p10, k0, i0, dH0, vf0, vb0)
+                        QSS_RX_STORE(a1, s1, s2, s10, k1, i1, dH1, vf1, vb1)
+                    } else {
+                        const double k0 = qss_exp(p0 + p1 * lnT - p2 * invT), i0 = qss_exp(dG0 - p10 * lnP0RT);
+                        QSS_RX_STORE(a0, p1, p2, p10, k0, i0, dH0, vf0, vb0)
+                    }
+                }
+            }
+#undef QSS_RX_FETCH
+#undef QSS_RX_READ
+#undef QSS_RX_STORE
         }
         __syncthreads();
         QSS_TICK(2);
