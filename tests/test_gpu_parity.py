@@ -131,6 +131,20 @@ def test_zero_concentrations_and_tmid_tie_break():
     print(g)
 
 
+def test_paper_style_sampling():
+    """States drawn the way the paper validates its Jacobian: C ~ U[1e-4, 1] mol/m^3 for every
+    species, T ~ U[300, 1300] K (both NASA ranges, very small rate constants at the cold end)."""
+    mech = qss_synth.config_mechanism(2)
+    n = 512 + 3
+    rng = np.random.default_rng(42)
+    ld = (n + 31) // 32 * 32
+    C = np.empty((mech.n_nqss, ld)); T = np.empty(ld)
+    C[:, :n] = rng.uniform(1e-4, 1.0, size=(mech.n_nqss, n)); T[:n] = rng.uniform(300.0, 1300.0, size=n)
+    C[:, n:] = C[:, :1]; T[n:] = T[0]
+    g = _check(mech, C, T, n, "cfg2 paper-style states")
+    print(g)
+
+
 def test_non_default_stream_graph_capture_and_padding():
     """qss_eval_* only enqueue on the caller's stream: a captured CUDA graph replays to the same result; ld > ncells
     with a large pad leaves the padding untouched."""
