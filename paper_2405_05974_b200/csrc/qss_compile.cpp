@@ -106,7 +106,7 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         for (int s = 0; s < 2; ++s) { int n = 0; for (const Term &x : R[j].side[s]) n += x.nu; if (n > 3) { why = "a reaction side has more than 3 molecules"; return false; } }
         for (const Term &x : R[j].net) if (x.nu < -7 || x.nu > 7) { why = "net stoichiometric coefficient out of range"; return false; }
     }
-    std::vector<int32_t> H, ce_tab;
+    std::vector<int32_t> H, ce_tab, cs_words;
     auto at = [&]() { return (int32_t)H.size(); };
     // closure gather
     {
@@ -294,7 +294,7 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         ptr.push_back((int32_t)all.size());                  // the T column has an empty stream
         // two harmless sentinel pairs: the kernel's software pipeline fetches two pairs ahead of the one it applies
         for (int u = 0; u < 4; ++u) all.insert(all.end(), null_rec, null_rec + 4);
-        v.h_cs = at(); H.insert(H.end(), all.begin(), all.end());
+        cs_words = all;                                      // placed at the end: constant bank if it fits, else global memory
         v.h_cs_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
     }
     // ---- dy/dx solve program: fixed-format row operations on the warp's dy/dx column,
@@ -419,6 +419,11 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         v.h_eff_off = at();
         for (size_t i = 0; i < off.size(); i += 2) H.push_back((int32_t)(off[i] | ((i + 1 < off.size() ? off[i + 1] : 0u) << 16)));
     }
+    // the column streams are the largest table: they go to the constant bank when they fit, otherwise to global memory (the
+    // kernel's software pipeline fetches them two pairs ahead, so the L2 latency is covered); QSS_CS_GLOBAL=1 forces the latter
+    if (H.size() & 1) H.push_back(0);
+    v.cs_global = ((int)(H.size() + cs_words.size()) > QSS_V1_HMAX || std::getenv("QSS_CS_GLOBAL")) ? 1 : 0;
+    if (!v.cs_global) { v.h_cs = at(); H.insert(H.end(), cs_words.begin(), cs_words.end()); }
     if ((int)H.size() > QSS_V1_HMAX) { why = "hot tables exceed the kernel-parameter budget of variant 1"; return false; }
     v.h_used = (int32_t)H.size();
     std::memcpy(v.h, H.data(), H.size() * sizeof(int32_t));
@@ -428,7 +433,8 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         v.i_wya_ptr = (int32_t)I.size(); I.insert(I.end(), wya_ptr.begin(), wya_ptr.end());   // [n_wy + 1] then the words
         I.insert(I.end(), wya_all.begin(), wya_all.end());
         I.insert(I.end(), ce_tab.begin(), ce_tab.end());
-        I.insert(I.end(), q_tab.begin(), q_tab.end());
+        I.insert(I.end(), q_tab.begin(), q_tab.end());       // (everything up to here is staged contiguously in shared memory)
+        if (v.cs_global) { while (I.size() & 3) I.push_back(0); v.h_cs = (int32_t)I.size(); I.insert(I.end(), cs_words.begin(), cs_words.end()); }
     }
     // ---- reaction records (appended to the int blob), in processing order
     {

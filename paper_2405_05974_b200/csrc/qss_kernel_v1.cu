@@ -75,7 +75,7 @@ __device__ __forceinline__ double ldg_keep(const double *q, unsigned long long p
         }                                                                              \
     } while (0)
 
-template <bool JAC>
+template <bool JAC, bool CSG>
 __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_constant__ QssV1 p) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const int N = p.N, Nq = p.Nq, M = p.M, nsp = p.nsp;
@@ -449,7 +449,12 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                         const int npair = (HT(p.h_cs_ptr, k + 1) - HT(p.h_cs_ptr, k)) >> 3;
                         const unsigned one = sml + (p.s_V + N) * 256;
 #define QSS_FETCH(XO, ra, rb, rA, rV)                                                    \
-    ra = ldc2(&p.h[XO]); rb = ldc2(&p.h[(XO) + 2]);                                      \
+    if (CSG) {                                                                           \
+        const int4 r4_ = ldg_keep(reinterpret_cast<const int4 *>(gI + (XO)), keep);      \
+        ra = make_int2(r4_.x, r4_.y); rb = make_int2(r4_.z, r4_.w);                      \
+    } else {                                                                             \
+        ra = ldc2(&p.h[XO]); rb = ldc2(&p.h[(XO) + 2]);                                  \
+    }                                                                                    \
     rA = sc[(size_t)(ra.x & 0xffff) * 32];                                               \
     rV = (ra.x & (1 << 20)) ? ldg_keep(gD + p.d_effv + ra.y, keep) : 1.0
 #define QSS_FACTORS(ra, f1, f2)                                                          \
@@ -641,9 +646,10 @@ size_t qss_v1_smem_bytes(const QssV1 &v) { return (size_t)v.smem_rows * 256; }
 size_t qss_v1_scratch_doubles(const QssV1 &v) { return (size_t)v.scratch_rows * 32; }
 
 cudaError_t qss_v1_prepare() {
-    cudaError_t e = cudaFuncSetAttribute(qss_v1_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    cudaError_t e = cudaFuncSetAttribute(qss_v1_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(qss_v1_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if ((e = cudaFuncSetAttribute(qss_v1_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024)) != cudaSuccess) return e;
+    return cudaFuncSetAttribute(qss_v1_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
 }
 
 cudaError_t qss_launch_v1(const QssV1 &v, bool jac, int nblocks, cudaStream_t stream) {
@@ -651,7 +657,8 @@ cudaError_t qss_launch_v1(const QssV1 &v, bool jac, int nblocks, cudaStream_t st
     if (nslab == 0) return cudaSuccess;
     const int grid = (int)(nslab < nblocks ? nslab : nblocks);
     const size_t smem = qss_v1_smem_bytes(v);
-    if (jac) qss_v1_kernel<true><<<grid, v.nw * 32, smem, stream>>>(v);
-    else qss_v1_kernel<false><<<grid, v.nw * 32, smem, stream>>>(v);
+    if (jac && v.cs_global) qss_v1_kernel<true, true><<<grid, v.nw * 32, smem, stream>>>(v);
+    else if (jac) qss_v1_kernel<true, false><<<grid, v.nw * 32, smem, stream>>>(v);
+    else qss_v1_kernel<false, false><<<grid, v.nw * 32, smem, stream>>>(v);
     return cudaGetLastError();
 }

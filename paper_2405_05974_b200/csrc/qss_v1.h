@@ -60,7 +60,8 @@ struct QssV1 {
     int32_t h_st_ptr, h_st;                          // third-body incidence: index of dQ_j/dM | sign bit
     int32_t h_eff_val, h_eff_off;                    // third-body (alpha - 1) doubles; V-row byte offsets, two 16-bit per word
     int32_t h_cw;                                    // [n_rounds*nw] Jacobian column of (round, warp), -1: none
-    int32_t h_cs_ptr, h_cs;                          // column streams (see qss_compile.cpp "column stream")
+    int32_t h_cs_ptr, h_cs;                          // column streams (see qss_compile.cpp "column stream"); h_cs is an offset into
+    int32_t cs_global;                               //   h, or into the global int blob when cs_global (tables too large for h)
     int32_t h_sp;                                    // dy/dx solve program: n_sp_ops pairs of fixed-format row operations
     int32_t h_wr_ptr;                                // [N+1] W_y rows: index of the first entry of each row
     int32_t h_rw;                                    // [nw][3] Jacobian rows of each warp's pass-B tile (-1: none)

@@ -104,6 +104,16 @@ def test_kernel_variants_selected_and_general_kernel_on_cfg2(monkeypatch):
     _check(mech, C, T, n, "cfg2 (variant 0)")
 
 
+def test_column_streams_in_global_memory(monkeypatch):
+    """When the hot tables do not fit the kernel-parameter constant bank the column streams move to global memory
+    (QSS_CS_GLOBAL=1 forces it): same results."""
+    monkeypatch.setenv("QSS_CS_GLOBAL", "1")
+    for mech, n, what in ((qss_synth.config_mechanism(2), 512 + 21, "cfg2 (streams in global memory)"),
+                          (qss_synth.toy_dag(), 77, "toy_dag (streams in global memory)")):
+        C, T = (qss_synth.config_states(2, n) if mech.n_reac > 100 else make_states(mech.n_nqss, n, seed=5))
+        _check(mech, C, T, n, what)
+
+
 def test_cfg4_field_small():
     mech = qss_synth.config_mechanism(4)
     C, T = qss_synth.config_states(4, 16 ** 3)           # 16^3 cells of the multipulse-shaped field
