@@ -112,6 +112,17 @@ def run_reference(args, cfg: int, rank: int):
         "gpu_launches": 0}))
 
 
+def _cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return None
+
+
 def _config(cfg, mech, n_cells, n_gpus):
     return {"workload": f"BASELINE.json configs[{cfg - 1}] (cfg{cfg}): synthetic QSS mechanism {mech.n_nqss} transported + "
                         f"{mech.n_qss} QSS species, {mech.n_reac} reactions; {n_cells} cells per GPU; Jacobian "
@@ -281,8 +292,14 @@ def main():
         t0 = time.perf_counter()
         oracle.evaluate(om, Cs, Ts, ns, want_jac=True)
         dt = time.perf_counter() - t0
+        n1 = max(32, ns // 16)      # single-thread figure on a 16x smaller sample
+        t0 = time.perf_counter()
+        oracle.evaluate(om, Cs, Ts, n1, want_jac=True, nthreads=1)
+        dt1 = time.perf_counter() - t0
         cpu = {"value": ns / dt, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
-               "sample": f"first {ns} cells of the same cfg{cfg} input, explicit-formula fp64 oracle, OpenMP over cells, {dt:.2f} s"}
+               "sample": f"first {ns} cells of the same cfg{cfg} input, explicit-formula fp64 oracle, OpenMP over cells, {dt:.2f} s",
+               "value_1thread": n1 / dt1, "sample_1thread": f"first {n1} cells, one thread, {dt1:.2f} s",
+               "cpu_model": _cpu_model()}
 
     print(json.dumps({
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
