@@ -101,6 +101,14 @@ int qss_mech_qss_order(const qss_mech_t *mech, int32_t *order, int32_t *group_of
  * n_groups, order[n_qss], group_of[n_qss] may each be NULL. Same return codes as qss_mech_create. */
 int qss_mech_validate(const qss_mech_desc_t *desc, int32_t *n_groups, int32_t *order, int32_t *group_of);
 
+/* Host-only check of the run-time specialisation (no CUDA call, no device needed): validates `desc`, generates the
+ * mechanism-specialised source of the Jacobian kernel (the paper's generated-code idea,
+ * PAPER.md L324-326, applied to pass A of the sweep) and compiles it with NVRTC for compute capability
+ * cc_major.cc_minor (10.0 = B200).  *image_bytes (may be NULL) receives the size of the device image.
+ * Returns QSS_OK; QSS_E_UNSUPPORTED when the mechanism does not fit kernel variant 1 (nothing to specialise);
+ * QSS_E_CUDA when NVRTC is missing or the compilation fails (qss_last_error() holds the compiler log). */
+int qss_mech_specialise_check(const qss_mech_desc_t *desc, int cc_major, int cc_minor, size_t *image_bytes);
+
 /* wdot (and optionally the closure's C_QSS) for ncells cells.  C, T, wdot, cqss_or_null, workspace are
  * DEVICE pointers, 16-byte aligned; stream is a cudaStream_t.  ncells == 0 is a no-op. */
 int qss_eval_wdot(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *C, const double *T,

@@ -16,7 +16,7 @@ from . import build as _build
 
 __all__ = ["lib", "QssMech", "QssError", "EXPORTS", "STATUS"]
 
-EXPORTS = ["qss_mech_create", "qss_mech_validate", "qss_mech_destroy", "qss_mech_info", "qss_mech_qss_order", "qss_eval_wdot",
+EXPORTS = ["qss_mech_create", "qss_mech_validate", "qss_mech_specialise_check", "qss_mech_destroy", "qss_mech_info", "qss_mech_qss_order", "qss_eval_wdot",
            "qss_eval_jac", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
 STATUS = {0: "QSS_OK", -1: "QSS_E_INVALID", -2: "QSS_E_QUADRATIC", -3: "QSS_E_QSS_FANOUT", -4: "QSS_E_NO_SINK",
           -5: "QSS_E_UNSUPPORTED", -6: "QSS_E_CUDA"}
@@ -61,6 +61,7 @@ def lib():
         vp, i64 = ct.c_void_p, ct.c_int64
         L.qss_mech_create.restype = ct.c_int; L.qss_mech_create.argtypes = [vp, ct.c_int, ct.POINTER(vp)]
         L.qss_mech_validate.restype = ct.c_int; L.qss_mech_validate.argtypes = [vp, vp, vp, vp]
+        L.qss_mech_specialise_check.restype = ct.c_int; L.qss_mech_specialise_check.argtypes = [vp, ct.c_int, ct.c_int, vp]
         L.qss_mech_destroy.restype = ct.c_int; L.qss_mech_destroy.argtypes = [vp]
         L.qss_mech_info.restype = ct.c_int; L.qss_mech_info.argtypes = [vp, ct.POINTER(_Info)]
         L.qss_mech_qss_order.restype = ct.c_int; L.qss_mech_qss_order.argtypes = [vp, vp, vp]
@@ -109,6 +110,16 @@ def validate(mech):
     _check(lib().qss_mech_validate(ct.addressof(d), ct.addressof(ng), order.ctypes.data, grp.ctypes.data))
     del keep
     return ng.value, order[:mech.n_qss], grp[:mech.n_qss]
+
+
+def specialise_check(mech, cc=(10, 0)) -> int:
+    """Host-only: generate the mechanism-specialised Jacobian kernel source and compile it with NVRTC for compute
+    capability `cc` (no device needed). Returns the size of the device image in bytes."""
+    d, keep = make_desc(mech)
+    nbytes = ct.c_size_t()
+    _check(lib().qss_mech_specialise_check(ct.addressof(d), int(cc[0]), int(cc[1]), ct.addressof(nbytes)))
+    del keep
+    return nbytes.value
 
 
 def _ptr(t):

@@ -10,6 +10,7 @@
 
 #include "../../include/qss.h"
 #include "qss_compile.h"
+#include "qss_jit.h"
 
 size_t qss_slab_ws_doubles(const QssTab &t, bool jac, int nwarp);
 cudaError_t qss_launch_slab(const QssTab &t, bool jac, int64_t ncells, int64_t ld, const double *C, const double *T,
@@ -33,6 +34,7 @@ struct qss_mech {
     cudaEvent_t ev[2] = {nullptr, nullptr};
     long long *timing = nullptr;   // device counters when QSS_TIMING=1 (variant 1 only)
     int variant = 0;          // 0: general slab kernel (workspace in global memory); 1: slab-smem kernel (qss_kernel_v1.cu)
+    QssJit *jit = nullptr;    // variant 1 with the Jacobian sweep's pass A specialised for this mechanism at run time (qss_jit.cpp)
 };
 
 namespace {
@@ -107,6 +109,15 @@ extern "C" int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech
         m->nblocks = m->n_sm;
         m->c.v1.gI = m->dI; m->c.v1.gD = m->dD;
         if (std::getenv("QSS_TIMING") && cudaMalloc(&m->timing, 16 * sizeof(long long)) == cudaSuccess) cudaMemset(m->timing, 0, 16 * sizeof(long long));
+        // Jacobian kernel specialised for this mechanism (NVRTC); QSS_JIT=0 keeps the table interpreter, which is also what
+        // runs when NVRTC is missing or the compilation fails (qss_mech_info.kernel_variant_jac tells which: 2 = specialised)
+        const char *jit_env = std::getenv("QSS_JIT");
+        if (!(jit_env && jit_env[0] == '0')) {
+            std::string jerr;
+            m->jit = qss_jit_create(m->c.v1_gen, prop.major, prop.minor, jerr);
+            if (!m->jit && (std::getenv("QSS_DEBUG") || (jit_env && jit_env[0] == '2'))) std::fprintf(stderr, "[qss] run-time specialisation unavailable: %s\n", jerr.c_str());
+            if (!m->jit && jit_env && jit_env[0] == '2') { cudaFree(m->dI); cudaFree(m->dD); cudaFree(m->timing); delete m; return fail(QSS_E_CUDA, "QSS_JIT=2: " + jerr); }
+        }
     }
     *out = m;
     return QSS_OK;
@@ -127,6 +138,21 @@ extern "C" int qss_mech_validate(const qss_mech_desc_t *desc, int32_t *n_groups,
     return QSS_OK;
 }
 
+extern "C" int qss_mech_specialise_check(const qss_mech_desc_t *desc, int cc_major, int cc_minor, size_t *image_bytes) {
+    QssCompiled c;
+    std::string err;
+    int rc;
+    try {
+        rc = qss_compile(desc, c, err);
+    } catch (const std::exception &e) {
+        rc = QSS_E_INVALID; err = std::string("mechanism compiler: ") + e.what();
+    }
+    if (rc != QSS_OK) return fail(rc, err);
+    if (!c.v1_ok) return fail(QSS_E_UNSUPPORTED, "kernel variant 1 does not apply: " + c.v1_why);
+    if (!qss_jit_compile_only(c.v1_gen, cc_major, cc_minor, image_bytes, err)) return fail(QSS_E_CUDA, err);
+    return QSS_OK;
+}
+
 extern "C" int qss_mech_destroy(qss_mech_t *m) {
     if (!m) return QSS_OK;
     DeviceGuard guard(m->device);
@@ -141,6 +167,7 @@ extern "C" int qss_mech_destroy(qss_mech_t *m) {
         }
         cudaFree(m->timing);
     }
+    qss_jit_destroy(m->jit);
     if (m->copy_stream) { cudaStreamDestroy(m->copy_stream); cudaEventDestroy(m->ev[0]); cudaEventDestroy(m->ev[1]); }
     cudaFree(m->dI); cudaFree(m->dD);
     delete m;
@@ -163,7 +190,7 @@ extern "C" int qss_mech_info(const qss_mech_t *m, qss_mech_info_t *o) {
     o->bytes_wdot = m->c.bytes_wdot; o->bytes_jac = m->c.bytes_jac;
     o->workspace_bytes_wdot = ws_bytes(m, false);
     o->workspace_bytes_jac = ws_bytes(m, true);
-    o->kernel_variant_wdot = m->variant; o->kernel_variant_jac = m->variant;
+    o->kernel_variant_wdot = m->variant; o->kernel_variant_jac = m->jit ? 2 : m->variant;
     return QSS_OK;
 }
 
@@ -199,7 +226,7 @@ extern "C" int qss_eval_jac(const qss_mech_t *m, int64_t ncells, int64_t ld, con
         QssV1 v = m->c.v1;
         v.C = C; v.T = T; v.wdot = wdot; v.cqss = nullptr; v.jac = jac; v.scratch = (double *)workspace; v.timing = m->timing;
         v.ncells = ncells; v.ld = ld; v.scratch_stride = (int64_t)qss_v1_scratch_doubles(v);
-        e = qss_launch_v1(v, true, m->nblocks, (cudaStream_t)stream);
+        e = m->jit ? qss_jit_launch(m->jit, v, m->nblocks, (cudaStream_t)stream) : qss_launch_v1(v, true, m->nblocks, (cudaStream_t)stream);
     } else {
         e = qss_launch_slab(m->c.tab, true, ncells, ld, C, T, wdot, nullptr, jac, (double *)workspace, m->nblocks, m->nwarp,
                             (cudaStream_t)stream);

@@ -231,15 +231,21 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     std::vector<std::vector<int32_t>> cs(N);
     std::vector<double> effv;                              // (alpha - 1) values, read from the double blob
     bool cs_ok = true;
+    // the same records, unpacked, for the run-time specialised pass A (qss_gen_pass_a below)
+    struct GenRec { int rowA, o1, o2, mag; bool has_val; double val; std::vector<std::pair<int, int>> tgt; };   // tgt: (species row, +1 / -1)
+    std::vector<std::vector<GenRec>> grec(N);
     auto push_record = [&](int k, int rowA, int o1, int o2, const std::vector<Term> &net, int sgn, bool has_val, double val) {
         for (int mag = 1; mag <= 7; ++mag) {                 // one record per magnitude |nu| (almost always only 1)
             std::vector<int> idx;
             int own = 0;                                     // the column's own row k is accumulated in a register: 1 add, 2 subtract
+            GenRec gr{rowA, o1, o2, mag, has_val, val, {}};
             for (const Term &x : net) if (std::abs(x.nu) == mag) {
+                gr.tgt.push_back({x.sp, sgn * x.nu < 0 ? -1 : 1});
                 if (x.sp == k) own = sgn * x.nu < 0 ? 2 : 1;
                 else idx.push_back(x.sp | (sgn * x.nu < 0 ? 0x80 : 0));
             }
             if (idx.empty() && !own) continue;
+            grec[k].push_back(gr);
             if (idx.size() > 8) { cs_ok = false; return; }
             const uint32_t none = (uint32_t)nsp * 0x01010101u;   // the junk row of the column buffer
             uint32_t w[2] = {none, none};
@@ -297,6 +303,8 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         cs_words = all;                                      // placed at the end: constant bank if it fits, else global memory
         v.h_cs_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
     }
+    struct GenOp { int a; std::vector<std::pair<int, int>> terms; int scale; };     // y[a] = (y[a] + sum F y[b]) * S; (F row, QSS index b); scale -1: none
+    std::vector<std::vector<GenOp>> ggops;
     // ---- dy/dx solve program: fixed-format row operations on the warp's dy/dx column,
     //          y[a] = (y[a] + F0 y[b0] + F1 y[b1] + F2 y[b2]) * S
     //      in the order cross-group terms, back-elimination (with U[m][k] = P[m][k] / D_k), forward substitution (S = 1/D),
@@ -318,22 +326,26 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
             } while (t < terms.size());
         };
         std::vector<Ops> gops(c.n_groups);
+        ggops.assign(c.n_groups, {});
         for (int g = 0; g < c.n_groups; ++g) {
             const std::vector<int> &mem = (*c.members)[g];
             const int sz = (int)mem.size(), base = v.s_CL + (*c.gbase)[g];
             for (int x = (*c.xp_begin)[g]; x < (*c.xp_end)[g]; ++x) {
                 const auto &e = (*c.xpl)[x];
                 emit(gops[g], yoff(e.first.first), {{v.s_XP + x, yoff(e.first.second)}}, one);
+                ggops[g].push_back({e.first.first, {{v.s_XP + x, e.first.second}}, -1});
             }
             for (int m = sz - 2; m >= 0; --m) {
-                std::vector<std::pair<int, int>> t;
-                for (int k = m + 1; k < sz; ++k) t.push_back({base + m * sz + k, yoff(mem[k])});
+                std::vector<std::pair<int, int>> t, tq;
+                for (int k = m + 1; k < sz; ++k) { t.push_back({base + m * sz + k, yoff(mem[k])}); tq.push_back({base + m * sz + k, mem[k]}); }
                 emit(gops[g], yoff(mem[m]), t, one);
+                if (!tq.empty()) ggops[g].push_back({mem[m], tq, -1});
             }
             for (int k = 0; k < sz; ++k) {
-                std::vector<std::pair<int, int>> t;
-                for (int jj = 0; jj < k; ++jj) t.push_back({base + k * sz + jj, yoff(mem[jj])});
+                std::vector<std::pair<int, int>> t, tq;
+                for (int jj = 0; jj < k; ++jj) { t.push_back({base + k * sz + jj, yoff(mem[jj])}); tq.push_back({base + k * sz + jj, mem[jj]}); }
                 emit(gops[g], yoff(mem[k]), t, base + sz * sz + 2 * sz + k);
+                ggops[g].push_back({mem[k], tq, base + sz * sz + 2 * sz + k});
             }
         }
         Ops chain[2];
@@ -473,6 +485,82 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         }
     }
     v.i_eff_ptr = out.tab.i_eff_ptr; v.i_eff_sp = out.tab.i_eff_sp;
+    // ---- run-time specialised pass A (compiled with NVRTC by qss_jit.cpp and included by qss_kernel_v1.cu under QSS_GEN):
+    //      the column lives in REGISTERS c0..c{nsp-1}; every record of the column stream becomes straight-line code with
+    //      immediate offsets (1 L2 read of A fetched `dist` records ahead, <= 2 shared-memory factors, 2 multiplications,
+    //      one add per target row); the dy/dx solve is the same row operations on registers; the column is then written
+    //      to the round buffer for pass B.  Same operations in the same order per row as the interpreter, except that the
+    //      interpreter applies the records of a column in paired order (rounding-order difference only).
+    {
+        std::string &g = out.v1_gen;
+        char b[256];
+        auto P = [&](const char *f, auto... a) { std::snprintf(b, sizeof b, f, a...); g += b; };
+        const int RS = nw * 256, one = voff(N), dist = 12;
+        g += "// generated by qss_compile.cpp for one mechanism: pass A of the Jacobian sweep (see qss_kernel_v1.cu)\n";
+        g += "__device__ __forceinline__ void qss_gen_pass_a(const int k, const unsigned sml, const double *sc, const unsigned colw) {\n";
+        g += "    double ";
+        for (int s = 0; s < nsp; ++s) P("c%d%s", s, s + 1 < nsp ? ", " : ";\n");
+        P("    if (k < %d) {\n", N);
+        for (int s = 0; s < nsp; ++s) P("        c%d = lS<%d>(sml);\n", s, (v.s_TV + s) * 256);
+        g += "    } else {\n";
+        for (int s = 0; s < nsp; ++s) P("        c%d = lG<%d>(sc);\n", s, (v.g_ET + s) * 256);
+        g += "    }\n    switch (k) {\n";
+        for (int k = 0; k < N; ++k) {
+            const std::vector<GenRec> &rr = grec[k];
+            const int n = (int)rr.size();
+            if (!n) continue;
+            P("    case %d: {\n", k);
+            auto load_A = [&](int i) { if (i < n) P("        const double A%d = lG<%d>(sc);\n", i, rr[i].rowA * 256); };
+            auto load_F = [&](int i) {
+                if (i >= n || rr[i].has_val) return;
+                if (rr[i].o1 != one) P("        const double f%d = lS<%d>(sml);\n", i, rr[i].o1);
+                if (rr[i].o2 != one) P("        const double h%d = lS<%d>(sml);\n", i, rr[i].o2);
+            };
+            for (int i = 0; i < dist; ++i) load_A(i);
+            load_F(0); load_F(1);
+            for (int i = 0; i < n; ++i) {
+                load_A(i + dist);
+                load_F(i + 2);
+                const GenRec &r = rr[i];
+                P("        const double p%d = A%d", i, i);
+                if (r.has_val) P(" * %.17g", r.val * r.mag);
+                else {
+                    if (r.o1 != one) P(" * f%d", i);
+                    if (r.o2 != one) P(" * h%d", i);
+                    if (r.mag > 1) P(" * %d.0", r.mag);
+                }
+                g += ";";
+                for (auto &t : r.tgt) P(" c%d %s= p%d;", t.first, t.second > 0 ? "+" : "-", i);
+                g += "\n";
+            }
+            g += "    } break;\n";
+        }
+        g += "    default: break;\n    }\n";
+        // dy/dx solve on the QSS rows c{N+q}; the operations of independent groups are interleaved
+        {
+            std::vector<const GenOp *> ch[2];
+            size_t len[2] = {0, 0};
+            for (int gi = 0; gi < c.n_groups; ++gi) {
+                const int w = v.n_xp > 0 ? 0 : (len[0] <= len[1] ? 0 : 1);
+                for (const GenOp &o : ggops[gi]) { ch[w].push_back(&o); len[w] += 1 + o.terms.size(); }
+            }
+            int uid = 0;
+            auto emit_op = [&](const GenOp &o) {
+                const int a = N + o.a;
+                for (size_t t = 0; t < o.terms.size(); ++t) P("    const double u%d_%d = lS<%d>(sml);\n", uid, (int)t, o.terms[t].first * 256);
+                if (o.scale >= 0) P("    const double u%d_s = lS<%d>(sml);\n", uid, o.scale * 256);
+                for (size_t t = 0; t < o.terms.size(); ++t) P("    c%d = fma(u%d_%d, c%d, c%d);\n", a, uid, (int)t, N + o.terms[t].second, a);
+                if (o.scale >= 0) P("    c%d *= u%d_s;\n", a, uid);
+                ++uid;
+            };
+            for (size_t i = 0; i < std::max(ch[0].size(), ch[1].size()); ++i) {
+                if (i < ch[0].size()) emit_op(*ch[0][i]);
+                if (i < ch[1].size()) emit_op(*ch[1][i]);
+            }
+        }
+        for (int s = 0; s < nsp; ++s) P("    sS<%d>(colw, c%d);\n", s * RS, s);
+        g += "}\n";
+    }
     return true;
 }
 
@@ -851,6 +939,9 @@ int qss_compile(const qss_mech_desc_t *d, QssCompiled &out, std::string &err) {
         V1Ctx vc{N, Nq, M, nsp, n_tb, n_groups, n_levels, cl_size, &R, &members, &gbase, &xp_begin, &xp_end, &lvl_of_group,
                  &pos_in_grp, &rorder, &ce, &xpl, &effc};
         out.v1_ok = build_v1(vc, out, out.v1_why);
+        if (const char *dump = std::getenv("QSS_GEN_DUMP")) {            // debugging aid: the generated source of pass A
+            if (FILE *f = std::fopen(dump, "w")) { std::fwrite(out.v1_gen.data(), 1, out.v1_gen.size(), f); std::fclose(f); }
+        }
         if (std::getenv("QSS_DEBUG"))
             std::fprintf(stderr, "[qss] variant 1: %s%s (hot table %d/%d words, smem rows %d, scratch rows %d, rounds %d, solve ops %d)\n",
                          out.v1_ok ? "ok" : "not applicable: ", out.v1_ok ? "" : out.v1_why.c_str(), out.v1.h_used, QSS_V1_HMAX,

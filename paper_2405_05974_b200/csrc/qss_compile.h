@@ -19,6 +19,7 @@ struct QssCompiled {
     QssV1 v1;                      // launch descriptor of kernel variant 1 (valid iff v1_ok)
     bool v1_ok = false;
     std::string v1_why;            // why variant 1 does not apply
+    std::string v1_gen;            // CUDA source of the mechanism-specialised pass A (qss_gen_pass_a), compiled at run time
 };
 
 // Validates `desc` and builds the tables. Returns QSS_OK or a negative qss_status with `err` set.

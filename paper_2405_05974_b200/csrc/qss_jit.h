@@ -1,0 +1,25 @@
+// Internal: run-time specialisation of kernel variant 1 (qss_jit.cpp -> qss_api.cu).
+//
+// The mechanism compiler (qss_compile.cpp) emits the Jacobian sweep's pass A for ONE mechanism as straight-line CUDA
+// source (`QssCompiled::v1_gen`).  qss_jit_create compiles qss_kernel_v1.cu (its source is embedded in libqss.so by
+// build.py) together with that source with NVRTC for the device's architecture and loads the result; the kernel it
+// launches is the same slab-smem kernel with `qss_gen_pass_a` in place of the column-stream interpreter.
+#ifndef QSS_JIT_H
+#define QSS_JIT_H
+#include <cuda_runtime.h>
+
+#include <string>
+
+#include "qss_v1.h"
+
+struct QssJit;
+
+// Returns NULL and sets `err` when NVRTC is not available or the compilation fails (the caller then keeps the
+// interpreter kernel, which computes the same thing).  Compiled images are cached per process by source text.
+QssJit *qss_jit_create(const std::string &gen_src, int cc_major, int cc_minor, std::string &err);
+// Compilation only (no device needed): used by qss_mech_specialise_check.
+bool qss_jit_compile_only(const std::string &gen_src, int cc_major, int cc_minor, size_t *image_bytes, std::string &err);
+cudaError_t qss_jit_launch(const QssJit *j, const QssV1 &v, int nblocks, cudaStream_t stream);
+void qss_jit_destroy(QssJit *j);
+
+#endif

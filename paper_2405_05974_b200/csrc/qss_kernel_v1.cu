@@ -14,14 +14,19 @@
 //     back, so no dependent chain builds up; then the dy/dx_k solve program runs in place on the QSS rows.  Pass B:
 //     the warps switch to ROWS and add W_y * dy/dx for all 12 columns of the round from a register tile (one W_y
 //     load and one table word per 12 FMAs); every entry leaves as one coalesced 256-byte streaming store.
+#ifndef __CUDACC_RTC__
 #include <cuda_runtime.h>
-#include <stdint.h>
+#endif
+
+#include "qss_stdint.h"
 
 #include "qss_tables.h"
 #include "qss_math.h"
 #include "qss_v1.h"
 
+#ifndef QSS_GEN          // (the run-time specialised build exports its one kernel by name)
 namespace {
+#endif
 
 constexpr double kLn10 = 2.302585092994045684017991454684;
 constexpr double kInvLn10 = 0.434294481903251827651128918916605;
@@ -65,6 +70,22 @@ __device__ __forceinline__ double ldg_keep(const double *q, unsigned long long p
     return v;
 }
 
+#ifdef QSS_GEN
+// run-time specialised build (qss_jit.cpp): loads / stores with immediate offsets for the generated pass A
+template <int O> __device__ __forceinline__ double lS(unsigned b) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(b), "n"(O) : "memory");
+    return v;
+}
+template <int O> __device__ __forceinline__ void sS(unsigned b, double v) { asm volatile("st.shared.f64 [%0+%1], %2;" ::"r"(b), "n"(O), "d"(v) : "memory"); }
+template <int O> __device__ __forceinline__ double lG(const double *b) {
+    double v;
+    asm volatile("ld.global.f64 %0, [%1+%2];" : "=d"(v) : "l"(b), "n"(O) : "memory");
+    return v;
+}
+#include "qss_gen.h"
+#endif
+
 // optional phase timing (QSS_TIMING=1): thread 0 of block 0 accumulates the cycles between block barriers
 #define QSS_TICK(ph)                                                                   \
     do {                                                                               \
@@ -75,8 +96,14 @@ __device__ __forceinline__ double ldg_keep(const double *q, unsigned long long p
         }                                                                              \
     } while (0)
 
+#ifdef QSS_GEN
+// run-time specialised build: one entry point, Jacobian on, column stream replaced by the generated pass A
+constexpr bool JAC = true, CSG = false;
+extern "C" __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_jit(const __grid_constant__ QssV1 p) {
+#else
 template <bool JAC, bool CSG>
 __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_constant__ QssV1 p) {
+#endif
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const int N = p.N, Nq = p.Nq, M = p.M, nsp = p.nsp;
     const int64_t ld = p.ld;
@@ -418,7 +445,12 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             for (int r = 0; r < p.n_rounds; ++r) {
                 // -- pass A: warp = column k.  [W_x; G_x][:,k] in shared memory, then (diag D - P) dy/dx_k = G_x[:,k]
                 const int k = HT(p.h_cw, r * nw + warp);
+#ifdef QSS_GEN
+                if (k >= 0) qss_gen_pass_a(k, sml, sc, colw);
+                if (false) {
+#else
                 if (k >= 0) {
+#endif
                     // initialise the column: rank-1 third-body vector (every species column) or the T-column vector;
                     // 8 rows are read before they are written so that the copies do not serialise on the load latency
                     if (k < N) {
@@ -637,6 +669,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
     }
 }
 
+#ifndef QSS_GEN
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------------
@@ -662,3 +695,4 @@ cudaError_t qss_launch_v1(const QssV1 &v, bool jac, int nblocks, cudaStream_t st
     else qss_v1_kernel<false, false><<<grid, v.nw * 32, smem, stream>>>(v);
     return cudaGetLastError();
 }
+#endif  // QSS_GEN

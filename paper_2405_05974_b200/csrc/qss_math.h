@@ -9,8 +9,10 @@
 // Preconditions: |x| < 2^30 (NaN gives NaN; +-inf gives NaN, not inf / 0).
 #ifndef QSS_MATH_H
 #define QSS_MATH_H
-#include <stdint.h>
+#include "qss_stdint.h"
+#ifndef __CUDACC_RTC__
 #include <string.h>
+#endif
 
 #ifdef __CUDACC__
 #define QSS_HD __host__ __device__ __forceinline__

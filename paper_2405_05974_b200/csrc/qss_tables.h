@@ -8,7 +8,7 @@
 // dir 0 = forward (reactants = the reaction's reactant side), dir 1 = reverse (reactants = product side).
 #ifndef QSS_TABLES_H
 #define QSS_TABLES_H
-#include <stdint.h>
+#include "qss_stdint.h"
 
 #define QSS_TH_STRIDE 24   // doubles per species in the thermo table
 #define QSS_RD_STRIDE 12   // doubles per reaction in the rate table

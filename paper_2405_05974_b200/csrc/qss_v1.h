@@ -10,7 +10,7 @@
 // L2-resident scratch slab.  DESIGN.md "Kernels" gives the layout and the reasons.
 #ifndef QSS_V1_H
 #define QSS_V1_H
-#include <stdint.h>
+#include "qss_stdint.h"
 
 #define QSS_V1_HMAX 8000        // 32-bit words of hot tables carried in the kernel parameters (<= 32 KB total)
 #define QSS_V1_NW 12            // warps per block = Jacobian columns per round
