@@ -112,7 +112,7 @@ extern "C" int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech
         // Jacobian kernel specialised for this mechanism (NVRTC); QSS_JIT=0 keeps the table interpreter, which is also what
         // runs when NVRTC is missing or the compilation fails (qss_mech_info.kernel_variant_jac tells which: 2 = specialised)
         const char *jit_env = std::getenv("QSS_JIT");
-        if (!(jit_env && jit_env[0] == '0')) {
+        if (!(jit_env && jit_env[0] == '0') && !m->c.v1_gen.empty()) {
             std::string jerr;
             m->jit = qss_jit_create(m->c.v1_gen, prop.major, prop.minor, jerr);
             if (!m->jit && (std::getenv("QSS_DEBUG") || (jit_env && jit_env[0] == '2'))) std::fprintf(stderr, "[qss] run-time specialisation unavailable: %s\n", jerr.c_str());

@@ -491,13 +491,13 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     //      one add per target row); the dy/dx solve is the same row operations on registers; the column is then written
     //      to the round buffer for pass B.  Same operations in the same order per row as the interpreter, except that the
     //      interpreter applies the records of a column in paired order (rounding-order difference only).
-    {
+    if (v.n_wy <= region) {                                  // (W_y must fit the time-shared region of the shared memory)
         std::string &g = out.v1_gen;
         char b[256];
         auto P = [&](const char *f, auto... a) { std::snprintf(b, sizeof b, f, a...); g += b; };
-        const int RS = nw * 256, one = voff(N), dist = 12;
+        const int one = voff(N), dist = 12;
         g += "// generated by qss_compile.cpp for one mechanism: pass A of the Jacobian sweep (see qss_kernel_v1.cu)\n";
-        g += "__device__ __forceinline__ void qss_gen_pass_a(const int k, const unsigned sml, const double *sc, const unsigned colw) {\n";
+        g += "__device__ __forceinline__ void qss_gen_column(const int k, const unsigned sml, const double *sc, double *jc, const long long rs, const bool active) {\n";
         g += "    double ";
         for (int s = 0; s < nsp; ++s) P("c%d%s", s, s + 1 < nsp ? ", " : ";\n");
         P("    if (k < %d) {\n", N);
@@ -558,8 +558,31 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
                 if (i < ch[1].size()) emit_op(*ch[1][i]);
             }
         }
-        for (int s = 0; s < nsp; ++s) P("    sS<%d>(colw, c%d);\n", s * RS, s);
-        g += "}\n";
+        // J[:, k] = W_x[:, k] + W_y dy/dx_k (Eq. 7) in place on the registers of the column: W_y (per cell, n_wy rows,
+        // row-major, ascending q within a row) was copied to shared memory behind the fixed state; then 35 coalesced stores
+        {
+            int e = 0;
+            for (auto &kv : wy) { P("    c%d = fma(lS<%d>(sml), c%d, c%d);\n", kv.first.first, (v.s_KAP + e) * 256, N + kv.first.second, kv.first.first); ++e; }
+        }
+        g += "    if (active) {\n";
+        for (int i = 0; i < N; ++i) P("        __stcs(jc + %d * rs, c%d);\n", i, i);
+        g += "    }\n}\n";
+        // columns of each warp: longest-processing-time assignment (the warps do not meet between columns)
+        {
+            std::vector<int> idx(N + 1);
+            for (int k = 0; k <= N; ++k) idx[k] = k;
+            auto cost = [&](int k) { return 300.0 + 2.0 * v.n_wy + (k < N ? 8.0 * grec[k].size() : 0.0); };
+            std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return cost(a) > cost(b); });
+            std::vector<std::vector<int>> bin(nw);
+            std::vector<double> load(nw, 0.0);
+            for (int k : idx) { const int w = (int)(std::min_element(load.begin(), load.end()) - load.begin()); bin[w].push_back(k); load[w] += cost(k); }
+            size_t depth = 0;
+            for (auto &bb : bin) depth = std::max(depth, bb.size());
+            P("#define QSS_GEN_DEPTH %d\n", (int)depth);
+            g += "__constant__ int qss_gen_cols[] = {";
+            for (int w = 0; w < nw; ++w) for (size_t d = 0; d < depth; ++d) P("%d, ", d < bin[w].size() ? bin[w][d] : -1);
+            g += "-1};\n";
+        }
     }
     return true;
 }

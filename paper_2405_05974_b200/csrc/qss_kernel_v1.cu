@@ -438,6 +438,24 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         if (JAC) {
             __syncthreads();
             QSS_TICK(6);
+#ifdef QSS_GEN
+            // ---- P8, specialised: W_y moves from the scratch slab to shared memory (the kappa region is free now); then each
+            //      warp takes its columns one after the other, everything in registers (qss_gen_column), no barrier between
+            for (int e0 = warp * 8; e0 < p.n_wy; e0 += nw * 8) {
+                double t[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) t[u] = ldg_pin(&SC(p.g_WY, min(e0 + u, p.n_wy - 1)));
+#pragma unroll
+                for (int u = 0; u < 8; ++u) if (e0 + u < p.n_wy) sts(sml + (p.s_KAP + e0 + u) * 256, t[u]);
+            }
+            __syncthreads();
+            QSS_TICK(11);
+            for (int d = 0; d < QSS_GEN_DEPTH; ++d) {
+                const int k = qss_gen_cols[warp * QSS_GEN_DEPTH + d];
+                if (k >= 0) qss_gen_column(k, sml, sc, p.jac + (size_t)(unsigned)k * (size_t)ld + cell, (long long)(N + 1) * ld, active);
+            }
+            QSS_TICK(13);
+#else
             // ---- P8: Jacobian sweep in rounds of nw columns (Eq. 7, Eq. 9)
             constexpr unsigned RS = QSS_V1_NW * 256;                 // byte stride between rows of a column buffer
             const unsigned colw = sml + (p.s_WX + warp) * 256;       // this warp's column of [W_x; G_x]: species row r at + r * RS
@@ -445,12 +463,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             for (int r = 0; r < p.n_rounds; ++r) {
                 // -- pass A: warp = column k.  [W_x; G_x][:,k] in shared memory, then (diag D - P) dy/dx_k = G_x[:,k]
                 const int k = HT(p.h_cw, r * nw + warp);
-#ifdef QSS_GEN
-                if (k >= 0) qss_gen_pass_a(k, sml, sc, colw);
-                if (false) {
-#else
                 if (k >= 0) {
-#endif
                     // initialise the column: rank-1 third-body vector (every species column) or the T-column vector;
                     // 8 rows are read before they are written so that the copies do not serialise on the load latency
                     if (k < N) {
@@ -664,6 +677,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                 __syncthreads();
                 QSS_TICK(8);
             }
+#endif
         }
         __syncthreads();      // shared memory and the scratch slab are reused by the next cell slab
     }

@@ -87,12 +87,12 @@ def test_configs_small(cfg, n):
 
 
 def test_kernel_variants_selected_and_general_kernel_on_cfg2(monkeypatch):
-    """cfg1/cfg2 run on kernel variant 1 (slab-smem), cfg3 on the general variant 0; QSS_VARIANT=0 forces the general
-    kernel, which must meet the same gates on cfg2."""
+    """cfg1/cfg2 run on kernel variant 1 (slab-smem), their Jacobian on its run-time specialised build (2); cfg3 on the
+    general variant 0; QSS_VARIANT=0 forces the general kernel, which must meet the same gates on cfg2."""
     import paper_2405_05974_b200 as qss
-    for cfg, want in ((1, 1), (2, 1), (3, 0)):
+    for cfg, want_jac, want_wdot in ((1, 2, 1), (2, 2, 1), (3, 0, 0)):
         qm = qss.QssMech(qss_synth.config_mechanism(cfg), 0)
-        assert qm.info.kernel_variant_jac == want and qm.info.kernel_variant_wdot == want
+        assert qm.info.kernel_variant_jac == want_jac and qm.info.kernel_variant_wdot == want_wdot
         qm.close()
     monkeypatch.setenv("QSS_VARIANT", "0")
     mech = qss_synth.config_mechanism(2)
@@ -104,10 +104,28 @@ def test_kernel_variants_selected_and_general_kernel_on_cfg2(monkeypatch):
     _check(mech, C, T, n, "cfg2 (variant 0)")
 
 
+def test_table_interpreter_when_specialisation_is_off(monkeypatch):
+    """QSS_JIT=0: the Jacobian sweep runs on the table interpreter of variant 1 (what a box without NVRTC gets): same
+    gates."""
+    import paper_2405_05974_b200 as qss
+    monkeypatch.setenv("QSS_JIT", "0")
+    mech = qss_synth.config_mechanism(2)
+    qm = qss.QssMech(mech, 0)
+    assert qm.info.kernel_variant_jac == 1
+    qm.close()
+    n = 1024 + 13
+    C, T = qss_synth.config_states(2, n)
+    _check(mech, C, T, n, "cfg2 (interpreter)")
+    mech = qss_synth.toy_dag()
+    C, T = make_states(mech.n_nqss, 77, seed=5)
+    _check(mech, C, T, 77, "toy_dag (interpreter)")
+
+
 def test_column_streams_in_global_memory(monkeypatch):
-    """When the hot tables do not fit the kernel-parameter constant bank the column streams move to global memory
-    (QSS_CS_GLOBAL=1 forces it): same results."""
+    """When the hot tables do not fit the kernel-parameter constant bank the column streams of the table interpreter move
+    to global memory (QSS_CS_GLOBAL=1 forces it): same results."""
     monkeypatch.setenv("QSS_CS_GLOBAL", "1")
+    monkeypatch.setenv("QSS_JIT", "0")
     for mech, n, what in ((qss_synth.config_mechanism(2), 512 + 21, "cfg2 (streams in global memory)"),
                           (qss_synth.toy_dag(), 77, "toy_dag (streams in global memory)")):
         C, T = (qss_synth.config_states(2, n) if mech.n_reac > 100 else make_states(mech.n_nqss, n, seed=5))

@@ -107,6 +107,16 @@ def test_validation_errors():
     assert e.value.code == -1
 
 
+def test_specialised_jacobian_kernel_compiles_without_a_gpu():
+    """Run-time specialisation, host side: the generated source of a mechanism's Jacobian columns compiles with NVRTC for
+    sm_100a (no device needed); a mechanism outside kernel variant 1 has nothing to specialise."""
+    for mech in (qss_synth.toy_dag(), qss_synth.config_mechanism(1)):
+        assert qss.specialise_check(mech, (10, 0)) > 10000
+    with pytest.raises(qss.QssError) as ei:
+        qss.specialise_check(qss_synth.config_mechanism(5), (10, 0))
+    assert ei.value.code == -5
+
+
 def test_branch_free_exp_against_float128(tmp_path):
     """csrc/qss_math.h compiled for the host: <= 1.5 ulp against libquadmath over the whole finite range."""
     src = tmp_path / "t.cpp"
