@@ -84,7 +84,10 @@ typedef struct {
     /* workspace the caller must supply to qss_eval_wdot / qss_eval_jac (device memory, 256-byte aligned);
      * independent of ncells */
     size_t  workspace_bytes_wdot, workspace_bytes_jac;
-    int32_t kernel_variant_wdot, kernel_variant_jac;   /* which kernel the library selected       */
+    /* which kernel the library selected: 0 general slab kernel, 1 slab-smem kernel (table
+     * interpreter), 2 slab-smem kernel with the Jacobian sweep specialised for this mechanism at qss_mech_create
+     * (NVRTC; takes seconds per mechanism and process, cached by source; falls back to 1 when NVRTC is missing) */
+    int32_t kernel_variant_wdot, kernel_variant_jac;
 } qss_mech_info_t;
 
 /* Validate `desc`, order the QSS groups (Tarjan SCC + topological order), build the static elimination

@@ -70,6 +70,45 @@ __device__ __forceinline__ double ldg_keep(const double *q, unsigned long long p
     return v;
 }
 
+// Third-body (type 1) and Troe fall-off (type 2) factor of a rate constant (Eq. 2; DESIGN.md readings
+// G5-G7): k (in: k_inf, out: the effective rate constant), dlm = d ln k / dM, dlnk = d ln k / dT.  Mc = sum alpha_k C_k.
+template <bool JACT>
+__device__ __forceinline__ void qss_pressure_factor(const int type, const double Mc, const double lnkinf, const double dlnkinf,
+                                                    const double t3, const double t4, const double t5, const double t6, const double t7,
+                                                    const double t8, const double t9, const double T, const double lnT, const double invT,
+                                                    double &k, double &dlm, double &dlnk) {
+    if (type == 1) {
+        k *= Mc;
+        dlm = qss_rcp(Mc);
+    } else {                                       // Troe fall-off
+        const double lnk0 = t3 + t4 * lnT - t5 * invT;
+        const double dlnk0 = (t4 + t5 * invT) * invT;
+        const double Pr = qss_exp(lnk0 - lnkinf) * Mc;
+        const double al = t6, i3 = t7, i1 = t8, T2s = t9;
+        const double e3 = qss_exp(-T * i3), e1x = qss_exp(-T * i1), e2 = qss_exp(-T2s * invT);
+        const double Fc = (1.0 - al) * e3 + al * e1x + e2;
+        const double L = log(Pr) * kInvLn10, Lc = log(Fc) * kInvLn10;
+        const double c = -0.4 - 0.67 * Lc, n = 0.75 - 1.27 * Lc;
+        const double num = L + c, den = n - 0.14 * num;
+        const double iden = qss_rcp(den);
+        const double f1 = num * iden;
+        const double ione_f = qss_rcp(1.0 + f1 * f1);
+        const double F = qss_exp(kLn10 * Lc * ione_f);
+        const double i1pr = qss_rcp(1.0 + Pr);
+        k = k * (Pr * i1pr) * F;
+        const double df1_dL = n * iden * iden;
+        const double dlF_dL = -2.0 * Lc * f1 * df1_dL * ione_f * ione_f;
+        dlm = (i1pr + dlF_dL) * qss_rcp(Mc);
+        if (JACT) {
+            const double dFc = -(1.0 - al) * i3 * e3 - al * i1 * e1x + T2s * invT * invT * e2;
+            const double df1_dLc = (-0.67 * den - num * (-1.27 + 0.14 * 0.67)) * iden * iden;
+            const double dlF_dLc = ione_f - 2.0 * Lc * f1 * df1_dLc * ione_f * ione_f;
+            const double delta = dlnk0 - dlnkinf;
+            dlnk = dlnkinf + delta * i1pr + dlF_dL * delta + dlF_dLc * dFc * qss_rcp(Fc);
+        }
+    }
+}
+
 #ifdef QSS_GEN
 // run-time specialised build (qss_jit.cpp): loads / stores with immediate offsets for the generated pass A
 template <int O> __device__ __forceinline__ double lS(unsigned b) {
@@ -200,36 +239,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                         Mc = fma(*reinterpret_cast<const double *>(&p.h[p.h_eff_val + 2 * e]), lds(sml + off), Mc);
                     }
                     double dlm;
-                    if (type == 1) {
-                        k *= Mc;
-                        dlm = qss_rcp(Mc);
-                    } else {                                       // Troe fall-off
-                        const double lnk0 = t3 + t4 * lnT - t5 * invT;
-                        const double dlnk0 = (t4 + t5 * invT) * invT;
-                        const double Pr = qss_exp(lnk0 - lnkinf) * Mc;
-                        const double al = t6, i3 = t7, i1 = t8, T2s = t9;
-                        const double e3 = qss_exp(-T * i3), e1x = qss_exp(-T * i1), e2 = qss_exp(-T2s * invT);
-                        const double Fc = (1.0 - al) * e3 + al * e1x + e2;
-                        const double L = log(Pr) * kInvLn10, Lc = log(Fc) * kInvLn10;
-                        const double c = -0.4 - 0.67 * Lc, n = 0.75 - 1.27 * Lc;
-                        const double num = L + c, den = n - 0.14 * num;
-                        const double iden = qss_rcp(den);
-                        const double f1 = num * iden;
-                        const double ione_f = qss_rcp(1.0 + f1 * f1);
-                        const double F = qss_exp(kLn10 * Lc * ione_f);
-                        const double i1pr = qss_rcp(1.0 + Pr);
-                        k = k * (Pr * i1pr) * F;
-                        const double df1_dL = n * iden * iden;
-                        const double dlF_dL = -2.0 * Lc * f1 * df1_dL * ione_f * ione_f;
-                        dlm = (i1pr + dlF_dL) * qss_rcp(Mc);
-                        if (JAC) {
-                            const double dFc = -(1.0 - al) * i3 * e3 - al * i1 * e1x + T2s * invT * invT * e2;
-                            const double df1_dLc = (-0.67 * den - num * (-1.27 + 0.14 * 0.67)) * iden * iden;
-                            const double dlF_dLc = ione_f - 2.0 * Lc * f1 * df1_dLc * ione_f * ione_f;
-                            const double delta = dlnk0 - dlnkinf;
-                            dlnk = dlnkinf + delta * i1pr + dlF_dL * delta + dlF_dLc * dFc * qss_rcp(Fc);
-                        }
-                    }
+                    qss_pressure_factor<JAC>(type, Mc, lnkinf, dlnkinf, t3, t4, t5, t6, t7, t8, t9, T, lnT, invT, k, dlm, dlnk);
                     if (JAC) SC(p.g_QM, tb) = dlm;
                 }
                 // reverse rate from the equilibrium constant; a disabled direction contributes nothing (G10)
