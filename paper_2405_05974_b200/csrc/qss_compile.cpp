@@ -583,6 +583,52 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
             for (int w = 0; w < nw; ++w) for (size_t d = 0; d < depth; ++d) P("%d, ", d < bin[w].size() ? bin[w][d] : -1);
             g += "-1};\n";
         }
+        // ---- P3 + P7 specialised: every closure slot, cross-group coupling and W_y entry is a signed sum of kappas (8-10
+        //      interpreter instructions per term, a dependent table -> kappa -> add chain); as straight-line code it is one
+        //      shared-memory read and one add per term (45 KB for cfg2: 8x fewer instructions, which pays for the instruction fetch)
+        {
+            struct Ent { std::string dst; std::vector<std::pair<int, int>> terms; };     // (byte offset of kappa, sign)
+            std::vector<Ent> ents;
+            for (auto &kv : *c.ce) {
+                Ent e; std::snprintf(b, sizeof b, "sS<%d>(sml, ", (v.s_CL + kv.first) * 256); e.dst = b;
+                for (int d : kv.second) e.terms.push_back({(v.s_KAP + d) * 256, 1});
+                ents.push_back(e);
+            }
+            for (size_t x = 0; x < c.xpl->size(); ++x) {
+                Ent e; std::snprintf(b, sizeof b, "sS<%d>(sml, ", (v.s_XP + (int)x) * 256); e.dst = b;
+                for (int d : (*c.xpl)[x].second) e.terms.push_back({(v.s_KAP + d) * 256, 1});
+                ents.push_back(e);
+            }
+            {
+                int eidx = 0;
+                for (auto &kv : wy) {
+                    Ent e; std::snprintf(b, sizeof b, "sG<%d>(sc, ", (v.g_WY + eidx) * 256); e.dst = b; ++eidx;
+                    for (int32_t w : kv.second) e.terms.push_back({v.s_KAP * 256 + (int)(w & 0x7fffffff), w < 0 ? -1 : 1});
+                    ents.push_back(e);
+                }
+            }
+            std::vector<int> idx(ents.size());
+            for (size_t i = 0; i < ents.size(); ++i) idx[i] = (int)i;
+            std::stable_sort(idx.begin(), idx.end(), [&](int a, int c2) { return ents[a].terms.size() > ents[c2].terms.size(); });
+            std::vector<std::vector<int>> bin(nw);
+            std::vector<double> load(nw, 0.0);
+            for (int i : idx) { const int w = (int)(std::min_element(load.begin(), load.end()) - load.begin()); bin[w].push_back(i); load[w] += 2.0 + ents[i].terms.size(); }
+            g += "__device__ __forceinline__ void qss_gen_gather(const int warp, const unsigned sml, double *sc) {\n    switch (warp) {\n";
+            for (int w = 0; w < nw; ++w) {
+                P("    case %d:\n", w);
+                for (int i : bin[w]) {
+                    g += "        " + ents[i].dst;
+                    if (ents[i].terms.empty()) g += "0.0";
+                    for (size_t t = 0; t < ents[i].terms.size(); ++t) {
+                        const auto &tm = ents[i].terms[t];
+                        P("%slS<%d>(sml)", t == 0 ? (tm.second < 0 ? "-" : "") : (tm.second < 0 ? " - " : " + "), tm.first);
+                    }
+                    g += ");\n";
+                }
+                g += "        break;\n";
+            }
+            g += "    default: break;\n    }\n}\n";
+        }
     }
     return true;
 }

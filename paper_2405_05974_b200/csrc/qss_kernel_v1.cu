@@ -117,6 +117,7 @@ template <int O> __device__ __forceinline__ double lS(unsigned b) {
     return v;
 }
 template <int O> __device__ __forceinline__ void sS(unsigned b, double v) { asm volatile("st.shared.f64 [%0+%1], %2;" ::"r"(b), "n"(O), "d"(v) : "memory"); }
+template <int O> __device__ __forceinline__ void sG(double *b, double v) { asm volatile("st.global.f64 [%0+%1], %2;" ::"l"(b), "n"(O), "d"(v) : "memory"); }
 template <int O> __device__ __forceinline__ double lG(const double *b) {
     double v;
     asm volatile("ld.global.f64 %0, [%1+%2];" : "=d"(v) : "l"(b), "n"(O) : "memory");
@@ -309,6 +310,10 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         }
         __syncthreads();
         QSS_TICK(2);
+#ifdef QSS_GEN
+        // ---- P3 + P7, specialised: signed sums of kappas as straight-line code (closure slots, couplings, W_y entries)
+        qss_gen_gather(warp, sml, sc);
+#else
         // ---- P3: closure assembly: every P / leak / p0 slot gathers the kappas feeding it (no atomics)
         for (int e = warp; e < p.n_centry; e += nw) {
             double acc = 0.0;
@@ -335,6 +340,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                 SC(p.g_WY, e) = acc;
             }
         }
+#endif
         __syncthreads();
         QSS_TICK(3);
         // ---- P4: closure solve, level by level of the condensed DAG; subtraction-free elimination
