@@ -583,6 +583,61 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
             for (int w = 0; w < nw; ++w) for (size_t d = 0; d < depth; ++d) P("%d, ", d < bin[w].size() ? bin[w][d] : -1);
             g += "-1};\n";
         }
+        // ---- P4 specialised: the closure solve of every group with its matrix in REGISTERS (the interpreter walks it through
+        //      shared memory: a chain of dependent ~30-cycle reads on one warp per group).  Same operations in the same order
+        //      as the interpreter (subtraction-free elimination, U = P / D for the dy/dx solves, forward substitution).
+        {
+            g += "__device__ __forceinline__ void qss_gen_closure(const int warp, const unsigned sml) {\n";
+            std::vector<std::vector<int>> by_level(c.n_levels);
+            for (int gi = 0; gi < c.n_groups; ++gi) by_level[(*c.lvl_of_group)[gi]].push_back(gi);
+            for (int l = 0; l < c.n_levels; ++l) {
+                g += "    switch (warp) {\n";
+                std::vector<std::vector<int>> bw(nw);
+                for (size_t i = 0; i < by_level[l].size(); ++i) bw[i % nw].push_back(by_level[l][i]);
+                for (int w = 0; w < nw; ++w) {
+                    if (bw[w].empty()) continue;
+                    P("    case %d: {\n", w);
+                    for (int gi : bw[w]) {
+                        const std::vector<int> &mem = (*c.members)[gi];
+                        const int sz = (int)mem.size(), base = v.s_CL + (*c.gbase)[gi];
+                        const int oL = base + sz * sz, oP0 = oL + sz, oID = oP0 + sz;
+                        g += "        {\n";
+                        for (int m = 0; m < sz; ++m) for (int j = 0; j < sz; ++j) if (m != j) P("            double a%d_%d = lS<%d>(sml);\n", m, j, (base + m * sz + j) * 256);
+                        for (int k = 0; k < sz; ++k) P("            double L%d = lS<%d>(sml), q%d = lS<%d>(sml), d%d;\n", k, (oL + k) * 256, k, (oP0 + k) * 256, k);
+                        for (int x = (*c.xp_begin)[gi]; x < (*c.xp_end)[gi]; ++x)
+                            P("            q%d += lS<%d>(sml) * lS<%d>(sml);\n", (*c.pos_in_grp)[(*c.xpl)[x].first.first], (v.s_XP + x) * 256, voff(N + 1 + (*c.xpl)[x].first.second));
+                        for (int k = sz - 1; k >= 1; --k) {
+                            P("            {   const double lk = L%d;\n                double Dk = lk;\n", k);
+                            for (int m = 0; m < k; ++m) P("                Dk += a%d_%d;\n", m, k);
+                            P("                const double iD = qss_rcp(Dk);\n                d%d = iD;\n", k);
+                            for (int jj = 0; jj < k; ++jj) {
+                                P("                {   const double f = a%d_%d * iD;\n                    L%d += f * lk;\n", k, jj, jj);
+                                for (int m = 0; m < k; ++m) if (m != jj) P("                    a%d_%d += a%d_%d * f;\n", m, jj, m, k);
+                                g += "                }\n";
+                            }
+                            g += "            }\n";
+                        }
+                        g += "            d0 = qss_rcp(L0);\n";
+                        for (int k = sz - 1; k >= 1; --k) {
+                            P("            {   const double iD = d%d, tk = q%d * iD;\n", k, k);
+                            for (int m = 0; m < k; ++m) P("                {   const double pmk = a%d_%d; a%d_%d = pmk * iD; q%d += pmk * tk; }\n", m, k, m, k, m);
+                            g += "            }\n";
+                        }
+                        for (int k = 0; k < sz; ++k) {
+                            P("            {   double acc = q%d;\n", k);
+                            for (int jj = 0; jj < k; ++jj) P("                acc += a%d_%d * q%d;\n", k, jj, jj);
+                            P("                acc *= d%d;\n                q%d = acc;\n                sS<%d>(sml, acc);\n            }\n", k, k, voff(N + 1 + mem[k]));
+                        }
+                        for (int m = 0; m < sz; ++m) for (int j = 0; j < sz; ++j) if (m != j) P("            sS<%d>(sml, a%d_%d);\n", (base + m * sz + j) * 256, m, j);
+                        for (int k = 0; k < sz; ++k) P("            sS<%d>(sml, d%d);\n", (oID + k) * 256, k);
+                        g += "        }\n";
+                    }
+                    g += "    } break;\n";
+                }
+                g += "    default: break;\n    }\n    __syncthreads();\n";
+            }
+            g += "}\n";
+        }
         // ---- P3 + P7 specialised: every closure slot, cross-group coupling and W_y entry is a signed sum of kappas (8-10
         //      interpreter instructions per term, a dependent table -> kappa -> add chain); as straight-line code it is one
         //      shared-memory read and one add per term (45 KB for cfg2: 8x fewer instructions, which pays for the instruction fetch)

@@ -345,6 +345,10 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         QSS_TICK(3);
         // ---- P4: closure solve, level by level of the condensed DAG; subtraction-free elimination
         //          (Eq. 6; readings G2, G8)
+#ifdef QSS_GEN
+        qss_gen_closure(warp, sml);        // (block barrier after every level inside)
+        QSS_TICK(4);
+#else
         for (int l = 0; l < p.n_levels; ++l) {
             for (int g = HT(p.h_level_ptr, l) + warp; g < HT(p.h_level_ptr, l + 1); g += nw) {
                 const int gi = p.h_group + g * QSS_GI_STRIDE;
@@ -384,6 +388,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             __syncthreads();
             QSS_TICK(4);
         }
+#endif
         // ---- P5: net rates of progress Q_j (Eq. 2), dQ/dT at fixed y and M, dQ/dM.  dlnk/dT, dlnKc/dT and dlnk/dM are L2
         //      reads (~700 cycles): those of 8 of the warp's reactions are in flight together.  dQ/dM goes to the scratch
         //      slab (the column streams read it) and to the dead g/RT rows of shared memory (the species sums read it).
