@@ -491,7 +491,7 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     //      one add per target row); the dy/dx solve is the same row operations on registers; the column is then written
     //      to the round buffer for pass B.  Same operations in the same order per row as the interpreter, except that the
     //      interpreter applies the records of a column in paired order (rounding-order difference only).
-    if (v.n_wy <= region) {                                  // (W_y must fit the time-shared region of the shared memory)
+    if (v.n_wy + N + nw <= region) {                         // (W_y and the staged inputs of the next slab must fit the time-shared region)
         std::string &g = out.v1_gen;
         char b[256];
         auto P = [&](const char *f, auto... a) { std::snprintf(b, sizeof b, f, a...); g += b; };

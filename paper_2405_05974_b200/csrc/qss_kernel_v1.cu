@@ -164,11 +164,28 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         const int64_t cell = slab * 32 + lane;
         const bool active = cell < p.ncells;
         const int64_t cc = active ? cell : p.ncells - 1;       // idle lanes of a ragged tail shadow the last cell
+#ifdef QSS_GEN
+        // ---- P0: the inputs of every slab but the block's first were fetched into spare shared-memory rows during the
+        //      previous slab's sweep (cp.async below); every warp waits for and moves the rows it fetched itself
+        double T;
+        const int st_row = p.s_KAP + p.n_wy;                     // [N] C rows, then one T row per warp
+        if (slab != blockIdx.x) {
+            asm volatile("cp.async.wait_all;" ::: "memory");
+            T = lds(sml + (st_row + N + warp) * 256);
+            for (int s = warp; s < N; s += nw) sts(sml + (p.s_V + s) * 256, lds(sml + (st_row + s) * 256));
+        } else {
+            T = p.T[cc];
+            for (int s = warp; s < N; s += nw) SM(p.s_V, s) = p.C[(size_t)s * ld + cc];
+        }
+        const double lnT = log(T), invT = 1.0 / T;
+        const double lnP0RT = kLnP0R - lnT;                    // ln(P0 / (R T))
+#else
         const double T = p.T[cc];
         const double lnT = log(T), invT = 1.0 / T;
         const double lnP0RT = kLnP0R - lnT;                    // ln(P0 / (R T))
         // ---- P0: stage the concentrations
         for (int s = warp; s < N; s += nw) SM(p.s_V, s) = p.C[(size_t)s * ld + cc];
+#endif
         if (warp == 0) { SM(p.s_V, N) = 1.0; SM(p.s_Z0, 0) = 0.0; SM(p.s_G, nsp) = 0.0; SM(p.s_H, nsp) = 0.0; }
         __syncthreads();
         QSS_TICK(0);
@@ -471,6 +488,13 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             }
             __syncthreads();
             QSS_TICK(11);
+            if (slab + gridDim.x < nslab) {      // inputs of the block's next slab -> spare rows behind W_y, under the sweep
+                const int64_t cell2 = (slab + gridDim.x) * 32 + lane;
+                const int64_t cc2 = cell2 < p.ncells ? cell2 : p.ncells - 1;
+                for (int s = warp; s < N; s += nw)
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sml + (st_row + s) * 256), "l"(p.C + (size_t)s * ld + cc2) : "memory");
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sml + (st_row + N + warp) * 256), "l"(p.T + cc2) : "memory");
+            }
             for (int d = 0; d < QSS_GEN_DEPTH; ++d) {
                 const int k = qss_gen_cols[warp * QSS_GEN_DEPTH + d];
                 if (k >= 0) qss_gen_column(k, sml, sc, p.jac + (size_t)(unsigned)k * (size_t)ld + cell, (long long)(N + 1) * ld, active);
