@@ -211,9 +211,15 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             const unsigned gbase = sml + p.s_G * 256, hbase = sml + p.s_H * 256, kbase = sml + p.s_KAP * 256;
             // records and Arrhenius parameters are stored in processing order; those of the warp's NEXT reaction are
             // fetched (L2 reads, the L1 is a few KB next to the shared memory) before the current one is evaluated
+            const int n_typed = p.n_tb;                            // third-body and fall-off reactions come first
+            // The typed reactions are latency-bound (one long chain of exponentials, logarithms and reciprocals per warp),
+            // the Arrhenius pairs issue-bound: half of the warps take the typed reactions first, the other half last, so
+            // that every scheduler always has both kinds to pick from.
+#pragma unroll 1
+            for (int pass = 0; pass < 2; ++pass) {
+            if ((pass == 0) == ((warp % 6) < 3)) {
             int4 nra = make_int4(0, 0, 0, 0), nrb = nra;
             double nq0 = 0.0, nq1 = 0.0, nq2 = 0.0, nq10 = 0.0;
-            const int n_typed = p.n_tb;                            // third-body and fall-off reactions come first
             if (warp < n_typed) {
                 nra = ldg_keep(reinterpret_cast<const int4 *>(gI + p.i_rrec + warp * QSS_V1_RREC), keep);
                 nrb = ldg_keep(reinterpret_cast<const int4 *>(gI + p.i_rrec + warp * QSS_V1_RREC + 4), keep);
@@ -270,7 +276,7 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
                 sts(kbase + j * 512 + 256, kb * vb);
                 if (JAC) { SC(p.g_DF, j) = dlnk; SC(p.g_DC, j) = dlnKc; }
             }
-                    QSS_TICK(14);
+            } else {
             // Arrhenius reactions, two at a time (four independent exponential chains): reads of both, arithmetic, stores
 #define QSS_RX_FETCH(R_, A_, B_, Q0_, Q1_, Q2_, Q10_)                                                            \
     if ((R_) < M) {                                                                                              \
@@ -324,6 +330,8 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
 #undef QSS_RX_FETCH
 #undef QSS_RX_READ
 #undef QSS_RX_STORE
+            }
+            }
         }
         __syncthreads();
         QSS_TICK(2);
