@@ -190,13 +190,29 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         __syncthreads();
         QSS_TICK(0);
         // ---- P1: NASA-7 thermo (readings G4, G9); total concentration
-        for (int s = warp; s < nsp; s += nw) {
-            const double *th = gD + p.d_thermo + s * QSS_TH_STRIDE;
-            const double *a = th + 1 + (T < th[0] ? 0 : 11);
-            const double h = a[0] + T * (a[1] + T * (a[2] + T * (a[3] + T * a[4]))) + a[5] * invT;
-            const double sR = a[0] * lnT + T * (a[6] + T * (a[7] + T * (a[8] + T * a[9]))) + a[10];
-            SM(p.s_H, s) = h;
-            SM(p.s_G, s) = h - sR;
+        //      the coefficients are L2 reads behind a data-dependent range select: those of three of the warp's species
+        //      are in flight together (two latencies per batch instead of two per species)
+        for (int s0 = warp; s0 < nsp; s0 += 3 * nw) {
+            const double *a[3];
+            double tm[3], cf[3][11];
+#pragma unroll
+            for (int u = 0; u < 3; ++u) tm[u] = ldg_keep(gD + p.d_thermo + min(s0 + u * nw, nsp - 1) * QSS_TH_STRIDE, keep);
+#pragma unroll
+            for (int u = 0; u < 3; ++u) {
+                a[u] = gD + p.d_thermo + min(s0 + u * nw, nsp - 1) * QSS_TH_STRIDE + 1 + (T < tm[u] ? 0 : 11);
+#pragma unroll
+                for (int i = 0; i < 11; ++i) cf[u][i] = ldg_keep(a[u] + i, keep);
+            }
+#pragma unroll
+            for (int u = 0; u < 3; ++u) {
+                const int s = s0 + u * nw;
+                if (s < nsp) {
+                    const double h = cf[u][0] + T * (cf[u][1] + T * (cf[u][2] + T * (cf[u][3] + T * cf[u][4]))) + cf[u][5] * invT;
+                    const double sR = cf[u][0] * lnT + T * (cf[u][6] + T * (cf[u][7] + T * (cf[u][8] + T * cf[u][9]))) + cf[u][10];
+                    SM(p.s_H, s) = h;
+                    SM(p.s_G, s) = h - sR;
+                }
+            }
         }
         if (warp == nw - 1) {
             double ct_ = 0.0;
