@@ -121,6 +121,22 @@ def test_table_interpreter_when_specialisation_is_off(monkeypatch):
     _check(mech, C, T, 77, "toy_dag (interpreter)")
 
 
+def test_specialised_and_interpreter_kernels_agree(monkeypatch):
+    """The run-time specialised Jacobian kernel (variant 2) and the table interpreter (variant 1) compute the same operations
+    per entry up to the order of the sums and FMA contraction: their Jacobians meet the parity gates against each other
+    (the oracle's running-error scale decides what "equal" means where terms cancel), their wdot agrees bit for bit (the wdot
+    path is the same code in both builds)."""
+    mech = qss_synth.config_mechanism(2)
+    n = 640 + 11
+    C, T = qss_synth.config_states(2, n)
+    a = _gpu_eval(mech, C, T, n)
+    monkeypatch.setenv("QSS_JIT", "0")
+    b = _gpu_eval(mech, C, T, n)
+    assert np.array_equal(a["wdot"][:, :n], b["wdot"][:, :n])
+    ref = oracle.evaluate(oracle.OracleMech(mech), C, T, n, want_jac=True, want_scale=True)
+    gates.assert_jac(a["jac"], b["jac"], ref["jscale"], n, "variant 2 against variant 1")
+
+
 def test_column_streams_in_global_memory(monkeypatch):
     """When the hot tables do not fit the kernel-parameter constant bank the column streams of the table interpreter move
     to global memory (QSS_CS_GLOBAL=1 forces it): same results."""
