@@ -30,7 +30,7 @@ if ROOT not in sys.path:
 
 METRIC = "cells/sec for wdot+analytical QSS Jacobian (fp64) per B200; % of roofline"
 UNIT = "cells/s"
-ORACLE_SAMPLE = {1: 4096, 2: 1 << 14, 3: 1 << 12, 4: 1 << 14, 5: 1 << 9}   # cells of the CPU-oracle sample
+ORACLE_SAMPLE = {1: 4096, 2: 1 << 15, 3: 1 << 12, 4: 1 << 15, 5: 1 << 9}   # cells of the CPU-oracle sample
 FP64_LANES_PER_SM = 64          # 148 SMs x 64 fp64 FMA lanes x 1.965 GHz
 
 
