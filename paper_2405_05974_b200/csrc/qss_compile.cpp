@@ -170,6 +170,7 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         }
         v.h_ss_ptr = at(); H.insert(H.end(), ptr.begin(), ptr.end());
         v.h_ss = at(); H.insert(H.end(), all.begin(), all.end());
+        H.push_back(0); H.push_back(0);                      // (the kernel's software pipeline reads two words past a list)
         v.h_st_ptr = at(); H.insert(H.end(), tptr.begin(), tptr.end());
         v.h_st = at(); H.insert(H.end(), tall.begin(), tall.end());
     }

@@ -472,16 +472,20 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
             for (int u = HT(p.h_ssw_ptr, warp); u < HT(p.h_ssw_ptr, warp + 1); ++u) {
                 const int s = HT(p.h_ssw, u);
                 double w = 0.0, et = 0.0, tv = 0.0;
+                // software pipeline: the table word two entries ahead and the values one entry ahead are read while the current
+                // entry is added (the words past the end of the list belong to the next list or table and address valid rows)
                 const int xe = HT(p.h_ss_ptr, s + 1);
-                for (int x = HT(p.h_ss_ptr, s); x < xe; ++x) {
-                    const int e = HT(p.h_ss, x), sg = e & 0x80000000;
-                    const unsigned a = kbase + (e & 0x7fffffff);
-                    const double q = lds(a);
-                    w += __hiloint2double(__double2hiint(q) ^ sg, __double2loint(q));
-                    if (JAC) {
-                        const double qt = lds(a + 256);
-                        et += __hiloint2double(__double2hiint(qt) ^ sg, __double2loint(qt));
-                    }
+                int x = HT(p.h_ss_ptr, s);
+                int e0 = HT(p.h_ss, x), e1 = HT(p.h_ss, x + 1);
+                double q0 = lds(kbase + (e0 & 0x7fffffff)), t0 = JAC ? lds(kbase + (e0 & 0x7fffffff) + 256) : 0.0;
+                for (; x < xe; ++x) {
+                    const int e2 = HT(p.h_ss, x + 2);
+                    const unsigned a1 = kbase + (e1 & 0x7fffffff);
+                    const double q1 = lds(a1), t1 = JAC ? lds(a1 + 256) : 0.0;
+                    const int sg = e0 & 0x80000000;
+                    w += __hiloint2double(__double2hiint(q0) ^ sg, __double2loint(q0));
+                    if (JAC) et += __hiloint2double(__double2hiint(t0) ^ sg, __double2loint(t0));
+                    e0 = e1; e1 = e2; q0 = q1; t0 = t1;
                 }
                 if (JAC) {
                     const int te = HT(p.h_st_ptr, s + 1);
