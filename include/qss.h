@@ -31,6 +31,11 @@
  * Preconditions NOT checked on the hot path: T > 0, C >= 0, every QSS species has a positive consumption
  * coefficient, third-body concentration > 0 for fall-off reactions.  NaN/Inf propagate.
  * There is no CPU fallback: without a CUDA device qss_mech_create fails with QSS_E_CUDA.
+ *
+ * Run-time specialisation: for mechanisms that fit the slab-smem kernel, qss_mech_create also generates CUDA source
+ * for this mechanism's Jacobian columns, closure gather and closure solve and compiles it with NVRTC (libnvrtc.so.12,
+ * opened with dlopen; seconds per mechanism and process).  Optional: without NVRTC the table-driven kernel computes the
+ * same thing (qss_mech_info.kernel_variant_jac tells which one runs; environment QSS_JIT=0 / 2).
  */
 #ifndef QSS_H
 #define QSS_H
