@@ -172,7 +172,9 @@ def main():
     C, T = qss_synth.config_states(cfg, n)
     n = min(n, C.shape[1]) if cfg == 4 else n
     ld = C.shape[1]
-    qm = qss.QssMech(mech, local)
+    t_create = time.perf_counter()
+    qm = qss.QssMech(mech, local)            # includes the run-time specialisation of the Jacobian kernel (NVRTC), untimed below
+    t_create = time.perf_counter() - t_create
     N = qm.N
     Cd = torch.from_numpy(C).to(dev); Td = torch.from_numpy(T).to(dev)
     J = torch.empty((N, N + 1, ld), dtype=torch.float64, device=dev)
@@ -306,7 +308,8 @@ def main():
         "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic", "config": _config(cfg, mech, n, world),
         "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps, "roofline": roof, "cpu_baseline": cpu,
-        "kernel_variant": {"wdot": info.kernel_variant_wdot, "jac": info.kernel_variant_jac}, "call": args.call}))
+        "kernel_variant": {"wdot": info.kernel_variant_wdot, "jac": info.kernel_variant_jac}, "mech_create_s": t_create,
+        "call": args.call}))
     if dist is not None:
         dist.destroy_process_group()
 
