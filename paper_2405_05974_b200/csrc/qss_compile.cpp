@@ -183,6 +183,16 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
             for (int u = 0; u < std::abs(e); ++u) wy[{x.sp, R[j].q[dir]}].push_back(((2 * j + dir) * 256) | (e < 0 ? (int32_t)0x80000000 : 0));
         }
     }
+    // the same sum direction by direction (specialised build): W_y dy/dx = sum over the enabled directions d that consume a QSS
+    // species q(d) of kappa_d dy_q(d)/dx nu_d -- one shared-memory read per DIRECTION instead of one per W_y entry
+    struct GenDir { int d, q; std::vector<std::pair<int, int>> tgt; };           // (transported species, signed coefficient)
+    std::vector<GenDir> gdir;
+    for (int j = 0; j < M; ++j) for (int dir = 0; dir < 2; ++dir) {
+        if (!((R[j].mask >> dir) & 1) || R[j].q[dir] < 0) continue;
+        GenDir gd{2 * j + dir, R[j].q[dir], {}};
+        for (const Term &x : R[j].net) if (x.sp < N) gd.tgt.push_back({x.sp, dir == 0 ? x.nu : -x.nu});
+        if (!gd.tgt.empty()) gdir.push_back(gd);
+    }
     std::vector<int32_t> wya_ptr{0}, wya_all;
     {
         std::vector<int32_t> rptr{0}, roff;
@@ -561,10 +571,23 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         }
         // J[:, k] = W_x[:, k] + W_y dy/dx_k (Eq. 7) in place on the registers of the column: W_y (per cell, n_wy rows,
         // row-major, ascending q within a row) was copied to shared memory behind the fixed state; then 35 coalesced stores
-        {
+        //   (by direction when that needs fewer rows than W_y has entries: kappa_d of the QSS-consuming directions was copied instead)
+        const bool by_dir = (int)gdir.size() <= v.n_wy && !std::getenv("QSS_GEN_WY");
+        if (by_dir) {
+            for (size_t r = 0; r < gdir.size(); ++r) {
+                P("    {   const double kd = lS<%d>(sml);\n", (v.s_KAP + (int)r) * 256);
+                for (auto &t : gdir[r].tgt) {
+                    const int a = std::abs(t.second);
+                    if (a == 1) P("        c%d = fma(%skd, c%d, c%d);\n", t.first, t.second < 0 ? "-" : "", N + gdir[r].q, t.first);
+                    else P("        c%d = fma(%skd * %d.0, c%d, c%d);\n", t.first, t.second < 0 ? "-" : "", a, N + gdir[r].q, t.first);
+                }
+                g += "    }\n";
+            }
+        } else {
             int e = 0;
             for (auto &kv : wy) { P("    c%d = fma(lS<%d>(sml), c%d, c%d);\n", kv.first.first, (v.s_KAP + e) * 256, N + kv.first.second, kv.first.first); ++e; }
         }
+        P("#define QSS_GEN_NROWS %d\n", by_dir ? (int)gdir.size() : v.n_wy);
         g += "    if (active) {\n";
         for (int i = 0; i < N; ++i) P("        __stcs(jc + %d * rs, c%d);\n", i, i);
         g += "    }\n}\n";
@@ -655,7 +678,13 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
                 for (int d : (*c.xpl)[x].second) e.terms.push_back({(v.s_KAP + d) * 256, 1});
                 ents.push_back(e);
             }
-            {
+            if (by_dir) {
+                for (size_t r = 0; r < gdir.size(); ++r) {       // kappa_d of the QSS-consuming directions -> scratch (kappa is overwritten by P5)
+                    Ent e; std::snprintf(b, sizeof b, "sG<%d>(sc, ", (v.g_WY + (int)r) * 256); e.dst = b;
+                    e.terms.push_back({(v.s_KAP + gdir[r].d) * 256, 1});
+                    ents.push_back(e);
+                }
+            } else {
                 int eidx = 0;
                 for (auto &kv : wy) {
                     Ent e; std::snprintf(b, sizeof b, "sG<%d>(sc, ", (v.g_WY + eidx) * 256); e.dst = b; ++eidx;

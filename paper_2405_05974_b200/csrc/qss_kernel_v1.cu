@@ -507,12 +507,13 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
 #ifdef QSS_GEN
             // ---- P8, specialised: W_y moves from the scratch slab to shared memory (the kappa region is free now); then each
             //      warp takes its columns one after the other, everything in registers (qss_gen_column), no barrier between
-            for (int e0 = warp * 8; e0 < p.n_wy; e0 += nw * 8) {
+            //      (QSS_GEN_NROWS rows: the W_y entries, or kappa_d of the QSS-consuming directions when those are fewer)
+            for (int e0 = warp * 8; e0 < QSS_GEN_NROWS; e0 += nw * 8) {
                 double t[8];
 #pragma unroll
-                for (int u = 0; u < 8; ++u) t[u] = ldg_pin(&SC(p.g_WY, min(e0 + u, p.n_wy - 1)));
+                for (int u = 0; u < 8; ++u) t[u] = ldg_pin(&SC(p.g_WY, min(e0 + u, QSS_GEN_NROWS - 1)));
 #pragma unroll
-                for (int u = 0; u < 8; ++u) if (e0 + u < p.n_wy) sts(sml + (p.s_KAP + e0 + u) * 256, t[u]);
+                for (int u = 0; u < 8; ++u) if (e0 + u < QSS_GEN_NROWS) sts(sml + (p.s_KAP + e0 + u) * 256, t[u]);
             }
             __syncthreads();
             QSS_TICK(11);
