@@ -16,9 +16,10 @@
 // float128 agreement, element null-space of every Jacobian column, N_q = 0 textbook Jacobian,
 // first-order FD convergence (App. C).
 //
-// Parity status: every function below is pinned by at least one of those; the Troe blending function
-// itself (not its limits or derivatives) has no independent library to compare against (Cantera is not
-// installed): "Troe F at intermediate Pr: parity unpinned" is recorded in DESIGN.md.
+// Parity status: every function below is pinned by at least one of those.  The Troe blending function at
+// intermediate Pr is pinned by hand-derived points (f1 = 0, +1, -1 and the pole of f1, each at two hand-computed
+// values of Fcent: tests/test_oracle_pins.py::test_troe_blending_hand_derived_points; every one of its five
+// constants and the roles of alpha, T***, T*, T** are separated: a mutation of any of them fails that test).
 #include "qss_oracle.h"
 
 #include <cmath>

@@ -178,8 +178,10 @@ def test_troe_lindemann_special_case():
 
 
 def test_troe_blending_and_limits():
-    """Troe F restated with mpmath at an intermediate Pr (a retyping check only: 'Troe F parity unpinned'
-    against any library), plus the high-pressure limit f1 -> -1/0.14 => F -> Fcent^(1/(1+0.14^-2))."""
+    """Troe F restated with mpmath at an intermediate Pr (a retyping check only; the pins of the blending function
+    are the hand-derived points of test_troe_blending_hand_derived_points below), plus the high-pressure limit
+    f1 -> -1/0.14 => F -> Fcent^(1/(1+0.14^-2)) (approached like 1/log10 Pr, hence the loose tolerance; the 0.14 itself
+    is pinned at the pole of f1 below)."""
     troe = (0.6, 120.0, 1500.0, 5000.0)
     m = _falloff_mech(troe)
     om = oracle.OracleMech(m)
@@ -205,6 +207,69 @@ def test_troe_blending_and_limits():
     _, kinf, Fc = k_ref(Chuge)
     expo = 1.0 / (1.0 + (1.0 / 0.14) ** 2)
     assert kf[0] == pytest.approx(float(kinf * Fc ** expo), rel=2e-2)     # approached like 1/log10(Pr)
+
+
+def _fcent_pinned(T, alpha, e3, e1, e2):
+    """Troe parameters for which the three exponentials of Fcent take the given VALUES at temperature T
+    (T*** = T/ln(1/e3), T* = T/ln(1/e1), T** = T ln(1/e2)), so that Fcent = (1-alpha) e3 + alpha e1 + e2 is a
+    number fixed by hand, not by any code."""
+    return (alpha, T / math.log(1.0 / e3), T / math.log(1.0 / e1), T * math.log(1.0 / e2))
+
+
+# (alpha, e3, e1, e2) -> Fcent by hand: 0.4*0.5 + 0.6*0.25 + 0.25 = 0.6 ; 0.75*0.125 + 0.25*0.5 + 0.0625 = 0.28125.
+# Swapping the roles of T*** and T* gives 0.65 / 0.46875, dropping the T** term 0.35 / 0.21875.
+_FCENT_CASES = [((0.6, 0.5, 0.25, 0.25), 0.6), ((0.25, 0.125, 0.5, 0.0625), 0.28125)]
+
+
+@pytest.mark.parametrize("case", [0, 1])
+@pytest.mark.parametrize("point", ["f1=0", "f1=+1", "f1=-1", "f1=inf"])
+def test_troe_blending_hand_derived_points(case, point):
+    """Pins the Troe blending F(Pr, Fcent) at intermediate Pr with values no code supplies (the rate forms are not in
+    the paper: the pins come from the mathematics).  With c = -0.4 - 0.67 log10 Fcent,
+    n = 0.75 - 1.27 log10 Fcent and f1 = (log10 Pr + c)/(n - 0.14 (log10 Pr + c)), log10 F = log10 Fcent/(1 + f1^2):
+      log10 Pr = -c             => f1 = 0    => F = Fcent
+      log10 Pr = n/1.14 - c     => f1 = +1   => F = Fcent^(1/2)
+      log10 Pr = -n/0.86 - c    => f1 = -1   => F = Fcent^(1/2)
+      log10 Pr = n/0.14 - c     => f1 = inf  => F = 1            (the pole of f1: pins the 0.14)
+    Each at two values of Fcent, so that every one of the five constants is separated: any single wrong or swapped
+    constant moves f1 away from the special value at one of these points and F changes in the 2nd-3rd digit."""
+    (alpha, e3, e1, e2), Fc = _FCENT_CASES[case]
+    T = 1400.0
+    m = _falloff_mech(_fcent_pinned(T, alpha, e3, e1, e2))
+    om = oracle.OracleMech(m)
+    kinf = _arr(1.0e10, 0.5, 2.0e4, T); k0 = _arr(1.0e12, -0.5, 1.0e4, T)
+    Lc = mp.log10(mp.mpf(Fc))
+    c = mp.mpf("-0.4") - mp.mpf("0.67") * Lc
+    n = mp.mpf("0.75") - mp.mpf("1.27") * Lc
+    L, F = {"f1=0": (-c, mp.mpf(Fc)), "f1=+1": (n / mp.mpf("1.14") - c, mp.sqrt(mp.mpf(Fc))),
+            "f1=-1": (-n / mp.mpf("0.86") - c, mp.sqrt(mp.mpf(Fc))), "f1=inf": (n / mp.mpf("0.14") - c, mp.mpf(1))}[point]
+    Pr = mp.mpf(10) ** L
+    M = Pr * kinf / k0                                  # third-body concentration that gives this Pr
+    C = np.array([float(M) * 0.25, float(M) * 0.25, 0.0])
+    C[2] = float((M - mp.mpf(C[0]) - mp.mpf(C[1])) / mp.mpf("2.5"))          # M = C0 + C1 + 2.5 C2
+    assert C[2] > 0
+    kf, _ = oracle.rate_constants(om, C, T)
+    tol = 1e-12 if point != "f1=inf" else 1e-10        # at the pole f1 ~ 1e15, F = Fcent^(1e-30)
+    assert kf[0] == pytest.approx(float(kinf * Pr / (1 + Pr) * F), rel=tol)
+    # the pin separates the constants: the neighbouring "wrong" values differ by far more than the tolerance
+    assert abs(float(mp.mpf(Fc) ** mp.mpf("0.5")) - Fc) > 1e-2
+
+
+def test_troe_chemkin_placeholder_parameters():
+    """CHEMKIN files use T*** ~ 1e-30 and T*, T** ~ 1e30 as placeholders for an absent term: the exponentials are then
+    exactly 0 / 1 / 0 and Fcent = alpha (the arguments -T/T*** = -1e33 are far outside any polynomial exp)."""
+    alpha = 0.37
+    m = _falloff_mech((alpha, 1.0e-30, 1.0e30, 1.0e30))
+    T = 1400.0
+    kinf = _arr(1.0e10, 0.5, 2.0e4, T); k0 = _arr(1.0e12, -0.5, 1.0e4, T)
+    Lc = mp.log10(mp.mpf(alpha))
+    c = mp.mpf("-0.4") - mp.mpf("0.67") * Lc
+    M = mp.mpf(10) ** (-c) * kinf / k0                  # f1 = 0 => F = Fcent = alpha
+    C = np.array([float(M) * 0.5, float(M) * 0.5, 0.0])
+    kf, _ = oracle.rate_constants(oracle.OracleMech(m), C, T)
+    Pr = k0 * (mp.mpf(C[0]) + mp.mpf(C[1])) / kinf
+    assert np.isfinite(kf[0])
+    assert kf[0] == pytest.approx(float(kinf * Pr / (1 + Pr) * alpha), rel=1e-12)
 
 
 # --------------------------------------------------------------------------------------------------
