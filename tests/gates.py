@@ -31,7 +31,9 @@ def wdot_gates(w, w_ref, S, n_cells=None):
     t2 = d <= bound2
     with np.errstate(divide="ignore", invalid="ignore"):
         ratio2 = np.where(bound2 > 0, d / bound2, np.where(d == 0, 0.0, np.inf))
+    t1_all = d <= WDOT_RTOL * np.abs(w_ref)
     return dict(finite=bool(finite), tier1_frac=float(t1.mean()) if t1.size else 1.0,
+                tier1_frac_unfiltered=float(t1_all.mean()) if t1_all.size else 1.0,
                 wellcond_frac=float(well.mean()) if well.size else 1.0,
                 tier2_all=bool(t2.all()), tier2_worst=float(ratio2.max()) if ratio2.size else 0.0)
 
@@ -55,6 +57,7 @@ def jac_gates(J, J_ref, J_scale, n_cells=None):
             # the guarded tier 2 still covers every column.
             well = s <= COL_COND_MAX * r
             out["col_wellcond_frac"] = float(well.mean()) if well.size else 1.0
+            out["col_tier1_frac_unfiltered"] = float(t1.mean()) if t1.size else 1.0
             t1 = t1[well]
         b2 = JAC_RTOL * r + JAC_GUARD * s
         with np.errstate(divide="ignore", invalid="ignore"):
@@ -71,17 +74,28 @@ def jac_gates(J, J_ref, J_scale, n_cells=None):
     return out
 
 
-def assert_wdot(w, w_ref, S, n_cells=None, what="wdot"):
+# Floors under the well-conditioned filter of tier 1 (reading G16): the filter depends on the ORACLE's data only
+# (S, w_ref, J_scale, J_ref), so a change that inflated the scales and hollowed out tier 1 would trip these.
+# Values: the fractions measured on the oracle (cfg1/2/3/5: wdot 0.987-0.996, columns 0.83-0.99; cfg4, the cold
+# 750 K background of the field where forward and reverse rates cancel: 0.96 / 0.48) minus a margin.
+WELLCOND_FLOOR = {1: (0.97, 0.75), 2: (0.97, 0.75), 3: (0.97, 0.75), 4: (0.93, 0.40), 5: (0.97, 0.75)}
+
+
+def assert_wdot(w, w_ref, S, n_cells=None, what="wdot", cfg=None):
     g = wdot_gates(w, w_ref, S, n_cells)
     assert g["finite"], f"{what}: non-finite values"
+    if cfg in WELLCOND_FLOOR:
+        assert g["wellcond_frac"] >= WELLCOND_FLOOR[cfg][0], f"{what}: well-conditioned fraction {g['wellcond_frac']:.4f} under its floor"
     assert g["tier1_frac"] >= TIER1_MIN_FRACTION, f"{what}: tier-1 pass fraction {g['tier1_frac']:.5f} < 0.99 ({g})"
     assert g["tier2_all"], f"{what}: tier-2 violated, worst ratio {g['tier2_worst']:.3g} ({g})"
     return g
 
 
-def assert_jac(J, J_ref, J_scale, n_cells=None, what="jac"):
+def assert_jac(J, J_ref, J_scale, n_cells=None, what="jac", cfg=None):
     g = jac_gates(J, J_ref, J_scale, n_cells)
     assert g["finite"], f"{what}: non-finite values"
+    if cfg in WELLCOND_FLOOR:
+        assert g["col_wellcond_frac"] >= WELLCOND_FLOOR[cfg][1], f"{what}: well-conditioned column fraction {g['col_wellcond_frac']:.4f} under its floor"
     for k in ("cell", "col"):
         assert g[f"{k}_tier1_frac"] >= TIER1_MIN_FRACTION, f"{what}: {k} tier-1 fraction {g[f'{k}_tier1_frac']:.5f} ({g})"
         assert g[f"{k}_tier2_all"], f"{what}: {k} tier-2 violated, worst {g[f'{k}_tier2_worst']:.3g} ({g})"

@@ -41,12 +41,12 @@ def _gpu_eval(mech, C, T, n_cells, want_jac=True):
     return out
 
 
-def _check(mech, C, T, n_cells, what, want_jac=True):
+def _check(mech, C, T, n_cells, what, want_jac=True, cfg=None):
     om = oracle.OracleMech(mech)
     ref = oracle.evaluate(om, C, T, n_cells, want_jac=want_jac, want_scale=want_jac)
     got = _gpu_eval(mech, C, T, n_cells, want_jac)
     n = n_cells
-    g = gates.assert_wdot(got["wdot"], ref["wdot"], ref["S"], n, what + " wdot")
+    g = gates.assert_wdot(got["wdot"], ref["wdot"], ref["S"], n, what + " wdot", cfg=cfg)
     if mech.n_qss:
         y, yr = got["cqss"][:, :n], ref["cqss"][:, :n]
         assert np.isfinite(y).all() and (y >= 0).all()
@@ -56,11 +56,14 @@ def _check(mech, C, T, n_cells, what, want_jac=True):
         assert np.isnan(got["wdot"][:, n:]).all(), what + ": wdot padding was written"
     if want_jac:
         gates.assert_wdot(got["wdot_from_jac"], ref["wdot"], ref["S"], n, what + " wdot (jac pass)")
-        gj = gates.assert_jac(got["jac"], ref["jac"], ref["jscale"], n, what + " jac")
+        gj = gates.assert_jac(got["jac"], ref["jac"], ref["jscale"], n, what + " jac", cfg=cfg)
         assert np.array_equal(got["jac"][:, :, :n], got["jac_only"][:, :, :n]), what + ": jac differs with/without wdot output"
         if C.shape[1] > n:
             assert np.isnan(got["jac"][:, :, n:]).all(), what + ": jac padding was written"
         g.update(gj)
+    if cfg is not None:      # G16 stays evidence: the unfiltered strict-tier fractions next to the filtered ones
+        print(f"[gates] {what}: wdot tier-1 {g['tier1_frac']:.4f} (unfiltered {g['tier1_frac_unfiltered']:.4f}, well-conditioned {g['wellcond_frac']:.4f})"
+              + (f"; columns tier-1 {g['col_tier1_frac']:.4f} (unfiltered {g['col_tier1_frac_unfiltered']:.4f}, well-conditioned {g['col_wellcond_frac']:.4f})" if want_jac else ""))
     return g
 
 
@@ -75,14 +78,14 @@ def test_toys(name):
 def test_cfg1_full():
     mech = qss_synth.config_mechanism(1)
     C, T = qss_synth.config_states(1)
-    _check(mech, C, T, 4096, "cfg1")
+    _check(mech, C, T, 4096, "cfg1", cfg=1)
 
 
 @pytest.mark.parametrize("cfg,n", [(2, 4096 + 37), (3, 1024 + 5), (5, 160 + 3)])
 def test_configs_small(cfg, n):
     mech = qss_synth.config_mechanism(cfg)
     C, T = qss_synth.config_states(cfg, n)
-    g = _check(mech, C, T, n, f"cfg{cfg}")
+    g = _check(mech, C, T, n, f"cfg{cfg}", cfg=cfg)
     print(f"cfg{cfg}", g)
 
 
@@ -151,7 +154,7 @@ def test_column_streams_in_global_memory(monkeypatch):
 def test_cfg4_field_small():
     mech = qss_synth.config_mechanism(4)
     C, T = qss_synth.config_states(4, 16 ** 3)           # 16^3 cells of the multipulse-shaped field
-    _check(mech, np.ascontiguousarray(C), np.ascontiguousarray(T), C.shape[1], "cfg4")
+    _check(mech, np.ascontiguousarray(C), np.ascontiguousarray(T), C.shape[1], "cfg4", cfg=4)
 
 
 @pytest.mark.parametrize("n", [1, 31, 32, 33])
@@ -289,8 +292,8 @@ def test_full_size_other_configs_sampled(cfg, nsample):
     del J, w
     Cs = np.ascontiguousarray(C[:, idx]); Ts = np.ascontiguousarray(T[idx])
     ref = oracle.evaluate(oracle.OracleMech(mech), Cs, Ts, want_jac=True, want_scale=True)
-    gates.assert_wdot(ws, ref["wdot"], ref["S"], what=f"cfg{cfg} full wdot")
-    gates.assert_jac(Js, ref["jac"], ref["jscale"], what=f"cfg{cfg} full jac")
+    gates.assert_wdot(ws, ref["wdot"], ref["S"], what=f"cfg{cfg} full wdot", cfg=cfg)
+    gates.assert_jac(Js, ref["jac"], ref["jscale"], what=f"cfg{cfg} full jac", cfg=cfg)
 
 
 def test_full_size_cfg2_sampled():
@@ -313,5 +316,5 @@ def test_full_size_cfg2_sampled():
     assert torch.isfinite(w).all() and torch.isfinite(J).all()
     Cs = np.ascontiguousarray(C[:, idx]); Ts = np.ascontiguousarray(T[idx])
     ref = oracle.evaluate(oracle.OracleMech(mech), Cs, Ts, want_jac=True, want_scale=True)
-    gates.assert_wdot(ws, ref["wdot"], ref["S"], what="cfg2 full wdot")
-    gates.assert_jac(Js, ref["jac"], ref["jscale"], what="cfg2 full jac")
+    gates.assert_wdot(ws, ref["wdot"], ref["S"], what="cfg2 full wdot", cfg=2)
+    gates.assert_jac(Js, ref["jac"], ref["jscale"], what="cfg2 full jac", cfg=2)

@@ -369,8 +369,13 @@ def test_double_oracle_meets_gates_against_float128(name):
     om = oracle.OracleMech(m)
     d = oracle.evaluate(om, C, T, n, want_scale=True)
     q = oracle.evaluate(om, C, T, n, want_scale=True, mode=oracle.EXPLICIT_F128)
-    gates.assert_wdot(d["wdot"], q["wdot"], q["S"], n, what=name)
-    gates.assert_jac(d["jac"], q["jac"], q["jscale"], n, what=name)
+    cfg = {"cfg1": 1, "cfg2": 2}.get(name)              # floors under the well-conditioned filter (gates.WELLCOND_FLOOR)
+    gw = gates.assert_wdot(d["wdot"], q["wdot"], q["S"], n, what=name, cfg=cfg)
+    gj = gates.assert_jac(d["jac"], q["jac"], q["jscale"], n, what=name, cfg=cfg)
+    # reading G16 as evidence: what the fp64 ORACLE itself reaches on the unfiltered strict tier against float128
+    print(f"[gates] oracle fp64 vs float128, {name}: wdot tier-1 unfiltered {gw['tier1_frac_unfiltered']:.4f} (filtered {gw['tier1_frac']:.4f}, "
+          f"well-conditioned {gw['wellcond_frac']:.4f}); columns unfiltered {gj['col_tier1_frac_unfiltered']:.4f} (filtered {gj['col_tier1_frac']:.4f}, "
+          f"well-conditioned {gj['col_wellcond_frac']:.4f})")
     assert np.allclose(d["cqss"][:, :n], q["cqss"][:, :n], rtol=1e-12)
 
 
