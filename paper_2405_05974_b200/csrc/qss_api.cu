@@ -35,6 +35,9 @@ struct qss_mech {
     long long *timing = nullptr;   // device counters when QSS_TIMING=1 (variant 1 only)
     int variant = 0;          // 0: general slab kernel (workspace in global memory); 1: slab-smem kernel (qss_kernel_v1.cu)
     QssJit *jit = nullptr;    // variant 1 with the Jacobian sweep's pass A specialised for this mechanism at run time (qss_jit.cpp)
+    QssJit *jit3 = nullptr;   // variant 3 (qss_kernel_v3.cu, generated per mechanism): the Jacobian kernel
+    double *dP3 = nullptr;    // variant 3: parameter blobs of the reaction-per-lane phases
+    int32_t *iP3 = nullptr;
 };
 
 namespace {
@@ -101,18 +104,40 @@ extern "C" int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech
     if (e == cudaSuccess && m->c.D.size()) e = cudaMemcpy(m->dD, m->c.D.data(), m->c.D.size() * sizeof(double), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(m->dI); cudaFree(m->dD); delete m; return cuda_fail(e, "cudaMemcpy(tables)"); }
     m->c.tab.I = m->dI; m->c.tab.D = m->dD;
-    // kernel selection: variant 1 when the mechanism fits it (QSS_VARIANT=0 in the environment forces the general kernel)
     const char *force = std::getenv("QSS_VARIANT");
-    if (m->c.v1_ok && !(force && force[0] == '0')) {
+    // kernel variant 3 (reaction-per-lane rate phases, everything generated per mechanism, NVRTC): the Jacobian kernel of
+    // choice when the mechanism fits it.  QSS_VARIANT=3 makes its absence an error; QSS_VARIANT=0/1/2 keep the older kernels.
+    const char *jit_env = std::getenv("QSS_JIT");            // QSS_JIT=0: no run-time compilation at all
+    const bool want3 = (!force || force[0] == '3') && !(jit_env && jit_env[0] == '0');
+    if (m->c.v3_ok && want3) {
+        std::string jerr;
+        m->jit3 = qss_jit3_create(m->c.v3.gen, true, prop.major, prop.minor, jerr);
+        if (m->jit3) {
+            const QssV3Host &h = m->c.v3;
+            if ((e = cudaMalloc(&m->dP3, h.dP.size() * sizeof(double))) == cudaSuccess) e = cudaMalloc(&m->iP3, h.iP.size() * sizeof(int32_t));
+            if (e == cudaSuccess) e = cudaMemcpy(m->dP3, h.dP.data(), h.dP.size() * sizeof(double), cudaMemcpyHostToDevice);
+            if (e == cudaSuccess) e = cudaMemcpy(m->iP3, h.iP.data(), h.iP.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) { qss_mech_destroy(m); return cuda_fail(e, "cudaMalloc/cudaMemcpy(variant 3 parameters)"); }
+        } else if (std::getenv("QSS_DEBUG") || (force && force[0] == '3')) {
+            std::fprintf(stderr, "[qss] kernel variant 3 unavailable: %s\n", jerr.c_str());
+        }
+        if (!m->jit3 && force && force[0] == '3') { qss_mech_destroy(m); return fail(QSS_E_CUDA, "QSS_VARIANT=3: " + jerr); }
+    } else if (force && force[0] == '3') {
+        const std::string w = m->c.v3_why;
+        qss_mech_destroy(m);
+        return fail(QSS_E_UNSUPPORTED, "QSS_VARIANT=3: kernel variant 3 does not apply: " + w);
+    }
+    if (m->jit3 && std::getenv("QSS_TIMING") && cudaMalloc(&m->timing, 32 * sizeof(long long)) == cudaSuccess) cudaMemset(m->timing, 0, 32 * sizeof(long long));
+    // kernel selection: variant 1 when the mechanism fits it (QSS_VARIANT=0 in the environment forces the general kernel)
+    if (m->c.v1_ok && !(force && force[0] == '0')) {   // (also the wdot-only kernel next to variant 3)
         if ((e = qss_v1_prepare()) != cudaSuccess) { cudaFree(m->dI); cudaFree(m->dD); delete m; return cuda_fail(e, "cudaFuncSetAttribute(variant 1)"); }
         m->variant = 1;
         m->nblocks = m->n_sm;
         m->c.v1.gI = m->dI; m->c.v1.gD = m->dD;
-        if (std::getenv("QSS_TIMING") && cudaMalloc(&m->timing, 16 * sizeof(long long)) == cudaSuccess) cudaMemset(m->timing, 0, 16 * sizeof(long long));
+        if (!m->timing && std::getenv("QSS_TIMING") && cudaMalloc(&m->timing, 16 * sizeof(long long)) == cudaSuccess) cudaMemset(m->timing, 0, 16 * sizeof(long long));
         // Jacobian kernel specialised for this mechanism (NVRTC); QSS_JIT=0 keeps the table interpreter, which is also what
         // runs when NVRTC is missing or the compilation fails (qss_mech_info.kernel_variant_jac tells which: 2 = specialised)
-        const char *jit_env = std::getenv("QSS_JIT");
-        if (!(jit_env && jit_env[0] == '0') && !m->c.v1_gen.empty()) {
+        if (!m->jit3 && !(jit_env && jit_env[0] == '0') && !m->c.v1_gen.empty()) {
             std::string jerr;
             m->jit = qss_jit_create(m->c.v1_gen, prop.major, prop.minor, jerr);
             if (!m->jit && (std::getenv("QSS_DEBUG") || (jit_env && jit_env[0] == '2'))) std::fprintf(stderr, "[qss] run-time specialisation unavailable: %s\n", jerr.c_str());
@@ -148,7 +173,11 @@ extern "C" int qss_mech_specialise_check(const qss_mech_desc_t *desc, int cc_maj
         rc = QSS_E_INVALID; err = std::string("mechanism compiler: ") + e.what();
     }
     if (rc != QSS_OK) return fail(rc, err);
-    if (!c.v1_ok) return fail(QSS_E_UNSUPPORTED, "kernel variant 1 does not apply: " + c.v1_why);
+    if (c.v3_ok) {
+        if (!qss_jit3_compile_only(c.v3.gen, true, cc_major, cc_minor, image_bytes, err)) return fail(QSS_E_CUDA, err);
+        return QSS_OK;
+    }
+    if (!c.v1_ok) return fail(QSS_E_UNSUPPORTED, "kernel variants 1-3 do not apply: " + c.v1_why + "; " + c.v3_why);
     if (!qss_jit_compile_only(c.v1_gen, cc_major, cc_minor, image_bytes, err)) return fail(QSS_E_CUDA, err);
     return QSS_OK;
 }
@@ -157,17 +186,24 @@ extern "C" int qss_mech_destroy(qss_mech_t *m) {
     if (!m) return QSS_OK;
     DeviceGuard guard(m->device);
     if (m->timing) {
-        long long t[16];
-        static const char *name[15] = {"P0 stage", "P1 thermo", "P2 Arrhenius+wait", "P3+P7 gather", "P4 closure", "P5 net rates", "P6 sums", "A: barrier wait", "B: barrier wait",
-                                        "B: tile", "B: stores", "A: init", "A: stream", "A: solve", "P2 third-body/fall-off"};
-        if (cudaMemcpy(t, m->timing, sizeof t, cudaMemcpyDeviceToHost) == cudaSuccess) {
+        long long t[32] = {0};
+        static const char *name1[15] = {"P0 stage", "P1 thermo", "P2 Arrhenius+wait", "P3+P7 gather", "P4 closure", "P5 net rates", "P6 sums", "A: barrier wait", "B: barrier wait",
+                                         "B: tile", "B: stores", "A: init", "A: stream", "A: solve", "P2 third-body/fall-off"};
+        static const char *name3[15] = {"P0 inputs", "P2 rate tasks", "P2 barrier wait", "P3 gather", "P4 closure", "P5 net tasks", "P6 sums", "kappa_d reload", "P8 columns",
+                                         "end barrier wait", "P2c kappa", "", "", "", ""};
+        const char **name = m->jit3 ? name3 : name1;
+        if (cudaMemcpy(t, m->timing, (m->jit3 ? 32 : 16) * sizeof(long long), cudaMemcpyDeviceToHost) == cudaSuccess) {
+            if (m->jit3) { std::fprintf(stderr, "[qss timing] rate phase per warp (cycles/1e6):"); for (int i = 16; i < 32; ++i) std::fprintf(stderr, " %.2f", (double)t[i] * 1e-6); std::fprintf(stderr, "\n"); }
             long long tot = 0;
             for (int i = 0; i < 15; ++i) tot += t[i];
             for (int i = 0; i < 15 && tot > 0; ++i) std::fprintf(stderr, "[qss timing] %-14s %6.2f %%\n", name[i], 100.0 * (double)t[i] / (double)tot);
         }
         cudaFree(m->timing);
     }
+    cudaDeviceSynchronize();          // no kernel of this handle may still run when its module is unloaded
     qss_jit_destroy(m->jit);
+    qss_jit_destroy(m->jit3);
+    cudaFree(m->dP3); cudaFree(m->iP3);
     if (m->copy_stream) { cudaStreamDestroy(m->copy_stream); cudaEventDestroy(m->ev[0]); cudaEventDestroy(m->ev[1]); }
     cudaFree(m->dI); cudaFree(m->dD);
     delete m;
@@ -175,6 +211,7 @@ extern "C" int qss_mech_destroy(qss_mech_t *m) {
 }
 
 static size_t ws_bytes(const qss_mech_t *m, bool jac) {
+    if (jac && m->jit3) return (size_t)m->c.v3.scratch_rows * 32 * sizeof(double) * (size_t)m->n_sm;
     if (m->variant == 1) return qss_v1_scratch_doubles(m->c.v1) * sizeof(double) * (size_t)m->nblocks;
     return qss_slab_ws_doubles(m->c.tab, jac, m->nwarp) * sizeof(double) * (size_t)m->nblocks;
 }
@@ -190,7 +227,7 @@ extern "C" int qss_mech_info(const qss_mech_t *m, qss_mech_info_t *o) {
     o->bytes_wdot = m->c.bytes_wdot; o->bytes_jac = m->c.bytes_jac;
     o->workspace_bytes_wdot = ws_bytes(m, false);
     o->workspace_bytes_jac = ws_bytes(m, true);
-    o->kernel_variant_wdot = m->variant; o->kernel_variant_jac = m->jit ? 2 : m->variant;
+    o->kernel_variant_wdot = m->variant; o->kernel_variant_jac = m->jit3 ? 3 : (m->jit ? 2 : m->variant);
     return QSS_OK;
 }
 
@@ -222,7 +259,13 @@ extern "C" int qss_eval_jac(const qss_mech_t *m, int64_t ncells, int64_t ld, con
     int rc = check_eval(m, ncells, ld, C, T, jac, workspace, workspace_bytes, m ? ws_bytes(m, true) : 0);
     if (rc != QSS_OK || ncells == 0) return rc;
     cudaError_t e;
-    if (m->variant == 1) {
+    if (m->jit3) {
+        QssV3 v;
+        v.C = C; v.T = T; v.wdot = wdot; v.cqss = nullptr; v.jac = jac; v.scratch = (double *)workspace;
+        v.ncells = ncells; v.ld = ld; v.scratch_stride = (int64_t)m->c.v3.scratch_rows * 32;
+        v.dP = m->dP3; v.iP = m->iP3; v.timing = m->timing;
+        e = qss_jit3_launch(m->jit3, v, m->n_sm, m->c.v3.nw, (size_t)m->c.v3.smem_bytes, (cudaStream_t)stream);
+    } else if (m->variant == 1) {
         QssV1 v = m->c.v1;
         v.C = C; v.T = T; v.wdot = wdot; v.cqss = nullptr; v.jac = jac; v.scratch = (double *)workspace; v.timing = m->timing;
         v.ncells = ncells; v.ld = ld; v.scratch_stride = (int64_t)qss_v1_scratch_doubles(v);

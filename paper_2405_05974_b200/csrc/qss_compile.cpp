@@ -6,6 +6,7 @@
 // gather / elimination schedules.  No symbolic expressions are generated (the paper's sympy + CSE path,
 // L262-276, is prior art here): the kernels interpret these tables.
 #include "qss_compile.h"
+#include "qss_ctx.h"
 
 #include <algorithm>
 #include <cmath>
@@ -15,18 +16,9 @@
 #include <cstring>
 #include <map>
 
+using namespace qssc;
+
 namespace {
-
-struct Term { int sp, nu; };
-
-struct Reaction {
-    int type, mask;
-    std::vector<Term> side[2];     // side[0] reactants, side[1] products (as given)
-    std::vector<Term> net;         // nu'' - nu', non-zero only
-    int q[2];                      // local QSS index consumed by direction 0 / 1, or -1
-    int dnu;
-    int tb;                        // index among third-body / fall-off reactions, or -1
-};
 
 std::string fmt(const char *f, int a = 0, int b = 0, int c = 0) {
     char buf[256];
@@ -85,16 +77,6 @@ int tarjan(int n, const std::vector<std::vector<int>> &adj, std::vector<int> &co
 // records, shared-memory / scratch layout.  Applies when the mechanism is small enough (see the checks below);
 // otherwise the general variant 0 is used.
 // ---------------------------------------------------------------------------------------------------------
-struct V1Ctx {
-    int N, Nq, M, nsp, n_tb, n_groups, n_levels, cl_size;
-    const std::vector<Reaction> *R;
-    const std::vector<std::vector<int>> *members;
-    const std::vector<int> *gbase, *xp_begin, *xp_end, *lvl_of_group, *pos_in_grp, *rorder;
-    const std::map<int, std::vector<int>> *ce;
-    const std::vector<std::pair<std::pair<int, int>, std::vector<int>>> *xpl;
-    const std::vector<std::vector<std::pair<int, double>>> *effc;
-};
-
 bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     const int N = c.N, Nq = c.Nq, M = c.M, nsp = c.nsp;
     const std::vector<Reaction> &R = *c.R;
@@ -1091,10 +1073,12 @@ int qss_compile(const qss_mech_desc_t *d, QssCompiled &out, std::string &err) {
     }
     {
         V1Ctx vc{N, Nq, M, nsp, n_tb, n_groups, n_levels, cl_size, &R, &members, &gbase, &xp_begin, &xp_end, &lvl_of_group,
-                 &pos_in_grp, &rorder, &ce, &xpl, &effc};
+                 &pos_in_grp, &rorder, &ce, &xpl, &effc, d};
         out.v1_ok = build_v1(vc, out, out.v1_why);
-        if (const char *dump = std::getenv("QSS_GEN_DUMP")) {            // debugging aid: the generated source of pass A
-            if (FILE *f = std::fopen(dump, "w")) { std::fwrite(out.v1_gen.data(), 1, out.v1_gen.size(), f); std::fclose(f); }
+        out.v3_ok = build_v3(vc, out, out.v3_why);
+        if (const char *dump = std::getenv("QSS_GEN_DUMP")) {            // debugging aid: the generated source (variant 3, else variant 2)
+            const std::string &g = out.v3_ok ? out.v3.gen : out.v1_gen;
+            if (FILE *f = std::fopen(dump, "w")) { std::fwrite(g.data(), 1, g.size(), f); std::fclose(f); }
         }
         if (std::getenv("QSS_DEBUG"))
             std::fprintf(stderr, "[qss] variant 1: %s%s (hot table %d/%d words, smem rows %d, scratch rows %d, rounds %d, solve ops %d)\n",

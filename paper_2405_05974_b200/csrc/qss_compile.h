@@ -7,6 +7,16 @@
 #include "../../include/qss.h"
 #include "qss_tables.h"
 #include "qss_v1.h"
+#include "qss_v3.h"
+
+// Host side of kernel variant 3 (qss_gen3.cpp): the generated header, the parameter blobs of the reaction-per-lane
+// phases and the launch geometry.
+struct QssV3Host {
+    std::string gen;               // text of qss_gen3.h for this mechanism
+    std::vector<double> dP;        // [QSS3_NDP][n_slot]
+    std::vector<int32_t> iP;       // [QSS3_NIP][n_slot]
+    int nw = 0, smem_bytes = 0, scratch_rows = 0, n_slot = 0, n_pp = 0, n_kq = 0, n_groups = 0;
+};
 
 struct QssCompiled {
     QssTab tab;                    // offsets filled in; I / D pointers are set after upload
@@ -20,6 +30,9 @@ struct QssCompiled {
     bool v1_ok = false;
     std::string v1_why;            // why variant 1 does not apply
     std::string v1_gen;            // CUDA source of the mechanism-specialised pass A (qss_gen_pass_a), compiled at run time
+    QssV3Host v3;                  // kernel variant 3 (valid iff v3_ok)
+    bool v3_ok = false;
+    std::string v3_why;
 };
 
 // Validates `desc` and builds the tables. Returns QSS_OK or a negative qss_status with `err` set.

@@ -4,9 +4,13 @@
 
 #include <dlfcn.h>
 #include <nvrtc.h>
+#include <sys/stat.h>
+#include <sys/types.h>
+#include <unistd.h>
 
 #include <cstdio>
 #include <cstdlib>
+#include <cstring>
 #include <map>
 #include <memory>
 #include <mutex>
@@ -59,27 +63,85 @@ const Nvrtc &nvrtc() {
 std::mutex g_mu;
 std::map<std::string, std::shared_ptr<std::vector<char>>> g_cubin;      // key: architecture + generated source
 
-std::shared_ptr<std::vector<char>> compile(const std::string &gen_src, const std::string &arch, std::string &err) {
-    const std::string key = arch + "\n" + gen_src;
+// ---- on-disk cache of compiled images: $QSS_CACHE_DIR, else $XDG_CACHE_HOME/libqss, else ~/.cache/libqss; QSS_CACHE=0
+//      turns it off.  The key hashes everything the image depends on (architecture, options, every embedded source, the
+//      generated header), so a new library build or another mechanism never finds a stale image.
+uint64_t fnv1a(const std::string &s, uint64_t h) {
+    for (unsigned char ch : s) { h ^= ch; h *= 1099511628211ull; }
+    return h;
+}
+
+std::string cache_path(const std::string &key) {
+    const char *off = std::getenv("QSS_CACHE");
+    if (off && off[0] == '0') return "";
+    std::string dir;
+    if (const char *d = std::getenv("QSS_CACHE_DIR")) dir = d;
+    else if (const char *x = std::getenv("XDG_CACHE_HOME")) dir = std::string(x) + "/libqss";
+    else if (const char *h = std::getenv("HOME")) dir = std::string(h) + "/.cache/libqss";
+    if (dir.empty()) return "";
+    std::string full = key;
+    for (int i = 0; i < qss_embed_count; ++i) { full += qss_embed_name[i]; full += qss_embed_text[i]; }
+    char name[64];
+    std::snprintf(name, sizeof name, "/%016llx%016llx.cubin", (unsigned long long)fnv1a(full, 14695981039346656037ull),
+                  (unsigned long long)fnv1a(full, 0x9e3779b97f4a7c15ull));
+    // mkdir -p (two levels are enough for the defaults)
+    const size_t cut = dir.find_last_of('/');
+    if (cut != std::string::npos && cut > 0) mkdir(dir.substr(0, cut).c_str(), 0700);
+    mkdir(dir.c_str(), 0700);
+    return dir + name;
+}
+
+std::shared_ptr<std::vector<char>> cache_load(const std::string &path) {
+    if (path.empty()) return nullptr;
+    FILE *f = std::fopen(path.c_str(), "rb");
+    if (!f) return nullptr;
+    std::fseek(f, 0, SEEK_END);
+    const long sz = std::ftell(f);
+    std::fseek(f, 0, SEEK_SET);
+    auto bin = std::make_shared<std::vector<char>>(sz > 0 ? (size_t)sz : 0);
+    const bool ok = sz > 64 && std::fread(bin->data(), 1, (size_t)sz, f) == (size_t)sz && std::memcmp(bin->data(), "\x7f" "ELF", 4) == 0;
+    std::fclose(f);
+    return ok ? bin : nullptr;
+}
+
+void cache_store(const std::string &path, const std::vector<char> &bin) {
+    if (path.empty()) return;
+    const std::string tmp = path + ".tmp" + std::to_string((long long)getpid());
+    FILE *f = std::fopen(tmp.c_str(), "wb");
+    if (!f) return;
+    const bool ok = std::fwrite(bin.data(), 1, bin.size(), f) == bin.size();
+    std::fclose(f);
+    if (!ok || std::rename(tmp.c_str(), path.c_str()) != 0) std::remove(tmp.c_str());
+}
+
+// main_name: embedded source that holds the kernel; gen_name / gen_src: the generated header it includes; defs: -D options
+std::shared_ptr<std::vector<char>> compile(const std::string &main_name, const std::string &gen_name, const std::string &gen_src,
+                                           const std::vector<std::string> &defs, const std::string &arch, std::string &err) {
+    std::string key = arch + "\n" + main_name + "\n";
+    for (const std::string &dd : defs) key += dd + "\n";
+    key += gen_src;
     std::lock_guard<std::mutex> lock(g_mu);
     auto it = g_cubin.find(key);
     if (it != g_cubin.end()) return it->second;
+    const std::string cpath = cache_path(key);
+    if (auto hit = cache_load(cpath)) { g_cubin[key] = hit; return hit; }
     const Nvrtc &n = nvrtc();
     if (!n.ok) { err = "NVRTC (libnvrtc.so.12) not found"; return nullptr; }
     std::vector<const char *> names, texts;
     const char *main_src = nullptr;
     for (int i = 0; i < qss_embed_count; ++i) {
-        if (std::string(qss_embed_name[i]) == "qss_kernel_v1.cu") main_src = qss_embed_text[i];
+        if (main_name == qss_embed_name[i]) main_src = qss_embed_text[i];
         else { names.push_back(qss_embed_name[i]); texts.push_back(qss_embed_text[i]); }
     }
     if (!main_src) { err = "kernel source not embedded"; return nullptr; }
-    names.push_back("qss_gen.h"); texts.push_back(gen_src.c_str());
+    names.push_back(gen_name.c_str()); texts.push_back(gen_src.c_str());
     nvrtcProgram prog = nullptr;
-    nvrtcResult r = n.createProgram(&prog, main_src, "qss_kernel_v1.cu", (int)names.size(), texts.data(), names.data());
+    nvrtcResult r = n.createProgram(&prog, main_src, main_name.c_str(), (int)names.size(), texts.data(), names.data());
     if (r != NVRTC_SUCCESS) { err = std::string("nvrtcCreateProgram: ") + n.getErrorString(r); return nullptr; }
     const std::string archopt = "--gpu-architecture=" + arch;
-    const char *opts[] = {archopt.c_str(), "-std=c++17", "-DQSS_GEN", "-lineinfo", "--fmad=true"};
-    r = n.compileProgram(prog, (int)(sizeof opts / sizeof opts[0]), opts);
+    std::vector<const char *> opts = {archopt.c_str(), "-std=c++17", "-lineinfo", "--fmad=true"};
+    for (const std::string &dd : defs) opts.push_back(dd.c_str());
+    r = n.compileProgram(prog, (int)opts.size(), opts.data());
     if (r != NVRTC_SUCCESS) {
         size_t ls = 0;
         n.getProgramLogSize(prog, &ls);
@@ -99,28 +161,21 @@ std::shared_ptr<std::vector<char>> compile(const std::string &gen_src, const std
     if (const char *dump = std::getenv("QSS_JIT_DUMP")) {       // debugging aid: the device image, for cuobjdump -sass
         if (FILE *f = std::fopen(dump, "wb")) { std::fwrite(bin->data(), 1, bin->size(), f); std::fclose(f); }
     }
+    cache_store(cpath, *bin);
     g_cubin[key] = bin;
     return bin;
 }
 
-}  // namespace
-
-bool qss_jit_compile_only(const std::string &gen_src, int cc_major, int cc_minor, size_t *image_bytes, std::string &err) {
+std::string arch_of(int cc_major, int cc_minor) {
     char arch[32];
     std::snprintf(arch, sizeof arch, "sm_%d%d%s", cc_major, cc_minor, cc_major >= 9 ? "a" : "");
-    std::shared_ptr<std::vector<char>> bin = compile(gen_src, arch, err);
-    if (bin && image_bytes) *image_bytes = bin->size();
-    return (bool)bin;
+    return arch;
 }
 
-QssJit *qss_jit_create(const std::string &gen_src, int cc_major, int cc_minor, std::string &err) {
-    char arch[32];
-    std::snprintf(arch, sizeof arch, "sm_%d%d%s", cc_major, cc_minor, cc_major >= 9 ? "a" : "");
-    std::shared_ptr<std::vector<char>> bin = compile(gen_src, arch, err);
-    if (!bin) return nullptr;
+QssJit *load_image(const std::vector<char> &bin, const char *kernel, std::string &err) {
     QssJit *j = new QssJit();
-    cudaError_t e = cudaLibraryLoadData(&j->lib, bin->data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
-    if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->kernel, j->lib, "qss_v1_jit");
+    cudaError_t e = cudaLibraryLoadData(&j->lib, bin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
+    if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->kernel, j->lib, kernel);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(reinterpret_cast<const void *>(j->kernel), cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) {
         err = std::string("loading the specialised kernel: ") + cudaGetErrorString(e);
@@ -130,6 +185,47 @@ QssJit *qss_jit_create(const std::string &gen_src, int cc_major, int cc_minor, s
         return nullptr;
     }
     return j;
+}
+
+}  // namespace
+
+std::vector<std::string> defs3(bool jac);
+
+bool qss_jit_compile_only(const std::string &gen_src, int cc_major, int cc_minor, size_t *image_bytes, std::string &err) {
+    std::shared_ptr<std::vector<char>> bin = compile("qss_kernel_v1.cu", "qss_gen.h", gen_src, {"-DQSS_GEN"}, arch_of(cc_major, cc_minor), err);
+    if (bin && image_bytes) *image_bytes = bin->size();
+    return (bool)bin;
+}
+
+QssJit *qss_jit_create(const std::string &gen_src, int cc_major, int cc_minor, std::string &err) {
+    std::shared_ptr<std::vector<char>> bin = compile("qss_kernel_v1.cu", "qss_gen.h", gen_src, {"-DQSS_GEN"}, arch_of(cc_major, cc_minor), err);
+    return bin ? load_image(*bin, "qss_v1_jit", err) : nullptr;
+}
+
+std::vector<std::string> defs3(bool jac) {
+    std::vector<std::string> d = {jac ? "-DQSS3_JAC=1" : "-DQSS3_JAC=0"};
+    if (std::getenv("QSS_TIMING")) d.push_back("-DQSS3_TIMING=1");
+    if (const char *x = std::getenv("QSS3_EXP")) d.push_back(std::string("-DQSS3_EXP=") + x);      // (experiments; removed before release)
+    return d;
+}
+
+bool qss_jit3_compile_only(const std::string &gen_src, bool jac, int cc_major, int cc_minor, size_t *image_bytes, std::string &err) {
+    std::shared_ptr<std::vector<char>> bin = compile("qss_kernel_v3.cu", "qss_gen3.h", gen_src, defs3(jac), arch_of(cc_major, cc_minor), err);
+    if (bin && image_bytes) *image_bytes = bin->size();
+    return (bool)bin;
+}
+
+QssJit *qss_jit3_create(const std::string &gen_src, bool jac, int cc_major, int cc_minor, std::string &err) {
+    std::shared_ptr<std::vector<char>> bin = compile("qss_kernel_v3.cu", "qss_gen3.h", gen_src, defs3(jac), arch_of(cc_major, cc_minor), err);
+    return bin ? load_image(*bin, jac ? "qss_v3_jac" : "qss_v3_wdot", err) : nullptr;
+}
+
+cudaError_t qss_jit3_launch(const QssJit *j, const QssV3 &v, int nblocks, int nw, size_t smem_bytes, cudaStream_t stream) {
+    const int64_t nslab = (v.ncells + 31) / 32;
+    if (nslab == 0) return cudaSuccess;
+    const int grid = (int)(nslab < nblocks ? nslab : nblocks);
+    void *args[] = {const_cast<QssV3 *>(&v)};
+    return cudaLaunchKernel(reinterpret_cast<const void *>(j->kernel), dim3(grid), dim3(nw * 32), args, smem_bytes, stream);
 }
 
 cudaError_t qss_jit_launch(const QssJit *j, const QssV1 &v, int nblocks, cudaStream_t stream) {

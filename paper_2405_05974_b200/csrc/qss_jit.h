@@ -11,6 +11,7 @@
 #include <string>
 
 #include "qss_v1.h"
+#include "qss_v3.h"
 
 struct QssJit;
 
@@ -21,5 +22,12 @@ QssJit *qss_jit_create(const std::string &gen_src, int cc_major, int cc_minor, s
 bool qss_jit_compile_only(const std::string &gen_src, int cc_major, int cc_minor, size_t *image_bytes, std::string &err);
 cudaError_t qss_jit_launch(const QssJit *j, const QssV1 &v, int nblocks, cudaStream_t stream);
 void qss_jit_destroy(QssJit *j);
+
+// Kernel variant 3 (qss_kernel_v3.cu + the generated qss_gen3.h): exists only as a run-time compiled program.  `jac`
+// selects the Jacobian build (kernel qss_v3_jac) or the wdot-only build (qss_v3_wdot).  Compiled images are cached per
+// process and on disk ($QSS_CACHE_DIR, default ~/.cache/libqss; QSS_CACHE=0 disables), keyed by a hash of every source.
+QssJit *qss_jit3_create(const std::string &gen_src, bool jac, int cc_major, int cc_minor, std::string &err);
+bool qss_jit3_compile_only(const std::string &gen_src, bool jac, int cc_major, int cc_minor, size_t *image_bytes, std::string &err);
+cudaError_t qss_jit3_launch(const QssJit *j, const QssV3 &v, int nblocks, int nw, size_t smem_bytes, cudaStream_t stream);
 
 #endif
