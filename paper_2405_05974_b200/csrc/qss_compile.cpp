@@ -1080,6 +1080,7 @@ int qss_compile(const qss_mech_desc_t *d, QssCompiled &out, std::string &err) {
             const std::string &g = out.v3_ok ? out.v3.gen : out.v1_gen;
             if (FILE *f = std::fopen(dump, "w")) { std::fwrite(g.data(), 1, g.size(), f); std::fclose(f); }
         }
+        if (std::getenv("QSS_DEBUG")) std::fprintf(stderr, "[qss] variant 3: %s%s\n", out.v3_ok ? "ok" : "not applicable: ", out.v3_ok ? "" : out.v3_why.c_str());
         if (std::getenv("QSS_DEBUG"))
             std::fprintf(stderr, "[qss] variant 1: %s%s (hot table %d/%d words, smem rows %d, scratch rows %d, rounds %d, solve ops %d)\n",
                          out.v1_ok ? "ok" : "not applicable: ", out.v1_ok ? "" : out.v1_why.c_str(), out.v1.h_used, QSS_V1_HMAX,

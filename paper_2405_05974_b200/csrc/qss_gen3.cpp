@@ -213,7 +213,7 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
     std::vector<Task> rsorted, nsorted;
     std::vector<int> rptr, nptr;
     {
-        const double rate_cost[3] = {130.0, 230.0, 800.0}, net_cost[3] = {1.0, 1.1, 1.1};
+        const double rate_cost[3] = {130.0, 240.0, 900.0}, net_cost[3] = {1.0, 1.1, 1.1};
         partition(rate_cost, 2, rsorted, rptr);
         partition(net_cost, 4, nsorted, nptr);
     }
@@ -293,29 +293,36 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
         for (const Task &t : nsorted) { d2.push_back(t.slot0); d2.push_back(t.c0); d2.push_back(t.c1); d2.push_back(0); }
         tput("T_RT_PTR", a2); tput("T_RT", b2); tput("T_NT_PTR", c2); tput("T_NT", d2);
     }
-    // ---- species sums: per species the added terms, then the subtracted terms, one table word (byte offset of the Q_j row)
-    //      per unit of |nu|, each list padded to a multiple of four words with the zero row; third-body lists: offset | sign bit
+    // ---- species sums: per species the added terms, then the subtracted terms, one table word (byte offset of the row) per
+    //      unit of |nu| (two 16-bit row numbers per 32-bit word), each list padded to a multiple of four words with the row that stays zero; T_SS_PTR: the Q_j lists
+    //      (wdot, T-column vector), T_ST_PTR: the dQ_j/dM lists (third-body vector), both index the same word array
     {
-        std::vector<std::vector<int32_t>> sp(nsp), sm(nsp), st(nsp);
+        std::vector<std::vector<int32_t>> sp(nsp), sm(nsp), tp(nsp), tm(nsp);
         for (int j = 0; j < M; ++j) if (R[j].mask) for (const Term &x : R[j].net) for (int u = 0; u < std::abs(x.nu); ++u) {
-            (x.nu > 0 ? sp : sm)[x.sp].push_back((R_KAP + pos[j]) * PITCH);
-            if (R[j].tb >= 0) st[x.sp].push_back(((R_DLM + R[j].tb) * PITCH) | (x.nu < 0 ? (int32_t)0x80000000 : 0));
+            (x.nu > 0 ? sp : sm)[x.sp].push_back(R_KAP + pos[j]);
+            if (R[j].tb >= 0) (x.nu > 0 ? tp : tm)[x.sp].push_back(R_DLM + R[j].tb);
         }
         std::vector<double> cost(nsp);
-        for (int s2 = 0; s2 < nsp; ++s2) cost[s2] = 10.0 + sp[s2].size() + sm[s2].size() + 1.5 * st[s2].size();
+        for (int s2 = 0; s2 < nsp; ++s2) cost[s2] = 16.0 + sp[s2].size() + sm[s2].size() + 0.6 * (tp[s2].size() + tm[s2].size());
         const std::vector<int> bin = lpt(cost, NW);
-        std::vector<int32_t> ptr{0}, all, tptr{0}, tall, wptr{0}, wall;
-        for (int s2 = 0; s2 < nsp; ++s2) {
-            for (auto *l : {&sp[s2], &sm[s2]}) {
+        std::vector<int32_t> ptr, all, tptr, wptr{0}, wall;
+        auto lists = [&](std::vector<std::vector<int32_t>> &a, std::vector<std::vector<int32_t>> &b2, std::vector<int32_t> &pp) {
+            pp.push_back((int32_t)all.size());
+            for (int s2 = 0; s2 < nsp; ++s2) for (auto *l : {&a[s2], &b2[s2]}) {
                 all.insert(all.end(), l->begin(), l->end());
-                while (all.size() % 4) all.push_back((R_KAP + M) * PITCH);
-                ptr.push_back((int32_t)all.size());
+                while (all.size() % 4) all.push_back(R_KAP + M);
+                pp.push_back((int32_t)all.size());
             }
-            tall.insert(tall.end(), st[s2].begin(), st[s2].end()); tptr.push_back((int32_t)tall.size());
-        }
+        };
+        lists(sp, sm, ptr);
+        lists(tp, tm, tptr);
+        for (int u = 0; u < 8; ++u) all.push_back(R_KAP + M);      // (the software pipeline reads two steps past a list)
+        // two 16-bit row numbers per word; the pointers count terms
+        std::vector<int32_t> packed;
+        for (size_t i = 0; i < all.size(); i += 2) packed.push_back(all[i] | (all[i + 1] << 16));
         for (int w = 0; w < NW; ++w) { for (int s2 = 0; s2 < nsp; ++s2) if (bin[s2] == w) wall.push_back(s2); wptr.push_back((int32_t)wall.size()); }
-        while (tabw.size() % 4) tabw.push_back(0);
-        tput("T_SS", all); tput("T_SS_PTR", ptr); tput("T_ST_PTR", tptr); tput("T_ST", tall); tput("T_SSW_PTR", wptr); tput("T_SSW", wall);
+        while (tabw.size() % 2) tabw.push_back(0);
+        tput("T_SS", packed); tput("T_SS_PTR", ptr); tput("T_ST_PTR", tptr); tput("T_SSW_PTR", wptr); tput("T_SSW", wall);
     }
     {
         if (rows & 1) ++rows;                                 // (the tables are read 16 bytes at a time)

@@ -186,8 +186,11 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
         // ---- P0: stage the concentrations
         for (int s = warp; s < N; s += nw) SM(p.s_V, s) = p.C[(size_t)s * ld + cc];
 #endif
-        if (warp == 0) { SM(p.s_V, N) = 1.0; SM(p.s_Z0, 0) = 0.0; SM(p.s_G, nsp) = 0.0; SM(p.s_H, nsp) = 0.0; }
+        if (warp == 0) { SM(p.s_V, N) = 1.0; SM(p.s_Z0, 0) = 0.0; }
         __syncthreads();
+        // (the zero rows behind g/RT and h/RT lie in the time-shared region and may coincide with staged input rows of other
+        //  warps: they are written only now, after every warp has moved its staged rows; P2, behind the next barrier, reads them)
+        if (warp == 0) { SM(p.s_G, nsp) = 0.0; SM(p.s_H, nsp) = 0.0; }
         QSS_TICK(0);
         // ---- P1: NASA-7 thermo (readings G4, G9); total concentration
         //      the coefficients are L2 reads behind a data-dependent range select: those of three of the warp's species

@@ -90,21 +90,36 @@ def test_configs_small(cfg, n):
 
 
 def test_kernel_variants_selected_and_general_kernel_on_cfg2(monkeypatch):
-    """cfg1/cfg2 run on kernel variant 1 (slab-smem), their Jacobian on its run-time specialised build (2); cfg3 on the
-    general variant 0; QSS_VARIANT=0 forces the general kernel, which must meet the same gates on cfg2."""
+    """cfg1/cfg2: the Jacobian runs on kernel variant 3 (generated per mechanism, reaction-per-lane rate phases), wdot alone on
+    variant 1 (slab-smem interpreter); cfg3 on the general variant 0.  QSS_VARIANT=2 selects the round-1 specialised kernel,
+    QSS_VARIANT=0 the general kernel: both must meet the same gates on cfg2.  A silent fall-back would show up here."""
     import paper_2405_05974_b200 as qss
-    for cfg, want_jac, want_wdot in ((1, 2, 1), (2, 2, 1), (3, 0, 0)):
+    for cfg, want_jac, want_wdot in ((1, 3, 1), (2, 3, 1), (3, 0, 0)):
         qm = qss.QssMech(qss_synth.config_mechanism(cfg), 0)
         assert qm.info.kernel_variant_jac == want_jac and qm.info.kernel_variant_wdot == want_wdot
         qm.close()
-    monkeypatch.setenv("QSS_VARIANT", "0")
     mech = qss_synth.config_mechanism(2)
-    qm = qss.QssMech(mech, 0)
-    assert qm.info.kernel_variant_jac == 0
-    qm.close()
     n = 256 + 9
     C, T = qss_synth.config_states(2, n)
-    _check(mech, C, T, n, "cfg2 (variant 0)")
+    for force, want in (("2", 2), ("0", 0)):
+        monkeypatch.setenv("QSS_VARIANT", force)
+        qm = qss.QssMech(mech, 0)
+        assert qm.info.kernel_variant_jac == want
+        qm.close()
+        _check(mech, C, T, n, f"cfg2 (variant {want})")
+
+
+@pytest.mark.parametrize("name", ["toy1", "toy2", "toy3", "toy_dag"])
+@pytest.mark.parametrize("variant", ["2", "3"])
+def test_many_slabs_per_block_on_small_mechanisms(name, variant, monkeypatch):
+    """More than 2 * 32 * n_SM cells, so that every persistent block takes a 2nd and later slab: their inputs come through the
+    cp.async staging rows (in variant 2 those rows could coincide with the zero rows of the thermo tables and a
+    staged T was overwritten with 0 -> NaN; no earlier test reached it, the toys ran one slab per block)."""
+    monkeypatch.setenv("QSS_VARIANT", variant)
+    mech = getattr(qss_synth, name)()
+    n = 20000 + 7
+    C, T = make_states(mech.n_nqss, n, seed=9)
+    _check(mech, C, T, n, f"{name} variant {variant}, many slabs")
 
 
 def test_table_interpreter_when_specialisation_is_off(monkeypatch):
