@@ -52,7 +52,8 @@ typedef enum {
     QSS_E_QSS_FANOUT = -3,   /* an enabled direction produces >= 2 QSS molecules                                  */
     QSS_E_NO_SINK = -4,      /* a QSS species cannot reach a transported species: closure structurally singular  */
     QSS_E_UNSUPPORTED = -5,  /* reaction type outside {0,1,2}, non-positive stoichiometric coefficient          */
-    QSS_E_CUDA = -6          /* a CUDA runtime call failed (message in qss_last_error)                         */
+    QSS_E_CUDA = -6,         /* a CUDA runtime call failed (message in qss_last_error)                         */
+    QSS_E_UNBALANCED = -7    /* strict_balance: a reaction does not conserve an element (needs comp)          */
 } qss_status;
 
 typedef struct qss_mech qss_mech_t;   /* opaque */
@@ -74,6 +75,9 @@ typedef struct {
     const double  *troe;                   /* [n_reac*4] alpha, T***, T*, T**, read for type 2 only           */
     const int32_t *eff_ptr, *eff_sp;       /* CSR non-unity third-body efficiencies, transported species only */
     const double  *eff_val;                /*   (third-body concentration M = sum_{k<N} alpha_k C_k, G7)      */
+    int32_t strict_balance;                /* != 0: qss_mech_create / _validate check sum_s nu_s comp[s][e] = 0 for every
+                                            * reaction and element and fail with QSS_E_UNBALANCED (comp must be given);
+                                            * the conservation pins of wdot and of the Jacobian's null space rest on it */
 } qss_mech_desc_t;
 
 typedef struct {

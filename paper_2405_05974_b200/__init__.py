@@ -19,7 +19,7 @@ __all__ = ["lib", "QssMech", "QssError", "EXPORTS", "STATUS"]
 EXPORTS = ["qss_mech_create", "qss_mech_validate", "qss_mech_specialise_check", "qss_mech_destroy", "qss_mech_info", "qss_mech_qss_order", "qss_eval_wdot",
            "qss_eval_jac", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
 STATUS = {0: "QSS_OK", -1: "QSS_E_INVALID", -2: "QSS_E_QUADRATIC", -3: "QSS_E_QSS_FANOUT", -4: "QSS_E_NO_SINK",
-          -5: "QSS_E_UNSUPPORTED", -6: "QSS_E_CUDA"}
+          -5: "QSS_E_UNSUPPORTED", -6: "QSS_E_CUDA", -7: "QSS_E_UNBALANCED"}
 
 
 class QssError(RuntimeError):
@@ -36,7 +36,8 @@ class _Desc(ct.Structure):
                 ("reac_ptr", ct.c_void_p), ("reac_sp", ct.c_void_p), ("reac_nu", ct.c_void_p),
                 ("prod_ptr", ct.c_void_p), ("prod_sp", ct.c_void_p), ("prod_nu", ct.c_void_p),
                 ("arr", ct.c_void_p), ("arr_low", ct.c_void_p), ("troe", ct.c_void_p),
-                ("eff_ptr", ct.c_void_p), ("eff_sp", ct.c_void_p), ("eff_val", ct.c_void_p)]
+                ("eff_ptr", ct.c_void_p), ("eff_sp", ct.c_void_p), ("eff_val", ct.c_void_p),
+                ("strict_balance", ct.c_int32)]
 
 
 class _Info(ct.Structure):
@@ -86,9 +87,10 @@ _DESC_SPEC = dict(elem_weight=np.float64, comp=np.int32, nasa_T=np.float64, nasa
                   troe=np.float64, eff_ptr=np.int32, eff_sp=np.int32, eff_val=np.float64)
 
 
-def make_desc(mech):
+def make_desc(mech, strict_balance=False):
     """qss_mech_desc_t from any object with the fields of qss_synth.Mechanism. Returns (desc, keepalive)."""
     d = _Desc()
+    d.strict_balance = 1 if strict_balance else 0
     d.n_elem, d.n_nqss, d.n_qss, d.n_reac = int(mech.n_elem), int(mech.n_nqss), int(mech.n_qss), int(mech.n_reac)
     keep = {}
     for name, dt in _DESC_SPEC.items():
@@ -101,9 +103,9 @@ def make_desc(mech):
     return d, keep
 
 
-def validate(mech):
+def validate(mech, strict_balance=False):
     """Host-only validation + QSS solve order (no CUDA). Returns (n_groups, order, group_of)."""
-    d, keep = make_desc(mech)
+    d, keep = make_desc(mech, strict_balance)
     ng = ct.c_int32()
     nq = max(int(mech.n_qss), 1)
     order = np.zeros(nq, dtype=np.int32); grp = np.zeros(nq, dtype=np.int32)
@@ -129,9 +131,9 @@ def _ptr(t):
 class QssMech:
     """A compiled mechanism on one CUDA device (qss_mech_create / qss_mech_destroy)."""
 
-    def __init__(self, mech, device: int = 0):
+    def __init__(self, mech, device: int = 0, strict_balance: bool = False):
         self._h = ct.c_void_p()
-        d, keep = make_desc(mech)
+        d, keep = make_desc(mech, strict_balance)
         _check(lib().qss_mech_create(ct.addressof(d), int(device), ct.byref(self._h)))
         del keep
         self.device = int(device)
@@ -161,8 +163,9 @@ class QssMech:
         return [int(self.info.group_size[g]) for g in range(min(self.info.n_groups, 64))]
 
     def workspace(self, jac: bool):
+        """Scratch slab of the kernels, one per (call kind, CUDA stream): evaluations enqueued on two streams must not share it."""
         import torch
-        key = bool(jac)
+        key = (bool(jac), torch.cuda.current_stream().cuda_stream)
         if key not in self._ws:
             nbytes = self.info.workspace_bytes_jac if jac else self.info.workspace_bytes_wdot
             self._ws[key] = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=f"cuda:{self.device}")

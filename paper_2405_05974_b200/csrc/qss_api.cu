@@ -5,12 +5,14 @@
 #include <algorithm>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 
 #include "../../include/qss.h"
 #include "qss_compile.h"
 #include "qss_jit.h"
+#include "qss_devtools.h"
 
 size_t qss_slab_ws_doubles(const QssTab &t, bool jac, int nwarp);
 cudaError_t qss_launch_slab(const QssTab &t, bool jac, int64_t ncells, int64_t ld, const double *C, const double *T,
@@ -30,7 +32,8 @@ struct qss_mech {
     int nwarp = 8;            // warps per block of the slab kernel
     int blocks_per_sm = 4;    // general kernel: 4 x 8 warps per SM (64 registers); measured 193 -> 123 ms on cfg3 vs 2 blocks
     int nblocks = 0;
-    cudaStream_t copy_stream = nullptr;   // qss_eval_jac_host: device-to-host copies overlap the next chunk's kernel
+    cudaStream_t copy_stream = nullptr;   // qss_eval_jac_host: device-to-host copies overlap the next chunk's kernel (created with the handle)
+    mutable std::mutex host_mu;           // qss_eval_jac_host calls on one handle are serialised (they share copy_stream and the event)
     cudaEvent_t ev[2] = {nullptr, nullptr};
     long long *timing = nullptr;   // device counters when QSS_TIMING=1 (variant 1 only)
     int variant = 0;          // 0: general slab kernel (workspace in global memory); 1: slab-smem kernel (qss_kernel_v1.cu)
@@ -95,7 +98,7 @@ extern "C" int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech
     cudaDeviceProp prop;
     if ((e = cudaGetDeviceProperties(&prop, device)) != cudaSuccess) { delete m; return cuda_fail(e, "cudaGetDeviceProperties"); }
     m->n_sm = prop.multiProcessorCount;
-    if (const char *bps = std::getenv("QSS_V0_BLOCKS_PER_SM")) m->blocks_per_sm = std::max(1, std::atoi(bps));   // tuning aid for the general kernel
+    if (const char *bps = qss_devenv("QSS_V0_BLOCKS_PER_SM")) m->blocks_per_sm = std::max(1, std::atoi(bps));   // tuning aid for the general kernel
     m->nblocks = m->n_sm * m->blocks_per_sm;
     const size_t nI = m->c.I.size() ? m->c.I.size() : 1, nD = m->c.D.size() ? m->c.D.size() : 1;
     if ((e = cudaMalloc(&m->dI, nI * sizeof(int32_t))) != cudaSuccess) { delete m; return cuda_fail(e, "cudaMalloc(tables)"); }
@@ -104,6 +107,8 @@ extern "C" int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech
     if (e == cudaSuccess && m->c.D.size()) e = cudaMemcpy(m->dD, m->c.D.data(), m->c.D.size() * sizeof(double), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(m->dI); cudaFree(m->dD); delete m; return cuda_fail(e, "cudaMemcpy(tables)"); }
     m->c.tab.I = m->dI; m->c.tab.D = m->dD;
+    if ((e = cudaStreamCreateWithFlags(&m->copy_stream, cudaStreamNonBlocking)) == cudaSuccess) e = cudaEventCreateWithFlags(&m->ev[0], cudaEventDisableTiming);
+    if (e != cudaSuccess) { qss_mech_destroy(m); return cuda_fail(e, "cudaStreamCreate / cudaEventCreate"); }
     const char *force = std::getenv("QSS_VARIANT");
     // kernel variant 3 (reaction-per-lane rate phases, everything generated per mechanism, NVRTC): the Jacobian kernel of
     // choice when the mechanism fits it.  QSS_VARIANT=3 makes its absence an error; QSS_VARIANT=0/1/2 keep the older kernels.
@@ -118,7 +123,7 @@ extern "C" int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech
             if (e == cudaSuccess) e = cudaMemcpy(m->dP3, h.dP.data(), h.dP.size() * sizeof(double), cudaMemcpyHostToDevice);
             if (e == cudaSuccess) e = cudaMemcpy(m->iP3, h.iP.data(), h.iP.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
             if (e != cudaSuccess) { qss_mech_destroy(m); return cuda_fail(e, "cudaMalloc/cudaMemcpy(variant 3 parameters)"); }
-        } else if (std::getenv("QSS_DEBUG") || (force && force[0] == '3')) {
+        } else if (qss_devenv("QSS_DEBUG") || (force && force[0] == '3')) {
             std::fprintf(stderr, "[qss] kernel variant 3 unavailable: %s\n", jerr.c_str());
         }
         if (!m->jit3 && force && force[0] == '3') { qss_mech_destroy(m); return fail(QSS_E_CUDA, "QSS_VARIANT=3: " + jerr); }
@@ -127,20 +132,20 @@ extern "C" int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech
         qss_mech_destroy(m);
         return fail(QSS_E_UNSUPPORTED, "QSS_VARIANT=3: kernel variant 3 does not apply: " + w);
     }
-    if (m->jit3 && std::getenv("QSS_TIMING") && cudaMalloc(&m->timing, 32 * sizeof(long long)) == cudaSuccess) cudaMemset(m->timing, 0, 32 * sizeof(long long));
+    if (m->jit3 && qss_devenv("QSS_TIMING") && cudaMalloc(&m->timing, 32 * sizeof(long long)) == cudaSuccess) cudaMemset(m->timing, 0, 32 * sizeof(long long));
     // kernel selection: variant 1 when the mechanism fits it (QSS_VARIANT=0 in the environment forces the general kernel)
     if (m->c.v1_ok && !(force && force[0] == '0')) {   // (also the wdot-only kernel next to variant 3)
         if ((e = qss_v1_prepare()) != cudaSuccess) { cudaFree(m->dI); cudaFree(m->dD); delete m; return cuda_fail(e, "cudaFuncSetAttribute(variant 1)"); }
         m->variant = 1;
         m->nblocks = m->n_sm;
         m->c.v1.gI = m->dI; m->c.v1.gD = m->dD;
-        if (!m->timing && std::getenv("QSS_TIMING") && cudaMalloc(&m->timing, 16 * sizeof(long long)) == cudaSuccess) cudaMemset(m->timing, 0, 16 * sizeof(long long));
+        if (!m->timing && qss_devenv("QSS_TIMING") && cudaMalloc(&m->timing, 16 * sizeof(long long)) == cudaSuccess) cudaMemset(m->timing, 0, 16 * sizeof(long long));
         // Jacobian kernel specialised for this mechanism (NVRTC); QSS_JIT=0 keeps the table interpreter, which is also what
         // runs when NVRTC is missing or the compilation fails (qss_mech_info.kernel_variant_jac tells which: 2 = specialised)
         if (!m->jit3 && !(jit_env && jit_env[0] == '0') && !m->c.v1_gen.empty()) {
             std::string jerr;
             m->jit = qss_jit_create(m->c.v1_gen, prop.major, prop.minor, jerr);
-            if (!m->jit && (std::getenv("QSS_DEBUG") || (jit_env && jit_env[0] == '2'))) std::fprintf(stderr, "[qss] run-time specialisation unavailable: %s\n", jerr.c_str());
+            if (!m->jit && (qss_devenv("QSS_DEBUG") || (jit_env && jit_env[0] == '2'))) std::fprintf(stderr, "[qss] run-time specialisation unavailable: %s\n", jerr.c_str());
             if (!m->jit && jit_env && jit_env[0] == '2') { cudaFree(m->dI); cudaFree(m->dD); cudaFree(m->timing); delete m; return fail(QSS_E_CUDA, "QSS_JIT=2: " + jerr); }
         }
     }
@@ -204,7 +209,8 @@ extern "C" int qss_mech_destroy(qss_mech_t *m) {
     qss_jit_destroy(m->jit);
     qss_jit_destroy(m->jit3);
     cudaFree(m->dP3); cudaFree(m->iP3);
-    if (m->copy_stream) { cudaStreamDestroy(m->copy_stream); cudaEventDestroy(m->ev[0]); cudaEventDestroy(m->ev[1]); }
+    if (m->copy_stream) cudaStreamDestroy(m->copy_stream);
+    if (m->ev[0]) cudaEventDestroy(m->ev[0]);
     cudaFree(m->dI); cudaFree(m->dD);
     delete m;
     return QSS_OK;
@@ -241,6 +247,7 @@ extern "C" int qss_eval_wdot(const qss_mech_t *m, int64_t ncells, int64_t ld, co
                              double *wdot, double *cqss, void *workspace, size_t workspace_bytes, void *stream) {
     int rc = check_eval(m, ncells, ld, C, T, wdot, workspace, workspace_bytes, m ? ws_bytes(m, false) : 0);
     if (rc != QSS_OK || ncells == 0) return rc;
+    DeviceGuard guard(m->device);          // the handle's tables and kernels live on its device; `stream` must belong to it
     cudaError_t e;
     if (m->variant == 1) {
         QssV1 v = m->c.v1;
@@ -258,6 +265,7 @@ extern "C" int qss_eval_jac(const qss_mech_t *m, int64_t ncells, int64_t ld, con
                             double *jac, double *wdot, void *workspace, size_t workspace_bytes, void *stream) {
     int rc = check_eval(m, ncells, ld, C, T, jac, workspace, workspace_bytes, m ? ws_bytes(m, true) : 0);
     if (rc != QSS_OK || ncells == 0) return rc;
+    DeviceGuard guard(m->device);
     cudaError_t e;
     if (m->jit3) {
         QssV3 v;
@@ -304,28 +312,25 @@ extern "C" int qss_eval_jac_host(const qss_mech_t *m, int64_t ncells, int64_t ld
     // Pipelined over chunks of cells: the kernel of chunk c runs on `stream` while the Jacobian of chunk c-1 streams back
     // to the host on an internal copy stream (the device-to-host copy of N(N+1) doubles per cell dominates the call).
     // The SoA arrays are copied as 2D blocks: `rows` rows of `chunk` cells with row pitch ld.
-    qss_mech *mm = const_cast<qss_mech *>(m);
+    std::lock_guard<std::mutex> lock(m->host_mu);
     DeviceGuard guard(m->device);
-    if (!mm->copy_stream) {
-        if ((e = cudaStreamCreateWithFlags(&mm->copy_stream, cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(e, "cudaStreamCreate");
-        for (int i = 0; i < 2; ++i)
-            if ((e = cudaEventCreateWithFlags(&mm->ev[i], cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e, "cudaEventCreate");
-    }
+    // on any failure: no copy into the caller's host buffers may still be pending when the call returns
+    auto bail = [&](int rc) { cudaStreamSynchronize(m->copy_stream); cudaStreamSynchronize(s); return rc; };
     const int64_t nchunk = ncells >= (1 << 16) ? 8 : 1;
     const int64_t chunk = ((ncells + nchunk - 1) / nchunk + 31) / 32 * 32;
-    if ((e = cudaMemcpyAsync(dT, Th, L, cudaMemcpyHostToDevice, s)) != cudaSuccess) return cuda_fail(e, "H2D T");
+    if ((e = cudaMemcpyAsync(dT, Th, L, cudaMemcpyHostToDevice, s)) != cudaSuccess) return bail(cuda_fail(e, "H2D T"));
     for (int64_t c0 = 0; c0 < ncells; c0 += chunk) {
         const int64_t nc = std::min(chunk, ncells - c0);
         const size_t wbytes = (size_t)nc * sizeof(double);
-        if ((e = cudaMemcpy2DAsync(dC + c0, L, Ch + c0, L, wbytes, N, cudaMemcpyHostToDevice, s)) != cudaSuccess) return cuda_fail(e, "H2D C");
+        if ((e = cudaMemcpy2DAsync(dC + c0, L, Ch + c0, L, wbytes, N, cudaMemcpyHostToDevice, s)) != cudaSuccess) return bail(cuda_fail(e, "H2D C"));
         int rc = qss_eval_jac(m, nc, ld, dC + c0, dT + c0, dJ + c0, wdoth ? dW + c0 : nullptr, ws, ws_bytes(m, true), stream);
-        if (rc != QSS_OK) return rc;
-        if ((e = cudaEventRecord(mm->ev[0], s)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
-        if ((e = cudaStreamWaitEvent(mm->copy_stream, mm->ev[0], 0)) != cudaSuccess) return cuda_fail(e, "cudaStreamWaitEvent");
-        if ((e = cudaMemcpy2DAsync(jach + c0, L, dJ + c0, L, wbytes, N * (N + 1), cudaMemcpyDeviceToHost, mm->copy_stream)) != cudaSuccess) return cuda_fail(e, "D2H jac");
-        if (wdoth && (e = cudaMemcpy2DAsync(wdoth + c0, L, dW + c0, L, wbytes, N, cudaMemcpyDeviceToHost, mm->copy_stream)) != cudaSuccess) return cuda_fail(e, "D2H wdot");
+        if (rc != QSS_OK) return bail(rc);
+        if ((e = cudaEventRecord(m->ev[0], s)) != cudaSuccess) return bail(cuda_fail(e, "cudaEventRecord"));
+        if ((e = cudaStreamWaitEvent(m->copy_stream, m->ev[0], 0)) != cudaSuccess) return bail(cuda_fail(e, "cudaStreamWaitEvent"));
+        if ((e = cudaMemcpy2DAsync(jach + c0, L, dJ + c0, L, wbytes, N * (N + 1), cudaMemcpyDeviceToHost, m->copy_stream)) != cudaSuccess) return bail(cuda_fail(e, "D2H jac"));
+        if (wdoth && (e = cudaMemcpy2DAsync(wdoth + c0, L, dW + c0, L, wbytes, N, cudaMemcpyDeviceToHost, m->copy_stream)) != cudaSuccess) return bail(cuda_fail(e, "D2H wdot"));
     }
-    if ((e = cudaStreamSynchronize(mm->copy_stream)) != cudaSuccess) return cuda_fail(e, "cudaStreamSynchronize(copy)");
+    if ((e = cudaStreamSynchronize(m->copy_stream)) != cudaSuccess) return bail(cuda_fail(e, "cudaStreamSynchronize(copy)"));
     if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return cuda_fail(e, "cudaStreamSynchronize");
     return QSS_OK;
 }

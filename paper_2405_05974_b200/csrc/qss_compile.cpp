@@ -7,6 +7,7 @@
 // L262-276, is prior art here): the kernels interpret these tables.
 #include "qss_compile.h"
 #include "qss_ctx.h"
+#include "qss_devtools.h"
 
 #include <algorithm>
 #include <cmath>
@@ -15,6 +16,7 @@
 #include <functional>
 #include <cstring>
 #include <map>
+#include <stdexcept>
 
 using namespace qssc;
 
@@ -487,7 +489,11 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
     if (v.n_wy + N + nw <= region) {                         // (W_y and the staged inputs of the next slab must fit the time-shared region)
         std::string &g = out.v1_gen;
         char b[256];
-        auto P = [&](const char *f, auto... a) { std::snprintf(b, sizeof b, f, a...); g += b; };
+        auto P = [&](const char *f, auto... a) {
+            const int n_ = std::snprintf(b, sizeof b, f, a...);
+            if (n_ < 0 || n_ >= (int)sizeof b) throw std::runtime_error("generated line exceeds the line buffer");
+            g += b;
+        };
         const int one = voff(N), dist = 12;
         g += "// generated by qss_compile.cpp for one mechanism: pass A of the Jacobian sweep (see qss_kernel_v1.cu)\n";
         g += "__device__ __forceinline__ void qss_gen_column(const int k, const unsigned sml, const double *sc, double *jc, const long long rs, const bool active) {\n";
@@ -554,7 +560,7 @@ bool build_v1(const V1Ctx &c, QssCompiled &out, std::string &why) {
         // J[:, k] = W_x[:, k] + W_y dy/dx_k (Eq. 7) in place on the registers of the column: W_y (per cell, n_wy rows,
         // row-major, ascending q within a row) was copied to shared memory behind the fixed state; then 35 coalesced stores
         //   (by direction when that needs fewer rows than W_y has entries: kappa_d of the QSS-consuming directions was copied instead)
-        const bool by_dir = (int)gdir.size() <= v.n_wy && !std::getenv("QSS_GEN_WY");
+        const bool by_dir = (int)gdir.size() <= v.n_wy && !qss_devenv("QSS_GEN_WY");
         if (by_dir) {
             for (size_t r = 0; r < gdir.size(); ++r) {
                 P("    {   const double kd = lS<%d>(sml);\n", (v.s_KAP + (int)r) * 256);
@@ -744,9 +750,31 @@ int qss_compile(const qss_mech_desc_t *d, QssCompiled &out, std::string &err) {
             }
         }
         for (auto &kv : net) if (kv.second != 0) r.net.push_back({kv.first, kv.second});
+        if (d->eff_ptr && (d->eff_ptr[j + 1] < d->eff_ptr[j] || d->eff_ptr[j] < 0)) { err = fmt("reaction %d: efficiency CSR pointers decrease", j); return QSS_E_INVALID; }
         if (r.type >= 1 && d->eff_ptr) {
-            for (int p = d->eff_ptr[j]; p < d->eff_ptr[j + 1]; ++p)
+            if (d->eff_ptr[j + 1] > d->eff_ptr[j] && (!d->eff_sp || !d->eff_val)) { err = "efficiency arrays are NULL"; return QSS_E_INVALID; }
+            for (int p = d->eff_ptr[j]; p < d->eff_ptr[j + 1]; ++p) {
                 if (d->eff_sp[p] < 0 || d->eff_sp[p] >= N) { err = fmt("reaction %d: third-body efficiency on species %d (must be transported)", j, d->eff_sp[p]); return QSS_E_INVALID; }
+                if (!std::isfinite(d->eff_val[p])) { err = fmt("reaction %d: non-finite third-body efficiency", j); return QSS_E_INVALID; }
+                for (int q = d->eff_ptr[j]; q < p; ++q)
+                    if (d->eff_sp[q] == d->eff_sp[p]) { err = fmt("reaction %d: third-body efficiency of species %d given twice", j, d->eff_sp[p]); return QSS_E_INVALID; }
+            }
+        }
+        if (r.type == 2) {
+            // fall-off parameters: alpha finite, T*** and T* positive (CHEMKIN placeholders such as 1e-30 / 1e30 are fine: the
+            // kernels saturate the exponentials), T** finite
+            const double *tp = d->troe + 4 * j;
+            if (!std::isfinite(tp[0]) || !(tp[1] > 0.0) || !(tp[2] > 0.0) || !std::isfinite(tp[1]) || !std::isfinite(tp[2]) || !std::isfinite(tp[3])) {
+                err = fmt("reaction %d: Troe parameters need finite alpha and T**, and finite positive T***, T*", j); return QSS_E_INVALID;
+            }
+        }
+    }
+    if (d->strict_balance) {                 // optional strict mode (SURVEY.md 8(b) "Errors"): every reaction conserves every element
+        if (!d->comp || d->n_elem < 1) { err = "strict_balance needs the element compositions (comp, n_elem)"; return QSS_E_INVALID; }
+        for (int j = 0; j < M; ++j) for (int e = 0; e < d->n_elem; ++e) {
+            long bal = 0;
+            for (const Term &x : R[j].net) bal += (long)x.nu * d->comp[(size_t)x.sp * d->n_elem + e];
+            if (bal != 0) { err = fmt("reaction %d does not conserve element %d (imbalance %d)", j, e, (int)bal); return QSS_E_UNBALANCED; }
         }
     }
     auto enabled = [&](int j, int dir) { return (R[j].mask >> dir) & 1; };
@@ -1076,12 +1104,12 @@ int qss_compile(const qss_mech_desc_t *d, QssCompiled &out, std::string &err) {
                  &pos_in_grp, &rorder, &ce, &xpl, &effc, d};
         out.v1_ok = build_v1(vc, out, out.v1_why);
         out.v3_ok = build_v3(vc, out, out.v3_why);
-        if (const char *dump = std::getenv("QSS_GEN_DUMP")) {            // debugging aid: the generated source (variant 3, else variant 2)
+        if (const char *dump = qss_devenv("QSS_GEN_DUMP")) {            // debugging aid: the generated source (variant 3, else variant 2)
             const std::string &g = out.v3_ok ? out.v3.gen : out.v1_gen;
             if (FILE *f = std::fopen(dump, "w")) { std::fwrite(g.data(), 1, g.size(), f); std::fclose(f); }
         }
-        if (std::getenv("QSS_DEBUG")) std::fprintf(stderr, "[qss] variant 3: %s%s\n", out.v3_ok ? "ok" : "not applicable: ", out.v3_ok ? "" : out.v3_why.c_str());
-        if (std::getenv("QSS_DEBUG"))
+        if (qss_devenv("QSS_DEBUG")) std::fprintf(stderr, "[qss] variant 3: %s%s\n", out.v3_ok ? "ok" : "not applicable: ", out.v3_ok ? "" : out.v3_why.c_str());
+        if (qss_devenv("QSS_DEBUG"))
             std::fprintf(stderr, "[qss] variant 1: %s%s (hot table %d/%d words, smem rows %d, scratch rows %d, rounds %d, solve ops %d)\n",
                          out.v1_ok ? "ok" : "not applicable: ", out.v1_ok ? "" : out.v1_why.c_str(), out.v1.h_used, QSS_V1_HMAX,
                          out.v1.smem_rows, out.v1.scratch_rows, out.v1.n_rounds, out.v1.n_sp_ops);

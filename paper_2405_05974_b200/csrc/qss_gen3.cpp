@@ -15,6 +15,7 @@
 //     (as in variant 2), the column of [W_x; G_x] in registers.
 #include "qss_compile.h"
 #include "qss_ctx.h"
+#include "qss_devtools.h"
 
 #include <algorithm>
 #include <cmath>
@@ -411,7 +412,7 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
     // ---- P8: one Jacobian column in registers: init, records, dy/dx solve, W_y dy/dx, stores --------------------------
     {
         int dist = 12, fdist = 4, sdist = 3, pdist = 8;      // loads run this many items ahead of their use
-        if (const char *e = std::getenv("QSS3_DIST")) std::sscanf(e, "%d,%d,%d,%d", &dist, &fdist, &sdist, &pdist);      // (experiments)
+        if (const char *e = qss_devenv("QSS3_DIST")) std::sscanf(e, "%d,%d,%d,%d", &dist, &fdist, &sdist, &pdist);
         G("__device__ __forceinline__ void qss_gen_column(const int k, const unsigned sml, const unsigned sml2, const double *sc, double *jc, const long long rs, const bool active) {\n    double ");
         for (int s = 0; s < nsp; ++s) G("c%d%s", s, s + 1 < nsp ? ", " : ";\n");
         G("    if (k < %d) {\n", N);

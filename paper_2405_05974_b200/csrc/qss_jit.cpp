@@ -1,6 +1,7 @@
 // Run-time specialisation of kernel variant 1: NVRTC compile of qss_kernel_v1.cu + the generated pass A, load, launch.
 // NVRTC is opened with dlopen so that libqss.so loads (and the interpreter kernels work) on a box without it.
 #include "qss_jit.h"
+#include "qss_devtools.h"
 
 #include <dlfcn.h>
 #include <nvrtc.h>
@@ -158,7 +159,7 @@ std::shared_ptr<std::vector<char>> compile(const std::string &main_name, const s
     if (r == NVRTC_SUCCESS && sz) r = n.getCUBIN(prog, bin->data());
     n.destroyProgram(&prog);
     if (r != NVRTC_SUCCESS || !sz) { err = std::string("nvrtcGetCUBIN: ") + n.getErrorString(r); return nullptr; }
-    if (const char *dump = std::getenv("QSS_JIT_DUMP")) {       // debugging aid: the device image, for cuobjdump -sass
+    if (const char *dump = qss_devenv("QSS_JIT_DUMP")) {       // debugging aid: the device image, for cuobjdump -sass
         if (FILE *f = std::fopen(dump, "wb")) { std::fwrite(bin->data(), 1, bin->size(), f); std::fclose(f); }
     }
     cache_store(cpath, *bin);
@@ -191,21 +192,26 @@ QssJit *load_image(const std::vector<char> &bin, const char *kernel, std::string
 
 std::vector<std::string> defs3(bool jac);
 
+std::vector<std::string> defs1() {
+    std::vector<std::string> d = {"-DQSS_GEN"};
+    if (qss_devenv("QSS_TIMING")) d.push_back("-DQSS_DEVTOOLS");
+    return d;
+}
+
 bool qss_jit_compile_only(const std::string &gen_src, int cc_major, int cc_minor, size_t *image_bytes, std::string &err) {
-    std::shared_ptr<std::vector<char>> bin = compile("qss_kernel_v1.cu", "qss_gen.h", gen_src, {"-DQSS_GEN"}, arch_of(cc_major, cc_minor), err);
+    std::shared_ptr<std::vector<char>> bin = compile("qss_kernel_v1.cu", "qss_gen.h", gen_src, defs1(), arch_of(cc_major, cc_minor), err);
     if (bin && image_bytes) *image_bytes = bin->size();
     return (bool)bin;
 }
 
 QssJit *qss_jit_create(const std::string &gen_src, int cc_major, int cc_minor, std::string &err) {
-    std::shared_ptr<std::vector<char>> bin = compile("qss_kernel_v1.cu", "qss_gen.h", gen_src, {"-DQSS_GEN"}, arch_of(cc_major, cc_minor), err);
+    std::shared_ptr<std::vector<char>> bin = compile("qss_kernel_v1.cu", "qss_gen.h", gen_src, defs1(), arch_of(cc_major, cc_minor), err);
     return bin ? load_image(*bin, "qss_v1_jit", err) : nullptr;
 }
 
 std::vector<std::string> defs3(bool jac) {
     std::vector<std::string> d = {jac ? "-DQSS3_JAC=1" : "-DQSS3_JAC=0"};
-    if (std::getenv("QSS_TIMING")) d.push_back("-DQSS3_TIMING=1");
-    if (const char *x = std::getenv("QSS3_EXP")) d.push_back(std::string("-DQSS3_EXP=") + x);      // (experiments; removed before release)
+    if (qss_devenv("QSS_TIMING")) d.push_back("-DQSS3_TIMING=1");
     return d;
 }
 

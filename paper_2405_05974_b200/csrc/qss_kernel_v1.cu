@@ -85,7 +85,7 @@ __device__ __forceinline__ void qss_pressure_factor(const int type, const double
         const double dlnk0 = (t4 + t5 * invT) * invT;
         const double Pr = qss_exp(lnk0 - lnkinf) * Mc;
         const double al = t6, i3 = t7, i1 = t8, T2s = t9;
-        const double e3 = qss_exp(-T * i3), e1x = qss_exp(-T * i1), e2 = qss_exp(-T2s * invT);
+        const double e3 = qss_exp_sat(-T * i3), e1x = qss_exp_sat(-T * i1), e2 = qss_exp_sat(-T2s * invT);
         const double Fc = (1.0 - al) * e3 + al * e1x + e2;
         const double L = log(Pr) * kInvLn10, Lc = log(Fc) * kInvLn10;
         const double c = -0.4 - 0.67 * Lc, n = 0.75 - 1.27 * Lc;
@@ -126,7 +126,10 @@ template <int O> __device__ __forceinline__ double lG(const double *b) {
 #include "qss_gen.h"
 #endif
 
-// optional phase timing (QSS_TIMING=1): thread 0 of block 0 accumulates the cycles between block barriers
+// optional phase timing (development builds, QSS_TIMING=1): thread 0 of block 0 accumulates the cycles between block barriers
+#ifndef QSS_DEVTOOLS
+#define QSS_TICK(ph) do { } while (0)
+#else
 #define QSS_TICK(ph)                                                                   \
     do {                                                                               \
         if (p.timing && blockIdx.x == 0 && threadIdx.x == 0) {                         \
@@ -135,6 +138,7 @@ template <int O> __device__ __forceinline__ double lG(const double *b) {
             tick_ = t_;                                                                \
         }                                                                              \
     } while (0)
+#endif
 
 #ifdef QSS_GEN
 // run-time specialised build: one entry point, Jacobian on, column stream replaced by the generated pass A
@@ -159,7 +163,9 @@ __global__ void __launch_bounds__(QSS_V1_NW * 32, 1) qss_v1_kernel(const __grid_
     for (int i = threadIdx.x; i < p.n_tab_words; i += blockDim.x) reinterpret_cast<int *>(qss_smem + (size_t)p.s_TAB * 32)[i] = __ldg(gI + p.i_wya_ptr + i);
     __syncthreads();
 
+#ifdef QSS_DEVTOOLS
     long long tick_ = clock64();
+#endif
     for (int64_t slab = blockIdx.x; slab < nslab; slab += gridDim.x) {
         const int64_t cell = slab * 32 + lane;
         const bool active = cell < p.ncells;

@@ -105,10 +105,6 @@ __device__ __forceinline__ int4 tab_rows4(const unsigned sm0, const int x) {
     return make_int4((a & 0xffff) * G_PITCH, (int)((unsigned)a >> 16) * G_PITCH, (b & 0xffff) * G_PITCH, (int)((unsigned)b >> 16) * G_PITCH);
 }
 
-__device__ __forceinline__ double qss_exp_sat(double x) {       // exp for arguments that may be placeholders (-T/1e-30, ...)
-    return qss_exp(fmin(fmax(x, -746.0), 710.0));
-}
-
 // Per-lane parameters of one reaction (lane = reaction): what every reaction type needs.  Loaded with pinned read-only
 // loads so that the first task of a slab can be fetched before the input phase (the L2 latency hides behind it).
 struct RateCommon {

@@ -74,7 +74,7 @@ __device__ __forceinline__ void rates(const QssTab &t, const CellCtx &cx, int j)
             const double dlnk0 = (rd[4] + rd[5] * invT) * invT;
             const double Pr = qss_exp(lnk0 - lnkinf) * Mc;
             const double al = rd[6], i3 = rd[7], i1 = rd[8], T2s = rd[9];
-            const double e3 = qss_exp(-T * i3), e1x = qss_exp(-T * i1), e2 = qss_exp(-T2s * invT);
+            const double e3 = qss_exp_sat(-T * i3), e1x = qss_exp_sat(-T * i1), e2 = qss_exp_sat(-T2s * invT);
             const double Fc = (1.0 - al) * e3 + al * e1x + e2;
             const double dFc = -(1.0 - al) * i3 * e3 - al * i1 * e1x + T2s * invT * invT * e2;
             const double L = log(Pr) * kInvLn10, Lc = log(Fc) * kInvLn10;

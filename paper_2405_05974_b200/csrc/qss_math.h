@@ -4,9 +4,10 @@
 //   n = rint(x log2 e) by the 1.5*2^52 trick, r = x - n ln2 (Cody-Waite, two constants), exp(r) by a degree-13 Taylor
 //   polynomial in Horner form (|r| <= 0.3466, truncation 4e-18), scaling by 2^n as two exponent-field factors so that
 //   results down to the denormals and up to overflow round correctly.  Measured against float128 expq on 10^7 arguments
-//   in [-745, 709]: max error 1.0 ulp, 0.86 ulp outside the denormal range (tests/test_host_math.py compiles this
-//   header for the host and repeats the measurement).
-// Preconditions: |x| < 2^30 (NaN gives NaN; +-inf gives NaN, not inf / 0).
+//   in [-745, 709]: max error 1.0 ulp, 0.86 ulp outside the denormal range (tests/test_host_logic.py compiles this
+//   header for the host and repeats the measurement with a 1.5 ulp bound).
+// Preconditions: |x| < 2^30 (NaN gives NaN; +-inf gives NaN, not inf / 0); arguments that may be larger (fall-off
+// placeholders) go through qss_exp_sat below.
 #ifndef QSS_MATH_H
 #define QSS_MATH_H
 #include "qss_stdint.h"
@@ -65,6 +66,12 @@ QSS_HD double qss_exp(double x) {
     n = n < -2000 ? -2000 : (n > 2000 ? 2000 : n);             // keeps both exponent fields valid for any finite x
     const int n1 = n >> 1, n2 = n - n1;
     return q * qss_pow2_factor(n1) * qss_pow2_factor(n2);
+}
+
+// exp for arguments that may lie far outside [-745, 709] (CHEMKIN placeholder Troe temperatures: -T/1e-30, -1e30/T):
+// saturates to exp(-746) = 0 and exp(710) = inf like the library function (NaN stays NaN).
+QSS_HD double qss_exp_sat(double x) {
+    return qss_exp(x < -746.0 ? -746.0 : (x > 710.0 ? 710.0 : x));
 }
 
 // The same exponential with the polynomial in Estrin form: 13 FMA + 3 multiplications in a dependent chain of depth 4

@@ -193,6 +193,24 @@ def test_zero_concentrations_and_tmid_tie_break():
     print(g)
 
 
+@pytest.mark.parametrize("env", [{}, {"QSS_VARIANT": "2"}, {"QSS_JIT": "0"}, {"QSS_VARIANT": "0"}])
+def test_chemkin_placeholder_troe_parameters(env, monkeypatch):
+    """CHEMKIN files write T*** ~ 1e-30 and T*, T** ~ 1e30 for an absent Troe term: the exponentials must saturate to 0 / 1 / 0 in
+    every kernel variant (the branch-free exp is only valid for |x| < 2^30 and returned inf / NaN there)."""
+    import dataclasses
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    mech = qss_synth.config_mechanism(2)
+    troe = mech.troe.copy()
+    idx = np.flatnonzero(mech.rtype == 2)
+    troe[idx[0::3], 1:] = (1.0e-30, 1.0e30, 1.0e30)
+    troe[idx[1::3], 3] = 1.0e30
+    mech = dataclasses.replace(mech, troe=troe)
+    n = 96 + 5
+    C, T = qss_synth.config_states(2, n)
+    _check(mech, C, T, n, f"cfg2 placeholder Troe {env}")
+
+
 def test_paper_style_sampling():
     """States drawn the way the paper validates its Jacobian: C ~ U[1e-4, 1] mol/m^3 for every
     species, T ~ U[300, 1300] K (both NASA ranges, very small rate constants at the cold end)."""
@@ -279,7 +297,7 @@ def test_bad_arguments_are_rejected():
         qm.eval_wdot(C, T, 64)                            # ncells > ld
     assert e.value.code == -1
     small = torch.empty(256, dtype=torch.uint8, device="cuda")
-    qm._ws[True] = small
+    qm._ws[(True, torch.cuda.current_stream().cuda_stream)] = small
     with pytest.raises(qss.QssError) as e:
         qm.eval_jac(C, T, 32)                             # workspace too small
     assert e.value.code == -1

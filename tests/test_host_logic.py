@@ -107,6 +107,49 @@ def test_validation_errors():
     assert e.value.code == -1
 
 
+def test_strict_element_balance_and_parameter_validation():
+    """strict_balance (QSS_E_UNBALANCED): every reaction must conserve every element; duplicate third-body
+    efficiencies and unusable Troe temperatures are rejected; CHEMKIN placeholders are accepted."""
+    for make in (qss_synth.toy1, qss_synth.toy_dag, lambda: qss_synth.config_mechanism(1), lambda: qss_synth.config_mechanism(2)):
+        qss.validate(make(), strict_balance=True)
+    m = qss_synth.config_mechanism(1)
+    comp = m.comp.copy(); comp[int(m.reac_sp[0]), 0] += 1
+    bad = _with(m, comp=comp)
+    qss.validate(bad)                                      # not strict: the compositions are not looked at
+    with pytest.raises(qss.QssError) as e:
+        qss.validate(bad, strict_balance=True)
+    assert e.value.code == -7
+    m2 = qss_synth.config_mechanism(2)
+    j = int(np.flatnonzero(m2.rtype == 2)[0])
+    for k, val in ((1, 0.0), (2, -5.0), (0, float("nan")), (3, float("inf"))):
+        troe = m2.troe.copy(); troe[j, k] = val
+        with pytest.raises(qss.QssError) as e:
+            qss.validate(_with(m2, troe=troe))
+        assert e.value.code == -1
+    troe = m2.troe.copy(); troe[j] = (0.4, 1e-30, 1e30, 1e30)
+    qss.validate(_with(m2, troe=troe))
+    jt = int(np.flatnonzero(np.diff(m2.eff_ptr) >= 2)[0])
+    eff_sp = m2.eff_sp.copy(); eff_sp[m2.eff_ptr[jt] + 1] = eff_sp[m2.eff_ptr[jt]]
+    with pytest.raises(qss.QssError) as e:
+        qss.validate(_with(m2, eff_sp=eff_sp))
+    assert e.value.code == -1
+
+
+def test_compiled_images_are_cached_on_disk(tmp_path, monkeypatch):
+    """qss_jit.cpp: the run-time compiled image of a mechanism is written to $QSS_CACHE_DIR, keyed by a hash of every source;
+    a second process-independent compilation of the same mechanism finds it (checked through the file set, no GPU needed)."""
+    monkeypatch.setenv("QSS_CACHE_DIR", str(tmp_path / "cache"))
+    n1 = qss.specialise_check(qss_synth.toy2(), (10, 0))
+    files = sorted(os.listdir(tmp_path / "cache"))
+    assert len(files) == 1 and files[0].endswith(".cubin") and os.path.getsize(tmp_path / "cache" / files[0]) == n1
+    qss.specialise_check(qss_synth.toy3(), (10, 0))
+    assert len(os.listdir(tmp_path / "cache")) == 2
+    monkeypatch.setenv("QSS_CACHE", "0")
+    monkeypatch.setenv("QSS_CACHE_DIR", str(tmp_path / "off"))
+    qss.specialise_check(qss_synth.toy1(), (10, 0))
+    assert not os.path.exists(tmp_path / "off")
+
+
 def test_specialised_jacobian_kernel_compiles_without_a_gpu():
     """Run-time specialisation, host side: the generated source of a mechanism's Jacobian columns compiles with NVRTC for
     sm_100a (no device needed); a mechanism outside kernel variant 1 has nothing to specialise."""
@@ -126,21 +169,28 @@ def test_branch_free_exp_against_float128(tmp_path):
 #include <random>
 #include <quadmath.h>
 int main() {
-  std::mt19937_64 g(1); double worst = 0;
+  std::mt19937_64 g(1); double worst = 0, worst_e = 0;
   std::uniform_real_distribution<double> u(-745.0, 709.0), s(-1.0, 1.0);
   for (int i = 0; i < 2000000; ++i) {
-    double x = (i & 1) ? u(g) : s(g), a = qss_exp(x); __float128 r = expq((__float128)x); double rd = (double)r;
+    double x = (i & 1) ? u(g) : s(g), a = qss_exp(x), b = qss_exp_e(x); __float128 r = expq((__float128)x); double rd = (double)r;
     if (rd == 0 || std::isinf(rd)) continue;
     double ulp = std::fabs(std::nextafter(rd, INFINITY) - rd), e = (double)fabsq((__float128)a - r) / ulp;
     if (e > worst) worst = e;
+    e = (double)fabsq((__float128)b - r) / ulp;
+    if (e > worst_e) worst_e = e;
   }
-  printf("%.4f %d %d %d\n", worst, qss_exp(0.0) == 1.0, qss_exp(-1000.0) == 0.0, std::isinf(qss_exp(1000.0)));
+  // saturating form for placeholder arguments (fall-off temperatures 1e-30 / 1e30): 0, 1 and inf like the library function
+  const int sat = qss_exp_sat(-1.4e33) == 0.0 && qss_exp_sat(-1e27) == 0.0 && qss_exp_sat(-2e9) == 0.0 && qss_exp_sat(-1.4e-27) == 1.0 &&
+                  std::isinf(qss_exp_sat(1e12)) && qss_exp_sat(-INFINITY) == 0.0 && qss_exp_sat(0.5) == qss_exp(0.5);
+  printf("%.4f %d %d %d %.4f %d\n", worst, qss_exp(0.0) == 1.0, qss_exp(-1000.0) == 0.0, std::isinf(qss_exp(1000.0)), worst_e, sat);
 }''')
     exe = tmp_path / "t"
     subprocess.run(["g++", "-O2", "-ffp-contract=off", "-I", os.path.join(ROOT, "paper_2405_05974_b200", "csrc"), "-o", str(exe),
                     str(src), "-lquadmath"], check=True)
-    worst, one, zero, inf = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()
+    worst, one, zero, inf, worst_e, sat = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()
     assert float(worst) <= 1.5 and one == "1" and zero == "1" and inf == "1"
+    assert float(worst_e) <= 2.5, worst_e            # Estrin form of the polynomial (kernel variant 3)
+    assert sat == "1"
 
 
 def test_cell_ranges_tile_the_cells():
