@@ -11,7 +11,7 @@ import numpy as np
 
 from . import build as _build
 
-EXPLICIT_F64, EXPLICIT_F128, JAC_DUAL, JAC_CSTEP, JAC_CONST_QSS = 0, 1, 2, 3, 4
+EXPLICIT_F64, EXPLICIT_F128, JAC_DUAL, JAC_CSTEP, JAC_CONST_QSS, JAC_ZERO_QSS = 0, 1, 2, 3, 4, 5
 
 _lib = None
 
@@ -32,6 +32,8 @@ def lib():
         _lib = ct.CDLL(_build.build())
         _lib.oracle_eval.restype = ct.c_int
         _lib.oracle_eval.argtypes = [ct.c_void_p, ct.c_int64, ct.c_int64] + [ct.c_void_p] * 7 + [ct.c_int, ct.c_int]
+        _lib.oracle_eval_energy.restype = ct.c_int
+        _lib.oracle_eval_energy.argtypes = [ct.c_void_p, ct.c_int64, ct.c_int64] + [ct.c_void_p] * 5 + [ct.c_int, ct.c_int]
         _lib.oracle_rate_constants.restype = ct.c_int
         _lib.oracle_rate_constants.argtypes = [ct.c_void_p, ct.c_void_p, ct.c_double, ct.c_void_p, ct.c_void_p]
         _lib.oracle_closure_check.restype = ct.c_int
@@ -84,6 +86,18 @@ def evaluate(om: OracleMech, C: np.ndarray, T: np.ndarray, n_cells: int | None =
     if rc != 0:
         raise RuntimeError(f"oracle_eval failed rc={rc}")
     out["cqss"] = out["cqss"][:Nq]
+    return out
+
+
+def evaluate_energy(om: OracleMech, C: np.ndarray, T: np.ndarray, n_cells: int | None = None, *, mode=EXPLICIT_F64, nthreads=0):
+    """Temperature right-hand side and energy row (NEXT-1). Returns dict(tdot [ld], erow [N+1, ld], escale [N+1, ld])."""
+    assert C.dtype == np.float64 and T.dtype == np.float64 and C.flags.c_contiguous and T.flags.c_contiguous
+    ld = C.shape[1]
+    n_cells = ld if n_cells is None else n_cells
+    out = dict(tdot=np.zeros(ld), erow=np.zeros((om.N + 1, ld)), escale=np.zeros((om.N + 1, ld)))
+    rc = lib().oracle_eval_energy(om._ptr(), n_cells, ld, _p(C), _p(T), _p(out["tdot"]), _p(out["erow"]), _p(out["escale"]), mode, nthreads)
+    if rc != 0:
+        raise RuntimeError(f"oracle_eval_energy failed rc={rc}")
     return out
 
 

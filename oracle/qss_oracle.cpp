@@ -311,14 +311,14 @@ template <class S> struct JacWork {
 
 template <class S>
 int eval_jac(const oracle_mech_t *m, const S *C, const S &T, Rates<S> &rt, Closure<S> &cl, WdotOut<S> &wo,
-             JacWork<S> &w, S *J /* [N*(N+1)] row-major */, S *Jscale /* may be null */, bool drop_chain) {
+             JacWork<S> &w, S *J /* [N*(N+1)] row-major */, S *Jscale /* may be null */, bool drop_chain, bool zero_qss = false) {
     const int N = m->n_nqss, Nq = m->n_qss, M = m->n_reac, nsp = N + Nq, NC = N + 1;
     if (eval_wdot(m, C, T, rt, cl, wo) != 0) return -1;
     w.E.assign((size_t)nsp * NC, S(0.0)); w.Eabs.assign((size_t)nsp * NC, S(0.0));
     w.Wy.assign((size_t)N * Nq, S(0.0)); w.Wyabs.assign((size_t)N * Nq, S(0.0));
     w.c.resize(nsp);
     for (int s = 0; s < N; ++s) w.c[s] = C[s];
-    for (int q = 0; q < Nq; ++q) w.c[N + q] = cl.y[q];
+    for (int q = 0; q < Nq; ++q) w.c[N + q] = zero_qss ? S(0.0) : cl.y[q];      // zero-QSS AJ: C_QSS := 0 in the partials
     w.net.assign(nsp, 0);
     for (int j = 0; j < M; ++j) {
         const Side rs = reactants(m, j), ps = products(m, j);
@@ -403,7 +403,7 @@ template <class S> struct Work { Rates<S> rt; Closure<S> cl; WdotOut<S> wo; JacW
 
 template <class S>
 int run_explicit(const oracle_mech_t *m, int64_t c, int64_t ld, const double *C, const double *T, double *wdot,
-                 double *cqss, double *Sc, double *jac, double *jscale, bool drop_chain, Work<S> &w) {
+                 double *cqss, double *Sc, double *jac, double *jscale, bool drop_chain, Work<S> &w, bool zero_qss = false) {
     const int N = m->n_nqss, Nq = m->n_qss, NC = N + 1;
     w.C.resize(N);
     for (int k = 0; k < N; ++k) w.C[k] = S(C[(size_t)k * ld + c]);
@@ -411,7 +411,7 @@ int run_explicit(const oracle_mech_t *m, int64_t c, int64_t ld, const double *C,
     int rc;
     if (jac || jscale) {
         w.J.resize((size_t)N * NC); w.Js.resize((size_t)N * NC);
-        rc = eval_jac(m, w.C.data(), Tc, w.rt, w.cl, w.wo, w.jw, w.J.data(), jscale ? w.Js.data() : (S *)0, drop_chain);
+        rc = eval_jac(m, w.C.data(), Tc, w.rt, w.cl, w.wo, w.jw, w.J.data(), jscale ? w.Js.data() : (S *)0, drop_chain, zero_qss);
         if (rc) return rc;
         for (int e = 0; e < N * NC; ++e) {
             if (jac) jac[(size_t)e * ld + c] = s_re(w.J[e]);
@@ -429,7 +429,140 @@ int run_explicit(const oracle_mech_t *m, int64_t c, int64_t ld, const double *C,
     return 0;
 }
 
+// ------------------------------------------------------------------------------------------------
+// NEXT-1: temperature right-hand side and the energy row of the (N+1) x (N+1) Jacobian (Eq. 7: "the
+// contribution of the heat release rate can be simply obtained from the species production rates").
+// Reading G17: adiabatic CONSTANT-VOLUME reactor, thermodynamic sums over the transported
+// species only (the QSS species carry no inventory: dC_q/dt = 0, L69-73):
+//     sum_i C_i cv_i dT/dt = - sum_i u_i wdot_i,   u_i = h_i - R T,  cv_i = cp_i - R      (molar, NASA-7)
+//  => Tdot = - T E / Cv,   E = sum_i (h_i/RT - 1) wdot_i,   Cv = sum_i C_i (cp_i/R - 1).
+// ------------------------------------------------------------------------------------------------
+template <class S> struct Thermo1 { S hRT, cpR, dcpR_dT; };
+template <class S> Thermo1<S> nasa_species(const oracle_mech_t *m, int s, const S &T) {     // low set for T < Tmid, else high (G9)
+    const double *a = (s_re(T) < m->nasa_T[3 * s + 1]) ? m->nasa_lo + 7 * s : m->nasa_hi + 7 * s;
+    const S T2 = T * T, T3 = T2 * T, T4 = T3 * T;
+    Thermo1<S> t;
+    t.hRT = S(a[0]) + S(a[1] / 2.0) * T + S(a[2] / 3.0) * T2 + S(a[3] / 4.0) * T3 + S(a[4] / 5.0) * T4 + S(a[5]) / T;
+    t.cpR = S(a[0]) + S(a[1]) * T + S(a[2]) * T2 + S(a[3]) * T3 + S(a[4]) * T4;
+    t.dcpR_dT = S(a[1]) + S(2.0 * a[2]) * T + S(3.0 * a[3]) * T2 + S(4.0 * a[4]) * T3;
+    return t;
+}
+
+// the right-hand side itself, templated: its dual-number / complex-step instantiations differentiate it mechanically
+template <class S> int eval_tdot(const oracle_mech_t *m, const S *C, const S &T, Rates<S> &rt, Closure<S> &cl, WdotOut<S> &wo, S &Tdot) {
+    if (eval_wdot(m, C, T, rt, cl, wo) != 0) return -1;
+    S E = S(0.0), Cv = S(0.0);
+    for (int i = 0; i < m->n_nqss; ++i) {
+        const Thermo1<S> t = nasa_species(m, i, T);
+        E = E + (t.hRT - S(1.0)) * wo.wdot[i];
+        Cv = Cv + C[i] * (t.cpR - S(1.0));
+    }
+    Tdot = S(0.0) - T * E / Cv;
+    return 0;
+}
+
+// explicit energy row from the species block J [N x (N+1)] and wdot (the plain differentiation of Tdot = -T E / Cv):
+//   d Tdot / d C_k = -(T / Cv) sum_i u_i J_ik - Tdot (cp_k/R - 1) / Cv                                     u_i = h_i/RT - 1
+//   d Tdot / d T   = Tdot / T - (T / Cv) sum_i (u_i J_iT + wdot_i (cp_i/R - h_i/RT) / T) - Tdot sum_i C_i d(cp_i/R)/dT / Cv
+// `scale` (may be null): the same sums with every term replaced by its absolute value (running-error scale for the gates).
+template <class S>
+void energy_row(const oracle_mech_t *m, const S *C, const S &T, const S *wdot, const S *J, const S *Jscale, S &Tdot, S *row, S *scale) {
+    const int N = m->n_nqss, NC = N + 1;
+    std::vector<Thermo1<S>> th(N);
+    S E = S(0.0), Eabs = S(0.0), Cv = S(0.0), dCv = S(0.0), dCvabs = S(0.0);
+    for (int i = 0; i < N; ++i) {
+        th[i] = nasa_species(m, i, T);
+        E = E + (th[i].hRT - S(1.0)) * wdot[i];
+        Eabs = Eabs + s_abs((th[i].hRT - S(1.0)) * wdot[i]);
+        Cv = Cv + C[i] * (th[i].cpR - S(1.0));
+        dCv = dCv + C[i] * th[i].dcpR_dT;
+        dCvabs = dCvabs + s_abs(C[i] * th[i].dcpR_dT);
+    }
+    Tdot = S(0.0) - T * E / Cv;
+    const S g = T / Cv;
+    for (int k = 0; k < NC; ++k) {
+        S e = S(0.0), ea = S(0.0);
+        for (int i = 0; i < N; ++i) {
+            e = e + (th[i].hRT - S(1.0)) * J[(size_t)i * NC + k];
+            if (scale) ea = ea + s_abs(th[i].hRT - S(1.0)) * Jscale[(size_t)i * NC + k];
+            if (k == N) {
+                const S dh = (th[i].cpR - th[i].hRT) / T * wdot[i];
+                e = e + dh; ea = ea + s_abs(dh);
+            }
+        }
+        if (k < N) {
+            row[k] = S(0.0) - g * e - Tdot * (th[k].cpR - S(1.0)) / Cv;
+            if (scale) scale[k] = s_abs(g) * ea + s_abs(g * Eabs / Cv * (th[k].cpR - S(1.0)));
+        } else {
+            row[k] = Tdot / T - g * e - Tdot * dCv / Cv;
+            if (scale) scale[k] = s_abs(Eabs / Cv) + s_abs(g) * ea + s_abs(g * Eabs / Cv) * dCvabs / s_abs(Cv);
+        }
+    }
+}
+
+template <class S>
+int run_energy(const oracle_mech_t *m, int64_t c, int64_t ld, const double *C, const double *T, double *tdot, double *erow, double *escale, Work<S> &w) {
+    const int N = m->n_nqss, NC = N + 1;
+    w.C.resize(N);
+    for (int k = 0; k < N; ++k) w.C[k] = S(C[(size_t)k * ld + c]);
+    const S Tc = S(T[c]);
+    w.J.resize((size_t)N * NC); w.Js.resize((size_t)N * NC);
+    if (eval_jac(m, w.C.data(), Tc, w.rt, w.cl, w.wo, w.jw, w.J.data(), w.Js.data(), false)) return -1;
+    std::vector<S> row(NC), sc(NC);
+    S Td;
+    energy_row(m, w.C.data(), Tc, w.wo.wdot.data(), w.J.data(), w.Js.data(), Td, row.data(), sc.data());
+    if (tdot) tdot[c] = s_re(Td);
+    for (int k = 0; k < NC; ++k) { if (erow) erow[(size_t)k * ld + c] = s_re(row[k]); if (escale) escale[(size_t)k * ld + c] = s_re(sc[k]); }
+    return 0;
+}
+
 }  // namespace
+
+// Temperature right-hand side tdot[c] and energy row erow[k*ld + c] (k < N: d Tdot/d C_k, k = N: d Tdot/d T); escale: the
+// running-error scale of the row.  mode: ORACLE_EXPLICIT_F64 / _F128 (explicit formulas), ORACLE_JAC_DUAL / _CSTEP (the row by
+// differentiating the right-hand side mechanically; tdot from the plain double routine, escale not written).
+extern "C" int oracle_eval_energy(const oracle_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T,
+                                  double *tdot, double *erow, double *escale, int mode, int nthreads) {
+    if (!m || !C || !T || ncells < 0 || ld < ncells || mode < 0 || mode > 3) return -1;
+    const int N = m->n_nqss, NC = N + 1;
+    if (nthreads <= 0) nthreads = oracle_max_threads();
+    int err = 0;
+#pragma omp parallel num_threads(nthreads)
+    {
+        Work<double> wd; Work<Quad> wq; Work<Dual> wdu; Work<Cplx> wc;
+#pragma omp for schedule(dynamic, 8)
+        for (int64_t c = 0; c < ncells; ++c) {
+            int rc = 0;
+            if (mode == ORACLE_EXPLICIT_F64) rc = run_energy<double>(m, c, ld, C, T, tdot, erow, escale, wd);
+            else if (mode == ORACLE_EXPLICIT_F128) rc = run_energy<Quad>(m, c, ld, C, T, tdot, erow, escale, wq);
+            else {
+                rc = run_energy<double>(m, c, ld, C, T, tdot, (double *)0, (double *)0, wd);
+                if (!rc && erow && mode == ORACLE_JAC_DUAL) {
+                    wdu.C.resize(N);
+                    for (int k = 0; k < N; ++k) { wdu.C[k] = Dual(C[(size_t)k * ld + c]); wdu.C[k].d.assign(NC, 0.0); wdu.C[k].d[k] = 1.0; }
+                    Dual Td(T[c]); Td.d.assign(NC, 0.0); Td.d[N] = 1.0;
+                    Dual out;
+                    rc = eval_tdot(m, wdu.C.data(), Td, wdu.rt, wdu.cl, wdu.wo, out);
+                    if (!rc) for (int k = 0; k < NC; ++k) erow[(size_t)k * ld + c] = dg(out, k);
+                } else if (!rc && erow) {
+                    const double h = 1e-30;
+                    wc.C.resize(N);
+                    for (int k = 0; k < NC && !rc; ++k) {
+                        for (int s = 0; s < N; ++s) wc.C[s] = Cplx(C[(size_t)s * ld + c], s == k ? h : 0.0);
+                        Cplx Tc(T[c], k == N ? h : 0.0), out;
+                        rc = eval_tdot(m, wc.C.data(), Tc, wc.rt, wc.cl, wc.wo, out);
+                        if (!rc) erow[(size_t)k * ld + c] = out.imag() / h;
+                    }
+                }
+            }
+            if (rc) {
+#pragma omp atomic write
+                err = rc;
+            }
+        }
+    }
+    return err;
+}
 
 extern "C" int oracle_max_threads(void) {
 #ifdef _OPENMP
@@ -441,7 +574,7 @@ extern "C" int oracle_max_threads(void) {
 
 extern "C" int oracle_eval(const oracle_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T,
                            double *wdot, double *cqss, double *Sc, double *jac, double *jscale, int mode, int nthreads) {
-    if (!m || !C || !T || ncells < 0 || ld < ncells || mode < 0 || mode > 4) return -1;
+    if (!m || !C || !T || ncells < 0 || ld < ncells || mode < 0 || mode > 5) return -1;
     const int N = m->n_nqss, NC = N + 1;
     if (nthreads <= 0) nthreads = oracle_max_threads();
     int err = 0;
@@ -451,8 +584,8 @@ extern "C" int oracle_eval(const oracle_mech_t *m, int64_t ncells, int64_t ld, c
 #pragma omp for schedule(dynamic, 8)
         for (int64_t c = 0; c < ncells; ++c) {
             int rc = 0;
-            if (mode == ORACLE_EXPLICIT_F64 || mode == ORACLE_JAC_CONST_QSS) {
-                rc = run_explicit<double>(m, c, ld, C, T, wdot, cqss, Sc, jac, jscale, mode == ORACLE_JAC_CONST_QSS, wd);
+            if (mode == ORACLE_EXPLICIT_F64 || mode == ORACLE_JAC_CONST_QSS || mode == ORACLE_JAC_ZERO_QSS) {
+                rc = run_explicit<double>(m, c, ld, C, T, wdot, cqss, Sc, jac, jscale, mode != ORACLE_EXPLICIT_F64, wd, mode == ORACLE_JAC_ZERO_QSS);
             } else if (mode == ORACLE_EXPLICIT_F128) {
                 rc = run_explicit<Quad>(m, c, ld, C, T, wdot, cqss, Sc, jac, jscale, false, wq);
             } else {

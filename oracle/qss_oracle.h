@@ -40,13 +40,21 @@ enum {
     ORACLE_EXPLICIT_F128  = 1,  /* same formulas in __float128, rounded to double at the end (referee)         */
     ORACLE_JAC_DUAL       = 2,  /* Jacobian by forward-mode dual numbers through the wdot routine              */
     ORACLE_JAC_CSTEP      = 3,  /* Jacobian by complex step (h = 1e-30) through the wdot routine               */
-    ORACLE_JAC_CONST_QSS  = 4   /* explicit formulas with the chain term W_y*Y_x dropped        */
+    ORACLE_JAC_CONST_QSS  = 4,  /* explicit formulas with the chain term W_y*Y_x dropped        */
+    ORACLE_JAC_ZERO_QSS   = 5   /* chain term dropped AND C_QSS := 0 in the partials ("zero QSS AJ") */
 };
 
 /* Any output pointer may be NULL (skipped). Returns 0, or -1 on a bad argument.
  * wdot/cqss/S are always from the explicit routine in the precision `mode` implies. */
 int oracle_eval(const oracle_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T,
                 double *wdot, double *cqss, double *S, double *jac, double *jscale, int mode, int nthreads);
+
+/* NEXT-1 (Eq. 7): temperature right-hand side of the adiabatic constant-volume reactor,
+ *   tdot[c] = -T sum_i (h_i/RT - 1) wdot_i / sum_i C_i (cp_i/R - 1)   (sums over the transported species, reading G17),
+ * and the energy row of the (N+1) x (N+1) Jacobian, erow[k*ld + c] = d Tdot / d C_k (k < N), d Tdot / d T (k = N);
+ * escale: running-error scale of the row (explicit modes only).  mode: ORACLE_EXPLICIT_F64 / _F128 / _JAC_DUAL / _JAC_CSTEP. */
+int oracle_eval_energy(const oracle_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T,
+                       double *tdot, double *erow, double *escale, int mode, int nthreads);
 
 /* One cell: effective forward / reverse rate constants (k including the third-body or fall-off factor,
  * kb = k / Kc; 0 for a disabled direction). kf, kb: [n_reac]. */
