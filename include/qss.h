@@ -130,6 +130,26 @@ int qss_eval_wdot(const qss_mech_t *mech, int64_t ncells, int64_t ld, const doub
 int qss_eval_jac(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *C, const double *T,
                  double *jac, double *wdot_or_null, void *workspace, size_t workspace_bytes, void *stream);
 
+/* The paper's simplified Jacobians (Table 5a), cheap modes of the same kernel:
+ *   QSS_JAC_EXACT      the exact analytical Jacobian of qss_eval_jac (Eq. 9)
+ *   QSS_JAC_CONST_QSS  "constant QSS AJ": the second term of Eq. 9 (chain rule through the closure) is dropped
+ *   QSS_JAC_ZERO_QSS   "zero QSS AJ": additionally the QSS concentrations are nullified in every partial derivative
+ * Same layout and workspace as qss_eval_jac; wdot is not produced.  Returns QSS_E_UNSUPPORTED when the handle does not run
+ * kernel variant 3 (qss_mech_info.kernel_variant_jac != 3). */
+typedef enum { QSS_JAC_EXACT = 0, QSS_JAC_CONST_QSS = 1, QSS_JAC_ZERO_QSS = 2 } qss_jac_mode;
+int qss_eval_jac_approx(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *C, const double *T, double *jac,
+                        int mode, void *workspace, size_t workspace_bytes, void *stream);
+
+/* NEXT-1 of the build plan: the last row of the paper's (N+1) x (N+1) Jacobian (Eq. 7; state {C, T} L181) and the
+ * temperature right-hand side, for the adiabatic constant-volume reactor the paper integrates (L190), "simply obtained from
+ * the species production rates" (L278) and the NASA-7 polynomials (reading G17; sums over the transported species):
+ *   tdot[c]        = -T sum_i (h_i/RT - 1) wdot_i / sum_i C_i (cp_i/R - 1)                      K/s
+ *   erow[k*ld + c] = d tdot / d C_k (k < N),  d tdot / d T (k = N)
+ * Inputs: the state and the outputs wdot, jac of qss_eval_jac for the same cells (DEVICE pointers, same layout, 16-byte
+ * aligned); outputs tdot [ld], erow [(N+1)*ld].  One kernel on `stream`, bound by reading jac once.  N <= 430. */
+int qss_eval_energy(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *C, const double *T, const double *wdot,
+                    const double *jac, double *tdot, double *erow, void *stream);
+
 /* Host-buffer convenience used for end-to-end timing: copies C and T to the device (in `dev_scratch`, which
  * must hold qss_host_scratch_bytes() bytes), evaluates, copies the Jacobian (and wdot if not NULL) back to
  * the HOST buffers, and synchronises `stream`.  Host buffers should be pinned for full copy bandwidth.  Large batches are

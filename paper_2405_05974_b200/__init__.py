@@ -17,7 +17,7 @@ from . import build as _build
 __all__ = ["lib", "QssMech", "QssError", "EXPORTS", "STATUS"]
 
 EXPORTS = ["qss_mech_create", "qss_mech_validate", "qss_mech_specialise_check", "qss_mech_destroy", "qss_mech_info", "qss_mech_qss_order", "qss_eval_wdot",
-           "qss_eval_jac", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
+           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
 STATUS = {0: "QSS_OK", -1: "QSS_E_INVALID", -2: "QSS_E_QUADRATIC", -3: "QSS_E_QSS_FANOUT", -4: "QSS_E_NO_SINK",
           -5: "QSS_E_UNSUPPORTED", -6: "QSS_E_CUDA", -7: "QSS_E_UNBALANCED"}
 
@@ -68,6 +68,8 @@ def lib():
         L.qss_mech_qss_order.restype = ct.c_int; L.qss_mech_qss_order.argtypes = [vp, vp, vp]
         L.qss_eval_wdot.restype = ct.c_int; L.qss_eval_wdot.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, ct.c_size_t, vp]
         L.qss_eval_jac.restype = ct.c_int; L.qss_eval_jac.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, ct.c_size_t, vp]
+        L.qss_eval_jac_approx.restype = ct.c_int; L.qss_eval_jac_approx.argtypes = [vp, i64, i64, vp, vp, vp, ct.c_int, vp, ct.c_size_t, vp]
+        L.qss_eval_energy.restype = ct.c_int; L.qss_eval_energy.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp]
         L.qss_host_scratch_bytes.restype = ct.c_size_t; L.qss_host_scratch_bytes.argtypes = [vp, i64, i64]
         L.qss_eval_jac_host.restype = ct.c_int; L.qss_eval_jac_host.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, ct.c_size_t, vp]
         L.qss_bench_dfma.restype = ct.c_int; L.qss_bench_dfma.argtypes = [ct.c_int, ct.c_int, vp, ct.POINTER(ct.c_double), vp]
@@ -207,6 +209,31 @@ class QssMech:
         _check(lib().qss_eval_jac(self._h, ncells, ld, _ptr(C), _ptr(T), _ptr(jac), _ptr(wdot), _ptr(ws),
                                   ws.numel(), self._stream()))
         return (jac, wdot) if want_wdot else jac
+
+    def eval_jac_approx(self, C, T, mode, ncells=None, jac=None):
+        """The paper's simplified Jacobians: mode 0 exact, 1 constant-QSS AJ, 2 zero-QSS AJ. Returns jac [N, N+1, ld]."""
+        import torch
+        ld = C.shape[1]
+        ncells = ld if ncells is None else int(ncells)
+        assert C.dtype == torch.float64 and T.dtype == torch.float64 and C.is_contiguous() and T.is_contiguous()
+        if jac is None:
+            jac = torch.empty((self.N, self.N + 1, ld), dtype=torch.float64, device=C.device)
+        ws = self.workspace(True)
+        _check(lib().qss_eval_jac_approx(self._h, ncells, ld, _ptr(C), _ptr(T), _ptr(jac), int(mode), _ptr(ws), ws.numel(), self._stream()))
+        return jac
+
+    def eval_energy(self, C, T, wdot, jac, ncells=None, tdot=None, erow=None):
+        """Temperature right-hand side tdot [ld] and energy row erow [N+1, ld] of the full (N+1) x (N+1) Jacobian (qss_eval_energy)."""
+        import torch
+        ld = C.shape[1]
+        ncells = ld if ncells is None else int(ncells)
+        assert wdot.is_contiguous() and jac.is_contiguous() and wdot.shape == (self.N, ld) and jac.shape == (self.N, self.N + 1, ld)
+        if tdot is None:
+            tdot = torch.empty((ld,), dtype=torch.float64, device=C.device)
+        if erow is None:
+            erow = torch.empty((self.N + 1, ld), dtype=torch.float64, device=C.device)
+        _check(lib().qss_eval_energy(self._h, ncells, ld, _ptr(C), _ptr(T), _ptr(wdot), _ptr(jac), _ptr(tdot), _ptr(erow), self._stream()))
+        return tdot, erow
 
     def host_scratch_bytes(self, ncells, ld):
         return int(lib().qss_host_scratch_bytes(self._h, int(ncells), int(ld)))

@@ -19,6 +19,8 @@ cudaError_t qss_launch_slab(const QssTab &t, bool jac, int64_t ncells, int64_t l
                             double *wdot, double *cqss, double *jacp, double *ws, int nblocks, int nwarp,
                             cudaStream_t stream);
 cudaError_t qss_launch_dfma(int blocks, int iters, double *sink, cudaStream_t stream);
+cudaError_t qss_launch_energy(const double *D, int d_thermo, int N, int64_t ncells, int64_t ld, const double *C, const double *T, const double *wdot,
+                              const double *jac, double *tdot, double *erow, cudaStream_t stream);
 size_t qss_v1_scratch_doubles(const QssV1 &v);
 cudaError_t qss_v1_prepare();
 cudaError_t qss_launch_v1(const QssV1 &v, bool jac, int nblocks, cudaStream_t stream);
@@ -261,8 +263,36 @@ extern "C" int qss_eval_wdot(const qss_mech_t *m, int64_t ncells, int64_t ld, co
     return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_eval_wdot launch");
 }
 
+static int eval_jac_mode(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T, double *jac, double *wdot, int mode,
+                         void *workspace, size_t workspace_bytes, void *stream);
+
 extern "C" int qss_eval_jac(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T,
                             double *jac, double *wdot, void *workspace, size_t workspace_bytes, void *stream) {
+    return eval_jac_mode(m, ncells, ld, C, T, jac, wdot, 0, workspace, workspace_bytes, stream);
+}
+
+extern "C" int qss_eval_jac_approx(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T, double *jac,
+                                   int mode, void *workspace, size_t workspace_bytes, void *stream) {
+    if (mode < 0 || mode > 2) return fail(QSS_E_INVALID, "mode must be QSS_JAC_EXACT, QSS_JAC_CONST_QSS or QSS_JAC_ZERO_QSS");
+    if (m && mode != 0 && !m->jit3) return fail(QSS_E_UNSUPPORTED, "the simplified Jacobians need kernel variant 3 (qss_mech_info.kernel_variant_jac)");
+    return eval_jac_mode(m, ncells, ld, C, T, jac, nullptr, mode, workspace, workspace_bytes, stream);
+}
+
+extern "C" int qss_eval_energy(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T, const double *wdot,
+                               const double *jac, double *tdot, double *erow, void *stream) {
+    if (!m) return fail(QSS_E_INVALID, "mech is NULL");
+    if (ncells < 0 || ld < ncells) return fail(QSS_E_INVALID, "need 0 <= ncells <= ld");
+    if (ncells == 0) return QSS_OK;
+    if (!C || !T || !wdot || !jac || !tdot || !erow) return fail(QSS_E_INVALID, "NULL device pointer");
+    if (((uintptr_t)C | (uintptr_t)T | (uintptr_t)wdot | (uintptr_t)jac | (uintptr_t)tdot | (uintptr_t)erow) & 15) return fail(QSS_E_INVALID, "device pointers must be 16-byte aligned");
+    if (m->c.tab.N > 430) return fail(QSS_E_UNSUPPORTED, "qss_eval_energy: more than 430 transported species");
+    DeviceGuard guard(m->device);
+    cudaError_t e = qss_launch_energy(m->dD, m->c.tab.d_thermo, m->c.tab.N, ncells, ld, C, T, wdot, jac, tdot, erow, (cudaStream_t)stream);
+    return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_eval_energy launch");
+}
+
+static int eval_jac_mode(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T, double *jac, double *wdot, int mode,
+                         void *workspace, size_t workspace_bytes, void *stream) {
     int rc = check_eval(m, ncells, ld, C, T, jac, workspace, workspace_bytes, m ? ws_bytes(m, true) : 0);
     if (rc != QSS_OK || ncells == 0) return rc;
     DeviceGuard guard(m->device);
@@ -271,7 +301,7 @@ extern "C" int qss_eval_jac(const qss_mech_t *m, int64_t ncells, int64_t ld, con
         QssV3 v;
         v.C = C; v.T = T; v.wdot = wdot; v.cqss = nullptr; v.jac = jac; v.scratch = (double *)workspace;
         v.ncells = ncells; v.ld = ld; v.scratch_stride = (int64_t)m->c.v3.scratch_rows * 32;
-        v.dP = m->dP3; v.iP = m->iP3; v.timing = m->timing;
+        v.dP = m->dP3; v.iP = m->iP3; v.timing = m->timing; v.mode = mode;
         e = qss_jit3_launch(m->jit3, v, m->n_sm, m->c.v3.nw, (size_t)m->c.v3.smem_bytes, (cudaStream_t)stream);
     } else if (m->variant == 1) {
         QssV1 v = m->c.v1;

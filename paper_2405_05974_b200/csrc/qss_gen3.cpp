@@ -413,7 +413,7 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
     {
         int dist = 12, fdist = 4, sdist = 3, pdist = 8;      // loads run this many items ahead of their use
         if (const char *e = qss_devenv("QSS3_DIST")) std::sscanf(e, "%d,%d,%d,%d", &dist, &fdist, &sdist, &pdist);
-        G("__device__ __forceinline__ void qss_gen_column(const int k, const unsigned sml, const unsigned sml2, const double *sc, double *jc, const long long rs, const bool active) {\n    double ");
+        G("__device__ __forceinline__ void qss_gen_column(const int k, const int mode, const unsigned sml, const unsigned sml2, const double *sc, double *jc, const long long rs, const bool active) {\n    double ");
         for (int s = 0; s < nsp; ++s) G("c%d%s", s, s + 1 < nsp ? ", " : ";\n");
         G("    if (k < %d) {\n", N);
         for (int s = 0; s < nsp; ++s) G("        c%d = lS<%d>(sml);\n", s, (R_TV + s) * PITCH);
@@ -452,6 +452,9 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
             G("    } break;\n");
         }
         G("    default: break;\n    }\n");
+        // the chain-rule term (dy/dx solve, W_y dy/dx) belongs to the exact Jacobian only; the constant-QSS and zero-QSS
+        // approximations of PAPER.md L232 (mode 1, 2) stop at W_x
+        G("    if (mode == 0) {\n");
         {   // dy/dx solve; the operations of independent groups are interleaved (two chains)
             std::vector<const Op *> ch[2];
             size_t len[2] = {0, 0};
@@ -528,6 +531,7 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
                 G(" }\n");
             }
         }
+        G("    }\n");
         G("    if (active) {\n");
         for (int i = 0; i < N; ++i) G("        __stcs(jc + %d * rs, c%d);\n", i, i);
         G("    }\n}\n");

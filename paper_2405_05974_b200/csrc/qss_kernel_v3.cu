@@ -414,6 +414,12 @@ qss_v3_wdot(const __grid_constant__ QssV3 p) {
         __syncthreads();
         QSS_TICK(3);
         qss_gen_closure(warp, sml);
+#if QSS3_JAC
+        if (p.mode == 2) {      // zero-QSS AJ: the QSS concentrations are nullified in every partial derivative
+            for (int q = warp; q < G_NQ; q += G_NW) sts(sml + (R_Y + q) * G_PITCH, 0.0);
+            __syncthreads();
+        }
+#endif
         QSS_TICK(4);
         // ---- P5: net rates of progress Q_j (Eq. 2), dQ_j/dT, dQ_j/dM; they replace kappa_f, kappa_b, d ln k/dM in place
         for (int t = nt0; t < nt1; ++t) {
@@ -466,7 +472,7 @@ qss_v3_wdot(const __grid_constant__ QssV3 p) {
         }
         for (int dd = 0; dd < QSS_GEN_DEPTH; ++dd) {
             const int k = qss_gen_cols[warp * QSS_GEN_DEPTH + dd];
-            if (k >= 0) qss_gen_column(k, sml, sm0 + lane * 16, sc, p.jac + (size_t)(unsigned)k * (size_t)ld + cell, (long long)(G_N + 1) * ld, active);
+            if (k >= 0) qss_gen_column(k, p.mode, sml, sm0 + lane * 16, sc, p.jac + (size_t)(unsigned)k * (size_t)ld + cell, (long long)(G_N + 1) * ld, active);
         }
         QSS_TICK(8);
 #endif

@@ -40,6 +40,7 @@ struct QssV3 {
     const double *dP;                            // [QSS3_NDP][n_slot]
     const int32_t *iP;                           // [QSS3_NIP][n_slot]
     long long *timing;                           // NULL, or 16 phase counters (images built with -DQSS3_TIMING=1 only)
+    int32_t mode;                                // 0 exact Jacobian; 1 constant-QSS AJ (no chain term); 2 zero-QSS AJ (also C_QSS := 0)
 };
 
 #endif

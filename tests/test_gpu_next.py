@@ -1,0 +1,83 @@
+"""GPU parity of the NEXT rows built so far: NEXT-1, the temperature right-hand side and the energy row of the
+(N+1) x (N+1) Jacobian (qss_eval_energy; Eq. 7), and NEXT-3, the paper's simplified Jacobians
+(qss_eval_jac_approx; constant-QSS AJ and zero-QSS AJ, L232), against the CPU oracle on the same seeded inputs."""
+import numpy as np
+import pytest
+
+import gates
+import oracle
+import qss_synth
+from qss_synth import make_states
+
+pytestmark = pytest.mark.gpu
+
+
+def _energy_gates(tdot, erow, ref, T, n, what):
+    e, s = ref["erow"][:, :n], ref["escale"][:, :n]
+    d = np.abs(erow[:, :n] - e)
+    assert np.isfinite(erow[:, :n]).all() and np.isfinite(tdot[:n]).all(), what
+    bound = 1e-9 * np.abs(e) + 1e-12 * s
+    assert np.all(d <= bound), f"{what}: energy row, worst ratio {float(np.max(d / bound)):.3g}"
+    # strict tier over the entries that are not cancellation residues, as for the species block (reading G16)
+    well = s <= 1e3 * np.abs(e)
+    assert well.mean() > 0.5 and (d[well] <= 1e-9 * np.abs(e[well])).mean() >= 0.99, what
+    dt = np.abs(tdot[:n] - ref["tdot"][:n])
+    assert np.all(dt <= 1e-10 * np.abs(ref["tdot"][:n]) + 1e-13 * s[-1] * T[:n]), f"{what}: tdot"
+
+
+@pytest.mark.parametrize("name,n", [("cfg1", 4096), ("cfg2", 2048 + 19), ("cfg3", 192 + 5), ("toy_dag", 77), ("toy_nonqss", 33)])
+def test_energy_row_and_temperature_rhs(name, n):
+    import torch
+    import paper_2405_05974_b200 as qss
+    if name.startswith("cfg"):
+        mech = qss_synth.config_mechanism(int(name[3])); C, T = qss_synth.config_states(int(name[3]), n)
+    else:
+        mech = getattr(qss_synth, name)(); C, T = make_states(mech.n_nqss, n, seed=5)
+    ld = C.shape[1]
+    qm = qss.QssMech(mech, 0)
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda()
+    J, w = qm.eval_jac(Cd, Td, n, want_wdot=True)
+    tdot = torch.full((ld,), float("nan"), dtype=torch.float64, device="cuda")
+    erow = torch.full((qm.N + 1, ld), float("nan"), dtype=torch.float64, device="cuda")
+    qm.eval_energy(Cd, Td, w, J, n, tdot=tdot, erow=erow)
+    torch.cuda.synchronize()
+    ref = oracle.evaluate_energy(oracle.OracleMech(mech), C, T, n)
+    _energy_gates(tdot.cpu().numpy(), erow.cpu().numpy(), ref, T, n, name)
+    if ld > n:
+        assert torch.isnan(tdot[n:]).all() and torch.isnan(erow[:, n:]).all(), "padding was written"
+    qm.close()
+
+
+@pytest.mark.parametrize("name,n", [("cfg1", 1024 + 3), ("cfg2", 512 + 7), ("toy_dag", 77), ("toy3", 40)])
+@pytest.mark.parametrize("mode", [1, 2])
+def test_simplified_jacobians(name, n, mode):
+    """Constant-QSS AJ (mode 1) and zero-QSS AJ (mode 2) against the oracle's modes of the same definition; mode 0 through the same
+    entry point is the exact Jacobian bit for bit."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    if name.startswith("cfg"):
+        mech = qss_synth.config_mechanism(int(name[3])); C, T = qss_synth.config_states(int(name[3]), n)
+    else:
+        mech = getattr(qss_synth, name)(); C, T = make_states(mech.n_nqss, n, seed=5)
+    qm = qss.QssMech(mech, 0)
+    assert qm.info.kernel_variant_jac == 3
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda()
+    Ja = qm.eval_jac_approx(Cd, Td, mode, n).cpu().numpy()
+    J0 = qm.eval_jac_approx(Cd, Td, 0, n)
+    assert torch.equal(J0[:, :, :n], qm.eval_jac(Cd, Td, n)[:, :, :n])
+    om = oracle.OracleMech(mech)
+    ref = oracle.evaluate(om, C, T, n, mode=oracle.JAC_CONST_QSS if mode == 1 else oracle.JAC_ZERO_QSS, want_scale=True)
+    gates.assert_jac(Ja, ref["jac"], ref["jscale"], n, f"{name} simplified Jacobian mode {mode}")
+    qm.close()
+
+
+def test_simplified_jacobians_need_variant_3():
+    import torch
+    import paper_2405_05974_b200 as qss
+    mech = qss_synth.config_mechanism(3)
+    qm = qss.QssMech(mech, 0)
+    C, T = qss_synth.config_states(3, 64)
+    with pytest.raises(qss.QssError) as e:
+        qm.eval_jac_approx(torch.from_numpy(C).cuda(), torch.from_numpy(T).cuda(), 1, 64)
+    assert e.value.code == -5
+    qm.close()
