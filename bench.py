@@ -32,6 +32,11 @@ METRIC = "cells/sec for wdot+analytical QSS Jacobian (fp64) per B200; % of roofl
 UNIT = "cells/s"
 ORACLE_SAMPLE = {1: 4096, 2: 1 << 15, 3: 1 << 12, 4: 1 << 15, 5: 1 << 9}   # cells of the CPU-oracle sample
 FP64_LANES_PER_SM = 64          # 148 SMs x 64 fp64 FMA lanes x 1.965 GHz
+EXPECTED_JAC_VARIANT = {1: 3, 2: 3, 4: 3, 3: 0, 5: 0}   # the kernel each BASELINE config is expected to run on
+CALLS = {"jac+wdot": "qss_eval_jac with the wdot output (the metric)", "jac": "qss_eval_jac alone", "wdot": "qss_eval_wdot alone",
+         "jac+wdot+energy": "qss_eval_jac with wdot, then qss_eval_energy: the full (N+1)x(N+1) Jacobian and the temperature right-hand side",
+         "energy": "qss_eval_energy alone (on a Jacobian computed before the timed region)",
+         "jac_const": "qss_eval_jac_approx, constant-QSS AJ", "jac_zero": "qss_eval_jac_approx, zero-QSS AJ"}
 
 
 def _peaks():
@@ -140,15 +145,21 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (1-based); default 2 = configs[1]")
     ap.add_argument("--cells", type=int, default=0, help="override the cell count (0 = the config's)")
-    ap.add_argument("--call", default="jac+wdot", choices=["jac+wdot", "jac", "wdot"],
-                    help="which C-ABI call a step is: qss_eval_jac with wdot output (the metric), qss_eval_jac alone, qss_eval_wdot alone")
+    ap.add_argument("--call", default="jac+wdot", choices=sorted(CALLS), help="which C-ABI call(s) a step is: " + "; ".join(f"{k}: {v}" for k, v in CALLS.items()))
+    ap.add_argument("--allow-fallback", action="store_true", help="do not fail when the library selected another kernel variant than the expected one")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    cfg = args.config
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # plain `python bench.py --gpus N`: launch the N ranks ourselves, the way the driver does (one process per GPU)
+        port = 29500 + os.getpid() % 2000
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.run(cmd).returncode)
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    cfg = args.config
     if args.impl == "reference":
         run_reference(args, cfg, rank)
         return
@@ -159,11 +170,16 @@ def main():
     import paper_2405_05974_b200 as qss
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: libqss has no CPU fallback")
+    ndev = torch.cuda.device_count()
+    local = local % ndev                     # more ranks than devices (a 1-GPU box): the ranks share a device, timing is then not a scaling number
     torch.cuda.set_device(local)
     dist = None
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if world <= ndev:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("gloo")  # NCCL refuses two ranks on one device; the group only carries the barrier and the max of the times
     dev = torch.device("cuda", local)
 
     mech = qss_synth.config_mechanism(cfg)
@@ -183,12 +199,27 @@ def main():
     stream = torch.cuda.current_stream()
 
     qm.workspace(False)
+    expect = EXPECTED_JAC_VARIANT.get(cfg)
+    forced = "QSS_VARIANT" in os.environ or "QSS_JIT" in os.environ
+    if expect is not None and qm.info.kernel_variant_jac != expect and not args.allow_fallback and not forced:
+        raise SystemExit(f"bench.py: cfg{cfg} ran on kernel variant {qm.info.kernel_variant_jac}, expected {expect} (run-time compilation unavailable?); "
+                         "--allow-fallback times it anyway")
+    tdot = torch.empty((ld,), dtype=torch.float64, device=dev); erow = torch.empty((N + 1, ld), dtype=torch.float64, device=dev)
+    if args.call == "energy":
+        qm.eval_jac(Cd, Td, n, jac=J, wdot=W, want_wdot=True)
+    launches_per_step = 2 if args.call == "jac+wdot+energy" else 1
 
     def step():
-        if args.call == "jac+wdot":
+        if args.call in ("jac+wdot", "jac+wdot+energy"):
             qm.eval_jac(Cd, Td, n, jac=J, wdot=W, want_wdot=True)
+            if args.call == "jac+wdot+energy":
+                qm.eval_energy(Cd, Td, W, J, n, tdot=tdot, erow=erow)
         elif args.call == "jac":
             qm.eval_jac(Cd, Td, n, jac=J)
+        elif args.call == "energy":
+            qm.eval_energy(Cd, Td, W, J, n, tdot=tdot, erow=erow)
+        elif args.call in ("jac_const", "jac_zero"):
+            qm.eval_jac_approx(Cd, Td, 1 if args.call == "jac_const" else 2, n, jac=J)
         else:
             qm.eval_wdot(Cd, Td, n, wdot=W)
 
@@ -219,7 +250,7 @@ def main():
     total_ms = evs[0].elapsed_time(evs[-1])
     launch_ms = [evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)]
     from paper_2405_05974_b200.shard import max_over_ranks
-    total_ms_max = max_over_ranks(total_ms, dist, dev)
+    total_ms_max = max_over_ranks(total_ms, dist, dev if (dist is None or dist.get_backend() == "nccl") else None)
     value = world * n * args.steps / (total_ms_max * 1e-3)
 
     # ---- end to end through the C-ABI host-buffer call: pinned host buffers, H2D + D2H inside the timed region
@@ -239,7 +270,7 @@ def main():
             qm.eval_jac_host(Ch, Th, Jh, Wh, scratch, n)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        e2e = {"value": world * n * ke / max_over_ranks(dt, dist, dev), "unit": UNIT,
+        e2e = {"value": world * n * ke / max_over_ranks(dt, dist, dev if (dist is None or dist.get_backend() == "nccl") else None), "unit": UNIT,
                "h2d_bytes_per_step": int((N + 1) * ld * 8), "d2h_bytes_per_step": int((N * (N + 1) + N) * ld * 8),
                "steps": ke, "api": "qss_eval_jac_host (C-ABI, pinned host buffers, copies + kernel + sync timed by wall clock)"}
         assert bool(torch.isfinite(Wh[:, :n]).all())
@@ -255,8 +286,10 @@ def main():
     avg_s = statistics.mean(launch_ms) * 1e-3
     if args.call == "wdot":
         bytes_cell, slots_cell = info.bytes_wdot, info.slots_wdot
+    elif args.call == "energy":        # reads C, T, wdot and J once, writes the row and tdot; 2 N (N+1) + ~30 N fp64 slots
+        bytes_cell, slots_cell = 8.0 * (N * (N + 1) + 2 * N + 1) + 8.0 * (N + 2), 2.0 * N * (N + 1) + 30.0 * N
     else:
-        bytes_cell, slots_cell = info.bytes_jac + (8.0 * N if args.call == "jac+wdot" else 0.0), info.slots_jac
+        bytes_cell, slots_cell = info.bytes_jac + (8.0 * N if args.call.startswith("jac+wdot") else 0.0), info.slots_jac
     bytes_launch = bytes_cell * n
     slots_launch = slots_cell * n
     fp64_peak_slots = sms * FP64_LANES_PER_SM * sm_max_mhz * 1e6
@@ -268,14 +301,14 @@ def main():
     roof["frac"] = roof["achieved"] / roof["peak"]
     traffic = None
     try:        # bytes of one launch from the committed ncu capture of the same workload and kernel variant, else null
-        with open(os.path.join(ROOT, "profiles", "r01_traffic.txt")) as f:
+        with open(os.path.join(ROOT, "profiles", "r02_traffic.txt")) as f:
             tj = json.load(f)
         if args.call == "jac+wdot" and tj["cfg"] == cfg and tj["cells"] == n and tj["kernel_variant"] == info.kernel_variant_jac:
             traffic = tj["dram_bytes_per_launch"]
     except Exception:
         traffic = None
-    roof.update({"traffic": traffic, "traffic_unit": "bytes per launch (dram read + write, ncu)", "kernel": {"jac+wdot": "qss jacobian kernel (qss_eval_jac, wdot output on)", "jac": "qss jacobian kernel (qss_eval_jac)",
-                            "wdot": "qss wdot kernel (qss_eval_wdot)"}[args.call],
+    roof.update({"traffic": traffic, "traffic_unit": "bytes per launch (dram read + write) from the committed ncu capture of this workload and kernel variant (profiles/r02_traffic.txt); not measurable inside this run",
+                 "kernel": "qss_energy_kernel" if args.call == "energy" else ("qss wdot kernel (qss_eval_wdot)" if args.call == "wdot" else f"qss jacobian kernel, variant {info.kernel_variant_jac} ({CALLS[args.call]})"),
                  "launch_ms_avg": avg_s * 1e3, "launch_ms_min": min(launch_ms),
                  "alg_fp64_slots_per_cell": slots_cell, "alg_bytes_per_cell": bytes_cell,
                  "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3,
@@ -307,7 +340,7 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic", "config": _config(cfg, mech, n, world),
-        "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps, "roofline": roof, "cpu_baseline": cpu,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * launches_per_step, "roofline": roof, "cpu_baseline": cpu,
         "kernel_variant": {"wdot": info.kernel_variant_wdot, "jac": info.kernel_variant_jac}, "mech_create_s": t_create,
         "call": args.call}))
     if dist is not None:
