@@ -62,7 +62,12 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
     const qss_mech_desc_t *d = c.desc;
     QssV3Host &v = out.v3;
     v = QssV3Host();
-    const int NW = 12, PITCH = 264, MAXROWS = (227 * 1024) / PITCH;
+    int NW = 12;                        // warps per block in every phase but the column sweep
+    if (const char *e = qss_devenv("QSS3_NW")) NW = std::atoi(e);
+    // registers per thread: at launch (all phases but the sweep), of the idle warps and of the column warps during the sweep
+    const int reg_base = std::min(255, 65536 / (NW * 32)) / 8 * 8, reg_idle = 24;
+    const int reg_col = NW > 12 ? reg_base + (NW - 12) * (reg_base - reg_idle) / 12 / 8 * 8 : reg_base;
+    const int NWC = 12, PITCH = 264, MAXROWS = (227 * 1024) / PITCH;      // NWC: column warps (one Jacobian column in ~160 registers each)
     if (M < 1) { why = "no reactions"; return false; }
     if (nsp > 60) { why = "more than 60 species: one Jacobian column does not fit the registers of a thread"; return false; }
     for (int j = 0; j < M; ++j)
@@ -264,8 +269,8 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
     // =================================================================================================================
     Gen G;
     G("// generated by qss_gen3.cpp for one mechanism (%d + %d species, %d reactions); compiled with qss_kernel_v3.cu\n", N, Nq, M);
-    G("#define G_N %d\n#define G_NQ %d\n#define G_M %d\n#define G_NSP %d\n#define G_MS %d\n#define G_NTB %d\n#define G_NW %d\n#define G_PITCH %d\n#define G_NSLOT %d\n",
-      N, Nq, M, nsp, MS, ntb, NW, PITCH, n_slot);
+    G("#define G_N %d\n#define G_NQ %d\n#define G_M %d\n#define G_NSP %d\n#define G_MS %d\n#define G_NTB %d\n#define G_NW %d\n#define G_NWC %d\n#define G_REG_BASE %d\n#define G_REG_IDLE %d\n#define G_REG_COL %d\n#define G_PITCH %d\n#define G_NSLOT %d\n",
+      N, Nq, M, nsp, MS, ntb, NW, NWC, reg_base, reg_idle, reg_col, PITCH, n_slot);
     G("#define R_V %d\n#define R_ONE %d\n#define R_Y %d\n#define R_T %d\n#define R_LNT %d\n#define R_INVT %d\n#define R_CT %d\n#define R_CL %d\n#define R_XP %d\n#define R_TV %d\n#define R_DLM %d\n#define R_KAP %d\n#define R_KQ %d\n#define R_STAGE %d\n",
       R_V, R_ONE, R_Y, R_T, R_LNT, R_INVT, R_CT, R_CL, R_XP, R_TV, R_DLM, R_KAP, R_KQ, R_STAGE);
     G("#define KQ_BASE %d\n", KQ_BASE);
@@ -543,16 +548,16 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
             cost[k] = 150.0 + prod_cost;
             if (k < N) for (const Rec &r : rec[k]) cost[k] += 6.0 * (3.0 + r.tgt.size());       // (stream code is fetched, not cached)
         }
-        const std::vector<int> bin = lpt(cost, NW);
+        const std::vector<int> bin = lpt(cost, NWC);
         size_t depth = 0;
-        std::vector<std::vector<int>> cols(NW);
+        std::vector<std::vector<int>> cols(NWC);
         for (int k = 0; k <= N; ++k) cols[bin[k]].push_back(k);
         for (auto &cw : cols) { std::stable_sort(cw.begin(), cw.end(), [&](int a, int b) { return cost[a] > cost[b]; }); depth = std::max(depth, cw.size()); }
         // every other warp takes its columns in the opposite order, so that the fetch-bound record streams of one half of the
         // warps run against the shared-memory-bound products of the other half
-        for (int w = 1; w < NW; w += 2) std::reverse(cols[w].begin(), cols[w].end());
+        for (int w = 1; w < NWC; w += 2) std::reverse(cols[w].begin(), cols[w].end());
         G("#define QSS_GEN_DEPTH %d\n__constant__ int qss_gen_cols[] = {", (int)depth);
-        for (int w = 0; w < NW; ++w) for (size_t dd = 0; dd < depth; ++dd) G("%d, ", dd < cols[w].size() ? cols[w][dd] : -1);
+        for (int w = 0; w < NWC; ++w) for (size_t dd = 0; dd < depth; ++dd) G("%d, ", dd < cols[w].size() ? cols[w][dd] : -1);
         G("-1};\n");
     }
     v.gen = G.s;

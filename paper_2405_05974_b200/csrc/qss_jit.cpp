@@ -212,6 +212,7 @@ QssJit *qss_jit_create(const std::string &gen_src, int cc_major, int cc_minor, s
 std::vector<std::string> defs3(bool jac) {
     std::vector<std::string> d = {jac ? "-DQSS3_JAC=1" : "-DQSS3_JAC=0"};
     if (qss_devenv("QSS_TIMING")) d.push_back("-DQSS3_TIMING=1");
+    if (const char *x = qss_devenv("QSS3_EXP")) d.push_back(std::string("-DQSS3_X=") + x);      // (development builds: experiment switches)
     return d;
 }
 

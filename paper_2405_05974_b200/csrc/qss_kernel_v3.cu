@@ -81,7 +81,12 @@ __device__ __forceinline__ double vfms(double a, double b, double c) {      // a
 #define QSS_TICK(ph) do { } while (0)
 #endif
 
+#ifndef QSS3_X
+#define QSS3_X 2
+#endif
+#if QSS3_X & 2
 #define qss_exp qss_exp_e
+#endif
 constexpr double kLn10 = 2.302585092994045684017991454684;
 constexpr double kInvLn10 = 0.434294481903251827651128918916605;
 
@@ -206,7 +211,7 @@ __device__ __forceinline__ void qss3_rate_task(const RateCommon &r, const int sl
     const double flo[3] = {2.0 * r.elo[3], 3.0 * r.elo[4], 4.0 * r.elo[5]}, fhi[3] = {2.0 * r.ehi[3], 3.0 * r.ehi[4], 4.0 * r.ehi[5]};
     const bool valid = (r.flags >> 4) & 1;
     const unsigned kap = sm0 + r.kap;
-    constexpr int STEP = TYPE == 2 ? 1 : 2;                      // two cells per step: four independent exponential chains
+    constexpr int STEP = (TYPE == 2 || !(QSS3_X & 1)) ? 1 : 2;     // two cells per step: four independent exponential chains
 #pragma unroll 1
     for (int c = c0; c < c1; c += STEP) {
         double kf[STEP], kb[STEP], dm[STEP], dk[STEP], dz[STEP];
@@ -333,7 +338,9 @@ qss_v3_wdot(const __grid_constant__ QssV3 p) {
         const int64_t cc = active ? cell : p.ncells - 1;          // idle lanes of a ragged tail shadow the last cell
         // the parameters of the warp's first rate task are fetched now (independent of the cells; L2 latency)
         RateCommon rc;
+#if QSS3_X & 4
         if (rt0 < rt1) qss3_load_common(rc, p, tab(sm0, T_RT + 4 * rt0 + 1) + lane);
+#endif
         // ---- P0: inputs.  Every slab but the block's first was fetched into the staging rows during the previous slab's
         //      column sweep (cp.async below); every warp waits for and moves the rows it fetched itself.
 #if QSS3_JAC
@@ -371,8 +378,13 @@ qss_v3_wdot(const __grid_constant__ QssV3 p) {
         // ---- P2: rate constants (Eq. 2), lane = reaction
         for (int t = rt0; t < rt1; ++t) {
             const int type = tab(sm0, T_RT + 4 * t), slot0 = tab(sm0, T_RT + 4 * t + 1), c0 = tab(sm0, T_RT + 4 * t + 2), c1 = tab(sm0, T_RT + 4 * t + 3);
+#if QSS3_X & 4
             const RateCommon cur = rc;
             if (t + 1 < rt1) qss3_load_common(rc, p, tab(sm0, T_RT + 4 * t + 5) + lane);      // the next task's parameters, under this one
+#else
+            qss3_load_common(rc, p, slot0 + lane);                // (128 registers per thread: no room for a second parameter set)
+            const RateCommon &cur = rc;
+#endif
             if (type == 0) qss3_rate_task<0>(cur, slot0, c0, c1, sm0, scb, p);
             else if (type == 1) qss3_rate_task<1>(cur, slot0, c0, c1, sm0, scb, p);
             else qss3_rate_task<2>(cur, slot0, c0, c1, sm0, scb, p);
@@ -470,10 +482,28 @@ qss_v3_wdot(const __grid_constant__ QssV3 p) {
                 asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sml + (R_STAGE + s) * G_PITCH), "l"(p.C + (size_t)s * ld + cc2) : "memory");
             if (warp == 0) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sml + (R_STAGE + G_N) * G_PITCH), "l"(p.T + cc2) : "memory");
         }
+#if G_NW > G_NWC
+        // More warps than columns in flight (a column needs ~160 registers, the other phases run G_NW warps at 128): the extra
+        // warp group hands its registers to the column warps for the sweep (setmaxnreg) and waits at the end-of-slab barrier.
+        if (warp < G_NWC) {
+            asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(G_REG_COL));
+            for (int dd = 0; dd < QSS_GEN_DEPTH; ++dd) {
+                const int k = qss_gen_cols[warp * QSS_GEN_DEPTH + dd];
+                if (k >= 0) qss_gen_column(k, p.mode, sml, sm0 + lane * 16, sc, p.jac + (size_t)(unsigned)k * (size_t)ld + cell, (long long)(G_N + 1) * ld, active);
+            }
+            asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(G_REG_BASE));
+            asm volatile("bar.arrive 1, %0;" ::"n"(G_NW * 32));
+        } else {
+            asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(G_REG_IDLE));
+            asm volatile("bar.sync 1, %0;" ::"n"(G_NW * 32));            // until the column warps have released their registers
+            asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(G_REG_BASE));
+        }
+#else
         for (int dd = 0; dd < QSS_GEN_DEPTH; ++dd) {
             const int k = qss_gen_cols[warp * QSS_GEN_DEPTH + dd];
             if (k >= 0) qss_gen_column(k, p.mode, sml, sm0 + lane * 16, sc, p.jac + (size_t)(unsigned)k * (size_t)ld + cell, (long long)(G_N + 1) * ld, active);
         }
+#endif
         QSS_TICK(8);
 #endif
         __syncthreads();      // shared memory and the scratch slab are reused by the next cell slab
