@@ -85,7 +85,7 @@ __device__ __forceinline__ double vfms(double a, double b, double c) {      // a
 #define QSS3_X 2
 #endif
 #if QSS3_X & 2
-#define qss_exp qss_exp_e
+#define qss_exp qss_exp_e        // (its constants as operands from the constant bank instead of literals: measured, no gain)
 #endif
 constexpr double kLn10 = 2.302585092994045684017991454684;
 constexpr double kInvLn10 = 0.434294481903251827651128918916605;
