@@ -41,6 +41,7 @@ struct qss_mech {
     int variant = 0;          // 0: general slab kernel (workspace in global memory); 1: slab-smem kernel (qss_kernel_v1.cu)
     QssJit *jit = nullptr;    // variant 1 with the Jacobian sweep's pass A specialised for this mechanism at run time (qss_jit.cpp)
     QssJit *jit3 = nullptr;   // variant 3 (qss_kernel_v3.cu, generated per mechanism): the Jacobian kernel
+    QssJit *jit3w = nullptr;  //   and its wdot-only build
     double *dP3 = nullptr;    // variant 3: parameter blobs of the reaction-per-lane phases
     int32_t *iP3 = nullptr;
 };
@@ -119,6 +120,7 @@ extern "C" int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech
     if (m->c.v3_ok && want3) {
         std::string jerr;
         m->jit3 = qss_jit3_create(m->c.v3.gen, true, prop.major, prop.minor, jerr);
+        if (m->jit3) m->jit3w = qss_jit3_create(m->c.v3.gen, false, prop.major, prop.minor, jerr);
         if (m->jit3) {
             const QssV3Host &h = m->c.v3;
             if ((e = cudaMalloc(&m->dP3, h.dP.size() * sizeof(double))) == cudaSuccess) e = cudaMalloc(&m->iP3, h.iP.size() * sizeof(int32_t));
@@ -210,6 +212,7 @@ extern "C" int qss_mech_destroy(qss_mech_t *m) {
     cudaDeviceSynchronize();          // no kernel of this handle may still run when its module is unloaded
     qss_jit_destroy(m->jit);
     qss_jit_destroy(m->jit3);
+    qss_jit_destroy(m->jit3w);
     cudaFree(m->dP3); cudaFree(m->iP3);
     if (m->copy_stream) cudaStreamDestroy(m->copy_stream);
     if (m->ev[0]) cudaEventDestroy(m->ev[0]);
@@ -235,7 +238,7 @@ extern "C" int qss_mech_info(const qss_mech_t *m, qss_mech_info_t *o) {
     o->bytes_wdot = m->c.bytes_wdot; o->bytes_jac = m->c.bytes_jac;
     o->workspace_bytes_wdot = ws_bytes(m, false);
     o->workspace_bytes_jac = ws_bytes(m, true);
-    o->kernel_variant_wdot = m->variant; o->kernel_variant_jac = m->jit3 ? 3 : (m->jit ? 2 : m->variant);
+    o->kernel_variant_wdot = m->jit3w ? 3 : m->variant; o->kernel_variant_jac = m->jit3 ? 3 : (m->jit ? 2 : m->variant);
     return QSS_OK;
 }
 
@@ -251,7 +254,12 @@ extern "C" int qss_eval_wdot(const qss_mech_t *m, int64_t ncells, int64_t ld, co
     if (rc != QSS_OK || ncells == 0) return rc;
     DeviceGuard guard(m->device);          // the handle's tables and kernels live on its device; `stream` must belong to it
     cudaError_t e;
-    if (m->variant == 1) {
+    if (m->jit3w) {
+        QssV3 v;
+        v.C = C; v.T = T; v.wdot = wdot; v.cqss = cqss; v.jac = nullptr; v.scratch = (double *)workspace;
+        v.ncells = ncells; v.ld = ld; v.scratch_stride = 0; v.dP = m->dP3; v.iP = m->iP3; v.timing = nullptr; v.mode = 0;
+        e = qss_jit3_launch(m->jit3w, v, m->n_sm, m->c.v3.nw, (size_t)m->c.v3.smem_bytes, (cudaStream_t)stream);
+    } else if (m->variant == 1) {
         QssV1 v = m->c.v1;
         v.C = C; v.T = T; v.wdot = wdot; v.cqss = cqss; v.jac = nullptr; v.scratch = (double *)workspace; v.timing = nullptr;
         v.ncells = ncells; v.ld = ld; v.scratch_stride = (int64_t)qss_v1_scratch_doubles(v);
