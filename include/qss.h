@@ -32,10 +32,18 @@
  * coefficient, third-body concentration > 0 for fall-off reactions.  NaN/Inf propagate.
  * There is no CPU fallback: without a CUDA device qss_mech_create fails with QSS_E_CUDA.
  *
- * Run-time specialisation: for mechanisms that fit the slab-smem kernel, qss_mech_create also generates CUDA source
- * for this mechanism's Jacobian columns, closure gather and closure solve and compiles it with NVRTC (libnvrtc.so.12,
- * opened with dlopen; seconds per mechanism and process).  Optional: without NVRTC the table-driven kernel computes the
- * same thing (qss_mech_info.kernel_variant_jac tells which one runs; environment QSS_JIT=0 / 2).
+ * Run-time specialisation: for mechanisms of up to 60 species, qss_mech_create generates
+ * CUDA source for this mechanism (every size a compile-time constant; closure and Jacobian columns as straight-line code)
+ * and compiles it with NVRTC (libnvrtc.so.12, opened with dlopen; seconds per mechanism, then read from an on-disk cache of
+ * device images: $QSS_CACHE_DIR, else $XDG_CACHE_HOME/libqss, else ~/.cache/libqss; QSS_CACHE=0 switches it off).
+ * Optional: without NVRTC the table-driven kernels compute the same thing (qss_mech_info.kernel_variant_jac tells which
+ * one runs).  Environment read at qss_mech_create by the release build: QSS_VARIANT=0..3 (force a variant, fail when it does
+ * not apply), QSS_JIT=0 (no run-time compilation) / 2 (failed compilation is an error), QSS_CACHE, QSS_CACHE_DIR,
+ * QSS_CS_GLOBAL (test knob of variant 1).  Nothing is read on the launch path.
+ *
+ * Threads: a handle may be used from several host threads; the device calls only enqueue work on the caller's stream (the
+ * caller orders kernels that share a workspace); qss_eval_jac_host serialises on a mutex of the handle.  qss_mech_destroy
+ * synchronises the device before it frees the tables, so work still in flight on any stream finishes first.
  */
 #ifndef QSS_H
 #define QSS_H
@@ -94,8 +102,9 @@ typedef struct {
      * independent of ncells */
     size_t  workspace_bytes_wdot, workspace_bytes_jac;
     /* which kernel the library selected: 0 general slab kernel, 1 slab-smem kernel (table
-     * interpreter), 2 slab-smem kernel with the Jacobian sweep specialised for this mechanism at qss_mech_create
-     * (NVRTC; takes seconds per mechanism and process, cached by source; falls back to 1 when NVRTC is missing) */
+     * interpreter), 2 slab-smem kernel with the Jacobian sweep specialised for this mechanism at qss_mech_create,
+     * 3 the kernel generated for this mechanism as a whole, rate phases with lane = reaction (NVRTC; images cached
+     * on disk; 2 and 3 fall back to 1 when NVRTC is missing) */
     int32_t kernel_variant_wdot, kernel_variant_jac;
 } qss_mech_info_t;
 
@@ -153,8 +162,9 @@ int qss_eval_energy(const qss_mech_t *mech, int64_t ncells, int64_t ld, const do
 /* Host-buffer convenience used for end-to-end timing: copies C and T to the device (in `dev_scratch`, which
  * must hold qss_host_scratch_bytes() bytes), evaluates, copies the Jacobian (and wdot if not NULL) back to
  * the HOST buffers, and synchronises `stream`.  Host buffers should be pinned for full copy bandwidth.  Large batches are
- * pipelined in chunks of cells: kernels run on `stream`, the copies back run on a stream owned by the handle (created on
- * first use, released by qss_mech_destroy), so this call is not capturable in a CUDA graph and not re-entrant per handle. */
+ * pipelined in chunks of cells: kernels run on `stream`, the copies back run on a stream owned by the handle (created by
+ * qss_mech_create, released by qss_mech_destroy), so this call is not capturable in a CUDA graph; concurrent calls on one
+ * handle are serialised by a mutex of the handle.  On an error both streams are synchronised before the call returns. */
 size_t qss_host_scratch_bytes(const qss_mech_t *mech, int64_t ncells, int64_t ld);
 int qss_eval_jac_host(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *C_host,
                       const double *T_host, double *jac_host, double *wdot_host_or_null,
