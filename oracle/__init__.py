@@ -39,6 +39,8 @@ def lib():
         _lib.oracle_closure_check.restype = ct.c_int
         _lib.oracle_closure_check.argtypes = [ct.c_void_p, ct.c_void_p, ct.c_double] + [ct.c_void_p] * 3
         _lib.oracle_max_threads.restype = ct.c_int
+        _lib.oracle_newton_solve.restype = ct.c_int
+        _lib.oracle_newton_solve.argtypes = [ct.c_int, ct.c_int64, ct.c_int64] + [ct.c_void_p] * 6 + [ct.c_int]
     return _lib
 
 
@@ -98,6 +100,25 @@ def evaluate_energy(om: OracleMech, C: np.ndarray, T: np.ndarray, n_cells: int |
     rc = lib().oracle_eval_energy(om._ptr(), n_cells, ld, _p(C), _p(T), _p(out["tdot"]), _p(out["erow"]), _p(out["escale"]), mode, nthreads)
     if rc != 0:
         raise RuntimeError(f"oracle_eval_energy failed rc={rc}")
+    return out
+
+
+def newton_solve(jac: np.ndarray, erow, gamma: np.ndarray, b: np.ndarray, n_cells: int | None = None, *, quad=False):
+    """NEXT-2: x = (I - gamma J)^-1 b per cell by Gaussian elimination with partial pivoting (qss_newton_oracle.cpp).
+    jac [N, N+1, ld], erow [N+1, ld] or None (then the N x N species block), gamma [ld], b [n, ld].
+    Returns dict(x [n, ld], info [ld])."""
+    N, ld = jac.shape[0], jac.shape[2]
+    n = N + 1 if erow is not None else N
+    assert jac.shape == (N, N + 1, ld) and b.shape == (n, ld) and gamma.shape == (ld,)
+    for a in (jac, gamma, b) + ((erow,) if erow is not None else ()):
+        assert a.dtype == np.float64 and a.flags.c_contiguous
+    assert erow is None or erow.shape == (N + 1, ld)
+    n_cells = ld if n_cells is None else n_cells
+    out = dict(x=np.zeros((n, ld)), info=np.zeros(ld, dtype=np.int32))
+    rc = lib().oracle_newton_solve(N, n_cells, ld, _p(jac), _p(erow) if erow is not None else None, _p(gamma), _p(b), _p(out["x"]),
+                                   _p(out["info"]), 1 if quad else 0)
+    if rc != 0:
+        raise RuntimeError(f"oracle_newton_solve failed rc={rc}")
     return out
 
 

@@ -56,6 +56,13 @@ int oracle_eval(const oracle_mech_t *m, int64_t ncells, int64_t ld, const double
 int oracle_eval_energy(const oracle_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T,
                        double *tdot, double *erow, double *escale, int mode, int nthreads);
 
+/* NEXT-2 (reading G20): x_c = (I - gamma_c J_c)^-1 b_c by Gaussian elimination with partial
+ * pivoting, J_c the (N+1) x (N+1) Jacobian (rows 0..N-1 jac, row N erow), or its N x N species block when erow == NULL.
+ * gamma [ncells], b and x [n*ld], info NULL or [ncells] (0, or k+1: zero pivot at step k).  quad != 0: __float128 arithmetic.
+ * (qss_newton_oracle.cpp) */
+int oracle_newton_solve(int N, int64_t ncells, int64_t ld, const double *jac, const double *erow, const double *gamma,
+                        const double *b, double *x, int32_t *info, int quad);
+
 /* One cell: effective forward / reverse rate constants (k including the third-body or fall-off factor,
  * kb = k / Kc; 0 for a disabled direction). kf, kb: [n_reac]. */
 int oracle_rate_constants(const oracle_mech_t *m, const double *C, double T, double *kf, double *kb);

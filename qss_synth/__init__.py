@@ -10,9 +10,11 @@ The paper's real mechanisms (13-4-CH4, 35-18 n-dodecane, 55-33 n-heptane; PAPER.
 from .mechanism import Mechanism, make_mechanism, CONFIGS, config_mechanism
 from .states import make_states, make_field_states, config_states
 from .toys import toy1, toy2, toy3, toy_dag, toy_nonqss
+from .newton import newton_inputs, newton_inputs_torch
 
 __all__ = [
     "Mechanism", "make_mechanism", "CONFIGS", "config_mechanism",
     "make_states", "make_field_states", "config_states",
     "toy1", "toy2", "toy3", "toy_dag", "toy_nonqss",
+    "newton_inputs", "newton_inputs_torch",
 ]

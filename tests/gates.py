@@ -100,3 +100,51 @@ def assert_jac(J, J_ref, J_scale, n_cells=None, what="jac", cfg=None):
         assert g[f"{k}_tier1_frac"] >= TIER1_MIN_FRACTION, f"{what}: {k} tier-1 fraction {g[f'{k}_tier1_frac']:.5f} ({g})"
         assert g[f"{k}_tier2_all"], f"{what}: {k} tier-2 violated, worst {g[f'{k}_tier2_worst']:.3g} ({g})"
     return g
+
+
+# ---- NEXT-2: the Newton solve x = (I - gamma J)^-1 b (reading G20) ------------------------------------
+# Gaussian elimination with partial pivoting is backward stable: the computed x solves (A + dA) x = b with
+# ||dA|| <= c n eps rho ||A|| (rho: growth factor, O(1) in practice).  Two implementations with different pivot choices
+# on near-ties and different rounding orders therefore agree to  ~ cond(A) * (eta_1 + eta_2), not to a fixed number of digits.
+NEWTON_ETA_MAX = 1e-13          # normwise backward error of EVERY cell (a property that holds at any size and any conditioning)
+NEWTON_RTOL = 1e-9              # forward agreement with the oracle on the well-conditioned cells (north_star's normwise 1e-9)
+NEWTON_COND_MAX = 1e4           # ... cond_inf(A) <= 1e4: 1e4 * 2e-13 << 1e-9
+NEWTON_WELLCOND_FLOOR = 0.5     # ... which must be at least half of the cells of a case (else the case tests nothing)
+
+
+def newton_matrix(jac, erow, gamma, cells):
+    """A [len(cells), n, n] = I - gamma J for the listed cells (numpy, from the SoA arrays)."""
+    N = jac.shape[0]
+    n = N + 1 if erow is not None else N
+    J = np.zeros((len(cells), n, n))
+    J[:, :N, :] = np.moveaxis(jac[:, :n, cells], 2, 0)
+    if erow is not None:
+        J[:, N, :] = erow[:, cells].T
+    return np.eye(n)[None] - gamma[cells][:, None, None] * J
+
+
+def newton_gates(A, b, x, x_ref=None):
+    """A [m, n, n], b, x, x_ref [m, n] (cells first).  Backward error per cell in extended precision; forward error against
+    x_ref on the cells with cond_inf(A) <= NEWTON_COND_MAX, and bounded by 4 cond eta_max on every cell."""
+    Al, xl, bl = A.astype(np.longdouble), x.astype(np.longdouble), b.astype(np.longdouble)
+    r = np.einsum("cij,cj->ci", Al, xl) - bl
+    normA = np.abs(A).sum(2).max(1)
+    eta = (np.abs(r).max(1) / (normA * np.abs(x).max(1) + np.abs(b).max(1))).astype(np.float64)
+    out = dict(finite=bool(np.isfinite(x).all()), eta_worst=float(eta.max()) if eta.size else 0.0,
+               eta_all=bool((eta <= NEWTON_ETA_MAX).all()))
+    if x_ref is not None:
+        cond = np.array([np.linalg.cond(a, np.inf) for a in A]) if len(A) else np.zeros(0)
+        err = np.abs(x - x_ref).max(1) / np.abs(x_ref).max(1)
+        well = cond <= NEWTON_COND_MAX
+        out.update(wellcond_frac=float(well.mean()) if well.size else 1.0,
+                   fwd_worst_wellcond=float(err[well].max()) if well.any() else 0.0,
+                   fwd_all_wellcond=bool((err[well] <= NEWTON_RTOL).all()),
+                   fwd_bound_all=bool((err <= np.maximum(4.0 * cond * NEWTON_ETA_MAX, NEWTON_RTOL * 1e-3)).all()),
+                   fwd_worst_over_bound=float((err / np.maximum(4.0 * cond * NEWTON_ETA_MAX, NEWTON_RTOL * 1e-3)).max()) if err.size else 0.0)
+    return out
+
+
+def assert_newton(g, floor=NEWTON_WELLCOND_FLOOR):
+    assert g["finite"] and g["eta_all"], g
+    if "fwd_all_wellcond" in g:
+        assert g["wellcond_frac"] >= floor and g["fwd_all_wellcond"] and g["fwd_bound_all"], g
