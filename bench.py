@@ -36,7 +36,9 @@ EXPECTED_JAC_VARIANT = {1: 3, 2: 3, 4: 3, 3: 0, 5: 0}   # the kernel each BASELI
 CALLS = {"jac+wdot": "qss_eval_jac with the wdot output (the metric)", "jac": "qss_eval_jac alone", "wdot": "qss_eval_wdot alone",
          "jac+wdot+energy": "qss_eval_jac with wdot, then qss_eval_energy: the full (N+1)x(N+1) Jacobian and the temperature right-hand side",
          "energy": "qss_eval_energy alone (on a Jacobian computed before the timed region)",
-         "jac_const": "qss_eval_jac_approx, constant-QSS AJ", "jac_zero": "qss_eval_jac_approx, zero-QSS AJ"}
+         "jac_const": "qss_eval_jac_approx, constant-QSS AJ", "jac_zero": "qss_eval_jac_approx, zero-QSS AJ",
+         "newton": "qss_newton_solve alone: x = (I - gamma J)^-1 (wdot, Tdot) on a full Jacobian computed before the timed region",
+         "jac+wdot+energy+newton": "qss_eval_jac with wdot, qss_eval_energy, qss_newton_solve: one Newton direction of an implicit step"}
 
 
 def _peaks():
@@ -205,15 +207,34 @@ def main():
         raise SystemExit(f"bench.py: cfg{cfg} ran on kernel variant {qm.info.kernel_variant_jac}, expected {expect} (run-time compilation unavailable?); "
                          "--allow-fallback times it anyway")
     tdot = torch.empty((ld,), dtype=torch.float64, device=dev); erow = torch.empty((N + 1, ld), dtype=torch.float64, device=dev)
-    if args.call == "energy":
+    B = X = gam = None
+    if "newton" in args.call:        # wdot and Tdot are written straight into the right-hand side (no copies in a step)
+        B = torch.empty((N + 1, ld), dtype=torch.float64, device=dev)
+        W = B[:N]; tdot = B[N]
+    if args.call in ("energy", "newton", "jac+wdot+energy+newton"):
         qm.eval_jac(Cd, Td, n, jac=J, wdot=W, want_wdot=True)
-    launches_per_step = 2 if args.call == "jac+wdot+energy" else 1
+    if "newton" in args.call:
+        # right-hand side (wdot, Tdot); gamma_c = theta_c / max|J_c|, theta log-uniform in [1e-2, 1e3] (seeded): from "explicit would do" to stiff
+        qm.eval_energy(Cd, Td, W, J, n, tdot=tdot, erow=erow)
+        X = torch.empty_like(B)
+        jmax = torch.maximum(J.abs().amax((0, 1)), erow.abs().amax(0))
+        g = torch.Generator(device=dev); g.manual_seed(7)
+        gam = torch.exp(np.log(10.0) * (torch.rand(ld, dtype=torch.float64, device=dev, generator=g) * 5.0 - 2.0)) / torch.where(jmax > 0, jmax, torch.ones_like(jmax))
+        del jmax
+        qm.newton_solve(J, erow, gam, B, n, x=X)        # (first call: run-time compilation, outside the timed region)
+        torch.cuda.synchronize()
+        assert bool(torch.isfinite(X[:, :n]).all())
+    launches_per_step = {"jac+wdot+energy": 2, "jac+wdot+energy+newton": 3}.get(args.call, 1)
 
     def step():
-        if args.call in ("jac+wdot", "jac+wdot+energy"):
+        if args.call in ("jac+wdot", "jac+wdot+energy", "jac+wdot+energy+newton"):
             qm.eval_jac(Cd, Td, n, jac=J, wdot=W, want_wdot=True)
-            if args.call == "jac+wdot+energy":
+            if args.call != "jac+wdot":
                 qm.eval_energy(Cd, Td, W, J, n, tdot=tdot, erow=erow)
+            if args.call == "jac+wdot+energy+newton":
+                qm.newton_solve(J, erow, gam, B, n, x=X)
+        elif args.call == "newton":
+            qm.newton_solve(J, erow, gam, B, n, x=X)
         elif args.call == "jac":
             qm.eval_jac(Cd, Td, n, jac=J)
         elif args.call == "energy":
@@ -288,6 +309,9 @@ def main():
         bytes_cell, slots_cell = info.bytes_wdot, info.slots_wdot
     elif args.call == "energy":        # reads C, T, wdot and J once, writes the row and tdot; 2 N (N+1) + ~30 N fp64 slots
         bytes_cell, slots_cell = 8.0 * (N * (N + 1) + 2 * N + 1) + 8.0 * (N + 2), 2.0 * N * (N + 1) + 30.0 * N
+    elif args.call == "newton":        # reads the (N+1)^2 matrix, b and gamma once, writes x; n^3/3 + n^2 fp64 FMA slots (elimination + substitutions)
+        nn = N + 1
+        bytes_cell, slots_cell = 8.0 * (nn * nn + 2 * nn + 1), nn ** 3 / 3.0 + nn * nn
     else:
         bytes_cell, slots_cell = info.bytes_jac + (8.0 * N if args.call.startswith("jac+wdot") else 0.0), info.slots_jac
     bytes_launch = bytes_cell * n
@@ -308,7 +332,7 @@ def main():
     except Exception:
         traffic = None
     roof.update({"traffic": traffic, "traffic_unit": "bytes per launch (dram read + write) from the committed ncu capture of this workload and kernel variant (profiles/r02_traffic.txt); not measurable inside this run",
-                 "kernel": "qss_energy_kernel" if args.call == "energy" else ("qss wdot kernel (qss_eval_wdot)" if args.call == "wdot" else f"qss jacobian kernel, variant {info.kernel_variant_jac} ({CALLS[args.call]})"),
+                 "kernel": "qss_energy_kernel" if args.call == "energy" else "qss_newton_kernel" if args.call == "newton" else ("qss wdot kernel (qss_eval_wdot)" if args.call == "wdot" else f"qss jacobian kernel, variant {info.kernel_variant_jac} ({CALLS[args.call]})"),
                  "launch_ms_avg": avg_s * 1e3, "launch_ms_min": min(launch_ms),
                  "alg_fp64_slots_per_cell": slots_cell, "alg_bytes_per_cell": bytes_cell,
                  "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3,

@@ -159,6 +159,22 @@ int qss_eval_jac_approx(const qss_mech_t *mech, int64_t ncells, int64_t ld, cons
 int qss_eval_energy(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *C, const double *T, const double *wdot,
                     const double *jac, double *tdot, double *erow, void *stream);
 
+/* NEXT-2: the dense direct solve of the Newton system that consumes the Jacobian (Eq. 7:
+ * "forming and inverting the chemical Jacobian ... to advance the Newton step"; L397: the MAGMA batched dense direct solve of
+ * Case 3).  The paper does not write the matrix; reading G20: the Newton matrix of an implicit multistep method,
+ *   x_c = (I - gamma_c J_c)^-1 b_c        per cell c, by Gaussian elimination with partial pivoting,
+ * J_c the (N+1) x (N+1) Jacobian of Eq. 7: rows 0..N-1 = jac (output of qss_eval_jac), row N = erow (output of qss_eval_energy).
+ * With erow == NULL the system is the N x N species block (columns 0..N-1 of jac; temperature frozen).  n = N + 1 or N.
+ * DEVICE pointers, 8-byte aligned, SoA cell innermost: jac [N*(N+1)*ld], erow [(N+1)*ld], gamma [ncells] (= h_c * beta: every
+ * cell has its own step size), b and x [n*ld]; x may alias b.  Nothing else is written.  A singular matrix gives non-finite x
+ * (no error).  One kernel on `stream`, no workspace; the matrix is read once from HBM.  n <= 40 (QSS_E_UNSUPPORTED above: the matrix
+ * is held in the registers of one warp).  The kernel is compiled for n with NVRTC on the FIRST call per handle and shape (seconds,
+ * or milliseconds from the on-disk cache; that first call must not be inside a stream capture; QSS_E_CUDA without NVRTC).
+ * qss_newton_specialise_check compiles the kernel for a compute capability without a device (build check). */
+int qss_newton_solve(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *jac, const double *erow_or_null,
+                     const double *gamma, const double *b, double *x, void *stream);
+int qss_newton_specialise_check(int n_species, int with_energy, int cc_major, int cc_minor, size_t *image_bytes_or_null);
+
 /* Host-buffer convenience used for end-to-end timing: copies C and T to the device (in `dev_scratch`, which
  * must hold qss_host_scratch_bytes() bytes), evaluates, copies the Jacobian (and wdot if not NULL) back to
  * the HOST buffers, and synchronises `stream`.  Host buffers should be pinned for full copy bandwidth.  Large batches are

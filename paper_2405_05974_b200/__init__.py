@@ -17,7 +17,7 @@ from . import build as _build
 __all__ = ["lib", "QssMech", "QssError", "EXPORTS", "STATUS"]
 
 EXPORTS = ["qss_mech_create", "qss_mech_validate", "qss_mech_specialise_check", "qss_mech_destroy", "qss_mech_info", "qss_mech_qss_order", "qss_eval_wdot",
-           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
+           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_newton_solve", "qss_newton_specialise_check", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
 STATUS = {0: "QSS_OK", -1: "QSS_E_INVALID", -2: "QSS_E_QUADRATIC", -3: "QSS_E_QSS_FANOUT", -4: "QSS_E_NO_SINK",
           -5: "QSS_E_UNSUPPORTED", -6: "QSS_E_CUDA", -7: "QSS_E_UNBALANCED"}
 
@@ -70,6 +70,8 @@ def lib():
         L.qss_eval_jac.restype = ct.c_int; L.qss_eval_jac.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, ct.c_size_t, vp]
         L.qss_eval_jac_approx.restype = ct.c_int; L.qss_eval_jac_approx.argtypes = [vp, i64, i64, vp, vp, vp, ct.c_int, vp, ct.c_size_t, vp]
         L.qss_eval_energy.restype = ct.c_int; L.qss_eval_energy.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp]
+        L.qss_newton_solve.restype = ct.c_int; L.qss_newton_solve.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp]
+        L.qss_newton_specialise_check.restype = ct.c_int; L.qss_newton_specialise_check.argtypes = [ct.c_int, ct.c_int, ct.c_int, ct.c_int, vp]
         L.qss_host_scratch_bytes.restype = ct.c_size_t; L.qss_host_scratch_bytes.argtypes = [vp, i64, i64]
         L.qss_eval_jac_host.restype = ct.c_int; L.qss_eval_jac_host.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, ct.c_size_t, vp]
         L.qss_bench_dfma.restype = ct.c_int; L.qss_bench_dfma.argtypes = [ct.c_int, ct.c_int, vp, ct.POINTER(ct.c_double), vp]
@@ -123,6 +125,14 @@ def specialise_check(mech, cc=(10, 0)) -> int:
     nbytes = ct.c_size_t()
     _check(lib().qss_mech_specialise_check(ct.addressof(d), int(cc[0]), int(cc[1]), ct.addressof(nbytes)))
     del keep
+    return nbytes.value
+
+
+def newton_specialise_check(n_species: int, with_energy: bool = True, cc=(10, 0)) -> int:
+    """Host-only: compile the Newton-solve kernel for a mechanism of `n_species` transported species with NVRTC (no device
+    needed). Returns the size of the device image in bytes."""
+    nbytes = ct.c_size_t()
+    _check(lib().qss_newton_specialise_check(int(n_species), 1 if with_energy else 0, int(cc[0]), int(cc[1]), ct.addressof(nbytes)))
     return nbytes.value
 
 
@@ -234,6 +244,19 @@ class QssMech:
             erow = torch.empty((self.N + 1, ld), dtype=torch.float64, device=C.device)
         _check(lib().qss_eval_energy(self._h, ncells, ld, _ptr(C), _ptr(T), _ptr(wdot), _ptr(jac), _ptr(tdot), _ptr(erow), self._stream()))
         return tdot, erow
+
+    def newton_solve(self, jac, erow, gamma, b, ncells=None, x=None):
+        """x = (I - gamma J)^-1 b per cell (qss_newton_solve); J = [jac; erow], or the N x N species block when erow is None."""
+        import torch
+        ld = jac.shape[2]
+        ncells = ld if ncells is None else int(ncells)
+        n = self.N + (1 if erow is not None else 0)
+        assert jac.is_contiguous() and jac.shape == (self.N, self.N + 1, ld) and b.is_contiguous() and b.shape == (n, ld)
+        assert gamma.is_contiguous() and gamma.numel() >= ncells and (erow is None or (erow.is_contiguous() and erow.shape == (self.N + 1, ld)))
+        if x is None:
+            x = torch.empty((n, ld), dtype=torch.float64, device=jac.device)
+        _check(lib().qss_newton_solve(self._h, ncells, ld, _ptr(jac), _ptr(erow), _ptr(gamma), _ptr(b), _ptr(x), self._stream()))
+        return x
 
     def host_scratch_bytes(self, ncells, ld):
         return int(lib().qss_host_scratch_bytes(self._h, int(ncells), int(ld)))

@@ -44,6 +44,9 @@ struct qss_mech {
     QssJit *jit3w = nullptr;  //   and its wdot-only build
     double *dP3 = nullptr;    // variant 3: parameter blobs of the reaction-per-lane phases
     int32_t *iP3 = nullptr;
+    int cc_major = 0, cc_minor = 0;
+    mutable int newton_blocks[2] = {0, 0};            //   persistent blocks of that kernel (SMs x resident blocks per SM)
+    mutable QssJit *newton[2] = {nullptr, nullptr};   // qss_newton_solve: [0] species block (n = N), [1] with the energy row (n = N + 1); built on first use
 };
 
 namespace {
@@ -101,6 +104,7 @@ extern "C" int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech
     cudaDeviceProp prop;
     if ((e = cudaGetDeviceProperties(&prop, device)) != cudaSuccess) { delete m; return cuda_fail(e, "cudaGetDeviceProperties"); }
     m->n_sm = prop.multiProcessorCount;
+    m->cc_major = prop.major; m->cc_minor = prop.minor;
     if (const char *bps = qss_devenv("QSS_V0_BLOCKS_PER_SM")) m->blocks_per_sm = std::max(1, std::atoi(bps));   // tuning aid for the general kernel
     m->nblocks = m->n_sm * m->blocks_per_sm;
     const size_t nI = m->c.I.size() ? m->c.I.size() : 1, nD = m->c.D.size() ? m->c.D.size() : 1;
@@ -213,6 +217,8 @@ extern "C" int qss_mech_destroy(qss_mech_t *m) {
     qss_jit_destroy(m->jit);
     qss_jit_destroy(m->jit3);
     qss_jit_destroy(m->jit3w);
+    qss_jit_destroy(m->newton[0]);
+    qss_jit_destroy(m->newton[1]);
     cudaFree(m->dP3); cudaFree(m->iP3);
     if (m->copy_stream) cudaStreamDestroy(m->copy_stream);
     if (m->ev[0]) cudaEventDestroy(m->ev[0]);
@@ -269,6 +275,46 @@ extern "C" int qss_eval_wdot(const qss_mech_t *m, int64_t ncells, int64_t ld, co
                             (cudaStream_t)stream);
     }
     return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_eval_wdot launch");
+}
+
+// ---- NEXT-2: the Newton solve (qss_newton_kernel.cu, compiled for this mechanism's matrix order on first use) ------------------
+static const int QSS_NEWTON_MAX_N = 40;     // two register rows of n + 1 doubles per lane: 164 registers at n = 40
+static int newton_cpb() {                  // cells (= warps) per block
+    if (const char *e = qss_devenv("QSS_NEWTON_CPB")) return std::atoi(e);      // (development builds)
+    return 8;                                // 64-byte segments per matrix entry; one block of 8 warps per SM (234 registers)
+}
+#define QSS_NEWTON_CPB newton_cpb()
+
+extern "C" int qss_newton_specialise_check(int n_species, int with_energy, int cc_major, int cc_minor, size_t *image_bytes) {
+    const int n = n_species + (with_energy ? 1 : 0);
+    if (n_species < 1 || n > QSS_NEWTON_MAX_N) return fail(QSS_E_UNSUPPORTED, "qss_newton_solve: matrix order outside 1..40");
+    std::string err;
+    if (!qss_jit_newton_compile_only(n, n_species + 1, with_energy != 0, QSS_NEWTON_CPB, cc_major, cc_minor, image_bytes, err)) return fail(QSS_E_CUDA, err);
+    return QSS_OK;
+}
+
+extern "C" int qss_newton_solve(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *jac, const double *erow, const double *gamma,
+                                const double *b, double *x, void *stream) {
+    if (!m) return fail(QSS_E_INVALID, "mech is NULL");
+    if (ncells < 0 || ld < ncells) return fail(QSS_E_INVALID, "need 0 <= ncells <= ld");
+    const int N = m->c.tab.N, n = N + (erow ? 1 : 0);
+    if (n > QSS_NEWTON_MAX_N) return fail(QSS_E_UNSUPPORTED, "qss_newton_solve: matrix order above 40 (the matrix does not fit a warp's registers)");
+    if (ncells == 0) return QSS_OK;
+    if (!jac || !gamma || !b || !x) return fail(QSS_E_INVALID, "NULL device pointer");
+    if (((uintptr_t)jac | (uintptr_t)erow | (uintptr_t)gamma | (uintptr_t)b | (uintptr_t)x) & 7) return fail(QSS_E_INVALID, "device pointers must be 8-byte aligned");
+    DeviceGuard guard(m->device);
+    const int which = erow ? 1 : 0;
+    {
+        std::lock_guard<std::mutex> lock(m->host_mu);
+        if (!m->newton[which]) {
+            std::string err;
+            m->newton[which] = qss_jit_newton_create(n, N + 1, erow != nullptr, QSS_NEWTON_CPB, m->cc_major, m->cc_minor, err);
+            if (!m->newton[which]) return fail(QSS_E_CUDA, "qss_newton_solve: run-time compilation failed (there is no other path): " + err);
+            m->newton_blocks[which] = m->n_sm * qss_jit_newton_blocks_per_sm(m->newton[which], n, QSS_NEWTON_CPB);
+        }
+    }
+    cudaError_t e = qss_jit_newton_launch(m->newton[which], n, QSS_NEWTON_CPB, m->newton_blocks[which], jac, erow, gamma, b, x, ncells, ld, (cudaStream_t)stream);
+    return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_newton_solve launch");
 }
 
 static int eval_jac_mode(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T, double *jac, double *wdot, int mode,

@@ -243,6 +243,54 @@ cudaError_t qss_jit_launch(const QssJit *j, const QssV1 &v, int nblocks, cudaStr
     return cudaLaunchKernel(reinterpret_cast<const void *>(j->kernel), dim3(grid), dim3(v.nw * 32), args, (size_t)v.smem_rows * 256, stream);
 }
 
+// ---- Newton solve ------------------------------------------------------------------------------------------------------
+namespace {
+std::string newton_gen(int n, int nj, bool has_e, int cpb) {
+    char buf[256];
+    int minb = 1;
+    if (const char *e = qss_devenv("QSS_NEWTON_MINB")) minb = std::atoi(e);      // (development builds: register limit experiments)
+    std::snprintf(buf, sizeof buf, "#define LU_N %d\n#define LU_NJ %d\n#define LU_HAS_E %d\n#define LU_CPB %d\n#define LU_MINB %d\n", n, nj, has_e ? 1 : 0, cpb, minb);
+    return buf;
+}
+struct QssNewtonArgs {          // = struct QssNewton of qss_newton_kernel.cu
+    const double *jac, *erow, *gamma, *b;
+    double *x;
+    int64_t ncells, ld;
+};
+}  // namespace
+
+bool qss_jit_newton_compile_only(int n, int nj, bool has_e, int cpb, int cc_major, int cc_minor, size_t *image_bytes, std::string &err) {
+    std::shared_ptr<std::vector<char>> bin = compile("qss_newton_kernel.cu", "qss_newton_gen.h", newton_gen(n, nj, has_e, cpb), {}, arch_of(cc_major, cc_minor), err);
+    if (bin && image_bytes) *image_bytes = bin->size();
+    return (bool)bin;
+}
+
+QssJit *qss_jit_newton_create(int n, int nj, bool has_e, int cpb, int cc_major, int cc_minor, std::string &err) {
+    std::shared_ptr<std::vector<char>> bin = compile("qss_newton_kernel.cu", "qss_newton_gen.h", newton_gen(n, nj, has_e, cpb), {}, arch_of(cc_major, cc_minor), err);
+    return bin ? load_image(*bin, "qss_newton_kernel", err) : nullptr;
+}
+
+size_t qss_jit_newton_smem(int n, int cpb) {
+    const size_t nc = (size_t)n + 1, pitch = nc | 1, ub = (nc + 4) & ~(size_t)1;
+    return ((size_t)2 * cpb * n * pitch + (size_t)cpb * 2 * ub + (size_t)cpb * n) * sizeof(double) + (size_t)cpb * n * sizeof(int);
+}
+
+int qss_jit_newton_blocks_per_sm(const QssJit *j, int n, int cpb) {
+    int nb = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, reinterpret_cast<const void *>(j->kernel), 32 * cpb, qss_jit_newton_smem(n, cpb)) != cudaSuccess) { cudaGetLastError(); nb = 1; }
+    return nb < 1 ? 1 : nb;
+}
+
+cudaError_t qss_jit_newton_launch(const QssJit *j, int n, int cpb, int max_blocks, const double *jac, const double *erow, const double *gamma,
+                                  const double *b, double *x, int64_t ncells, int64_t ld, cudaStream_t stream) {
+    if (ncells == 0) return cudaSuccess;
+    QssNewtonArgs a = {jac, erow, gamma, b, x, ncells, ld};
+    void *args[] = {&a};
+    const int64_t ntiles = (ncells + cpb - 1) / cpb;
+    const int64_t grid = ntiles < max_blocks ? ntiles : max_blocks;          // persistent blocks: tile t, t + grid, ...
+    return cudaLaunchKernel(reinterpret_cast<const void *>(j->kernel), dim3((unsigned)grid), dim3(32 * cpb), args, qss_jit_newton_smem(n, cpb), stream);
+}
+
 void qss_jit_destroy(QssJit *j) {
     if (!j) return;
     if (j->lib) cudaLibraryUnload(j->lib);

@@ -30,4 +30,13 @@ QssJit *qss_jit3_create(const std::string &gen_src, bool jac, int cc_major, int 
 bool qss_jit3_compile_only(const std::string &gen_src, bool jac, int cc_major, int cc_minor, size_t *image_bytes, std::string &err);
 cudaError_t qss_jit3_launch(const QssJit *j, const QssV3 &v, int nblocks, int nw, size_t smem_bytes, cudaStream_t stream);
 
+// Newton solve (qss_newton_kernel.cu): compiled for one matrix order n (= N + 1 with the energy row, else N), nj = N + 1 columns
+// of the Jacobian array, cpb cells (= warps) per block.  Same caches as above.
+QssJit *qss_jit_newton_create(int n, int nj, bool has_e, int cpb, int cc_major, int cc_minor, std::string &err);
+bool qss_jit_newton_compile_only(int n, int nj, bool has_e, int cpb, int cc_major, int cc_minor, size_t *image_bytes, std::string &err);
+size_t qss_jit_newton_smem(int n, int cpb);
+int qss_jit_newton_blocks_per_sm(const QssJit *j, int n, int cpb);
+cudaError_t qss_jit_newton_launch(const QssJit *j, int n, int cpb, int max_blocks, const double *jac, const double *erow, const double *gamma,
+                                  const double *b, double *x, int64_t ncells, int64_t ld, cudaStream_t stream);
+
 #endif
