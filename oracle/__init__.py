@@ -122,6 +122,38 @@ def newton_solve(jac: np.ndarray, erow, gamma: np.ndarray, b: np.ndarray, n_cell
     return out
 
 
+def bdf1_advance(om: OracleMech, C: np.ndarray, T: np.ndarray, dt: np.ndarray, nsub: int, newton_iters: int, n_cells: int | None = None,
+                 *, history=False):
+    """NEXT-4 (0D constant-volume reactor, the interval "divided into substeps over which the chemical state is
+    advanced"; L183-188: implicit scheme, Newton method with the chemical Jacobian; reading G21): `nsub` backward-Euler
+    substeps of size dt[c] per cell, each solved by `newton_iters` full Newton iterations, step by step as written:
+        phi = (C, T),  f = (wdot, Tdot);   phi_0 = phi^n
+        F(phi_m) = phi_m - phi^n - h f(phi_m);   (I - h J(phi_m)) delta = -F(phi_m);   phi_{m+1} = phi_m + delta,  C := max(C, 0)
+        phi^{n+1} = phi_{newton_iters}
+    with J the full (N+1) x (N+1) Jacobian (species block + energy row) and the linear solve of `newton_solve`.
+    Returns (C, T) after the last substep (new arrays, padding untouched); with history=True also the list of T after every substep."""
+    ld = C.shape[1]
+    n = ld if n_cells is None else n_cells
+    N = om.N
+    C = C.copy(); T = T.copy()
+    h = np.ascontiguousarray(dt, dtype=np.float64)
+    hist = []
+    for _ in range(nsub):
+        Cn, Tn = C.copy(), T.copy()
+        for _m in range(newton_iters):
+            ev = evaluate(om, C, T, n, want_jac=True)
+            en = evaluate_energy(om, C, T, n)
+            jac, erow = ev["jac"], en["erow"]
+            b = np.zeros((N + 1, ld))
+            b[:N, :n] = (Cn[:, :n] - C[:, :n]) + h[:n] * ev["wdot"][:, :n]
+            b[N, :n] = (Tn[:n] - T[:n]) + h[:n] * en["tdot"][:n]
+            x = newton_solve(np.ascontiguousarray(jac), np.ascontiguousarray(erow), h, b, n)["x"]
+            C[:, :n] = np.maximum(C[:, :n] + x[:N, :n], 0.0)
+            T[:n] = T[:n] + x[N, :n]
+        hist.append(T.copy())
+    return (C, T, hist) if history else (C, T)
+
+
 def rate_constants(om: OracleMech, C1: np.ndarray, T: float):
     C1 = np.ascontiguousarray(C1, dtype=np.float64)
     kf = np.zeros(om.M); kb = np.zeros(om.M)
