@@ -38,7 +38,8 @@ CALLS = {"jac+wdot": "qss_eval_jac with the wdot output (the metric)", "jac": "q
          "energy": "qss_eval_energy alone (on a Jacobian computed before the timed region)",
          "jac_const": "qss_eval_jac_approx, constant-QSS AJ", "jac_zero": "qss_eval_jac_approx, zero-QSS AJ",
          "newton": "qss_newton_solve alone: x = (I - gamma J)^-1 (wdot, Tdot) on a full Jacobian computed before the timed region",
-         "jac+wdot+energy+newton": "qss_eval_jac with wdot, qss_eval_energy, qss_newton_solve: one Newton direction of an implicit step"}
+         "jac+wdot+energy+newton": "qss_eval_jac with wdot, qss_eval_energy, qss_newton_solve: one Newton direction of an implicit step",
+         "bdf1": "qss_bdf1_advance: one backward-Euler substep with two full Newton iterations (10 kernel launches), state restored before every step"}
 
 
 def _peaks():
@@ -224,7 +225,21 @@ def main():
         qm.newton_solve(J, erow, gam, B, n, x=X)        # (first call: run-time compilation, outside the timed region)
         torch.cuda.synchronize()
         assert bool(torch.isfinite(X[:, :n]).all())
-    launches_per_step = {"jac+wdot+energy": 2, "jac+wdot+energy+newton": 3}.get(args.call, 1)
+    launches_per_step = {"jac+wdot+energy": 2, "jac+wdot+energy+newton": 3, "bdf1": 10}.get(args.call, 1)
+    if args.call == "bdf1":
+        # h_c = 3 / max|J_c| at the initial state (a few of the fastest time scales per substep); the state is restored before every step
+        del J
+        torch.cuda.empty_cache()
+        Jt, Wt = qm.eval_jac(Cd, Td, n, want_wdot=True)
+        td0, er0 = qm.eval_energy(Cd, Td, Wt, Jt, n)
+        jmax = torch.maximum(Jt.abs().amax((0, 1)), er0.abs().amax(0))
+        dtd = 3.0 / torch.where(jmax > 0, jmax, torch.ones_like(jmax))
+        del Jt, Wt, td0, er0, jmax
+        torch.cuda.empty_cache()
+        C0, T0 = Cd.clone(), Td.clone()
+        bdf_ws = qm.bdf1_advance(Cd, Td, dtd, 1, 2, n)
+        torch.cuda.synchronize()
+        J = None
 
     def step():
         if args.call in ("jac+wdot", "jac+wdot+energy", "jac+wdot+energy+newton"):
@@ -235,6 +250,9 @@ def main():
                 qm.newton_solve(J, erow, gam, B, n, x=X)
         elif args.call == "newton":
             qm.newton_solve(J, erow, gam, B, n, x=X)
+        elif args.call == "bdf1":
+            Cd.copy_(C0); Td.copy_(T0)
+            qm.bdf1_advance(Cd, Td, dtd, 1, 2, n, workspace=bdf_ws)
         elif args.call == "jac":
             qm.eval_jac(Cd, Td, n, jac=J)
         elif args.call == "energy":
@@ -312,6 +330,10 @@ def main():
     elif args.call == "newton":        # reads the (N+1)^2 matrix, b and gamma once, writes x; n^3/3 + n^2 fp64 FMA slots (elimination + substitutions)
         nn = N + 1
         bytes_cell, slots_cell = 8.0 * (nn * nn + 2 * nn + 1), nn ** 3 / 3.0 + nn * nn
+    elif args.call == "bdf1":          # two Newton iterations: the three heavy calls twice (the residual / update kernels move 5 (N+1) doubles each)
+        nn = N + 1
+        bytes_cell = 2.0 * ((info.bytes_jac + 8.0 * N) + (8.0 * (N * nn + 2 * N + 1) + 8.0 * (N + 2)) + 8.0 * (nn * nn + 2 * nn + 1) + 8.0 * 9 * nn)
+        slots_cell = 2.0 * (info.slots_jac + 2.0 * N * nn + 30.0 * N + nn ** 3 / 3.0 + nn * nn)
     else:
         bytes_cell, slots_cell = info.bytes_jac + (8.0 * N if args.call.startswith("jac+wdot") else 0.0), info.slots_jac
     bytes_launch = bytes_cell * n
@@ -332,7 +354,7 @@ def main():
     except Exception:
         traffic = None
     roof.update({"traffic": traffic, "traffic_unit": "bytes per launch (dram read + write) from the committed ncu capture of this workload and kernel variant (profiles/r02_traffic.txt); not measurable inside this run",
-                 "kernel": "qss_energy_kernel" if args.call == "energy" else "qss_newton_kernel" if args.call == "newton" else ("qss wdot kernel (qss_eval_wdot)" if args.call == "wdot" else f"qss jacobian kernel, variant {info.kernel_variant_jac} ({CALLS[args.call]})"),
+                 "kernel": "qss_energy_kernel" if args.call == "energy" else "qss_newton_kernel" if args.call == "newton" else "the 10 launches of one substep (jacobian, energy row, residual, solve, update; twice)" if args.call == "bdf1" else ("qss wdot kernel (qss_eval_wdot)" if args.call == "wdot" else f"qss jacobian kernel, variant {info.kernel_variant_jac} ({CALLS[args.call]})"),
                  "launch_ms_avg": avg_s * 1e3, "launch_ms_min": min(launch_ms),
                  "alg_fp64_slots_per_cell": slots_cell, "alg_bytes_per_cell": bytes_cell,
                  "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3,

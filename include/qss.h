@@ -175,6 +175,22 @@ int qss_newton_solve(const qss_mech_t *mech, int64_t ncells, int64_t ld, const d
                      const double *gamma, const double *b, double *x, void *stream);
 int qss_newton_specialise_check(int n_species, int with_energy, int cc_major, int cc_minor, size_t *image_bytes_or_null);
 
+/* NEXT-4 (first half): 0-D constant-volume integrator, the paper's validation workload (the
+ * interval "divided into substeps over which the chemical state is advanced ... to mimic timestepping in a fluid simulation";
+ * L183-188: implicit scheme, Newton method with the chemical Jacobian).  The paper integrates with CVODE (variable order, variable
+ * step), which it does not specify; reading G21: `nsub` backward-Euler substeps of size dt[c] PER CELL, each solved by
+ * `newton_iters` full Newton iterations with the exact (N+1) x (N+1) Jacobian re-evaluated in every iteration:
+ *     phi = (C, T), f = (wdot, Tdot);  F(phi_m) = phi_m - phi^n - h f(phi_m);  (I - h J(phi_m)) delta = -F(phi_m);
+ *     phi_{m+1} = phi_m + delta, C := max(C, 0)
+ * No step-size control and no convergence test: the launch sequence is fixed (5 kernels per Newton iteration: qss_eval_jac,
+ * qss_eval_energy, residual, qss_newton_solve, update; 2 copies per substep), nothing synchronises, and the call can be captured
+ * in a CUDA graph after one warm-up call (run-time compilation of the solve).  C [N*ld] and T [ld] are updated IN PLACE (DEVICE
+ * pointers, 16-byte aligned, ld even); dt [ncells]; `workspace`: qss_bdf1_workspace_bytes(mech, ld) bytes of device memory, 256-byte
+ * aligned (holds the Jacobian: 8 N (N+1) ld bytes).  N + 1 <= 40 (limit of qss_newton_solve). */
+size_t qss_bdf1_workspace_bytes(const qss_mech_t *mech, int64_t ld);
+int qss_bdf1_advance(const qss_mech_t *mech, int64_t ncells, int64_t ld, double *C, double *T, const double *dt, int nsub,
+                     int newton_iters, void *workspace, size_t workspace_bytes, void *stream);
+
 /* Host-buffer convenience used for end-to-end timing: copies C and T to the device (in `dev_scratch`, which
  * must hold qss_host_scratch_bytes() bytes), evaluates, copies the Jacobian (and wdot if not NULL) back to
  * the HOST buffers, and synchronises `stream`.  Host buffers should be pinned for full copy bandwidth.  Large batches are

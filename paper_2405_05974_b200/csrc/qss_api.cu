@@ -371,6 +371,57 @@ static int eval_jac_mode(const qss_mech_t *m, int64_t ncells, int64_t ld, const 
 
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
+
+// ---- NEXT-4: 0-D constant-volume integrator (backward-Euler substeps, full Newton iterations; qss_driver.cu) --------------------
+cudaError_t qss_launch_bdf1_residual(int N, int64_t ncells, int64_t ld, const double *C, const double *T, const double *phin, const double *F,
+                                     const double *dt, double *b, cudaStream_t stream);
+cudaError_t qss_launch_bdf1_update(int N, int64_t ncells, int64_t ld, double *C, double *T, const double *x, cudaStream_t stream);
+
+extern "C" size_t qss_bdf1_workspace_bytes(const qss_mech_t *m, int64_t ld) {
+    if (!m || ld < 0) return 0;
+    const size_t N = (size_t)m->c.tab.N, row = align256((size_t)ld * sizeof(double));
+    // jac N (N+1) rows | F N+1 | erow N+1 | phi^n N+1 | b (and x in place) N+1 | workspace of qss_eval_jac
+    return row * (N * (N + 1) + 4 * (N + 1)) + align256(ws_bytes(m, true)) + 256;
+}
+
+extern "C" int qss_bdf1_advance(const qss_mech_t *m, int64_t ncells, int64_t ld, double *C, double *T, const double *dt, int nsub, int newton_iters,
+                                void *workspace, size_t workspace_bytes, void *stream) {
+    if (!m) return fail(QSS_E_INVALID, "mech is NULL");
+    if (ncells < 0 || ld < ncells || nsub < 0 || newton_iters < 1) return fail(QSS_E_INVALID, "need 0 <= ncells <= ld, nsub >= 0, newton_iters >= 1");
+    const int N = m->c.tab.N;
+    if (N + 1 > QSS_NEWTON_MAX_N) return fail(QSS_E_UNSUPPORTED, "qss_bdf1_advance: more than 39 transported species (limit of qss_newton_solve)");
+    if (ncells == 0 || nsub == 0) return QSS_OK;
+    if (!C || !T || !dt) return fail(QSS_E_INVALID, "NULL device pointer");
+    if (ld & 1) return fail(QSS_E_INVALID, "qss_bdf1_advance: ld must be even (16-byte aligned rows)");
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < qss_bdf1_workspace_bytes(m, ld)) return fail(QSS_E_INVALID, "workspace is NULL, misaligned or smaller than qss_bdf1_workspace_bytes");
+    DeviceGuard guard(m->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    // the rows of one array are contiguous with stride ld (the layout every call of the library uses)
+    const size_t nrow = (size_t)ld;
+    char *p = (char *)workspace;
+    auto take = [&](size_t rows) { double *q = (double *)p; p += align256(rows * nrow * sizeof(double)); return q; };
+    double *jac = take((size_t)N * (N + 1)), *F = take(N + 1), *erow = take(N + 1), *phin = take(N + 1), *b = take(N + 1);
+    void *ws = (void *)(((uintptr_t)p + 255) & ~(uintptr_t)255);
+    const size_t wsb = ws_bytes(m, true);
+    for (int s = 0; s < nsub; ++s) {
+        cudaError_t e = cudaMemcpyAsync(phin, C, (size_t)N * nrow * sizeof(double), cudaMemcpyDeviceToDevice, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(phin + (size_t)N * nrow, T, nrow * sizeof(double), cudaMemcpyDeviceToDevice, st);
+        if (e != cudaSuccess) return cuda_fail(e, "qss_bdf1_advance: saving the state");
+        for (int it = 0; it < newton_iters; ++it) {
+            int rc = eval_jac_mode(m, ncells, ld, C, T, jac, F, 0, ws, wsb, stream);                       // J species block, wdot -> F[0..N-1]
+            if (rc == QSS_OK) rc = qss_eval_energy(m, ncells, ld, C, T, F, jac, F + (size_t)N * nrow, erow, stream);   // Tdot -> F[N], energy row
+            if (rc != QSS_OK) return rc;
+            e = qss_launch_bdf1_residual(N, ncells, ld, C, T, phin, F, dt, b, st);
+            if (e != cudaSuccess) return cuda_fail(e, "qss_bdf1_advance: residual kernel");
+            rc = qss_newton_solve(m, ncells, ld, jac, erow, dt, b, b, stream);                             // gamma = h: (I - h J) delta = b, in place
+            if (rc != QSS_OK) return rc;
+            e = qss_launch_bdf1_update(N, ncells, ld, C, T, b, st);
+            if (e != cudaSuccess) return cuda_fail(e, "qss_bdf1_advance: update kernel");
+        }
+    }
+    return QSS_OK;
+}
+
 extern "C" size_t qss_host_scratch_bytes(const qss_mech_t *m, int64_t ncells, int64_t ld) {
     if (!m || ncells < 0 || ld < ncells) return 0;
     const size_t N = m->c.tab.N, L = (size_t)ld * sizeof(double);

@@ -1,0 +1,51 @@
+// NEXT-4 (first half): the element-wise kernels of the 0-D constant-volume integrator qss_bdf1_advance
+// (the interval "divided into substeps over which the chemical state is advanced"; L183-188: implicit scheme, Newton
+// method with the chemical Jacobian; reading G21).  The heavy steps of a Newton iteration are the library's own calls
+// (qss_eval_jac, qss_eval_energy, qss_newton_solve); what is left is the residual and the update of the state phi = (C, T):
+//     b     = (phi^n - phi_m) + h f(phi_m)           f = (wdot, Tdot), rows 0..N-1 and N of `F`
+//     phi_{m+1} = phi_m + delta,   C := max(C, 0)
+// SoA, cell innermost: every access is a coalesced row; thread = (row, cell).
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace {
+
+__global__ void __launch_bounds__(256) qss_bdf1_residual_kernel(int N, int64_t ncells, int64_t ld, const double *__restrict__ C, const double *__restrict__ T,
+                                                                 const double *__restrict__ phin, const double *__restrict__ F,
+                                                                 const double *__restrict__ dt, double *__restrict__ b) {
+    const int64_t c = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (c >= ncells) return;
+    const double h = dt[c];
+    for (int i = blockIdx.y; i <= N; i += gridDim.y) {
+        const double phi = i < N ? C[(size_t)i * ld + c] : T[c];
+        b[(size_t)i * ld + c] = (phin[(size_t)i * ld + c] - phi) + h * F[(size_t)i * ld + c];
+    }
+}
+
+__global__ void __launch_bounds__(256) qss_bdf1_update_kernel(int N, int64_t ncells, int64_t ld, double *__restrict__ C, double *__restrict__ T,
+                                                               const double *__restrict__ x) {
+    const int64_t c = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (c >= ncells) return;
+    for (int i = blockIdx.y; i <= N; i += gridDim.y) {
+        const double d = x[(size_t)i * ld + c];
+        if (i < N) C[(size_t)i * ld + c] = fmax(C[(size_t)i * ld + c] + d, 0.0);
+        else T[c] = T[c] + d;
+    }
+}
+
+}  // namespace
+
+cudaError_t qss_launch_bdf1_residual(int N, int64_t ncells, int64_t ld, const double *C, const double *T, const double *phin, const double *F,
+                                     const double *dt, double *b, cudaStream_t stream) {
+    if (ncells == 0) return cudaSuccess;
+    const dim3 grid((unsigned)((ncells + 255) / 256), (unsigned)(N + 1 < 8 ? N + 1 : 8));
+    qss_bdf1_residual_kernel<<<grid, 256, 0, stream>>>(N, ncells, ld, C, T, phin, F, dt, b);
+    return cudaGetLastError();
+}
+
+cudaError_t qss_launch_bdf1_update(int N, int64_t ncells, int64_t ld, double *C, double *T, const double *x, cudaStream_t stream) {
+    if (ncells == 0) return cudaSuccess;
+    const dim3 grid((unsigned)((ncells + 255) / 256), (unsigned)(N + 1 < 8 ? N + 1 : 8));
+    qss_bdf1_update_kernel<<<grid, 256, 0, stream>>>(N, ncells, ld, C, T, x);
+    return cudaGetLastError();
+}
