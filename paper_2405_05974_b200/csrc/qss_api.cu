@@ -356,7 +356,9 @@ static int eval_jac_mode(const qss_mech_t *m, int64_t ncells, int64_t ld, const 
         v.C = C; v.T = T; v.wdot = wdot; v.cqss = nullptr; v.jac = jac; v.scratch = (double *)workspace;
         v.ncells = ncells; v.ld = ld; v.scratch_stride = (int64_t)m->c.v3.scratch_rows * 32;
         v.dP = m->dP3; v.iP = m->iP3; v.timing = m->timing; v.mode = mode;
-        e = qss_jit3_launch(m->jit3, v, m->n_sm, m->c.v3.nw, (size_t)m->c.v3.smem_bytes, (cudaStream_t)stream);
+        int nb3 = m->n_sm;
+        if (const char *bx = qss_devenv("QSS3_BLOCKS")) nb3 = std::max(1, std::min(m->n_sm, std::atoi(bx)));      // (development builds: fewer SMs)
+        e = qss_jit3_launch(m->jit3, v, nb3, m->c.v3.nw, (size_t)m->c.v3.smem_bytes, (cudaStream_t)stream);
     } else if (m->variant == 1) {
         QssV1 v = m->c.v1;
         v.C = C; v.T = T; v.wdot = wdot; v.cqss = nullptr; v.jac = jac; v.scratch = (double *)workspace; v.timing = m->timing;

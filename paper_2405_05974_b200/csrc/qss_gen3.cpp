@@ -362,6 +362,87 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
         }
         G("    default: break;\n    }\n}\n");
     }
+    // ---- P2c and P6 as straight-line code (one part per warp): kappa_d = k_d prod C, and the species sums.  MEASURED AND NOT USED
+    //      (development builds, QSS3_EXP bits 8 / 16): the table loops spend 4-6x as many instructions on the same work, but the
+    //      7.6 k instructions of once-per-slab code arrive at ~4.5 bytes per clock and SM: 12.2 / 12.7 ms against 11.5 ms.
+    int exp_bits = 0;
+    if (const char *e = qss_devenv("QSS3_EXP")) exp_bits = std::atoi(e);
+    if (exp_bits & 24) {
+    {
+        std::vector<std::vector<int>> fac(2 * MS);                      // V rows of the transported reactant molecules per direction row
+        std::vector<int> kqe(2 * MS, -1);
+        for (int j = 0; j < M; ++j) for (int dir = 0; dir < 2; ++dir) {
+            const int e = erow(2 * j + dir);
+            for (int sp2 : slots[2 * j + dir]) if (vrow(sp2) != R_ONE) fac[e].push_back(vrow(sp2));
+            kqe[e] = kq_row[2 * j + dir];
+        }
+        std::vector<double> cost(2 * MS);
+        for (int e = 0; e < 2 * MS; ++e) cost[e] = 4.0 + 2.0 * fac[e].size() + (kqe[e] >= 0 ? 1.0 : 0.0);
+        // contiguous ranges of rows per warp (neighbouring rows: the same shared-memory banks pattern as the table loop)
+        double total = 0.0; for (double x : cost) total += x;
+        G("__device__ __forceinline__ void qss_gen_kappa(const int warp, const unsigned sml, double *sc) {\n    switch (warp) {\n");
+        int e = 0; double acc = 0.0;
+        for (int w = 0; w < NW; ++w) {
+            G("    case %d:\n", w);
+            const double upto = total * (w + 1) / NW;
+            while (e < 2 * MS && (acc + 0.5 * cost[e] <= upto || w == NW - 1)) {
+                G("        { const double k = lS<%d>(sml); const double kp = k", (R_KAP + e) * PITCH);
+                for (int r : fac[e]) G(" * lS<%d>(sml)", r * PITCH);
+                G("; sS<%d>(sml, kp);", (R_KAP + e) * PITCH);
+                G("\n#if QSS3_JAC\n          sc[%d] = k;", (S_K + e) * 32);
+                if (kqe[e] >= 0) G(" sc[%d] = kp;", (S_KQ + kqe[e]) * 32);
+                G("\n#endif\n        }\n");
+                acc += cost[e]; ++e;
+            }
+            G("        break;\n");
+        }
+        G("    default: break;\n    }\n}\n");
+    }
+    {
+        std::vector<std::vector<int>> sp(nsp), sm(nsp), tp(nsp), tm(nsp);
+        for (int j = 0; j < M; ++j) if (R[j].mask) for (const Term &x : R[j].net) for (int u = 0; u < std::abs(x.nu); ++u) {
+            (x.nu > 0 ? sp : sm)[x.sp].push_back((R_KAP + pos[j]) * PITCH);
+            if (R[j].tb >= 0) (x.nu > 0 ? tp : tm)[x.sp].push_back((R_DLM + R[j].tb) * PITCH);
+        }
+        std::vector<double> cost(nsp);
+        for (int s2 = 0; s2 < nsp; ++s2) cost[s2] = 6.0 + 2.0 * (sp[s2].size() + sm[s2].size()) + (tp[s2].size() + tm[s2].size());
+        const std::vector<int> bin = lpt(cost, NW);
+        // a signed sum with four partial sums: name = (sum of plus rows + off) - (sum of minus rows + off)
+        auto emit_sum = [&](const char *name, const std::vector<int> &plus, const std::vector<int> &minus, int off) {
+            for (int sign = 0; sign < 2; ++sign) {
+                const std::vector<int> &l = sign ? minus : plus;
+                const char *pre = sign ? "m" : "p";
+                const int na = (int)std::min<size_t>(4, l.size());
+                for (int a = 0; a < na; ++a) G("            double %s%s%d = lS<%d>(sml);\n", name, pre, a, l[a] + off);
+                for (size_t t = 4; t < l.size(); ++t) G("            %s%s%d += lS<%d>(sml);\n", name, pre, (int)(t % 4), l[t] + off);
+                G("            const double %s%s = ", name, pre);
+                if (na == 0) G("0.0");
+                else if (na == 1) G("%s%s0", name, pre);
+                else if (na == 2) G("%s%s0 + %s%s1", name, pre, name, pre);
+                else if (na == 3) G("(%s%s0 + %s%s1) + %s%s2", name, pre, name, pre, name, pre);
+                else G("(%s%s0 + %s%s1) + (%s%s2 + %s%s3)", name, pre, name, pre, name, pre, name, pre);
+                G(";\n");
+            }
+            G("            const double %s = %sp - %sm;\n", name, name, name);
+        };
+        G("__device__ __forceinline__ void qss_gen_sums(const int warp, const unsigned sml, double *sc, double *wdot, const long long ld, const bool active) {\n    switch (warp) {\n");
+        for (int w = 0; w < NW; ++w) {
+            G("    case %d:\n", w);
+            for (int s2 = 0; s2 < nsp; ++s2) if (bin[s2] == w) {
+                G("        {\n");
+                emit_sum("w", sp[s2], sm[s2], 0);
+                if (s2 < N) G("            if (wdot && active) wdot[%d * ld] = w;\n", s2);
+                G("#if QSS3_JAC\n");
+                emit_sum("et", sp[s2], sm[s2], MS * PITCH);
+                emit_sum("tv", tp[s2], tm[s2], 0);
+                G("            sS<%d>(sml, tv); sc[%d] = et;\n", (R_TV + s2) * PITCH, (S_ET + s2) * 32);
+                G("#endif\n        }\n");
+            }
+            G("        break;\n");
+        }
+        G("    default: break;\n    }\n}\n");
+    }
+    }
     // ---- P4: closure solve of every group with its matrix in registers (subtraction-free elimination, Eq. 6
     //      L150-157, L159-171; readings G2, G8), level by level of the condensed DAG; also prepares U = P / D for dy/dx
     {

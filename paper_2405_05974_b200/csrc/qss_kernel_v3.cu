@@ -398,6 +398,9 @@ qss_v3_wdot(const __grid_constant__ QssV3 p) {
         // ---- P2c: kappa_d = k_d times the transported reactant molecules (Eq. 6), in place, four directions per step; k_d
         //      itself leaves for the scratch slab (the column records read it), kappa_d of the QSS-consuming directions too
         //      (their rows are reused for Q_j).  Table word: V rows of the three molecules (6 bits each) | (kq row + 1) << 18.
+#if QSS3_X & 8
+        qss_gen_kappa(warp, sml, sc);
+#else
         for (int e = warp * 4; e < 2 * G_MS; e += G_NW * 4) {
             const int4 wa = tab4(sm0, T_KAP + e);
             const int w[4] = {wa.x, wa.y, wa.z, wa.w};
@@ -417,6 +420,7 @@ qss_v3_wdot(const __grid_constant__ QssV3 p) {
 #endif
             }
         }
+#endif
         __syncthreads();
         QSS_TICK(10);
         NetParams np;        // (the first net-rate task's parameters: fetched under the closure phases)
@@ -450,6 +454,9 @@ qss_v3_wdot(const __grid_constant__ QssV3 p) {
 #pragma unroll
         for (int u = 0; u < G_KQ_PER_WARP; ++u) kq[u] = ldg_pin(sc + (size_t)(S_KQ + min(warp * G_KQ_PER_WARP + u, G_NKQ - 1)) * 32);
 #endif
+#if QSS3_X & 16
+        qss_gen_sums(warp, sml, sc, p.wdot ? p.wdot + cell : nullptr, ld, active);
+#else
         for (int u = tab(sm0, T_SSW_PTR + warp); u < tab(sm0, T_SSW_PTR + warp + 1); ++u) {
             const int s = tab(sm0, T_SSW + u);
             double w, et, tv, unused;
@@ -461,6 +468,7 @@ qss_v3_wdot(const __grid_constant__ QssV3 p) {
             sc[(size_t)(S_ET + s) * 32] = et;
 #endif
         }
+#endif
         if (p.cqss && active)
             for (int q = warp; q < G_NQ; q += G_NW) p.cqss[(size_t)q * ld + cell] = lds(sml + (R_Y + q) * G_PITCH);
 #if QSS3_JAC
@@ -501,7 +509,11 @@ qss_v3_wdot(const __grid_constant__ QssV3 p) {
 #else
         for (int dd = 0; dd < QSS_GEN_DEPTH; ++dd) {
             const int k = qss_gen_cols[warp * QSS_GEN_DEPTH + dd];
+#if QSS3_X & 32      // (timing experiment, WRONG results: every column of a warp runs the code of the warp's first column -> a third of the once-per-slab code)
+            if (k >= 0) qss_gen_column(qss_gen_cols[warp * QSS_GEN_DEPTH], p.mode, sml, sm0 + lane * 16, sc, p.jac + (size_t)(unsigned)k * (size_t)ld + cell, (long long)(G_N + 1) * ld, active);
+#else
             if (k >= 0) qss_gen_column(k, p.mode, sml, sm0 + lane * 16, sc, p.jac + (size_t)(unsigned)k * (size_t)ld + cell, (long long)(G_N + 1) * ld, active);
+#endif
         }
 #endif
         QSS_TICK(8);
