@@ -245,13 +245,19 @@ cudaError_t qss_jit_launch(const QssJit *j, const QssV1 &v, int nblocks, cudaStr
 
 // ---- Newton solve ------------------------------------------------------------------------------------------------------
 namespace {
+bool newton_packed() {          // the mapping of qss_newton_kernel.cu: rows of 8 cells packed over a block (1) or one warp per cell (0)
+    if (const char *e = qss_devenv("QSS_NEWTON_PACKED")) return std::atoi(e) != 0;      // (development builds: measured 14.7 against 14.1 ms)
+    return false;
+}
 std::string newton_gen(int n, int nj, bool has_e, int cpb) {
-    char buf[256];
-    int minb = 1;
+    char buf[320];
+    int minb = newton_packed() ? 2 : 1;
     if (const char *e = qss_devenv("QSS_NEWTON_MINB")) minb = std::atoi(e);      // (development builds: register limit experiments)
-    std::snprintf(buf, sizeof buf, "#define LU_N %d\n#define LU_NJ %d\n#define LU_HAS_E %d\n#define LU_CPB %d\n#define LU_MINB %d\n", n, nj, has_e ? 1 : 0, cpb, minb);
+    std::snprintf(buf, sizeof buf, "#define LU_N %d\n#define LU_NJ %d\n#define LU_HAS_E %d\n#define LU_CPB %d\n#define LU_MINB %d\n#define LU_PACKED %d\n",
+                  n, nj, has_e ? 1 : 0, cpb, minb, newton_packed() ? 1 : 0);
     return buf;
 }
+int newton_threads(int n, int cpb) { return newton_packed() ? (cpb * n + 31) / 32 * 32 : 32 * cpb; }
 struct QssNewtonArgs {          // = struct QssNewton of qss_newton_kernel.cu
     const double *jac, *erow, *gamma, *b;
     double *x;
@@ -272,12 +278,13 @@ QssJit *qss_jit_newton_create(int n, int nj, bool has_e, int cpb, int cc_major, 
 
 size_t qss_jit_newton_smem(int n, int cpb) {
     const size_t nc = (size_t)n + 1, pitch = nc | 1, ub = (nc + 4) & ~(size_t)1;
+    if (newton_packed()) return ((size_t)cpb * n * pitch + (size_t)cpb * ((nc + 5) & ~(size_t)1) + (size_t)cpb * n) * sizeof(double) + (size_t)2 * cpb * sizeof(unsigned);
     return ((size_t)2 * cpb * n * pitch + (size_t)cpb * 2 * ub + (size_t)cpb * n) * sizeof(double) + (size_t)cpb * n * sizeof(int);
 }
 
 int qss_jit_newton_blocks_per_sm(const QssJit *j, int n, int cpb) {
     int nb = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, reinterpret_cast<const void *>(j->kernel), 32 * cpb, qss_jit_newton_smem(n, cpb)) != cudaSuccess) { cudaGetLastError(); nb = 1; }
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, reinterpret_cast<const void *>(j->kernel), newton_threads(n, cpb), qss_jit_newton_smem(n, cpb)) != cudaSuccess) { cudaGetLastError(); nb = 1; }
     return nb < 1 ? 1 : nb;
 }
 
@@ -288,7 +295,7 @@ cudaError_t qss_jit_newton_launch(const QssJit *j, int n, int cpb, int max_block
     void *args[] = {&a};
     const int64_t ntiles = (ncells + cpb - 1) / cpb;
     const int64_t grid = ntiles < max_blocks ? ntiles : max_blocks;          // persistent blocks: tile t, t + grid, ...
-    return cudaLaunchKernel(reinterpret_cast<const void *>(j->kernel), dim3((unsigned)grid), dim3(32 * cpb), args, qss_jit_newton_smem(n, cpb), stream);
+    return cudaLaunchKernel(reinterpret_cast<const void *>(j->kernel), dim3((unsigned)grid), dim3(newton_threads(n, cpb)), args, qss_jit_newton_smem(n, cpb), stream);
 }
 
 void qss_jit_destroy(QssJit *j) {
