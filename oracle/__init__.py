@@ -122,6 +122,25 @@ def newton_solve(jac: np.ndarray, erow, gamma: np.ndarray, b: np.ndarray, n_cell
     return out
 
 
+def evaluate_fdT(om: OracleMech, C: np.ndarray, T: np.ndarray, n_cells: int | None = None):
+    """NEXT-3, the paper's own temperature column (d wdot / dT "via finite difference by computing the species'
+    production rate twice at different temperatures"; L234: central differences, perturbation 1e-4; reading G22):
+        dT = 1e-4 T,  T+ = T + dT,  T- = T - dT,   J[:, N] = (wdot(C, T+) - wdot(C, T-)) / (T+ - T-)
+    (the perturbation is taken relative to T; the divisor is the difference of the rounded temperatures).  The species columns are the
+    explicit ones.  Returns the dict of `evaluate` with that column replaced."""
+    ld = C.shape[1]
+    n = ld if n_cells is None else n_cells
+    out = evaluate(om, C, T, n, want_jac=True, want_scale=True)
+    dT = 1e-4 * T
+    Tp = T + dT
+    Tm = T - dT
+    wp = evaluate(om, C, np.ascontiguousarray(Tp), n, want_jac=False)["wdot"]
+    wm = evaluate(om, C, np.ascontiguousarray(Tm), n, want_jac=False)["wdot"]
+    out["jac"][:, om.N, :n] = (wp[:, :n] - wm[:, :n]) / (Tp[:n] - Tm[:n])
+    out["wdot_p"], out["wdot_m"], out["Tp"], out["Tm"] = wp, wm, Tp, Tm
+    return out
+
+
 def bdf1_advance(om: OracleMech, C: np.ndarray, T: np.ndarray, dt: np.ndarray, nsub: int, newton_iters: int, n_cells: int | None = None,
                  *, history=False):
     """NEXT-4 (0D constant-volume reactor, the interval "divided into substeps over which the chemical state is

@@ -160,3 +160,23 @@ def test_simplified_jacobians_coincide_with_the_exact_one_where_they_must():
 
     print("Eq.-10 error on cfg1: constant-QSS %.3g, zero-QSS %.3g; worst column %.3g / %.3g" % (eps(cq), eps(zq), worst_col(cq), worst_col(zq)))
     assert worst_col(cq) > 1e-2 and worst_col(zq) > 1e-2 and not np.allclose(cq, zq)
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_finite_difference_temperature_column_against_the_analytic_one(cfg):
+    """NEXT-3 (reading G22): the central difference with dT = 1e-4 T has a truncation error of
+    (dT^2 / 6) w''' -- about 1e-8..1e-6 of the column -- and really is a difference (not the analytic column copied)."""
+    m = config_mechanism(cfg); n = 64
+    om = oracle.OracleMech(m)
+    C, T = config_states(cfg, n)
+    fd = oracle.evaluate_fdT(om, C, T, n); ex = oracle.evaluate(om, C, T, n, want_scale=True)
+    N = m.n_nqss
+    assert np.array_equal(fd["jac"][:, :N, :n], ex["jac"][:, :N, :n])
+    a, b, s = fd["jac"][:, N, :n], ex["jac"][:, N, :n], ex["jscale"][:, N, :n]
+    well = s <= 1e3 * np.abs(b)
+    rel = np.abs(a - b)[well] / np.abs(b)[well]
+    print("cfg%d FD-in-T column vs analytic: median %.2e, 99th percentile %.2e, well-conditioned %.2f" % (cfg, np.median(rel), np.quantile(rel, 0.99), well.mean()))
+    assert well.mean() > 0.5 and np.median(rel) < 1e-6 and np.quantile(rel, 0.9) < 1e-4
+    assert np.median(rel) > 1e-13                                        # a finite difference, not the analytic column
+    # the perturbed temperatures are symmetric to rounding and the divisor is their exact difference
+    assert np.allclose((fd["Tp"][:n] - fd["Tm"][:n]) / T[:n], 2e-4, rtol=1e-10)
