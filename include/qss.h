@@ -175,6 +175,17 @@ int qss_newton_solve(const qss_mech_t *mech, int64_t ncells, int64_t ld, const d
                      const double *gamma, const double *b, double *x, void *stream);
 int qss_newton_specialise_check(int n_species, int with_energy, int cc_major, int cc_minor, size_t *image_bytes_or_null);
 
+/* NEXT-3: the paper's own treatment of the temperature column (d wdot / dT "via finite difference by computing the
+ * species' production rate twice at different temperatures"; L234: central differences, perturbation 1e-4; reading G22).
+ * Same outputs as qss_eval_jac, except that column N of jac is
+ *     (wdot(C, T+) - wdot(C, T-)) / (T+ - T-),     dT = 1e-4 T,  T+ = T + dT,  T- = T - dT   (every operation rounded on its own)
+ * instead of the analytic derivative (which this library computes by default, reading G6).  Four launches of the library's kernels
+ * (Jacobian, two wdot evaluations, two element-wise kernels) on `stream`.  workspace: qss_jac_fdt_workspace_bytes(mech, ld) bytes of
+ * device memory, 256-byte aligned; ld even.  A comparison mode: slower and less accurate than the analytic column. */
+size_t qss_jac_fdt_workspace_bytes(const qss_mech_t *mech, int64_t ld);
+int qss_eval_jac_fdt(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *C, const double *T, double *jac,
+                     double *wdot_or_null, void *workspace, size_t workspace_bytes, void *stream);
+
 /* NEXT-4 (first half): 0-D constant-volume integrator, the paper's validation workload (the
  * interval "divided into substeps over which the chemical state is advanced ... to mimic timestepping in a fluid simulation";
  * L183-188: implicit scheme, Newton method with the chemical Jacobian).  The paper integrates with CVODE (variable order, variable

@@ -17,7 +17,7 @@ from . import build as _build
 __all__ = ["lib", "QssMech", "QssError", "EXPORTS", "STATUS"]
 
 EXPORTS = ["qss_mech_create", "qss_mech_validate", "qss_mech_specialise_check", "qss_mech_destroy", "qss_mech_info", "qss_mech_qss_order", "qss_eval_wdot",
-           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_newton_solve", "qss_newton_specialise_check", "qss_bdf1_workspace_bytes", "qss_bdf1_advance", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
+           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_newton_solve", "qss_newton_specialise_check", "qss_bdf1_workspace_bytes", "qss_bdf1_advance", "qss_jac_fdt_workspace_bytes", "qss_eval_jac_fdt", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
 STATUS = {0: "QSS_OK", -1: "QSS_E_INVALID", -2: "QSS_E_QUADRATIC", -3: "QSS_E_QSS_FANOUT", -4: "QSS_E_NO_SINK",
           -5: "QSS_E_UNSUPPORTED", -6: "QSS_E_CUDA", -7: "QSS_E_UNBALANCED"}
 
@@ -71,6 +71,8 @@ def lib():
         L.qss_eval_jac_approx.restype = ct.c_int; L.qss_eval_jac_approx.argtypes = [vp, i64, i64, vp, vp, vp, ct.c_int, vp, ct.c_size_t, vp]
         L.qss_eval_energy.restype = ct.c_int; L.qss_eval_energy.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp]
         L.qss_newton_solve.restype = ct.c_int; L.qss_newton_solve.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp]
+        L.qss_jac_fdt_workspace_bytes.restype = ct.c_size_t; L.qss_jac_fdt_workspace_bytes.argtypes = [vp, i64]
+        L.qss_eval_jac_fdt.restype = ct.c_int; L.qss_eval_jac_fdt.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, ct.c_size_t, vp]
         L.qss_bdf1_workspace_bytes.restype = ct.c_size_t; L.qss_bdf1_workspace_bytes.argtypes = [vp, i64]
         L.qss_bdf1_advance.restype = ct.c_int; L.qss_bdf1_advance.argtypes = [vp, i64, i64, vp, vp, vp, ct.c_int, ct.c_int, vp, ct.c_size_t, vp]
         L.qss_newton_specialise_check.restype = ct.c_int; L.qss_newton_specialise_check.argtypes = [ct.c_int, ct.c_int, ct.c_int, ct.c_int, vp]
@@ -259,6 +261,19 @@ class QssMech:
             x = torch.empty((n, ld), dtype=torch.float64, device=jac.device)
         _check(lib().qss_newton_solve(self._h, ncells, ld, _ptr(jac), _ptr(erow), _ptr(gamma), _ptr(b), _ptr(x), self._stream()))
         return x
+
+    def eval_jac_fdT(self, C, T, ncells=None, jac=None, wdot=None, want_wdot=False):
+        """Jacobian with the temperature column by central finite differences of wdot (qss_eval_jac_fdt)."""
+        import torch
+        ld = C.shape[1]
+        ncells = ld if ncells is None else int(ncells)
+        if jac is None:
+            jac = torch.empty((self.N, self.N + 1, ld), dtype=torch.float64, device=C.device)
+        if wdot is None and want_wdot:
+            wdot = torch.empty((self.N, ld), dtype=torch.float64, device=C.device)
+        ws = torch.empty(int(lib().qss_jac_fdt_workspace_bytes(self._h, ld)), dtype=torch.uint8, device=C.device)
+        _check(lib().qss_eval_jac_fdt(self._h, ncells, ld, _ptr(C), _ptr(T), _ptr(jac), _ptr(wdot), _ptr(ws), ws.numel(), self._stream()))
+        return (jac, wdot) if want_wdot else jac
 
     def bdf1_advance(self, C, T, dt, nsub, newton_iters, ncells=None, workspace=None):
         """Advances (C, T) IN PLACE by `nsub` backward-Euler substeps of size dt per cell (qss_bdf1_advance)."""

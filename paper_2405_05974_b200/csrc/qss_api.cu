@@ -374,6 +374,39 @@ static int eval_jac_mode(const qss_mech_t *m, int64_t ncells, int64_t ld, const 
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 
+// ---- NEXT-3: temperature column by finite differences (reading G22; kernels in qss_driver.cu) ---------------
+cudaError_t qss_launch_fdT_perturb(int64_t ncells, const double *T, double *Tp, double *Tm, cudaStream_t stream);
+cudaError_t qss_launch_fdT_column(int N, int64_t ncells, int64_t ld, const double *wp, const double *wm, const double *Tp, const double *Tm, double *jac,
+                                  cudaStream_t stream);
+
+extern "C" size_t qss_jac_fdt_workspace_bytes(const qss_mech_t *m, int64_t ld) {
+    if (!m || ld < 0) return 0;
+    const size_t row = align256((size_t)ld * sizeof(double));
+    return std::max(align256(ws_bytes(m, true)), align256(ws_bytes(m, false))) + row * (2 + 2 * (size_t)m->c.tab.N) + 256;
+}
+
+extern "C" int qss_eval_jac_fdt(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T, double *jac, double *wdot,
+                                void *workspace, size_t workspace_bytes, void *stream) {
+    if (!m) return fail(QSS_E_INVALID, "mech is NULL");
+    if (ld & 1) return fail(QSS_E_INVALID, "qss_eval_jac_fdt: ld must be even (16-byte aligned rows)");
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < qss_jac_fdt_workspace_bytes(m, ld)) return fail(QSS_E_INVALID, "workspace is NULL, misaligned or smaller than qss_jac_fdt_workspace_bytes");
+    const size_t wsk = std::max(align256(ws_bytes(m, true)), align256(ws_bytes(m, false)));
+    int rc = eval_jac_mode(m, ncells, ld, C, T, jac, wdot, 0, workspace, wsk, stream);          // species columns (and the analytic T column, overwritten below)
+    if (rc != QSS_OK || ncells == 0) return rc;
+    DeviceGuard guard(m->device);
+    const int N = m->c.tab.N;
+    char *p = (char *)workspace + wsk;
+    auto take = [&](size_t rows) { double *q = (double *)p; p += align256(rows * (size_t)ld * sizeof(double)); return q; };
+    double *Tp = take(1), *Tm = take(1), *wp = take(N), *wm = take(N);
+    cudaError_t e = qss_launch_fdT_perturb(ncells, T, Tp, Tm, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "qss_eval_jac_fdt: perturbation kernel");
+    rc = qss_eval_wdot(m, ncells, ld, C, Tp, wp, nullptr, workspace, wsk, stream);
+    if (rc == QSS_OK) rc = qss_eval_wdot(m, ncells, ld, C, Tm, wm, nullptr, workspace, wsk, stream);
+    if (rc != QSS_OK) return rc;
+    e = qss_launch_fdT_column(N, ncells, ld, wp, wm, Tp, Tm, jac, (cudaStream_t)stream);
+    return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_eval_jac_fdt: column kernel");
+}
+
 // ---- NEXT-4: 0-D constant-volume integrator (backward-Euler substeps, full Newton iterations; qss_driver.cu) --------------------
 cudaError_t qss_launch_bdf1_residual(int N, int64_t ncells, int64_t ld, const double *C, const double *T, const double *phin, const double *F,
                                      const double *dt, double *b, cudaStream_t stream);

@@ -49,3 +49,42 @@ cudaError_t qss_launch_bdf1_update(int N, int64_t ncells, int64_t ld, double *C,
     qss_bdf1_update_kernel<<<grid, 256, 0, stream>>>(N, ncells, ld, C, T, x);
     return cudaGetLastError();
 }
+
+// ---- NEXT-3: the temperature column by finite differences ("computing the species' production rate twice at
+// different temperatures"; L234: central differences, perturbation 1e-4; reading G22): the two element-wise steps around
+// the two qss_eval_wdot calls.  dT = 1e-4 T, T+ = T + dT, T- = T - dT (each operation rounded on its own: no contraction, so
+// that the oracle's numpy expression gives the same bits), column = (w+ - w-) / (T+ - T-).
+namespace {
+
+__global__ void __launch_bounds__(256) qss_fdT_perturb_kernel(int64_t ncells, const double *__restrict__ T, double *__restrict__ Tp, double *__restrict__ Tm) {
+    const int64_t c = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (c >= ncells) return;
+    const double t = T[c], d = __dmul_rn(1e-4, t);
+    Tp[c] = __dadd_rn(t, d);
+    Tm[c] = __dsub_rn(t, d);
+}
+
+__global__ void __launch_bounds__(256) qss_fdT_column_kernel(int N, int64_t ncells, int64_t ld, const double *__restrict__ wp, const double *__restrict__ wm,
+                                                              const double *__restrict__ Tp, const double *__restrict__ Tm, double *__restrict__ jac) {
+    const int64_t c = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (c >= ncells) return;
+    const double h = __dsub_rn(Tp[c], Tm[c]);
+    for (int i = blockIdx.y; i < N; i += gridDim.y)
+        jac[((size_t)i * (N + 1) + N) * ld + c] = __ddiv_rn(__dsub_rn(wp[(size_t)i * ld + c], wm[(size_t)i * ld + c]), h);
+}
+
+}  // namespace
+
+cudaError_t qss_launch_fdT_perturb(int64_t ncells, const double *T, double *Tp, double *Tm, cudaStream_t stream) {
+    if (ncells == 0) return cudaSuccess;
+    qss_fdT_perturb_kernel<<<(unsigned)((ncells + 255) / 256), 256, 0, stream>>>(ncells, T, Tp, Tm);
+    return cudaGetLastError();
+}
+
+cudaError_t qss_launch_fdT_column(int N, int64_t ncells, int64_t ld, const double *wp, const double *wm, const double *Tp, const double *Tm, double *jac,
+                                  cudaStream_t stream) {
+    if (ncells == 0) return cudaSuccess;
+    const dim3 grid((unsigned)((ncells + 255) / 256), (unsigned)(N < 8 ? N : 8));
+    qss_fdT_column_kernel<<<grid, 256, 0, stream>>>(N, ncells, ld, wp, wm, Tp, Tm, jac);
+    return cudaGetLastError();
+}

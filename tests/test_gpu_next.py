@@ -81,3 +81,33 @@ def test_simplified_jacobians_need_variant_3():
         qm.eval_jac_approx(torch.from_numpy(C).cuda(), torch.from_numpy(T).cuda(), 1, 64)
     assert e.value.code == -5
     qm.close()
+
+
+@pytest.mark.parametrize("name,n", [("cfg1", 1024 + 2), ("cfg2", 512 + 6), ("cfg3", 96)])
+def test_finite_difference_temperature_column(name, n):
+    """NEXT-3 (reading G22): qss_eval_jac_fdt against oracle.evaluate_fdT.  The species columns are the exact
+    kernel's (bit for bit); the T column is a difference of two wdot evaluations, so its gate is the wdot gate of both, divided
+    by the step: |d col| <= (tol(w+) + tol(w-)) / (T+ - T-), tol(w) = 1e-10 |w| + 1e-13 S."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    cfg = int(name[3])
+    mech = qss_synth.config_mechanism(cfg); C, T = qss_synth.config_states(cfg, n)
+    qm = qss.QssMech(mech, 0)
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda()
+    J, w = qm.eval_jac_fdT(Cd, Td, n, want_wdot=True)
+    Jex = qm.eval_jac(Cd, Td, n)
+    torch.cuda.synchronize()
+    J = J.cpu().numpy(); Jex = Jex.cpu().numpy()
+    N = qm.N
+    assert np.array_equal(J[:, :N, :n], Jex[:, :N, :n])
+    ref = oracle.evaluate_fdT(oracle.OracleMech(mech), C, T, n)
+    h = (ref["Tp"] - ref["Tm"])[:n]
+    S = ref["S"][:, :n]
+    bound = (1e-10 * (np.abs(ref["wdot_p"][:, :n]) + np.abs(ref["wdot_m"][:, :n])) + 2.02e-13 * S) / h
+    d = np.abs(J[:, N, :n] - ref["jac"][:, N, :n])
+    assert np.isfinite(J[:, N, :n]).all()
+    print("%s FD-in-T column: worst |d| / bound %.3g" % (name, float((d / bound).max())))
+    assert (d <= bound).all()
+    g = gates.wdot_gates(w.cpu().numpy(), ref["wdot"], ref["S"], n)
+    assert g["finite"] and g["tier2_all"]
+    qm.close()
