@@ -175,6 +175,17 @@ int qss_newton_solve(const qss_mech_t *mech, int64_t ncells, int64_t ld, const d
                      const double *gamma, const double *b, double *x, void *stream);
 int qss_newton_specialise_check(int n_species, int with_energy, int cc_major, int cc_minor, size_t *image_bytes_or_null);
 
+/* NEXT-3: sparsity (Table 4: fraction of non-zero entries of the AJ; the chain term of Eq. 9 roughly doubles it).
+ * qss_mech_jac_pattern: host only, no device: pattern[i*(N+1) + k] = 1 when entry (row i, column k; k = N: T) of the Jacobian of
+ * `mode` (qss_jac_mode) can be non-zero for some state, else 0 -- those entries are exactly 0.0 in the output of qss_eval_jac /
+ * qss_eval_jac_approx for every state.  The description is validated as in qss_mech_create.
+ * qss_jac_pack: packed[e*ld + c] = jac[idx[e]*ld + c] for e < nnz: the rows idx[e] (= i*(N+1) + k of the wanted entries; DEVICE array)
+ * of the dense SoA Jacobian gathered into nnz consecutive rows, the layout a batched sparse solver takes with the pattern as its
+ * index arrays.  DEVICE pointers, 16-byte aligned, ld even; one kernel on `stream`. */
+int qss_mech_jac_pattern(const qss_mech_desc_t *desc, int mode, uint8_t *pattern);
+int qss_jac_pack(const qss_mech_t *mech, int64_t ncells, int64_t ld, int32_t nnz, const int32_t *idx, const double *jac,
+                 double *packed, void *stream);
+
 /* NEXT-3: the paper's own treatment of the temperature column (d wdot / dT "via finite difference by computing the
  * species' production rate twice at different temperatures"; L234: central differences, perturbation 1e-4; reading G22).
  * Same outputs as qss_eval_jac, except that column N of jac is

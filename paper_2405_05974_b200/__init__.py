@@ -17,7 +17,7 @@ from . import build as _build
 __all__ = ["lib", "QssMech", "QssError", "EXPORTS", "STATUS"]
 
 EXPORTS = ["qss_mech_create", "qss_mech_validate", "qss_mech_specialise_check", "qss_mech_destroy", "qss_mech_info", "qss_mech_qss_order", "qss_eval_wdot",
-           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_newton_solve", "qss_newton_specialise_check", "qss_bdf1_workspace_bytes", "qss_bdf1_advance", "qss_jac_fdt_workspace_bytes", "qss_eval_jac_fdt", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
+           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_newton_solve", "qss_newton_specialise_check", "qss_bdf1_workspace_bytes", "qss_bdf1_advance", "qss_jac_fdt_workspace_bytes", "qss_eval_jac_fdt", "qss_mech_jac_pattern", "qss_jac_pack", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
 STATUS = {0: "QSS_OK", -1: "QSS_E_INVALID", -2: "QSS_E_QUADRATIC", -3: "QSS_E_QSS_FANOUT", -4: "QSS_E_NO_SINK",
           -5: "QSS_E_UNSUPPORTED", -6: "QSS_E_CUDA", -7: "QSS_E_UNBALANCED"}
 
@@ -71,6 +71,8 @@ def lib():
         L.qss_eval_jac_approx.restype = ct.c_int; L.qss_eval_jac_approx.argtypes = [vp, i64, i64, vp, vp, vp, ct.c_int, vp, ct.c_size_t, vp]
         L.qss_eval_energy.restype = ct.c_int; L.qss_eval_energy.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp]
         L.qss_newton_solve.restype = ct.c_int; L.qss_newton_solve.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp]
+        L.qss_mech_jac_pattern.restype = ct.c_int; L.qss_mech_jac_pattern.argtypes = [vp, ct.c_int, vp]
+        L.qss_jac_pack.restype = ct.c_int; L.qss_jac_pack.argtypes = [vp, i64, i64, ct.c_int32, vp, vp, vp, vp]
         L.qss_jac_fdt_workspace_bytes.restype = ct.c_size_t; L.qss_jac_fdt_workspace_bytes.argtypes = [vp, i64]
         L.qss_eval_jac_fdt.restype = ct.c_int; L.qss_eval_jac_fdt.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, ct.c_size_t, vp]
         L.qss_bdf1_workspace_bytes.restype = ct.c_size_t; L.qss_bdf1_workspace_bytes.argtypes = [vp, i64]
@@ -130,6 +132,16 @@ def specialise_check(mech, cc=(10, 0)) -> int:
     _check(lib().qss_mech_specialise_check(ct.addressof(d), int(cc[0]), int(cc[1]), ct.addressof(nbytes)))
     del keep
     return nbytes.value
+
+
+def jac_pattern(mech, mode: int = 0):
+    """Host-only: structural non-zero pattern [N, N+1] (uint8) of the Jacobian of `mode` (qss_mech_jac_pattern)."""
+    import numpy as np
+    d, keep = make_desc(mech)
+    pat = np.zeros((mech.n_nqss, mech.n_nqss + 1), dtype=np.uint8)
+    _check(lib().qss_mech_jac_pattern(ct.addressof(d), int(mode), pat.ctypes.data))
+    del keep
+    return pat
 
 
 def newton_specialise_check(n_species: int, with_energy: bool = True, cc=(10, 0)) -> int:
@@ -274,6 +286,17 @@ class QssMech:
         ws = torch.empty(int(lib().qss_jac_fdt_workspace_bytes(self._h, ld)), dtype=torch.uint8, device=C.device)
         _check(lib().qss_eval_jac_fdt(self._h, ncells, ld, _ptr(C), _ptr(T), _ptr(jac), _ptr(wdot), _ptr(ws), ws.numel(), self._stream()))
         return (jac, wdot) if want_wdot else jac
+
+    def jac_pack(self, jac, idx, ncells=None, packed=None):
+        """Rows idx (int32 CUDA tensor of i*(N+1)+k) of the dense Jacobian gathered into [len(idx), ld] (qss_jac_pack)."""
+        import torch
+        ld = jac.shape[2]
+        ncells = ld if ncells is None else int(ncells)
+        assert jac.is_contiguous() and idx.dtype == torch.int32 and idx.is_contiguous()
+        if packed is None:
+            packed = torch.empty((idx.numel(), ld), dtype=torch.float64, device=jac.device)
+        _check(lib().qss_jac_pack(self._h, ncells, ld, idx.numel(), _ptr(idx), _ptr(jac), _ptr(packed), self._stream()))
+        return packed
 
     def bdf1_advance(self, C, T, dt, nsub, newton_iters, ncells=None, workspace=None):
         """Advances (C, T) IN PLACE by `nsub` backward-Euler substeps of size dt per cell (qss_bdf1_advance)."""

@@ -374,6 +374,36 @@ static int eval_jac_mode(const qss_mech_t *m, int64_t ncells, int64_t ld, const 
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 
+// ---- NEXT-3: structural sparsity pattern (qss_pattern.cpp) and packed output (qss_driver.cu) -----------------------------------
+int qss_pattern_build(const qss_mech_desc_t *d, int mode, uint8_t *pat);
+cudaError_t qss_launch_jac_pack(int nnz, int64_t ncells, int64_t ld, const int32_t *idx, const double *jac, double *out, cudaStream_t stream);
+
+extern "C" int qss_mech_jac_pattern(const qss_mech_desc_t *desc, int mode, uint8_t *pattern) {
+    if (!desc || !pattern) return fail(QSS_E_INVALID, "NULL argument");
+    if (mode < 0 || mode > 2) return fail(QSS_E_INVALID, "mode must be QSS_JAC_EXACT, QSS_JAC_CONST_QSS or QSS_JAC_ZERO_QSS");
+    QssCompiled c;
+    std::string err;
+    int rc;
+    try {
+        rc = qss_compile(desc, c, err);                                 // (validation: the pattern is defined for mechanisms the library accepts)
+    } catch (const std::exception &e) {
+        rc = QSS_E_INVALID; err = std::string("mechanism compiler: ") + e.what();
+    }
+    if (rc != QSS_OK) return fail(rc, err);
+    return qss_pattern_build(desc, mode, pattern);
+}
+
+extern "C" int qss_jac_pack(const qss_mech_t *m, int64_t ncells, int64_t ld, int32_t nnz, const int32_t *idx, const double *jac, double *packed, void *stream) {
+    if (!m) return fail(QSS_E_INVALID, "mech is NULL");
+    if (ncells < 0 || ld < ncells || nnz < 0 || (ld & 1)) return fail(QSS_E_INVALID, "need 0 <= ncells <= ld, ld even, nnz >= 0");
+    if (ncells == 0 || nnz == 0) return QSS_OK;
+    if (!idx || !jac || !packed) return fail(QSS_E_INVALID, "NULL device pointer");
+    if (((uintptr_t)jac | (uintptr_t)packed) & 15) return fail(QSS_E_INVALID, "device pointers must be 16-byte aligned");
+    DeviceGuard guard(m->device);
+    cudaError_t e = qss_launch_jac_pack(nnz, ncells, ld, idx, jac, packed, (cudaStream_t)stream);
+    return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_jac_pack launch");
+}
+
 // ---- NEXT-3: temperature column by finite differences (reading G22; kernels in qss_driver.cu) ---------------
 cudaError_t qss_launch_fdT_perturb(int64_t ncells, const double *T, double *Tp, double *Tm, cudaStream_t stream);
 cudaError_t qss_launch_fdT_column(int N, int64_t ncells, int64_t ld, const double *wp, const double *wm, const double *Tp, const double *Tm, double *jac,

@@ -88,3 +88,26 @@ cudaError_t qss_launch_fdT_column(int N, int64_t ncells, int64_t ld, const doubl
     qss_fdT_column_kernel<<<grid, 256, 0, stream>>>(N, ncells, ld, wp, wm, Tp, Tm, jac);
     return cudaGetLastError();
 }
+
+// ---- NEXT-3: packed Jacobian (Table 4): row e of the output = row idx[e] of the dense SoA Jacobian (cells innermost, so a
+// row is contiguous: the pack is a gather of whole rows, 16 bytes per thread)
+namespace {
+__global__ void __launch_bounds__(256) qss_jac_pack_kernel(int nnz, int64_t ncells, int64_t ld, const int32_t *__restrict__ idx, const double *__restrict__ jac,
+                                                            double *__restrict__ out) {
+    const int64_t c = ((int64_t)blockIdx.x * 256 + threadIdx.x) * 2;
+    if (c >= ncells) return;
+    for (int e = blockIdx.y; e < nnz; e += gridDim.y) {
+        const double *src = jac + (size_t)idx[e] * ld + c;
+        double *dst = out + (size_t)e * ld + c;
+        if (c + 1 < ncells) *reinterpret_cast<double2 *>(dst) = *reinterpret_cast<const double2 *>(src);
+        else dst[0] = src[0];
+    }
+}
+}  // namespace
+
+cudaError_t qss_launch_jac_pack(int nnz, int64_t ncells, int64_t ld, const int32_t *idx, const double *jac, double *out, cudaStream_t stream) {
+    if (ncells == 0 || nnz == 0) return cudaSuccess;
+    const dim3 grid((unsigned)((ncells + 511) / 512), (unsigned)(nnz < 64 ? nnz : 64));
+    qss_jac_pack_kernel<<<grid, 256, 0, stream>>>(nnz, ncells, ld, idx, jac, out);
+    return cudaGetLastError();
+}

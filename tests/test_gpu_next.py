@@ -111,3 +111,34 @@ def test_finite_difference_temperature_column(name, n):
     g = gates.wdot_gates(w.cpu().numpy(), ref["wdot"], ref["S"], n)
     assert g["finite"] and g["tier2_all"]
     qm.close()
+
+
+@pytest.mark.parametrize("name,n", [("cfg1", 512 + 3), ("toy3", 70), ("cfg2", 256)])
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_sparsity_pattern_and_packed_output(name, n, mode):
+    """NEXT-3 (Table 4): outside the structural pattern the kernel's Jacobian is exactly 0.0; qss_jac_pack gathers the
+    pattern's rows bit for bit (the dense output stays the reference, which is gated against the oracle elsewhere)."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    mech = qss_synth.config_mechanism(int(name[3])) if name.startswith("cfg") else getattr(qss_synth, name)()
+    if name.startswith("cfg"):
+        C, T = qss_synth.config_states(int(name[3]), n)
+    else:
+        C, T = make_states(mech.n_nqss, n, seed=5)
+    qm = qss.QssMech(mech, 0)
+    if mode and qm.info.kernel_variant_jac != 3:
+        pytest.skip("simplified Jacobians need kernel variant 3")
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda()
+    J = qm.eval_jac_approx(Cd, Td, mode, n)
+    pat = qss.jac_pattern(mech, mode).astype(bool)
+    Jh = J.cpu().numpy()
+    assert (Jh[:, :, :n][~pat] == 0.0).all()
+    idx = torch.from_numpy(np.flatnonzero(pat.ravel()).astype(np.int32)).cuda()
+    ld = C.shape[1]
+    packed = torch.full((idx.numel(), ld), float("nan"), dtype=torch.float64, device="cuda")
+    qm.jac_pack(J, idx, n, packed=packed)
+    torch.cuda.synchronize()
+    ph = packed.cpu().numpy()
+    assert np.array_equal(ph[:, :n], Jh.reshape(-1, ld)[np.flatnonzero(pat.ravel())][:, :n])
+    assert np.isnan(ph[:, n + (n & 1):]).all()                           # (16-byte stores: at most one padding cell behind an odd count is written)
+    qm.close()

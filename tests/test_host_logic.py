@@ -227,3 +227,27 @@ def test_two_rank_sharding_and_timing_reduction_gloo():
     [p.join(60) for p in ps]
     assert out[0][1:3] == (0, 512) and out[1][1:3] == (512, 1000)
     assert out[0][3] == 2.0 and out[1][3] == 2.0          # max over ranks
+
+
+@pytest.mark.parametrize("name", ["toy3", "toy_dag", "cfg1", "cfg2"])
+def test_structural_jacobian_pattern_against_the_oracle(name):
+    """NEXT-3 (Table 4): qss_mech_jac_pattern is host logic; every numerically non-zero entry of the oracle's Jacobian (any
+    of 40 random states, the paper's sampling) lies inside the structural pattern of the same mode, and on the generic synthetic
+    mechanisms the two coincide; the chain term only ever adds entries (exact >= constant-QSS >= zero-QSS)."""
+    import oracle
+    mech = qss_synth.config_mechanism(int(name[3])) if name.startswith("cfg") else getattr(qss_synth, name)()
+    N = mech.n_nqss; n = 40
+    rng = np.random.default_rng(1)
+    C = np.ascontiguousarray(rng.uniform(1e-4, 1.0, size=(N, n))); T = rng.uniform(300.0, 1300.0, size=n)
+    om = oracle.OracleMech(mech)
+    pats = []
+    for mode, omode in ((0, oracle.EXPLICIT_F64), (1, oracle.JAC_CONST_QSS), (2, oracle.JAC_ZERO_QSS)):
+        pat = qss.jac_pattern(mech, mode).astype(bool)
+        with np.errstate(all="ignore"):
+            num = (oracle.evaluate(om, C, T, mode=omode)["jac"] != 0).any(2)
+        assert not (num & ~pat).any(), (name, mode)
+        if name.startswith("cfg"):
+            assert np.array_equal(num, pat), (name, mode)
+        pats.append(pat)
+        print("%s mode %d: fill of the N x N block %.3f" % (name, mode, pat[:, :N].mean()))
+    assert not (pats[1] & ~pats[0]).any() and not (pats[2] & ~pats[1]).any()
