@@ -1,0 +1,141 @@
+"""Mechanism front-end (NEXT-4, second half; paper_2405_05974_b200/frontend.py): CHEMKIN-format ingestion and the three
+linearisation methods of PAPER.md section 2.2 (L73-122, Algorithm 1).  Host logic; the mechanism text below is made up for the
+test (species A2, B2, AB ..., invented rate parameters): no published mechanism is reproduced."""
+from __future__ import annotations
+
+import itertools
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2405_05974_b200 as qss
+from paper_2405_05974_b200 import frontend as fe
+
+
+def nasa_record(name, comp, a1, a6, a7, tlow=300.0, thigh=3500.0, tmid=1000.0):
+    """Four fixed-column lines; the same constant-cp fit in both ranges (cp/R = a1, h/RT = a1 + a6/T, s/R = a1 ln T + a7)."""
+    c = "".join("%-2s%3d" % (e, n) for e, n in comp) + " " * (5 * (4 - len(comp)))
+    l1 = "%-18s%-6s%s%s%10.2f%10.2f%8.2f" % (name, "test", c, "G", tlow, thigh, tmid)
+    l1 = l1.ljust(79) + "1"
+    co = [a1, 0.0, 0.0, 0.0, 0.0, a6, a7] * 2
+    f = ["%15.8E" % v for v in co]
+    return "\n".join([l1, ("".join(f[0:5])).ljust(79) + "2", ("".join(f[5:10])).ljust(79) + "3", ("".join(f[10:14])).ljust(79) + "4"])
+
+
+SPECIES = [("A2", [("H", 2)], 3.5, -1000.0, 1.0), ("B2", [("O", 2)], 3.6, -1100.0, 2.0), ("AB", [("H", 1), ("O", 1)], 3.7, 4000.0, 3.0),
+           ("A2B", [("H", 2), ("O", 1)], 4.2, -29000.0, 1.5), ("A", [("H", 1)], 2.5, 25000.0, -0.5), ("B", [("O", 1)], 2.6, 29000.0, 0.5),
+           ("AB2", [("H", 1), ("O", 2)], 4.5, 1000.0, 2.5), ("A2B2", [("H", 2), ("O", 2)], 5.0, -17000.0, 2.2)]
+
+TEXT = """! a made-up H/O-shaped test mechanism
+ELEMENTS H O END
+SPECIES A2 B2 AB
+        A2B A B AB2 A2B2 END
+THERMO ALL
+   300.000  1000.000  3500.000
+%s
+END
+REACTIONS
+A + B2 <=> B + AB            3.5E+15  -0.40   16600.0   ! bimolecular, cal/mol
+B + A2 = A + AB              5.0E+04   2.67    6290.0
+AB + A2 <=> A + A2B          2.2E+08   1.51    3430.0
+2AB <=> B + A2B              3.6E+04   2.40   -2110.0
+A + B2 + M <=> AB2 + M       2.8E+18  -0.86       0.0
+   A2B/11.0/ B2/0.78/ A/2.0/
+A + AB2 => 2AB               7.1E+13   0.00     295.0
+AB + AB (+M) <=> A2B2 (+M)   7.4E+13  -0.37       0.0
+   LOW / 2.3E+18 -0.90 -1700.0 /
+   TROE / 0.735 94.0 1756.0 5182.0 /
+   A2/2.0/ A2B/6.0/
+AB2 + AB2 <=> A2B2 + B2      1.3E+11   0.00   -1630.0
+  DUPLICATE
+AB2 + AB2 <=> A2B2 + B2      4.2E+14   0.00   12000.0
+  DUPLICATE
+A2B2 + A (+M) <=> A2B + AB (+M)  2.4E+13  0.00  3970.0
+   LOW / 1.0E+17 0.0 1000.0 /   TROE / 0.5 100.0 2000.0 /
+END
+""" % "\n".join(nasa_record(n, c, a1, a6, a7) for n, c, a1, a6, a7 in SPECIES)
+
+
+def test_parse_layout_units_and_thermo():
+    d = fe.parse_chemkin(TEXT, qss=["A", "B"])
+    assert d.species == ["A2", "B2", "AB", "A2B", "AB2", "A2B2", "A", "B"] and (d.n_nqss, d.n_qss, d.n_reac) == (6, 2, 10)
+    sp = d.species.index
+    assert d.side(0, 0) == [(sp("A"), 1), (sp("B2"), 1)] and d.side(0, 1) == [(sp("B"), 1), (sp("AB"), 1)]
+    assert d.side(3, 0) == [(sp("AB"), 2)] and d.side(5, 1) == [(sp("AB"), 2)] and d.side(6, 0) == [(sp("AB"), 2)]
+    assert list(d.rtype) == [0, 0, 0, 0, 1, 0, 2, 0, 0, 2] and list(d.dir_mask) == [3, 3, 3, 3, 3, 1, 3, 3, 3, 3]
+    # cm^3-mol-s -> m^3-mol-s, cal -> J: bimolecular 1e-6, two reactants + M 1e-12, fall-off k_inf (2 reactants) 1e-6, k_0 1e-12
+    assert np.isclose(d.arr[0, 0], 3.5e15 * 1e-6) and np.isclose(d.arr[0, 2], 16600.0 * 4.184) and d.arr[0, 1] == -0.40
+    assert np.isclose(d.arr[4, 0], 2.8e18 * 1e-12) and np.isclose(d.arr[6, 0], 7.4e13 * 1e-6) and np.isclose(d.arr_low[6, 0], 2.3e18 * 1e-12)
+    assert np.isclose(d.arr_low[6, 2], -1700.0 * 4.184) and list(d.troe[6]) == [0.735, 94.0, 1756.0, 5182.0] and list(d.troe[9]) == [0.5, 100.0, 2000.0, 1e30]
+    # efficiencies: CSR on transported species; the QSS species' one is dropped with a warning
+    e4 = {d.species[s]: v for s, v in zip(d.eff_sp[d.eff_ptr[4]:d.eff_ptr[5]], d.eff_val[d.eff_ptr[4]:d.eff_ptr[5]])}
+    assert e4 == {"A2B": 11.0, "B2": 0.78} and any("efficiency of the QSS species A" in w for w in d.warnings)
+    # thermo: composition, ranges, HIGH range first in the file, LOW second
+    assert list(d.comp[sp("A2B")]) == [2, 1] and list(d.nasa_T[sp("A2B")]) == [300.0, 1000.0, 3500.0]
+    assert np.allclose(d.nasa_hi[sp("A2B")], [4.2, 0, 0, 0, 0, -29000.0, 1.5]) and np.allclose(d.nasa_lo[sp("A")], [2.5, 0, 0, 0, 0, 25000.0, -0.5])
+    assert np.allclose(d.elem_weight, [1.008, 15.999])
+    # the description is one the library takes (strict element balance included) and the oracle evaluates
+    ng, order, grp = qss.validate(d, strict_balance=True)
+    assert ng >= 1 and sorted(order) == [0, 1]
+    C = np.ascontiguousarray(np.random.default_rng(0).uniform(0.01, 1.0, size=(6, 4))); T = np.array([900.0, 1200.0, 1500.0, 2000.0])
+    out = oracle.evaluate(oracle.OracleMech(d), C, T)
+    assert np.isfinite(out["jac"]).all() and np.abs(out["wdot"]).max() > 0
+    a = d.comp[:6].astype(float)
+    assert np.abs(a.T @ out["wdot"]).max() <= 1e-9 * (np.abs(a).T @ out["S"]).max()       # elements conserved: stoichiometry and order intact
+
+
+@pytest.mark.parametrize("bad,msg", [("A + XX <=> B + AB 1.0 0 0", "unknown species"), ("A + B2 <=> B + AB 1.0 0 0\n REV / 1 0 0 /", "REV"),
+                                     ("A + B2 (+A2B) <=> AB2 (+A2B) 1.0 0 0", "collision partners"), ("A + B2 + M <=> AB2 1.0 0 0", "one side"),
+                                     ("AB + AB (+M) <=> A2B2 (+M) 1.0 0 0", "LOW and TROE"), ("A + B2 <=> B + AB 1.0 0", "cannot read")])
+def test_what_is_not_read_is_an_error(bad, msg):
+    text = TEXT[:TEXT.index("REACTIONS")] + "REACTIONS\n" + bad + "\nEND\n"
+    with pytest.raises(fe.MechanismError) as e:
+        fe.parse_chemkin(text)
+    assert msg in str(e.value)
+    with pytest.raises(fe.MechanismError):
+        fe.parse_chemkin(TEXT.replace("SPECIES A2 B2 AB", "SPECIES A2 B2 AB ZZ"))                  # no thermo record
+    with pytest.raises(fe.MechanismError):
+        fe.parse_chemkin(TEXT, qss=["NOPE"])
+
+
+def test_linearisation_methods():
+    """QSS = {A, B, AB2}: quadratic couplings in `A + AB2 => 2AB` (reactants A + AB2) and in both `AB2 + AB2 <=> A2B2 + B2`."""
+    d = fe.parse_chemkin(TEXT, qss=["A", "B", "AB2"])
+    qc = fe.quadratic_couplings(d)
+    by_eq = {(d.equations[j], s) for j, s in qc}
+    assert by_eq == {("A+AB2=>2AB", 0), ("AB2+AB2<=>A2B2+B2", 0)} and len(qc) == 3
+    with pytest.raises(qss.QssError) as e:
+        qss.validate(d)
+    assert e.value.code == -2                                           # QSS_E_QUADRATIC
+    # species method: Algorithm 1 against brute force over ALL subsets of ALL QSS species by growing size
+    sets = fe.species_linearisation_sets(d)
+    def clean(gone):
+        return all(sum(nu for sp, nu in d.side(j, s) if sp >= d.n_nqss and sp not in gone) < 2 for j in range(d.n_reac) for s in (0, 1))
+    brute = []
+    for i in range(1, d.n_qss + 1):
+        brute = [c for c in itertools.combinations(range(d.n_nqss, d.n_sp), i) if clean(set(c))]
+        if brute:
+            break
+    assert sorted(sets) == sorted(brute) and len(sets[0]) == len(brute[0])
+    ds = fe.linearise(d, "species")
+    assert ds.n_qss == d.n_qss - len(sets[0]) and not fe.quadratic_couplings(ds)
+    qss.validate(ds, strict_balance=True)
+    assert sorted(ds.species) == sorted(d.species) and ds.species[:d.n_nqss] == d.species[:d.n_nqss]
+    # a chosen set
+    d2 = fe.linearise(d, "species", sets[-1])
+    assert [d.species[x] for x in sets[-1]] == d2.species[d.n_nqss:d.n_nqss + len(sets[-1])]
+    # reaction method: every coupled reaction loses both directions; the rest is untouched; the library takes the result
+    dr = fe.linearise(d, "reaction")
+    coupled = {j for j, _ in qc}
+    assert all(dr.dir_mask[j] == 0 for j in coupled) and all(dr.dir_mask[j] == d.dir_mask[j] for j in range(d.n_reac) if j not in coupled)
+    qss.validate(dr, strict_balance=True)
+    # one-sided method: only the consuming direction goes; what stays produces two QSS molecules -> the closure refuses it
+    do = fe.linearise(d, "one_sided")
+    j = d.equations.index("AB2+AB2<=>A2B2+B2")
+    assert do.dir_mask[j] == 2 and do.dir_mask[d.equations.index("A+AB2=>2AB")] == 0
+    with pytest.raises(qss.QssError) as e:
+        qss.validate(do)
+    assert e.value.code == -3                                           # QSS_E_QSS_FANOUT
+    with pytest.raises(fe.MechanismError):
+        fe.linearise(d, "nonsense")

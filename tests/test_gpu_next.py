@@ -142,3 +142,27 @@ def test_sparsity_pattern_and_packed_output(name, n, mode):
     assert np.array_equal(ph[:, :n], Jh.reshape(-1, ld)[np.flatnonzero(pat.ravel())][:, :n])
     assert np.isnan(ph[:, n + (n & 1):]).all()                           # (16-byte stores: at most one padding cell behind an odd count is written)
     qm.close()
+
+
+def test_parsed_mechanism_runs_on_the_kernels():
+    """NEXT-4, second half: CHEMKIN-format text -> frontend.parse_chemkin -> linearisation -> qss_mech_create -> the Jacobian kernel,
+    against the oracle on the same description (third-body, fall-off with a three-parameter Troe line, an irreversible reaction,
+    duplicates)."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    from paper_2405_05974_b200 import frontend as fe
+    from test_frontend import TEXT
+    d = fe.linearise(fe.parse_chemkin(TEXT, qss=["A", "B", "AB2"]), "reaction")
+    n = 200
+    rng = np.random.default_rng(2)
+    C = np.ascontiguousarray(10.0 ** rng.uniform(-4.0, 1.0, size=(d.n_nqss, n))); T = rng.uniform(700.0, 2400.0, size=n)
+    qm = qss.QssMech(d, 0, strict_balance=True)
+    J, w = qm.eval_jac(torch.from_numpy(C).cuda(), torch.from_numpy(T).cuda(), n, want_wdot=True)
+    torch.cuda.synchronize()
+    ref = oracle.evaluate(oracle.OracleMech(d), C, T, n, want_scale=True)
+    gw = gates.wdot_gates(w.cpu().numpy(), ref["wdot"], ref["S"], n)
+    gj = gates.jac_gates(J.cpu().numpy(), ref["jac"], ref["jscale"], n)
+    print("parsed mechanism: kernel variant %d; wdot tier 1 %.3f, tier 2 worst %.3g; Jacobian tier 2 %s" % (qm.info.kernel_variant_jac, gw["tier1_frac"], gw["tier2_worst"], gj.get("cell_tier2_all")))
+    assert gw["finite"] and gw["tier2_all"] and gw["tier1_frac"] >= 0.99
+    assert gj["finite"] and all(v for k, v in gj.items() if k.endswith("tier2_all"))
+    qm.close()
