@@ -35,6 +35,7 @@ FP64_LANES_PER_SM = 64          # 148 SMs x 64 fp64 FMA la
 EXPECTED_JAC_VARIANT = {1: 3, 2: 3, 4: 3, 3: 0, 5: 0}   # the kernel each BASELINE config is expected to run on
 CALLS = {"jac+wdot": "qss_eval_jac with the wdot output (the metric)", "jac": "qss_eval_jac alone", "wdot": "qss_eval_wdot alone",
          "jac+wdot+energy": "qss_eval_jac with wdot, then qss_eval_energy: the full (N+1)x(N+1) Jacobian and the temperature right-hand side",
+         "jac_full": "qss_eval_jac_full: the full (N+1)x(N+1) Jacobian, wdot and Tdot in one call (two launches)",
          "energy": "qss_eval_energy alone (on a Jacobian computed before the timed region)",
          "jac_const": "qss_eval_jac_approx, constant-QSS AJ", "jac_zero": "qss_eval_jac_approx, zero-QSS AJ",
          "newton": "qss_newton_solve alone: x = (I - gamma J)^-1 (wdot, Tdot) on a full Jacobian computed before the timed region",
@@ -225,7 +226,7 @@ def main():
         qm.newton_solve(J, erow, gam, B, n, x=X)        # (first call: run-time compilation, outside the timed region)
         torch.cuda.synchronize()
         assert bool(torch.isfinite(X[:, :n]).all())
-    launches_per_step = {"jac+wdot+energy": 2, "jac+wdot+energy+newton": 3, "bdf1": 10}.get(args.call, 1)
+    launches_per_step = {"jac+wdot+energy": 2, "jac+wdot+energy+newton": 3, "bdf1": 10, "jac_full": 2}.get(args.call, 1)
     if args.call == "bdf1":
         # h_c = 3 / max|J_c| at the initial state (a few of the fastest time scales per substep); the state is restored before every step
         del J
@@ -253,6 +254,8 @@ def main():
         elif args.call == "bdf1":
             Cd.copy_(C0); Td.copy_(T0)
             qm.bdf1_advance(Cd, Td, dtd, 1, 2, n, workspace=bdf_ws)
+        elif args.call == "jac_full":
+            qm.eval_jac_full(Cd, Td, n, jac=J, wdot=W, tdot=tdot, erow=erow)
         elif args.call == "jac":
             qm.eval_jac(Cd, Td, n, jac=J)
         elif args.call == "energy":
@@ -336,6 +339,8 @@ def main():
         slots_cell = 2.0 * (info.slots_jac + 2.0 * N * nn + 30.0 * N + nn ** 3 / 3.0 + nn * nn)
     else:
         bytes_cell, slots_cell = info.bytes_jac + (8.0 * N if args.call.startswith("jac+wdot") else 0.0), info.slots_jac
+        if args.call == "jac_full":      # + wdot, Tdot, the energy row; + 2 N (N+1) + ~30 N slots for the row
+            bytes_cell += 8.0 * (2 * N + 2); slots_cell += 2.0 * N * (N + 1) + 30.0 * N
     bytes_launch = bytes_cell * n
     slots_launch = slots_cell * n
     fp64_peak_slots = sms * FP64_LANES_PER_SM * sm_max_mhz * 1e6

@@ -175,6 +175,12 @@ int qss_newton_solve(const qss_mech_t *mech, int64_t ncells, int64_t ld, const d
                      const double *gamma, const double *b, double *x, void *stream);
 int qss_newton_specialise_check(int n_species, int with_energy, int cc_major, int cc_minor, size_t *image_bytes_or_null);
 
+/* NEXT-1 in one call: the full (N+1) x (N+1) Jacobian of Eq. 7 (L185) and both right-hand sides: the outputs of qss_eval_jac (jac,
+ * wdot) AND of qss_eval_energy (tdot, erow) for the same cells; all four are required.  Two launches on `stream` (the Jacobian
+ * kernel, then the energy-row kernel at 0.81 of the HBM peak).  Arguments, layout and workspace as qss_eval_jac. */
+int qss_eval_jac_full(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *C, const double *T, double *jac, double *wdot,
+                      double *tdot, double *erow, void *workspace, size_t workspace_bytes, void *stream);
+
 /* NEXT-3: sparsity (Table 4: fraction of non-zero entries of the AJ; the chain term of Eq. 9 roughly doubles it).
  * qss_mech_jac_pattern: host only, no device: pattern[i*(N+1) + k] = 1 when entry (row i, column k; k = N: T) of the Jacobian of
  * `mode` (qss_jac_mode) can be non-zero for some state, else 0 -- those entries are exactly 0.0 in the output of qss_eval_jac /

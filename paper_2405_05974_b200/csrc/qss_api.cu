@@ -374,6 +374,17 @@ static int eval_jac_mode(const qss_mech_t *m, int64_t ncells, int64_t ld, const 
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 
+// ---- NEXT-1 in one call: the full (N+1) x (N+1) Jacobian and both right-hand sides (the two launches in sequence; a version with
+// the energy row formed inside the sweep of kernel variant 3 was built and measured at 14.0 ms against 13.6 ms: DESIGN.md section 6)
+extern "C" int qss_eval_jac_full(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T, double *jac, double *wdot,
+                                 double *tdot, double *erow, void *workspace, size_t workspace_bytes, void *stream) {
+    if (!m) return fail(QSS_E_INVALID, "mech is NULL");
+    if (!wdot || !tdot || !erow) return fail(QSS_E_INVALID, "qss_eval_jac_full: wdot, tdot and erow are required");
+    int rc = eval_jac_mode(m, ncells, ld, C, T, jac, wdot, 0, workspace, workspace_bytes, stream);
+    if (rc != QSS_OK || ncells == 0) return rc;
+    return qss_eval_energy(m, ncells, ld, C, T, wdot, jac, tdot, erow, stream);
+}
+
 // ---- NEXT-3: structural sparsity pattern (qss_pattern.cpp) and packed output (qss_driver.cu) -----------------------------------
 int qss_pattern_build(const qss_mech_desc_t *d, int mode, uint8_t *pat);
 cudaError_t qss_launch_jac_pack(int nnz, int64_t ncells, int64_t ld, const int32_t *idx, const double *jac, double *out, cudaStream_t stream);
@@ -473,8 +484,7 @@ extern "C" int qss_bdf1_advance(const qss_mech_t *m, int64_t ncells, int64_t ld,
         if (e == cudaSuccess) e = cudaMemcpyAsync(phin + (size_t)N * nrow, T, nrow * sizeof(double), cudaMemcpyDeviceToDevice, st);
         if (e != cudaSuccess) return cuda_fail(e, "qss_bdf1_advance: saving the state");
         for (int it = 0; it < newton_iters; ++it) {
-            int rc = eval_jac_mode(m, ncells, ld, C, T, jac, F, 0, ws, wsb, stream);                       // J species block, wdot -> F[0..N-1]
-            if (rc == QSS_OK) rc = qss_eval_energy(m, ncells, ld, C, T, F, jac, F + (size_t)N * nrow, erow, stream);   // Tdot -> F[N], energy row
+            int rc = qss_eval_jac_full(m, ncells, ld, C, T, jac, F, F + (size_t)N * nrow, erow, ws, wsb, stream);      // J, wdot -> F[0..N-1], Tdot -> F[N], energy row
             if (rc != QSS_OK) return rc;
             e = qss_launch_bdf1_residual(N, ncells, ld, C, T, phin, F, dt, b, st);
             if (e != cudaSuccess) return cuda_fail(e, "qss_bdf1_advance: residual kernel");

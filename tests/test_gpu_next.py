@@ -166,3 +166,29 @@ def test_parsed_mechanism_runs_on_the_kernels():
     assert gw["finite"] and gw["tier2_all"] and gw["tier1_frac"] >= 0.99
     assert gj["finite"] and all(v for k, v in gj.items() if k.endswith("tier2_all"))
     qm.close()
+
+
+@pytest.mark.parametrize("name,n", [("cfg1", 4096), ("cfg2", 2048 + 19), ("toy_dag", 77), ("cfg3", 96 + 5)])
+def test_full_jacobian_in_one_call(name, n):
+    """qss_eval_jac_full: jac and wdot bit for bit those of qss_eval_jac; tdot and the energy row against the oracle with the gates
+    of qss_eval_energy."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    if name.startswith("cfg"):
+        mech = qss_synth.config_mechanism(int(name[3])); C, T = qss_synth.config_states(int(name[3]), n)
+    else:
+        mech = getattr(qss_synth, name)(); C, T = make_states(mech.n_nqss, n, seed=5)
+    ld = C.shape[1]
+    qm = qss.QssMech(mech, 0)
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda()
+    J0, w0 = qm.eval_jac(Cd, Td, n, want_wdot=True)
+    tdot = torch.full((ld,), float("nan"), dtype=torch.float64, device="cuda")
+    erow = torch.full((qm.N + 1, ld), float("nan"), dtype=torch.float64, device="cuda")
+    J, w, _, _ = qm.eval_jac_full(Cd, Td, n, tdot=tdot, erow=erow)
+    torch.cuda.synchronize()
+    assert torch.equal(J[:, :, :n], J0[:, :, :n]) and torch.equal(w[:, :n], w0[:, :n])
+    ref = oracle.evaluate_energy(oracle.OracleMech(mech), C, T, n)
+    _energy_gates(tdot.cpu().numpy(), erow.cpu().numpy(), ref, T, n, name + " (one call)")
+    if ld > n:
+        assert torch.isnan(tdot[n:]).all() and torch.isnan(erow[:, n:]).all(), "padding was written"
+    qm.close()
