@@ -175,6 +175,19 @@ int qss_newton_solve(const qss_mech_t *mech, int64_t ncells, int64_t ld, const d
                      const double *gamma, const double *b, double *x, void *stream);
 int qss_newton_specialise_check(int n_species, int with_energy, int cc_major, int cc_minor, size_t *image_bytes_or_null);
 
+/* Allocation-free variant of qss_eval_wdot, for callers that cannot provide (or allocate) a workspace: code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc.  Same inputs, outputs, layout and results as qss_eval_wdot; the
+ * workspace is a static device array of QSS_STATIC_SCRATCH_BYTES bytes inside the library, which every GPU that loads the library
+ * holds until the process exits (its device address is taken once per device at qss_mech_create).  The call launches the general
+ * slab kernel (kernel variant 0, whatever variant the handle selected for qss_eval_wdot) with as many persistent blocks as fit the
+ * array, and calls no allocating routine.  Limit: a mechanism whose ONE-block workspace exceeds the array is rejected with
+ * QSS_E_UNSUPPORTED (more than 131 072 doubles of per-cell workspace, roughly 30 000 reactions; the BASELINE configs need
+ * 0.03-2.3 MB per block); any ncells is accepted.  Every call on a device shares the array: calls that overlap on the GPU (two streams, two handles, two threads) race;
+ * order them on one stream.  Nothing in the array has to start at zero: the kernel writes every row before it reads it. */
+#define QSS_STATIC_SCRATCH_BYTES (32u << 20)
+int qss_eval_wdot_static(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *C, const double *T, double *wdot,
+                         double *cqss_or_null, void *stream);
+
 /* NEXT-1 in one call: the full (N+1) x (N+1) Jacobian of Eq. 7 (L185) and both right-hand sides: the outputs of qss_eval_jac (jac,
  * wdot) AND of qss_eval_energy (tdot, erow) for the same cells; all four are required.  Two launches on `stream` (the Jacobian
  * kernel, then the energy-row kernel at 0.81 of the HBM peak).  Arguments, layout and workspace as qss_eval_jac. */

@@ -17,7 +17,7 @@ from . import build as _build
 __all__ = ["lib", "QssMech", "QssError", "EXPORTS", "STATUS"]
 
 EXPORTS = ["qss_mech_create", "qss_mech_validate", "qss_mech_specialise_check", "qss_mech_destroy", "qss_mech_info", "qss_mech_qss_order", "qss_eval_wdot",
-           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_newton_solve", "qss_newton_specialise_check", "qss_bdf1_workspace_bytes", "qss_bdf1_advance", "qss_jac_fdt_workspace_bytes", "qss_eval_jac_fdt", "qss_mech_jac_pattern", "qss_jac_pack", "qss_eval_jac_full", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
+           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_newton_solve", "qss_newton_specialise_check", "qss_bdf1_workspace_bytes", "qss_bdf1_advance", "qss_jac_fdt_workspace_bytes", "qss_eval_jac_fdt", "qss_mech_jac_pattern", "qss_jac_pack", "qss_eval_jac_full", "qss_eval_wdot_static", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
 STATUS = {0: "QSS_OK", -1: "QSS_E_INVALID", -2: "QSS_E_QUADRATIC", -3: "QSS_E_QSS_FANOUT", -4: "QSS_E_NO_SINK",
           -5: "QSS_E_UNSUPPORTED", -6: "QSS_E_CUDA", -7: "QSS_E_UNBALANCED"}
 
@@ -71,6 +71,7 @@ def lib():
         L.qss_eval_jac_approx.restype = ct.c_int; L.qss_eval_jac_approx.argtypes = [vp, i64, i64, vp, vp, vp, ct.c_int, vp, ct.c_size_t, vp]
         L.qss_eval_energy.restype = ct.c_int; L.qss_eval_energy.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp]
         L.qss_newton_solve.restype = ct.c_int; L.qss_newton_solve.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp]
+        L.qss_eval_wdot_static.restype = ct.c_int; L.qss_eval_wdot_static.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
         L.qss_eval_jac_full.restype = ct.c_int; L.qss_eval_jac_full.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp, ct.c_size_t, vp]
         L.qss_mech_jac_pattern.restype = ct.c_int; L.qss_mech_jac_pattern.argtypes = [vp, ct.c_int, vp]
         L.qss_jac_pack.restype = ct.c_int; L.qss_jac_pack.argtypes = [vp, i64, i64, ct.c_int32, vp, vp, vp, vp]
@@ -248,6 +249,15 @@ class QssMech:
         ws = self.workspace(True)
         _check(lib().qss_eval_jac_approx(self._h, ncells, ld, _ptr(C), _ptr(T), _ptr(jac), int(mode), _ptr(ws), ws.numel(), self._stream()))
         return jac
+
+    def eval_wdot_static(self, C, T, ncells=None, wdot=None, cqss=None):
+        """wdot through the allocation-free entry point (qss_eval_wdot_static): `wdot` (and `cqss`) are the caller's tensors; no
+        workspace is passed and nothing is allocated by the library.  Calls that overlap on the GPU race."""
+        ld = C.shape[1]
+        ncells = ld if ncells is None else int(ncells)
+        assert wdot is not None and wdot.is_contiguous() and wdot.shape == (self.N, ld)
+        _check(lib().qss_eval_wdot_static(self._h, ncells, ld, _ptr(C), _ptr(T), _ptr(wdot), _ptr(cqss), self._stream()))
+        return wdot
 
     def eval_jac_full(self, C, T, ncells=None, jac=None, wdot=None, tdot=None, erow=None):
         """Full (N+1) x (N+1) Jacobian and both right-hand sides in one call (qss_eval_jac_full). Returns (jac, wdot, tdot, erow)."""

@@ -15,6 +15,10 @@
 #include "qss_devtools.h"
 
 size_t qss_slab_ws_doubles(const QssTab &t, bool jac, int nwarp);
+cudaError_t qss_static_scratch_setup(int device);
+size_t qss_static_scratch_capacity();
+cudaError_t qss_launch_slab_static(const QssTab &t, int device, int64_t ncells, int64_t ld, const double *C, const double *T, double *wdot,
+                                   double *cqss, int nblocks, int nwarp, cudaStream_t stream, int *blocks_out);
 cudaError_t qss_launch_slab(const QssTab &t, bool jac, int64_t ncells, int64_t ld, const double *C, const double *T,
                             double *wdot, double *cqss, double *jacp, double *ws, int nblocks, int nwarp,
                             cudaStream_t stream);
@@ -45,6 +49,7 @@ struct qss_mech {
     double *dP3 = nullptr;    // variant 3: parameter blobs of the reaction-per-lane phases
     int32_t *iP3 = nullptr;
     int cc_major = 0, cc_minor = 0;
+    bool static_scratch_ok = false;   // qss_static_scratch_setup succeeded on this device
     mutable int newton_blocks[2] = {0, 0};            //   persistent blocks of that kernel (SMs x resident blocks per SM)
     mutable QssJit *newton[2] = {nullptr, nullptr};   // qss_newton_solve: [0] species block (n = N), [1] with the energy row (n = N + 1); built on first use
 };
@@ -105,6 +110,8 @@ extern "C" int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech
     if ((e = cudaGetDeviceProperties(&prop, device)) != cudaSuccess) { delete m; return cuda_fail(e, "cudaGetDeviceProperties"); }
     m->n_sm = prop.multiProcessorCount;
     m->cc_major = prop.major; m->cc_minor = prop.minor;
+    m->static_scratch_ok = qss_static_scratch_setup(device) == cudaSuccess;      // address of the static workspace of qss_eval_wdot_static (no allocation)
+    if (!m->static_scratch_ok) cudaGetLastError();
     if (const char *bps = qss_devenv("QSS_V0_BLOCKS_PER_SM")) m->blocks_per_sm = std::max(1, std::atoi(bps));   // tuning aid for the general kernel
     m->nblocks = m->n_sm * m->blocks_per_sm;
     const size_t nI = m->c.I.size() ? m->c.I.size() : 1, nD = m->c.D.size() ? m->c.D.size() : 1;
@@ -373,6 +380,27 @@ static int eval_jac_mode(const qss_mech_t *m, int64_t ncells, int64_t ld, const 
 
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
+
+// ---- allocation-free entry point: wdot with the workspace in a static device array (qss_kernels.cu) ------------------------------
+extern "C" int qss_eval_wdot_static(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T, double *wdot,
+                                    double *cqss, void *stream) {
+    if (!m) return fail(QSS_E_INVALID, "mech is NULL");
+    if (ncells < 0 || ld < ncells) return fail(QSS_E_INVALID, "need 0 <= ncells <= ld");
+    if (ncells == 0) return QSS_OK;
+    if (!C || !T || !wdot) return fail(QSS_E_INVALID, "C, T or the output pointer is NULL");
+    if (((uintptr_t)C | (uintptr_t)T | (uintptr_t)wdot | (uintptr_t)cqss) & 15) return fail(QSS_E_INVALID, "device pointers must be 16-byte aligned");
+    if (!m->static_scratch_ok) return fail(QSS_E_CUDA, "qss_eval_wdot_static: the address of the static workspace could not be taken at qss_mech_create");
+    const size_t per_block = qss_slab_ws_doubles(m->c.tab, false, m->nwarp) * sizeof(double);
+    if (per_block > qss_static_scratch_capacity()) {
+        char msg[200];
+        std::snprintf(msg, sizeof msg, "qss_eval_wdot_static: one block of this mechanism needs %zu bytes of workspace, the static array holds %zu (QSS_STATIC_SCRATCH_BYTES); use qss_eval_wdot",
+                      per_block, qss_static_scratch_capacity());
+        return fail(QSS_E_UNSUPPORTED, msg);
+    }
+    DeviceGuard guard(m->device);
+    cudaError_t e = qss_launch_slab_static(m->c.tab, m->device, ncells, ld, C, T, wdot, cqss, m->nblocks, m->nwarp, (cudaStream_t)stream, nullptr);
+    return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_eval_wdot_static launch");
+}
 
 // ---- NEXT-1 in one call: the full (N+1) x (N+1) Jacobian and both right-hand sides (the two launches in sequence; a version with
 // the energy row formed inside the sweep of kernel variant 3 was built and measured at 14.0 ms against 13.6 ms: DESIGN.md section 6)

@@ -349,3 +349,51 @@ cudaError_t qss_launch_dfma(int blocks, int iters, double *sink, cudaStream_t st
     qss_dfma_kernel<<<blocks, 256, 0, stream>>>(iters, sink);
     return cudaGetLastError();
 }
+
+// ---------------------------------------------------------------------------------------------------
+// Allocation-free variant of the general slab kernel (qss_eval_wdot_static, include/qss.h): the per-cell workspace that
+// qss_eval_wdot takes from the caller lives in a file-scope device array of QSS_STATIC_SCRATCH_BYTES bytes, which every GPU that
+// loads this library holds until the process exits.  The array's name is a device symbol: host code may not pass it to a
+// kernel; its device address comes from cudaGetSymbolAddress, taken once per device at handle creation (qss_static_scratch_setup,
+// with that device current) and cached here.  The launch uses as many persistent blocks as fit the array.
+// The kernel writes every workspace row of a slab before it reads it (the caller-supplied workspace of qss_eval_wdot is
+// uninitialised memory too), so nothing has to be cleared between calls; calls that overlap on the GPU share the array and race.
+// ---------------------------------------------------------------------------------------------------
+#define QSS_STATIC_SCRATCH_BYTES_ (32u << 20)
+static __device__ __align__(256) unsigned char qss_static_scratch[QSS_STATIC_SCRATCH_BYTES_];
+
+namespace {
+constexpr int QSS_STATIC_MAX_DEVICES = 64;
+double *g_static_ptr[QSS_STATIC_MAX_DEVICES] = {nullptr};      // device address of qss_static_scratch per device ordinal
+}
+
+// Set-up, once per device, with `device` current (called by qss_mech_create): no allocation, the array came with the module.
+cudaError_t qss_static_scratch_setup(int device) {
+    if (device < 0 || device >= QSS_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    if (g_static_ptr[device]) return cudaSuccess;
+    void *p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&p, qss_static_scratch);
+    if (e != cudaSuccess) return e;
+    g_static_ptr[device] = (double *)p;
+    return cudaSuccess;
+}
+
+size_t qss_static_scratch_capacity() { return (size_t)QSS_STATIC_SCRATCH_BYTES_; }
+
+// wdot (and C_QSS) by the general slab kernel with the static workspace.  *blocks_out: persistent blocks used.  Returns
+// cudaErrorMemoryAllocation when not even one block's workspace fits the array, cudaErrorNotReady when set-up has not run.
+cudaError_t qss_launch_slab_static(const QssTab &t, int device, int64_t ncells, int64_t ld, const double *C, const double *T, double *wdot,
+                                   double *cqss, int nblocks, int nwarp, cudaStream_t stream, int *blocks_out) {
+    const int64_t nslab = (ncells + 31) / 32;
+    if (nslab == 0) return cudaSuccess;
+    if (device < 0 || device >= QSS_STATIC_MAX_DEVICES || !g_static_ptr[device]) return cudaErrorNotReady;
+    const size_t per_block = qss_slab_ws_doubles(t, false, nwarp) * sizeof(double);
+    const size_t fit = per_block ? (size_t)QSS_STATIC_SCRATCH_BYTES_ / per_block : (size_t)nblocks;
+    if (fit == 0) return cudaErrorMemoryAllocation;
+    int grid = (int)(nslab < nblocks ? nslab : nblocks);
+    if ((size_t)grid > fit) grid = (int)fit;
+    if (blocks_out) *blocks_out = grid;
+    qss_slab_kernel<false><<<grid, nwarp * 32, 0, stream>>>(t, ncells, ld, C, T, wdot, cqss, nullptr, g_static_ptr[device],
+                                                           (int64_t)qss_slab_ws_doubles(t, false, nwarp));
+    return cudaGetLastError();
+}
