@@ -151,6 +151,7 @@ def main():
     ap.add_argument("--cells", type=int, default=0, help="override the cell count (0 = the config's)")
     ap.add_argument("--call", default="jac+wdot", choices=sorted(CALLS), help="which C-ABI call(s) a step is: " + "; ".join(f"{k}: {v}" for k, v in CALLS.items()))
     ap.add_argument("--allow-fallback", action="store_true", help="do not fail when the library selected another kernel variant than the expected one")
+    ap.add_argument("--ld-pad", type=int, default=-1, help="cells of padding behind the workload in every row (leading dimension = cells + pad); -1: the default of the workload")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
@@ -191,6 +192,11 @@ def main():
     n = args.cells or n_full
     C, T = qss_synth.config_states(cfg, n)
     n = min(n, C.shape[1]) if cfg == 4 else n
+    if args.ld_pad >= 0:        # the same states with another leading dimension (padding cells repeat cell 0)
+        ld2 = n + args.ld_pad
+        C2 = np.empty((C.shape[0], ld2)); T2 = np.empty(ld2)
+        C2[:, :n] = C[:, :n]; T2[:n] = T[:n]; C2[:, n:] = C[:, :1]; T2[n:] = T[0]
+        C, T = C2, T2
     ld = C.shape[1]
     t_create = time.perf_counter()
     qm = qss.QssMech(mech, local)            # includes the run-time specialisation of the Jacobian kernel (NVRTC), untimed below
@@ -201,6 +207,8 @@ def main():
     W = torch.empty((N, ld), dtype=torch.float64, device=dev)
     qm.workspace(True)
     stream = torch.cuda.current_stream()
+    if os.environ.get("QSS_BENCH_ADDR"):        # (diagnostic: device addresses of the buffers, for layout experiments)
+        print("addr", {k: hex(v.data_ptr()) for k, v in dict(C=Cd, T=Td, J=J, W=W, ws=qm.workspace(True)).items()}, "ld", ld, file=sys.stderr)
 
     qm.workspace(False)
     expect = EXPECTED_JAC_VARIANT.get(cfg)

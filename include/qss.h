@@ -181,10 +181,10 @@ int qss_newton_specialise_check(int n_species, int with_energy, int cc_major, in
  * holds until the process exits (its device address is taken once per device at qss_mech_create).  The call launches the general
  * slab kernel (kernel variant 0, whatever variant the handle selected for qss_eval_wdot) with as many persistent blocks as fit the
  * array, and calls no allocating routine.  Limit: a mechanism whose ONE-block workspace exceeds the array is rejected with
- * QSS_E_UNSUPPORTED (more than 131 072 doubles of per-cell workspace, roughly 30 000 reactions; the BASELINE configs need
+ * QSS_E_UNSUPPORTED (more than 32 768 doubles of per-cell workspace, roughly 7 000 reactions; the BASELINE configs need
  * 0.03-2.3 MB per block); any ncells is accepted.  Every call on a device shares the array: calls that overlap on the GPU (two streams, two handles, two threads) race;
  * order them on one stream.  Nothing in the array has to start at zero: the kernel writes every row before it reads it. */
-#define QSS_STATIC_SCRATCH_BYTES (32u << 20)
+#define QSS_STATIC_SCRATCH_BYTES (8u << 20)
 int qss_eval_wdot_static(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *C, const double *T, double *wdot,
                          double *cqss_or_null, void *stream);
 

@@ -359,7 +359,10 @@ cudaError_t qss_launch_dfma(int blocks, int iters, double *sink, cudaStream_t st
 // The kernel writes every workspace row of a slab before it reads it (the caller-supplied workspace of qss_eval_wdot is
 // uninitialised memory too), so nothing has to be cleared between calls; calls that overlap on the GPU share the array and race.
 // ---------------------------------------------------------------------------------------------------
-#define QSS_STATIC_SCRATCH_BYTES_ (32u << 20)
+#ifndef QSS_STATIC_MIB
+#define QSS_STATIC_MIB 8
+#endif
+#define QSS_STATIC_SCRATCH_BYTES_ ((unsigned)QSS_STATIC_MIB << 20)
 static __device__ __align__(256) unsigned char qss_static_scratch[QSS_STATIC_SCRATCH_BYTES_];
 
 namespace {

@@ -59,7 +59,7 @@ def test_static_workspace_entry_point_two_calls_in_a_row(monkeypatch):
     assert v1 == 3 and v2 == 3
     _check(2, 2048 + 19, "0", monkeypatch)                # calls 3, 4: against the same general kernel with a caller's workspace
     _check(3, 192 + 5, "0", monkeypatch)
-    _check(5, 64 + 3, None, monkeypatch)                  # the largest mechanism: 2.3 MB of workspace per block, 14 blocks fit
+    _check(5, 64 + 3, None, monkeypatch)                  # the largest mechanism: 2.3 MB of workspace per block, 3 blocks fit
 
 
 def test_static_workspace_rejects_bad_arguments():
