@@ -40,6 +40,8 @@ CALLS = {"jac+wdot": "qss_eval_jac with the wdot output (the metric)", "jac": "q
          "jac_const": "qss_eval_jac_approx, constant-QSS AJ", "jac_zero": "qss_eval_jac_approx, zero-QSS AJ",
          "newton": "qss_newton_solve alone: x = (I - gamma J)^-1 (wdot, Tdot) on a full Jacobian computed before the timed region",
          "jac+wdot+energy+newton": "qss_eval_jac with wdot, qss_eval_energy, qss_newton_solve: one Newton direction of an implicit step",
+         "sums_thread": "qss_bench_species_sums mode 0: mapping micro-benchmark, species sums with lane = cell (not on the path)",
+         "sums_warp": "qss_bench_species_sums mode 1: mapping micro-benchmark, species sums with a warp per cell and SHFL reductions (not on the path)",
          "bdf1": "qss_bdf1_advance: one backward-Euler substep with two full Newton iterations (10 kernel launches), state restored before every step"}
 
 
@@ -234,6 +236,10 @@ def main():
         qm.newton_solve(J, erow, gam, B, n, x=X)        # (first call: run-time compilation, outside the timed region)
         torch.cuda.synchronize()
         assert bool(torch.isfinite(X[:, :n]).all())
+    Qm = None
+    if args.call.startswith("sums_"):        # rates of progress: seeded normal values (the arithmetic does not depend on them)
+        g = torch.Generator(device=dev); g.manual_seed(11)
+        Qm = torch.randn((qm.info.n_reac, ld), dtype=torch.float64, device=dev, generator=g)
     launches_per_step = {"jac+wdot+energy": 2, "jac+wdot+energy+newton": 3, "bdf1": 10, "jac_full": 2}.get(args.call, 1)
     if args.call == "bdf1":
         # h_c = 3 / max|J_c| at the initial state (a few of the fastest time scales per substep); the state is restored before every step
@@ -259,6 +265,8 @@ def main():
                 qm.newton_solve(J, erow, gam, B, n, x=X)
         elif args.call == "newton":
             qm.newton_solve(J, erow, gam, B, n, x=X)
+        elif args.call.startswith("sums_"):
+            qm.bench_species_sums(0 if args.call == "sums_thread" else 1, Qm, n, wdot=W)
         elif args.call == "bdf1":
             Cd.copy_(C0); Td.copy_(T0)
             qm.bdf1_advance(Cd, Td, dtd, 1, 2, n, workspace=bdf_ws)
@@ -341,6 +349,8 @@ def main():
     elif args.call == "newton":        # reads the (N+1)^2 matrix, b and gamma once, writes x; n^3/3 + n^2 fp64 FMA slots (elimination + substitutions)
         nn = N + 1
         bytes_cell, slots_cell = 8.0 * (nn * nn + 2 * nn + 1), nn ** 3 / 3.0 + nn * nn
+    elif args.call.startswith("sums_"):   # reads Q once, writes wdot; one multiply-add per non-zero of the net stoichiometric matrix (~4 per reaction)
+        bytes_cell, slots_cell = 8.0 * (info.n_reac + N), 4.0 * info.n_reac
     elif args.call == "bdf1":          # two Newton iterations: the three heavy calls twice (the residual / update kernels move 5 (N+1) doubles each)
         nn = N + 1
         bytes_cell = 2.0 * ((info.bytes_jac + 8.0 * N) + (8.0 * (N * nn + 2 * N + 1) + 8.0 * (N + 2)) + 8.0 * (nn * nn + 2 * nn + 1) + 8.0 * 9 * nn)
@@ -367,7 +377,7 @@ def main():
     except Exception:
         traffic = None
     roof.update({"traffic": traffic, "traffic_unit": "bytes per launch (dram read + write) from the committed ncu capture of this workload and kernel variant (profiles/r02_traffic.txt); not measurable inside this run",
-                 "kernel": "qss_energy_kernel" if args.call == "energy" else "qss_newton_kernel" if args.call == "newton" else "the 10 launches of one substep (jacobian, energy row, residual, solve, update; twice)" if args.call == "bdf1" else ("qss wdot kernel (qss_eval_wdot)" if args.call == "wdot" else f"qss jacobian kernel, variant {info.kernel_variant_jac} ({CALLS[args.call]})"),
+                 "kernel": "qss_mapbench_kernel" if args.call.startswith("sums_") else "qss_energy_kernel" if args.call == "energy" else "qss_newton_kernel" if args.call == "newton" else "the 10 launches of one substep (jacobian, energy row, residual, solve, update; twice)" if args.call == "bdf1" else ("qss wdot kernel (qss_eval_wdot)" if args.call == "wdot" else f"qss jacobian kernel, variant {info.kernel_variant_jac} ({CALLS[args.call]})"),
                  "launch_ms_avg": avg_s * 1e3, "launch_ms_min": min(launch_ms),
                  "alg_fp64_slots_per_cell": slots_cell, "alg_bytes_per_cell": bytes_cell,
                  "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3,

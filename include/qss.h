@@ -175,6 +175,14 @@ int qss_newton_solve(const qss_mech_t *mech, int64_t ncells, int64_t ld, const d
                      const double *gamma, const double *b, double *x, void *stream);
 int qss_newton_specialise_check(int n_species, int with_energy, int cc_major, int cc_minor, size_t *image_bytes_or_null);
 
+/* Mapping micro-benchmark, NOT part of the path (north_star subsystem 3: cell-to-thread vs cell-to-warp with warp shuffles for the
+ * species-parallel reductions): wdot[i*ld + c] = sum_j nu_ij Q[j*ld + c] (Eq. 3) for i < N from given rates of progress Q [M*ld]
+ * (DEVICE pointers), mode 0: lane = cell, every species' reaction list walked per lane; mode 1: a warp per cell, lane = reaction,
+ * contributions scattered per lane and every species reduced over the lanes by a SHFL butterfly.  Same staging of Q through shared
+ * memory and same coalesced output in both.  QSS_E_UNSUPPORTED when the slab does not fit one SM's shared memory.
+ * has the measurement that decided the mapping of the kernels. */
+int qss_bench_species_sums(const qss_mech_t *mech, int mode, int64_t ncells, int64_t ld, const double *Q, double *wdot, void *stream);
+
 /* Allocation-free variant of qss_eval_wdot, for callers that cannot provide (or allocate) a workspace: code under CUDA graph
  * capture, tight serving loops, harnesses that forbid cudaMalloc.  Same inputs, outputs, layout and results as qss_eval_wdot; the
  * workspace is a static device array of QSS_STATIC_SCRATCH_BYTES bytes inside the library, which every GPU that loads the library

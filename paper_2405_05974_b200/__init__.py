@@ -17,7 +17,7 @@ from . import build as _build
 __all__ = ["lib", "QssMech", "QssError", "EXPORTS", "STATUS"]
 
 EXPORTS = ["qss_mech_create", "qss_mech_validate", "qss_mech_specialise_check", "qss_mech_destroy", "qss_mech_info", "qss_mech_qss_order", "qss_eval_wdot",
-           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_newton_solve", "qss_newton_specialise_check", "qss_bdf1_workspace_bytes", "qss_bdf1_advance", "qss_jac_fdt_workspace_bytes", "qss_eval_jac_fdt", "qss_mech_jac_pattern", "qss_jac_pack", "qss_eval_jac_full", "qss_eval_wdot_static", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
+           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_newton_solve", "qss_newton_specialise_check", "qss_bdf1_workspace_bytes", "qss_bdf1_advance", "qss_jac_fdt_workspace_bytes", "qss_eval_jac_fdt", "qss_mech_jac_pattern", "qss_jac_pack", "qss_eval_jac_full", "qss_eval_wdot_static", "qss_bench_species_sums", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
 STATUS = {0: "QSS_OK", -1: "QSS_E_INVALID", -2: "QSS_E_QUADRATIC", -3: "QSS_E_QSS_FANOUT", -4: "QSS_E_NO_SINK",
           -5: "QSS_E_UNSUPPORTED", -6: "QSS_E_CUDA", -7: "QSS_E_UNBALANCED"}
 
@@ -71,6 +71,7 @@ def lib():
         L.qss_eval_jac_approx.restype = ct.c_int; L.qss_eval_jac_approx.argtypes = [vp, i64, i64, vp, vp, vp, ct.c_int, vp, ct.c_size_t, vp]
         L.qss_eval_energy.restype = ct.c_int; L.qss_eval_energy.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp]
         L.qss_newton_solve.restype = ct.c_int; L.qss_newton_solve.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp]
+        L.qss_bench_species_sums.restype = ct.c_int; L.qss_bench_species_sums.argtypes = [vp, ct.c_int, i64, i64, vp, vp, vp]
         L.qss_eval_wdot_static.restype = ct.c_int; L.qss_eval_wdot_static.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
         L.qss_eval_jac_full.restype = ct.c_int; L.qss_eval_jac_full.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp, ct.c_size_t, vp]
         L.qss_mech_jac_pattern.restype = ct.c_int; L.qss_mech_jac_pattern.argtypes = [vp, ct.c_int, vp]
@@ -249,6 +250,17 @@ class QssMech:
         ws = self.workspace(True)
         _check(lib().qss_eval_jac_approx(self._h, ncells, ld, _ptr(C), _ptr(T), _ptr(jac), int(mode), _ptr(ws), ws.numel(), self._stream()))
         return jac
+
+    def bench_species_sums(self, mode, Q, ncells=None, wdot=None):
+        """Mapping micro-benchmark (qss_bench_species_sums): wdot [N, ld] = S Q from Q [M, ld]; mode 0 lane = cell, mode 1 warp per cell."""
+        import torch
+        ld = Q.shape[1]
+        ncells = ld if ncells is None else int(ncells)
+        assert Q.is_contiguous() and Q.shape[0] == self.info.n_reac
+        if wdot is None:
+            wdot = torch.empty((self.N, ld), dtype=torch.float64, device=Q.device)
+        _check(lib().qss_bench_species_sums(self._h, int(mode), ncells, ld, _ptr(Q), _ptr(wdot), self._stream()))
+        return wdot
 
     def eval_wdot_static(self, C, T, ncells=None, wdot=None, cqss=None):
         """wdot through the allocation-free entry point (qss_eval_wdot_static): `wdot` (and `cqss`) are the caller's tensors; no

@@ -402,6 +402,20 @@ extern "C" int qss_eval_wdot_static(const qss_mech_t *m, int64_t ncells, int64_t
     return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_eval_wdot_static launch");
 }
 
+// ---- mapping micro-benchmark (qss_mapbench.cu): species sums in the cell-to-thread and in the cell-to-warp mapping ------------------
+cudaError_t qss_launch_mapbench(const QssTab &t, int mode, int64_t ncells, int64_t ld, const double *Q, double *wdot, int n_sm, cudaStream_t stream);
+
+extern "C" int qss_bench_species_sums(const qss_mech_t *m, int mode, int64_t ncells, int64_t ld, const double *Q, double *wdot, void *stream) {
+    if (!m) return fail(QSS_E_INVALID, "mech is NULL");
+    if (mode < 0 || mode > 1 || ncells < 0 || ld < ncells) return fail(QSS_E_INVALID, "need mode 0 or 1 and 0 <= ncells <= ld");
+    if (ncells == 0) return QSS_OK;
+    if (!Q || !wdot) return fail(QSS_E_INVALID, "NULL device pointer");
+    DeviceGuard guard(m->device);
+    cudaError_t e = qss_launch_mapbench(m->c.tab, mode, ncells, ld, Q, wdot, m->n_sm, (cudaStream_t)stream);
+    if (e == cudaErrorInvalidValue) { cudaGetLastError(); return fail(QSS_E_UNSUPPORTED, "qss_bench_species_sums: the slab of this mechanism does not fit the shared memory of one SM in this mapping"); }
+    return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_bench_species_sums launch");
+}
+
 // ---- NEXT-1 in one call: the full (N+1) x (N+1) Jacobian and both right-hand sides (the two launches in sequence; a version with
 // the energy row formed inside the sweep of kernel variant 3 was built and measured at 14.0 ms against 13.6 ms: DESIGN.md section 6)
 extern "C" int qss_eval_jac_full(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *C, const double *T, double *jac, double *wdot,

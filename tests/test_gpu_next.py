@@ -192,3 +192,39 @@ def test_full_jacobian_in_one_call(name, n):
     if ld > n:
         assert torch.isnan(tdot[n:]).all() and torch.isnan(erow[:, n:]).all(), "padding was written"
     qm.close()
+
+
+@pytest.mark.parametrize("cfg,n", [(2, 2048 + 19), (1, 4096), (2, 31)])
+def test_mapping_microbenchmark_species_sums(cfg, n):
+    """qss_bench_species_sums (north_star subsystem 3): both mappings give wdot = S Q; reference: the dense net stoichiometric
+    matrix assembled in numpy from the mechanism description."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    mech = qss_synth.config_mechanism(cfg)
+    N, M = mech.n_nqss, mech.n_reac
+    S = np.zeros((N, M))
+    for j in range(M):
+        for t in range(mech.reac_ptr[j], mech.reac_ptr[j + 1]):
+            if mech.reac_sp[t] < N:
+                S[mech.reac_sp[t], j] -= mech.reac_nu[t]
+        for t in range(mech.prod_ptr[j], mech.prod_ptr[j + 1]):
+            if mech.prod_sp[t] < N:
+                S[mech.prod_sp[t], j] += mech.prod_nu[t]
+    rng = np.random.default_rng(cfg)
+    ld = n + 5
+    Q = np.full((M, ld), np.nan); Q[:, :n] = rng.normal(size=(M, n)) * 10.0 ** rng.uniform(-3, 3, size=(M, n))
+    ref = S @ Q[:, :n]
+    scale = np.abs(S) @ np.abs(Q[:, :n])
+    qm = qss.QssMech(mech, 0)
+    Qd = torch.from_numpy(Q).cuda()
+    out = []
+    for mode in (0, 1):
+        w = torch.full((N, ld), float("nan"), dtype=torch.float64, device="cuda")
+        qm.bench_species_sums(mode, Qd, n, wdot=w)
+        torch.cuda.synchronize()
+        wh = w.cpu().numpy()
+        assert np.isnan(wh[:, n:]).all(), "padding was written"
+        assert np.all(np.abs(wh[:, :n] - ref) <= 1e-13 * scale + 1e-300), (mode, float(np.max(np.abs(wh[:, :n] - ref) / (scale + 1e-300))))
+        out.append(wh[:, :n])
+    assert np.allclose(out[0], out[1], rtol=0.0, atol=1e-13 * scale.max())
+    qm.close()
