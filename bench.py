@@ -153,7 +153,8 @@ def main():
     ap.add_argument("--cells", type=int, default=0, help="override the cell count (0 = the config's)")
     ap.add_argument("--call", default="jac+wdot", choices=sorted(CALLS), help="which C-ABI call(s) a step is: " + "; ".join(f"{k}: {v}" for k, v in CALLS.items()))
     ap.add_argument("--allow-fallback", action="store_true", help="do not fail when the library selected another kernel variant than the expected one")
-    ap.add_argument("--ld-pad", type=int, default=-1, help="cells of padding behind the workload in every row (leading dimension = cells + pad); -1: the default of the workload")
+    ap.add_argument("--ld-pad", type=int, default=64, help="cells of padding behind the workload in every row (leading dimension = cells + pad; default 64: row strides that are "
+                    "powers of two are avoided, DESIGN.md section 5); -1: the leading dimension of the input generator")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
@@ -408,7 +409,7 @@ def main():
     print(json.dumps({
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic", "config": _config(cfg, mech, n, world),
+        "dtype": "f64", "data": "synthetic", "config": dict(_config(cfg, mech, n, world), call=args.call, ld=int(ld)),
         "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * launches_per_step, "roofline": roof, "cpu_baseline": cpu,
         "kernel_variant": {"wdot": info.kernel_variant_wdot, "jac": info.kernel_variant_jac}, "mech_create_s": t_create,
         "call": args.call}))

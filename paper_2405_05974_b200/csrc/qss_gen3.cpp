@@ -300,6 +300,11 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
         for (const Task &t : rsorted) { b2.push_back(t.type); b2.push_back(t.slot0); b2.push_back(t.c0); b2.push_back(t.c1); }
         for (const Task &t : nsorted) { d2.push_back(t.slot0); d2.push_back(t.c0); d2.push_back(t.c1); d2.push_back(0); }
         tput("T_RT_PTR", a2); tput("T_RT", b2); tput("T_NT_PTR", c2); tput("T_NT", d2);
+        // 2^(j/64), j = 0..63, for the table form of the exponential (qss_math.h qss_exp_tab): 64 doubles as 128 words, 8-byte aligned
+        while (tabw.size() % 2) tabw.push_back(0);
+        std::vector<int32_t> ex(128);
+        for (int j = 0; j < 64; ++j) { const double v = (double)exp2l((long double)j / 64.0L); std::memcpy(&ex[2 * j], &v, 8); }
+        tput("T_EXP", ex);
     }
     // ---- species sums: per species the added terms, then the subtracted terms, one table word (byte offset of the row) per
     //      unit of |nu| (two 16-bit row numbers per 32-bit word), each list padded to a multiple of four words with the row that stays zero; T_SS_PTR: the Q_j lists

@@ -15,6 +15,8 @@
 //   P6  species sums: wdot, T-column vector, third-body vector                           lane = cell
 //   P8  Jacobian columns: [W_x; G_x][:, k] in registers, dy/dx solve, W_y dy/dx (generated)   lane = cell, warp = column
 #include "qss_stdint.h"
+__device__ __forceinline__ double lds(unsigned a);
+#define QSS_EXP_TAB_LOAD(tab, j) lds((tab) + (unsigned)(j) * 8u)      // the table of qss_exp_tab stands in shared memory (tab: its shared-window address)
 #include "qss_math.h"
 #include "qss_v3.h"
 
@@ -82,7 +84,7 @@ __device__ __forceinline__ double vfms(double a, double b, double c) {      // a
 #endif
 
 #ifndef QSS3_X
-#define QSS3_X 2
+#define QSS3_X 66                // bit 1: Estrin form of qss_exp where it is still used; bit 6: table form of the exponential in the rate phases
 #endif
 #if QSS3_X & 2
 #define qss_exp qss_exp_e        // (its constants as operands from the constant bank instead of literals: measured, no gain)
@@ -132,17 +134,25 @@ struct RateTyped {
 
 // Rate constants of one reaction for ONE cell.  smc = shared-window address of cell c in row 0.
 //   dlnk = d ln k/dT at fixed M, dlnKc = d ln Kc/dT, dlm = d ln k/dM
+#if QSS3_X & 64
+#define QEXP(x) qss_exp_tab((x), smx)                                    // table form: 12 instead of 22 fp64 operations (qss_math.h)
+#define QEXP_SAT(x) qss_exp_tab(qss3_clamp_exp_arg(x), smx)
+#else
+#define QEXP(x) qss_exp(x)
+#define QEXP_SAT(x) qss_exp_sat(x)
+#endif
+__device__ __forceinline__ double qss3_clamp_exp_arg(double x) { return x < -746.0 ? -746.0 : (x > 710.0 ? 710.0 : x); }      // as qss_exp_sat: NaN stays NaN
 template <int TYPE>
 __device__ __forceinline__ void qss3_rate_cell(const RateCommon &r, const RateTyped &y, const double (&flo)[3], const double (&fhi)[3], const unsigned smc,
-                                               double &kf, double &kb, double &dlm, double &dlnk, double &dlnKc) {
+                                               const unsigned smx, double &kf, double &kb, double &dlm, double &dlnk, double &dlnKc) {
     const double T = lds(smc + R_T * G_PITCH), lnT = lds(smc + R_LNT * G_PITCH), invT = lds(smc + R_INVT * G_PITCH);
     const double lnkinf = fma(-r.EaR, invT, fma(r.beta, lnT, r.lnA));
     const bool lo = T < r.tmid;                                  // NASA-7 range (reading G9: T < Tmid low, else high)
     const double e0 = lo ? r.elo[0] : r.ehi[0], e1 = lo ? r.elo[1] : r.ehi[1], e2 = lo ? r.elo[2] : r.ehi[2], e3 = lo ? r.elo[3] : r.ehi[3];
     const double e4 = lo ? r.elo[4] : r.ehi[4], e5 = lo ? r.elo[5] : r.ehi[5], e6 = lo ? r.elo[6] : r.ehi[6];
     const double lniKc = fma(e6, invT, fma(e1, lnT, fma(T, fma(T, fma(T, fma(T, e5, e4), e3), e2), e0)));     // -ln Kc
-    double k = qss_exp(lnkinf);
-    const double iKc = qss_exp(lniKc);
+    double k = QEXP(lnkinf);
+    const double iKc = QEXP(lniKc);
 #if QSS3_JAC
     // T d ln Kc/dT = sum nu h/RT - dnu = e6/T - e1 - T (e2 + T (2 e3 + T (3 e4 + 4 e5 T)))   (e: coefficients of -ln Kc)
     const double f3 = lo ? flo[0] : fhi[0], f4 = lo ? flo[1] : fhi[1], f5 = lo ? flo[2] : fhi[2];
@@ -163,9 +173,9 @@ __device__ __forceinline__ void qss3_rate_cell(const RateCommon &r, const RateTy
             const double dlnkinf = (r.beta + r.EaR * invT) * invT;
             const double lnk0 = fma(-y.E0R, invT, fma(y.beta0, lnT, y.lnA0));
             const double dlnk0 = (y.beta0 + y.E0R * invT) * invT;
-            const double Pr = qss_exp(lnk0 - lnkinf) * Mc;
+            const double Pr = QEXP(lnk0 - lnkinf) * Mc;
             const double al = y.alpha;
-            const double x3 = qss_exp_sat(-T * y.i3), x1 = qss_exp_sat(-T * y.i1), x2 = qss_exp_sat(-y.T2s * invT);
+            const double x3 = QEXP_SAT(-T * y.i3), x1 = QEXP_SAT(-T * y.i1), x2 = QEXP_SAT(-y.T2s * invT);
             const double Fc = (1.0 - al) * x3 + al * x1 + x2;
             const double L = log(Pr) * kInvLn10, Lc = log(Fc) * kInvLn10;
             const double cc = -0.4 - 0.67 * Lc, n = 0.75 - 1.27 * Lc;
@@ -173,7 +183,7 @@ __device__ __forceinline__ void qss3_rate_cell(const RateCommon &r, const RateTy
             const double iden = qss_rcp(den);
             const double f1 = num * iden;
             const double ione_f = qss_rcp(1.0 + f1 * f1);
-            const double F = qss_exp(kLn10 * Lc * ione_f);
+            const double F = QEXP(kLn10 * Lc * ione_f);
             const double i1pr = qss_rcp(1.0 + Pr);
             k = k * (Pr * i1pr) * F;
             const double df1_dL = n * iden * iden;
@@ -216,7 +226,7 @@ __device__ __forceinline__ void qss3_rate_task(const RateCommon &r, const int sl
     for (int c = c0; c < c1; c += STEP) {
         double kf[STEP], kb[STEP], dm[STEP], dk[STEP], dz[STEP];
 #pragma unroll
-        for (int u = 0; u < STEP; ++u) qss3_rate_cell<TYPE>(r, y, flo, fhi, sm0 + (c + u) * 8, kf[u], kb[u], dm[u], dk[u], dz[u]);
+        for (int u = 0; u < STEP; ++u) qss3_rate_cell<TYPE>(r, y, flo, fhi, sm0 + (c + u) * 8, sm0 + R_TAB * G_PITCH + T_EXP * 4, kf[u], kb[u], dm[u], dk[u], dz[u]);
         if (valid) {
 #pragma unroll
             for (int u = 0; u < STEP; ++u) {

@@ -123,4 +123,36 @@ QSS_HD double qss_rcp(double x) {
 #endif
 }
 
+// The same function with a table of 2^(j/64), j = 0..63: exp(x) = 2^k 2^(j/64) exp(r), |r| <= ln2/128, exp(r) by a polynomial of
+// degree 5 (truncation 3.5e-17): 12 fp64 operations instead of 22.  `tab` is whatever QSS_EXP_TAB_LOAD reads element j from (a
+// pointer by default; the kernels define the macro as a shared-memory read).  Valid for |x| < 2^24 like qss_exp; max error 1 ulp.
+#ifndef QSS_EXP_TAB_LOAD
+#define QSS_EXP_TAB_LOAD(tab, j) ((tab)[j])
+#endif
+template <class TAB>
+QSS_HD double qss_exp_tab(double x, TAB tab) {
+    const double kShift = 6755399441055744.0;                 // 1.5 * 2^52
+    const double k64L2E = 92.33248261689366;                  // 64 / ln 2
+    const double kHi = 0.01083042469326756;                   // ln 2 / 64, 32 significant bits (n kHi is exact for |n| < 2^20)
+    const double kLo = 2.9815858269852933e-12;
+    const double t = fma(x, k64L2E, kShift);
+#ifdef __CUDA_ARCH__
+    int n = __double2loint(t);
+#else
+    uint64_t tb;
+    memcpy(&tb, &t, 8);
+    int n = (int)(uint32_t)tb;
+#endif
+    const double nf = t - kShift;
+    double r = fma(nf, -kHi, x);
+    r = fma(nf, -kLo, r);
+    const double r2 = r * r;
+    const double a1 = fma(r, 1.6666666666666666e-01, 0.5), a2 = fma(r, 8.333333333333333e-03, 4.1666666666666664e-02);
+    const double p = fma(fma(a2, r2, a1), r2, r);              // exp(r) - 1
+    n = n < -128000 ? -128000 : (n > 128000 ? 128000 : n);     // keeps both exponent fields valid for any finite x
+    const double tj = QSS_EXP_TAB_LOAD(tab, n & 63);
+    const int k = n >> 6, k1 = k >> 1, k2 = k - k1;
+    return fma(tj, p, tj) * qss_pow2_factor(k1) * qss_pow2_factor(k2);
+}
+
 #endif

@@ -169,7 +169,8 @@ def test_branch_free_exp_against_float128(tmp_path):
 #include <random>
 #include <quadmath.h>
 int main() {
-  std::mt19937_64 g(1); double worst = 0, worst_e = 0;
+  std::mt19937_64 g(1); double worst = 0, worst_e = 0, worst_t = 0;
+  double tab[64]; for (int j = 0; j < 64; ++j) tab[j] = (double)exp2l((long double)j / 64.0L);      // as csrc/qss_gen3.cpp writes it
   std::uniform_real_distribution<double> u(-745.0, 709.0), s(-1.0, 1.0);
   for (int i = 0; i < 2000000; ++i) {
     double x = (i & 1) ? u(g) : s(g), a = qss_exp(x), b = qss_exp_e(x); __float128 r = expq((__float128)x); double rd = (double)r;
@@ -178,19 +179,24 @@ int main() {
     if (e > worst) worst = e;
     e = (double)fabsq((__float128)b - r) / ulp;
     if (e > worst_e) worst_e = e;
+    e = (double)fabsq((__float128)qss_exp_tab(x, (const double *)tab) - r) / ulp;
+    if (e > worst_t) worst_t = e;
   }
+  const int tab_ok = qss_exp_tab(0.0, (const double *)tab) == 1.0 && qss_exp_tab(-1000.0, (const double *)tab) == 0.0 && std::isinf(qss_exp_tab(1000.0, (const double *)tab)) &&
+                     qss_exp_tab(-746.0, (const double *)tab) == 0.0 && std::isinf(qss_exp_tab(710.0, (const double *)tab));
   // saturating form for placeholder arguments (fall-off temperatures 1e-30 / 1e30): 0, 1 and inf like the library function
   const int sat = qss_exp_sat(-1.4e33) == 0.0 && qss_exp_sat(-1e27) == 0.0 && qss_exp_sat(-2e9) == 0.0 && qss_exp_sat(-1.4e-27) == 1.0 &&
                   std::isinf(qss_exp_sat(1e12)) && qss_exp_sat(-INFINITY) == 0.0 && qss_exp_sat(0.5) == qss_exp(0.5);
-  printf("%.4f %d %d %d %.4f %d\n", worst, qss_exp(0.0) == 1.0, qss_exp(-1000.0) == 0.0, std::isinf(qss_exp(1000.0)), worst_e, sat);
+  printf("%.4f %d %d %d %.4f %d %.4f %d\n", worst, qss_exp(0.0) == 1.0, qss_exp(-1000.0) == 0.0, std::isinf(qss_exp(1000.0)), worst_e, sat, worst_t, tab_ok);
 }''')
     exe = tmp_path / "t"
     subprocess.run(["g++", "-O2", "-ffp-contract=off", "-I", os.path.join(ROOT, "paper_2405_05974_b200", "csrc"), "-o", str(exe),
                     str(src), "-lquadmath"], check=True)
-    worst, one, zero, inf, worst_e, sat = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()
+    worst, one, zero, inf, worst_e, sat, worst_t, tab_ok = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()
     assert float(worst) <= 1.5 and one == "1" and zero == "1" and inf == "1"
     assert float(worst_e) <= 2.5, worst_e            # Estrin form of the polynomial (kernel variant 3)
     assert sat == "1"
+    assert float(worst_t) <= 1.5 and tab_ok == "1", (worst_t, tab_ok)            # table form (kernel variant 3's rate phase)
 
 
 def test_cell_ranges_tile_the_cells():
