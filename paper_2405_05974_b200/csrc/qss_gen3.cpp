@@ -219,7 +219,7 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
     std::vector<Task> rsorted, nsorted;
     std::vector<int> rptr, nptr;
     {
-        double rate_cost[3] = {130.0, 240.0, 900.0};      // per cell and group, fitted to the measured per-warp times
+        double rate_cost[3] = {130.0, 200.0, 700.0};      // per cell and group, fitted to the measured per-warp times (with the table exponential)
         const double net_cost[3] = {1.0, 1.1, 1.1};
         if (const char *e = qss_devenv("QSS3_W")) std::sscanf(e, "%lf,%lf,%lf", &rate_cost[0], &rate_cost[1], &rate_cost[2]);
         partition(rate_cost, 2, rsorted, rptr);
