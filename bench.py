@@ -42,7 +42,7 @@ CALLS = {"jac+wdot": "qss_eval_jac with the wdot output (the metric)", "jac": "q
          "jac+wdot+energy+newton": "qss_eval_jac with wdot, qss_eval_energy, qss_newton_solve: one Newton direction of an implicit step",
          "sums_thread": "qss_bench_species_sums mode 0: mapping micro-benchmark, species sums with lane = cell (not on the path)",
          "sums_warp": "qss_bench_species_sums mode 1: mapping micro-benchmark, species sums with a warp per cell and SHFL reductions (not on the path)",
-         "bdf1": "qss_bdf1_advance: one backward-Euler substep with two full Newton iterations (10 kernel launches), state restored before every step"}
+         "bdf1": "qss_bdf1_advance: one backward-Euler substep with two full Newton iterations (two kernels each: Jacobian, fused Newton step), state restored before every step"}
 
 
 def _peaks():
@@ -241,7 +241,7 @@ def main():
     if args.call.startswith("sums_"):        # rates of progress: seeded normal values (the arithmetic does not depend on them)
         g = torch.Generator(device=dev); g.manual_seed(11)
         Qm = torch.randn((qm.info.n_reac, ld), dtype=torch.float64, device=dev, generator=g)
-    launches_per_step = {"jac+wdot+energy": 2, "jac+wdot+energy+newton": 3, "bdf1": 10, "jac_full": 2}.get(args.call, 1)
+    launches_per_step = {"jac+wdot+energy": 2, "jac+wdot+energy+newton": 3, "bdf1": 4, "jac_full": 2}.get(args.call, 1)
     if args.call == "bdf1":
         # h_c = 3 / max|J_c| at the initial state (a few of the fastest time scales per substep); the state is restored before every step
         del J
@@ -378,7 +378,7 @@ def main():
     except Exception:
         traffic = None
     roof.update({"traffic": traffic, "traffic_unit": "bytes per launch (dram read + write) from the committed ncu capture of this workload and kernel variant (profiles/r02_traffic.txt); not measurable inside this run",
-                 "kernel": "qss_mapbench_kernel" if args.call.startswith("sums_") else "qss_energy_kernel" if args.call == "energy" else "qss_newton_kernel" if args.call == "newton" else "the 10 launches of one substep (jacobian, energy row, residual, solve, update; twice)" if args.call == "bdf1" else ("qss wdot kernel (qss_eval_wdot)" if args.call == "wdot" else f"qss jacobian kernel, variant {info.kernel_variant_jac} ({CALLS[args.call]})"),
+                 "kernel": "qss_mapbench_kernel" if args.call.startswith("sums_") else "qss_energy_kernel" if args.call == "energy" else "qss_newton_kernel" if args.call == "newton" else "the 4 launches of one substep (Jacobian kernel, fused Newton step; twice)" if args.call == "bdf1" else ("qss wdot kernel (qss_eval_wdot)" if args.call == "wdot" else f"qss jacobian kernel, variant {info.kernel_variant_jac} ({CALLS[args.call]})"),
                  "launch_ms_avg": avg_s * 1e3, "launch_ms_min": min(launch_ms),
                  "alg_fp64_slots_per_cell": slots_cell, "alg_bytes_per_cell": bytes_cell,
                  "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3,

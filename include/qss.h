@@ -232,9 +232,11 @@ int qss_eval_jac_fdt(const qss_mech_t *mech, int64_t ncells, int64_t ld, const d
  * `newton_iters` full Newton iterations with the exact (N+1) x (N+1) Jacobian re-evaluated in every iteration:
  *     phi = (C, T), f = (wdot, Tdot);  F(phi_m) = phi_m - phi^n - h f(phi_m);  (I - h J(phi_m)) delta = -F(phi_m);
  *     phi_{m+1} = phi_m + delta, C := max(C, 0)
- * No step-size control and no convergence test: the launch sequence is fixed (5 kernels per Newton iteration: qss_eval_jac,
+ * No step-size control and no convergence test: the launch sequence is fixed (2 kernels per Newton iteration: the Jacobian kernel,
+ * then ONE kernel that forms the energy row and the right-hand side in shared memory, solves and updates (C, T) in place -- neither
+ * the energy row nor the right-hand side reaches HBM; without run-time compilation of that kernel the five calls qss_eval_jac,
  * qss_eval_energy, residual, qss_newton_solve, update; 2 copies per substep), nothing synchronises, and the call can be captured
- * in a CUDA graph after one warm-up call (run-time compilation of the solve).  C [N*ld] and T [ld] are updated IN PLACE (DEVICE
+ * in a CUDA graph after one warm-up call (run-time compilation).  C [N*ld] and T [ld] are updated IN PLACE (DEVICE
  * pointers, 16-byte aligned, ld even); dt [ncells]; `workspace`: qss_bdf1_workspace_bytes(mech, ld) bytes of device memory, 256-byte
  * aligned (holds the Jacobian: 8 N (N+1) ld bytes).  N + 1 <= 40 (limit of qss_newton_solve). */
 size_t qss_bdf1_workspace_bytes(const qss_mech_t *mech, int64_t ld);

@@ -51,6 +51,9 @@ struct qss_mech {
     int cc_major = 0, cc_minor = 0;
     bool static_scratch_ok = false;   // qss_static_scratch_setup succeeded on this device
     mutable int newton_blocks[2] = {0, 0};            //   persistent blocks of that kernel (SMs x resident blocks per SM)
+    mutable QssJit *newton_step = nullptr;            // qss_bdf1_advance: the fused Newton step (energy row, right-hand side, solve, update), built on first use
+    mutable int newton_step_blocks = 0;
+    mutable bool newton_step_tried = false;
     mutable QssJit *newton[2] = {nullptr, nullptr};   // qss_newton_solve: [0] species block (n = N), [1] with the energy row (n = N + 1); built on first use
 };
 
@@ -224,6 +227,7 @@ extern "C" int qss_mech_destroy(qss_mech_t *m) {
     qss_jit_destroy(m->jit);
     qss_jit_destroy(m->jit3);
     qss_jit_destroy(m->jit3w);
+    qss_jit_destroy(m->newton_step);
     qss_jit_destroy(m->newton[0]);
     qss_jit_destroy(m->newton[1]);
     cudaFree(m->dP3); cudaFree(m->iP3);
@@ -521,11 +525,30 @@ extern "C" int qss_bdf1_advance(const qss_mech_t *m, int64_t ncells, int64_t ld,
     double *jac = take((size_t)N * (N + 1)), *F = take(N + 1), *erow = take(N + 1), *phin = take(N + 1), *b = take(N + 1);
     void *ws = (void *)(((uintptr_t)p + 255) & ~(uintptr_t)255);
     const size_t wsb = ws_bytes(m, true);
+    QssJit *step = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(m->host_mu);
+        if (!m->newton_step_tried) {
+            m->newton_step_tried = true;
+            std::string jerr;
+            if (!qss_devenv("QSS_BDF1_UNFUSED")) m->newton_step = qss_jit_newton_step_create(N + 1, N + 1, QSS_NEWTON_CPB, m->cc_major, m->cc_minor, jerr);
+            if (m->newton_step) m->newton_step_blocks = m->n_sm * qss_jit_newton_step_blocks_per_sm(m->newton_step, N + 1, QSS_NEWTON_CPB);
+            else if (qss_devenv("QSS_DEBUG")) std::fprintf(stderr, "[qss] fused Newton step unavailable: %s\n", jerr.c_str());
+        }
+        step = m->newton_step;      // NULL: the five-launch sequence below (same arithmetic up to the summation order of the energy row)
+    }
     for (int s = 0; s < nsub; ++s) {
         cudaError_t e = cudaMemcpyAsync(phin, C, (size_t)N * nrow * sizeof(double), cudaMemcpyDeviceToDevice, st);
         if (e == cudaSuccess) e = cudaMemcpyAsync(phin + (size_t)N * nrow, T, nrow * sizeof(double), cudaMemcpyDeviceToDevice, st);
         if (e != cudaSuccess) return cuda_fail(e, "qss_bdf1_advance: saving the state");
         for (int it = 0; it < newton_iters; ++it) {
+            if (step) {      // two launches per iteration: the Jacobian kernel (J, wdot), then energy row + right-hand side + solve + update in one kernel
+                int rc = eval_jac_mode(m, ncells, ld, C, T, jac, F, 0, ws, wsb, stream);
+                if (rc != QSS_OK) return rc;
+                e = qss_jit_newton_step_launch(step, N + 1, QSS_NEWTON_CPB, m->newton_step_blocks, jac, F, phin, dt, m->dD + m->c.tab.d_thermo, C, T, ncells, ld, st);
+                if (e != cudaSuccess) return cuda_fail(e, "qss_bdf1_advance: fused Newton step");
+                continue;
+            }
             int rc = qss_eval_jac_full(m, ncells, ld, C, T, jac, F, F + (size_t)N * nrow, erow, ws, wsb, stream);      // J, wdot -> F[0..N-1], Tdot -> F[N], energy row
             if (rc != QSS_OK) return rc;
             e = qss_launch_bdf1_residual(N, ncells, ld, C, T, phin, F, dt, b, st);

@@ -298,6 +298,42 @@ cudaError_t qss_jit_newton_launch(const QssJit *j, int n, int cpb, int max_block
     return cudaLaunchKernel(reinterpret_cast<const void *>(j->kernel), dim3((unsigned)grid), dim3(newton_threads(n, cpb)), args, qss_jit_newton_smem(n, cpb), stream);
 }
 
+// ---- fused Newton step (qss_newton_step_kernel) ----------------------------------------------------------------------------
+namespace {
+struct QssStepArgs {            // = struct QssStep of qss_newton_kernel.cu
+    const double *jac, *wdot, *phin, *dt, *thermo;
+    double *C, *T;
+    int64_t ncells, ld;
+};
+}  // namespace
+
+QssJit *qss_jit_newton_step_create(int n, int nj, int cpb, int cc_major, int cc_minor, std::string &err) {
+    if (newton_packed()) { err = "the fused step exists for the warp-per-cell mapping only"; return nullptr; }
+    std::shared_ptr<std::vector<char>> bin = compile("qss_newton_kernel.cu", "qss_newton_gen.h", newton_gen(n, nj, true, cpb), {}, arch_of(cc_major, cc_minor), err);
+    return bin ? load_image(*bin, "qss_newton_step_kernel", err) : nullptr;
+}
+
+size_t qss_jit_newton_step_smem(int n, int cpb) {
+    const size_t nc = (size_t)n + 1, pitch = nc | 1, ub = (nc + 4) & ~(size_t)1, N = (size_t)n - 1, aux = 3 * N + 2;
+    return ((size_t)2 * cpb * n * pitch + (size_t)2 * cpb * aux + (size_t)cpb * 2 * ub + (size_t)cpb * n + (size_t)cpb * 2 * N) * sizeof(double) + (size_t)cpb * n * sizeof(int);
+}
+
+int qss_jit_newton_step_blocks_per_sm(const QssJit *j, int n, int cpb) {
+    int nb = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, reinterpret_cast<const void *>(j->kernel), 32 * cpb, qss_jit_newton_step_smem(n, cpb)) != cudaSuccess) { cudaGetLastError(); nb = 1; }
+    return nb < 1 ? 1 : nb;
+}
+
+cudaError_t qss_jit_newton_step_launch(const QssJit *j, int n, int cpb, int max_blocks, const double *jac, const double *wdot, const double *phin,
+                                       const double *dt, const double *thermo, double *C, double *T, int64_t ncells, int64_t ld, cudaStream_t stream) {
+    if (ncells == 0) return cudaSuccess;
+    QssStepArgs a = {jac, wdot, phin, dt, thermo, C, T, ncells, ld};
+    void *args[] = {&a};
+    const int64_t ntiles = (ncells + cpb - 1) / cpb;
+    const int64_t grid = ntiles < max_blocks ? ntiles : max_blocks;
+    return cudaLaunchKernel(reinterpret_cast<const void *>(j->kernel), dim3((unsigned)grid), dim3(32 * cpb), args, qss_jit_newton_step_smem(n, cpb), stream);
+}
+
 void qss_jit_destroy(QssJit *j) {
     if (!j) return;
     if (j->lib) cudaLibraryUnload(j->lib);

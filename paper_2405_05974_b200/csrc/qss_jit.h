@@ -36,6 +36,13 @@ QssJit *qss_jit_newton_create(int n, int nj, bool has_e, int cpb, int cc_major, 
 bool qss_jit_newton_compile_only(int n, int nj, bool has_e, int cpb, int cc_major, int cc_minor, size_t *image_bytes, std::string &err);
 size_t qss_jit_newton_smem(int n, int cpb);
 int qss_jit_newton_blocks_per_sm(const QssJit *j, int n, int cpb);
+// One Newton iteration of qss_bdf1_advance behind the Jacobian kernel (qss_newton_step_kernel of the same image, n = N + 1 only): energy row,
+// right-hand side, solve and update of (C, T) in place.  thermo: device NASA-7 table of the transported species ([N][24], qss_tables.h).
+QssJit *qss_jit_newton_step_create(int n, int nj, int cpb, int cc_major, int cc_minor, std::string &err);
+size_t qss_jit_newton_step_smem(int n, int cpb);
+int qss_jit_newton_step_blocks_per_sm(const QssJit *j, int n, int cpb);
+cudaError_t qss_jit_newton_step_launch(const QssJit *j, int n, int cpb, int max_blocks, const double *jac, const double *wdot, const double *phin,
+                                       const double *dt, const double *thermo, double *C, double *T, int64_t ncells, int64_t ld, cudaStream_t stream);
 cudaError_t qss_jit_newton_launch(const QssJit *j, int n, int cpb, int max_blocks, const double *jac, const double *erow, const double *gamma,
                                   const double *b, double *x, int64_t ncells, int64_t ld, cudaStream_t stream);
 
