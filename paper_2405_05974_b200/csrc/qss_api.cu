@@ -35,8 +35,9 @@ struct qss_mech {
     int n_sm = 0;
     int32_t *dI = nullptr;
     double *dD = nullptr;
-    int nwarp = 8;            // warps per block of the slab kernel
-    int blocks_per_sm = 4;    // general kernel: 4 x 8 warps per SM (64 registers); measured 193 -> 123 ms on cfg3 vs 2 blocks
+    int nwarp = 32;           // warps per block of the general slab kernel
+    int blocks_per_sm = 1;    // general kernel: 1 x 32 warps per SM (64 registers): a quarter of the workspace slabs in flight; measured on cfg3 /
+                              // cfg5: 108.8 / 306.9 ms against 122.6 / 324.7 ms with 4 blocks of 8 warps (193 ms with 2 x 8)
     int nblocks = 0;
     cudaStream_t copy_stream = nullptr;   // qss_eval_jac_host: device-to-host copies overlap the next chunk's kernel (created with the handle)
     mutable std::mutex host_mu;           // qss_eval_jac_host calls on one handle are serialised (they share copy_stream and the event)
@@ -116,6 +117,7 @@ extern "C" int qss_mech_create(const qss_mech_desc_t *desc, int device, qss_mech
     m->static_scratch_ok = qss_static_scratch_setup(device) == cudaSuccess;      // address of the static workspace of qss_eval_wdot_static (no allocation)
     if (!m->static_scratch_ok) cudaGetLastError();
     if (const char *bps = qss_devenv("QSS_V0_BLOCKS_PER_SM")) m->blocks_per_sm = std::max(1, std::atoi(bps));   // tuning aid for the general kernel
+    if (const char *nw = qss_devenv("QSS_V0_NWARP")) m->nwarp = std::max(1, std::min(32, std::atoi(nw)));
     m->nblocks = m->n_sm * m->blocks_per_sm;
     const size_t nI = m->c.I.size() ? m->c.I.size() : 1, nD = m->c.D.size() ? m->c.D.size() : 1;
     if ((e = cudaMalloc(&m->dI, nI * sizeof(int32_t))) != cudaSuccess) { delete m; return cuda_fail(e, "cudaMalloc(tables)"); }

@@ -170,7 +170,7 @@ __device__ __forceinline__ void closure_group(const QssTab &t, const CellCtx &cx
 }
 
 template <bool JAC>
-__global__ void __launch_bounds__(256) qss_slab_kernel(const QssTab t, const int64_t ncells, const int64_t ld,
+__global__ void __launch_bounds__(1024) qss_slab_kernel(const QssTab t, const int64_t ncells, const int64_t ld,
                                                        const double *__restrict__ C, const double *__restrict__ Tin,
                                                        double *__restrict__ wdot, double *__restrict__ cqss,
                                                        double *__restrict__ jac, double *__restrict__ wsbase,
