@@ -1,4 +1,4 @@
-"""Mechanism front-end (second half): CHEMKIN-format text -> the flat description `qss_mech_create` takes, and
+"""Mechanism front-end (second half): CHEMKIN-format or Cantera-YAML-format text -> the flat description `qss_mech_create` takes, and
 the three linearisation methods of PAPER.md section 2.2 (L77-122, Algorithm 1) that make a QSS choice admissible for the
 algebraic closure.  Host logic only (numpy); nothing here runs on the path.
 
@@ -222,6 +222,26 @@ def _side(text: str, species: Sequence[str], eq: str):
     return out, has_m
 
 
+def _equation(eq: str, species: Sequence[str]):
+    """`A+B(+M)<=>C(+M)` -> (reactants, products, reversible, third body `+ M`, fall-off `(+M)`)."""
+    body = eq.replace(" ", "").upper()
+    falloff = "(+M)" in body
+    if re.search(r"\(\+[^M)]", body) or re.search(r"\(\+M[^)]", body):
+        raise MechanismError(f"{eq}: explicit collision partners are not read")
+    body = body.replace("(+M)", "")
+    if "<=>" in body: lhs, rhs, rev = *body.split("<=>", 1), True
+    elif "=>" in body: lhs, rhs, rev = *body.split("=>", 1), False
+    elif "=" in body: lhs, rhs, rev = *body.split("=", 1), True
+    else: raise MechanismError(f"{eq}: no '=' in the reaction")
+    re_, m1 = _side(lhs, species, eq)
+    pr_, m2 = _side(rhs, species, eq)
+    if m1 != m2:
+        raise MechanismError(f"{eq}: M on one side only")
+    if falloff and m1:
+        raise MechanismError(f"{eq}: both +M and (+M)")
+    return re_, pr_, rev, m1, falloff
+
+
 def _reactions(lines: Sequence[str], species: Sequence[str]):
     e_unit, header = CAL, " ".join(ln.replace("\0HEADER", "") for ln in lines if ln.startswith("\0HEADER")).upper().split()
     for tok in header:
@@ -267,23 +287,9 @@ def _reactions(lines: Sequence[str], species: Sequence[str]):
         except ValueError:
             raise MechanismError(f"cannot read the rate parameters of {ln!r}")
         eq = "".join(f[:-3])
-        body = eq.upper()
-        falloff = "(+M)" in body
-        if re.search(r"\(\+[^M)]", body) or re.search(r"\(\+M[^)]", body):
-            raise MechanismError(f"{eq}: explicit collision partners are not read")
-        body = body.replace("(+M)", "")
-        if "<=>" in body: lhs, rhs, rev = *body.split("<=>", 1), True
-        elif "=>" in body: lhs, rhs, rev = *body.split("=>", 1), False
-        elif "=" in body: lhs, rhs, rev = *body.split("=", 1), True
-        else: raise MechanismError(f"{eq}: no '=' in the reaction")
-        re_, m1 = _side(lhs, species, eq)
-        pr_, m2 = _side(rhs, species, eq)
-        if m1 != m2:
-            raise MechanismError(f"{eq}: M on one side only")
-        if falloff and m1:
-            raise MechanismError(f"{eq}: both +M and (+M)")
+        re_, pr_, rev, m1, falloff = _equation(eq, species)
         recs.append(dict(eq=eq, reac=re_, prod=pr_, rev=rev, type=2 if falloff else (1 if m1 else 0), A=A, beta=beta, Ea=Ea * e_unit,
-                         low=None, troe=None, eff=[], e_unit=e_unit))
+                         low=None, troe=None, eff=[], e_unit=e_unit, vol_unit=1e-6))
     for r in recs:
         if r["type"] == 2 and (r["low"] is None or r["troe"] is None):
             raise MechanismError(f"{r['eq']}: a fall-off reaction needs LOW and TROE (Lindemann form is not read)")
@@ -312,6 +318,12 @@ def parse_chemkin(text: str, qss: Sequence[str] = ()) -> MechanismDescription:
             raise MechanismError(f"QSS species {q} is not in SPECIES")
     thermo = _thermo(sec["THERMO"], names, elements)
     recs = _reactions(sec["REACTIONS"], names)
+    return _assemble(elements, names, qset, thermo, recs)
+
+
+def _assemble(elements, names, qset, thermo, recs) -> MechanismDescription:
+    """Flat description from parsed parts.  thermo[name] = (composition dict, (Tlow, Tmid, Thigh), a_low[7], a_high[7]); a reaction record
+    carries A in (vol_unit m^3 per quantity)^(order - 1) / s and activation energies already multiplied into J/mol where noted."""
     order = [s for s in names if s not in qset] + [s for s in names if s in qset]       # file order inside each class
     new_of = {names.index(s): i for i, s in enumerate(order)}
     N, Nq, M = len(names) - len(qset), len(qset), len(recs)
@@ -334,9 +346,9 @@ def parse_chemkin(text: str, qss: Sequence[str] = ()) -> MechanismDescription:
         rtype[j] = r["type"]; mask[j] = 3 if r["rev"] else 1
         # cm^3-mol-s -> m^3-mol-s: a rate constant of order n carries (cm^3/mol)^(n-1); a third body adds one order; the
         # fall-off limits: k_inf order n, k_0 order n + 1
-        arr[j] = (r["A"] * 1e-6 ** (order_f - 1 + (1 if r["type"] == 1 else 0)), r["beta"], r["Ea"])
+        arr[j] = (r["A"] * r["vol_unit"] ** (order_f - 1 + (1 if r["type"] == 1 else 0)), r["beta"], r["Ea"])
         if r["type"] == 2:
-            low[j] = (r["low"][0] * 1e-6 ** order_f, r["low"][1], r["low"][2] * r["e_unit"])
+            low[j] = (r["low"][0] * r["vol_unit"] ** order_f, r["low"][1], r["low"][2] * r["e_unit"])
             t4 = list(r["troe"]) + ([1e30] if len(r["troe"]) == 3 else [])
             troe[j] = t4
         for sp_, val in r["eff"]:
@@ -351,6 +363,120 @@ def parse_chemkin(text: str, qss: Sequence[str] = ()) -> MechanismDescription:
         nasa_T=nT, nasa_lo=lo, nasa_hi=hi, rtype=rtype, dir_mask=mask, reac_ptr=i32(rp), reac_sp=i32(rs), reac_nu=i32(rn),
         prod_ptr=i32(pp), prod_sp=i32(ps), prod_nu=i32(pn), arr=arr, arr_low=low, troe=troe, eff_ptr=i32(ep), eff_sp=i32(es),
         eff_val=np.asarray(ev, dtype=np.float64), species=order, elements=list(elements), equations=[r["eq"] for r in recs], warnings=warnings)
+
+
+# ---------------------------------------------------------------------------------------------------------------------------
+# Cantera-YAML-format text (the subset that matches the CHEMKIN subset above)
+# ---------------------------------------------------------------------------------------------------------------------------
+_YAML_EA = {"cal/mol": CAL, "kcal/mol": 1e3 * CAL, "J/mol": 1.0, "kJ/mol": 1e3, "J/kmol": 1e-3, "K": R_GAS}
+_YAML_LEN = {"m": 1.0, "cm": 1e-2}
+_YAML_QTY = {"mol": 1.0, "kmol": 1e3}
+
+
+def parse_yaml(text: str, qss: Sequence[str] = ()) -> MechanismDescription:
+    """Cantera-YAML-format mechanism text -> flat description.  Read: a top-level `units` mapping (length m | cm, quantity mol | kmol,
+    activation-energy cal/mol | kcal/mol | J/mol | kJ/mol | J/kmol | K; defaults m, kmol, J/kmol as in that format), the element and
+    species lists of the FIRST phase, `species` entries with `composition` and `thermo: {model: NASA7, temperature-ranges: [lo, mid, hi],
+    data: [[a1..a7 low], [a1..a7 high]]}`, `reactions` entries with `equation`, `rate-constant: {A, b, Ea}`, `type: three-body` (or `+ M`
+    in the equation) with `efficiencies`, `type: falloff` with `low-P-rate-constant`, `high-P-rate-constant`, `Troe: {A, T3, T1[, T2]}`;
+    `duplicate`.  Numbers only: quantities written as strings with units, other reaction types or rate forms raise MechanismError."""
+    import yaml
+    try:
+        doc = yaml.safe_load(text)
+    except yaml.YAMLError as e:
+        raise MechanismError(f"not YAML: {e}")
+    if not isinstance(doc, dict) or "phases" not in doc or "species" not in doc or "reactions" not in doc:
+        raise MechanismError("the document needs `phases`, `species` and `reactions`")
+    un = doc.get("units", {}) or {}
+    try:
+        length, qty, e_unit = _YAML_LEN[un.get("length", "m")], _YAML_QTY[un.get("quantity", "kmol")], _YAML_EA[un.get("activation-energy", "J/kmol")]
+    except KeyError as e:
+        raise MechanismError(f"units: {e} is not read")
+    for k in un:
+        if k not in ("length", "quantity", "activation-energy", "time", "mass", "pressure", "temperature", "energy"):
+            raise MechanismError(f"units: {k} is not read")
+    if un.get("time", "s") != "s":
+        raise MechanismError("units: time other than s is not read")
+    vol_unit = length ** 3 / qty
+    phase = doc["phases"][0]
+    elements = [str(e).upper() for e in phase.get("elements", [])]
+    names = [str(x).upper() for x in phase.get("species", [])]
+    if not elements or not names or any(isinstance(x, dict) for x in phase.get("species", [])):
+        raise MechanismError("the first phase needs plain `elements` and `species` lists")
+    for e in elements:
+        if e not in ATOMIC_WEIGHT:
+            raise MechanismError(f"element {e}: atomic weight not known to the front-end")
+    qset = [q.upper() for q in qss]
+    for q in qset:
+        if q not in names:
+            raise MechanismError(f"QSS species {q} is not in the phase")
+
+    def num(v, what):
+        if isinstance(v, bool) or not isinstance(v, (int, float)):
+            raise MechanismError(f"{what}: {v!r} is not a plain number (quantities with units are not read)")
+        return float(v)
+
+    thermo = {}
+    for sp in doc["species"]:
+        name = str(sp.get("name", "")).upper()
+        th = sp.get("thermo", {})
+        if th.get("model") != "NASA7":
+            raise MechanismError(f"{name}: thermo model {th.get('model')!r} is not read")
+        tr, data = th.get("temperature-ranges", []), th.get("data", [])
+        if len(tr) != 3 or len(data) != 2 or any(len(d) != 7 for d in data):
+            raise MechanismError(f"{name}: NASA7 needs three temperatures and two sets of seven coefficients")
+        comp = {}
+        for sym, cnt in (sp.get("composition", {}) or {}).items():
+            c = num(cnt, f"{name}: composition")
+            if c != int(c) or str(sym).upper() not in elements:
+                raise MechanismError(f"{name}: composition {sym}: {cnt}")
+            if int(c):
+                comp[str(sym).upper()] = int(c)
+        if name in names and name not in thermo:
+            thermo[name] = (comp, tuple(num(x, f"{name}: temperature") for x in tr), [num(x, name) for x in data[0]], [num(x, name) for x in data[1]])
+    missing = [x for x in names if x not in thermo]
+    if missing:
+        raise MechanismError(f"no species entry for {missing}")
+
+    def rate(d, eq):
+        if not isinstance(d, dict) or set(d) != {"A", "b", "Ea"}:
+            raise MechanismError(f"{eq}: a rate constant needs exactly A, b, Ea")
+        return num(d["A"], eq), num(d["b"], eq), num(d["Ea"], eq) * e_unit
+
+    recs = []
+    for r in doc["reactions"]:
+        eq = str(r.get("equation", ""))
+        for k in r:
+            if k not in ("equation", "rate-constant", "type", "efficiencies", "low-P-rate-constant", "high-P-rate-constant", "Troe", "duplicate", "note"):
+                raise MechanismError(f"{eq}: {k} is not read")
+        re_, pr_, rev, m1, falloff = _equation(eq, names)
+        typ = r.get("type", "falloff" if falloff else ("three-body" if m1 else "elementary"))
+        if typ == "elementary" and (m1 or falloff) or typ == "three-body" and not m1 or typ == "falloff" and not falloff or typ not in ("elementary", "three-body", "falloff"):
+            raise MechanismError(f"{eq}: type {typ!r} does not match the equation or is not read")
+        rec = dict(eq=eq.replace(" ", ""), reac=re_, prod=pr_, rev=rev, type={"elementary": 0, "three-body": 1, "falloff": 2}[typ], low=None, troe=None,
+                   eff=[], e_unit=1.0, vol_unit=vol_unit)
+        if typ == "falloff":
+            if "Troe" not in r or "low-P-rate-constant" not in r or "high-P-rate-constant" not in r or "rate-constant" in r:
+                raise MechanismError(f"{eq}: a fall-off reaction needs low-P-rate-constant, high-P-rate-constant and Troe (Lindemann form is not read)")
+            rec["A"], rec["beta"], rec["Ea"] = rate(r["high-P-rate-constant"], eq)
+            rec["low"] = list(rate(r["low-P-rate-constant"], eq))
+            tro = r["Troe"]
+            if not isinstance(tro, dict) or not {"A", "T3", "T1"} <= set(tro) or not set(tro) <= {"A", "T3", "T1", "T2"}:
+                raise MechanismError(f"{eq}: Troe needs A, T3, T1 and optionally T2")
+            rec["troe"] = [num(tro["A"], eq), num(tro["T3"], eq), num(tro["T1"], eq)] + ([num(tro["T2"], eq)] if "T2" in tro else [])
+        else:
+            if "rate-constant" not in r or "Troe" in r or "low-P-rate-constant" in r:
+                raise MechanismError(f"{eq}: needs rate-constant only")
+            rec["A"], rec["beta"], rec["Ea"] = rate(r["rate-constant"], eq)
+        eff = r.get("efficiencies", {}) or {}
+        if eff and typ == "elementary":
+            raise MechanismError(f"{eq}: efficiencies without a third body")
+        for sp_, val in eff.items():
+            if str(sp_).upper() not in names:
+                raise MechanismError(f"{eq}: efficiency of unknown species {sp_}")
+            rec["eff"].append((names.index(str(sp_).upper()), num(val, eq)))
+        recs.append(rec)
+    return _assemble(elements, names, qset, thermo, recs)
 
 
 # ---------------------------------------------------------------------------------------------------------------------------

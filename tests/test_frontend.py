@@ -139,3 +139,71 @@ def test_linearisation_methods():
     assert e.value.code == -3                                           # QSS_E_QSS_FANOUT
     with pytest.raises(fe.MechanismError):
         fe.linearise(d, "nonsense")
+
+
+YAML = """
+units: {length: cm, quantity: mol, activation-energy: cal/mol}
+phases:
+- name: gas
+  thermo: ideal-gas
+  elements: [H, O]
+  species: [A2, B2, AB, A2B, A, B, AB2, A2B2]
+species:
+%s
+reactions:
+- equation: A + B2 <=> B + AB
+  rate-constant: {A: 3.5e+15, b: -0.40, Ea: 16600.0}
+- equation: B + A2 = A + AB
+  rate-constant: {A: 5.0e+04, b: 2.67, Ea: 6290.0}
+- equation: AB + A2 <=> A + A2B
+  rate-constant: {A: 2.2e+08, b: 1.51, Ea: 3430.0}
+- equation: 2 AB <=> B + A2B
+  rate-constant: {A: 3.6e+04, b: 2.40, Ea: -2110.0}
+- equation: A + B2 + M <=> AB2 + M
+  type: three-body
+  rate-constant: {A: 2.8e+18, b: -0.86, Ea: 0.0}
+  efficiencies: {A2B: 11.0, B2: 0.78, A: 2.0}
+- equation: A + AB2 => 2 AB
+  rate-constant: {A: 7.1e+13, b: 0.0, Ea: 295.0}
+- equation: AB + AB (+M) <=> A2B2 (+M)
+  type: falloff
+  low-P-rate-constant: {A: 2.3e+18, b: -0.90, Ea: -1700.0}
+  high-P-rate-constant: {A: 7.4e+13, b: -0.37, Ea: 0.0}
+  Troe: {A: 0.735, T3: 94.0, T1: 1756.0, T2: 5182.0}
+  efficiencies: {A2: 2.0, A2B: 6.0}
+- equation: AB2 + AB2 <=> A2B2 + B2
+  duplicate: true
+  rate-constant: {A: 1.3e+11, b: 0.0, Ea: -1630.0}
+- equation: AB2 + AB2 <=> A2B2 + B2
+  duplicate: true
+  rate-constant: {A: 4.2e+14, b: 0.0, Ea: 12000.0}
+- equation: A2B2 + A (+M) <=> A2B + AB (+M)
+  type: falloff
+  low-P-rate-constant: {A: 1.0e+17, b: 0.0, Ea: 1000.0}
+  high-P-rate-constant: {A: 2.4e+13, b: 0.0, Ea: 3970.0}
+  Troe: {A: 0.5, T3: 100.0, T1: 2000.0}
+""" % "\n".join("- name: %s\n  composition: {%s}\n  thermo:\n    model: NASA7\n    temperature-ranges: [300.0, 1000.0, 3500.0]\n    data:\n    - [%r, 0.0, 0.0, 0.0, 0.0, %r, %r]\n    - [%r, 0.0, 0.0, 0.0, 0.0, %r, %r]"
+                % (n, ", ".join("%s: %d" % (e, k) for e, k in c), a1, a6, a7, a1, a6, a7) for n, c, a1, a6, a7 in SPECIES)
+
+
+def test_yaml_ingestion_gives_the_same_description_as_chemkin():
+    """The same made-up mechanism in the Cantera-YAML format: every array of the flat description equals the CHEMKIN one's (the thermo
+    coefficients up to the 9 digits the fixed-column records carry); other units convert (kmol, m, J/kmol defaults)."""
+    a = fe.parse_chemkin(TEXT, qss=["A", "B"]); b = fe.parse_yaml(YAML, qss=["A", "B"])
+    assert a.species == b.species and a.elements == b.elements and a.equations == b.equations
+    for f in ("rtype", "dir_mask", "reac_ptr", "reac_sp", "reac_nu", "prod_ptr", "prod_sp", "prod_nu", "eff_ptr", "eff_sp", "comp"):
+        assert np.array_equal(getattr(a, f), getattr(b, f)), f
+    for f in ("arr", "arr_low", "troe", "eff_val", "nasa_T", "elem_weight"):
+        assert np.allclose(getattr(a, f), getattr(b, f), rtol=1e-14, atol=0.0), f
+    assert np.allclose(a.nasa_lo, b.nasa_lo, rtol=1e-8) and np.allclose(a.nasa_hi, b.nasa_hi, rtol=1e-8)
+    qss.validate(b, strict_balance=True)
+    # the format's default units: m, kmol, J/kmol -> a bimolecular A is per (m^3/kmol), Ea per kmol
+    si = YAML.replace("units: {length: cm, quantity: mol, activation-energy: cal/mol}\n", "")
+    c = fe.parse_yaml(si, qss=["A", "B"])
+    assert np.isclose(c.arr[0, 0], 3.5e15 * 1e-3) and np.isclose(c.arr[0, 2], 16600.0 * 1e-3) and np.isclose(c.arr[4, 0], 2.8e18 * 1e-6)
+    # what is not read is an error
+    for bad, msg in ((YAML.replace("Ea: 295.0", "Ea: 295.0 cal/mol"), "not a plain number"), (YAML.replace("type: three-body", "type: pressure-dependent-Arrhenius"), "type"),
+                     (YAML.replace("model: NASA7", "model: NASA9", 1), "NASA9"), (YAML.replace("length: cm", "length: mm"), "units")):
+        with pytest.raises(fe.MechanismError) as e:
+            fe.parse_yaml(bad)
+        assert msg in str(e.value), (msg, str(e.value))
