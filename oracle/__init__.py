@@ -173,6 +173,54 @@ def bdf1_advance(om: OracleMech, C: np.ndarray, T: np.ndarray, dt: np.ndarray, n
     return (C, T, hist) if history else (C, T)
 
 
+def ignition_advance(om: OracleMech, C, T, dt, t, t_end, n_attempts, newton_iters, n_cells=None, *, rtol=1e-6, atol_C=1e-12, atol_T=1e-6,
+                     T0=None, dT_ign=400.0, t_ign=None, grow=1.5, shrink=0.25, trace=None):
+    """NEXT-4, adaptive form of `bdf1_advance` (substeps inside which the integrator "employs its own variable size
+    time-stepping strategy"; ignition delay L126: "the earliest time after which the initial temperature increased by at least 400K";
+    DESIGN.md reading G23).  `n_attempts` attempts per cell, each: h = min(dt, t_end - t) (0 once t_end is reached: the identity),
+    `newton_iters` full Newton iterations of the backward-Euler step as in `bdf1_advance`, then with delta = the LAST Newton update
+        err = max( max_i |delta_i| / (atol_C + rtol |C_i|),  |delta_T| / (atol_T + rtol |T|) )      (C, T: the iterate it was added to)
+    ACCEPT when err <= 1, everything is finite and the new T > 0: t += h, dt := grow dt, and t_ign := t (new) if it is still NaN and
+    T_new - T0 >= dT_ign; else REJECT: (C, T) back to the start of the attempt, dt := shrink dt.
+    All arrays are per cell and updated in copies: returns dict(C, T, dt, t, t_ign, accepted [ld] (count), err_last [ld]).
+    `trace`: a list that receives err of every attempt (for tests that exclude decisions within rounding of the threshold)."""
+    ld = C.shape[1]
+    n = ld if n_cells is None else n_cells
+    N = om.N
+    C = C.copy(); T = T.copy(); dt = np.array(dt, dtype=np.float64); t = np.array(t, dtype=np.float64)
+    t_ign = np.full(ld, np.nan) if t_ign is None else np.array(t_ign, dtype=np.float64)
+    T0 = T.copy() if T0 is None else np.asarray(T0, dtype=np.float64)
+    accepted = np.zeros(ld, dtype=np.int64); err_last = np.zeros(ld)
+    for _a in range(n_attempts):
+        Cn, Tn = C.copy(), T.copy()
+        h = np.zeros(ld); h[:n] = np.minimum(dt[:n], np.maximum(t_end - t[:n], 0.0))
+        with np.errstate(all="ignore"):
+            for _m in range(newton_iters):
+                ev = evaluate(om, C, T, n, want_jac=True); en = evaluate_energy(om, C, T, n)
+                b = np.zeros((N + 1, ld))
+                b[:N, :n] = (Cn[:, :n] - C[:, :n]) + h[:n] * ev["wdot"][:, :n]
+                b[N, :n] = (Tn[:n] - T[:n]) + h[:n] * en["tdot"][:n]
+                x = newton_solve(np.ascontiguousarray(ev["jac"]), np.ascontiguousarray(en["erow"]), np.ascontiguousarray(h), b, n)["x"]
+                if _m == newton_iters - 1:
+                    eC = (np.abs(x[:N, :n]) / (atol_C + rtol * np.abs(C[:, :n]))).max(0)
+                    eT = np.abs(x[N, :n]) / (atol_T + rtol * np.abs(T[:n]))
+                    err = np.where(np.isnan(eC) | np.isnan(eT), np.inf, np.maximum(eC, eT))
+                C[:, :n] = np.maximum(C[:, :n] + x[:N, :n], 0.0)
+                T[:n] = T[:n] + x[N, :n]
+            ok = (err <= 1.0) & np.isfinite(C[:, :n]).all(0) & np.isfinite(T[:n]) & (T[:n] > 0.0)
+        if trace is not None:
+            trace.append(err.copy())
+        err_last[:n] = err
+        rej = ~ok
+        C[:, :n][:, rej] = Cn[:, :n][:, rej]; T[:n][rej] = Tn[:n][rej]
+        t[:n] = np.where(ok, t[:n] + h[:n], t[:n])
+        dt[:n] = np.where(ok, grow * dt[:n], shrink * dt[:n])
+        accepted[:n] += ok
+        ign = ok & np.isnan(t_ign[:n]) & (T[:n] - T0[:n] >= dT_ign)
+        t_ign[:n] = np.where(ign, t[:n], t_ign[:n])
+    return dict(C=C, T=T, dt=dt, t=t, t_ign=t_ign, accepted=accepted, err_last=err_last)
+
+
 def rate_constants(om: OracleMech, C1: np.ndarray, T: float):
     C1 = np.ascontiguousarray(C1, dtype=np.float64)
     kf = np.zeros(om.M); kb = np.zeros(om.M)

@@ -90,3 +90,48 @@ def test_zero_step_is_the_identity():
     C, T = config_states(1, 4)
     Cn, Tn = oracle.bdf1_advance(om, C, T, np.zeros(C.shape[1]), 2, 2)
     assert np.array_equal(Cn, C) and np.array_equal(Tn, T)
+
+
+def test_adaptive_integrator_reaches_t_end_and_matches_radau():
+    """oracle.ignition_advance (reading G23): every cell reaches t_end exactly (the last step is clipped), rejected attempts leave the
+    state untouched and shrink the step, and the result agrees with scipy's Radau on the oracle's right-hand side to the order of the
+    method's error at the accepted step sizes (backward Euler: first order; the Newton tolerance only controls the solve)."""
+    m = toy_dag(); om = oracle.OracleMech(m); N = m.n_nqss
+    C, T = make_states(N, 4, seed=4)
+    tau = _time_scale(om, C, T)
+    t_end = float(2.0 * tau[:4].min())
+    out = oracle.ignition_advance(om, C, T, 0.02 * tau, np.zeros(C.shape[1]), t_end, 400, 3, 4, rtol=1e-9, atol_C=1e-14 * np.abs(C).max(), atol_T=1e-9)
+    assert np.all(out["t"][:4] == t_end)                                # reached exactly: h = min(dt, t_end - t), then h = 0
+    assert (out["accepted"][:4] >= 5).all()
+    for c in range(4):
+        sol = solve_ivp(_rhs(om, N), (0.0, t_end), np.concatenate([C[:, c], [T[c]]]), method="Radau", rtol=1e-11, atol=1e-14 * np.abs(C[:, c]).max())
+        y = np.concatenate([out["C"][:, c], [out["T"][c]]])
+        assert np.abs(y - sol.y[:, -1]).max() / np.abs(sol.y[:, -1]).max() < 0.05
+    # a step far too large for three Newton iterations is rejected: state unchanged, step shrunk, nothing accepted, time not advanced
+    big = oracle.ignition_advance(om, C, T, 1e6 * tau, np.zeros(C.shape[1]), 1e9 * float(tau.max()), 1, 1, 4, rtol=1e-12, atol_C=0.0, atol_T=0.0)
+    assert (big["accepted"][:4] == 0).all() and np.array_equal(big["C"], C) and np.array_equal(big["T"], T)
+    assert np.allclose(big["dt"][:4], 0.25e6 * tau[:4]) and (big["t"][:4] == 0).all()
+    # with everything accepted and no growth the adaptive form IS the fixed-step integrator
+    fix = oracle.bdf1_advance(om, C, T, 0.01 * tau, 5, 4, 4)
+    ada = oracle.ignition_advance(om, C, T, 0.01 * tau, np.zeros(C.shape[1]), 1e9, 5, 4, 4, rtol=1.0, atol_C=1e300, atol_T=1e300, grow=1.0)
+    assert np.array_equal(ada["C"][:, :4], fix[0][:, :4]) and np.array_equal(ada["T"][:4], fix[1][:4]) and (ada["accepted"][:4] == 5).all()
+
+
+def test_ignition_time_is_the_first_accepted_time_above_the_threshold():
+    m = config_mechanism(1); om = oracle.OracleMech(m)
+    C, T = config_states(1, 8)
+    tau = _time_scale(om, C, T)
+    out = oracle.ignition_advance(om, C, T, 0.5 * tau, np.zeros(C.shape[1]), 1e9, 30, 3, 8, dT_ign=1e-3, rtol=1e-6)
+    moved = np.abs(out["T"][:8] - T[:8]) > 0
+    assert moved.any()
+    up = out["T"][:8] - T[:8] >= 1e-3
+    assert np.all(np.isnan(out["t_ign"][:8]) | (out["t_ign"][:8] <= out["t"][:8])) and np.all(np.isfinite(out["t_ign"][:8])[up])
+    assert np.isfinite(out["t_ign"][:8]).any()
+    # replay with a trace of T: t_ign is the time of the first accepted state at or above T0 + dT_ign
+    t = np.zeros(C.shape[1]); dt = 0.5 * tau; Cc, Tc = C, T; tig = None; first = np.full(8, np.nan)
+    for a in range(30):
+        o = oracle.ignition_advance(om, Cc, Tc, dt, t, 1e9, 1, 3, 8, dT_ign=1e-3, rtol=1e-6, T0=T, t_ign=tig)
+        Cc, Tc, dt, t, tig = o["C"], o["T"], o["dt"], o["t"], o["t_ign"]
+        hit = np.isnan(first) & (Tc[:8] - T[:8] >= 1e-3)
+        first[hit] = t[:8][hit]
+    assert np.array_equal(first, out["t_ign"][:8], equal_nan=True) and np.array_equal(Tc[:8], out["T"][:8])
