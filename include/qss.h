@@ -243,6 +243,19 @@ size_t qss_bdf1_workspace_bytes(const qss_mech_t *mech, int64_t ld);
 int qss_bdf1_advance(const qss_mech_t *mech, int64_t ncells, int64_t ld, double *C, double *T, const double *dt, int nsub,
                      int newton_iters, void *workspace, size_t workspace_bytes, void *stream);
 
+/* NEXT-4, adaptive form with ignition time (the integrator "employs its own variable size time-stepping strategy";
+ * L126: ignition delay = "the earliest time after which the initial temperature increased by at least 400K"; reading G23).
+ * `n_attempts` attempts per cell, each one backward-Euler step of size h = min(dt[c], t_end - t[c]) (0 once t_end is reached: the
+ * identity) solved by `newton_iters` full Newton iterations as in qss_bdf1_advance; with delta the LAST Newton update the attempt is
+ * ACCEPTED when  max( max_i |delta_i| / (atol_C + rtol |C_i|), |delta_T| / (atol_T + rtol |T|) ) <= 1  and the new state is finite with
+ * T > 0:  t[c] += h, dt[c] *= 1.5, and t_ign[c] = t[c] if it is still NaN and T - T0[c] >= dT_ign;  else REJECTED: (C, T) of the start
+ * of the attempt are restored and dt[c] *= 0.25.  C, T, dt, t, t_ign are DEVICE arrays updated in place (t_ign, T0 may be NULL; fill
+ * t_ign with NaN before the first call); the launch sequence is fixed (2 kernels per Newton iteration, 2 copies per attempt), nothing
+ * synchronises.  Workspace as qss_bdf1_advance; ld even; N + 1 <= 40.  Needs run-time compilation (QSS_E_CUDA without NVRTC). */
+int qss_ignition_advance(const qss_mech_t *mech, int64_t ncells, int64_t ld, double *C, double *T, double *dt, double *t, double t_end,
+                         double *t_ign_or_null, const double *T0_or_null, double dT_ign, int n_attempts, int newton_iters, double rtol,
+                         double atol_C, double atol_T, void *workspace, size_t workspace_bytes, void *stream);
+
 /* Host-buffer convenience used for end-to-end timing: copies C and T to the device (in `dev_scratch`, which
  * must hold qss_host_scratch_bytes() bytes), evaluates, copies the Jacobian (and wdot if not NULL) back to
  * the HOST buffers, and synchronises `stream`.  Host buffers should be pinned for full copy bandwidth.  Large batches are

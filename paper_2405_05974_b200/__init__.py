@@ -17,7 +17,7 @@ from . import build as _build
 __all__ = ["lib", "QssMech", "QssError", "EXPORTS", "STATUS"]
 
 EXPORTS = ["qss_mech_create", "qss_mech_validate", "qss_mech_specialise_check", "qss_mech_destroy", "qss_mech_info", "qss_mech_qss_order", "qss_eval_wdot",
-           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_newton_solve", "qss_newton_specialise_check", "qss_bdf1_workspace_bytes", "qss_bdf1_advance", "qss_jac_fdt_workspace_bytes", "qss_eval_jac_fdt", "qss_mech_jac_pattern", "qss_jac_pack", "qss_eval_jac_full", "qss_eval_wdot_static", "qss_bench_species_sums", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
+           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_newton_solve", "qss_newton_specialise_check", "qss_bdf1_workspace_bytes", "qss_bdf1_advance", "qss_ignition_advance", "qss_jac_fdt_workspace_bytes", "qss_eval_jac_fdt", "qss_mech_jac_pattern", "qss_jac_pack", "qss_eval_jac_full", "qss_eval_wdot_static", "qss_bench_species_sums", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
 STATUS = {0: "QSS_OK", -1: "QSS_E_INVALID", -2: "QSS_E_QUADRATIC", -3: "QSS_E_QSS_FANOUT", -4: "QSS_E_NO_SINK",
           -5: "QSS_E_UNSUPPORTED", -6: "QSS_E_CUDA", -7: "QSS_E_UNBALANCED"}
 
@@ -76,6 +76,8 @@ def lib():
         L.qss_eval_jac_full.restype = ct.c_int; L.qss_eval_jac_full.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp, ct.c_size_t, vp]
         L.qss_mech_jac_pattern.restype = ct.c_int; L.qss_mech_jac_pattern.argtypes = [vp, ct.c_int, vp]
         L.qss_jac_pack.restype = ct.c_int; L.qss_jac_pack.argtypes = [vp, i64, i64, ct.c_int32, vp, vp, vp, vp]
+        L.qss_ignition_advance.restype = ct.c_int
+        L.qss_ignition_advance.argtypes = [vp, i64, i64, vp, vp, vp, vp, ct.c_double, vp, vp, ct.c_double, ct.c_int, ct.c_int, ct.c_double, ct.c_double, ct.c_double, vp, ct.c_size_t, vp]
         L.qss_jac_fdt_workspace_bytes.restype = ct.c_size_t; L.qss_jac_fdt_workspace_bytes.argtypes = [vp, i64]
         L.qss_eval_jac_fdt.restype = ct.c_int; L.qss_eval_jac_fdt.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, ct.c_size_t, vp]
         L.qss_bdf1_workspace_bytes.restype = ct.c_size_t; L.qss_bdf1_workspace_bytes.argtypes = [vp, i64]
@@ -345,6 +347,22 @@ class QssMech:
         if workspace is None or workspace.numel() < need:
             workspace = torch.empty(need, dtype=torch.uint8, device=C.device)
         _check(lib().qss_bdf1_advance(self._h, ncells, ld, _ptr(C), _ptr(T), _ptr(dt), int(nsub), int(newton_iters), _ptr(workspace), workspace.numel(), self._stream()))
+        return workspace
+
+    def ignition_advance(self, C, T, dt, t, t_end, n_attempts, newton_iters, ncells=None, t_ign=None, T0=None, dT_ign=400.0, rtol=1e-6,
+                         atol_C=1e-12, atol_T=1e-6, workspace=None):
+        """Adaptive backward-Euler attempts with ignition time (qss_ignition_advance); C, T, dt, t, t_ign are updated IN PLACE."""
+        import torch
+        ld = C.shape[1]
+        ncells = ld if ncells is None else int(ncells)
+        for a in (C, T, dt, t):
+            assert a.is_contiguous() and a.dtype == torch.float64
+        need = int(lib().qss_bdf1_workspace_bytes(self._h, ld))
+        if workspace is None or workspace.numel() < need:
+            workspace = torch.empty(need, dtype=torch.uint8, device=C.device)
+        _check(lib().qss_ignition_advance(self._h, ncells, ld, _ptr(C), _ptr(T), _ptr(dt), _ptr(t), float(t_end), _ptr(t_ign), _ptr(T0), float(dT_ign),
+                                          int(n_attempts), int(newton_iters), float(rtol), float(atol_C), float(atol_T), _ptr(workspace), workspace.numel(),
+                                          self._stream()))
         return workspace
 
     def host_scratch_bytes(self, ncells, ld):

@@ -564,6 +564,59 @@ extern "C" int qss_bdf1_advance(const qss_mech_t *m, int64_t ncells, int64_t ld,
     return QSS_OK;
 }
 
+
+// ---- NEXT-4: adaptive form with ignition time (reading G23) ---------------------------------------------------------------
+extern "C" int qss_ignition_advance(const qss_mech_t *m, int64_t ncells, int64_t ld, double *C, double *T, double *dt, double *t, double t_end,
+                                    double *t_ign, const double *T0, double dT_ign, int n_attempts, int newton_iters, double rtol, double atol_C,
+                                    double atol_T, void *workspace, size_t workspace_bytes, void *stream) {
+    if (!m) return fail(QSS_E_INVALID, "mech is NULL");
+    if (ncells < 0 || ld < ncells || n_attempts < 0 || newton_iters < 1) return fail(QSS_E_INVALID, "need 0 <= ncells <= ld, n_attempts >= 0, newton_iters >= 1");
+    if (!(rtol >= 0.0) || !(atol_C >= 0.0) || !(atol_T >= 0.0) || !(rtol + atol_C > 0.0) || !(rtol + atol_T > 0.0)) return fail(QSS_E_INVALID, "tolerances must be non-negative and not both zero");
+    const int N = m->c.tab.N;
+    if (N + 1 > QSS_NEWTON_MAX_N) return fail(QSS_E_UNSUPPORTED, "qss_ignition_advance: more than 39 transported species (limit of qss_newton_solve)");
+    if (ncells == 0 || n_attempts == 0) return QSS_OK;
+    if (!C || !T || !dt || !t || (t_ign && !T0)) return fail(QSS_E_INVALID, "NULL device pointer (T0 is required with t_ign)");
+    if (ld & 1) return fail(QSS_E_INVALID, "qss_ignition_advance: ld must be even (16-byte aligned rows)");
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < qss_bdf1_workspace_bytes(m, ld)) return fail(QSS_E_INVALID, "workspace is NULL, misaligned or smaller than qss_bdf1_workspace_bytes");
+    DeviceGuard guard(m->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    QssJit *step = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(m->host_mu);
+        if (!m->newton_step_tried) {
+            m->newton_step_tried = true;
+            std::string jerr;
+            m->newton_step = qss_jit_newton_step_create(N + 1, N + 1, QSS_NEWTON_CPB, m->cc_major, m->cc_minor, jerr);
+            if (m->newton_step) m->newton_step_blocks = m->n_sm * qss_jit_newton_step_blocks_per_sm(m->newton_step, N + 1, QSS_NEWTON_CPB);
+        }
+        step = m->newton_step;
+    }
+    if (!step) return fail(QSS_E_CUDA, "qss_ignition_advance needs the run-time compiled Newton step kernel (NVRTC unavailable)");
+    const size_t nrow = (size_t)ld;
+    char *p = (char *)workspace;
+    auto take = [&](size_t rows) { double *q = (double *)p; p += align256(rows * nrow * sizeof(double)); return q; };
+    double *jac = take((size_t)N * (N + 1)), *F = take(N + 1);
+    (void)take(N + 1);                                          // (the energy row of the unfused sequence: not used here)
+    double *phin = take(N + 1);
+    (void)take(N + 1);
+    void *ws = (void *)(((uintptr_t)p + 255) & ~(uintptr_t)255);
+    const size_t wsb = ws_bytes(m, true);
+    QssStepAdapt ad = {1, t, dt, t_ign, T0, t_end, rtol, atol_C, atol_T, dT_ign, 1.5, 0.25};
+    for (int a = 0; a < n_attempts; ++a) {
+        cudaError_t e = cudaMemcpyAsync(phin, C, (size_t)N * nrow * sizeof(double), cudaMemcpyDeviceToDevice, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(phin + (size_t)N * nrow, T, nrow * sizeof(double), cudaMemcpyDeviceToDevice, st);
+        if (e != cudaSuccess) return cuda_fail(e, "qss_ignition_advance: saving the state");
+        for (int it = 0; it < newton_iters; ++it) {
+            int rc = eval_jac_mode(m, ncells, ld, C, T, jac, F, 0, ws, wsb, stream);
+            if (rc != QSS_OK) return rc;
+            ad.adapt = it == newton_iters - 1 ? 2 : 1;
+            e = qss_jit_newton_step_launch(step, N + 1, QSS_NEWTON_CPB, m->newton_step_blocks, jac, F, phin, dt, m->dD + m->c.tab.d_thermo, C, T, ncells, ld, st, &ad);
+            if (e != cudaSuccess) return cuda_fail(e, "qss_ignition_advance: Newton step");
+        }
+    }
+    return QSS_OK;
+}
+
 extern "C" size_t qss_host_scratch_bytes(const qss_mech_t *m, int64_t ncells, int64_t ld) {
     if (!m || ncells < 0 || ld < ncells) return 0;
     const size_t N = m->c.tab.N, L = (size_t)ld * sizeof(double);

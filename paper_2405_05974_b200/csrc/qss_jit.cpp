@@ -304,6 +304,10 @@ struct QssStepArgs {            // = struct QssStep of qss_newton_kernel.cu
     const double *jac, *wdot, *phin, *dt, *thermo;
     double *C, *T;
     int64_t ncells, ld;
+    int adapt;
+    double *tcur, *dtio, *tign;
+    const double *T0;
+    double t_end, rtol, atolC, atolT, dT_ign, grow, shrink;
 };
 }  // namespace
 
@@ -325,9 +329,14 @@ int qss_jit_newton_step_blocks_per_sm(const QssJit *j, int n, int cpb) {
 }
 
 cudaError_t qss_jit_newton_step_launch(const QssJit *j, int n, int cpb, int max_blocks, const double *jac, const double *wdot, const double *phin,
-                                       const double *dt, const double *thermo, double *C, double *T, int64_t ncells, int64_t ld, cudaStream_t stream) {
+                                       const double *dt, const double *thermo, double *C, double *T, int64_t ncells, int64_t ld, cudaStream_t stream,
+                                       const QssStepAdapt *ad) {
     if (ncells == 0) return cudaSuccess;
-    QssStepArgs a = {jac, wdot, phin, dt, thermo, C, T, ncells, ld};
+    QssStepArgs a = {jac, wdot, phin, dt, thermo, C, T, ncells, ld, 0, nullptr, nullptr, nullptr, nullptr, 0, 0, 0, 0, 0, 0, 0};
+    if (ad) {
+        a.adapt = ad->adapt; a.tcur = ad->tcur; a.dtio = ad->dtio; a.tign = ad->tign; a.T0 = ad->T0;
+        a.t_end = ad->t_end; a.rtol = ad->rtol; a.atolC = ad->atolC; a.atolT = ad->atolT; a.dT_ign = ad->dT_ign; a.grow = ad->grow; a.shrink = ad->shrink;
+    }
     void *args[] = {&a};
     const int64_t ntiles = (ncells + cpb - 1) / cpb;
     const int64_t grid = ntiles < max_blocks ? ntiles : max_blocks;

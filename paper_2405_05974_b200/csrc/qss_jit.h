@@ -41,8 +41,15 @@ int qss_jit_newton_blocks_per_sm(const QssJit *j, int n, int cpb);
 QssJit *qss_jit_newton_step_create(int n, int nj, int cpb, int cc_major, int cc_minor, std::string &err);
 size_t qss_jit_newton_step_smem(int n, int cpb);
 int qss_jit_newton_step_blocks_per_sm(const QssJit *j, int n, int cpb);
+struct QssStepAdapt {           // adaptive form (qss_ignition_advance): per-cell time, step size, ignition time; tolerances (reading G23)
+    int adapt;                  // 1: a Newton iteration of an attempt, 2: its last one (accept / reject)
+    double *tcur, *dtio, *tign;
+    const double *T0;
+    double t_end, rtol, atolC, atolT, dT_ign, grow, shrink;
+};
 cudaError_t qss_jit_newton_step_launch(const QssJit *j, int n, int cpb, int max_blocks, const double *jac, const double *wdot, const double *phin,
-                                       const double *dt, const double *thermo, double *C, double *T, int64_t ncells, int64_t ld, cudaStream_t stream);
+                                       const double *dt, const double *thermo, double *C, double *T, int64_t ncells, int64_t ld, cudaStream_t stream,
+                                       const QssStepAdapt *adapt = nullptr);
 cudaError_t qss_jit_newton_launch(const QssJit *j, int n, int cpb, int max_blocks, const double *jac, const double *erow, const double *gamma,
                                   const double *b, double *x, int64_t ncells, int64_t ld, cudaStream_t stream);
 

@@ -74,3 +74,45 @@ def test_zero_substeps_and_unsupported():
         qm3.bdf1_advance(torch.from_numpy(C3).cuda(), torch.from_numpy(T3).cuda(), torch.zeros(C3.shape[1], dtype=torch.float64, device="cuda"), 1, 1, 32)
     assert e.value.code == -5
     qm3.close()
+
+
+@pytest.mark.parametrize("name,n,attempts,iters,rtol", [("cfg1", 257, 12, 3, 1e-6), ("cfg2", 64 + 5, 8, 3, 1e-6), ("toy_dag", 40, 20, 2, 1e-8)])
+def test_adaptive_integrator_with_ignition_time_against_oracle(name, n, attempts, iters, rtol):
+    """qss_ignition_advance against oracle.ignition_advance (reading G23).  Accept / reject are decisions on a floating-point number:
+    both sides take them in fp64 from the same definition; cells where the oracle's criterion comes within 1e-6 of the threshold in any
+    attempt are excluded (printed), the others must agree in EVERYTHING: number of accepted attempts, times, step sizes bit for bit,
+    ignition times, and the state within the tolerance of the fixed-step test."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    if name.startswith("cfg"):
+        mech = qss_synth.config_mechanism(int(name[3])); C, T = qss_synth.config_states(int(name[3]), n)
+    else:
+        mech = getattr(qss_synth, name)(); C, T = make_states(mech.n_nqss, n, seed=5)
+    om = oracle.OracleMech(mech)
+    ld = C.shape[1]
+    dt0 = _dt(om, C, T, n, 30.0, 3)                                     # deliberately too large for many cells: rejections happen
+    t_end = float(np.median(dt0[:n]) * 6.0)
+    dT_ign = 0.05
+    trace = []
+    ref = oracle.ignition_advance(om, C, T, dt0, np.zeros(ld), t_end, attempts, iters, n, rtol=rtol, dT_ign=dT_ign, trace=trace)
+    qm = qss.QssMech(mech, 0)
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda(); T0d = Td.clone()
+    dtd = torch.from_numpy(dt0).cuda(); td = torch.zeros(ld, dtype=torch.float64, device="cuda")
+    tig = torch.full((ld,), float("nan"), dtype=torch.float64, device="cuda")
+    qm.ignition_advance(Cd, Td, dtd, td, t_end, attempts, iters, n, t_ign=tig, T0=T0d, dT_ign=dT_ign, rtol=rtol)
+    torch.cuda.synchronize()
+    Cg, Tg, dtg, tg, tigg = (x.cpu().numpy() for x in (Cd, Td, dtd, td, tig))
+    tr = np.array(trace)                                                 # [attempts, n]
+    sure = ~(np.abs(tr - 1.0) <= 1e-6).any(0) & np.isfinite(ref["T"][:n])
+    rejected = int((attempts - ref["accepted"][:n][sure]).sum())
+    print("%s: %d of %d cells compared, %d rejected attempts among them, %d ignition times, reached t_end: %d"
+          % (name, int(sure.sum()), n, rejected, int(np.isfinite(ref["t_ign"][:n][sure]).sum()), int((ref["t"][:n][sure] == t_end).sum())))
+    assert sure.mean() >= 0.95 and rejected > 0
+    assert np.array_equal(tg[:n][sure], ref["t"][:n][sure]) and np.array_equal(dtg[:n][sure], ref["dt"][:n][sure])
+    assert np.array_equal(tigg[:n][sure], ref["t_ign"][:n][sure], equal_nan=True)
+    eC = (np.abs(Cg[:, :n] - ref["C"][:, :n]).max(0) / np.abs(ref["C"][:, :n]).max(0))[sure]
+    eT = (np.abs(Tg[:n] - ref["T"][:n]) / ref["T"][:n])[sure]
+    assert eC.max() <= 1e-8 and eT.max() <= 1e-10, (eC.max(), eT.max())
+    if ld > n:
+        assert np.array_equal(Cg[:, n:], C[:, n:], equal_nan=True) and np.array_equal(tg[n:], np.zeros(ld - n))
+    qm.close()
