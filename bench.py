@@ -42,6 +42,7 @@ CALLS = {"jac+wdot": "qss_eval_jac with the wdot output (the metric)", "jac": "q
          "jac+wdot+energy+newton": "qss_eval_jac with wdot, qss_eval_energy, qss_newton_solve: one Newton direction of an implicit step",
          "sums_thread": "qss_bench_species_sums mode 0: mapping micro-benchmark, species sums with lane = cell (not on the path)",
          "sums_warp": "qss_bench_species_sums mode 1: mapping micro-benchmark, species sums with a warp per cell and SHFL reductions (not on the path)",
+         "ignition": "qss_ignition_advance: one adaptive attempt with two full Newton iterations (accept / reject, step control and ignition time on the device), state restored before every step",
          "bdf1": "qss_bdf1_advance: one backward-Euler substep with two full Newton iterations (two kernels each: Jacobian, fused Newton step), state restored before every step"}
 
 
@@ -241,8 +242,8 @@ def main():
     if args.call.startswith("sums_"):        # rates of progress: seeded normal values (the arithmetic does not depend on them)
         g = torch.Generator(device=dev); g.manual_seed(11)
         Qm = torch.randn((qm.info.n_reac, ld), dtype=torch.float64, device=dev, generator=g)
-    launches_per_step = {"jac+wdot+energy": 2, "jac+wdot+energy+newton": 3, "bdf1": 4, "jac_full": 2}.get(args.call, 1)
-    if args.call == "bdf1":
+    launches_per_step = {"jac+wdot+energy": 2, "jac+wdot+energy+newton": 3, "bdf1": 4, "ignition": 4, "jac_full": 2}.get(args.call, 1)
+    if args.call in ("bdf1", "ignition"):
         # h_c = 3 / max|J_c| at the initial state (a few of the fastest time scales per substep); the state is restored before every step
         del J
         torch.cuda.empty_cache()
@@ -256,6 +257,8 @@ def main():
         bdf_ws = qm.bdf1_advance(Cd, Td, dtd, 1, 2, n)
         torch.cuda.synchronize()
         J = None
+        if args.call == "ignition":
+            dt0 = dtd.clone(); tcur = torch.zeros(ld, dtype=torch.float64, device=dev); tign = torch.full((ld,), float("nan"), dtype=torch.float64, device=dev)
 
     def step():
         if args.call in ("jac+wdot", "jac+wdot+energy", "jac+wdot+energy+newton"):
@@ -271,6 +274,9 @@ def main():
         elif args.call == "bdf1":
             Cd.copy_(C0); Td.copy_(T0)
             qm.bdf1_advance(Cd, Td, dtd, 1, 2, n, workspace=bdf_ws)
+        elif args.call == "ignition":
+            Cd.copy_(C0); Td.copy_(T0); dtd.copy_(dt0); tcur.zero_()
+            qm.ignition_advance(Cd, Td, dtd, tcur, 1.0e30, 1, 2, n, t_ign=tign, T0=T0, workspace=bdf_ws)
         elif args.call == "jac_full":
             qm.eval_jac_full(Cd, Td, n, jac=J, wdot=W, tdot=tdot, erow=erow)
         elif args.call == "jac":
@@ -352,7 +358,7 @@ def main():
         bytes_cell, slots_cell = 8.0 * (nn * nn + 2 * nn + 1), nn ** 3 / 3.0 + nn * nn
     elif args.call.startswith("sums_"):   # reads Q once, writes wdot; one multiply-add per non-zero of the net stoichiometric matrix (~4 per reaction)
         bytes_cell, slots_cell = 8.0 * (info.n_reac + N), 4.0 * info.n_reac
-    elif args.call == "bdf1":          # two Newton iterations: the three heavy calls twice (the residual / update kernels move 5 (N+1) doubles each)
+    elif args.call in ("bdf1", "ignition"):          # two Newton iterations: the three heavy calls twice (the residual / update kernels move 5 (N+1) doubles each)
         nn = N + 1
         bytes_cell = 2.0 * ((info.bytes_jac + 8.0 * N) + (8.0 * (N * nn + 2 * N + 1) + 8.0 * (N + 2)) + 8.0 * (nn * nn + 2 * nn + 1) + 8.0 * 9 * nn)
         slots_cell = 2.0 * (info.slots_jac + 2.0 * N * nn + 30.0 * N + nn ** 3 / 3.0 + nn * nn)
@@ -378,7 +384,7 @@ def main():
     except Exception:
         traffic = None
     roof.update({"traffic": traffic, "traffic_unit": "bytes per launch (dram read + write) from the committed ncu capture of this workload and kernel variant (profiles/r02_traffic.txt); not measurable inside this run",
-                 "kernel": "qss_mapbench_kernel" if args.call.startswith("sums_") else "qss_energy_kernel" if args.call == "energy" else "qss_newton_kernel" if args.call == "newton" else "the 4 launches of one substep (Jacobian kernel, fused Newton step; twice)" if args.call == "bdf1" else ("qss wdot kernel (qss_eval_wdot)" if args.call == "wdot" else f"qss jacobian kernel, variant {info.kernel_variant_jac} ({CALLS[args.call]})"),
+                 "kernel": "qss_mapbench_kernel" if args.call.startswith("sums_") else "qss_energy_kernel" if args.call == "energy" else "qss_newton_kernel" if args.call == "newton" else "the 4 launches of one substep (Jacobian kernel, fused Newton step; twice)" if args.call in ("bdf1", "ignition") else ("qss wdot kernel (qss_eval_wdot)" if args.call == "wdot" else f"qss jacobian kernel, variant {info.kernel_variant_jac} ({CALLS[args.call]})"),
                  "launch_ms_avg": avg_s * 1e3, "launch_ms_min": min(launch_ms),
                  "alg_fp64_slots_per_cell": slots_cell, "alg_bytes_per_cell": bytes_cell,
                  "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3,
