@@ -228,3 +228,35 @@ def test_mapping_microbenchmark_species_sums(cfg, n):
         out.append(wh[:, :n])
     assert np.allclose(out[0], out[1], rtol=0.0, atol=1e-13 * scale.max())
     qm.close()
+
+
+def test_full_size_cfg2_padded_leading_dimension_full_jacobian_sampled():
+    """BASELINE.json configs[1] at full size in the layout bench.py times (leading dimension = 2^20 + 64): qss_eval_jac_full; 128
+    sampled cells against the oracle (species block, wdot, energy row, Tdot); the 64 padding cells of every row stay untouched."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    mech = qss_synth.config_mechanism(2)
+    C0, T0 = qss_synth.config_states(2)
+    n = qss_synth.CONFIGS[2]["n_cells"]; ld = n + 64
+    C = np.empty((C0.shape[0], ld)); T = np.empty(ld)
+    C[:, :n] = C0[:, :n]; T[:n] = T0[:n]; C[:, n:] = C0[:, :1]; T[n:] = T0[0]
+    qm = qss.QssMech(mech, 0)
+    N = qm.N
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda()
+    f64 = dict(dtype=torch.float64, device="cuda")
+    J = torch.empty((N, N + 1, ld), **f64); w = torch.empty((N, ld), **f64); td = torch.empty((ld,), **f64); er = torch.empty((N + 1, ld), **f64)
+    for a in (J, w, td, er):
+        a[..., n:] = float("nan")
+    qm.eval_jac_full(Cd, Td, n, jac=J, wdot=w, tdot=td, erow=er)
+    torch.cuda.synchronize()
+    assert torch.isfinite(J[:, :, :n]).all() and torch.isfinite(w[:, :n]).all() and torch.isfinite(er[:, :n]).all() and torch.isfinite(td[:n]).all()
+    assert torch.isnan(J[:, :, n:]).all() and torch.isnan(w[:, n:]).all() and torch.isnan(er[:, n:]).all() and torch.isnan(td[n:]).all()
+    idx = np.sort(np.random.default_rng(7).choice(n, size=128, replace=False)); idx[0], idx[-1] = 0, n - 1
+    it = torch.from_numpy(idx).cuda()
+    Cs = np.ascontiguousarray(C[:, idx]); Ts = np.ascontiguousarray(T[idx])
+    om = oracle.OracleMech(mech)
+    ref = oracle.evaluate(om, Cs, Ts, want_jac=True, want_scale=True)
+    gates.assert_wdot(w[:, it].cpu().numpy(), ref["wdot"], ref["S"], what="cfg2 full (padded ld) wdot", cfg=2)
+    gates.assert_jac(J[:, :, it].cpu().numpy(), ref["jac"], ref["jscale"], what="cfg2 full (padded ld) jac", cfg=2)
+    _energy_gates(td[it].cpu().numpy(), er[:, it].cpu().numpy(), oracle.evaluate_energy(om, Cs, Ts), Ts, 128, "cfg2 full (padded ld)")
+    qm.close()
