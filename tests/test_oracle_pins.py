@@ -7,6 +7,7 @@ null space of every Jacobian column, and first-order convergence of one-sided fi
 (App. C). No GPU is involved anywhere in this file.
 """
 import math
+import os
 
 import mpmath as mp
 import numpy as np
@@ -489,3 +490,17 @@ def test_finite_difference_converges_at_first_order():
         errs.append(np.mean(e))
     assert 5.0 < errs[0] / errs[1] < 20.0, errs
     assert 5.0 < errs[1] / errs[2] < 20.0, errs
+
+
+def test_golden_regression():
+    """tests/golden/oracle_toys.txt (written by tests/golden/make_golden.py from the oracle alone): the oracle reproduces its stored
+    values; a change of its arithmetic has to come with a regenerated fixture and the passage that justifies it."""
+    import importlib.util
+    here = os.path.dirname(os.path.abspath(__file__))
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "golden", "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec); spec.loader.exec_module(mg)
+    stored = np.loadtxt(os.path.join(here, "golden", "oracle_toys.txt"), comments="#")
+    now = np.concatenate([mg.values(name, n) for name, n in mg.CASES])
+    assert stored.shape == now.shape
+    scale = np.maximum(np.abs(stored), 1e-300)
+    assert np.all(np.abs(now - stored) <= 1e-12 * scale + 1e-280), float(np.max(np.abs(now - stored) / scale))
