@@ -72,6 +72,12 @@ def _p(a):
     return None if a is None else a.ctypes.data
 
 
+def _threads(nthreads: int, n_cells: int) -> int:
+    """nthreads = 0 means "all", but never more threads than there are groups of 8 cells: a team of many threads for a handful of cells
+    costs far more than the work (the cells are independent, so the results do not depend on it)."""
+    return nthreads if nthreads > 0 else max(1, min(max_threads(), (n_cells + 7) // 8))
+
+
 def evaluate(om: OracleMech, C: np.ndarray, T: np.ndarray, n_cells: int | None = None, *, want_jac=True,
              want_scale=False, mode=EXPLICIT_F64, nthreads=0):
     """C [N, ld], T [ld] float64. Returns dict(wdot [N,ld], cqss [Nq,ld], S [N,ld], jac [N,N+1,ld], jscale)."""
@@ -84,7 +90,7 @@ def evaluate(om: OracleMech, C: np.ndarray, T: np.ndarray, n_cells: int | None =
     out["jac"] = np.zeros((N, N + 1, ld)) if want_jac else None
     out["jscale"] = np.zeros((N, N + 1, ld)) if (want_jac and want_scale) else None
     rc = lib().oracle_eval(om._ptr(), n_cells, ld, _p(C), _p(T), _p(out["wdot"]), _p(out["cqss"]), _p(out["S"]),
-                           _p(out["jac"]), _p(out["jscale"]), mode, nthreads)
+                           _p(out["jac"]), _p(out["jscale"]), mode, _threads(nthreads, n_cells))
     if rc != 0:
         raise RuntimeError(f"oracle_eval failed rc={rc}")
     out["cqss"] = out["cqss"][:Nq]
@@ -97,7 +103,7 @@ def evaluate_energy(om: OracleMech, C: np.ndarray, T: np.ndarray, n_cells: int |
     ld = C.shape[1]
     n_cells = ld if n_cells is None else n_cells
     out = dict(tdot=np.zeros(ld), erow=np.zeros((om.N + 1, ld)), escale=np.zeros((om.N + 1, ld)))
-    rc = lib().oracle_eval_energy(om._ptr(), n_cells, ld, _p(C), _p(T), _p(out["tdot"]), _p(out["erow"]), _p(out["escale"]), mode, nthreads)
+    rc = lib().oracle_eval_energy(om._ptr(), n_cells, ld, _p(C), _p(T), _p(out["tdot"]), _p(out["erow"]), _p(out["escale"]), mode, _threads(nthreads, n_cells))
     if rc != 0:
         raise RuntimeError(f"oracle_eval_energy failed rc={rc}")
     return out

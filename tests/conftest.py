@@ -3,6 +3,7 @@ import sys
 
 import pytest
 
+os.environ.setdefault("OMP_WAIT_POLICY", "PASSIVE")      # the oracle's OpenMP threads sleep between calls instead of spinning (many tiny calls in the tests)
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)

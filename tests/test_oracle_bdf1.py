@@ -16,8 +16,8 @@ from qss_synth import config_mechanism, config_states, make_states, toy3, toy_da
 def _rhs(om, N):
     def f(t, y):
         C = np.ascontiguousarray(np.maximum(y[:N], 0.0)[:, None]); T = np.array([y[N]])
-        w = oracle.evaluate(om, C, T, 1, want_jac=False)["wdot"][:, 0]
-        td = oracle.evaluate_energy(om, C, T, 1)["tdot"][0]
+        w = oracle.evaluate(om, C, T, 1, want_jac=False, nthreads=1)["wdot"][:, 0]          # (one cell: no thread team)
+        td = oracle.evaluate_energy(om, C, T, 1, nthreads=1)["tdot"][0]
         return np.concatenate([w, [td]])
     return f
 
