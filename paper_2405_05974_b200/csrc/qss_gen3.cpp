@@ -66,10 +66,8 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
     if (const char *e = qss_devenv("QSS3_NW")) NW = std::atoi(e);
     // registers per thread: at launch (all phases but the sweep), of the idle warps and of the column warps during the sweep
     const int reg_base = std::min(255, 65536 / (NW * 32)) / 8 * 8, reg_idle = 24;
-    // (development switch QSS3_PAIR: two Jacobian columns per pass over the solve factors and kappa_d, 8 column warps of 240 registers)
-    const bool pair = qss_devenv("QSS3_PAIR") && std::atoi(qss_devenv("QSS3_PAIR")) != 0 && NW == 12 && 4 * nsp <= 216;
-    const int reg_col = pair ? 240 : NW > 12 ? reg_base + (NW - 12) * (reg_base - reg_idle) / 12 / 8 * 8 : reg_base;
-    const int NWC = pair ? 8 : 12, PITCH = 264, MAXROWS = (227 * 1024) / PITCH;      // NWC: column warps (one Jacobian column in ~160 registers each)
+    const int reg_col = NW > 12 ? reg_base + (NW - 12) * (reg_base - reg_idle) / 12 / 8 * 8 : reg_base;
+    const int NWC = 12, PITCH = 264, MAXROWS = (227 * 1024) / PITCH;      // NWC: column warps (one Jacobian column in ~160 registers each)
     if (M < 1) { why = "no reactions"; return false; }
     if (nsp > 60) { why = "more than 60 species: one Jacobian column does not fit the registers of a thread"; return false; }
     for (int j = 0; j < M; ++j)
@@ -505,7 +503,7 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
         G("}\n");
     }
     // ---- P8: one Jacobian column in registers: init, records, dy/dx solve, W_y dy/dx, stores --------------------------
-    if (!pair) {
+    {
         int dist = 12, fdist = 4, sdist = 3, pdist = 8;      // loads run this many items ahead of their use
         if (const char *e = qss_devenv("QSS3_DIST")) std::sscanf(e, "%d,%d,%d,%d", &dist, &fdist, &sdist, &pdist);
         G("__device__ __forceinline__ void qss_gen_column(const int k, const int mode, const unsigned sml, const unsigned sml2, const double *sc, double *jc, const long long rs, const bool active) {\n    double ");
@@ -650,169 +648,6 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
         for (int w = 0; w < NWC; ++w) for (size_t dd = 0; dd < depth; ++dd) G("%d, ", dd < cols[w].size() ? cols[w][dd] : -1);
         G("-1};\n");
     }
-    // ---- P8, pair form (development switch): columns k0 (registers c*) and k1 (registers e*) share every read of the solve
-    //      factors and of kappa_d; a column is always in the same role, so its record stream exists once
-    auto gen_pair_columns = [&]() {
-        int dist = 5, fdist = 2, sdist = 2, pdist = 3;
-        if (const char *e = qss_devenv("QSS3_DIST")) std::sscanf(e, "%d,%d,%d,%d", &dist, &fdist, &sdist, &pdist);
-        std::vector<double> cost(N + 1);
-        for (int k = 0; k <= N; ++k) { cost[k] = 0.0; if (k < N) for (const Rec &r : rec[k]) cost[k] += 3.0 + r.tgt.size(); }
-        std::vector<int> by(N + 1);
-        for (int k = 0; k <= N; ++k) by[k] = k;
-        std::stable_sort(by.begin(), by.end(), [&](int a, int b) { return cost[a] > cost[b]; });      // the T column (no records) is last
-        std::vector<std::pair<int, int>> pr;
-        for (int i = 0, j = N; i <= j; ++i, --j) pr.push_back({by[i], i < j ? by[j] : -1});
-        std::vector<char> role(N + 1, 0);
-        for (auto &q : pr) if (q.second >= 0) role[q.second] = 1;
-        G("__device__ __forceinline__ void qss_gen_column2(const int k0, const int k1, const int mode, const unsigned sml, const unsigned sml2, const double *sc, double *jc0, double *jc1, const long long rs, const bool active) {\n    double ");
-        for (int s = 0; s < nsp; ++s) G("c%d, e%d%s", s, s, s + 1 < nsp ? ", " : ";\n");
-        for (int s = 0; s < nsp; ++s) G("    c%d = lS<%d>(sml);\n", s, (R_TV + s) * PITCH);
-        G("    if (k1 == %d) {\n", N);
-        for (int s = 0; s < nsp; ++s) G("        e%d = lG<%d>(sc);\n", s, (S_ET + s) * 256);
-        G("    } else {\n");
-        for (int s = 0; s < nsp; ++s) G("        e%d = c%d;\n", s, s);
-        G("    }\n");
-        for (int rl = 0; rl < 2; ++rl) {
-            const char v = rl ? 'e' : 'c';
-            G("    switch (%s) {\n", rl ? "k1" : "k0");
-            for (int k = 0; k < N; ++k) {
-                if (role[k] != rl) continue;
-                const std::vector<Rec> &rr = rec[k];
-                const int n = (int)rr.size();
-                if (!n) continue;
-                G("    case %d: {\n", k);
-                auto load_A = [&](int i) { if (i < n) { if (rr[i].from_smem) G("        const double A%d = lS<%d>(sml);\n", i, rr[i].src); else G("        const double A%d = lG<%d>(sc);\n", i, rr[i].src); } };
-                auto load_F = [&](int i) {
-                    if (i >= n) return;
-                    if (rr[i].f1 >= 0) G("        const double f%d = lS<%d>(sml);\n", i, rr[i].f1);
-                    if (rr[i].f2 >= 0) G("        const double h%d = lS<%d>(sml);\n", i, rr[i].f2);
-                };
-                for (int i = 0; i < dist; ++i) load_A(i);
-                for (int i = 0; i < fdist; ++i) load_F(i);
-                for (int i = 0; i < n; ++i) {
-                    load_A(i + dist);
-                    load_F(i + fdist);
-                    const Rec &r = rr[i];
-                    if (r.from_smem) G("        const double p%d = vmul(A%d, %.17g)", i, i, r.lit);
-                    else if (r.f1 >= 0) G("        const double p%d = vmul(A%d, f%d)", i, i, i);
-                    else G("        const double p%d = A%d", i, i);
-                    if (r.f2 >= 0) G(" * h%d", i);
-                    G(";");
-                    for (auto &t : r.tgt) {
-                        const int a = std::abs(t.second);
-                        if (a == 1) G(" %c%d %s= p%d;", v, t.first, t.second > 0 ? "+" : "-", i);
-                        else G(" %c%d = fma(%s%d.0, p%d, %c%d);", v, t.first, t.second > 0 ? "" : "-", a, i, v, t.first);
-                    }
-                    G("\n");
-                }
-                G("    } break;\n");
-            }
-            G("    default: break;\n    }\n");
-        }
-        G("    if (mode == 0) {\n");
-        {
-            std::vector<const Op *> ch[2];
-            size_t len[2] = {0, 0};
-            for (int gi = 0; gi < c.n_groups; ++gi) {
-                const int w = c.xpl->empty() ? (len[0] <= len[1] ? 0 : 1) : 0;
-                for (const Op &o : gops[gi]) { ch[w].push_back(&o); len[w] += 1 + o.terms.size(); }
-            }
-            std::vector<const Op *> seq;
-            for (size_t i = 0; i < std::max(ch[0].size(), ch[1].size()); ++i) {
-                if (i < ch[0].size()) seq.push_back(ch[0][i]);
-                if (i < ch[1].size()) seq.push_back(ch[1][i]);
-            }
-            auto load_op = [&](int i) {
-                if (i >= (int)seq.size()) return;
-                const Op &o = *seq[i];
-                for (size_t t = 0; t < o.terms.size(); ++t) G("    const double u%d_%d = lS<%d>(sml);\n", i, (int)t, o.terms[t].first * PITCH);
-                if (o.scale >= 0) G("    const double u%d_s = lS<%d>(sml);\n", i, o.scale * PITCH);
-            };
-            for (int i = 0; i < sdist; ++i) load_op(i);
-            for (int i = 0; i < (int)seq.size(); ++i) {
-                load_op(i + sdist);
-                const Op &o = *seq[i];
-                const int a = N + o.a;
-                for (size_t t = 0; t < o.terms.size(); ++t) {
-                    if (t == 0) G("    vfma(c%d, u%d_%d, c%d);", a, i, (int)t, N + o.terms[t].second);
-                    else G("    c%d = fma(u%d_%d, c%d, c%d);", a, i, (int)t, N + o.terms[t].second, a);
-                    G(" e%d = fma(u%d_%d, e%d, e%d);\n", a, i, (int)t, N + o.terms[t].second, a);
-                }
-                if (o.scale >= 0) {
-                    if (o.terms.empty()) G("    c%d = vmul(c%d, u%d_s);", a, a, i); else G("    c%d *= u%d_s;", a, i);
-                    G(" e%d *= u%d_s;\n", a, i);
-                }
-            }
-        }
-        {
-            std::vector<int> first_use((n_kq + 1) / 2, -1);
-            for (int i = 0; i < (int)kq.size(); ++i) for (int dir = 0; dir < 2; ++dir)
-                if (kq[i].idx[dir] >= 0 && first_use[kq[i].idx[dir] / 2] < 0) first_use[kq[i].idx[dir] / 2] = i;
-            auto load_k = [&](int i) {
-                if (i >= (int)kq.size()) return;
-                for (size_t pp = 0; pp < first_use.size(); ++pp) if (first_use[pp] == i) G("    const double2 kq%d = lS2<%d>(sml2);\n", (int)pp, KQ_BASE + (int)pp * 528);
-            };
-            for (int i = 0; i < pdist; ++i) load_k(i);
-            for (int i = 0; i < (int)kq.size(); ++i) {
-                load_k(i + pdist);
-                const KqRec &r = kq[i];
-                if (r.idx[0] >= 0 && r.idx[1] >= 0) {
-                    char ka[32], kb[32];
-                    std::snprintf(ka, sizeof ka, "kq%d.%c", r.idx[0] / 2, r.idx[0] % 2 ? 'y' : 'x');
-                    std::snprintf(kb, sizeof kb, "kq%d.%c", r.idx[1] / 2, r.idx[1] % 2 ? 'y' : 'x');
-                    G("    {   const double t = vfms(%s, c%d, %s * c%d), t2 = fma(%s, e%d, -(%s * e%d));", ka, N + r.q[0], kb, N + r.q[1], ka, N + r.q[0], kb, N + r.q[1]);
-                    for (auto &t : r.tgt) {
-                        const int a = std::abs(t.second);
-                        if (a == 1) G(" c%d %s= t; e%d %s= t2;", t.first, t.second > 0 ? "+" : "-", t.first, t.second > 0 ? "+" : "-");
-                        else G(" c%d = fma(%s%d.0, t, c%d); e%d = fma(%s%d.0, t2, e%d);", t.first, t.second > 0 ? "" : "-", a, t.first, t.first, t.second > 0 ? "" : "-", a, t.first);
-                    }
-                } else {
-                    const int dir = r.idx[0] >= 0 ? 0 : 1, sg = dir == 0 ? 1 : -1;
-                    char kn[32];
-                    std::snprintf(kn, sizeof kn, "kq%d.%c", r.idx[dir] / 2, r.idx[dir] % 2 ? 'y' : 'x');
-                    int anchor = -1;
-                    for (size_t u = 0; u < r.tgt.size(); ++u) if (std::abs(r.tgt[u].second) == 1) { anchor = (int)u; break; }
-                    G("    {  ");
-                    if (anchor < 0) G(" const double t = vmul(%s, c%d), t2 = %s * e%d;", kn, N + r.q[dir], kn, N + r.q[dir]);
-                    else {
-                        const bool pos = sg * r.tgt[anchor].second > 0;
-                        G(" %s(c%d, %s, c%d); e%d = fma(%s%s, e%d, e%d);", pos ? "vfma" : "vfnma", r.tgt[anchor].first, kn, N + r.q[dir],
-                          r.tgt[anchor].first, pos ? "" : "-", kn, N + r.q[dir], r.tgt[anchor].first);
-                    }
-                    for (size_t u = 0; u < r.tgt.size(); ++u) {
-                        if ((int)u == anchor) continue;
-                        const int sv = sg * r.tgt[u].second, a = std::abs(sv), tt = r.tgt[u].first;
-                        if (anchor < 0) G(" c%d = fma(%s%d.0, t, c%d); e%d = fma(%s%d.0, t2, e%d);", tt, sv > 0 ? "" : "-", a, tt, tt, sv > 0 ? "" : "-", a, tt);
-                        else if (a == 1) G(" c%d = fma(%s%s, c%d, c%d); e%d = fma(%s%s, e%d, e%d);", tt, sv > 0 ? "" : "-", kn, N + r.q[dir], tt, tt, sv > 0 ? "" : "-", kn, N + r.q[dir], tt);
-                        else G(" c%d = fma(%s%d.0 * %s, c%d, c%d); e%d = fma(%s%d.0 * %s, e%d, e%d);", tt, sv > 0 ? "" : "-", a, kn, N + r.q[dir], tt, tt, sv > 0 ? "" : "-", a, kn, N + r.q[dir], tt);
-                    }
-                }
-                G(" }\n");
-            }
-        }
-        G("    }\n    if (active) {\n");
-        for (int i = 0; i < N; ++i) G("        __stcs(jc0 + %d * rs, c%d);\n", i, i);
-        G("        if (k1 >= 0) {\n");
-        for (int i = 0; i < N; ++i) G("            __stcs(jc1 + %d * rs, e%d);\n", i, i);
-        G("        }\n    }\n}\n");
-        // pairs of each warp: longest-processing-time assignment by the records of the two columns
-        std::vector<double> pc(pr.size());
-        double prod_cost = 0.0;
-        for (const KqRec &r : kq) prod_cost += 3.0 + 2.0 * r.tgt.size();
-        for (size_t i = 0; i < pr.size(); ++i) pc[i] = 150.0 + prod_cost + 6.0 * (cost[pr[i].first] + (pr[i].second >= 0 ? cost[pr[i].second] : 0.0));
-        const std::vector<int> bin = lpt(pc, NWC);
-        size_t depth = 0;
-        std::vector<std::vector<int>> cols(NWC);
-        for (size_t i = 0; i < pr.size(); ++i) cols[bin[i]].push_back((int)i);
-        for (auto &cw : cols) depth = std::max(depth, cw.size());
-        for (int w = 1; w < NWC; w += 2) std::reverse(cols[w].begin(), cols[w].end());
-        G("#define QSS3_PAIRS 1\n#define QSS_GEN_DEPTH %d\n__constant__ int qss_gen_cols[] = {", (int)depth);
-        for (int w = 0; w < NWC; ++w) for (size_t dd = 0; dd < depth; ++dd) {
-            if (dd < cols[w].size()) G("%d, %d, ", pr[cols[w][dd]].first, pr[cols[w][dd]].second); else G("-1, -1, ");
-        }
-        G("-1};\n");
-    };
-    if (pair) gen_pair_columns();
     v.gen = G.s;
     v.nw = NW; v.smem_bytes = rows * PITCH; v.scratch_rows = srows; v.n_slot = n_slot;
     v.n_pp = 0; v.n_kq = n_kq; v.n_groups = (int)groups.size();

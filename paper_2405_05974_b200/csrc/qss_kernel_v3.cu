@@ -505,18 +505,10 @@ qss_v3_wdot(const __grid_constant__ QssV3 p) {
         // warp group hands its registers to the column warps for the sweep (setmaxnreg) and waits at the end-of-slab barrier.
         if (warp < G_NWC) {
             asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(G_REG_COL));
-#ifdef QSS3_PAIRS
-            for (int dd = 0; dd < QSS_GEN_DEPTH; ++dd) {
-                const int k0 = qss_gen_cols[(warp * QSS_GEN_DEPTH + dd) * 2], k1 = qss_gen_cols[(warp * QSS_GEN_DEPTH + dd) * 2 + 1];
-                if (k0 >= 0) qss_gen_column2(k0, k1, p.mode, sml, sm0 + lane * 16, sc, p.jac + (size_t)(unsigned)k0 * (size_t)ld + cell,
-                                             p.jac + (size_t)(unsigned)(k1 < 0 ? k0 : k1) * (size_t)ld + cell, (long long)(G_N + 1) * ld, active);
-            }
-#else
             for (int dd = 0; dd < QSS_GEN_DEPTH; ++dd) {
                 const int k = qss_gen_cols[warp * QSS_GEN_DEPTH + dd];
                 if (k >= 0) qss_gen_column(k, p.mode, sml, sm0 + lane * 16, sc, p.jac + (size_t)(unsigned)k * (size_t)ld + cell, (long long)(G_N + 1) * ld, active);
             }
-#endif
             asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(G_REG_BASE));
             asm volatile("bar.arrive 1, %0;" ::"n"(G_NW * 32));
         } else {
