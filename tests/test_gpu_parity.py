@@ -210,6 +210,31 @@ def test_chemkin_placeholder_troe_parameters(env, monkeypatch):
     _check(mech, C, T, n, f"cfg2 placeholder Troe {env}")
 
 
+@pytest.mark.parametrize("env", [{}, {"QSS_JIT": "0"}, {"QSS_VARIANT": "0"}])
+def test_species_with_their_own_mid_temperatures(env, monkeypatch):
+    """Real NASA-7 data give every species its own Tmid (the synthetic configs use 1000 K throughout).  Then a reaction's species
+    sit in different ranges for T between their breakpoints, the folded -ln Kc coefficients of the generated kernel do not exist
+     and the library must take another variant by itself -- with the same parity."""
+    import dataclasses
+    import paper_2405_05974_b200 as qss
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    mech = qss_synth.config_mechanism(2)
+    rng = np.random.default_rng(17)
+    nasa_T = mech.nasa_T.copy()
+    nasa_T[:, 1] = rng.uniform(900.0, 1500.0, size=nasa_T.shape[0])
+    mech = dataclasses.replace(mech, nasa_T=nasa_T)
+    qm = qss.QssMech(mech, 0)
+    variants = (qm.info.kernel_variant_wdot, qm.info.kernel_variant_jac)
+    qm.close()
+    assert 3 not in variants, variants
+    n = 160 + 3
+    C, T = qss_synth.config_states(2, n)
+    T[: n // 2] = rng.uniform(880.0, 1520.0, size=n // 2)          # half of the cells between the breakpoints
+    T[3] = nasa_T[0, 1]; T[4] = nasa_T[40, 1]                        # exactly at a species' Tmid (G9: high range)
+    _check(mech, C, np.ascontiguousarray(T), n, f"cfg2 per-species Tmid {env} variants {variants}")
+
+
 def test_paper_style_sampling():
     """States drawn the way the paper validates its Jacobian: C ~ U[1e-4, 1] mol/m^3 for every
     species, T ~ U[300, 1300] K (both NASA ranges, very small rate constants at the cold end)."""
