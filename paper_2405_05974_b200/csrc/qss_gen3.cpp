@@ -142,13 +142,14 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
     auto vrow = [&](int sp) { return sp < N ? R_V + sp : R_ONE; };                 // a QSS molecule reads 1.0 (y is not known yet)
     const double RGAS = 8.31446261815324;
     const long double LNP0R = std::log((long double)101325.0 / (long double)RGAS);
+    bool has_corr = false;                  // some reaction's species have different NASA-7 mid temperatures
     for (size_t g = 0; g < groups.size(); ++g) for (int l = 0; l < 32; ++l) {
         const int slot = 32 * (int)g + l;
         // a padding lane computes a harmless reaction and stores nothing
         IP(QSS3_I_KAP, slot) = R_KAP * PITCH; IP(QSS3_I_TB, slot) = -1;
         IP(QSS3_I_QF, slot) = IP(QSS3_I_QB, slot) = R_ONE * PITCH;
         for (int u = 0; u < QSS3_MAX_EFF; ++u) IP(QSS3_I_EFFS + u, slot) = R_ONE * PITCH;
-        DP(QSS3_D_TMID, slot) = 1000.0; DP(QSS3_D_I3, slot) = 1.0; DP(QSS3_D_I1, slot) = 1.0; DP(QSS3_D_ALPHA, slot) = 0.5;
+        DP(QSS3_D_TMID, slot) = DP(QSS3_D_TMAX, slot) = 1000.0; DP(QSS3_D_I3, slot) = 1.0; DP(QSS3_D_I1, slot) = 1.0; DP(QSS3_D_ALPHA, slot) = 0.5;
         if (l >= groups[g].count) continue;
         const int j = order[groups[g].first + l];
         const Reaction &r = R[j];
@@ -160,24 +161,42 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
             DP(QSS3_D_T2S, slot) = d->troe[4 * j + 3];
         }
         // -ln Kc = sum nu g/RT - dnu ln(P0/RT) as seven coefficients per NASA-7 range (reading G4; g/RT =
-        // a1 (1 - lnT) - a2 T/2 - a3 T^2/6 - a4 T^3/12 - a5 T^4/20 + a6/T - a7).  The species of a reaction must share Tmid.
+        // a1 (1 - lnT) - a2 T/2 - a3 T^2/6 - a4 T^3/12 - a5 T^4/20 + a6/T - a7).  ELO holds below the smallest Tmid of the
+        // reaction's species, EHI at and above the largest; between them (real thermodynamic data: every species has its own
+        // Tmid) the kernel adds to ELO the difference nu (hi - lo) of every species that is already in its high range.
+        DP(QSS3_D_TMAX, slot) = DP(QSS3_D_TMID, slot);
         if (r.mask & 2) {
-            double tmid = 0.0; bool have = false;
+            double tmin = 0.0, tmax = 0.0; bool have = false;
             for (const Term &x : r.net) {
                 const double tm = d->nasa_T[3 * x.sp + 1];
-                if (have && tm != tmid) { why = "the species of a reaction have different NASA-7 mid temperatures"; return false; }
-                tmid = tm; have = true;
+                tmin = have ? std::min(tmin, tm) : tm; tmax = have ? std::max(tmax, tm) : tm; have = true;
             }
-            DP(QSS3_D_TMID, slot) = have ? tmid : 1000.0;
+            DP(QSS3_D_TMID, slot) = have ? tmin : 1000.0;
+            DP(QSS3_D_TMAX, slot) = have ? tmax : 1000.0;
+            const size_t st = (size_t)n_slot;
+            auto fold = [&](const long double (&As)[7], long double dnu, double *e) {
+                e[0 * st] = (double)(As[0] - As[6] - dnu * LNP0R);
+                e[1 * st] = (double)(-As[0] + dnu);
+                e[2 * st] = (double)(-As[1] / 2.0L); e[3 * st] = (double)(-As[2] / 6.0L); e[4 * st] = (double)(-As[3] / 12.0L); e[5 * st] = (double)(-As[4] / 20.0L);
+                e[6 * st] = (double)As[5];
+            };
             for (int rg = 0; rg < 2; ++rg) {
                 long double As[7] = {0, 0, 0, 0, 0, 0, 0};
                 for (const Term &x : r.net) { const double *a = (rg == 0 ? d->nasa_lo : d->nasa_hi) + 7 * x.sp; for (int i = 0; i < 7; ++i) As[i] += (long double)x.nu * (long double)a[i]; }
-                double *e = &DP((rg == 0 ? QSS3_D_ELO : QSS3_D_EHI), slot);
-                const size_t st = (size_t)n_slot;
-                e[0 * st] = (double)(As[0] - As[6] - (long double)r.dnu * LNP0R);
-                e[1 * st] = (double)(-As[0] + (long double)r.dnu);
-                e[2 * st] = (double)(-As[1] / 2.0L); e[3 * st] = (double)(-As[2] / 6.0L); e[4 * st] = (double)(-As[3] / 12.0L); e[5 * st] = (double)(-As[4] / 20.0L);
-                e[6 * st] = (double)As[5];
+                fold(As, (long double)r.dnu, &DP((rg == 0 ? QSS3_D_ELO : QSS3_D_EHI), slot));
+            }
+            if (have && tmin != tmax) {
+                if (r.net.size() > (size_t)QSS3_MAX_CORR) { why = "a reaction changes more than 8 species that have their own NASA-7 mid temperatures"; return false; }
+                int nc = 0;
+                for (const Term &x : r.net) {
+                    long double As[7];
+                    for (int i = 0; i < 7; ++i) As[i] = (long double)x.nu * ((long double)d->nasa_hi[7 * x.sp + i] - (long double)d->nasa_lo[7 * x.sp + i]);
+                    DP(QSS3_D_CORR + 8 * nc, slot) = d->nasa_T[3 * x.sp + 1];
+                    fold(As, 0.0L, &DP(QSS3_D_CORR + 8 * nc + 1, slot));
+                    ++nc;
+                }
+                IP(QSS3_I_NCORR, slot) = nc;
+                has_corr = true;
             }
         }
         int ne = 0;
@@ -276,6 +295,7 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
     G("#define R_V %d\n#define R_ONE %d\n#define R_Y %d\n#define R_T %d\n#define R_LNT %d\n#define R_INVT %d\n#define R_CT %d\n#define R_CL %d\n#define R_XP %d\n#define R_TV %d\n#define R_DLM %d\n#define R_KAP %d\n#define R_KQ %d\n#define R_STAGE %d\n",
       R_V, R_ONE, R_Y, R_T, R_LNT, R_INVT, R_CT, R_CL, R_XP, R_TV, R_DLM, R_KAP, R_KQ, R_STAGE);
     G("#define KQ_BASE %d\n", KQ_BASE);
+    G("#define G_HAS_CORR %d\n", has_corr ? 1 : 0);
     G("#define S_K %d\n#define S_KQ %d\n#define S_ET %d\n#define S_DT %d\n#define G_NKQ %d\n#define G_KQ_PER_WARP %d\n#define G_SROWS %d\n", S_K, S_KQ, S_ET, S_DT, n_kq,
       std::max(1, (n_kq + NW - 1) / NW), srows);
     // ---- interpreter tables (int32 words, appended to the int parameter blob, staged in shared memory once per block)

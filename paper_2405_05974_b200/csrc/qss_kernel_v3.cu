@@ -117,6 +117,11 @@ __device__ __forceinline__ int4 tab_rows4(const unsigned sm0, const int x) {
 struct RateCommon {
     double lnA, beta, EaR, tmid, elo[7], ehi[7];
     int flags, kap, tb;
+#if G_HAS_CORR
+    double tmax;                 // species with their own NASA-7 mid temperatures: [tmid, tmax) is corrected species by species
+    int ncorr;
+    const double *corr;          // p.dP + QSS3_D_CORR rows of this lane's slot
+#endif
 };
 __device__ __forceinline__ void qss3_load_common(RateCommon &r, const QssV3 &p, const int slot) {
     const double *dP = p.dP + slot;
@@ -126,6 +131,10 @@ __device__ __forceinline__ void qss3_load_common(RateCommon &r, const QssV3 &p, 
     r.EaR = ldg_nc(dP + (size_t)QSS3_D_EAR * G_NSLOT); r.tmid = ldg_nc(dP + (size_t)QSS3_D_TMID * G_NSLOT);
 #pragma unroll
     for (int i = 0; i < 7; ++i) { r.elo[i] = ldg_nc(dP + (size_t)(QSS3_D_ELO + i) * G_NSLOT); r.ehi[i] = ldg_nc(dP + (size_t)(QSS3_D_EHI + i) * G_NSLOT); }
+#if G_HAS_CORR
+    r.tmax = ldg_nc(dP + (size_t)QSS3_D_TMAX * G_NSLOT); r.ncorr = ldg_nc(iP + (size_t)QSS3_I_NCORR * G_NSLOT);
+    r.corr = dP + (size_t)QSS3_D_CORR * G_NSLOT;
+#endif
 }
 struct RateTyped {
     double lnA0, beta0, E0R, alpha, i3, i1, T2s, effv[QSS3_MAX_EFF];
@@ -148,14 +157,39 @@ __device__ __forceinline__ void qss3_rate_cell(const RateCommon &r, const RateTy
     const double T = lds(smc + R_T * G_PITCH), lnT = lds(smc + R_LNT * G_PITCH), invT = lds(smc + R_INVT * G_PITCH);
     const double lnkinf = fma(-r.EaR, invT, fma(r.beta, lnT, r.lnA));
     const bool lo = T < r.tmid;                                  // NASA-7 range (reading G9: T < Tmid low, else high)
+#if G_HAS_CORR
+    double e0 = lo ? r.elo[0] : r.ehi[0], e1 = lo ? r.elo[1] : r.ehi[1], e2 = lo ? r.elo[2] : r.ehi[2], e3 = lo ? r.elo[3] : r.ehi[3];
+    double e4 = lo ? r.elo[4] : r.ehi[4], e5 = lo ? r.elo[5] : r.ehi[5], e6 = lo ? r.elo[6] : r.ehi[6];
+    const bool between = !lo && T < r.tmax;                      // some species of the reaction are in their high range, some are not
+    if (between) {                                               // (a band of a few hundred K; the lanes of the other reactions wait)
+        e0 = r.elo[0]; e1 = r.elo[1]; e2 = r.elo[2]; e3 = r.elo[3]; e4 = r.elo[4]; e5 = r.elo[5]; e6 = r.elo[6];
+        // (no branch on the species' range: every load of the loop is independent of the others, so they overlap in the L2)
+#pragma unroll 2
+        for (int i = 0; i < r.ncorr; ++i) {
+            const double *cp = r.corr + (size_t)(8 * i) * G_NSLOT;
+            const double tm = __ldg(cp);
+            const double d0 = __ldg(cp + (size_t)1 * G_NSLOT), d1 = __ldg(cp + (size_t)2 * G_NSLOT), d2 = __ldg(cp + (size_t)3 * G_NSLOT);
+            const double d3 = __ldg(cp + (size_t)4 * G_NSLOT), d4 = __ldg(cp + (size_t)5 * G_NSLOT), d5 = __ldg(cp + (size_t)6 * G_NSLOT);
+            const double d6 = __ldg(cp + (size_t)7 * G_NSLOT);
+            const double m = T < tm ? 0.0 : 1.0;
+            e0 = fma(m, d0, e0); e1 = fma(m, d1, e1); e2 = fma(m, d2, e2); e3 = fma(m, d3, e3);
+            e4 = fma(m, d4, e4); e5 = fma(m, d5, e5); e6 = fma(m, d6, e6);
+        }
+    }
+#else
     const double e0 = lo ? r.elo[0] : r.ehi[0], e1 = lo ? r.elo[1] : r.ehi[1], e2 = lo ? r.elo[2] : r.ehi[2], e3 = lo ? r.elo[3] : r.ehi[3];
     const double e4 = lo ? r.elo[4] : r.ehi[4], e5 = lo ? r.elo[5] : r.ehi[5], e6 = lo ? r.elo[6] : r.ehi[6];
+#endif
     const double lniKc = fma(e6, invT, fma(e1, lnT, fma(T, fma(T, fma(T, fma(T, e5, e4), e3), e2), e0)));     // -ln Kc
     double k = QEXP(lnkinf);
     const double iKc = QEXP(lniKc);
 #if QSS3_JAC
     // T d ln Kc/dT = sum nu h/RT - dnu = e6/T - e1 - T (e2 + T (2 e3 + T (3 e4 + 4 e5 T)))   (e: coefficients of -ln Kc)
+#if G_HAS_CORR
+    const double f3 = between ? 2.0 * e3 : lo ? flo[0] : fhi[0], f4 = between ? 3.0 * e4 : lo ? flo[1] : fhi[1], f5 = between ? 4.0 * e5 : lo ? flo[2] : fhi[2];
+#else
     const double f3 = lo ? flo[0] : fhi[0], f4 = lo ? flo[1] : fhi[1], f5 = lo ? flo[2] : fhi[2];
+#endif
     const double w = fma(T, fma(T, fma(T, f5, f4), f3), e2);
     dlnKc = (r.flags & 2) ? (fma(e6, invT, -e1) - T * w) * invT : 0.0;
     dlnk = (r.beta + r.EaR * invT) * invT;

@@ -6,17 +6,18 @@
 #include "qss_stdint.h"
 
 // doubles / ints per rate-task slot in the parameter blobs (slot = 32 * group + lane: one reaction; layout [param][slot])
-#define QSS3_NDP 33
+#define QSS3_NDP 98
 #define QSS3_NIP 14
 #define QSS3_MAX_EFF 8           // non-unity third-body efficiencies per reaction held in registers
+#define QSS3_MAX_CORR 8          // species of a reaction with their own NASA-7 breakpoint (range corrections of -ln Kc)
 
 // double parameters
 #define QSS3_D_LNA 0             // ln A, beta, Ea/R (high-pressure limit for fall-off reactions)
 #define QSS3_D_BETA 1
 #define QSS3_D_EAR 2
-#define QSS3_D_TMID 3            // NASA-7 range breakpoint shared by the species of the reaction
-#define QSS3_D_ELO 4             // [7] coefficients of -ln Kc below Tmid: e0 + e1 lnT + T(e2 + T(e3 + T(e4 + T e5))) + e6/T
-#define QSS3_D_EHI 11            // [7] the same at and above Tmid
+#define QSS3_D_TMID 3            // smallest NASA-7 range breakpoint Tmid among the species of the reaction
+#define QSS3_D_ELO 4             // [7] coefficients of -ln Kc below it: e0 + e1 lnT + T(e2 + T(e3 + T(e4 + T e5))) + e6/T
+#define QSS3_D_EHI 11            // [7] the same at and above the LARGEST Tmid of the reaction's species
 #define QSS3_D_LNA0 18           // low-pressure limit ln A0, beta0, E0/R
 #define QSS3_D_BETA0 19
 #define QSS3_D_E0R 20
@@ -25,6 +26,8 @@
 #define QSS3_D_I1 23
 #define QSS3_D_T2S 24
 #define QSS3_D_EFFV 25           // [8] alpha_k - 1
+#define QSS3_D_TMAX 33           // largest Tmid among the species of the reaction (= QSS3_D_TMID when they share one)
+#define QSS3_D_CORR 34           // [QSS3_MAX_CORR][8] per species: its Tmid, then the 7 coefficients nu (hi - lo) that its high range adds to ELO
 // int parameters
 #define QSS3_I_FLAGS 0           // mask (bits 0-1) | type << 2 | valid << 4 | n_eff << 8
 #define QSS3_I_KAP 1             // byte offset of the k_f / kappa_f / Q_j row (the reverse row follows G_M rows later)
@@ -32,6 +35,7 @@
 #define QSS3_I_QF 3              // byte offset of the V row of the QSS reactant of the forward direction (none: the 1.0 row)
 #define QSS3_I_QB 4
 #define QSS3_I_EFFS 5            // [8] byte offsets of the V rows of the species with non-unity efficiency
+#define QSS3_I_NCORR 13          // entries of QSS3_D_CORR (0 when the species share Tmid)
 
 struct QssV3 {
     const double *C, *T;
