@@ -155,6 +155,12 @@ def test_specialised_jacobian_kernel_compiles_without_a_gpu():
     sm_100a (no device needed); a mechanism outside kernel variant 1 has nothing to specialise."""
     for mech in (qss_synth.toy_dag(), qss_synth.config_mechanism(1)):
         assert qss.specialise_check(mech, (10, 0)) > 10000
+    # species with their own NASA-7 mid temperatures: the image carries the range-correction path of the rate tasks (G_HAS_CORR)
+    import dataclasses
+    mech = qss_synth.config_mechanism(1)
+    nasa_T = mech.nasa_T.copy()
+    nasa_T[:, 1] = np.linspace(950.0, 1400.0, nasa_T.shape[0])
+    assert qss.specialise_check(dataclasses.replace(mech, nasa_T=nasa_T), (10, 0)) > qss.specialise_check(mech, (10, 0))
     with pytest.raises(qss.QssError) as ei:
         qss.specialise_check(qss_synth.config_mechanism(5), (10, 0))
     assert ei.value.code == -5
