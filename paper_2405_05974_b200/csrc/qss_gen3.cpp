@@ -163,7 +163,7 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
         // -ln Kc = sum nu g/RT - dnu ln(P0/RT) as seven coefficients per NASA-7 range (reading G4; g/RT =
         // a1 (1 - lnT) - a2 T/2 - a3 T^2/6 - a4 T^3/12 - a5 T^4/20 + a6/T - a7).  ELO holds below the smallest Tmid of the
         // reaction's species, EHI at and above the largest; between them (real thermodynamic data: every species has its own
-        // Tmid) the kernel adds to ELO the difference nu (hi - lo) of every species that is already in its high range.
+        // Tmid) there is one more set per interval between consecutive breakpoints, fetched by the kernel when a cell needs it.
         DP(QSS3_D_TMAX, slot) = DP(QSS3_D_TMID, slot);
         if (r.mask & 2) {
             double tmin = 0.0, tmax = 0.0; bool have = false;
@@ -186,16 +186,22 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
                 fold(As, (long double)r.dnu, &DP((rg == 0 ? QSS3_D_ELO : QSS3_D_EHI), slot));
             }
             if (have && tmin != tmax) {
-                if (r.net.size() > (size_t)QSS3_MAX_CORR) { why = "a reaction changes more than 8 species that have their own NASA-7 mid temperatures"; return false; }
-                int nc = 0;
-                for (const Term &x : r.net) {
-                    long double As[7];
-                    for (int i = 0; i < 7; ++i) As[i] = (long double)x.nu * ((long double)d->nasa_hi[7 * x.sp + i] - (long double)d->nasa_lo[7 * x.sp + i]);
-                    DP(QSS3_D_CORR + 8 * nc, slot) = d->nasa_T[3 * x.sp + 1];
-                    fold(As, 0.0L, &DP(QSS3_D_CORR + 8 * nc + 1, slot));
-                    ++nc;
+                std::vector<double> bp;                       // distinct breakpoints, ascending
+                for (const Term &x : r.net) bp.push_back(d->nasa_T[3 * x.sp + 1]);
+                std::sort(bp.begin(), bp.end());
+                bp.erase(std::unique(bp.begin(), bp.end()), bp.end());
+                if (bp.size() > (size_t)QSS3_MAX_CORR) { why = "the species of a reaction have more than 8 different NASA-7 mid temperatures"; return false; }
+                const int nb = (int)bp.size() - 2;            // inner breakpoints
+                for (int i = 0; i < nb; ++i) DP(QSS3_D_CORR + i, slot) = bp[i + 1];
+                for (int iv = 0; iv <= nb; ++iv) {            // interval [bp[iv], bp[iv + 1]): species s is in its high range iff Tmid_s <= bp[iv]
+                    long double As[7] = {0, 0, 0, 0, 0, 0, 0};
+                    for (const Term &x : r.net) {
+                        const double *a = (d->nasa_T[3 * x.sp + 1] <= bp[iv] ? d->nasa_hi : d->nasa_lo) + 7 * x.sp;
+                        for (int i = 0; i < 7; ++i) As[i] += (long double)x.nu * (long double)a[i];
+                    }
+                    fold(As, (long double)r.dnu, &DP(QSS3_D_CORR + 8 + 7 * iv, slot));
                 }
-                IP(QSS3_I_NCORR, slot) = nc;
+                IP(QSS3_I_NCORR, slot) = nb;
                 has_corr = true;
             }
         }

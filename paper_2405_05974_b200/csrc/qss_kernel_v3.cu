@@ -118,7 +118,7 @@ struct RateCommon {
     double lnA, beta, EaR, tmid, elo[7], ehi[7];
     int flags, kap, tb;
 #if G_HAS_CORR
-    double tmax;                 // species with their own NASA-7 mid temperatures: [tmid, tmax) is corrected species by species
+    double tmax;                 // species with their own NASA-7 mid temperatures: [tmid, tmax) has one coefficient set per interval
     int ncorr;
     const double *corr;          // p.dP + QSS3_D_CORR rows of this lane's slot
 #endif
@@ -162,19 +162,12 @@ __device__ __forceinline__ void qss3_rate_cell(const RateCommon &r, const RateTy
     double e4 = lo ? r.elo[4] : r.ehi[4], e5 = lo ? r.elo[5] : r.ehi[5], e6 = lo ? r.elo[6] : r.ehi[6];
     const bool between = !lo && T < r.tmax;                      // some species of the reaction are in their high range, some are not
     if (between) {                                               // (a band of a few hundred K; the lanes of the other reactions wait)
-        e0 = r.elo[0]; e1 = r.elo[1]; e2 = r.elo[2]; e3 = r.elo[3]; e4 = r.elo[4]; e5 = r.elo[5]; e6 = r.elo[6];
-        // (no branch on the species' range: every load of the loop is independent of the others, so they overlap in the L2)
-#pragma unroll 2
-        for (int i = 0; i < r.ncorr; ++i) {
-            const double *cp = r.corr + (size_t)(8 * i) * G_NSLOT;
-            const double tm = __ldg(cp);
-            const double d0 = __ldg(cp + (size_t)1 * G_NSLOT), d1 = __ldg(cp + (size_t)2 * G_NSLOT), d2 = __ldg(cp + (size_t)3 * G_NSLOT);
-            const double d3 = __ldg(cp + (size_t)4 * G_NSLOT), d4 = __ldg(cp + (size_t)5 * G_NSLOT), d5 = __ldg(cp + (size_t)6 * G_NSLOT);
-            const double d6 = __ldg(cp + (size_t)7 * G_NSLOT);
-            const double m = T < tm ? 0.0 : 1.0;
-            e0 = fma(m, d0, e0); e1 = fma(m, d1, e1); e2 = fma(m, d2, e2); e3 = fma(m, d3, e3);
-            e4 = fma(m, d4, e4); e5 = fma(m, d5, e5); e6 = fma(m, d6, e6);
-        }
+        int iv = 0;                                              // inner breakpoints at or below T: all loads independent
+#pragma unroll
+        for (int i = 0; i < QSS3_MAX_CORR - 2; ++i) if (i < r.ncorr) iv += T < __ldg(r.corr + (size_t)i * G_NSLOT) ? 0 : 1;
+        const double *cp = r.corr + (size_t)(8 + 7 * iv) * G_NSLOT;
+        e0 = __ldg(cp); e1 = __ldg(cp + (size_t)1 * G_NSLOT); e2 = __ldg(cp + (size_t)2 * G_NSLOT); e3 = __ldg(cp + (size_t)3 * G_NSLOT);
+        e4 = __ldg(cp + (size_t)4 * G_NSLOT); e5 = __ldg(cp + (size_t)5 * G_NSLOT); e6 = __ldg(cp + (size_t)6 * G_NSLOT);
     }
 #else
     const double e0 = lo ? r.elo[0] : r.ehi[0], e1 = lo ? r.elo[1] : r.ehi[1], e2 = lo ? r.elo[2] : r.ehi[2], e3 = lo ? r.elo[3] : r.ehi[3];

@@ -6,10 +6,10 @@
 #include "qss_stdint.h"
 
 // doubles / ints per rate-task slot in the parameter blobs (slot = 32 * group + lane: one reaction; layout [param][slot])
-#define QSS3_NDP 98
+#define QSS3_NDP 91
 #define QSS3_NIP 14
 #define QSS3_MAX_EFF 8           // non-unity third-body efficiencies per reaction held in registers
-#define QSS3_MAX_CORR 8          // species of a reaction with their own NASA-7 breakpoint (range corrections of -ln Kc)
+#define QSS3_MAX_CORR 8          // distinct NASA-7 breakpoints Tmid among the species of one reaction
 
 // double parameters
 #define QSS3_D_LNA 0             // ln A, beta, Ea/R (high-pressure limit for fall-off reactions)
@@ -27,7 +27,9 @@
 #define QSS3_D_T2S 24
 #define QSS3_D_EFFV 25           // [8] alpha_k - 1
 #define QSS3_D_TMAX 33           // largest Tmid among the species of the reaction (= QSS3_D_TMID when they share one)
-#define QSS3_D_CORR 34           // [QSS3_MAX_CORR][8] per species: its Tmid, then the 7 coefficients nu (hi - lo) that its high range adds to ELO
+#define QSS3_D_CORR 34           // [8 + 7 x 7] reactions whose species have different Tmid: up to 6 breakpoints strictly between TMID and TMAX
+                                 // (ascending, rows 0..5), then one coefficient set of -ln Kc per interval between consecutive breakpoints
+                                 // (set i at rows 8 + 7 i .. 8 + 7 i + 6, i = number of inner breakpoints <= T)
 // int parameters
 #define QSS3_I_FLAGS 0           // mask (bits 0-1) | type << 2 | valid << 4 | n_eff << 8
 #define QSS3_I_KAP 1             // byte offset of the k_f / kappa_f / Q_j row (the reverse row follows G_M rows later)
@@ -35,7 +37,7 @@
 #define QSS3_I_QF 3              // byte offset of the V row of the QSS reactant of the forward direction (none: the 1.0 row)
 #define QSS3_I_QB 4
 #define QSS3_I_EFFS 5            // [8] byte offsets of the V rows of the species with non-unity efficiency
-#define QSS3_I_NCORR 13          // entries of QSS3_D_CORR (0 when the species share Tmid)
+#define QSS3_I_NCORR 13          // inner breakpoints in QSS3_D_CORR
 
 struct QssV3 {
     const double *C, *T;

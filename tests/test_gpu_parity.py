@@ -214,7 +214,7 @@ def test_chemkin_placeholder_troe_parameters(env, monkeypatch):
 def test_species_with_their_own_mid_temperatures(env, monkeypatch):
     """Real NASA-7 data give every species its own Tmid (the synthetic configs use 1000 K throughout).  Then a reaction's species
     sit in different ranges for T between their breakpoints: the generated kernel folds -ln Kc below the smallest and above the
-    largest Tmid of a reaction and corrects species by species in between (qss_gen3.cpp); the other variants evaluate g/RT per
+    largest Tmid of a reaction and once per interval between consecutive breakpoints in between (qss_gen3.cpp); the other variants evaluate g/RT per
     species.  Same parity gates for all of them."""
     import dataclasses
     import paper_2405_05974_b200 as qss
