@@ -216,6 +216,7 @@ bool build_v3(const V1Ctx &c, QssCompiled &out, std::string &why) {
         IP(QSS3_I_QF, slot) = (r.q[0] >= 0 ? R_Y + r.q[0] : R_ONE) * PITCH;
         IP(QSS3_I_QB, slot) = (r.q[1] >= 0 ? R_Y + r.q[1] : R_ONE) * PITCH;
     }
+    if (!has_corr) v.dP.resize((size_t)QSS3_D_TMAX * n_slot);      // (the rows behind the efficiencies are read by images with G_HAS_CORR only)
     // ---- tasks: (group, cell chunk) dealt to the warps by cost -------------------------------------------------------
     // A warp takes a CONTIGUOUS stretch of the line "group 0 cells 0..31, group 1 cells 0..31, ..." of equal cost, so that it
     // loads the parameters of at most two or three groups per slab and every group is loaded about once per block.
