@@ -106,12 +106,13 @@ def run_reference(args, cfg: int, rank: int):
     C, T = qss_synth.config_states(cfg, n)
     n = min(n, C.shape[1])
     om = oracle.OracleMech(mech)
-    cores = oracle.max_threads()
+    # every host core this process may use, also under torchrun (which exports OMP_NUM_THREADS=1 to its ranks)
+    cores = max(oracle.max_threads(), len(os.sched_getaffinity(0)))
     for _ in range(args.warmup):
-        oracle.evaluate(om, C, T, min(n, 256), want_jac=True)
+        oracle.evaluate(om, C, T, min(n, 256), want_jac=True, nthreads=cores)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle.evaluate(om, C, T, n, want_jac=True)
+        oracle.evaluate(om, C, T, n, want_jac=True, nthreads=cores)
     dt = (time.perf_counter() - t0) / args.steps
     v = n / dt
     sample = f"first {n} cells of cfg{cfg} per step (explicit-formula fp64 oracle, OpenMP over cells)"
