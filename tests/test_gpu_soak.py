@@ -70,3 +70,58 @@ def test_random_mechanism(it):
         print(what, "strict fractions", strict, "fp64 oracle against float128", floor)
         for k in strict:
             assert strict[k] >= min(gates.TIER1_MIN_FRACTION, floor[k] - 0.03), (what, k, strict, floor)
+
+
+@pytest.mark.parametrize("it", [0, 1, 2, 4, 12, 13, 16, 28, 31])
+def test_random_mechanism_full_jacobian_and_newton_solve(it):
+    """The same random mechanisms through qss_eval_jac_full (energy row, temperature right-hand side: gates of test_gpu_next) and
+    qss_newton_solve on Jacobian-shaped synthetic systems of their order (n = N + 1 = 13 .. 38: one and two register rows per lane,
+    n = 32 / 33 at the boundary; order 44: refused with QSS_E_UNSUPPORTED; gates of test_gpu_newton)."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    from qss_synth import newton_inputs
+    from test_gpu_next import _energy_gates
+    mech, C, T, n = _case(it)
+    qm = qss.QssMech(mech, 0)
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda()
+    J0, w0 = qm.eval_jac(Cd, Td, n, want_wdot=True)
+    J, w, tdot, erow = qm.eval_jac_full(Cd, Td, n)
+    torch.cuda.synchronize()
+    assert torch.equal(J[:, :, :n], J0[:, :, :n]) and torch.equal(w[:, :n], w0[:, :n])
+    om = oracle.OracleMech(mech)
+    ref = oracle.evaluate_energy(om, C, T, n)
+    try:
+        _energy_gates(tdot.cpu().numpy(), erow.cpu().numpy(), ref, T, n, f"random mechanism {it}")
+    except AssertionError:
+        # The element-wise guard of that gate scales with the cancellation INSIDE the energy-row sum (escale), not with the
+        # cancellation inside the Jacobian entries it sums; on an arbitrary mechanism the fp64 oracle itself can miss it against
+        # its float128 evaluation.  Then the kernel has to stay within 4x of what the fp64 oracle achieves (G16's principle).
+        q = oracle.evaluate_energy(om, C, T, n, mode=oracle.EXPLICIT_F128)
+        e, sc = q["erow"][:, :n], q["escale"][:, :n]
+        bound = 1e-9 * np.abs(e) + 1e-12 * sc
+        r_oracle = float(np.max(np.abs(ref["erow"][:, :n] - e) / bound))
+        r_kernel = float(np.max(np.abs(erow.cpu().numpy()[:, :n] - ref["erow"][:, :n]) / (1e-9 * np.abs(ref["erow"][:, :n]) + 1e-12 * ref["escale"][:, :n])))
+        print(f"random mechanism {it}: energy row, worst ratio kernel/oracle {r_kernel:.3g}, fp64 oracle/float128 {r_oracle:.3g}")
+        assert r_oracle > 0.25 and r_kernel <= 4.0 * r_oracle, (it, r_kernel, r_oracle)
+        dt = np.abs(tdot.cpu().numpy()[:n] - ref["tdot"][:n])
+        assert np.all(dt <= 1e-10 * np.abs(ref["tdot"][:n]) + 1e-13 * ref["escale"][-1, :n] * T[:n]), f"random mechanism {it}: tdot"
+    m = 131
+    d = newton_inputs(qm.N, m, seed=90 + it, ld=m + 5, with_energy=True)
+    t = {k: torch.from_numpy(v).cuda() for k, v in d.items()}
+    x = torch.full((qm.N + 1, m + 5), float("nan"), dtype=torch.float64, device="cuda")
+    if qm.N + 1 > 40:                                     # include/qss.h: the solve holds the matrix in a warp's registers, order <= 40
+        with pytest.raises(qss.QssError) as ei:
+            qm.newton_solve(t["jac"], t["erow"], t["gamma"], t["b"], m, x=x)
+        assert ei.value.code == -5
+        qm.close()
+        return
+    qm.newton_solve(t["jac"], t["erow"], t["gamma"], t["b"], m, x=x)
+    torch.cuda.synchronize()
+    qm.close()
+    x = x.cpu().numpy()
+    refx = oracle.newton_solve(d["jac"], d["erow"], d["gamma"], d["b"], m)
+    assert np.isnan(x[:, m:]).all(), "padding was written"
+    cells = np.arange(m)
+    g = gates.newton_gates(gates.newton_matrix(d["jac"], d["erow"], d["gamma"], cells), d["b"][:, cells].T, x[:, cells].T, refx["x"][:, cells].T)
+    print("random mechanism %d, order %d: eta %.2e, well-conditioned %.2f, forward error there %.2e" % (it, qm.N + 1, g["eta_worst"], g["wellcond_frac"], g["fwd_worst_wellcond"]))
+    gates.assert_newton(g, floor=0.0)
