@@ -125,3 +125,26 @@ def test_random_mechanism_full_jacobian_and_newton_solve(it):
     g = gates.newton_gates(gates.newton_matrix(d["jac"], d["erow"], d["gamma"], cells), d["b"][:, cells].T, x[:, cells].T, refx["x"][:, cells].T)
     print("random mechanism %d, order %d: eta %.2e, well-conditioned %.2f, forward error there %.2e" % (it, qm.N + 1, g["eta_worst"], g["wellcond_frac"], g["fwd_worst_wellcond"]))
     gates.assert_newton(g, floor=0.0)
+
+
+@pytest.mark.parametrize("it", [6, 13, 29])
+def test_random_mechanism_many_slabs_per_block(it):
+    """20011 cells: every persistent block runs four or five slabs, so the staging of the next slab's inputs under the sweep and the
+    reuse of the shared-memory rows and of the scratch slab are exercised on mechanisms whose row layout differs from the configs'."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    mech = _case(it)[0]
+    n = 20011
+    C, T = make_states(mech.n_nqss, n, seed=100 + it)
+    qm = qss.QssMech(mech, 0)
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda()
+    J, w = qm.eval_jac(Cd, Td, n, want_wdot=True)
+    w2, _ = qm.eval_wdot(Cd, Td, n, want_cqss=True)
+    torch.cuda.synchronize()
+    qm.close()
+    ref = oracle.evaluate(oracle.OracleMech(mech), C, T, n, want_jac=True, want_scale=True)
+    for g in (gates.wdot_gates(w.cpu().numpy(), ref["wdot"], ref["S"], n), gates.wdot_gates(w2.cpu().numpy(), ref["wdot"], ref["S"], n)):
+        assert g["finite"] and g["tier2_all"] and g["tier1_frac"] >= gates.TIER1_MIN_FRACTION, (it, g)
+    gj = gates.jac_gates(J.cpu().numpy(), ref["jac"], ref["jscale"], n)
+    assert gj["finite"] and gj["cell_tier2_all"] and gj["col_tier2_all"] and gj["col_tier1_frac"] >= gates.TIER1_MIN_FRACTION, (it, gj)
+    assert gj["cell_tier1_frac"] >= 0.95, (it, gj)          # (0.966 on mechanism 29, the fp64 oracle's own fraction against float128: see above)
