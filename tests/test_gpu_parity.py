@@ -236,6 +236,40 @@ def test_species_with_their_own_mid_temperatures(env, monkeypatch):
     _check(mech, C, np.ascontiguousarray(T), n, f"cfg2 per-species Tmid {env} variants {variants}")
 
 
+@pytest.mark.parametrize("env", [{}, {"QSS_VARIANT": "2"}, {"QSS_VARIANT": "0"}])
+def test_extreme_temperatures_and_concentration_scales(env, monkeypatch):
+    """Outside the sampled ranges: T = 200 .. 6000 K (beyond both NASA ranges: the polynomials extrapolate, rate constants span
+    hundreds of decades), whole cells scaled by 1e-150 .. 1e12.  Where the preconditions of include/qss.h fail (a cell scaled into
+    underflow, a cell with one species only, an all-zero cell: a QSS species without consumption, M = 0) the oracle's result is
+    not finite and the kernel's must not be either: no silent number."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    mech = qss_synth.config_mechanism(2)
+    n = 64
+    C, T = qss_synth.config_states(2, n)
+    C = C.copy(); T = T.copy()
+    T[0:6] = (250.0, 300.0, 3500.0, 5000.0, 200.0, 6000.0)
+    C[:, 6] *= 1e-20; C[:, 7] *= 1e-150; C[:, 9] *= 1e6; C[:, 10] *= 1e12
+    bad = [8, 11, 12, 13]
+    C[:, 8] *= 1e-300
+    C[:, 11] = 0.0; C[3, 11] = 1.0
+    C[:, 12] = 5e-324
+    C[:, 13] = 0.0
+    good = np.array([c for c in range(n) if c not in bad])
+    with np.errstate(all="ignore"):
+        ref = oracle.evaluate(oracle.OracleMech(mech), C, T, n, want_jac=True, want_scale=True)
+    got = _gpu_eval(mech, C, T, n)
+    for c in bad:
+        fin_ref = np.isfinite(ref["wdot"][:, c]).all() and np.isfinite(ref["jac"][:, :, c]).all()
+        fin_got = np.isfinite(got["wdot"][:, c]).all() and np.isfinite(got["jac"][:, :, c]).all()
+        assert fin_got == fin_ref, (c, fin_ref, fin_got)
+    gw = gates.wdot_gates(got["wdot"][:, good], ref["wdot"][:, good], ref["S"][:, good], len(good))
+    gj = gates.jac_gates(got["jac"][:, :, good], ref["jac"][:, :, good], ref["jscale"][:, :, good], len(good))
+    print(env, "wdot tier 2 worst %.2g; Jacobian tier 2 worst %.2g / %.2g" % (gw["tier2_worst"], gj["cell_tier2_worst"], gj["col_tier2_worst"]))
+    assert gw["finite"] and gw["tier2_all"] and gj["finite"] and gj["cell_tier2_all"] and gj["col_tier2_all"]
+    assert gw["tier1_frac"] >= 0.99 and gj["cell_tier1_frac"] >= 0.99
+
+
 def test_paper_style_sampling():
     """States drawn the way the paper validates its Jacobian: C ~ U[1e-4, 1] mol/m^3 for every
     species, T ~ U[300, 1300] K (both NASA ranges, very small rate constants at the cold end)."""
