@@ -116,3 +116,51 @@ def test_adaptive_integrator_with_ignition_time_against_oracle(name, n, attempts
     if ld > n:
         assert np.array_equal(Cg[:, n:], C[:, n:], equal_nan=True) and np.array_equal(tg[n:], np.zeros(ld - n))
     qm.close()
+
+
+def test_integrator_sequence_and_newton_solve_replay_from_a_cuda_graph():
+    """qss_bdf1_advance is a FIXED launch sequence on the caller's stream (no host decision, no allocation, no synchronisation:
+    include/qss.h), and so are qss_eval_jac_full and qss_newton_solve: captured once in a CUDA graph and replayed on restored
+    inputs they give bit for bit what the eager calls gave."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    mech = qss_synth.config_mechanism(2)
+    n = 200
+    C, T = qss_synth.config_states(2, n)
+    ld = C.shape[1]
+    om = oracle.OracleMech(mech)
+    dt = _dt(om, C, T, n, 3.0, 3)
+    qm = qss.QssMech(mech, 0)
+    C0 = torch.from_numpy(C).cuda(); T0 = torch.from_numpy(T).cuda(); dtd = torch.from_numpy(dt).cuda()
+    Ce, Te = C0.clone(), T0.clone()
+    ws = qm.bdf1_advance(Ce, Te, dtd, 2, 3, n)                                   # eager, default stream
+    J0, w0, td0, er0 = qm.eval_jac_full(Ce, Te, n)
+    gamma = dtd.clone()
+    b = torch.cat([w0, td0[None, :]], 0).contiguous()
+    x0 = qm.newton_solve(J0, er0, gamma, b, n)
+    torch.cuda.synchronize()
+    Cg, Tg = C0.clone(), T0.clone()
+    J = torch.empty_like(J0); w = torch.empty_like(w0); td = torch.empty_like(td0); er = torch.empty_like(er0); x = torch.empty_like(x0)
+    bg = torch.empty_like(b)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        qm.bdf1_advance(Cg, Tg, dtd, 2, 3, n, workspace=ws)                      # warm-up on the side stream (run-time compilation done)
+        qm.eval_jac_full(Cg, Tg, n, jac=J, wdot=w, tdot=td, erow=er)
+        qm.newton_solve(J, er, gamma, b, n, x=x)
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            qm.bdf1_advance(Cg, Tg, dtd, 2, 3, n, workspace=ws)
+            qm.eval_jac_full(Cg, Tg, n, jac=J, wdot=w, tdot=td, erow=er)
+            bg[: qm.N].copy_(w); bg[qm.N].copy_(td)
+            qm.newton_solve(J, er, gamma, bg, n, x=x)
+        for _ in range(2):                                                       # two replays, inputs restored before each
+            Cg.copy_(C0); Tg.copy_(T0)
+            for a in (J, w, td, er, x, bg):
+                a.fill_(float("nan"))
+            g.replay()
+        s.synchronize()
+    assert torch.equal(Cg[:, :n], Ce[:, :n]) and torch.equal(Tg[:n], Te[:n])
+    assert torch.equal(J[:, :, :n], J0[:, :, :n]) and torch.equal(er[:, :n], er0[:, :n]) and torch.equal(x[:, :n], x0[:, :n])
+    qm.close()
