@@ -270,6 +270,29 @@ def test_extreme_temperatures_and_concentration_scales(env, monkeypatch):
     assert gw["tier1_frac"] >= 0.99 and gj["cell_tier1_frac"] >= 0.99
 
 
+@pytest.mark.parametrize("cfg,n", [(2, (1 << 18) + 77), (1, 1 << 18), (3, 1 << 14)])
+def test_run_to_run_bit_identity(cfg, n):
+    """No kernel uses atomics or depends on the order in which warps or blocks run: repeated calls on the same inputs, with dozens
+    of slabs per persistent block, return the same bits (a race between the warps of a block or between a block's consecutive slabs
+    would show here; compute-sanitizer is not available on this pool)."""
+    import paper_2405_05974_b200 as qss
+    torch = _torch()
+    mech = qss_synth.config_mechanism(cfg)
+    C, T = qss_synth.config_states(cfg, n)
+    qm = qss.QssMech(mech, 0)
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda()
+    J0, w0 = qm.eval_jac(Cd, Td, n, want_wdot=True)
+    ww0, y0 = qm.eval_wdot(Cd, Td, n, want_cqss=True)
+    assert torch.equal(w0[:, :n], ww0[:, :n])              # the two kernels compute wdot by the same operations
+    for _ in range(4):
+        J, w = qm.eval_jac(Cd, Td, n, want_wdot=True)
+        ww, y = qm.eval_wdot(Cd, Td, n, want_cqss=True)
+        torch.cuda.synchronize()
+        assert torch.equal(J[:, :, :n], J0[:, :, :n]) and torch.equal(w[:, :n], w0[:, :n])
+        assert torch.equal(ww[:, :n], ww0[:, :n]) and torch.equal(y[:, :n], y0[:, :n])
+    qm.close()
+
+
 def test_paper_style_sampling():
     """States drawn the way the paper validates its Jacobian: C ~ U[1e-4, 1] mol/m^3 for every
     species, T ~ U[300, 1300] K (both NASA ranges, very small rate constants at the cold end)."""
