@@ -286,14 +286,17 @@ int eval_wdot(const oracle_mech_t *m, const S *C, const S &T, Rates<S> &rt, Clos
         }
         const S Q = rate[0] - rate[1], Sabs = rate[0] + rate[1];
         const Side re = reactants(m, j), pr = products(m, j);
-        for (int i = 0; i < pr.n; ++i) if (pr.sp[i] < N) { out.wdot[pr.sp[i]] = out.wdot[pr.sp[i]] + S((double)pr.nu[i]) * Q; }
-        for (int i = 0; i < re.n; ++i) if (re.sp[i] < N) { out.wdot[re.sp[i]] = out.wdot[re.sp[i]] - S((double)re.nu[i]) * Q; }
-        // scale S_i = sum_j |nu_ij| (r_f + r_r) with the NET coefficient nu_ij = nu'' - nu'
+        // Eq. 3: wdot_i = sum_j nu_ij Q_j with the NET coefficient nu_ij = nu'' - nu'; a species that stands on
+        // both sides of a reaction with the same coefficient (a collision partner written out) gets no term at all.  The scale
+        // S_i = sum_j |nu_ij| (r_f + r_r) uses the same coefficient.
         for (int s = 0; s < N; ++s) {
             int net = 0;
             for (int i = 0; i < pr.n; ++i) if (pr.sp[i] == s) net += pr.nu[i];
             for (int i = 0; i < re.n; ++i) if (re.sp[i] == s) net -= re.nu[i];
-            if (net != 0) out.Sscale[s] = out.Sscale[s] + S((double)std::abs(net)) * Sabs;
+            if (net != 0) {
+                out.wdot[s] = out.wdot[s] + S((double)net) * Q;
+                out.Sscale[s] = out.Sscale[s] + S((double)std::abs(net)) * Sabs;
+            }
         }
     }
     return 0;
