@@ -207,3 +207,88 @@ def test_yaml_ingestion_gives_the_same_description_as_chemkin():
         with pytest.raises(fe.MechanismError) as e:
             fe.parse_yaml(bad)
         assert msg in str(e.value), (msg, str(e.value))
+
+
+# ---- the same ingestion on the syntax real mechanism files use -----------------------------------------------------------------
+_NAMES2 = {"A2": "H2", "B2": "O2", "AB": "OH", "A2B": "H2O", "A": "H", "B": "O", "AB2": "HO2", "A2B2": "H2O2"}
+TEXT2 = """! lower-case keywords, D exponents, tabs, species names with brackets and dashes, a THERMO block without ALL,
+! every species with its own mid temperature, LOW / TROE with blanks, a three-parameter TROE line, DUPLICATE / DUP
+elements
+h  o
+end
+species
+H2 O2 OH H2O
+H O HO2 H2O2 CH2(S) C2H4OOH1-2
+end
+thermo
+   300.000  1000.000  5000.000
+%s
+end
+reactions   cal/mole  moles
+H+O2<=>O+OH                 3.547D+15 -0.406 1.6599E+4   ! D exponent, no blanks in the equation
+O+H2=H+OH\t\t0.508E+05   2.67   0.629E+04
+2OH(+M)<=>H2O2(+M)          1.11e14 -0.37 0.0
+     low  /  2.01E+17   -0.584  -2293.00/
+     troe/  0.7346   94.00  1756.00  5182.00 /
+     H2/2.00/ H2O/6.00/
+H+O2(+M)=HO2(+M)  1.475E+12 0.60 0.00
+   LOW/6.366E+20 -1.72 524.8/
+   TROE/0.8 1E-30 1E+30/
+   H2/2.0/ H2O/11./ O2/0.78/
+H+OH+M=H2O+M     3.800E+22 -2.00 0.0
+   H2/2.5/ H2O/12/
+HO2+H=>2OH        7.079E+13 0.00 295.0
+HO2+HO2=H2O2+O2   4.200E+14 0.00 1.1982E+04
+ DUPLICATE
+HO2+HO2=H2O2+O2   1.300E+11 0.00 -1.6293E+3
+ DUP
+CH2(S)+H2=>H2+H+H   1.0E+13 0.0 0.0
+C2H4OOH1-2=>H2O2+CH2(S)  2.0E+10 0.5 1000.0
+end
+""" % "\n".join([nasa_record(_NAMES2[n], c, a1, a6, a7, tmid=1000.0 + 37.0 * i) for i, (n, c, a1, a6, a7) in enumerate(SPECIES)]
+                + [nasa_record("CH2(S)", [("H", 2)], 3.4, 500.0, 1.0, tmid=1392.0),
+                   nasa_record("C2H4OOH1-2", [("H", 2), ("O", 2)], 5.1, -15000.0, 2.0, tmid=1388.0)])
+
+
+def test_parse_the_syntax_of_real_mechanism_files():
+    d = fe.parse_chemkin(TEXT2, qss=["CH2(S)", "O"])
+    assert d.n_reac == 10 and d.n_qss == 2 and d.n_nqss == 8
+    assert list(d.rtype) == [0, 0, 2, 2, 1, 0, 0, 0, 0, 0]
+    assert sorted(d.nasa_T[:, 1]) == sorted([1000.0 + 37.0 * i for i in range(8)] + [1392.0, 1388.0])
+    assert list(d.troe[2]) == [0.7346, 94.0, 1756.0, 5182.0] and list(d.troe[3]) == [0.8, 1e-30, 1e30, 1e30]
+    assert np.isclose(d.arr[0, 0], 3.547e15 * 1e-6) and np.isclose(d.arr[0, 2], 1.6599e4 * 4.184)      # cm^3/mol/s -> m^3/mol/s, cal -> J
+    dl = fe.linearise(d, "reaction")
+    assert dl.n_reac == 10                                   # no quadratic coupling among {CH2(S), O} in this set
+    qss.validate(dl)
+
+
+def test_species_on_both_sides_of_a_reaction_gets_no_term():
+    """PAPER.md Eq. 3 (L62-64): wdot_i = sum_j nu_ij Q_j with the NET coefficient.  A collision partner written out on both sides
+    (A + B => B + C) has nu = 0: its production rate is exactly zero, however fast the reaction is, and the other species see
+    k [A][B] (closed form).  In TEXT2 (CH2(S) + H2 => H2 + 2 H next to slow H2 reactions) the float64 oracle then agrees with its
+    float128 evaluation within the wdot gates; accumulated side by side, -Q + Q would leave rounding noise of Q ~ 1e11 in a rate of 1e-2."""
+    import gates
+    text = """ELEMENTS H O END
+SPECIES A2 B2 AB END
+THERMO ALL
+   300.000  1000.000  3500.000
+%s
+END
+REACTIONS MOLES KELVINS
+A2 + B2 => B2 + 2AB     1.0E+20  0.0  0.0
+END
+""" % "\n".join([nasa_record("A2", [("H", 2)], 3.5, -1000.0, 1.0), nasa_record("B2", [("O", 2)], 3.6, -1100.0, 2.0), nasa_record("AB", [("H", 1)], 2.5, 25000.0, -0.5)])
+    d = fe.parse_chemkin(text, qss=[])
+    C = np.array([[0.3], [7.0], [0.01]]); T = np.array([1234.0])
+    w = oracle.evaluate(oracle.OracleMech(d), C, T, 1, want_jac=False)["wdot"][:, 0]
+    q = 1.0e20 * 1e-6 * 0.3 * 7.0                                   # cm^3/mol/s -> m^3/mol/s
+    assert w[1] == 0.0 and np.isclose(w[0], -q, rtol=1e-14) and np.isclose(w[2], 2.0 * q, rtol=1e-14)
+    d2 = fe.linearise(fe.parse_chemkin(TEXT2, qss=["CH2(S)", "O"]), "reaction")
+    n = 64
+    rng = np.random.default_rng(4)
+    C = np.ascontiguousarray(10.0 ** rng.uniform(-4.0, 1.0, size=(d2.n_nqss, n))); T = rng.uniform(900.0, 1500.0, size=n)
+    om = oracle.OracleMech(d2)
+    r64 = oracle.evaluate(om, C, T, n, want_jac=False)
+    r128 = oracle.evaluate(om, C, T, n, want_jac=False, mode=oracle.EXPLICIT_F128)
+    g = gates.wdot_gates(r64["wdot"], r128["wdot"], r128["S"], n)
+    assert g["tier2_all"] and g["tier1_frac"] >= 0.99, g

@@ -168,6 +168,32 @@ def test_parsed_mechanism_runs_on_the_kernels():
     qm.close()
 
 
+def test_parsed_mechanism_with_per_species_mid_temperatures():
+    """The syntax and the thermodynamic data of real mechanism files (test_frontend.TEXT2: every species its own Tmid, three-parameter
+    Troe line, duplicates, irreversible steps) through the generated kernel: the range-interval sets of -ln Kc (qss_gen3.cpp)."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    from paper_2405_05974_b200 import frontend as fe
+    from test_frontend import TEXT2
+    d = fe.linearise(fe.parse_chemkin(TEXT2, qss=["CH2(S)", "O"]), "reaction")
+    n = 300
+    rng = np.random.default_rng(4)
+    C = np.ascontiguousarray(10.0 ** rng.uniform(-4.0, 1.0, size=(d.n_nqss, n)))
+    T = rng.uniform(900.0, 1500.0, size=n)                  # mostly BETWEEN the species' breakpoints (1000 .. 1392 K)
+    T[:8] = sorted(set(d.nasa_T[:, 1]))[:8]                 # and exactly on some of them
+    qm = qss.QssMech(d, 0)
+    assert qm.info.kernel_variant_jac == 3
+    J, w = qm.eval_jac(torch.from_numpy(C).cuda(), torch.from_numpy(T).cuda(), n, want_wdot=True)
+    torch.cuda.synchronize()
+    ref = oracle.evaluate(oracle.OracleMech(d), C, T, n, want_scale=True)
+    gw = gates.wdot_gates(w.cpu().numpy(), ref["wdot"], ref["S"], n)
+    gj = gates.jac_gates(J.cpu().numpy(), ref["jac"], ref["jscale"], n)
+    print("parsed mechanism, per-species Tmid: wdot tier 1 %.3f, tier 2 worst %.3g; Jacobian cell tier 1 %.3f" % (gw["tier1_frac"], gw["tier2_worst"], gj["cell_tier1_frac"]))
+    assert gw["finite"] and gw["tier2_all"] and gw["tier1_frac"] >= 0.99
+    assert gj["finite"] and gj["cell_tier2_all"] and gj["col_tier2_all"] and gj["cell_tier1_frac"] >= 0.99
+    qm.close()
+
+
 @pytest.mark.parametrize("name,n", [("cfg1", 4096), ("cfg2", 2048 + 19), ("toy_dag", 77), ("cfg3", 96 + 5)])
 def test_full_jacobian_in_one_call(name, n):
     """qss_eval_jac_full: jac and wdot bit for bit those of qss_eval_jac; tdot and the energy row against the oracle with the gates
