@@ -244,6 +244,11 @@ HO2+HO2=H2O2+O2   1.300E+11 0.00 -1.6293E+3
  DUP
 CH2(S)+H2=>H2+H+H   1.0E+13 0.0 0.0
 C2H4OOH1-2=>H2O2+CH2(S)  2.0E+10 0.5 1000.0
+O+H2O2=>O+2OH   3.0E+12 0.0 500.0                 ! a QSS species as the collision partner, written out on both sides
+CH2(S)+H2O<=>CH2(S)+H+OH  1.0E+11 0.0 9000.0
+O+H2O2(+M)=>O+2OH(+M)   3.0E+12 0.0 500.0
+ LOW/1.0E+16 0.0 100.0/
+ TROE/0.6 100.0 1800.0/
 end
 """ % "\n".join([nasa_record(_NAMES2[n], c, a1, a6, a7, tmid=1000.0 + 37.0 * i) for i, (n, c, a1, a6, a7) in enumerate(SPECIES)]
                 + [nasa_record("CH2(S)", [("H", 2)], 3.4, 500.0, 1.0, tmid=1392.0),
@@ -252,13 +257,13 @@ end
 
 def test_parse_the_syntax_of_real_mechanism_files():
     d = fe.parse_chemkin(TEXT2, qss=["CH2(S)", "O"])
-    assert d.n_reac == 10 and d.n_qss == 2 and d.n_nqss == 8
-    assert list(d.rtype) == [0, 0, 2, 2, 1, 0, 0, 0, 0, 0]
+    assert d.n_reac == 13 and d.n_qss == 2 and d.n_nqss == 8
+    assert list(d.rtype) == [0, 0, 2, 2, 1, 0, 0, 0, 0, 0, 0, 0, 2]
     assert sorted(d.nasa_T[:, 1]) == sorted([1000.0 + 37.0 * i for i in range(8)] + [1392.0, 1388.0])
     assert list(d.troe[2]) == [0.7346, 94.0, 1756.0, 5182.0] and list(d.troe[3]) == [0.8, 1e-30, 1e30, 1e30]
     assert np.isclose(d.arr[0, 0], 3.547e15 * 1e-6) and np.isclose(d.arr[0, 2], 1.6599e4 * 4.184)      # cm^3/mol/s -> m^3/mol/s, cal -> J
     dl = fe.linearise(d, "reaction")
-    assert dl.n_reac == 10                                   # no quadratic coupling among {CH2(S), O} in this set
+    assert dl.n_reac == 13                                   # no quadratic coupling among {CH2(S), O} in this set
     qss.validate(dl)
 
 
