@@ -148,3 +148,35 @@ def test_random_mechanism_many_slabs_per_block(it):
     gj = gates.jac_gates(J.cpu().numpy(), ref["jac"], ref["jscale"], n)
     assert gj["finite"] and gj["cell_tier2_all"] and gj["col_tier2_all"] and gj["col_tier1_frac"] >= gates.TIER1_MIN_FRACTION, (it, gj)
     assert gj["cell_tier1_frac"] >= 0.95, (it, gj)          # (0.966 on mechanism 29, the fp64 oracle's own fraction against float128: see above)
+
+
+@pytest.mark.parametrize("it", [2, 13, 28])
+def test_random_mechanism_adaptive_integrator(it):
+    """qss_ignition_advance on random mechanisms of order 32, 13 and 31 (the comparison of test_gpu_bdf1: accept / reject decisions,
+    times and step sizes bit for bit, ignition times, states; cells within 1e-6 of the acceptance threshold are left out)."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    from test_gpu_bdf1 import _dt
+    mech, C, T, n = _case(it)
+    n = min(n, 80); attempts, iters, rtol, dT_ign = 8, 3, 1e-6, 0.05
+    om = oracle.OracleMech(mech)
+    ld = C.shape[1]
+    dt0 = _dt(om, C, T, n, 30.0, 3)
+    t_end = float(np.median(dt0[:n]) * 6.0)
+    trace = []
+    ref = oracle.ignition_advance(om, C, T, dt0, np.zeros(ld), t_end, attempts, iters, n, rtol=rtol, dT_ign=dT_ign, trace=trace)
+    qm = qss.QssMech(mech, 0)
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda(); T0d = Td.clone()
+    dtd = torch.from_numpy(dt0).cuda(); td = torch.zeros(ld, dtype=torch.float64, device="cuda")
+    tig = torch.full((ld,), float("nan"), dtype=torch.float64, device="cuda")
+    qm.ignition_advance(Cd, Td, dtd, td, t_end, attempts, iters, n, t_ign=tig, T0=T0d, dT_ign=dT_ign, rtol=rtol)
+    torch.cuda.synchronize()
+    qm.close()
+    Cg, Tg, dtg, tg, tigg = (x.cpu().numpy() for x in (Cd, Td, dtd, td, tig))
+    sure = ~(np.abs(np.array(trace) - 1.0) <= 1e-6).any(0) & np.isfinite(ref["T"][:n])
+    assert sure.mean() >= 0.9 and int((attempts - ref["accepted"][:n][sure]).sum()) > 0
+    assert np.array_equal(tg[:n][sure], ref["t"][:n][sure]) and np.array_equal(dtg[:n][sure], ref["dt"][:n][sure])
+    assert np.array_equal(tigg[:n][sure], ref["t_ign"][:n][sure], equal_nan=True)
+    eC = (np.abs(Cg[:, :n] - ref["C"][:, :n]).max(0) / np.abs(ref["C"][:, :n]).max(0))[sure]
+    eT = (np.abs(Tg[:n] - ref["T"][:n]) / ref["T"][:n])[sure]
+    assert eC.max() <= 1e-8 and eT.max() <= 1e-10, (eC.max(), eT.max())
