@@ -180,3 +180,38 @@ def test_random_mechanism_adaptive_integrator(it):
     eC = (np.abs(Cg[:, :n] - ref["C"][:, :n]).max(0) / np.abs(ref["C"][:, :n]).max(0))[sure]
     eT = (np.abs(Tg[:n] - ref["T"][:n]) / ref["T"][:n])[sure]
     assert eC.max() <= 1e-8 and eT.max() <= 1e-10, (eC.max(), eT.max())
+
+
+@pytest.mark.parametrize("it", [0, 4, 13, 34])
+def test_random_mechanism_cheap_jacobians_pattern_and_fixed_step_integrator(it):
+    """The remaining entry points on random mechanisms: constant-QSS and zero-QSS Jacobians against the oracle's (tier 2), entries
+    outside the structural pattern exactly zero, qss_bdf1_advance against the oracle's integrator (tolerances of test_gpu_bdf1)."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    from test_gpu_bdf1 import _dt
+    mech, C, T, n = _case(it)
+    n = min(n, 96)
+    om = oracle.OracleMech(mech)
+    qm = qss.QssMech(mech, 0)
+    Cd = torch.from_numpy(C).cuda(); Td = torch.from_numpy(T).cuda()
+    for mode, omode in ((1, oracle.JAC_CONST_QSS), (2, oracle.JAC_ZERO_QSS)):
+        J = qm.eval_jac_approx(Cd, Td, mode, n)
+        J = J[0] if isinstance(J, tuple) else J
+        ref = oracle.evaluate(om, C, T, n, want_jac=True, want_scale=True, mode=omode)
+        g = gates.jac_gates(J.cpu().numpy(), ref["jac"], ref["jscale"], n)
+        assert g["finite"] and g["cell_tier2_all"] and g["col_tier2_all"], (it, mode, g)
+    pat = qss.jac_pattern(mech, 0)
+    J = qm.eval_jac(Cd, Td, n).cpu().numpy()[:, :, :n]
+    assert not (pat == 0).any() or np.abs(J[pat == 0]).max() == 0.0
+    dt = _dt(om, C, T, n, 2.0, 3)
+    Cr, Tr = oracle.bdf1_advance(om, C, T, dt, 2, 3, n)
+    C2 = torch.from_numpy(C).cuda(); T2 = torch.from_numpy(T).cuda()
+    qm.bdf1_advance(C2, T2, torch.from_numpy(dt).cuda(), 2, 3, n)
+    torch.cuda.synchronize()
+    qm.close()
+    Cg, Tg = C2.cpu().numpy(), T2.cpu().numpy()
+    ok = np.isfinite(Tr[:n]) & np.isfinite(Cr[:, :n]).all(0)
+    assert ok.mean() >= 0.9 and not np.isfinite(Tg[:n][~ok]).any()
+    eC = (np.abs(Cg[:, :n] - Cr[:, :n]).max(0) / np.abs(Cr[:, :n]).max(0))[ok]
+    eT = (np.abs(Tg[:n] - Tr[:n]) / Tr[:n])[ok]
+    assert eC.max() <= 1e-8 and eT.max() <= 1e-10, (it, eC.max(), eT.max())
