@@ -214,6 +214,15 @@ int qss_mech_jac_pattern(const qss_mech_desc_t *desc, int mode, uint8_t *pattern
 int qss_jac_pack(const qss_mech_t *mech, int64_t ncells, int64_t ld, int32_t nnz, const int32_t *idx, const double *jac,
                  double *packed, void *stream);
 
+/* NEXT-2, output layout for external batched solvers (the Jacobian goes to a batched dense direct solver, which
+ * wants one contiguous matrix per cell).  qss_jac_to_aos: out[c][i][j] = J_c[i][j] for the cells c < ncells, rows i < N from `jac`
+ * (layout of qss_eval_jac), and, when erow != NULL, row N from `erow` (layout of qss_eval_energy): rows = N or N + 1, cols = N + 1;
+ * row-major out[(c*rows + i)*cols + j], or column-major (LAPACK) out[(c*cols + j)*rows + i] when col_major != 0.  `out`: DEVICE,
+ * ncells*rows*cols doubles, 8-byte aligned, written completely for c < ncells; must not overlap the inputs.  Pure data movement
+ * (bit-exact), one kernel on `stream`, no workspace.  Errors: QSS_E_INVALID (NULL pointer, ncells < 0, ld < ncells). */
+int qss_jac_to_aos(const qss_mech_t *mech, int64_t ncells, int64_t ld, const double *jac, const double *erow_or_null, int col_major,
+                   double *out, void *stream);
+
 /* NEXT-3: the paper's own treatment of the temperature column (d wdot / dT "via finite difference by computing the
  * species' production rate twice at different temperatures"; L234: central differences, perturbation 1e-4; reading G22).
  * Same outputs as qss_eval_jac, except that column N of jac is

@@ -17,7 +17,7 @@ from . import build as _build
 __all__ = ["lib", "QssMech", "QssError", "EXPORTS", "STATUS"]
 
 EXPORTS = ["qss_mech_create", "qss_mech_validate", "qss_mech_specialise_check", "qss_mech_destroy", "qss_mech_info", "qss_mech_qss_order", "qss_eval_wdot",
-           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_newton_solve", "qss_newton_specialise_check", "qss_bdf1_workspace_bytes", "qss_bdf1_advance", "qss_ignition_advance", "qss_jac_fdt_workspace_bytes", "qss_eval_jac_fdt", "qss_mech_jac_pattern", "qss_jac_pack", "qss_eval_jac_full", "qss_eval_wdot_static", "qss_bench_species_sums", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
+           "qss_eval_jac", "qss_eval_jac_approx", "qss_eval_energy", "qss_newton_solve", "qss_newton_specialise_check", "qss_bdf1_workspace_bytes", "qss_bdf1_advance", "qss_ignition_advance", "qss_jac_fdt_workspace_bytes", "qss_eval_jac_fdt", "qss_mech_jac_pattern", "qss_jac_pack", "qss_jac_to_aos", "qss_eval_jac_full", "qss_eval_wdot_static", "qss_bench_species_sums", "qss_host_scratch_bytes", "qss_eval_jac_host", "qss_bench_dfma", "qss_last_error"]
 STATUS = {0: "QSS_OK", -1: "QSS_E_INVALID", -2: "QSS_E_QUADRATIC", -3: "QSS_E_QSS_FANOUT", -4: "QSS_E_NO_SINK",
           -5: "QSS_E_UNSUPPORTED", -6: "QSS_E_CUDA", -7: "QSS_E_UNBALANCED"}
 
@@ -76,6 +76,7 @@ def lib():
         L.qss_eval_jac_full.restype = ct.c_int; L.qss_eval_jac_full.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp, ct.c_size_t, vp]
         L.qss_mech_jac_pattern.restype = ct.c_int; L.qss_mech_jac_pattern.argtypes = [vp, ct.c_int, vp]
         L.qss_jac_pack.restype = ct.c_int; L.qss_jac_pack.argtypes = [vp, i64, i64, ct.c_int32, vp, vp, vp, vp]
+        L.qss_jac_to_aos.restype = ct.c_int; L.qss_jac_to_aos.argtypes = [vp, i64, i64, vp, vp, ct.c_int, vp, vp]
         L.qss_ignition_advance.restype = ct.c_int
         L.qss_ignition_advance.argtypes = [vp, i64, i64, vp, vp, vp, vp, ct.c_double, vp, vp, ct.c_double, ct.c_int, ct.c_int, ct.c_double, ct.c_double, ct.c_double, vp, ct.c_size_t, vp]
         L.qss_jac_fdt_workspace_bytes.restype = ct.c_size_t; L.qss_jac_fdt_workspace_bytes.argtypes = [vp, i64]
@@ -336,6 +337,19 @@ class QssMech:
             packed = torch.empty((idx.numel(), ld), dtype=torch.float64, device=jac.device)
         _check(lib().qss_jac_pack(self._h, ncells, ld, idx.numel(), _ptr(idx), _ptr(jac), _ptr(packed), self._stream()))
         return packed
+
+    def jac_to_aos(self, jac, erow=None, ncells=None, col_major=False, out=None):
+        """One contiguous matrix per cell for external batched solvers (qss_jac_to_aos): [ncells, rows, N+1] row-major, or
+        [ncells, N+1, rows] (the column-major matrix) when col_major; rows = N + 1 with the energy row, else N."""
+        import torch
+        ld = jac.shape[2]
+        ncells = ld if ncells is None else int(ncells)
+        rows = self.N + 1 if erow is not None else self.N
+        assert jac.is_contiguous() and (erow is None or erow.is_contiguous())
+        if out is None:
+            out = torch.empty((ncells, self.N + 1, rows) if col_major else (ncells, rows, self.N + 1), dtype=torch.float64, device=jac.device)
+        _check(lib().qss_jac_to_aos(self._h, ncells, ld, _ptr(jac), _ptr(erow), int(bool(col_major)), _ptr(out), self._stream()))
+        return out
 
     def bdf1_advance(self, C, T, dt, nsub, newton_iters, ncells=None, workspace=None):
         """Advances (C, T) IN PLACE by `nsub` backward-Euler substeps of size dt per cell (qss_bdf1_advance)."""

@@ -463,6 +463,22 @@ extern "C" int qss_jac_pack(const qss_mech_t *m, int64_t ncells, int64_t ld, int
     return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_jac_pack launch");
 }
 
+// ---- NEXT-2: AoS export for external batched solvers (kernel in qss_driver.cu) --------------------------------------------------------
+cudaError_t qss_launch_jac_aos(int N, int rows, int64_t ncells, int64_t ld, const double *jac, const double *erow, int col_major, double *out,
+                               cudaStream_t stream);
+
+extern "C" int qss_jac_to_aos(const qss_mech_t *m, int64_t ncells, int64_t ld, const double *jac, const double *erow, int col_major, double *out,
+                              void *stream) {
+    if (!m) return fail(QSS_E_INVALID, "mech is NULL");
+    if (ncells < 0 || ld < ncells) return fail(QSS_E_INVALID, "need 0 <= ncells <= ld");
+    if (ncells == 0) return QSS_OK;
+    if (!jac || !out) return fail(QSS_E_INVALID, "NULL device pointer");
+    DeviceGuard guard(m->device);
+    const int N = m->c.tab.N;
+    cudaError_t e = qss_launch_jac_aos(N, erow ? N + 1 : N, ncells, ld, jac, erow, col_major != 0, out, (cudaStream_t)stream);
+    return e == cudaSuccess ? QSS_OK : cuda_fail(e, "qss_jac_to_aos launch");
+}
+
 // ---- NEXT-3: temperature column by finite differences (reading G22; kernels in qss_driver.cu) ---------------
 cudaError_t qss_launch_fdT_perturb(int64_t ncells, const double *T, double *Tp, double *Tm, cudaStream_t stream);
 cudaError_t qss_launch_fdT_column(int N, int64_t ncells, int64_t ld, const double *wp, const double *wm, const double *Tp, const double *Tm, double *jac,

@@ -111,3 +111,41 @@ cudaError_t qss_launch_jac_pack(int nnz, int64_t ncells, int64_t ld, const int32
     qss_jac_pack_kernel<<<grid, 256, 0, stream>>>(nnz, ncells, ld, idx, jac, out);
     return cudaGetLastError();
 }
+
+// ---- NEXT-2 ("optional AoS output layout for external batched solvers"; the Jacobian is handed
+// to a batched dense solver that wants one contiguous matrix per cell): the SoA Jacobian [entry][cell] (and the energy row) as
+// out[cell][rows][cols], row-major or column-major.  A tile of 32 output entries x 32 cells goes through shared memory: reads are
+// coalesced over cells, writes over the entries of one cell.  Pure data movement: bit-exact.
+namespace {
+__global__ void __launch_bounds__(256) qss_jac_aos_kernel(int N, int rows, int64_t ncells, int64_t ld, const double *__restrict__ jac,
+                                                           const double *__restrict__ erow, int col_major, double *__restrict__ out) {
+    __shared__ double tile[32][33];
+    const int cols = N + 1, E = rows * cols;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t c0 = (int64_t)blockIdx.x * 32;
+    const int o0 = blockIdx.y * 32;
+    for (int u = w; u < 32; u += 8) {                          // output entry o0 + u of the cells c0 .. c0 + 31
+        const int o = o0 + u;
+        const int64_t c = c0 + lane;
+        if (o < E && c < ncells) {
+            const int i = col_major ? o % rows : o / cols, j = col_major ? o / rows : o % cols;
+            tile[u][lane] = i < N ? jac[((size_t)i * cols + j) * ld + c] : erow[(size_t)j * ld + c];
+        }
+    }
+    __syncthreads();
+    for (int u = w; u < 32; u += 8) {                          // cell c0 + u, output entries o0 .. o0 + 31
+        const int64_t c = c0 + u;
+        const int o = o0 + lane;
+        if (o < E && c < ncells) out[(size_t)c * E + o] = tile[lane][u];
+    }
+}
+}  // namespace
+
+cudaError_t qss_launch_jac_aos(int N, int rows, int64_t ncells, int64_t ld, const double *jac, const double *erow, int col_major, double *out,
+                               cudaStream_t stream) {
+    if (ncells == 0) return cudaSuccess;
+    const int E = rows * (N + 1);
+    const dim3 grid((unsigned)((ncells + 31) / 32), (unsigned)((E + 31) / 32));
+    qss_jac_aos_kernel<<<grid, 256, 0, stream>>>(N, rows, ncells, ld, jac, erow, col_major, out);
+    return cudaGetLastError();
+}

@@ -220,6 +220,37 @@ def test_full_jacobian_in_one_call(name, n):
     qm.close()
 
 
+@pytest.mark.parametrize("cfg,n", [(2, 1000 + 7), (1, 4096), (2, 1), (3, 37)])
+def test_aos_export_for_external_batched_solvers(cfg, n):
+    """qss_jac_to_aos is an index permutation: bit for bit the numpy transpose of the SoA arrays, row-major and column-major, with
+    and without the energy row; padding cells are not read into the output; the row-major matrices solve like qss_newton_solve's
+    (torch.linalg.solve on I - gamma J of a few cells, a LIBRARY routine standing in for the external solver)."""
+    import torch
+    import paper_2405_05974_b200 as qss
+    mech = qss_synth.config_mechanism(cfg)
+    N = mech.n_nqss
+    rng = np.random.default_rng(cfg + n)
+    ld = n + 9
+    jac = np.full((N, N + 1, ld), np.nan); erow = np.full((N + 1, ld), np.nan)
+    jac[:, :, :n] = rng.normal(size=(N, N + 1, n)); erow[:, :n] = rng.normal(size=(N + 1, n))
+    qm = qss.QssMech(mech, 0)
+    Jd = torch.from_numpy(jac).cuda(); Ed = torch.from_numpy(erow).cuda()
+    full = np.concatenate([jac, erow[None]], 0)                                    # [N+1, N+1, ld]
+    for with_e in (True, False):
+        src = full if with_e else jac
+        for cm in (False, True):
+            out = qm.jac_to_aos(Jd, Ed if with_e else None, n, col_major=cm).cpu().numpy()
+            want = np.transpose(src[:, :, :n], (2, 1, 0) if cm else (2, 0, 1))
+            assert out.shape == want.shape and np.array_equal(out, want), (with_e, cm)
+    if N + 1 <= 40 and n >= 4:
+        gamma = np.full(ld, 1e-2); b = rng.normal(size=(N + 1, ld))
+        x = qm.newton_solve(Jd, Ed, torch.from_numpy(gamma).cuda(), torch.from_numpy(b).cuda(), n).cpu().numpy()
+        A = torch.eye(N + 1, dtype=torch.float64, device="cuda")[None] - 1e-2 * qm.jac_to_aos(Jd, Ed, n)[:4]
+        xs = torch.linalg.solve(A, torch.from_numpy(np.ascontiguousarray(b[:, :4].T)).cuda()).cpu().numpy()
+        assert np.allclose(xs, x[:, :4].T, rtol=1e-9, atol=1e-12)
+    qm.close()
+
+
 @pytest.mark.parametrize("cfg,n", [(2, 2048 + 19), (1, 4096), (2, 31)])
 def test_mapping_microbenchmark_species_sums(cfg, n):
     """qss_bench_species_sums (north_star subsystem 3): both mappings give wdot = S Q; reference: the dense net stoichiometric
