@@ -114,29 +114,38 @@ cudaError_t qss_launch_jac_pack(int nnz, int64_t ncells, int64_t ld, const int32
 
 // ---- NEXT-2 ("optional AoS output layout for external batched solvers"; the Jacobian is handed
 // to a batched dense solver that wants one contiguous matrix per cell): the SoA Jacobian [entry][cell] (and the energy row) as
-// out[cell][rows][cols], row-major or column-major.  A tile of 32 output entries x 32 cells goes through shared memory: reads are
+// out[cell][rows][cols], row-major or column-major.  A tile of 64 output entries x 64 cells goes through shared memory: reads are
 // coalesced over cells, writes over the entries of one cell.  Pure data movement: bit-exact.
 namespace {
 __global__ void __launch_bounds__(256) qss_jac_aos_kernel(int N, int rows, int64_t ncells, int64_t ld, const double *__restrict__ jac,
                                                            const double *__restrict__ erow, int col_major, double *__restrict__ out) {
-    __shared__ double tile[32][33];
+    constexpr int TC = 64, TE = 64;                            // tile: 64 cells x 64 output entries (512-byte runs on both sides)
+    __shared__ double tile[TE][TC + 1];
     const int cols = N + 1, E = rows * cols;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int64_t c0 = (int64_t)blockIdx.x * 32;
-    const int o0 = blockIdx.y * 32;
-    for (int u = w; u < 32; u += 8) {                          // output entry o0 + u of the cells c0 .. c0 + 31
+    const int n_et = (E + TE - 1) / TE;                        // consecutive blocks: consecutive entry tiles of the same cells, so
+    const int64_t c0 = (int64_t)(blockIdx.x / n_et) * TC;      // that their writes fill those cells' matrices front to back
+    const int o0 = (int)(blockIdx.x % n_et) * TE;
+    for (int u = w; u < TE; u += 8) {                          // output entry o0 + u of the cells c0 .. c0 + 63
         const int o = o0 + u;
-        const int64_t c = c0 + lane;
-        if (o < E && c < ncells) {
-            const int i = col_major ? o % rows : o / cols, j = col_major ? o / rows : o % cols;
-            tile[u][lane] = i < N ? jac[((size_t)i * cols + j) * ld + c] : erow[(size_t)j * ld + c];
+        if (o >= E) break;
+        const int i = col_major ? o % rows : o / cols, j = col_major ? o / rows : o % cols;
+        const double *src = i < N ? jac + ((size_t)i * cols + j) * ld : erow + (size_t)j * ld;
+#pragma unroll
+        for (int h = 0; h < TC; h += 32) {
+            const int64_t c = c0 + h + lane;
+            if (c < ncells) tile[u][h + lane] = src[c];
         }
     }
     __syncthreads();
-    for (int u = w; u < 32; u += 8) {                          // cell c0 + u, output entries o0 .. o0 + 31
+    for (int u = w; u < TC; u += 8) {                          // cell c0 + u, output entries o0 .. o0 + 63
         const int64_t c = c0 + u;
-        const int o = o0 + lane;
-        if (o < E && c < ncells) out[(size_t)c * E + o] = tile[lane][u];
+        if (c >= ncells) break;
+#pragma unroll
+        for (int h = 0; h < TE; h += 32) {
+            const int o = o0 + h + lane;
+            if (o < E) out[(size_t)c * E + o] = tile[h + lane][u];
+        }
     }
 }
 }  // namespace
@@ -145,7 +154,9 @@ cudaError_t qss_launch_jac_aos(int N, int rows, int64_t ncells, int64_t ld, cons
                                cudaStream_t stream) {
     if (ncells == 0) return cudaSuccess;
     const int E = rows * (N + 1);
-    const dim3 grid((unsigned)((ncells + 31) / 32), (unsigned)((E + 31) / 32));
+    const int64_t nblocks = ((ncells + 63) / 64) * ((E + 63) / 64);
+    if (nblocks > 0x7fffffffLL) return cudaErrorInvalidValue;
+    const dim3 grid((unsigned)nblocks);
     qss_jac_aos_kernel<<<grid, 256, 0, stream>>>(N, rows, ncells, ld, jac, erow, col_major, out);
     return cudaGetLastError();
 }
