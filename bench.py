@@ -38,6 +38,7 @@ CALLS = {"jac+wdot": "qss_eval_jac with the wdot output (the metric)", "jac": "q
          "jac_full": "qss_eval_jac_full: the full (N+1)x(N+1) Jacobian, wdot and Tdot in one call (two launches)",
          "energy": "qss_eval_energy alone (on a Jacobian computed before the timed region)",
          "jac_const": "qss_eval_jac_approx, constant-QSS AJ", "jac_zero": "qss_eval_jac_approx, zero-QSS AJ",
+         "aos": "qss_jac_to_aos alone: the (N+1) x (N+1) Jacobian (computed before the timed region) as one contiguous row-major matrix per cell",
          "newton": "qss_newton_solve alone: x = (I - gamma J)^-1 (wdot, Tdot) on a full Jacobian computed before the timed region",
          "jac+wdot+energy+newton": "qss_eval_jac with wdot, qss_eval_energy, qss_newton_solve: one Newton direction of an implicit step",
          "sums_thread": "qss_bench_species_sums mode 0: mapping micro-benchmark, species sums with lane = cell (not on the path)",
@@ -226,8 +227,12 @@ def main():
     if "newton" in args.call:        # wdot and Tdot are written straight into the right-hand side (no copies in a step)
         B = torch.empty((N + 1, ld), dtype=torch.float64, device=dev)
         W = B[:N]; tdot = B[N]
-    if args.call in ("energy", "newton", "jac+wdot+energy+newton"):
+    if args.call in ("energy", "newton", "jac+wdot+energy+newton", "aos"):
         qm.eval_jac(Cd, Td, n, jac=J, wdot=W, want_wdot=True)
+    AOS = None
+    if args.call == "aos":
+        qm.eval_energy(Cd, Td, W, J, n, tdot=tdot, erow=erow)
+        AOS = torch.empty((n, N + 1, N + 1), dtype=torch.float64, device=dev)
     if "newton" in args.call:
         # right-hand side (wdot, Tdot); gamma_c = theta_c / max|J_c|, theta log-uniform in [1e-2, 1e3] (seeded): from "explicit would do" to stiff
         qm.eval_energy(Cd, Td, W, J, n, tdot=tdot, erow=erow)
@@ -284,6 +289,8 @@ def main():
             qm.eval_jac(Cd, Td, n, jac=J)
         elif args.call == "energy":
             qm.eval_energy(Cd, Td, W, J, n, tdot=tdot, erow=erow)
+        elif args.call == "aos":
+            qm.jac_to_aos(J, erow, n, out=AOS)
         elif args.call in ("jac_const", "jac_zero"):
             qm.eval_jac_approx(Cd, Td, 1 if args.call == "jac_const" else 2, n, jac=J)
         else:
@@ -354,6 +361,8 @@ def main():
         bytes_cell, slots_cell = info.bytes_wdot, info.slots_wdot
     elif args.call == "energy":        # reads C, T, wdot and J once, writes the row and tdot; 2 N (N+1) + ~30 N fp64 slots
         bytes_cell, slots_cell = 8.0 * (N * (N + 1) + 2 * N + 1) + 8.0 * (N + 2), 2.0 * N * (N + 1) + 30.0 * N
+    elif args.call == "aos":           # reads and writes the (N+1)^2 matrix once; no arithmetic
+        bytes_cell, slots_cell = 16.0 * (N + 1) * (N + 1), 0.0
     elif args.call == "newton":        # reads the (N+1)^2 matrix, b and gamma once, writes x; n^3/3 + n^2 fp64 FMA slots (elimination + substitutions)
         nn = N + 1
         bytes_cell, slots_cell = 8.0 * (nn * nn + 2 * nn + 1), nn ** 3 / 3.0 + nn * nn
@@ -385,7 +394,7 @@ def main():
     except Exception:
         traffic = None
     roof.update({"traffic": traffic, "traffic_unit": "bytes per launch (dram read + write) from the committed ncu capture of this workload and kernel variant (profiles/r02_traffic.txt); not measurable inside this run",
-                 "kernel": "qss_mapbench_kernel" if args.call.startswith("sums_") else "qss_energy_kernel" if args.call == "energy" else "qss_newton_kernel" if args.call == "newton" else "the 4 launches of one substep (Jacobian kernel, fused Newton step; twice)" if args.call in ("bdf1", "ignition") else ("qss wdot kernel (qss_eval_wdot)" if args.call == "wdot" else f"qss jacobian kernel, variant {info.kernel_variant_jac} ({CALLS[args.call]})"),
+                 "kernel": "qss_mapbench_kernel" if args.call.startswith("sums_") else "qss_energy_kernel" if args.call == "energy" else "qss_jac_aos_kernel" if args.call == "aos" else "qss_newton_kernel" if args.call == "newton" else "the 4 launches of one substep (Jacobian kernel, fused Newton step; twice)" if args.call in ("bdf1", "ignition") else ("qss wdot kernel (qss_eval_wdot)" if args.call == "wdot" else f"qss jacobian kernel, variant {info.kernel_variant_jac} ({CALLS[args.call]})"),
                  "launch_ms_avg": avg_s * 1e3, "launch_ms_min": min(launch_ms),
                  "alg_fp64_slots_per_cell": slots_cell, "alg_bytes_per_cell": bytes_cell,
                  "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3,
